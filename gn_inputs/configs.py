@@ -1,0 +1,113 @@
+"""The five BASELINE.json workloads as seeded synthetic inputs.
+
+Each entry fixes what BASELINE.json leaves open with the reading listed in DESIGN.md
+(SURVEY.md section 8(c) readings #5, #12, #16-#20).  A config can be generated at a reduced vertex
+count for tests: the box side is shrunk so the vertex density (and with it the degree and delay
+distributions away from the boundary) stays that of the full-size config.
+
+Only inputs are made here; the dictionaries below are data (parameter tables), not arithmetic.
+"""
+from __future__ import annotations
+
+import math
+
+from .generate import Network, geometric_network
+
+MASTER_SEED = 0x09083934
+
+CONFIG_NAMES = {
+    1: "cfg1_n100_2d",
+    2: "cfg2_n10k_2d_ei_obs",
+    3: "cfg3_n100k_3d_exp",
+    4: "cfg4_n1m_3d_rgg",
+    5: "cfg5_batch4096x1000_2d_obs",
+}
+
+
+def _cls(a, d, rate_hz, kick=10.0, tau_syn_ms=2.0):
+    """One row of gn_class_params.  b = 0.2, c = -65, k2/k1/k0 = 0.04/5/140, v_peak = 30
+    (the (a,b,c,d) form of PAPER.md:216-233 eq. 23-24; reading #1), refractory 2 ms."""
+    return dict(a=a, b=0.2, c_reset=-65.0, d=d, k2=0.04, k1=5.0, k0=140.0, v_peak=30.0,
+                tau_syn_ms=tau_syn_ms, refractory_ms=2.0, drive_rate_hz=rate_hz, drive_kick=kick)
+
+
+def _rs(rate):  # regular spiking, excitatory
+    return _cls(0.02, 8.0, rate)
+
+
+def _fs(rate):  # fast spiking, inhibitory
+    return _cls(0.1, 2.0, rate)
+
+
+def _p_within_cube(rho):  # P(two uniform points in a unit cube are closer than rho), rho <= 1
+    return 4 * math.pi * rho ** 3 / 3 - 3 * math.pi * rho ** 4 / 2 + 8 * rho ** 5 / 5 - rho ** 6 / 6
+
+
+def _radius_for_degree_cube(n, side, degree):
+    lo, hi = 0.0, 1.0
+    for _ in range(200):
+        mid = 0.5 * (lo + hi)
+        if (n - 1) * _p_within_cube(mid) < degree:
+            lo = mid
+        else:
+            hi = mid
+    return side * lo
+
+
+def make_config(k: int, n: int | None = None, n_networks: int | None = None,
+                seed: int | None = None) -> tuple[Network, dict]:
+    """Return (Network, cfg) for BASELINE config k (1..5).
+
+    `n` overrides the vertex count (per network for config 5) keeping the vertex density;
+    `n_networks` overrides config 5's batch size.  cfg carries every scalar gn_create needs
+    plus `steps` (the config's nominal run length) and `name`.
+    """
+    seed = (MASTER_SEED + k) if seed is None else seed
+    base = dict(dt_ms=0.1, tau_ca_ms=500.0, ca_jump=1.0, obs_gain=1.0, obs_offset=0.0,
+                obs_sigma=0.05, obs_stride=0, seed=seed, name=CONFIG_NAMES[k])
+    if k == 1:
+        n_full, dim, side = 100, 2, 1.0
+        n = n or n_full
+        side *= (n / n_full) ** (1 / dim)
+        net = geometric_network(seed, n, dim, side, 0.15, p0=0.5, w_exc=(0.0, 8.0))
+        cfg = dict(base, ring_slots=16, speed=0.1, classes=[_rs(10.0)], steps=10_000)
+    elif k == 2:
+        n_full, dim, side = 10_000, 2, 3.0
+        n = n or n_full
+        side *= (n / n_full) ** (1 / dim)
+        # reading #16: radius 0.15 mm, p = 0.665 => mean out-degree 50 away from the boundary
+        net = geometric_network(seed, n, dim, side, 0.15, p0=0.665, frac_inh=0.2,
+                                w_exc=(0.0, 6.0), w_inh=(-12.0, 0.0))
+        cfg = dict(base, ring_slots=16, speed=0.1, classes=[_rs(5.0), _fs(5.0)], steps=10_000,
+                   obs_stride=1)
+    elif k == 3:
+        n_full, dim, side = 100_000, 3, 1.0
+        n = n or n_full
+        side *= (n / n_full) ** (1 / dim)
+        # reading #17: p = 0.3 exp(-d / 0.05 mm), cut off at the delay cap 63 * speed * dt
+        net = geometric_network(seed, n, dim, side, 0.315, kind=1, p0=0.3, lam=0.05, frac_inh=0.2,
+                                w_exc=(0.0, 6.0), w_inh=(-12.0, 0.0))
+        cfg = dict(base, ring_slots=64, speed=0.05, classes=[_rs(5.0), _fs(5.0)], steps=20_000)
+    elif k == 4:
+        n_full, dim, side = 1_000_000, 3, 2.0
+        n = n or n_full
+        # reading #18: radius calibrated (closed form) to mean out-degree 200 at FULL size
+        radius = _radius_for_degree_cube(n_full, side, 200.0)
+        side *= (n / n_full) ** (1 / dim)
+        net = geometric_network(seed, n, dim, side, radius, p0=1.0, frac_inh=0.2,
+                                w_exc=(0.0, 6.0), w_inh=(-12.0, 0.0))
+        cfg = dict(base, ring_slots=128, speed=0.006, classes=[_rs(2.0), _fs(2.0)], steps=10_000)
+        net.meta["radius"] = radius
+    elif k == 5:
+        n_per = n or 1000
+        nb = n_networks or 4096
+        side = (n_per / 1000) ** 0.5
+        # reading #19: 20 % of vertices inhibitory, their out-weights sign-flipped; delays 1..31
+        net = geometric_network(seed, n_per, 2, side, 0.08, p0=1.0, frac_inh=0.2,
+                                w_exc=(0.0, 8.0), w_inh=(-8.0, 0.0), n_networks=nb)
+        cfg = dict(base, ring_slots=32, speed=0.0259, classes=[_rs(10.0), _rs(10.0)], steps=5_000,
+                   obs_stride=100)
+    else:
+        raise ValueError("config must be 1..5")
+    net.meta.update(config=k, side=side, seed=seed)
+    return net, cfg

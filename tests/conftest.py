@@ -1,0 +1,21 @@
+import os
+import sys
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+
+def pytest_configure(config):
+    config.addinivalue_line("markers", "gpu: needs a CUDA device (run with -m gpu on a B200)")
+
+
+@pytest.fixture(scope="session", autouse=True)
+def _build_cpu_libs():
+    """gcc-build the input generator and the oracle once per session (CPU only)."""
+    import gn_inputs
+    import oracle
+    gn_inputs.build_lib()
+    oracle.build_lib()
