@@ -1,0 +1,169 @@
+/*
+ * gn.h -- C ABI of the geometric-network simulation step on one B200 (sm_100a).
+ *
+ * The operation is the per-timestep transition of Buibas & Silva's framework (arxiv 0908.3934;
+ * line numbers below are /root/reference/PAPER.md):
+ *
+ *   y_j(t + dt) = H_j( y_j(t), Y_j(t), u_j(t), Theta_j )                     :68-71  eq. 5
+ *
+ * with  y_j = {V, W, r, c} an Izhikevich simple-model vertex with hard reset (:227-229 eq. 24,
+ * :303 eq. 28), an exponential post-synaptic current (:283-286 eq. 26) and a calcium state
+ * (:364 H_c);  Y_j(t) the delayed, weighted spikes of the other vertices,
+ * sum_k w_kj spd(V_k(t - tau_kj)) (:311 eq. 30, spd = [V >= V_peak] :316 eq. 31) with
+ * tau_kj = |x_k - x_j| / s (:251 eq. 25);  u_j(t) the external control (:77-79 eq. 7); and the
+ * observation I_j = n c_j + b + N(0, gamma^2) averaged over camera frames (:370-374).
+ * DESIGN.md lists every reading taken where the paper is silent or garbled and the exact fp32
+ * operation sequence ("arithmetic contract") the kernels follow.
+ *
+ * Conventions
+ *   - Every function returns GN_OK (0) or a negative GN_E_* code; nothing throws, exits or keeps
+ *     global state.  gn_last_error() gives a NUL-terminated message for the last failure on a
+ *     handle (or, with NULL, of the last failed gn_create on this thread).
+ *   - Memory: the library never allocates device memory.  gn_create carves everything out of a
+ *     caller-supplied DEVICE workspace (gn_query_workspace bytes, 256-byte aligned) that must
+ *     outlive the handle.  Input arrays of gn_create may be host or device pointers (they are
+ *     copied with cudaMemcpyDefault) and may be freed once gn_create returns.
+ *   - Streams: all work is enqueued on the cudaStream_t given to gn_create (pass torch's current
+ *     stream).  Functions with a host destination synchronise that stream before returning;
+ *     device destinations are written asynchronously on it.
+ *   - Vertex ids are the caller's.  Step index t counts completed steps from 0.
+ *   - There is no CPU fallback: without a CUDA device every call fails with GN_E_CUDA.
+ */
+#ifndef GN_H_
+#define GN_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define GN_OK 0
+#define GN_E_INVALID_ARG (-1)         /* NULL pointer, bad scalar, unsupported size               */
+#define GN_E_BAD_GRAPH (-2)           /* row offsets not monotone / target out of range / delay   */
+                                      /* 0 or >= ring_slots / edge crossing networks / class id   */
+#define GN_E_OVERFLOW_RISK (-3)       /* some target's sum |w_fx| (+ largest kick) >= 2^31        */
+#define GN_E_WORKSPACE_TOO_SMALL (-4)
+#define GN_E_RANGE_EVICTED (-5)       /* raster / trace range not (or no longer) held             */
+#define GN_E_CUDA (-6)                /* a CUDA runtime call failed; see gn_last_error            */
+
+#define GN_MAX_CLASSES 8
+
+typedef struct gn_net gn_net;
+
+/* One vertex class (e.g. 0 = regular-spiking excitatory, 1 = fast-spiking inhibitory).
+ * dV/dt = k2 V^2 + k1 V + k0 - W + r + U,  dW/dt = a (b V - W);  V >= v_peak: V <- c_reset,
+ * W <- W + d  (eq. 23-24 in its (a,b,c,d) parametrisation, reading #1). */
+typedef struct {
+    float a, b, c_reset, d;
+    float k2, k1, k0, v_peak;
+    float tau_syn_ms;       /* exponential PSC time constant 1/a of eq. 26 (:283-286); <= 0 selects  */
+                            /* direct injection: the arriving weight jumps V itself                  */
+    float refractory_ms;    /* absolute refractory hold after a spike (:259, reading #6)             */
+    float drive_rate_hz;    /* Bernoulli(rate*dt) kick per step from the counter generator           */
+    float drive_kick;       /* kick weight, injected like an arriving event (reading #12)            */
+} gn_class_params;
+
+typedef struct {
+    uint32_t n_vertices;            /* N (total over all networks in batched mode)                   */
+    uint32_t dim;                   /* 2 or 3: columns of `positions`                                */
+    uint64_t n_edges;               /* E < 2^32                                                      */
+    uint32_t n_networks;            /* 1, or B independent networks stepped together (block-diagonal)*/
+    uint32_t ring_slots;            /* 2 <= D <= 255; every delay satisfies 1 <= delay <= D-1        */
+    float    dt_ms;                 /* time step                                                     */
+    float    speed;                 /* conduction speed, position units per ms (delays == NULL)      */
+    uint32_t n_classes;             /* 1 .. GN_MAX_CLASSES                                           */
+    float    tau_ca_ms, ca_jump;    /* calcium filter c <- c (1 - dt/tau_ca) + ca_jump*fired (:364)  */
+    float    obs_gain, obs_offset, obs_sigma;   /* n, b, gamma of I = n c + b + N(0,gamma^2) (:370)  */
+    uint32_t obs_stride;            /* steps averaged per camera frame (:374); 0 = observation off   */
+    uint32_t raster_capacity_steps; /* device raster window (most recent steps kept); 0 = none kept  */
+    uint32_t trace_capacity_frames; /* device trace window (most recent frames kept)                 */
+    uint64_t seed;                  /* key of the counter generator (drive stream 5, noise stream 6) */
+} gn_config;
+
+/* `which` of gn_read_state / gn_write_state, with the element type of the caller's buffer.       */
+enum {
+    GN_V = 0,         /* float  [N]      membrane potential                                          */
+    GN_W = 1,         /* float  [N]      recovery variable                                           */
+    GN_R = 2,         /* float  [N]      post-synaptic current r                                     */
+    GN_CA = 3,        /* float  [N]      calcium c (maintained only when obs_stride > 0)             */
+    GN_REFR = 4,      /* uint8  [N]      refractory steps left                                       */
+    GN_RING = 5,      /* int32  [D][N]   delay ring, fixed point 2^-16.  After T completed steps     */
+                      /*                 slot s holds the arrivals due at steps a = s (mod D),       */
+                      /*                 T <= a <= T + D - 2; slot (T-1) mod D is zero               */
+    GN_STEP = 6,      /* uint64 [1]      completed steps t                                           */
+    GN_COUNTERS = 7,  /* uint64 [4]      { steps, spikes, delivered events, kicks }                  */
+    GN_DELAYS = 8,    /* uint8  [E]      per-edge delay in steps (as given, or eq. 25)               */
+    GN_WEIGHTS_FX = 9,/* int32  [E]      per-edge weight, rint(w * 2^16)                             */
+    GN_BIAS = 10      /* float  [N]      user control U_j (write only through gn_write_state)        */
+};
+
+/* Bytes of device workspace gn_create needs for this configuration.
+ * Errors: GN_E_INVALID_ARG (NULL, N = 0, dim not 2/3, D < 2 or > 255, E >= 2^32, n_classes out of
+ * range, dt <= 0, obs_stride > 0 with trace_capacity_frames = 0). */
+int gn_query_workspace(const gn_config *cfg, size_t *bytes);
+
+/*
+ * Build a network on the device.
+ *   classes       [n_classes]
+ *   positions     [N][dim] float, row-major.  May be NULL when `delays` is given.
+ *   row_offsets   [N+1] CSR by SOURCE vertex: out-edges of i are row_offsets[i] .. row_offsets[i+1]-1
+ *   targets       [E] target vertex of each edge
+ *   weights       [E] fp32; quantised here to int32 fixed point, w_fx = rint(w * 65536) (ties to even)
+ *   delays        [E] steps, or NULL => max(1, ceil(|x_i - x_j| / (speed * dt))) in double (eq. 25)
+ *   vertex_class  [N] class id < n_classes
+ *   bias          [N] constant user control U_j added inside eq. 28's bracket, or NULL (none)
+ *   net_offsets   [n_networks + 1] first vertex of each network (batched mode), or NULL when
+ *                 n_networks == 1; an edge whose endpoints lie in different networks is rejected
+ *   workspace     device memory, >= gn_query_workspace bytes, 256-byte aligned; owned by the caller
+ *   cuda_stream   cudaStream_t (NULL = legacy default stream)
+ * Initial state (reading #15): V = -70, W = b V, r = c = 0, not refractory, ring empty, t = 0.
+ * Synchronises the stream once (validation results are read back).  On failure *out = NULL.
+ * Errors: INVALID_ARG, BAD_GRAPH, OVERFLOW_RISK, WORKSPACE_TOO_SMALL, CUDA.
+ */
+int gn_create(const gn_config *cfg, const gn_class_params *classes, const float *positions,
+              const uint64_t *row_offsets, const uint32_t *targets, const float *weights,
+              const uint8_t *delays, const uint8_t *vertex_class, const float *bias,
+              const uint32_t *net_offsets, void *workspace, size_t workspace_bytes,
+              void *cuda_stream, gn_net **out);
+
+/* Advance n_steps time steps: per step, ring-slot read-and-clear + drive + vertex update + spike
+ * detection/compaction (one kernel), event delivery into the delay ring (one kernel), and at
+ * frame boundaries the observation kernel.  Asynchronous: no host synchronisation inside. */
+int gn_step(gn_net *net, uint64_t n_steps);
+
+/* Copy state out.  dst_bytes must be at least the size listed at the enum.  dst_is_device != 0:
+ * dst is device memory, written asynchronously on the stream.  Errors: INVALID_ARG, CUDA. */
+int gn_read_state(gn_net *net, int which, void *dst, size_t dst_bytes, int dst_is_device);
+
+/* Overwrite V, W, R, CA (float [N]), REFR (uint8 [N]) or BIAS (float [N]; enables the bias term).
+ * For checkpoint/restore and controlled experiments (PAPER.md:77-79 user control). */
+int gn_write_state(gn_net *net, int which, const void *src, size_t src_bytes, int src_is_device);
+
+/* Spike raster of steps t0 .. t0+n_steps-1 as bit words: bit (j mod 32) of bits[s][j / 32] is
+ * spd(V_j(t0 + s)) (eq. 31); row length ceil(N/32) words.  Errors: RANGE_EVICTED if any step is
+ * not yet simulated or older than raster_capacity_steps. */
+int gn_read_raster(gn_net *net, uint64_t t0, uint64_t n_steps, uint32_t *bits, size_t dst_bytes,
+                   int dst_is_device);
+
+/* Observation trace, frames frame0 .. frame0+n_frames-1, trace[f][j] = I_j of frame f
+ * (PAPER.md:370-374); frame f covers steps f*obs_stride .. (f+1)*obs_stride-1.
+ * Errors: INVALID_ARG if observation is off, RANGE_EVICTED as for the raster. */
+int gn_observe(gn_net *net, uint64_t frame0, uint64_t n_frames, float *trace, size_t dst_bytes,
+               int dst_is_device);
+
+/* Test hook: out[i] = 32-bit word of the counter generator for vertex first_vertex + i at index
+ * idx on `stream_id` (Philox4x32-10; counter {vertex/4, idx lo, idx hi, stream_id}, key = seed;
+ * word vertex mod 4).  `out` is DEVICE memory.  Lets the known-answer vectors reach the device
+ * implementation. */
+int gn_debug_words(void *cuda_stream, uint64_t seed, uint32_t stream_id, uint64_t idx,
+                   uint32_t first_vertex, uint32_t n, uint32_t *out);
+
+const char *gn_last_error(const gn_net *net);
+int gn_destroy(gn_net *net);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GN_H_ */

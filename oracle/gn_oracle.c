@@ -85,7 +85,8 @@ uint32_t orc_word(uint64_t seed, uint32_t stream, uint32_t j, uint64_t idx)
 
 /* Standard normal for (vertex j, frame): Box-Muller on two words of the vertex group's block.
  * Vertices j mod 4 in {0,1} share words (x0,x1), {2,3} share (x2,x3); even j takes the cosine
- * branch, odd j the sine branch.  u_a in (0,1), u_b in [0,1), both 24-bit. */
+ * branch, odd j the sine branch.  u_a = (k + 1/2) 2^-23 in (0,1) from the top 23 bits, u_b = k 2^-24
+ * in [0,1) from the top 24 bits (both exact in binary32 as well as in double). */
 double orc_gauss(uint64_t seed, uint32_t j, uint64_t frame)
 {
     uint32_t ctr[4] = { j >> 2, (uint32_t)frame, (uint32_t)(frame >> 32), ORC_STREAM_NOISE };
@@ -93,7 +94,7 @@ double orc_gauss(uint64_t seed, uint32_t j, uint64_t frame)
     uint32_t x[4];
     orc_philox4x32_10(ctr, key, x);
     uint32_t xa = x[(j & 2)], xb = x[(j & 2) + 1];
-    double ua = ((double)(xa >> 8) + 0.5) * (1.0 / 16777216.0);
+    double ua = ((double)(xa >> 9) + 0.5) * (1.0 / 8388608.0);
     double ub = (double)(xb >> 8) * (1.0 / 16777216.0);
     double rad = sqrt(-2.0 * log(ua));
     double ang = 6.283185307179586476925286766559 * ub;

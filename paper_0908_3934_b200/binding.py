@@ -1,0 +1,221 @@
+"""Thin ctypes binding of include/gn.h -- argument marshalling only.
+
+Every step of the path runs inside libgn.so's CUDA kernels; PyTorch supplies device memory (the
+workspace and destination tensors) and the stream.  There is no CPU fallback: if the library is
+missing it is built with nvcc, and if that fails the import raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+
+import numpy as np
+
+from .build import build
+
+GN_OK = 0
+GN_E_INVALID_ARG, GN_E_BAD_GRAPH, GN_E_OVERFLOW_RISK = -1, -2, -3
+GN_E_WORKSPACE_TOO_SMALL, GN_E_RANGE_EVICTED, GN_E_CUDA = -4, -5, -6
+GN_V, GN_W, GN_R, GN_CA, GN_REFR, GN_RING, GN_STEP, GN_COUNTERS, GN_DELAYS, GN_WEIGHTS_FX, GN_BIAS = range(11)
+GN_MAX_CLASSES = 8
+
+CLASS_FIELDS = ("a", "b", "c_reset", "d", "k2", "k1", "k0", "v_peak", "tau_syn_ms",
+                "refractory_ms", "drive_rate_hz", "drive_kick")
+
+
+class gn_class_params(C.Structure):
+    _fields_ = [(f, C.c_float) for f in CLASS_FIELDS]
+
+
+class gn_config(C.Structure):
+    _fields_ = [("n_vertices", C.c_uint32), ("dim", C.c_uint32), ("n_edges", C.c_uint64),
+                ("n_networks", C.c_uint32), ("ring_slots", C.c_uint32), ("dt_ms", C.c_float),
+                ("speed", C.c_float), ("n_classes", C.c_uint32), ("tau_ca_ms", C.c_float),
+                ("ca_jump", C.c_float), ("obs_gain", C.c_float), ("obs_offset", C.c_float),
+                ("obs_sigma", C.c_float), ("obs_stride", C.c_uint32),
+                ("raster_capacity_steps", C.c_uint32), ("trace_capacity_frames", C.c_uint32),
+                ("seed", C.c_uint64)]
+
+
+EXPORTS = ("gn_query_workspace", "gn_create", "gn_step", "gn_read_state", "gn_write_state",
+           "gn_read_raster", "gn_observe", "gn_debug_words", "gn_last_error", "gn_destroy")
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    global _lib
+    if _lib is None:
+        L = C.CDLL(build())
+        vp, u64, u32, i32, sz = C.c_void_p, C.c_uint64, C.c_uint32, C.c_int, C.c_size_t
+        L.gn_query_workspace.argtypes = [C.POINTER(gn_config), C.POINTER(sz)]
+        L.gn_create.argtypes = [C.POINTER(gn_config), C.POINTER(gn_class_params), vp, vp, vp, vp, vp, vp, vp, vp,
+                                vp, sz, vp, C.POINTER(vp)]
+        L.gn_step.argtypes = [vp, u64]
+        L.gn_read_state.argtypes = [vp, i32, vp, sz, i32]
+        L.gn_write_state.argtypes = [vp, i32, vp, sz, i32]
+        L.gn_read_raster.argtypes = [vp, u64, u64, vp, sz, i32]
+        L.gn_observe.argtypes = [vp, u64, u64, vp, sz, i32]
+        L.gn_debug_words.argtypes = [vp, u64, u32, u64, u32, u32, vp]
+        L.gn_last_error.argtypes = [vp]
+        L.gn_last_error.restype = C.c_char_p
+        L.gn_destroy.argtypes = [vp]
+        for name in EXPORTS:
+            if name != "gn_last_error":
+                getattr(L, name).restype = i32
+        _lib = L
+    return _lib
+
+
+class GnError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"gn error {code}: {msg}")
+        self.code = code
+
+
+def _check(rc, handle=None):
+    if rc != GN_OK:
+        raise GnError(rc, lib().gn_last_error(handle).decode())
+
+
+def _ptr(a):
+    """Host numpy array, torch tensor (host or device) or None -> void pointer."""
+    if a is None:
+        return None
+    if isinstance(a, np.ndarray):
+        assert a.flags["C_CONTIGUOUS"]
+        return a.ctypes.data_as(C.c_void_p)
+    assert a.is_contiguous()
+    return C.c_void_p(a.data_ptr())
+
+
+def make_config(n_vertices, dim, n_edges, ring_slots, dt_ms, speed, n_classes, *, n_networks=1, tau_ca_ms=500.0,
+                ca_jump=1.0, obs_gain=1.0, obs_offset=0.0, obs_sigma=0.0, obs_stride=0, raster_capacity_steps=0,
+                trace_capacity_frames=0, seed=0) -> gn_config:
+    return gn_config(n_vertices, dim, n_edges, n_networks, ring_slots, dt_ms, speed, n_classes, tau_ca_ms, ca_jump,
+                     obs_gain, obs_offset, obs_sigma, obs_stride, raster_capacity_steps, trace_capacity_frames, seed)
+
+
+def gn_query_workspace(cfg: gn_config) -> int:
+    n = C.c_size_t(0)
+    _check(lib().gn_query_workspace(C.byref(cfg), C.byref(n)))
+    return n.value
+
+
+class GnNet:
+    """Owner of one gn_net handle and of the torch workspace tensor behind it."""
+
+    def __init__(self, handle, workspace, cfg, stream):
+        self.handle, self.workspace, self.cfg, self.stream = handle, workspace, cfg, stream
+        self.n, self.e, self.d = cfg.n_vertices, cfg.n_edges, cfg.ring_slots
+        self.words = (self.n + 31) // 32
+
+    def __del__(self):
+        self.destroy()
+
+    def destroy(self):
+        if getattr(self, "handle", None):
+            lib().gn_destroy(self.handle)
+            self.handle = None
+            self.workspace = None
+
+
+def gn_create(cfg: gn_config, classes, positions, row_offsets, targets, weights, delays, vertex_class,
+              bias=None, net_offsets=None, device="cuda:0", workspace=None) -> GnNet:
+    """classes: sequence of dicts with CLASS_FIELDS.  Arrays: numpy (host) or torch tensors."""
+    import torch
+    if not torch.cuda.is_available():
+        raise GnError(GN_E_CUDA, "no CUDA device: this library has no CPU fallback")
+    dev = torch.device(device)
+    need = gn_query_workspace(cfg)
+    if workspace is None:
+        workspace = torch.empty(need, dtype=torch.uint8, device=dev)
+    tab = (gn_class_params * len(classes))(*[gn_class_params(*[c[f] for f in CLASS_FIELDS]) for c in classes])
+    handle = C.c_void_p(None)
+    with torch.cuda.device(dev):
+        stream = torch.cuda.current_stream(dev)
+        rc = lib().gn_create(C.byref(cfg), tab, _ptr(positions), _ptr(row_offsets), _ptr(targets), _ptr(weights),
+                             _ptr(delays), _ptr(vertex_class), _ptr(bias), _ptr(net_offsets),
+                             C.c_void_p(workspace.data_ptr()), workspace.numel(), C.c_void_p(stream.cuda_stream),
+                             C.byref(handle))
+    _check(rc)
+    return GnNet(handle, workspace, cfg, stream)
+
+
+def gn_step(net: GnNet, n_steps: int) -> None:
+    _check(lib().gn_step(net.handle, int(n_steps)), net.handle)
+
+
+_STATE_DTYPE = {GN_V: np.float32, GN_W: np.float32, GN_R: np.float32, GN_CA: np.float32, GN_REFR: np.uint8,
+                GN_RING: np.int32, GN_STEP: np.uint64, GN_COUNTERS: np.uint64, GN_DELAYS: np.uint8,
+                GN_WEIGHTS_FX: np.int32, GN_BIAS: np.float32}
+
+
+def _state_shape(net, which):
+    return {GN_RING: (net.d, net.n), GN_STEP: (1,), GN_COUNTERS: (4,), GN_DELAYS: (net.e,),
+            GN_WEIGHTS_FX: (net.e,)}.get(which, (net.n,))
+
+
+def gn_read_state(net: GnNet, which: int, out=None):
+    """Host numpy result by default; pass a torch CUDA tensor as `out` for a device destination."""
+    if out is None:
+        out = np.empty(_state_shape(net, which), dtype=_STATE_DTYPE[which])
+    is_dev = not isinstance(out, np.ndarray)
+    nbytes = out.numel() * out.element_size() if is_dev else out.nbytes
+    _check(lib().gn_read_state(net.handle, which, _ptr(out), nbytes, int(is_dev)), net.handle)
+    return out
+
+
+def gn_write_state(net: GnNet, which: int, src) -> None:
+    is_dev = not isinstance(src, np.ndarray)
+    if not is_dev:
+        src = np.ascontiguousarray(src, dtype=_STATE_DTYPE[which])
+    nbytes = src.numel() * src.element_size() if is_dev else src.nbytes
+    _check(lib().gn_write_state(net.handle, which, _ptr(src), nbytes, int(is_dev)), net.handle)
+
+
+def gn_read_raster(net: GnNet, t0: int, n_steps: int, out=None):
+    if out is None:
+        out = np.empty((n_steps, net.words), dtype=np.uint32)
+    is_dev = not isinstance(out, np.ndarray)
+    nbytes = out.numel() * out.element_size() if is_dev else out.nbytes
+    _check(lib().gn_read_raster(net.handle, int(t0), int(n_steps), _ptr(out), nbytes, int(is_dev)), net.handle)
+    return out
+
+
+def gn_observe(net: GnNet, frame0: int, n_frames: int, out=None):
+    if out is None:
+        out = np.empty((n_frames, net.n), dtype=np.float32)
+    is_dev = not isinstance(out, np.ndarray)
+    nbytes = out.numel() * out.element_size() if is_dev else out.nbytes
+    _check(lib().gn_observe(net.handle, int(frame0), int(n_frames), _ptr(out), nbytes, int(is_dev)), net.handle)
+    return out
+
+
+def gn_debug_words(seed: int, stream_id: int, idx: int, first_vertex: int, n: int, device="cuda:0"):
+    import torch
+    out = torch.empty(n, dtype=torch.int32, device=device)
+    st = torch.cuda.current_stream(out.device)
+    _check(lib().gn_debug_words(C.c_void_p(st.cuda_stream), seed, stream_id, idx, first_vertex, n,
+                                C.c_void_p(out.data_ptr())))
+    return out.cpu().numpy().view(np.uint32)
+
+
+def gn_destroy(net: GnNet) -> None:
+    net.destroy()
+
+
+def create_from_inputs(net_in, cfg_in, *, delays=None, bias=None, raster_capacity_steps=0,
+                       trace_capacity_frames=0, device="cuda:0") -> GnNet:
+    """Convenience: build from a gn_inputs.Network + config dict (marshalling only)."""
+    obs = int(cfg_in.get("obs_stride", 0))
+    cfg = make_config(net_in.n_vertices, net_in.dim, net_in.n_edges, cfg_in["ring_slots"], cfg_in["dt_ms"],
+                      cfg_in["speed"], len(cfg_in["classes"]), n_networks=net_in.n_networks,
+                      tau_ca_ms=cfg_in["tau_ca_ms"], ca_jump=cfg_in["ca_jump"], obs_gain=cfg_in["obs_gain"],
+                      obs_offset=cfg_in["obs_offset"], obs_sigma=cfg_in["obs_sigma"], obs_stride=obs,
+                      raster_capacity_steps=raster_capacity_steps,
+                      trace_capacity_frames=trace_capacity_frames if obs else 0, seed=cfg_in["seed"])
+    return gn_create(cfg, cfg_in["classes"], net_in.positions, net_in.row_offsets, net_in.targets, net_in.weights,
+                     None if delays is None else np.ascontiguousarray(delays, dtype=np.uint8),
+                     net_in.vertex_class,
+                     None if bias is None else np.ascontiguousarray(bias, dtype=np.float32),
+                     net_in.net_offsets, device=device)

@@ -1,0 +1,432 @@
+// gn_api.cu -- host logic of the C ABI declared in include/gn.h: validation, workspace layout,
+// uploads, step sequencing and read-back.  No arithmetic of the method runs here; every step of
+// the path is a kernel in gn_kernels.cu.
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+
+#include "gn_internal.h"
+
+namespace {
+
+thread_local char g_create_error[256] = "";
+
+struct Layout {
+    size_t V, W, r, c, acc, bias, refr, cls, ring, row, tgt, wfx, dly, active, n_active, counters;
+    size_t raster, trace, scratch_row64, scratch_abs, scratch_pos, scratch_net, scratch_chk, total;
+};
+
+inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+int check_config(const gn_config *cfg, char *err, size_t errn)
+{
+    auto fail = [&](const char *m) { snprintf(err, errn, "%s", m); return GN_E_INVALID_ARG; };
+    if (!cfg) return fail("cfg is NULL");
+    if (cfg->n_vertices == 0 || cfg->n_vertices > 0xFFFFFF00u) return fail("n_vertices must be in [1, 2^32-256]");
+    if (cfg->dim != 2 && cfg->dim != 3) return fail("dim must be 2 or 3");
+    if (cfg->n_edges >= 0xFFFFFFFFull) return fail("n_edges must be < 2^32 - 1");
+    if (cfg->ring_slots < 2 || cfg->ring_slots > 255) return fail("ring_slots must be in [2, 255]");
+    if (cfg->n_classes < 1 || cfg->n_classes > GN_MAX_CLASSES) return fail("n_classes must be in [1, GN_MAX_CLASSES]");
+    if (!(cfg->dt_ms > 0.0f)) return fail("dt_ms must be > 0");
+    if (cfg->n_networks < 1 || cfg->n_networks > cfg->n_vertices) return fail("n_networks must be in [1, n_vertices]");
+    if (cfg->obs_stride > 0 && cfg->trace_capacity_frames == 0) return fail("obs_stride > 0 needs trace_capacity_frames > 0");
+    if (cfg->obs_stride > 0 && !(cfg->tau_ca_ms > 0.0f)) return fail("obs_stride > 0 needs tau_ca_ms > 0");
+    return GN_OK;
+}
+
+Layout make_layout(const gn_config *cfg)
+{
+    const size_t N = cfg->n_vertices, Npad = (N + 127) / 128 * 128, E = cfg->n_edges, D = cfg->ring_slots;
+    const bool obs = cfg->obs_stride > 0;
+    Layout L{};
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off = align256(off + bytes); return o; };
+    L.V = take(Npad * 4); L.W = take(Npad * 4); L.r = take(Npad * 4);
+    L.c = take(obs ? Npad * 4 : 0); L.acc = take(obs ? Npad * 4 : 0);
+    L.bias = take(Npad * 4);
+    L.refr = take(Npad); L.cls = take(Npad);
+    L.ring = take(D * Npad * 4);
+    L.row = take((Npad + 1) * 4); L.tgt = take(E * 4); L.wfx = take(E * 4); L.dly = take(E);
+    L.active = take(2 * Npad * 4); L.n_active = take(8); L.counters = take(32);
+    L.raster = take((size_t)cfg->raster_capacity_steps * (Npad / 32) * 4);
+    L.trace = take(obs ? (size_t)cfg->trace_capacity_frames * Npad * 4 : 0);
+    L.scratch_row64 = take((N + 1) * 8); L.scratch_abs = take(N * 8);
+    L.scratch_pos = take(N * cfg->dim * 4); L.scratch_net = take(((size_t)cfg->n_networks + 1) * 4);
+    L.scratch_chk = take(sizeof(GnCheck));
+    L.total = off;
+    return L;
+}
+
+}  // namespace
+
+struct gn_net {
+    gn_config cfg;
+    GnDev dev;
+    Layout lay;
+    cudaStream_t stream;
+    uint8_t *ws;
+    uint64_t t;          // steps enqueued so far
+    bool has_bias;
+    char err[256];
+};
+
+namespace {
+
+int set_err(gn_net *net, int code, const char *fmt, ...)
+{
+    char *dst = net ? net->err : g_create_error;
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(dst, 256, fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define GN_CUDA(net, call)                                                                        \
+    do {                                                                                          \
+        cudaError_t e_ = (call);                                                                  \
+        if (e_ != cudaSuccess)                                                                    \
+            return set_err(net, GN_E_CUDA, "%s failed: %s", #call, cudaGetErrorString(e_));        \
+    } while (0)
+
+}  // namespace
+
+extern "C" {
+
+int gn_query_workspace(const gn_config *cfg, size_t *bytes)
+{
+    if (!bytes) { snprintf(g_create_error, sizeof g_create_error, "bytes is NULL"); return GN_E_INVALID_ARG; }
+    int rc = check_config(cfg, g_create_error, sizeof g_create_error);
+    if (rc) return rc;
+    *bytes = make_layout(cfg).total;
+    return GN_OK;
+}
+
+int gn_create(const gn_config *cfg, const gn_class_params *classes, const float *positions,
+              const uint64_t *row_offsets, const uint32_t *targets, const float *weights,
+              const uint8_t *delays, const uint8_t *vertex_class, const float *bias,
+              const uint32_t *net_offsets, void *workspace, size_t workspace_bytes,
+              void *cuda_stream, gn_net **out)
+{
+    if (out) *out = nullptr;
+    int rc = check_config(cfg, g_create_error, sizeof g_create_error);
+    if (rc) return rc;
+    if (!out || !classes || !row_offsets || !vertex_class || !workspace)
+        return set_err(nullptr, GN_E_INVALID_ARG, "NULL argument (out/classes/row_offsets/vertex_class/workspace)");
+    if (cfg->n_edges && (!targets || !weights))
+        return set_err(nullptr, GN_E_INVALID_ARG, "targets/weights are NULL with n_edges > 0");
+    if (cfg->n_edges && !delays && !positions)
+        return set_err(nullptr, GN_E_INVALID_ARG, "need delays or positions");
+    if (!delays && !(cfg->speed > 0.0f))
+        return set_err(nullptr, GN_E_INVALID_ARG, "speed must be > 0 when delays == NULL");
+    if (cfg->n_networks > 1 && !net_offsets)
+        return set_err(nullptr, GN_E_INVALID_ARG, "n_networks > 1 needs net_offsets");
+    if (((uintptr_t)workspace & 255u) != 0)
+        return set_err(nullptr, GN_E_INVALID_ARG, "workspace must be 256-byte aligned");
+    const Layout L = make_layout(cfg);
+    if (workspace_bytes < L.total)
+        return set_err(nullptr, GN_E_WORKSPACE_TOO_SMALL, "workspace has %zu bytes, need %zu", workspace_bytes, L.total);
+
+    int n_dev = 0;
+    GN_CUDA(nullptr, cudaGetDeviceCount(&n_dev));
+    if (n_dev < 1) return set_err(nullptr, GN_E_CUDA, "no CUDA device");
+    cudaPointerAttributes attr{};
+    GN_CUDA(nullptr, cudaPointerGetAttributes(&attr, workspace));
+    if (attr.type != cudaMemoryTypeDevice && attr.type != cudaMemoryTypeManaged)
+        return set_err(nullptr, GN_E_INVALID_ARG, "workspace is not device memory");
+
+    gn_net *net = new (std::nothrow) gn_net();
+    if (!net) return set_err(nullptr, GN_E_INVALID_ARG, "out of host memory");
+    net->cfg = *cfg;
+    net->lay = L;
+    net->stream = (cudaStream_t)cuda_stream;
+    net->ws = (uint8_t *)workspace;
+    net->t = 0;
+    net->has_bias = bias != nullptr;
+    net->err[0] = 0;
+
+    const uint32_t N = cfg->n_vertices, Npad = (N + 127) / 128 * 128;
+    const uint64_t E = cfg->n_edges;
+    uint8_t *ws = net->ws;
+    GnDev &d = net->dev;
+    memset(&d, 0, sizeof d);
+    d.N = N; d.Npad = Npad; d.D = cfg->ring_slots; d.words_pad = Npad / 32; d.n_classes = cfg->n_classes;
+    d.obs_stride = cfg->obs_stride; d.raster_cap = cfg->raster_capacity_steps;
+    d.trace_cap = cfg->obs_stride ? cfg->trace_capacity_frames : 0;
+    d.seed_lo = (uint32_t)cfg->seed; d.seed_hi = (uint32_t)(cfg->seed >> 32);
+    d.dt = cfg->dt_ms;
+    // constants: computed once in double, rounded once
+    d.keep_c = cfg->obs_stride ? (float)(1.0 - (double)cfg->dt_ms / (double)cfg->tau_ca_ms) : 0.0f;
+    d.ca_jump = cfg->ca_jump;
+    d.obs_gain = cfg->obs_gain; d.obs_offset = cfg->obs_offset; d.obs_sigma = cfg->obs_sigma;
+    d.inv_stride = cfg->obs_stride ? (float)(1.0 / (double)cfg->obs_stride) : 0.0f;
+    d.V = (float *)(ws + L.V); d.W = (float *)(ws + L.W); d.r = (float *)(ws + L.r);
+    d.c = cfg->obs_stride ? (float *)(ws + L.c) : nullptr;
+    d.acc = cfg->obs_stride ? (float *)(ws + L.acc) : nullptr;
+    d.bias = (float *)(ws + L.bias);
+    d.refr = ws + L.refr; d.cls = ws + L.cls;
+    d.ring = (int32_t *)(ws + L.ring);
+    d.row = (uint32_t *)(ws + L.row); d.tgt = (uint32_t *)(ws + L.tgt);
+    d.wfx = (int32_t *)(ws + L.wfx); d.dly = ws + L.dly;
+    d.active = (uint32_t *)(ws + L.active); d.n_active = (uint32_t *)(ws + L.n_active);
+    d.counters = (unsigned long long *)(ws + L.counters);
+    d.raster = (uint32_t *)(ws + L.raster);
+    d.trace = cfg->obs_stride ? (float *)(ws + L.trace) : nullptr;
+    for (uint32_t k = 0; k < cfg->n_classes; ++k) {
+        const gn_class_params &c = classes[k];
+        GnClassDev &q = d.cls_tab[k];
+        q.a = c.a; q.b = c.b; q.c_reset = c.c_reset; q.d = c.d;
+        q.k2 = c.k2; q.k1 = c.k1; q.k0 = c.k0; q.v_peak = c.v_peak;
+        q.direct = !(c.tau_syn_ms > 0.0f);
+        q.keep_s = q.direct ? 0.0f : (float)(1.0 - (double)cfg->dt_ms / (double)c.tau_syn_ms);
+        const double R = nearbyint((double)c.refractory_ms / (double)cfg->dt_ms);
+        if (!(R >= 0.0) || R > 255.0) {
+            delete net;
+            return set_err(nullptr, GN_E_INVALID_ARG, "class %u: refractory_ms / dt_ms must round to 0..255 steps", k);
+        }
+        q.R = (uint32_t)R;
+        const double pthr = (((double)c.drive_rate_hz * (double)cfg->dt_ms) * 1e-3) * 4294967296.0;
+        q.drive_thr = !(pthr > 0.0) ? 0u : (pthr >= 4294967295.0 ? 4294967295u : (uint32_t)floor(pthr));
+        const double kick = nearbyint((double)c.drive_kick * 65536.0);
+        if (!(fabs(kick) < 2147483648.0)) {
+            delete net;
+            return set_err(nullptr, GN_E_INVALID_ARG, "class %u: drive_kick out of the fixed-point range", k);
+        }
+        q.kick_fx = (int32_t)kick;
+        if (q.drive_thr) d.any_drive = 1u;
+    }
+
+    cudaStream_t st = net->stream;
+    uint64_t *row64 = (uint64_t *)(ws + L.scratch_row64);
+    unsigned long long *abs_in = (unsigned long long *)(ws + L.scratch_abs);
+    float *pos_d = (float *)(ws + L.scratch_pos);
+    uint32_t *net_d = (uint32_t *)(ws + L.scratch_net);
+    GnCheck *chk_d = (GnCheck *)(ws + L.scratch_chk);
+
+#define GN_CREATE_CUDA(call)                                                                      \
+    do {                                                                                          \
+        cudaError_t e_ = (call);                                                                  \
+        if (e_ != cudaSuccess) {                                                                  \
+            delete net;                                                                           \
+            return set_err(nullptr, GN_E_CUDA, "%s failed: %s", #call, cudaGetErrorString(e_));    \
+        }                                                                                         \
+    } while (0)
+
+    // zero everything the step loop accumulates into or reads before writing
+    GN_CREATE_CUDA(cudaMemsetAsync(ws, 0, L.tgt, st));                       // state, bias, refr, cls, ring, row
+    GN_CREATE_CUDA(cudaMemsetAsync(ws + L.active, 0, L.scratch_row64 - L.active, st));   // lists, counters, raster, trace
+    GN_CREATE_CUDA(cudaMemsetAsync(abs_in, 0, (size_t)N * 8, st));
+    GN_CREATE_CUDA(cudaMemsetAsync(chk_d, 0, sizeof(GnCheck), st));
+    // uploads (host or device sources)
+    GN_CREATE_CUDA(cudaMemcpyAsync(row64, row_offsets, ((size_t)N + 1) * 8, cudaMemcpyDefault, st));
+    GN_CREATE_CUDA(cudaMemcpyAsync(d.cls, vertex_class, N, cudaMemcpyDefault, st));
+    if (E) {
+        GN_CREATE_CUDA(cudaMemcpyAsync(d.tgt, targets, E * 4, cudaMemcpyDefault, st));
+        GN_CREATE_CUDA(cudaMemcpyAsync(d.wfx, weights, E * 4, cudaMemcpyDefault, st));   // fp32 bits, quantised in place
+        if (delays) GN_CREATE_CUDA(cudaMemcpyAsync(d.dly, delays, E, cudaMemcpyDefault, st));
+        else GN_CREATE_CUDA(cudaMemcpyAsync(pos_d, positions, (size_t)N * cfg->dim * 4, cudaMemcpyDefault, st));
+    }
+    if (bias) GN_CREATE_CUDA(cudaMemcpyAsync(d.bias, bias, (size_t)N * 4, cudaMemcpyDefault, st));
+    if (net_offsets)
+        GN_CREATE_CUDA(cudaMemcpyAsync(net_d, net_offsets, ((size_t)cfg->n_networks + 1) * 4, cudaMemcpyDefault, st));
+    // device-side conversion and validation
+    GN_CREATE_CUDA(gnk_convert_rows(d, row64, E, chk_d, st));
+    GN_CREATE_CUDA(gnk_init_state(d, chk_d, st));
+    GnCheck chk{};
+    GN_CREATE_CUDA(cudaMemcpyAsync(&chk, chk_d, sizeof chk, cudaMemcpyDeviceToHost, st));
+    GN_CREATE_CUDA(cudaStreamSynchronize(st));
+    if (chk.bad_row || chk.bad_class) {
+        delete net;
+        return set_err(nullptr, GN_E_BAD_GRAPH, chk.bad_row ? "row_offsets: not monotone, row_offsets[0] != 0 or row_offsets[N] != n_edges"
+                                                            : "vertex_class: id >= n_classes");
+    }
+    if (net_offsets) {   // host check of the (small) network table
+        // read back from the device copy so device-resident inputs work too
+        uint32_t first = 0, last = 0;
+        GN_CREATE_CUDA(cudaMemcpyAsync(&first, net_d, 4, cudaMemcpyDeviceToHost, st));
+        GN_CREATE_CUDA(cudaMemcpyAsync(&last, net_d + cfg->n_networks, 4, cudaMemcpyDeviceToHost, st));
+        GN_CREATE_CUDA(cudaStreamSynchronize(st));
+        if (first != 0 || last != N) {
+            delete net;
+            return set_err(nullptr, GN_E_BAD_GRAPH, "net_offsets must start at 0 and end at n_vertices");
+        }
+    }
+    if (E) {
+        GN_CREATE_CUDA(gnk_quantise(d, E, chk_d, st));
+        if (!delays) GN_CREATE_CUDA(gnk_delays_from_positions(d, pos_d, cfg->dim, cfg->speed, st));
+        GN_CREATE_CUDA(gnk_validate(d, net_offsets ? net_d : nullptr, cfg->n_networks, abs_in, chk_d, st));
+    }
+    GN_CREATE_CUDA(gnk_check_overflow(d, abs_in, chk_d, st));
+    GN_CREATE_CUDA(cudaMemcpyAsync(&chk, chk_d, sizeof chk, cudaMemcpyDeviceToHost, st));
+    GN_CREATE_CUDA(cudaStreamSynchronize(st));
+#undef GN_CREATE_CUDA
+    if (chk.bad_target || chk.bad_delay || chk.cross_net || chk.bad_weight) {
+        delete net;
+        return set_err(nullptr, GN_E_BAD_GRAPH, "%s",
+                       chk.bad_target ? "targets: id >= n_vertices"
+                       : chk.bad_delay ? "delay outside [1, ring_slots-1]"
+                       : chk.cross_net ? "edge crosses two networks"
+                                       : "weight is NaN or outside the int32 fixed-point range");
+    }
+    if (chk.overflow) {
+        delete net;
+        return set_err(nullptr, GN_E_OVERFLOW_RISK, "some target's sum |w_fx| + |kick_fx| exceeds 2^31 - 1");
+    }
+    *out = net;
+    return GN_OK;
+}
+
+int gn_step(gn_net *net, uint64_t n_steps)
+{
+    if (!net) return GN_E_INVALID_ARG;
+    const GnDev &d = net->dev;
+    for (uint64_t s = 0; s < n_steps; ++s) {
+        const uint64_t t = net->t;
+        GN_CUDA(net, gnk_update(d, t, net->has_bias, net->stream));
+        if (net->cfg.n_edges) GN_CUDA(net, gnk_deliver(d, t, net->stream));
+        if (d.obs_stride && (t + 1) % d.obs_stride == 0)
+            GN_CUDA(net, gnk_observe(d, (t + 1) / d.obs_stride - 1, net->stream));
+        net->t = t + 1;
+    }
+    return GN_OK;
+}
+
+static int copy_out(gn_net *net, void *dst, const void *src, size_t bytes, int dst_is_device)
+{
+    GN_CUDA(net, cudaMemcpyAsync(dst, src, bytes, dst_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, net->stream));
+    if (!dst_is_device) GN_CUDA(net, cudaStreamSynchronize(net->stream));
+    return GN_OK;
+}
+
+int gn_read_state(gn_net *net, int which, void *dst, size_t dst_bytes, int dst_is_device)
+{
+    if (!net) return GN_E_INVALID_ARG;
+    if (!dst) return set_err(net, GN_E_INVALID_ARG, "dst is NULL");
+    const GnDev &d = net->dev;
+    const size_t N = d.N, E = net->cfg.n_edges;
+    const void *src = nullptr;
+    size_t need = 0;
+    switch (which) {
+    case GN_V: src = d.V; need = N * 4; break;
+    case GN_W: src = d.W; need = N * 4; break;
+    case GN_R: src = d.r; need = N * 4; break;
+    case GN_CA:
+        if (!d.c) return set_err(net, GN_E_INVALID_ARG, "calcium is not maintained when obs_stride == 0");
+        src = d.c; need = N * 4; break;
+    case GN_REFR: src = d.refr; need = N; break;
+    case GN_BIAS:
+        if (!net->has_bias) return set_err(net, GN_E_INVALID_ARG, "no bias set");
+        src = d.bias; need = N * 4; break;
+    case GN_RING: need = (size_t)d.D * N * 4; break;
+    case GN_STEP: src = d.counters; need = 8; break;
+    case GN_COUNTERS: src = d.counters; need = 32; break;
+    case GN_DELAYS: src = d.dly; need = E; break;
+    case GN_WEIGHTS_FX: src = d.wfx; need = E * 4; break;
+    default: return set_err(net, GN_E_INVALID_ARG, "unknown state id %d", which);
+    }
+    if (dst_bytes < need) return set_err(net, GN_E_INVALID_ARG, "dst has %zu bytes, need %zu", dst_bytes, need);
+    if (need == 0) return GN_OK;
+    if (which == GN_RING) {   // internal rows are Npad wide; the caller's are N wide
+        GN_CUDA(net, cudaMemcpy2DAsync(dst, N * 4, d.ring, (size_t)d.Npad * 4, N * 4, d.D,
+                                       dst_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, net->stream));
+        if (!dst_is_device) GN_CUDA(net, cudaStreamSynchronize(net->stream));
+        return GN_OK;
+    }
+    return copy_out(net, dst, src, need, dst_is_device);
+}
+
+int gn_write_state(gn_net *net, int which, const void *src, size_t src_bytes, int src_is_device)
+{
+    if (!net) return GN_E_INVALID_ARG;
+    if (!src) return set_err(net, GN_E_INVALID_ARG, "src is NULL");
+    const GnDev &d = net->dev;
+    const size_t N = d.N;
+    void *dst = nullptr;
+    size_t need = N * 4;
+    switch (which) {
+    case GN_V: dst = d.V; break;
+    case GN_W: dst = d.W; break;
+    case GN_R: dst = d.r; break;
+    case GN_CA:
+        if (!d.c) return set_err(net, GN_E_INVALID_ARG, "calcium is not maintained when obs_stride == 0");
+        dst = d.c; break;
+    case GN_REFR: dst = d.refr; need = N; break;
+    case GN_BIAS: dst = d.bias; break;
+    default: return set_err(net, GN_E_INVALID_ARG, "state id %d is not writable", which);
+    }
+    if (src_bytes < need) return set_err(net, GN_E_INVALID_ARG, "src has %zu bytes, need %zu", src_bytes, need);
+    GN_CUDA(net, cudaMemcpyAsync(dst, src, need, src_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, net->stream));
+    if (!src_is_device) GN_CUDA(net, cudaStreamSynchronize(net->stream));
+    if (which == GN_BIAS) net->has_bias = true;
+    return GN_OK;
+}
+
+// Rows [i0, i0+n) of a circular device window of `cap` rows, `pitch_src` bytes apart, into a dense
+// destination of `width` bytes per row.
+static int copy_window(gn_net *net, void *dst, const uint8_t *base, size_t pitch_src, size_t width, uint64_t cap,
+                       uint64_t i0, uint64_t n, int dst_is_device)
+{
+    const cudaMemcpyKind kind = dst_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+    uint64_t done = 0;
+    while (done < n) {
+        const uint64_t r0 = (i0 + done) % cap;
+        const uint64_t chunk = (n - done < cap - r0) ? n - done : cap - r0;
+        GN_CUDA(net, cudaMemcpy2DAsync((uint8_t *)dst + done * width, width, base + r0 * pitch_src, pitch_src, width,
+                                       chunk, kind, net->stream));
+        done += chunk;
+    }
+    if (!dst_is_device) GN_CUDA(net, cudaStreamSynchronize(net->stream));
+    return GN_OK;
+}
+
+int gn_read_raster(gn_net *net, uint64_t t0, uint64_t n_steps, uint32_t *bits, size_t dst_bytes, int dst_is_device)
+{
+    if (!net) return GN_E_INVALID_ARG;
+    const GnDev &d = net->dev;
+    const size_t words = ((size_t)d.N + 31) / 32;
+    if (n_steps == 0) return GN_OK;
+    if (!bits) return set_err(net, GN_E_INVALID_ARG, "bits is NULL");
+    if (dst_bytes < n_steps * words * 4) return set_err(net, GN_E_INVALID_ARG, "dst has %zu bytes, need %zu", dst_bytes, (size_t)(n_steps * words * 4));
+    if (t0 + n_steps > net->t || d.raster_cap == 0 || t0 + d.raster_cap < net->t)
+        return set_err(net, GN_E_RANGE_EVICTED, "raster steps [%llu, %llu) not held: simulated %llu, window %u",
+                       (unsigned long long)t0, (unsigned long long)(t0 + n_steps), (unsigned long long)net->t, d.raster_cap);
+    return copy_window(net, bits, (const uint8_t *)d.raster, (size_t)d.words_pad * 4, words * 4, d.raster_cap, t0, n_steps, dst_is_device);
+}
+
+int gn_observe(gn_net *net, uint64_t frame0, uint64_t n_frames, float *trace, size_t dst_bytes, int dst_is_device)
+{
+    if (!net) return GN_E_INVALID_ARG;
+    const GnDev &d = net->dev;
+    if (!d.obs_stride) return set_err(net, GN_E_INVALID_ARG, "observation is off (obs_stride == 0)");
+    if (n_frames == 0) return GN_OK;
+    if (!trace) return set_err(net, GN_E_INVALID_ARG, "trace is NULL");
+    const uint64_t have = net->t / d.obs_stride;
+    if (dst_bytes < n_frames * d.N * 4) return set_err(net, GN_E_INVALID_ARG, "dst has %zu bytes, need %zu", dst_bytes, (size_t)(n_frames * d.N * 4));
+    if (frame0 + n_frames > have || frame0 + d.trace_cap < have)
+        return set_err(net, GN_E_RANGE_EVICTED, "frames [%llu, %llu) not held: emitted %llu, window %u",
+                       (unsigned long long)frame0, (unsigned long long)(frame0 + n_frames), (unsigned long long)have, d.trace_cap);
+    return copy_window(net, trace, (const uint8_t *)d.trace, (size_t)d.Npad * 4, (size_t)d.N * 4, d.trace_cap, frame0, n_frames, dst_is_device);
+}
+
+int gn_debug_words(void *cuda_stream, uint64_t seed, uint32_t stream_id, uint64_t idx, uint32_t first_vertex,
+                   uint32_t n, uint32_t *out)
+{
+    if (!out && n) return set_err(nullptr, GN_E_INVALID_ARG, "out is NULL");
+    GN_CUDA(nullptr, gnk_debug_words(seed, stream_id, idx, first_vertex, n, out, (cudaStream_t)cuda_stream));
+    return GN_OK;
+}
+
+const char *gn_last_error(const gn_net *net) { return net ? net->err : g_create_error; }
+
+int gn_destroy(gn_net *net)
+{
+    if (!net) return GN_E_INVALID_ARG;
+    cudaError_t e = cudaStreamSynchronize(net->stream);
+    delete net;
+    return e == cudaSuccess ? GN_OK : GN_E_CUDA;
+}
+
+}  // extern "C"

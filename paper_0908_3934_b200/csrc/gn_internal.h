@@ -1,0 +1,74 @@
+// gn_internal.h -- device-side view of one network and the kernel launchers (sm_100a only).
+// Shared by gn_api.cu (host logic of the C ABI) and gn_kernels.cu (every step of the hot path).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/gn.h"
+
+// Per-class constants, derived once on the host in double and rounded once (DESIGN.md
+// "Arithmetic contract"); 13 words each, staged into shared memory by the update kernel.
+struct GnClassDev {
+    float a, b, c_reset, d;
+    float k2, k1, k0, v_peak;
+    float keep_s;        // (float)(1 - dt/tau_s)
+    uint32_t direct;     // tau_syn_ms <= 0
+    uint32_t R;          // refractory steps, round(refractory_ms / dt)
+    uint32_t drive_thr;  // floor(rate * dt * 1e-3 * 2^32)
+    int32_t kick_fx;     // rint(kick * 2^16)
+};
+static_assert(sizeof(GnClassDev) == 13 * 4, "GnClassDev must stay 13 words");
+
+// Everything a kernel needs, passed by value (kernel parameter space).
+struct GnDev {
+    uint32_t N, Npad;        // Npad = N rounded up to 128: one warp of the update kernel owns 128 vertices
+    uint32_t D;              // ring slots
+    uint32_t words_pad;      // Npad / 32 raster words per step
+    uint32_t n_classes;
+    uint32_t obs_stride, raster_cap, trace_cap;
+    uint32_t seed_lo, seed_hi;
+    uint32_t any_drive;      // some class has drive_thr > 0
+    float dt, keep_c, ca_jump;
+    float obs_gain, obs_offset, obs_sigma, inv_stride;
+    // vertex state, SoA, each Npad long
+    float *V, *W, *r, *c, *acc, *bias;
+    uint8_t *refr, *cls;
+    // delay ring [D][Npad], int32 fixed point 2^-16
+    int32_t *ring;
+    // CSR by source
+    uint32_t *row;           // [Npad + 1]
+    uint32_t *tgt;           // [E]
+    int32_t *wfx;            // [E]
+    uint8_t *dly;            // [E]
+    // per-step active list, double buffered by step parity
+    uint32_t *active;        // [2][Npad]
+    uint32_t *n_active;      // [2]
+    unsigned long long *counters;   // steps, spikes, delivered events, kicks
+    uint32_t *raster;        // [raster_cap][words_pad]
+    float *trace;            // [trace_cap][Npad]
+    GnClassDev cls_tab[GN_MAX_CLASSES];
+};
+
+// Flags written by the create-time validation kernels.
+struct GnCheck {
+    uint32_t bad_row, bad_target, bad_delay, bad_class, bad_weight, cross_net, overflow;
+    uint32_t pad;
+};
+
+// ---- launchers (gn_kernels.cu).  All asynchronous on `st`; return the launch error. ----
+cudaError_t gnk_update(const GnDev &p, uint64_t t, bool has_bias, cudaStream_t st);
+cudaError_t gnk_deliver(const GnDev &p, uint64_t t, cudaStream_t st);
+cudaError_t gnk_observe(const GnDev &p, uint64_t frame, cudaStream_t st);
+cudaError_t gnk_init_state(const GnDev &p, GnCheck *chk, cudaStream_t st);
+cudaError_t gnk_convert_rows(const GnDev &p, const uint64_t *row64, uint64_t n_edges, GnCheck *chk,
+                             cudaStream_t st);
+cudaError_t gnk_quantise(const GnDev &p, uint64_t n_edges, GnCheck *chk, cudaStream_t st);
+cudaError_t gnk_delays_from_positions(const GnDev &p, const float *pos, uint32_t dim, float speed,
+                                      cudaStream_t st);
+cudaError_t gnk_validate(const GnDev &p, const uint32_t *net_of_vertex_offsets, uint32_t n_networks,
+                         unsigned long long *abs_in, GnCheck *chk, cudaStream_t st);
+cudaError_t gnk_check_overflow(const GnDev &p, const unsigned long long *abs_in, GnCheck *chk,
+                               cudaStream_t st);
+cudaError_t gnk_debug_words(uint64_t seed, uint32_t stream_id, uint64_t idx, uint32_t first,
+                            uint32_t n, uint32_t *out, cudaStream_t st);

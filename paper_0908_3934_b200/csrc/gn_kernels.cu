@@ -1,0 +1,475 @@
+// gn_kernels.cu -- every step of the hot path as hand-written CUDA for sm_100a.
+//
+//   gn_update_kernel   ring-slot read-and-clear + drive + Izhikevich/PSC/calcium update +
+//                      spike detection, raster bits and ballot/popc compaction
+//   gn_deliver_kernel  warp-per-active-source CSR expansion, int32 RED into the delay ring  (a4)
+//   gn_observe_kernel  frame mean -> gain/offset + Gaussian noise -> trace row              (a5)
+//   create-time kernels: row conversion, weight quantisation, eq. 25 delays, validation.
+//
+// Arithmetic contract: every floating-point operation of the update is an explicit
+// round-to-nearest intrinsic in a fixed order, so the result is bit-identical to the fp32-faithful
+// CPU oracle.  Delivery and the drive decision are integer; atomics are order-independent.
+// Paper line numbers refer to /root/reference/PAPER.md.
+#include "gn_internal.h"
+
+namespace {
+
+constexpr int kUpdateThreads = 256;          // 8 warps x 128 vertices = 1024 vertices per CTA
+constexpr int kVertsPerThread = 4;           // one 128-bit load per SoA array
+constexpr int kDeliverThreads = 256;
+constexpr uint32_t kStreamDrive = 5, kStreamNoise = 6;
+
+// ---- Philox4x32-10 (Salmon et al., SC'11), from its published description -------------------
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                              uint32_t k0, uint32_t k1, uint32_t (&out)[4])
+{
+#pragma unroll
+    for (int round = 0; round < 10; ++round) {
+        const uint32_t lo0 = 0xD2511F53u * c0, hi0 = __umulhi(0xD2511F53u, c0);
+        const uint32_t lo1 = 0xCD9E8D57u * c2, hi1 = __umulhi(0xCD9E8D57u, c2);
+        c0 = hi1 ^ c1 ^ k0;
+        c1 = lo1;
+        c2 = hi0 ^ c3 ^ k1;
+        c3 = lo0;
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// ---- one vertex, one step: eq. 24 + :303 eq. 28 + :283-286 eq. 26 ------------
+// Reads the state at t, writes the state at t+1, returns spd(V(t)) gated by refractoriness.
+template <bool BIAS>
+__device__ __forceinline__ bool vertex_step(const GnClassDev &q, const float dt, const int32_t I_fx,
+                                            const float U, float &V, float &W, float &r, uint32_t &refr)
+{
+    const float If = __fmul_rn(__int2float_rn(I_fx), 0x1p-16f);
+    const bool fired = (refr == 0u) && (V >= q.v_peak);                  // eq. 31 (>=)
+    const float u1 = __fmaf_rn(q.b, V, -W);
+    const float u2 = __fmul_rn(q.a, u1);
+    const float W_euler = __fmaf_rn(dt, u2, W);                          // eq. 24, W line
+    float Vn, Wn;
+    if (fired) {                                                         // eq. 24 "otherwise"
+        Vn = q.c_reset;
+        Wn = __fadd_rn(W, q.d);
+        refr = q.R;
+    } else if (refr > 0u) {                                              // refractory hold (reading #6)
+        Vn = q.c_reset;
+        Wn = W_euler;
+        refr -= 1u;
+    } else {                                                             // eq. 28, V < V_peak
+        const float t1 = __fmaf_rn(q.k2, V, q.k1);
+        const float t2 = __fmaf_rn(t1, V, q.k0);
+        const float t3 = __fsub_rn(t2, W);
+        float t4 = q.direct ? t3 : __fadd_rn(t3, r);
+        if (BIAS) t4 = __fadd_rn(t4, U);
+        Vn = __fmaf_rn(dt, t4, V);
+        if (q.direct) Vn = __fadd_rn(Vn, If);
+        Wn = W_euler;
+    }
+    if (!q.direct) r = __fmaf_rn(q.keep_s, r, If);                       // eq. 26
+    V = Vn;
+    W = Wn;
+    return fired;
+}
+
+// ---- a1 + a2 + a3 (+ calcium of a5) ---------------------------------------------------------------
+// Thread g owns vertices 4g .. 4g+3 (128-bit SoA loads); a warp owns 128 vertices = 4 raster words.
+template <bool OBS, bool BIAS>
+__global__ void __launch_bounds__(kUpdateThreads)
+gn_update_kernel(const GnDev p, const uint64_t t, const uint32_t slot, const uint32_t parity,
+                 const uint32_t raster_row)
+{
+    __shared__ GnClassDev s_cls[GN_MAX_CLASSES];
+    __shared__ uint32_t s_cnt[kUpdateThreads / 32];
+    __shared__ uint32_t s_kick[kUpdateThreads / 32];
+    __shared__ uint32_t s_base;
+
+    if (threadIdx.x < p.n_classes * 13u)
+        reinterpret_cast<uint32_t *>(s_cls)[threadIdx.x] = reinterpret_cast<const uint32_t *>(p.cls_tab)[threadIdx.x];
+    if (blockIdx.x == 0 && threadIdx.x == 0) p.n_active[parity ^ 1u] = 0u;   // list of step t+1
+    __syncthreads();
+
+    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    const uint32_t g = blockIdx.x * kUpdateThreads + threadIdx.x;
+    const uint32_t j0 = g * kVertsPerThread;
+    uint32_t nib = 0u, kicks = 0u;                                        // bit q: vertex j0+q fired / kicked
+
+    if (j0 < p.Npad) {
+        // a1: read this step's ring slot, clear it only if something arrived
+        int4 *slot_ptr = reinterpret_cast<int4 *>(p.ring + (size_t)slot * p.Npad + j0);
+        int4 I4 = *slot_ptr;
+        if ((I4.x | I4.y | I4.z | I4.w) != 0) *slot_ptr = make_int4(0, 0, 0, 0);
+        float4 V4 = *reinterpret_cast<const float4 *>(p.V + j0);
+        float4 W4 = *reinterpret_cast<const float4 *>(p.W + j0);
+        float4 r4 = *reinterpret_cast<const float4 *>(p.r + j0);
+        const uchar4 rf4 = *reinterpret_cast<const uchar4 *>(p.refr + j0);
+        const uchar4 cl4 = *reinterpret_cast<const uchar4 *>(p.cls + j0);
+        float4 U4 = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (BIAS) U4 = *reinterpret_cast<const float4 *>(p.bias + j0);
+        float4 c4 = make_float4(0.f, 0.f, 0.f, 0.f), a4 = c4;
+        if (OBS) {
+            c4 = *reinterpret_cast<const float4 *>(p.c + j0);
+            a4 = *reinterpret_cast<const float4 *>(p.acc + j0);
+        }
+
+        int32_t I[4] = {I4.x, I4.y, I4.z, I4.w};
+        float V[4] = {V4.x, V4.y, V4.z, V4.w}, W[4] = {W4.x, W4.y, W4.z, W4.w};
+        float r[4] = {r4.x, r4.y, r4.z, r4.w}, U[4] = {U4.x, U4.y, U4.z, U4.w};
+        float c[4] = {c4.x, c4.y, c4.z, c4.w}, acc[4] = {a4.x, a4.y, a4.z, a4.w};
+        uint32_t refr[4] = {rf4.x, rf4.y, rf4.z, rf4.w};
+        const uint32_t cl[4] = {cl4.x, cl4.y, cl4.z, cl4.w};
+
+        // drive: one Philox block per 4 vertices, counter {j/4, t lo, t hi, 5}, word j mod 4
+        uint32_t x[4] = {0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu};
+        if (p.any_drive)
+            philox4x32_10(g, (uint32_t)t, (uint32_t)(t >> 32), kStreamDrive, p.seed_lo, p.seed_hi, x);
+
+        uint32_t refr_changed = 0u;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const GnClassDev &k = s_cls[cl[q]];
+            const bool live = (j0 + q) < p.N;
+            if (live && x[q] < k.drive_thr) {                              // Bernoulli kick (reading #12)
+                I[q] += k.kick_fx;
+                kicks |= 1u << q;
+            }
+            const uint32_t refr_old = refr[q];
+            const bool fired = vertex_step<BIAS>(k, p.dt, I[q], U[q], V[q], W[q], r[q], refr[q]) && live;
+            refr_changed |= (refr[q] != refr_old);
+            if (fired) nib |= 1u << q;
+            if (OBS) {
+                c[q] = __fmaf_rn(p.keep_c, c[q], fired ? p.ca_jump : 0.0f);   // H_c
+                acc[q] = __fadd_rn(acc[q], c[q]);
+            }
+        }
+        *reinterpret_cast<float4 *>(p.V + j0) = make_float4(V[0], V[1], V[2], V[3]);
+        *reinterpret_cast<float4 *>(p.W + j0) = make_float4(W[0], W[1], W[2], W[3]);
+        *reinterpret_cast<float4 *>(p.r + j0) = make_float4(r[0], r[1], r[2], r[3]);
+        if (refr_changed)
+            *reinterpret_cast<uchar4 *>(p.refr + j0) = make_uchar4(refr[0], refr[1], refr[2], refr[3]);
+        if (OBS) {
+            *reinterpret_cast<float4 *>(p.c + j0) = make_float4(c[0], c[1], c[2], c[3]);
+            *reinterpret_cast<float4 *>(p.acc + j0) = make_float4(acc[0], acc[1], acc[2], acc[3]);
+        }
+    }
+
+    // a3: raster bits.  Lane l holds bits 4*(l%8) .. +3 of word l/8 of this warp's 4 words.
+    uint32_t word = nib << (4u * (lane & 7u));
+    word |= __shfl_xor_sync(0xFFFFFFFFu, word, 1);
+    word |= __shfl_xor_sync(0xFFFFFFFFu, word, 2);
+    word |= __shfl_xor_sync(0xFFFFFFFFu, word, 4);
+    if (p.raster_cap && (lane & 7u) == 0u && j0 < p.Npad)
+        p.raster[(size_t)raster_row * p.words_pad + (j0 >> 5)] = word;
+
+    // a3: compaction.  Ballot per vertex slot q, popc ranks, one global atomic per CTA.
+    uint32_t b[4], warp_total = 0u, warp_kicks = 0u;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        b[q] = __ballot_sync(0xFFFFFFFFu, (nib >> q) & 1u);
+        warp_total += __popc(b[q]);
+        warp_kicks += __popc(__ballot_sync(0xFFFFFFFFu, (kicks >> q) & 1u));
+    }
+    if (lane == 0) {
+        s_cnt[warp] = warp_total;
+        s_kick[warp] = warp_kicks;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        uint32_t total = 0u, ktotal = 0u;
+#pragma unroll
+        for (int w = 0; w < kUpdateThreads / 32; ++w) {
+            total += s_cnt[w];
+            ktotal += s_kick[w];
+        }
+        uint32_t base = 0u;
+        if (total) {
+            base = atomicAdd(&p.n_active[parity], total);
+            atomicAdd(&p.counters[1], (unsigned long long)total);
+        }
+        if (ktotal) atomicAdd(&p.counters[3], (unsigned long long)ktotal);
+        if (blockIdx.x == 0) p.counters[0] = t + 1ull;
+        s_base = base;
+    }
+    __syncthreads();
+    if (warp_total) {
+        uint32_t off = s_base;
+        for (uint32_t w = 0; w < warp; ++w) off += s_cnt[w];
+        uint32_t *list = p.active + (size_t)parity * p.Npad;
+        const uint32_t lt = (1u << lane) - 1u;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            if ((nib >> q) & 1u) list[off + __popc(b[q] & lt)] = j0 + q;
+            off += __popc(b[q]);
+        }
+    }
+}
+
+// ---- a4: event delivery -------------------------------------------------------------------------------
+// One warp per active source; lanes stride over the source's CSR row (coalesced target / weight /
+// delay reads); each edge is one int32 reduction (RED.ADD, no return) into ring[(t+delay) mod D][tgt].
+// PAPER.md:311 eq. 30 / :297.
+__global__ void __launch_bounds__(kDeliverThreads)
+gn_deliver_kernel(const GnDev p, const uint32_t slot_t, const uint32_t parity)
+{
+    const uint32_t lane = threadIdx.x & 31u;
+    const uint32_t warp_global = (blockIdx.x * kDeliverThreads + threadIdx.x) >> 5;
+    const uint32_t n_warps = (gridDim.x * kDeliverThreads) >> 5;
+    const uint32_t n = p.n_active[parity];
+    const uint32_t *__restrict__ list = p.active + (size_t)parity * p.Npad;
+    const uint32_t *__restrict__ row = p.row;
+    const uint32_t *__restrict__ tgt = p.tgt;
+    const int32_t *__restrict__ wfx = p.wfx;
+    const uint8_t *__restrict__ dly = p.dly;
+    unsigned long long events = 0ull;
+    for (uint32_t idx = warp_global; idx < n; idx += n_warps) {
+        const uint32_t src = list[idx];
+        const uint32_t beg = row[src], end = row[src + 1];
+        for (uint32_t e = beg + lane; e < end; e += 32u) {
+            const uint32_t m = tgt[e];
+            const int32_t w = wfx[e];
+            uint32_t s = slot_t + (uint32_t)dly[e];
+            if (s >= p.D) s -= p.D;
+            atomicAdd(p.ring + (size_t)s * p.Npad + m, w);
+        }
+        events += (unsigned long long)(end - beg);
+    }
+    if (lane == 0 && events) atomicAdd(&p.counters[2], events);
+}
+
+// ---- a5: one camera frame -------------------------------------------------------------------------------
+// z_j = n * mean(c_j over the frame) + b + gamma * N(0,1).  Box-Muller on the
+// vertex group's Philox block: counter {j/4, frame lo, frame hi, 6}; vertices 0,1 use words (x0,x1),
+// vertices 2,3 use (x2,x3); even vertex = cosine branch, odd = sine branch.
+__global__ void __launch_bounds__(256)
+gn_observe_kernel(const GnDev p, const uint64_t frame, const uint32_t trace_row)
+{
+    const uint32_t g = blockIdx.x * 256u + threadIdx.x;
+    const uint32_t j0 = g * 4u;
+    if (j0 >= p.Npad) return;
+    const float4 a4 = *reinterpret_cast<const float4 *>(p.acc + j0);
+    float z[4] = {0.f, 0.f, 0.f, 0.f};
+    if (p.obs_sigma != 0.0f) {
+        uint32_t x[4];
+        philox4x32_10(g, (uint32_t)frame, (uint32_t)(frame >> 32), kStreamNoise, p.seed_lo, p.seed_hi, x);
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const float ua = __fmaf_rn((float)(x[2 * h] >> 9), 0x1p-23f, 0x1p-24f);   // (k + 1/2) 2^-23
+            const float ub2 = __fmul_rn((float)(x[2 * h + 1] >> 8), 0x1p-23f);         // 2 * u_b
+            const float rad = sqrtf(-2.0f * logf(ua));
+            float sn, cs;
+            sincospif(ub2, &sn, &cs);
+            z[2 * h] = rad * cs;
+            z[2 * h + 1] = rad * sn;
+        }
+    }
+    const float acc[4] = {a4.x, a4.y, a4.z, a4.w};
+    float out[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q)
+        out[q] = p.obs_gain * (acc[q] * p.inv_stride) + p.obs_offset + p.obs_sigma * z[q];
+    *reinterpret_cast<float4 *>(p.trace + (size_t)trace_row * p.Npad + j0) = make_float4(out[0], out[1], out[2], out[3]);
+    *reinterpret_cast<float4 *>(p.acc + j0) = make_float4(0.f, 0.f, 0.f, 0.f);
+}
+
+// ---- create-time kernels --------------------------------------------------------------------------------
+__global__ void gn_init_state_kernel(const GnDev p, GnCheck *chk)
+{
+    const uint32_t j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= p.Npad) return;
+    uint32_t k = p.cls[j];
+    if (j >= p.N) k = 0u;
+    if (k >= p.n_classes) {
+        chk->bad_class = 1u;
+        k = 0u;
+    }
+    p.V[j] = -70.0f;                                        // reading #15
+    p.W[j] = __fmul_rn(p.cls_tab[k].b, -70.0f);
+    p.r[j] = 0.0f;
+    p.refr[j] = 0;
+    if (p.c) { p.c[j] = 0.0f; p.acc[j] = 0.0f; }
+}
+
+__global__ void gn_convert_rows_kernel(const GnDev p, const uint64_t *row64, const uint64_t n_edges, GnCheck *chk)
+{
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i > p.Npad) return;
+    if (i > p.N) { p.row[i] = (uint32_t)n_edges; return; }
+    const uint64_t v = row64[i];
+    if (i == 0 && v != 0ull) chk->bad_row = 1u;
+    if (i == p.N && v != n_edges) chk->bad_row = 1u;
+    if (i < p.N && row64[i + 1] < v) chk->bad_row = 1u;
+    if (v > n_edges) chk->bad_row = 1u;
+    p.row[i] = (uint32_t)(v > n_edges ? n_edges : v);
+}
+
+// w_fx = rint(w * 2^16), ties to even, in place over the fp32 weights (w * 2^16 is exact in binary32).
+__global__ void gn_quantise_kernel(const GnDev p, const uint64_t n_edges, GnCheck *chk)
+{
+    for (uint64_t e = blockIdx.x * (uint64_t)blockDim.x + threadIdx.x; e < n_edges; e += (uint64_t)gridDim.x * blockDim.x) {
+        const float s = __fmul_rn(__int_as_float(p.wfx[e]), 65536.0f);
+        if (!(fabsf(s) < 2147483648.0f)) {                  // also catches NaN
+            chk->bad_weight = 1u;
+            p.wfx[e] = 0;
+        } else {
+            p.wfx[e] = __float2int_rn(s);
+        }
+    }
+}
+
+// PAPER.md:251 eq. 25 in steps: max(1, ceil(|x_i - x_j| / (speed * dt))), double, no contraction.
+__global__ void gn_delays_kernel(const GnDev p, const float *__restrict__ pos, const uint32_t dim, const float speed)
+{
+    const uint32_t lane = threadIdx.x & 31u;
+    const uint32_t i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    if (i >= p.N) return;
+    const double per_step = __dmul_rn((double)speed, (double)p.dt);
+    double xi[3] = {0.0, 0.0, 0.0};
+    for (uint32_t k = 0; k < dim; ++k) xi[k] = (double)pos[(size_t)i * dim + k];
+    for (uint32_t e = p.row[i] + lane; e < p.row[i + 1]; e += 32u) {
+        const uint32_t m = p.tgt[e];
+        double d2 = 0.0;
+        if (m < p.N) {
+            for (uint32_t k = 0; k < dim; ++k) {
+                const double d = __dsub_rn(xi[k], (double)pos[(size_t)m * dim + k]);
+                d2 = __dadd_rn(d2, __dmul_rn(d, d));
+            }
+        }
+        double steps = ceil(__ddiv_rn(__dsqrt_rn(d2), per_step));
+        if (!(steps >= 1.0)) steps = 1.0;                   // coincident points (reading #7); NaN -> flagged below
+        if (steps > 255.0) steps = 255.0;                   // >= D is rejected by the validation kernel
+        p.dly[e] = (uint8_t)steps;
+    }
+}
+
+// Per edge: target range, delay range, same network; per target: sum of |w_fx| (overflow bound).
+__global__ void gn_validate_kernel(const GnDev p, const uint32_t *__restrict__ net_offsets, const uint32_t n_networks,
+                                   unsigned long long *abs_in, GnCheck *chk)
+{
+    const uint32_t lane = threadIdx.x & 31u;
+    const uint32_t i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    if (i >= p.N) return;
+    uint32_t lo_v = 0u, hi_v = p.N;                          // vertex range of i's network
+    if (net_offsets) {
+        uint32_t lo = 0u, hi = n_networks;                   // find b with net_offsets[b] <= i < net_offsets[b+1]
+        while (hi - lo > 1u) {
+            const uint32_t mid = (lo + hi) >> 1;
+            if (net_offsets[mid] <= i) lo = mid; else hi = mid;
+        }
+        lo_v = net_offsets[lo];
+        hi_v = net_offsets[lo + 1];
+    }
+    for (uint32_t e = p.row[i] + lane; e < p.row[i + 1]; e += 32u) {
+        const uint32_t m = p.tgt[e];
+        const uint32_t d = p.dly[e];
+        if (d < 1u || d > p.D - 1u) chk->bad_delay = 1u;
+        if (m >= p.N) { chk->bad_target = 1u; continue; }
+        if (m < lo_v || m >= hi_v) chk->cross_net = 1u;
+        const int32_t w = p.wfx[e];
+        const unsigned long long a = (unsigned long long)(w < 0 ? -(long long)w : (long long)w);
+        if (a) atomicAdd(&abs_in[m], a);
+    }
+}
+
+__global__ void gn_check_overflow_kernel(const GnDev p, const unsigned long long *__restrict__ abs_in, GnCheck *chk)
+{
+    const uint32_t j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= p.N) return;
+    uint32_t k = p.cls[j];
+    if (k >= p.n_classes) k = 0u;
+    const long long kick = p.cls_tab[k].kick_fx;
+    const unsigned long long bound = abs_in[j] + (unsigned long long)(kick < 0 ? -kick : kick);
+    if (bound > 2147483647ull) chk->overflow = 1u;
+}
+
+__global__ void gn_debug_words_kernel(const uint32_t seed_lo, const uint32_t seed_hi, const uint32_t stream_id,
+                                      const uint64_t idx, const uint32_t first, const uint32_t n, uint32_t *out)
+{
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const uint32_t j = first + i;
+    uint32_t x[4];
+    philox4x32_10(j >> 2, (uint32_t)idx, (uint32_t)(idx >> 32), stream_id, seed_lo, seed_hi, x);
+    out[i] = x[j & 3u];
+}
+
+inline uint32_t ceil_div(uint64_t a, uint64_t b) { return (uint32_t)((a + b - 1) / b); }
+
+}  // namespace
+
+// ---- launchers ------------------------------------------------------------------------------------------
+cudaError_t gnk_update(const GnDev &p, uint64_t t, bool has_bias, cudaStream_t st)
+{
+    const uint32_t grid = ceil_div(p.Npad / kVertsPerThread, kUpdateThreads);
+    const uint32_t slot = (uint32_t)(t % p.D), parity = (uint32_t)(t & 1ull);
+    const uint32_t raster_row = p.raster_cap ? (uint32_t)(t % p.raster_cap) : 0u;
+    const bool obs = p.obs_stride != 0u;
+    if (obs && has_bias) gn_update_kernel<true, true><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, parity, raster_row);
+    else if (obs) gn_update_kernel<true, false><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, parity, raster_row);
+    else if (has_bias) gn_update_kernel<false, true><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, parity, raster_row);
+    else gn_update_kernel<false, false><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, parity, raster_row);
+    return cudaGetLastError();
+}
+
+cudaError_t gnk_deliver(const GnDev &p, uint64_t t, cudaStream_t st)
+{
+    // enough warps for one source each up to full residency (148 SMs x 8 CTAs), never more than N
+    uint32_t grid = ceil_div(p.N, kDeliverThreads / 32);
+    if (grid > 148u * 8u) grid = 148u * 8u;
+    gn_deliver_kernel<<<grid, kDeliverThreads, 0, st>>>(p, (uint32_t)(t % p.D), (uint32_t)(t & 1ull));
+    return cudaGetLastError();
+}
+
+cudaError_t gnk_observe(const GnDev &p, uint64_t frame, cudaStream_t st)
+{
+    gn_observe_kernel<<<ceil_div(p.Npad / 4, 256), 256, 0, st>>>(p, frame, (uint32_t)(frame % p.trace_cap));
+    return cudaGetLastError();
+}
+
+cudaError_t gnk_init_state(const GnDev &p, GnCheck *chk, cudaStream_t st)
+{
+    gn_init_state_kernel<<<ceil_div(p.Npad, 256), 256, 0, st>>>(p, chk);
+    return cudaGetLastError();
+}
+
+cudaError_t gnk_convert_rows(const GnDev &p, const uint64_t *row64, uint64_t n_edges, GnCheck *chk, cudaStream_t st)
+{
+    gn_convert_rows_kernel<<<ceil_div((uint64_t)p.Npad + 1, 256), 256, 0, st>>>(p, row64, n_edges, chk);
+    return cudaGetLastError();
+}
+
+cudaError_t gnk_quantise(const GnDev &p, uint64_t n_edges, GnCheck *chk, cudaStream_t st)
+{
+    if (n_edges == 0) return cudaSuccess;
+    uint32_t grid = ceil_div(n_edges, 256);
+    if (grid > 148u * 32u) grid = 148u * 32u;
+    gn_quantise_kernel<<<grid, 256, 0, st>>>(p, n_edges, chk);
+    return cudaGetLastError();
+}
+
+cudaError_t gnk_delays_from_positions(const GnDev &p, const float *pos, uint32_t dim, float speed, cudaStream_t st)
+{
+    gn_delays_kernel<<<ceil_div((uint64_t)p.N * 32, 256), 256, 0, st>>>(p, pos, dim, speed);
+    return cudaGetLastError();
+}
+
+cudaError_t gnk_validate(const GnDev &p, const uint32_t *net_offsets, uint32_t n_networks,
+                         unsigned long long *abs_in, GnCheck *chk, cudaStream_t st)
+{
+    gn_validate_kernel<<<ceil_div((uint64_t)p.N * 32, 256), 256, 0, st>>>(p, net_offsets, n_networks, abs_in, chk);
+    return cudaGetLastError();
+}
+
+cudaError_t gnk_check_overflow(const GnDev &p, const unsigned long long *abs_in, GnCheck *chk, cudaStream_t st)
+{
+    gn_check_overflow_kernel<<<ceil_div(p.N, 256), 256, 0, st>>>(p, abs_in, chk);
+    return cudaGetLastError();
+}
+
+cudaError_t gnk_debug_words(uint64_t seed, uint32_t stream_id, uint64_t idx, uint32_t first, uint32_t n,
+                            uint32_t *out, cudaStream_t st)
+{
+    if (n == 0) return cudaSuccess;
+    gn_debug_words_kernel<<<ceil_div(n, 256), 256, 0, st>>>((uint32_t)seed, (uint32_t)(seed >> 32), stream_id, idx, first, n, out);
+    return cudaGetLastError();
+}
