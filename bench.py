@@ -1,0 +1,369 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the geometric-network hot path on B200 (contract in the task prompt).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W]            # our arm (CUDA library via the C ABI)
+  python bench.py --impl reference [--steps K] [--warmup W]      # the CPU oracle on the host cores
+
+Workload (config.workload): BASELINE.json configs[3] -- the 1M-vertex / ~200M-edge 3D random geometric
+graph the real-time-factor target is quoted on.  One bench "step" is
+`sim_steps_per_step` (default 100 = 10 ms simulated) consecutive passes of the whole hot path
+(a1 ring read-and-clear + drive, a2 vertex update, a3 detect/compact/raster, a4 event delivery;
+a5 observation when the config has it), so the default K=100 is the config's full 10,000-step run.
+`value` = simulated vertex-steps per second with every input resident in HBM.  L2 is not flushed
+between steps: the working set (512 MB ring + 1.8 GB edges + 16 MB state) is >> the 126 MB L2.
+
+One JSON line on stdout (rank 0).  Everything else goes to stderr.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC, UNIT = "vertex-steps/s", "vertex-steps/s"
+UPDATE_BYTES_PER_VERTEX = 35.125       # V,W,r r+w 24, ring slot r+clear 8, refr 2, class 1, raster bit 1/8
+UPDATE_BYTES_PER_VERTEX_OBS = 12.0     # + c r+w 8, frame accumulator amortised / trace row 4 per frame (counted per step as 4)
+EVENT_BYTES = 17.0                     # edge record 9 (target 4, weight 4, delay 1) + ring word read-modify-write 8
+SOURCE_BYTES = 12.0                    # two row offsets + active-list entry per fired source
+SECTOR_EVENT_BYTES = 73.0              # 9 + one 32 B sector fetched + one written back (ring >> L2)
+
+
+def log(*a):
+    print(*a, file=sys.stderr, flush=True)
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, burst copy)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception as e:   # no nvidia-smi: report that, do not invent clocks
+            log("clock sampler unavailable:", e)
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        self.thread.join(timeout=2)
+        sm, smax, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0]))
+                smax.append(float(r[1]))
+                for nm, v in zip(names, r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(nm)
+            except Exception:
+                continue
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(smax)), "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def workload_name(net_in, cfg, args):
+    return (f"BASELINE configs[{args.config - 1}] {cfg['name']}: N={net_in.n_vertices}, E={net_in.n_edges}, "
+            f"D={cfg['ring_slots']}, dt={cfg['dt_ms']} ms")
+
+
+# ---------------------------------------------------------------------------------------------------
+def run_reference(args):
+    """The oracle, as it stands, on the host cores: same config / metric / unit; each bench step is a
+    bounded sample (a few simulated steps of the full-size network) so the run ends in minutes."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from gn_inputs import make_config
+    from oracle import Oracle
+    cores = len(os.sched_getaffinity(0))
+    t0 = time.time()
+    net_in, cfg = make_config(args.config, n=args.n)
+    cfg = dict(cfg, obs_stride=0 if args.config == 4 else cfg["obs_stride"])
+    log(f"[reference] inputs in {time.time() - t0:.1f} s: N={net_in.n_vertices} E={net_in.n_edges}")
+    o = Oracle(net_in, cfg, "fp32", threads=cores)
+    t0 = time.time()
+    o.step(1)
+    t1 = max(time.time() - t0, 1e-6)
+    budget = 90.0
+    s_ref = int(max(1, min(args.sim_steps, budget / (args.steps + args.warmup) / t1)))
+    for _ in range(args.warmup):
+        o.step(s_ref)
+    c0 = o.counters()
+    t0 = time.time()
+    for _ in range(args.steps):
+        o.step(s_ref)
+    dt = time.time() - t0
+    c1 = o.counters()
+    n = net_in.n_vertices
+    value = n * s_ref * args.steps / dt
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": 0, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": workload_name(net_in, cfg, args), "sim_steps_per_step": s_ref,
+                   "note": "oracle/gn_oracle.c fp32-faithful mode, OpenMP over vertices / fired sources, from rest"},
+        "events_per_s": (c1["delivered"] - c0["delivered"]) / dt,
+        "real_time_factor": s_ref * args.steps * cfg["dt_ms"] * 1e-3 / dt,
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
+                         "sample": f"{(args.steps + args.warmup) * s_ref + 1} simulated steps of the full network from rest; "
+                                   f"timed {args.steps * s_ref}"},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ---------------------------------------------------------------------------------------------------
+def cpu_baseline(net_in, cfg, budget_s=20.0):
+    from oracle import Oracle
+    cores = len(os.sched_getaffinity(0))
+    o = Oracle(net_in, cfg, "fp32", threads=cores)
+    t0 = time.time()
+    o.step(2)
+    per = max((time.time() - t0) / 2, 1e-6)
+    n_steps = int(max(5, min(2000, budget_s / per)))
+    c0 = o.counters()
+    t0 = time.time()
+    o.step(n_steps)
+    dt = time.time() - t0
+    c1 = o.counters()
+    return {"value": net_in.n_vertices * n_steps / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{n_steps} simulated steps of the same full-size network from rest (fp32-faithful mode, OpenMP), "
+                      f"{c1['delivered'] - c0['delivered']} events delivered",
+            "events_per_s": (c1["delivered"] - c0["delivered"]) / dt,
+            "real_time_factor": n_steps * cfg["dt_ms"] * 1e-3 / dt}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=4)
+    ap.add_argument("--n", type=int, default=None, help="override the vertex count (debugging only)")
+    ap.add_argument("--sim-steps", type=int, default=100, help="simulated steps per bench step")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (this library has no CPU fallback)")
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    import paper_0908_3934_b200 as gn
+    from gn_inputs import MASTER_SEED, make_config
+
+    K, W, S = args.steps, max(args.warmup, 3), args.sim_steps
+    t0 = time.time()
+    # replicas only: rank r steps its own independent network of the same recipe
+    net_in, cfg = make_config(args.config, n=args.n, seed=MASTER_SEED + args.config + 1000 * rank)
+    N, E = net_in.n_vertices, net_in.n_edges
+    log(f"[rank {rank}] inputs in {time.time() - t0:.1f} s: N={N} E={E} mean out-degree {E / N:.1f}")
+    obs = int(cfg["obs_stride"])
+    frames_per_step = S // obs if obs else 0
+
+    def create(arrays=None):
+        a = arrays or dict(pos=net_in.positions, row=net_in.row_offsets, tgt=net_in.targets, w=net_in.weights,
+                           cls=net_in.vertex_class, net=net_in.net_offsets)
+        c = gn.make_config(N, net_in.dim, E, cfg["ring_slots"], cfg["dt_ms"], cfg["speed"], len(cfg["classes"]),
+                           n_networks=net_in.n_networks, tau_ca_ms=cfg["tau_ca_ms"], ca_jump=cfg["ca_jump"],
+                           obs_gain=cfg["obs_gain"], obs_offset=cfg["obs_offset"], obs_sigma=cfg["obs_sigma"],
+                           obs_stride=obs, raster_capacity_steps=S, trace_capacity_frames=max(frames_per_step, 1) if obs else 0,
+                           seed=cfg["seed"])
+        return gn.gn_create(c, cfg["classes"], a["pos"], a["row"], a["tgt"], a["w"], None, a["cls"], None, a["net"],
+                            device=dev)
+
+    def counters(g):
+        c = gn.gn_read_state(g, gn.GN_COUNTERS)
+        return int(c[0]), int(c[1]), int(c[2])
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident arm ------------------------------------------------------------------------
+    g = create()
+    for _ in range(W):
+        gn.gn_step(g, S)
+    barrier()
+    c0 = counters(g)
+    _, l0 = gn.gn_profile_read(g)
+    sampler = ClockSampler(local)
+    sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    for _ in range(K):
+        gn.gn_step(g, S)
+    ev1.record()
+    barrier()
+    clocks = sampler.stop()
+    ms = ev0.elapsed_time(ev1)
+    c1 = counters(g)
+    _, l1 = gn.gn_profile_read(g)
+    launches = int(l1[3] - l0[3])
+    if dist is not None:
+        tms = torch.tensor([ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
+        ms = float(tms.item())
+        tot = torch.tensor([c1[1] - c0[1], c1[2] - c0[2]], device=dev, dtype=torch.float64)
+        dist.all_reduce(tot)
+        spikes, events = float(tot[0]), float(tot[1])
+    else:
+        spikes, events = c1[1] - c0[1], c1[2] - c0[2]
+    sec = ms * 1e-3
+    sim_steps = K * S
+    value = world * N * sim_steps / sec
+
+    # ---- per-kernel pass: the same K steps again, every launch bracketed by CUDA events ------------
+    gn.gn_profile(g, True)
+    cp0 = counters(g)
+    gn.gn_step(g, sim_steps)
+    kms, kn = gn.gn_profile_read(g)
+    gn.gn_profile(g, False)
+    cp1 = counters(g)
+    peak, peak_src = peaks()
+    names = ["gn_update_kernel (a1-a3)", "gn_deliver_kernel (a4)", "gn_observe_kernel (a5)"]
+    p_events, p_spikes = cp1[2] - cp0[2], cp1[1] - cp0[1]
+    kbytes = [N * (UPDATE_BYTES_PER_VERTEX + (UPDATE_BYTES_PER_VERTEX_OBS if obs else 0.0)),
+              (p_events * EVENT_BYTES + p_spikes * SOURCE_BYTES) / max(int(kn[1]), 1),
+              N * 8.0]
+    kernels = []
+    for k in range(3):
+        if kn[k] == 0:
+            continue
+        avg_s = kms[k] * 1e-3 / kn[k]
+        kernels.append({"kernel": names[k], "launches": int(kn[k]), "avg_us": avg_s * 1e6, "share": float(kms[k] / kms.sum()),
+                        "bytes_per_launch": kbytes[k], "achieved": kbytes[k] / avg_s / 1e9, "frac": kbytes[k] / avg_s / 1e9 / peak})
+    dom = max(kernels, key=lambda r: r["share"])
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")   # per-launch DRAM bytes from the committed ncu --set full capture
+    if os.path.exists(tpath):
+        try:
+            traffic = json.load(open(tpath)).get(dom["kernel"].split()[0])
+        except Exception:
+            traffic = None
+    roofline = {"bound": "hbm", "kernel": dom["kernel"], "achieved": dom["achieved"], "peak": peak, "unit": "GB/s",
+                "frac": dom["frac"], "traffic": traffic, "peak_source": peak_src,
+                "timing": "second pass of the same K steps with a CUDA event at every kernel boundary (gn_profile)",
+                "kernels": kernels}
+    if dom["kernel"].startswith("gn_deliver"):
+        sect = (p_events * SECTOR_EVENT_BYTES + p_spikes * SOURCE_BYTES) / max(int(kn[1]), 1)
+        roofline["sector_granular"] = {"bytes_per_launch": sect, "achieved": sect / (dom["avg_us"] * 1e-6) / 1e9,
+                                       "frac": sect / (dom["avg_us"] * 1e-6) / 1e9 / peak}
+    del g
+
+    # ---- end to end through the C ABI with HOST buffers ----------------------------------------------
+    e2e = None
+    if not args.no_e2e:
+        pin = lambda a: None if a is None else torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+        host = dict(pos=pin(net_in.positions), row=pin(net_in.row_offsets.view(np.int64)), tgt=pin(net_in.targets.view(np.int32)),
+                    w=pin(net_in.weights), cls=pin(net_in.vertex_class),
+                    net=None if net_in.net_offsets is None else pin(net_in.net_offsets.view(np.int32)))
+        words = (N + 31) // 32
+        rast_host = torch.empty((S, words), dtype=torch.int32).pin_memory()
+        v_host = torch.empty(N, dtype=torch.float32).pin_memory()
+        z_host = torch.empty((max(frames_per_step, 1), N), dtype=torch.float32).pin_memory() if obs else None
+        h2d = sum(t.numel() * t.element_size() for t in host.values() if t is not None)
+        d2h = rast_host.numel() * 4 + (z_host.numel() * 4 if obs else 0) + v_host.numel() * 4 / K
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        g2 = create(host)                                    # host -> device of every input, validation, quantisation, delays
+        for k in range(K):
+            gn.gn_step(g2, S)
+            gn.gn_read_raster(g2, k * S, S, rast_host.numpy().view(np.uint32))   # device -> host of the step's result
+            if obs:
+                gn.gn_observe(g2, k * frames_per_step, frames_per_step, z_host.numpy())
+        gn.gn_read_state(g2, gn.GN_V, v_host.numpy())
+        e1.record()
+        barrier()
+        ems = e0.elapsed_time(e1)
+        if dist is not None:
+            tms = torch.tensor([ems], device=dev, dtype=torch.float64)
+            dist.all_reduce(tms, op=dist.ReduceOp.MAX)
+            ems = float(tms.item())
+        e2e = {"value": world * N * sim_steps / (ems * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d / K,
+               "d2h_bytes_per_step": d2h, "ms_total": ems,
+               "what": "gn_create from pinned host arrays (upload + validation + quantisation + eq. 25 delays) + K x "
+                       "[gn_step(S) + gn_read_raster of the S steps to pinned host memory] + final V to host"}
+        del g2
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic",
+        "config": {"workload": workload_name(net_in, cfg, args), "sim_steps_per_step": S,
+                   "l2": "no flush: working set (ring + edges + state) >> 126 MB L2",
+                   "parallelism": "single GPU" if world == 1 else f"{world} independent replicas (no collective)"},
+        "events_per_s": events / sec, "real_time_factor": sim_steps * cfg["dt_ms"] * 1e-3 / sec,
+        "us_per_sim_step": ms * 1e3 / sim_steps,
+        "mean_rate_hz": spikes / (world * N * sim_steps * cfg["dt_ms"] * 1e-3),
+        "events_per_sim_step": events / world / sim_steps,
+        "roofline": roofline, "clocks": clocks, "gpu_launches": launches, "e2e": e2e,
+    }
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline(net_in, cfg)
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -37,7 +37,8 @@ class gn_config(C.Structure):
 
 
 EXPORTS = ("gn_query_workspace", "gn_create", "gn_step", "gn_read_state", "gn_write_state",
-           "gn_read_raster", "gn_observe", "gn_debug_words", "gn_last_error", "gn_destroy")
+           "gn_read_raster", "gn_observe", "gn_debug_words", "gn_profile", "gn_profile_read", "gn_last_error",
+           "gn_destroy")
 
 _lib = None
 
@@ -56,6 +57,8 @@ def lib() -> C.CDLL:
         L.gn_read_raster.argtypes = [vp, u64, u64, vp, sz, i32]
         L.gn_observe.argtypes = [vp, u64, u64, vp, sz, i32]
         L.gn_debug_words.argtypes = [vp, u64, u32, u64, u32, u32, vp]
+        L.gn_profile.argtypes = [vp, i32]
+        L.gn_profile_read.argtypes = [vp, vp, vp]
         L.gn_last_error.argtypes = [vp]
         L.gn_last_error.restype = C.c_char_p
         L.gn_destroy.argtypes = [vp]
@@ -198,6 +201,18 @@ def gn_debug_words(seed: int, stream_id: int, idx: int, first_vertex: int, n: in
     _check(lib().gn_debug_words(C.c_void_p(st.cuda_stream), seed, stream_id, idx, first_vertex, n,
                                 C.c_void_p(out.data_ptr())))
     return out.cpu().numpy().view(np.uint32)
+
+
+def gn_profile(net: GnNet, enable: bool) -> None:
+    _check(lib().gn_profile(net.handle, int(bool(enable))), net.handle)
+
+
+def gn_profile_read(net: GnNet):
+    """-> (ms[3] summed device time of update / delivery / observation, launches[4])."""
+    ms = np.zeros(3, dtype=np.float64)
+    n = np.zeros(4, dtype=np.uint64)
+    _check(lib().gn_profile_read(net.handle, _ptr(ms), _ptr(n)), net.handle)
+    return ms, n
 
 
 def gn_destroy(net: GnNet) -> None:

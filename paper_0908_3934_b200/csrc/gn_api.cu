@@ -7,6 +7,7 @@
 #include <string.h>
 
 #include <new>
+#include <vector>
 
 #include "gn_internal.h"
 
@@ -70,6 +71,14 @@ struct gn_net {
     uint8_t *ws;
     uint64_t t;          // steps enqueued so far
     bool has_bias;
+    // measuring mode (gn_profile)
+    bool profile;
+    std::vector<cudaEvent_t> ev;      // pool, reused chunk after chunk
+    std::vector<uint8_t> ev_kind;     // kernel that runs between event i and event i+1 (0xFF = none)
+    size_t ev_used;
+    double prof_ms[3];
+    uint64_t prof_n[3];
+    uint64_t launches;                // every kernel launched by gn_step since gn_create
     char err[256];
 };
 
@@ -146,6 +155,10 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
     net->ws = (uint8_t *)workspace;
     net->t = 0;
     net->has_bias = bias != nullptr;
+    net->profile = false;
+    net->ev_used = 0;
+    net->launches = 0;
+    for (int k = 0; k < 3; ++k) { net->prof_ms[k] = 0.0; net->prof_n[k] = 0; }
     net->err[0] = 0;
 
     const uint32_t N = cfg->n_vertices, Npad = (N + 127) / 128 * 128;
@@ -279,18 +292,85 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
     return GN_OK;
 }
 
+// ---- measuring mode: one event at every kernel boundary, collected every kProfChunk steps ----------
+static const size_t kProfChunk = 256;
+
+static int prof_mark(gn_net *net, uint8_t kind_after)
+{
+    if (net->ev_used == net->ev.size()) {
+        cudaEvent_t e;
+        GN_CUDA(net, cudaEventCreate(&e));
+        net->ev.push_back(e);
+        net->ev_kind.push_back(0xFF);
+    }
+    GN_CUDA(net, cudaEventRecord(net->ev[net->ev_used], net->stream));
+    net->ev_kind[net->ev_used] = kind_after;
+    net->ev_used++;
+    return GN_OK;
+}
+
+static int prof_collect(gn_net *net)
+{
+    if (net->ev_used == 0) return GN_OK;
+    GN_CUDA(net, cudaStreamSynchronize(net->stream));
+    for (size_t i = 0; i + 1 < net->ev_used; ++i) {
+        const uint8_t k = net->ev_kind[i];
+        if (k > 2) continue;
+        float ms = 0.f;
+        GN_CUDA(net, cudaEventElapsedTime(&ms, net->ev[i], net->ev[i + 1]));
+        net->prof_ms[k] += (double)ms;
+        net->prof_n[k] += 1;
+    }
+    net->ev_used = 0;
+    return GN_OK;
+}
+
 int gn_step(gn_net *net, uint64_t n_steps)
 {
     if (!net) return GN_E_INVALID_ARG;
     const GnDev &d = net->dev;
     for (uint64_t s = 0; s < n_steps; ++s) {
         const uint64_t t = net->t;
+        const bool prof = net->profile;
+        int rc;
+        if (prof && (rc = prof_mark(net, 0))) return rc;
         GN_CUDA(net, gnk_update(d, t, net->has_bias, net->stream));
-        if (net->cfg.n_edges) GN_CUDA(net, gnk_deliver(d, t, net->stream));
-        if (d.obs_stride && (t + 1) % d.obs_stride == 0)
+        net->launches++;
+        if (net->cfg.n_edges) {
+            if (prof && (rc = prof_mark(net, 1))) return rc;
+            GN_CUDA(net, gnk_deliver(d, t, net->stream));
+            net->launches++;
+        }
+        if (d.obs_stride && (t + 1) % d.obs_stride == 0) {
+            if (prof && (rc = prof_mark(net, 2))) return rc;
             GN_CUDA(net, gnk_observe(d, (t + 1) / d.obs_stride - 1, net->stream));
+            net->launches++;
+        }
+        if (prof && (rc = prof_mark(net, 0xFF))) return rc;
         net->t = t + 1;
+        if (prof && (s + 1) % kProfChunk == 0 && (rc = prof_collect(net))) return rc;
     }
+    if (net->profile) return prof_collect(net);
+    return GN_OK;
+}
+
+int gn_profile(gn_net *net, int enable)
+{
+    if (!net) return GN_E_INVALID_ARG;
+    net->profile = enable != 0;
+    if (enable) {
+        for (int k = 0; k < 3; ++k) { net->prof_ms[k] = 0.0; net->prof_n[k] = 0; }
+        net->ev_used = 0;
+    }
+    return GN_OK;
+}
+
+int gn_profile_read(gn_net *net, double ms[3], uint64_t launches[4])
+{
+    if (!net) return GN_E_INVALID_ARG;
+    if (!ms || !launches) return set_err(net, GN_E_INVALID_ARG, "NULL output");
+    for (int k = 0; k < 3; ++k) { ms[k] = net->prof_ms[k]; launches[k] = net->prof_n[k]; }
+    launches[3] = net->launches;
     return GN_OK;
 }
 
@@ -425,6 +505,7 @@ int gn_destroy(gn_net *net)
 {
     if (!net) return GN_E_INVALID_ARG;
     cudaError_t e = cudaStreamSynchronize(net->stream);
+    for (cudaEvent_t ev : net->ev) cudaEventDestroy(ev);
     delete net;
     return e == cudaSuccess ? GN_OK : GN_E_CUDA;
 }
