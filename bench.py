@@ -184,6 +184,8 @@ def main():
     ap.add_argument("--config", type=int, default=4)
     ap.add_argument("--n", type=int, default=None, help="override the vertex count (debugging only)")
     ap.add_argument("--sim-steps", type=int, default=100, help="simulated steps per bench step")
+    ap.add_argument("--delivery", default="auto", choices=["auto", "ring", "queue"], help="gn_config.delivery_mode")
+    ap.add_argument("--queue-group", type=int, default=0, help="gn_config.queue_group (0 = library default)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -222,7 +224,8 @@ def main():
                            n_networks=net_in.n_networks, tau_ca_ms=cfg["tau_ca_ms"], ca_jump=cfg["ca_jump"],
                            obs_gain=cfg["obs_gain"], obs_offset=cfg["obs_offset"], obs_sigma=cfg["obs_sigma"],
                            obs_stride=obs, raster_capacity_steps=S, trace_capacity_frames=max(frames_per_step, 1) if obs else 0,
-                           seed=cfg["seed"])
+                           seed=cfg["seed"], delivery_mode={"auto": 0, "ring": 1, "queue": 2}[args.delivery],
+                           queue_group=args.queue_group)
         return gn.gn_create(c, cfg["classes"], a["pos"], a["row"], a["tgt"], a["w"], None, a["cls"], None, a["net"],
                             device=dev)
 
@@ -255,7 +258,7 @@ def main():
     ms = ev0.elapsed_time(ev1)
     c1 = counters(g)
     _, l1 = gn.gn_profile_read(g)
-    launches = int(l1[3] - l0[3])
+    launches = int(l1[4] - l0[4])
     if dist is not None:
         tms = torch.tensor([ms], device=dev, dtype=torch.float64)
         dist.all_reduce(tms, op=dist.ReduceOp.MAX)
@@ -277,18 +280,28 @@ def main():
     gn.gn_profile(g, False)
     cp1 = counters(g)
     peak, peak_src = peaks()
-    names = ["gn_update_kernel (a1-a3)", "gn_deliver_kernel (a4)", "gn_observe_kernel (a5)"]
+    queue_mode = kn[3] > 0
+    names = ["gn_update_kernel (a1-a3)", "gn_route_kernel (a4, queue mode)" if queue_mode else "gn_deliver_kernel (a4)",
+             "gn_observe_kernel (a5)", "gn_fold_kernel (a4, queue mode)"]
     p_events, p_spikes = cp1[2] - cp0[2], cp1[1] - cp0[1]
+    # algorithmic bytes per launch: ring mode, one kernel does the whole 17 B event;
+    # queue mode splits it: routing reads the 9 B edge record (+12 B per fired source), folding does the 8 B ring RMW
     kbytes = [N * (UPDATE_BYTES_PER_VERTEX + (UPDATE_BYTES_PER_VERTEX_OBS if obs else 0.0)),
-              (p_events * EVENT_BYTES + p_spikes * SOURCE_BYTES) / max(int(kn[1]), 1),
-              N * 8.0]
+              (p_events * (9.0 if queue_mode else EVENT_BYTES) + p_spikes * SOURCE_BYTES) / max(int(kn[1]), 1),
+              N * 8.0,
+              p_events * 8.0 / max(int(kn[3]), 1)]
     kernels = []
-    for k in range(3):
+    for k in range(4):
         if kn[k] == 0:
             continue
         avg_s = kms[k] * 1e-3 / kn[k]
         kernels.append({"kernel": names[k], "launches": int(kn[k]), "avg_us": avg_s * 1e6, "share": float(kms[k] / kms.sum()),
                         "bytes_per_launch": kbytes[k], "achieved": kbytes[k] / avg_s / 1e9, "frac": kbytes[k] / avg_s / 1e9 / peak})
+    a4_s = (kms[1] + kms[3]) * 1e-3
+    a4 = {"what": "a4 delivery as a whole (routing + folding), 17 B per event + 12 B per fired source",
+          "bytes": p_events * EVENT_BYTES + p_spikes * SOURCE_BYTES, "ms": a4_s * 1e3,
+          "achieved": (p_events * EVENT_BYTES + p_spikes * SOURCE_BYTES) / max(a4_s, 1e-12) / 1e9}
+    a4["frac"] = a4["achieved"] / peak
     dom = max(kernels, key=lambda r: r["share"])
     traffic = None
     tpath = os.path.join(ROOT, "profiles", "traffic.json")   # per-launch DRAM bytes from the committed ncu --set full capture
@@ -300,8 +313,8 @@ def main():
     roofline = {"bound": "hbm", "kernel": dom["kernel"], "achieved": dom["achieved"], "peak": peak, "unit": "GB/s",
                 "frac": dom["frac"], "traffic": traffic, "peak_source": peak_src,
                 "timing": "second pass of the same K steps with a CUDA event at every kernel boundary (gn_profile)",
-                "kernels": kernels}
-    if dom["kernel"].startswith("gn_deliver"):
+                "kernels": kernels, "a4_delivery": a4, "profile_pass_events_per_sim_step": p_events / sim_steps}
+    if dom["kernel"].startswith("gn_deliver"):   # ring mode only: what DRAM moves when every event misses L2
         sect = (p_events * SECTOR_EVENT_BYTES + p_spikes * SOURCE_BYTES) / max(int(kn[1]), 1)
         roofline["sector_granular"] = {"bytes_per_launch": sect, "achieved": sect / (dom["avg_us"] * 1e-6) / 1e9,
                                        "frac": sect / (dom["avg_us"] * 1e-6) / 1e9 / peak}

@@ -80,7 +80,23 @@ typedef struct {
     uint32_t raster_capacity_steps; /* device raster window (most recent steps kept); 0 = none kept  */
     uint32_t trace_capacity_frames; /* device trace window (most recent frames kept)                 */
     uint64_t seed;                  /* key of the counter generator (drive stream 5, noise stream 6) */
+    /* How eq. 30's sum reaches the ring (the RESULT is identical in every mode: integer adds commute). */
+    uint32_t delivery_mode;         /* GN_DELIVER_AUTO (0), GN_DELIVER_RING, GN_DELIVER_QUEUE          */
+    uint32_t queue_group;           /* queue mode: ring slots per event bucket, power of two in 1..16; */
+                                    /* 0 = default (8)                                                */
+    uint64_t queue_capacity;        /* queue mode: events one bucket holds before later ones fall     */
+                                    /* back to direct ring adds; 0 = default queue_group * ceil(E/16) */
 } gn_config;
+
+/* delivery_mode.  RING: every event is one int32 reduction straight into ring[(t+delay) mod D][target]
+ * (best while the ring fits L2).  QUEUE: events are appended, as (ring cell, weight) records, to the
+ * bucket of the slot group they are due in; a bucket is folded into its ring rows just before the
+ * first of them is consumed, when those rows are L2-resident (best when the ring is >> L2: sequential
+ * 8-byte appends instead of a 32-byte DRAM sector read-modify-write per event).  AUTO picks QUEUE when
+ * the ring exceeds 48 MB and D >= 32, else RING. */
+#define GN_DELIVER_AUTO 0
+#define GN_DELIVER_RING 1
+#define GN_DELIVER_QUEUE 2
 
 /* `which` of gn_read_state / gn_write_state, with the element type of the caller's buffer.       */
 enum {
@@ -129,8 +145,8 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
               void *cuda_stream, gn_net **out);
 
 /* Advance n_steps time steps: per step, ring-slot read-and-clear + drive + vertex update + spike
- * detection/compaction (one kernel), event delivery into the delay ring (one kernel), and at
- * frame boundaries the observation kernel.  Asynchronous: no host synchronisation inside. */
+ * detection/compaction (one kernel), event delivery (one kernel; in queue mode a routing kernel per step plus
+ * a bucket fold every queue_group steps), and at frame boundaries the observation kernel.  Asynchronous: no host synchronisation inside. */
 int gn_step(gn_net *net, uint64_t n_steps);
 
 /* Copy state out.  dst_bytes must be at least the size listed at the enum.  dst_is_device != 0:
@@ -164,10 +180,11 @@ int gn_debug_words(void *cuda_stream, uint64_t seed, uint32_t stream_id, uint64_
  * CUDA events on the net's stream (and synchronises every few hundred steps to collect them), so the
  * step is slower than normal: a measuring mode, never the mode a throughput number is taken in.
  * gn_profile_read: ms[k] = summed device time, launches[k] = launch count of kernel k since the last
- * gn_profile(net, 1): k = 0 update (a1-a3), 1 delivery (a4), 2 observation (a5).  launches[3] is the
- * total number of kernels this handle has launched since gn_create, profiling or not. */
+ * gn_profile(net, 1): k = 0 update (a1-a3), 1 delivery (a4: ring reductions or queue routing),
+ * 2 observation (a5), 3 bucket fold (a4, queue mode).  launches[4] is the total number of kernels this
+ * handle has launched since gn_create, profiling or not. */
 int gn_profile(gn_net *net, int enable);
-int gn_profile_read(gn_net *net, double ms[3], uint64_t launches[4]);
+int gn_profile_read(gn_net *net, double ms[4], uint64_t launches[5]);
 
 const char *gn_last_error(const gn_net *net);
 int gn_destroy(gn_net *net);

@@ -17,6 +17,7 @@ GN_E_INVALID_ARG, GN_E_BAD_GRAPH, GN_E_OVERFLOW_RISK = -1, -2, -3
 GN_E_WORKSPACE_TOO_SMALL, GN_E_RANGE_EVICTED, GN_E_CUDA = -4, -5, -6
 GN_V, GN_W, GN_R, GN_CA, GN_REFR, GN_RING, GN_STEP, GN_COUNTERS, GN_DELAYS, GN_WEIGHTS_FX, GN_BIAS = range(11)
 GN_MAX_CLASSES = 8
+GN_DELIVER_AUTO, GN_DELIVER_RING, GN_DELIVER_QUEUE = 0, 1, 2
 
 CLASS_FIELDS = ("a", "b", "c_reset", "d", "k2", "k1", "k0", "v_peak", "tau_syn_ms",
                 "refractory_ms", "drive_rate_hz", "drive_kick")
@@ -33,7 +34,8 @@ class gn_config(C.Structure):
                 ("ca_jump", C.c_float), ("obs_gain", C.c_float), ("obs_offset", C.c_float),
                 ("obs_sigma", C.c_float), ("obs_stride", C.c_uint32),
                 ("raster_capacity_steps", C.c_uint32), ("trace_capacity_frames", C.c_uint32),
-                ("seed", C.c_uint64)]
+                ("seed", C.c_uint64), ("delivery_mode", C.c_uint32), ("queue_group", C.c_uint32),
+                ("queue_capacity", C.c_uint64)]
 
 
 EXPORTS = ("gn_query_workspace", "gn_create", "gn_step", "gn_read_state", "gn_write_state",
@@ -93,9 +95,11 @@ def _ptr(a):
 
 def make_config(n_vertices, dim, n_edges, ring_slots, dt_ms, speed, n_classes, *, n_networks=1, tau_ca_ms=500.0,
                 ca_jump=1.0, obs_gain=1.0, obs_offset=0.0, obs_sigma=0.0, obs_stride=0, raster_capacity_steps=0,
-                trace_capacity_frames=0, seed=0) -> gn_config:
+                trace_capacity_frames=0, seed=0, delivery_mode=GN_DELIVER_AUTO, queue_group=0,
+                queue_capacity=0) -> gn_config:
     return gn_config(n_vertices, dim, n_edges, n_networks, ring_slots, dt_ms, speed, n_classes, tau_ca_ms, ca_jump,
-                     obs_gain, obs_offset, obs_sigma, obs_stride, raster_capacity_steps, trace_capacity_frames, seed)
+                     obs_gain, obs_offset, obs_sigma, obs_stride, raster_capacity_steps, trace_capacity_frames, seed,
+                     delivery_mode, queue_group, queue_capacity)
 
 
 def gn_query_workspace(cfg: gn_config) -> int:
@@ -208,9 +212,9 @@ def gn_profile(net: GnNet, enable: bool) -> None:
 
 
 def gn_profile_read(net: GnNet):
-    """-> (ms[3] summed device time of update / delivery / observation, launches[4])."""
-    ms = np.zeros(3, dtype=np.float64)
-    n = np.zeros(4, dtype=np.uint64)
+    """-> (ms[4] summed device time of update / delivery / observation / bucket fold, launches[5])."""
+    ms = np.zeros(4, dtype=np.float64)
+    n = np.zeros(5, dtype=np.uint64)
     _check(lib().gn_profile_read(net.handle, _ptr(ms), _ptr(n)), net.handle)
     return ms, n
 
@@ -220,7 +224,8 @@ def gn_destroy(net: GnNet) -> None:
 
 
 def create_from_inputs(net_in, cfg_in, *, delays=None, bias=None, raster_capacity_steps=0,
-                       trace_capacity_frames=0, device="cuda:0") -> GnNet:
+                       trace_capacity_frames=0, device="cuda:0", delivery_mode=GN_DELIVER_AUTO, queue_group=0,
+                       queue_capacity=0) -> GnNet:
     """Convenience: build from a gn_inputs.Network + config dict (marshalling only)."""
     obs = int(cfg_in.get("obs_stride", 0))
     cfg = make_config(net_in.n_vertices, net_in.dim, net_in.n_edges, cfg_in["ring_slots"], cfg_in["dt_ms"],
@@ -228,7 +233,8 @@ def create_from_inputs(net_in, cfg_in, *, delays=None, bias=None, raster_capacit
                       tau_ca_ms=cfg_in["tau_ca_ms"], ca_jump=cfg_in["ca_jump"], obs_gain=cfg_in["obs_gain"],
                       obs_offset=cfg_in["obs_offset"], obs_sigma=cfg_in["obs_sigma"], obs_stride=obs,
                       raster_capacity_steps=raster_capacity_steps,
-                      trace_capacity_frames=trace_capacity_frames if obs else 0, seed=cfg_in["seed"])
+                      trace_capacity_frames=trace_capacity_frames if obs else 0, seed=cfg_in["seed"],
+                      delivery_mode=delivery_mode, queue_group=queue_group, queue_capacity=queue_capacity)
     return gn_create(cfg, cfg_in["classes"], net_in.positions, net_in.row_offsets, net_in.targets, net_in.weights,
                      None if delays is None else np.ascontiguousarray(delays, dtype=np.uint8),
                      net_in.vertex_class,

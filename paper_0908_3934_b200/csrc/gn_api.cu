@@ -16,7 +16,8 @@ namespace {
 thread_local char g_create_error[256] = "";
 
 struct Layout {
-    size_t V, W, r, c, acc, bias, refr, cls, ring, row, tgt, wfx, dly, active, n_active, counters;
+    size_t V, W, r, c, acc, bias, refr, cls, ring, row, tgt, wfx, dly, active, n_active, counters, q_count;
+    size_t s_tgt, s_wfx, s_dly, queue;
     size_t raster, trace, scratch_row64, scratch_abs, scratch_pos, scratch_net, scratch_chk, total;
 };
 
@@ -35,7 +36,35 @@ int check_config(const gn_config *cfg, char *err, size_t errn)
     if (cfg->n_networks < 1 || cfg->n_networks > cfg->n_vertices) return fail("n_networks must be in [1, n_vertices]");
     if (cfg->obs_stride > 0 && cfg->trace_capacity_frames == 0) return fail("obs_stride > 0 needs trace_capacity_frames > 0");
     if (cfg->obs_stride > 0 && !(cfg->tau_ca_ms > 0.0f)) return fail("obs_stride > 0 needs tau_ca_ms > 0");
+    if (cfg->delivery_mode > GN_DELIVER_QUEUE) return fail("delivery_mode must be GN_DELIVER_AUTO, _RING or _QUEUE");
+    const uint32_t qg = cfg->queue_group;
+    if (qg != 0 && (qg > 16 || (qg & (qg - 1)) != 0)) return fail("queue_group must be 0 or a power of two in 1..16");
     return GN_OK;
+}
+
+// Resolved delivery plan: mode, log2(slots per bucket), buckets, records per bucket.
+struct QueuePlan {
+    bool on;
+    uint32_t q_log, q_nb;
+    uint64_t q_cap;
+};
+
+QueuePlan make_plan(const gn_config *cfg)
+{
+    const uint64_t N = cfg->n_vertices, Npad = (N + 127) / 128 * 128, E = cfg->n_edges, D = cfg->ring_slots;
+    QueuePlan q{};
+    uint32_t group = cfg->queue_group ? cfg->queue_group : 8u;
+    while (group > 1 && (Npad * group > 0xFFFFFFFFull || group > D)) group >>= 1;   // cell offsets are 32-bit
+    q.on = cfg->delivery_mode == GN_DELIVER_QUEUE ||
+           (cfg->delivery_mode == GN_DELIVER_AUTO && D >= 32 && D * Npad * 4 > (48ull << 20));
+    if (E == 0) q.on = false;
+    q.q_log = 0;
+    while ((1u << q.q_log) < group) q.q_log++;
+    q.q_nb = (uint32_t)((D + group - 1) / group);
+    uint64_t cap = cfg->queue_capacity ? cfg->queue_capacity : (uint64_t)group * ((E + 15) / 16);
+    if (cap < 64) cap = 64;
+    q.q_cap = (cap + 31) / 32 * 32;
+    return q;
 }
 
 Layout make_layout(const gn_config *cfg)
@@ -52,8 +81,12 @@ Layout make_layout(const gn_config *cfg)
     L.ring = take(D * Npad * 4);
     L.row = take((Npad + 1) * 4); L.tgt = take(E * 4); L.wfx = take(E * 4); L.dly = take(E);
     L.active = take(2 * Npad * 4); L.n_active = take(8); L.counters = take(32);
+    const QueuePlan qp = make_plan(cfg);
+    L.q_count = take(256 * 8);
     L.raster = take((size_t)cfg->raster_capacity_steps * (Npad / 32) * 4);
     L.trace = take(obs ? (size_t)cfg->trace_capacity_frames * Npad * 4 : 0);
+    L.s_tgt = take(qp.on ? E * 4 : 0); L.s_wfx = take(qp.on ? E * 4 : 0); L.s_dly = take(qp.on ? E : 0);
+    L.queue = take(qp.on ? (size_t)qp.q_nb * qp.q_cap * 8 : 0);
     L.scratch_row64 = take((N + 1) * 8); L.scratch_abs = take(N * 8);
     L.scratch_pos = take(N * cfg->dim * 4); L.scratch_net = take(((size_t)cfg->n_networks + 1) * 4);
     L.scratch_chk = take(sizeof(GnCheck));
@@ -76,8 +109,8 @@ struct gn_net {
     std::vector<cudaEvent_t> ev;      // pool, reused chunk after chunk
     std::vector<uint8_t> ev_kind;     // kernel that runs between event i and event i+1 (0xFF = none)
     size_t ev_used;
-    double prof_ms[3];
-    uint64_t prof_n[3];
+    double prof_ms[4];
+    uint64_t prof_n[4];
     uint64_t launches;                // every kernel launched by gn_step since gn_create
     char err[256];
 };
@@ -158,7 +191,7 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
     net->profile = false;
     net->ev_used = 0;
     net->launches = 0;
-    for (int k = 0; k < 3; ++k) { net->prof_ms[k] = 0.0; net->prof_n[k] = 0; }
+    for (int k = 0; k < 4; ++k) { net->prof_ms[k] = 0.0; net->prof_n[k] = 0; }
     net->err[0] = 0;
 
     const uint32_t N = cfg->n_vertices, Npad = (N + 127) / 128 * 128;
@@ -187,6 +220,14 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
     d.active = (uint32_t *)(ws + L.active); d.n_active = (uint32_t *)(ws + L.n_active);
     d.counters = (unsigned long long *)(ws + L.counters);
     d.raster = (uint32_t *)(ws + L.raster);
+    const QueuePlan qp = make_plan(cfg);
+    d.queue_mode = qp.on ? 1u : 0u;
+    d.q_log = qp.q_log; d.q_nb = qp.q_nb; d.q_cap = qp.q_cap;
+    d.q_count = (unsigned long long *)(ws + L.q_count);
+    if (qp.on) {
+        d.s_tgt = (uint32_t *)(ws + L.s_tgt); d.s_wfx = (int32_t *)(ws + L.s_wfx); d.s_dly = ws + L.s_dly;
+        d.queue = (uint2 *)(ws + L.queue);
+    }
     d.trace = cfg->obs_stride ? (float *)(ws + L.trace) : nullptr;
     for (uint32_t k = 0; k < cfg->n_classes; ++k) {
         const gn_class_params &c = classes[k];
@@ -230,7 +271,7 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
 
     // zero everything the step loop accumulates into or reads before writing
     GN_CREATE_CUDA(cudaMemsetAsync(ws, 0, L.tgt, st));                       // state, bias, refr, cls, ring, row
-    GN_CREATE_CUDA(cudaMemsetAsync(ws + L.active, 0, L.scratch_row64 - L.active, st));   // lists, counters, raster, trace
+    GN_CREATE_CUDA(cudaMemsetAsync(ws + L.active, 0, L.s_tgt - L.active, st));   // lists, counters, bucket counts, raster, trace
     GN_CREATE_CUDA(cudaMemsetAsync(abs_in, 0, (size_t)N * 8, st));
     GN_CREATE_CUDA(cudaMemsetAsync(chk_d, 0, sizeof(GnCheck), st));
     // uploads (host or device sources)
@@ -273,6 +314,7 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
         GN_CREATE_CUDA(gnk_validate(d, net_offsets ? net_d : nullptr, cfg->n_networks, abs_in, chk_d, st));
     }
     GN_CREATE_CUDA(gnk_check_overflow(d, abs_in, chk_d, st));
+    if (d.queue_mode) GN_CREATE_CUDA(gnk_sort_rows(d, st));
     GN_CREATE_CUDA(cudaMemcpyAsync(&chk, chk_d, sizeof chk, cudaMemcpyDeviceToHost, st));
     GN_CREATE_CUDA(cudaStreamSynchronize(st));
 #undef GN_CREATE_CUDA
@@ -315,7 +357,7 @@ static int prof_collect(gn_net *net)
     GN_CUDA(net, cudaStreamSynchronize(net->stream));
     for (size_t i = 0; i + 1 < net->ev_used; ++i) {
         const uint8_t k = net->ev_kind[i];
-        if (k > 2) continue;
+        if (k > 3) continue;
         float ms = 0.f;
         GN_CUDA(net, cudaEventElapsedTime(&ms, net->ev[i], net->ev[i + 1]));
         net->prof_ms[k] += (double)ms;
@@ -333,12 +375,23 @@ int gn_step(gn_net *net, uint64_t n_steps)
         const uint64_t t = net->t;
         const bool prof = net->profile;
         int rc;
+        uint32_t reset_bucket = 0xFFFFFFFFu;
+        if (d.queue_mode) {                       // fold the bucket whose first ring row is consumed now
+            const uint32_t slot = (uint32_t)(t % d.D);
+            if ((slot & ((1u << d.q_log) - 1u)) == 0u) {
+                reset_bucket = slot >> d.q_log;
+                if (prof && (rc = prof_mark(net, 3))) return rc;
+                GN_CUDA(net, gnk_fold(d, reset_bucket, net->stream));
+                net->launches++;
+            }
+        }
         if (prof && (rc = prof_mark(net, 0))) return rc;
-        GN_CUDA(net, gnk_update(d, t, net->has_bias, net->stream));
+        GN_CUDA(net, gnk_update(d, t, net->has_bias, reset_bucket, net->stream));
         net->launches++;
         if (net->cfg.n_edges) {
             if (prof && (rc = prof_mark(net, 1))) return rc;
-            GN_CUDA(net, gnk_deliver(d, t, net->stream));
+            if (d.queue_mode) GN_CUDA(net, gnk_route(d, t, net->stream));
+            else GN_CUDA(net, gnk_deliver(d, t, net->stream));
             net->launches++;
         }
         if (d.obs_stride && (t + 1) % d.obs_stride == 0) {
@@ -359,18 +412,18 @@ int gn_profile(gn_net *net, int enable)
     if (!net) return GN_E_INVALID_ARG;
     net->profile = enable != 0;
     if (enable) {
-        for (int k = 0; k < 3; ++k) { net->prof_ms[k] = 0.0; net->prof_n[k] = 0; }
+        for (int k = 0; k < 4; ++k) { net->prof_ms[k] = 0.0; net->prof_n[k] = 0; }
         net->ev_used = 0;
     }
     return GN_OK;
 }
 
-int gn_profile_read(gn_net *net, double ms[3], uint64_t launches[4])
+int gn_profile_read(gn_net *net, double ms[4], uint64_t launches[5])
 {
     if (!net) return GN_E_INVALID_ARG;
     if (!ms || !launches) return set_err(net, GN_E_INVALID_ARG, "NULL output");
-    for (int k = 0; k < 3; ++k) { ms[k] = net->prof_ms[k]; launches[k] = net->prof_n[k]; }
-    launches[3] = net->launches;
+    for (int k = 0; k < 4; ++k) { ms[k] = net->prof_ms[k]; launches[k] = net->prof_n[k]; }
+    launches[4] = net->launches;
     return GN_OK;
 }
 
@@ -410,6 +463,10 @@ int gn_read_state(gn_net *net, int which, void *dst, size_t dst_bytes, int dst_i
     if (dst_bytes < need) return set_err(net, GN_E_INVALID_ARG, "dst has %zu bytes, need %zu", dst_bytes, need);
     if (need == 0) return GN_OK;
     if (which == GN_RING) {   // internal rows are Npad wide; the caller's are N wide
+        if (d.queue_mode) {   // pending records are deferred ring adds: apply them all (a no-op for the results)
+            for (uint32_t b = 0; b < d.q_nb; ++b) GN_CUDA(net, gnk_fold(d, b, net->stream));
+            GN_CUDA(net, cudaMemsetAsync(d.q_count, 0, (size_t)d.q_nb * 8, net->stream));
+        }
         GN_CUDA(net, cudaMemcpy2DAsync(dst, N * 4, d.ring, (size_t)d.Npad * 4, N * 4, d.D,
                                        dst_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, net->stream));
         if (!dst_is_device) GN_CUDA(net, cudaStreamSynchronize(net->stream));

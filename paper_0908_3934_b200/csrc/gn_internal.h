@@ -41,6 +41,16 @@ struct GnDev {
     uint32_t *tgt;           // [E]
     int32_t *wfx;            // [E]
     uint8_t *dly;            // [E]
+    // queue mode: rows re-sorted by delay, and one event bucket per group of
+    // 2^q_log ring slots
+    uint32_t queue_mode;     // 0 ring, 1 queue
+    uint32_t q_log, q_nb;    // slots per bucket = 1 << q_log; buckets = ceil(D / 2^q_log)
+    uint32_t *s_tgt;         // [E] the CSR rows again, each sorted by delay
+    int32_t *s_wfx;          // [E]
+    uint8_t *s_dly;          // [E]
+    uint2 *queue;            // [q_nb][q_cap] records {cell offset inside the bucket's ring rows, w_fx}
+    unsigned long long q_cap;
+    unsigned long long *q_count;   // [q_nb] records appended (may exceed q_cap: the excess went direct)
     // per-step active list, double buffered by step parity
     uint32_t *active;        // [2][Npad]
     uint32_t *n_active;      // [2]
@@ -57,8 +67,11 @@ struct GnCheck {
 };
 
 // ---- launchers (gn_kernels.cu).  All asynchronous on `st`; return the launch error. ----
-cudaError_t gnk_update(const GnDev &p, uint64_t t, bool has_bias, cudaStream_t st);
+cudaError_t gnk_update(const GnDev &p, uint64_t t, bool has_bias, uint32_t reset_bucket, cudaStream_t st);
 cudaError_t gnk_deliver(const GnDev &p, uint64_t t, cudaStream_t st);
+cudaError_t gnk_route(const GnDev &p, uint64_t t, cudaStream_t st);
+cudaError_t gnk_fold(const GnDev &p, uint32_t bucket, cudaStream_t st);
+cudaError_t gnk_sort_rows(const GnDev &p, cudaStream_t st);
 cudaError_t gnk_observe(const GnDev &p, uint64_t frame, cudaStream_t st);
 cudaError_t gnk_init_state(const GnDev &p, GnCheck *chk, cudaStream_t st);
 cudaError_t gnk_convert_rows(const GnDev &p, const uint64_t *row64, uint64_t n_edges, GnCheck *chk,

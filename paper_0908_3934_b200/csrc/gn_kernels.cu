@@ -18,6 +18,7 @@ constexpr int kUpdateThreads = 256;          // 8 warps x 128 vertices = 1024 ve
 constexpr int kVertsPerThread = 4;           // one 128-bit load per SoA array
 constexpr int kDeliverThreads = 256;
 constexpr uint32_t kStreamDrive = 5, kStreamNoise = 6;
+constexpr uint32_t kNoBucket = 0xFFFFFFFFu;
 
 // ---- Philox4x32-10 (Salmon et al., SC'11), from its published description -------------------
 __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
@@ -78,7 +79,7 @@ __device__ __forceinline__ bool vertex_step(const GnClassDev &q, const float dt,
 template <bool OBS, bool BIAS>
 __global__ void __launch_bounds__(kUpdateThreads)
 gn_update_kernel(const GnDev p, const uint64_t t, const uint32_t slot, const uint32_t parity,
-                 const uint32_t raster_row)
+                 const uint32_t raster_row, const uint32_t reset_bucket)
 {
     __shared__ GnClassDev s_cls[GN_MAX_CLASSES];
     __shared__ uint32_t s_cnt[kUpdateThreads / 32];
@@ -87,7 +88,10 @@ gn_update_kernel(const GnDev p, const uint64_t t, const uint32_t slot, const uin
 
     if (threadIdx.x < p.n_classes * 13u)
         reinterpret_cast<uint32_t *>(s_cls)[threadIdx.x] = reinterpret_cast<const uint32_t *>(p.cls_tab)[threadIdx.x];
-    if (blockIdx.x == 0 && threadIdx.x == 0) p.n_active[parity ^ 1u] = 0u;   // list of step t+1
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        p.n_active[parity ^ 1u] = 0u;                                        // list of step t+1
+        if (reset_bucket != kNoBucket) p.q_count[reset_bucket] = 0ull;      // folded just before this launch
+    }
     __syncthreads();
 
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
@@ -235,6 +239,192 @@ gn_deliver_kernel(const GnDev p, const uint32_t slot_t, const uint32_t parity)
         events += (unsigned long long)(end - beg);
     }
     if (lane == 0 && events) atomicAdd(&p.counters[2], events);
+}
+
+// ---- a4, queue mode: routing -----------------------------------------------------------------------------
+// When the ring is far larger than L2 every direct reduction costs a 32-byte DRAM sector fetch and a
+// write-back.  Queue mode defers the add: an event due in ring slot s is appended as the 8-byte record
+// {cell offset, w_fx} to the bucket of slot group s >> q_log; gn_fold_kernel adds a whole bucket into its
+// 2^q_log ring rows just before the first of them is consumed, when those rows sit in L2.  Integer adds
+// commute, so ring contents at every consumption are identical to direct delivery (eq. 30).
+//
+// Rows are sorted by delay at create time, so the events of one source that share a bucket are one
+// contiguous run of its row: run heads do the bookkeeping (one shared-memory atomic per run), and a CTA
+// reserves space in a bucket once per pass over kRouteSources sources (one global atomic per bucket).
+// Events due in the current group (its rows were already folded) and events of a pass that would overflow
+// a bucket go straight to the ring.
+constexpr int kRouteThreads = 512;
+constexpr int kRouteWarps = kRouteThreads / 32;
+constexpr uint32_t kDirect = 0xFFFFu;
+constexpr unsigned long long kOverflow = ~0ull;
+
+struct RouteRun {
+    uint32_t key, s, head_lane, rank, len;
+    bool valid, head;
+};
+
+// Classify the 32 edges e0 .. e0+31 of a delay-sorted row: key = bucket, or kDirect for slots of the
+// current group that are still ahead of the slot pointer (d < dlim, no wrap).
+__device__ __forceinline__ RouteRun route_scan(const GnDev &p, const uint32_t slot_t, const uint32_t dlim,
+                                               const uint32_t e, const uint32_t end, const uint32_t lane)
+{
+    RouteRun r;
+    r.valid = e < end;
+    const uint32_t d = r.valid ? (uint32_t)p.s_dly[e] : 0u;
+    r.s = slot_t + d;
+    if (r.s >= p.D) r.s -= p.D;
+    r.key = !r.valid ? 0xFFFFFFFFu : (d < dlim ? kDirect : (r.s >> p.q_log));
+    const uint32_t prev = __shfl_up_sync(0xFFFFFFFFu, r.key, 1);
+    r.head = r.valid && (lane == 0u || r.key != prev);
+    const uint32_t hm = __ballot_sync(0xFFFFFFFFu, r.head);
+    const uint32_t n_valid = __popc(__ballot_sync(0xFFFFFFFFu, r.valid));
+    r.head_lane = 31u - __clz(hm & (0xFFFFFFFFu >> (31u - lane)));
+    const uint32_t above = hm & ~((2u << r.head_lane) - 1u);
+    const uint32_t next = above ? (uint32_t)(__ffs(above) - 1) : n_valid;
+    r.len = next - r.head_lane;
+    r.rank = lane - r.head_lane;
+    return r;
+}
+
+__global__ void __launch_bounds__(kRouteThreads, 2)
+gn_route_kernel(const GnDev p, const uint32_t slot_t, const uint32_t parity)
+{
+    __shared__ uint32_t s_cnt[256], s_cur[256];
+    __shared__ unsigned long long s_base[256];
+    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    const uint32_t n = p.n_active[parity];
+    const uint32_t *__restrict__ list = p.active + (size_t)parity * p.Npad;
+    const uint32_t *__restrict__ row = p.row;
+    const uint32_t g_cur = slot_t >> p.q_log;
+    uint32_t g_end = (g_cur + 1u) << p.q_log;
+    if (g_end > p.D) g_end = p.D;
+    const uint32_t dlim = g_end - slot_t;
+    // sources per pass: one per warp while the step is quiet, two when there is plenty of work
+    const uint32_t per_warp = (n >= 2u * kRouteWarps * gridDim.x) ? 2u : 1u;
+    const uint32_t per_pass = per_warp * kRouteWarps;
+    unsigned long long events = 0ull;
+
+    for (uint32_t c0 = blockIdx.x * per_pass; c0 < n; c0 += gridDim.x * per_pass) {
+        if (threadIdx.x < 256) s_cnt[threadIdx.x] = 0u;
+        __syncthreads();
+        // phase 1: how many records this pass appends to each bucket
+        for (uint32_t k = 0; k < per_warp; ++k) {
+            const uint32_t idx = c0 + k * kRouteWarps + warp;
+            if (idx >= n) break;
+            const uint32_t src = list[idx];
+            const uint32_t beg = row[src], end = row[src + 1];
+            for (uint32_t e0 = beg; e0 < end; e0 += 32u) {
+                const RouteRun r = route_scan(p, slot_t, dlim, e0 + lane, end, lane);
+                if (r.head && r.key != kDirect) atomicAdd(&s_cnt[r.key], r.len);
+            }
+            events += (unsigned long long)(end - beg);
+        }
+        __syncthreads();
+        // phase 2: reserve the space, one global atomic per bucket
+        if (threadIdx.x < p.q_nb) {
+            const uint32_t c = s_cnt[threadIdx.x];
+            unsigned long long base = kOverflow;
+            if (c) {
+                const unsigned long long got = atomicAdd(&p.q_count[threadIdx.x], (unsigned long long)c);
+                if (got + c <= p.q_cap) {
+                    base = got;
+                } else {                                  // bucket full: this pass delivers these directly;
+                    uint2 *q = p.queue + (size_t)threadIdx.x * p.q_cap;   // neutralise what it reserved
+                    for (unsigned long long i = got; i < p.q_cap; ++i) q[i] = make_uint2(0u, 0u);
+                }
+            }
+            s_base[threadIdx.x] = base;
+            s_cur[threadIdx.x] = 0u;
+        }
+        __syncthreads();
+        // phase 3: append the records (or reduce straight into the ring)
+        for (uint32_t k = 0; k < per_warp; ++k) {
+            const uint32_t idx = c0 + k * kRouteWarps + warp;
+            if (idx >= n) break;
+            const uint32_t src = list[idx];
+            const uint32_t beg = row[src], end = row[src + 1];
+            for (uint32_t e0 = beg; e0 < end; e0 += 32u) {
+                const uint32_t e = e0 + lane;
+                const RouteRun r = route_scan(p, slot_t, dlim, e, end, lane);
+                uint32_t pos = 0u;
+                if (r.head && r.key != kDirect) pos = atomicAdd(&s_cur[r.key], r.len);
+                pos = __shfl_sync(0xFFFFFFFFu, pos, r.head_lane & 31u);
+                if (r.valid) {
+                    const uint32_t m = p.s_tgt[e];
+                    const int32_t w = p.s_wfx[e];
+                    const unsigned long long base = (r.key == kDirect) ? kOverflow : s_base[r.key];
+                    if (base == kOverflow) {
+                        atomicAdd(p.ring + (size_t)r.s * p.Npad + m, w);
+                    } else {
+                        const uint32_t cell = (r.s - (r.key << p.q_log)) * p.Npad + m;
+                        p.queue[(size_t)r.key * p.q_cap + base + pos + r.rank] = make_uint2(cell, (uint32_t)w);
+                    }
+                }
+            }
+        }
+        __syncthreads();
+    }
+    if (lane == 0 && events) atomicAdd(&p.counters[2], events);
+}
+
+// ---- a4, queue mode: fold one bucket into its ring rows --------------------------------------------------
+__global__ void __launch_bounds__(256)
+gn_fold_kernel(const GnDev p, const uint32_t bucket)
+{
+    unsigned long long n = p.q_count[bucket];
+    if (n > p.q_cap) n = p.q_cap;
+    int32_t *rows = p.ring + ((size_t)bucket << p.q_log) * p.Npad;
+    const uint4 *q4 = reinterpret_cast<const uint4 *>(p.queue + (size_t)bucket * p.q_cap);
+    const unsigned long long pairs = n >> 1;
+    const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+    for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < pairs; i += stride) {
+        const uint4 v = __ldcs(q4 + i);
+        if (v.y) atomicAdd(rows + v.x, (int32_t)v.y);
+        if (v.w) atomicAdd(rows + v.z, (int32_t)v.w);
+    }
+    if ((n & 1ull) && blockIdx.x == 0 && threadIdx.x == 0) {
+        const uint2 v = p.queue[(size_t)bucket * p.q_cap + n - 1];
+        if (v.y) atomicAdd(rows + v.x, (int32_t)v.y);
+    }
+}
+
+// ---- create time, queue mode: copy every CSR row sorted by delay (counting sort, one warp per row) --------
+__global__ void __launch_bounds__(256)
+gn_sort_rows_kernel(const GnDev p)
+{
+    __shared__ uint32_t s_hist[8][256];
+    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    uint32_t *h = s_hist[warp];
+    const uint32_t n_warps = (gridDim.x * blockDim.x) >> 5;
+    for (uint32_t i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; i < p.N; i += n_warps) {
+        const uint32_t beg = p.row[i], end = p.row[i + 1];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) h[lane * 8 + k] = 0u;
+        __syncwarp();
+        for (uint32_t e = beg + lane; e < end; e += 32u) atomicAdd(&h[p.dly[e]], 1u);
+        __syncwarp();
+        uint32_t c[8], sum = 0u;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) { c[k] = h[lane * 8 + k]; sum += c[k]; }
+        uint32_t incl = sum;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t v = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+            if (lane >= (uint32_t)o) incl += v;
+        }
+        uint32_t run = incl - sum;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) { h[lane * 8 + k] = run; run += c[k]; }
+        __syncwarp();
+        for (uint32_t e = beg + lane; e < end; e += 32u) {
+            const uint32_t d = p.dly[e];
+            const uint32_t pos = beg + atomicAdd(&h[d], 1u);
+            p.s_tgt[pos] = p.tgt[e];
+            p.s_wfx[pos] = p.wfx[e];
+            p.s_dly[pos] = (uint8_t)d;
+        }
+        __syncwarp();
+    }
 }
 
 // ---- a5: one camera frame -------------------------------------------------------------------------------
@@ -398,16 +588,16 @@ inline uint32_t ceil_div(uint64_t a, uint64_t b) { return (uint32_t)((a + b - 1)
 }  // namespace
 
 // ---- launchers ------------------------------------------------------------------------------------------
-cudaError_t gnk_update(const GnDev &p, uint64_t t, bool has_bias, cudaStream_t st)
+cudaError_t gnk_update(const GnDev &p, uint64_t t, bool has_bias, uint32_t reset_bucket, cudaStream_t st)
 {
     const uint32_t grid = ceil_div(p.Npad / kVertsPerThread, kUpdateThreads);
     const uint32_t slot = (uint32_t)(t % p.D), parity = (uint32_t)(t & 1ull);
     const uint32_t raster_row = p.raster_cap ? (uint32_t)(t % p.raster_cap) : 0u;
     const bool obs = p.obs_stride != 0u;
-    if (obs && has_bias) gn_update_kernel<true, true><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, parity, raster_row);
-    else if (obs) gn_update_kernel<true, false><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, parity, raster_row);
-    else if (has_bias) gn_update_kernel<false, true><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, parity, raster_row);
-    else gn_update_kernel<false, false><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, parity, raster_row);
+    if (obs && has_bias) gn_update_kernel<true, true><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, parity, raster_row, reset_bucket);
+    else if (obs) gn_update_kernel<true, false><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, parity, raster_row, reset_bucket);
+    else if (has_bias) gn_update_kernel<false, true><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, parity, raster_row, reset_bucket);
+    else gn_update_kernel<false, false><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, parity, raster_row, reset_bucket);
     return cudaGetLastError();
 }
 
@@ -417,6 +607,28 @@ cudaError_t gnk_deliver(const GnDev &p, uint64_t t, cudaStream_t st)
     uint32_t grid = ceil_div(p.N, kDeliverThreads / 32);
     if (grid > 148u * 8u) grid = 148u * 8u;
     gn_deliver_kernel<<<grid, kDeliverThreads, 0, st>>>(p, (uint32_t)(t % p.D), (uint32_t)(t & 1ull));
+    return cudaGetLastError();
+}
+
+cudaError_t gnk_route(const GnDev &p, uint64_t t, cudaStream_t st)
+{
+    uint32_t grid = ceil_div(p.N, kRouteWarps);
+    if (grid > 148u * 2u) grid = 148u * 2u;                      // two 512-thread CTAs per SM, persistent loop
+    gn_route_kernel<<<grid, kRouteThreads, 0, st>>>(p, (uint32_t)(t % p.D), (uint32_t)(t & 1ull));
+    return cudaGetLastError();
+}
+
+cudaError_t gnk_fold(const GnDev &p, uint32_t bucket, cudaStream_t st)
+{
+    gn_fold_kernel<<<148u * 8u, 256, 0, st>>>(p, bucket);
+    return cudaGetLastError();
+}
+
+cudaError_t gnk_sort_rows(const GnDev &p, cudaStream_t st)
+{
+    uint32_t grid = ceil_div((uint64_t)p.N * 32, 256);
+    if (grid > 148u * 8u) grid = 148u * 8u;
+    gn_sort_rows_kernel<<<grid, 256, 0, st>>>(p);
     return cudaGetLastError();
 }
 

@@ -28,17 +28,26 @@ def test_library_exports_every_declared_symbol():
 
 def test_structs_match_header_layout():
     assert C.sizeof(gn.gn_class_params) == 12 * 4
-    # uint32 x2, uint64, uint32 x2, float x2, uint32, float x5, uint32 x3, (pad), uint64
-    assert C.sizeof(gn.gn_config) == 80
+    # uint32 x2, uint64, uint32 x2, float x2, uint32, float x5, uint32 x3, (pad), uint64, uint32 x2, uint64
+    assert C.sizeof(gn.gn_config) == 96
     assert gn.gn_config.seed.offset == 72 and gn.gn_config.n_edges.offset == 8
+    assert gn.gn_config.delivery_mode.offset == 80 and gn.gn_config.queue_capacity.offset == 88
 
 
 def test_query_workspace_sizes_and_errors():
-    cfg = gn.make_config(1_000_000, 3, 200_000_000, 128, 0.1, 0.006, 2, raster_capacity_steps=0)
+    cfg = gn.make_config(1_000_000, 3, 200_000_000, 128, 0.1, 0.006, 2, raster_capacity_steps=0,
+                         delivery_mode=gn.GN_DELIVER_RING)
     need = gn.gn_query_workspace(cfg)
+    # queue mode (what AUTO picks here: ring 512 MB >> L2): delay-sorted row copies + 16 buckets of 8 * E/16 records
+    auto = gn.gn_query_workspace(gn.make_config(1_000_000, 3, 200_000_000, 128, 0.1, 0.006, 2))
+    assert auto - need == pytest.approx(200_000_000 * 9 + 16 * 8 * 12_500_000 * 8, rel=1e-3)
+    for bad_q in (dict(delivery_mode=3), dict(queue_group=3), dict(queue_group=32)):
+        with pytest.raises(gn.GnError):
+            gn.gn_query_workspace(gn.make_config(10, 2, 5, 16, 0.1, 0.1, 1, **bad_q))
     ring, edges = 128 * 1_000_064 * 4, 200_000_000 * 9
     assert ring + edges < need < ring + edges + 120_000_000
-    bigger = gn.gn_query_workspace(gn.make_config(1_000_000, 3, 200_000_000, 128, 0.1, 0.006, 2, raster_capacity_steps=1000))
+    bigger = gn.gn_query_workspace(gn.make_config(1_000_000, 3, 200_000_000, 128, 0.1, 0.006, 2, raster_capacity_steps=1000,
+                                                      delivery_mode=gn.GN_DELIVER_RING))
     assert bigger - need == pytest.approx(1000 * 1_000_064 / 8, rel=1e-3)
     for bad in (dict(n_vertices=0), dict(dim=4), dict(ring_slots=1), dict(ring_slots=256), dict(n_classes=0),
                 dict(n_classes=9), dict(dt_ms=0.0), dict(n_edges=2 ** 32)):

@@ -31,10 +31,10 @@ def gn():
     return m
 
 
-def _make(gn, net, cfg, steps, delays=None, bias=None):
+def _make(gn, net, cfg, steps, delays=None, bias=None, **delivery):
     frames = steps // cfg["obs_stride"] if cfg.get("obs_stride", 0) else 0
     return gn.create_from_inputs(net, cfg, delays=delays, bias=bias, raster_capacity_steps=steps,
-                                 trace_capacity_frames=max(frames, 1))
+                                 trace_capacity_frames=max(frames, 1), **delivery)
 
 
 def _compare_exact(gn, g, o, t_done):
@@ -52,8 +52,8 @@ def _compare_exact(gn, g, o, t_done):
     assert (int(c[0]), int(c[1]), int(c[2]), int(c[3])) == (oc["steps"], oc["spikes"], oc["delivered"], oc["kicks"])
 
 
-def _run_exact(gn, net, cfg, steps, chunk, delays=None, bias=None, threads=4):
-    g = _make(gn, net, cfg, steps, delays, bias)
+def _run_exact(gn, net, cfg, steps, chunk, delays=None, bias=None, threads=4, **delivery):
+    g = _make(gn, net, cfg, steps, delays, bias, **delivery)
     o = Oracle(net, cfg, "fp32", delays=delays, bias=bias, threads=threads)
     if net.n_edges:
         np.testing.assert_array_equal(gn.gn_read_state(g, gn.GN_DELAYS).astype(np.uint32), o.delays())
@@ -120,6 +120,41 @@ def test_config_bit_exact_2000_steps(gn, k, n, nb, steps, chunk):
         np.testing.assert_allclose(zg, zo, rtol=1e-6, atol=1e-5)
         np.testing.assert_array_equal(gn.gn_read_state(g, gn.GN_CA).view(np.uint32),
                                       o.state(ob.CA).astype(np.float32).view(np.uint32))
+
+
+# ---- queue-mode delivery (deferred ring adds): same results, bit for bit -----------------------------
+QUEUE_CASES = [
+    # k, n, n_networks, steps, chunk, queue_group, queue_capacity
+    (4, 9_001, None, 2000, 500, 8, 0),        # the mode config 4 runs in: D=128, 16 buckets of 8 slots
+    (4, 9_001, None, 1000, 1000, 8, 0),       # ring never read back (no flush) until the end
+    (4, 5_003, None, 1200, 300, 16, 0),       # 8 buckets of 16 slots
+    (4, 5_003, None, 1200, 300, 1, 0),        # one bucket per slot: folded every step
+    (4, 5_003, None, 1200, 300, 8, 4096),     # buckets overflow: the excess is delivered directly
+    (4, 5_003, None, 600, 300, 4, 64),        # overflow on nearly every pass
+    (3, 6_007, None, 1500, 500, 8, 0),        # D=64
+    (2, None, None, 1000, 250, 4, 0),         # D=16 (observation on)
+    (2, 3_000, None, 600, 200, 8, 0),         # D=16: two buckets
+    (5, 1000, 6, 1000, 250, 8, 0),            # batched, D=32
+    (1, None, None, 2000, 500, 2, 0),         # N=100
+]
+
+
+@pytest.mark.parametrize("k,n,nb,steps,chunk,group,cap", QUEUE_CASES)
+def test_queue_mode_bit_exact(gn, k, n, nb, steps, chunk, group, cap):
+    net, cfg = make_config(k, n=n, n_networks=nb)
+    g, o, rast = _run_exact(gn, net, cfg, steps, chunk, delivery_mode=gn.GN_DELIVER_QUEUE, queue_group=group,
+                            queue_capacity=cap)
+    assert o.counters()["delivered"] > 0, "degenerate test: nothing delivered"
+
+
+def test_queue_mode_ring_depth_not_a_multiple_of_the_group(gn):
+    """D = 37 with groups of 8: the last bucket holds 5 slots; explicit delays up to D-1."""
+    rng = np.random.default_rng(11)
+    net, cfg = make_config(2, n=2_500)
+    cfg = dict(cfg, ring_slots=37, obs_stride=0)
+    delays = rng.integers(1, 37, size=net.n_edges).astype(np.uint8)
+    _, o, _ = _run_exact(gn, net, cfg, 900, 300, delays=delays, delivery_mode=gn.GN_DELIVER_QUEUE, queue_group=8)
+    assert o.counters()["delivered"] > 0
 
 
 @pytest.mark.parametrize("k,n,nb,steps", [(1, None, None, 2000), (2, None, None, 2000), (4, 9_001, None, 2000)])
