@@ -17,7 +17,7 @@ thread_local char g_create_error[256] = "";
 
 struct Layout {
     size_t V, W, r, c, acc, bias, refr, cls, ring, row, tgt, wfx, dly, active, n_active, counters, q_count;
-    size_t s_tgt, s_wfx, s_dly, queue;
+    size_t s_tgt, s_wfx, s_dly, q_seg, queue;
     size_t raster, trace, scratch_row64, scratch_abs, scratch_pos, scratch_net, scratch_chk, total;
 };
 
@@ -54,10 +54,11 @@ QueuePlan make_plan(const gn_config *cfg)
     const uint64_t N = cfg->n_vertices, Npad = (N + 127) / 128 * 128, E = cfg->n_edges, D = cfg->ring_slots;
     QueuePlan q{};
     uint32_t group = cfg->queue_group ? cfg->queue_group : 8u;
-    while (group > 1 && (Npad * group > 0xFFFFFFFFull || group > D)) group >>= 1;   // cell offsets are 32-bit
+    // cell offsets are 32-bit; the ring depth must be a whole number of groups
+    while (group > 1 && (Npad * group > 0xFFFFFFFFull || D % group != 0)) group >>= 1;
     q.on = cfg->delivery_mode == GN_DELIVER_QUEUE ||
            (cfg->delivery_mode == GN_DELIVER_AUTO && D >= 32 && D * Npad * 4 > (48ull << 20));
-    if (E == 0) q.on = false;
+    if (E == 0 || D / group > 64) q.on = false;      // gn_route_kernel stages at most 64 buckets
     q.q_log = 0;
     while ((1u << q.q_log) < group) q.q_log++;
     q.q_nb = (uint32_t)((D + group - 1) / group);
@@ -86,6 +87,7 @@ Layout make_layout(const gn_config *cfg)
     L.raster = take((size_t)cfg->raster_capacity_steps * (Npad / 32) * 4);
     L.trace = take(obs ? (size_t)cfg->trace_capacity_frames * Npad * 4 : 0);
     L.s_tgt = take(qp.on ? E * 4 : 0); L.s_wfx = take(qp.on ? E * 4 : 0); L.s_dly = take(qp.on ? E : 0);
+    L.q_seg = take(qp.on ? N * D * 2 : 0);
     L.queue = take(qp.on ? (size_t)qp.q_nb * qp.q_cap * 8 : 0);
     L.scratch_row64 = take((N + 1) * 8); L.scratch_abs = take(N * 8);
     L.scratch_pos = take(N * cfg->dim * 4); L.scratch_net = take(((size_t)cfg->n_networks + 1) * 4);
@@ -226,6 +228,7 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
     d.q_count = (unsigned long long *)(ws + L.q_count);
     if (qp.on) {
         d.s_tgt = (uint32_t *)(ws + L.s_tgt); d.s_wfx = (int32_t *)(ws + L.s_wfx); d.s_dly = ws + L.s_dly;
+        d.q_seg = (uint16_t *)(ws + L.q_seg);
         d.queue = (uint2 *)(ws + L.queue);
     }
     d.trace = cfg->obs_stride ? (float *)(ws + L.trace) : nullptr;
@@ -314,7 +317,7 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
         GN_CREATE_CUDA(gnk_validate(d, net_offsets ? net_d : nullptr, cfg->n_networks, abs_in, chk_d, st));
     }
     GN_CREATE_CUDA(gnk_check_overflow(d, abs_in, chk_d, st));
-    if (d.queue_mode) GN_CREATE_CUDA(gnk_sort_rows(d, st));
+    if (d.queue_mode) GN_CREATE_CUDA(gnk_sort_rows(d, chk_d, st));
     GN_CREATE_CUDA(cudaMemcpyAsync(&chk, chk_d, sizeof chk, cudaMemcpyDeviceToHost, st));
     GN_CREATE_CUDA(cudaStreamSynchronize(st));
 #undef GN_CREATE_CUDA
@@ -325,6 +328,13 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
                        : chk.bad_delay ? "delay outside [1, ring_slots-1]"
                        : chk.cross_net ? "edge crosses two networks"
                                        : "weight is NaN or outside the int32 fixed-point range");
+    }
+    if (chk.big_degree) {      // the 16-bit segment table cannot describe this graph
+        if (cfg->delivery_mode == GN_DELIVER_QUEUE) {
+            delete net;
+            return set_err(nullptr, GN_E_INVALID_ARG, "GN_DELIVER_QUEUE needs every out-degree <= 65535");
+        }
+        d.queue_mode = 0u;     // AUTO: same results through the ring path
     }
     if (chk.overflow) {
         delete net;

@@ -48,6 +48,7 @@ struct GnDev {
     uint32_t *s_tgt;         // [E] the CSR rows again, each sorted by delay
     int32_t *s_wfx;          // [E]
     uint8_t *s_dly;          // [E]
+    uint16_t *q_seg;         // [N][2^q_log][q_nb] segment boundaries of every delay-sorted row (gn_route_kernel)
     uint2 *queue;            // [q_nb][q_cap] records {cell offset inside the bucket's ring rows, w_fx}
     unsigned long long q_cap;
     unsigned long long *q_count;   // [q_nb] records appended (may exceed q_cap: the excess went direct)
@@ -63,7 +64,7 @@ struct GnDev {
 // Flags written by the create-time validation kernels.
 struct GnCheck {
     uint32_t bad_row, bad_target, bad_delay, bad_class, bad_weight, cross_net, overflow;
-    uint32_t pad;
+    uint32_t big_degree;     // some out-degree > 65535: the 16-bit segment table of queue mode cannot hold it
 };
 
 // ---- launchers (gn_kernels.cu).  All asynchronous on `st`; return the launch error. ----
@@ -71,7 +72,7 @@ cudaError_t gnk_update(const GnDev &p, uint64_t t, bool has_bias, uint32_t reset
 cudaError_t gnk_deliver(const GnDev &p, uint64_t t, cudaStream_t st);
 cudaError_t gnk_route(const GnDev &p, uint64_t t, cudaStream_t st);
 cudaError_t gnk_fold(const GnDev &p, uint32_t bucket, cudaStream_t st);
-cudaError_t gnk_sort_rows(const GnDev &p, cudaStream_t st);
+cudaError_t gnk_sort_rows(const GnDev &p, GnCheck *chk, cudaStream_t st);
 cudaError_t gnk_observe(const GnDev &p, uint64_t frame, cudaStream_t st);
 cudaError_t gnk_init_state(const GnDev &p, GnCheck *chk, cudaStream_t st);
 cudaError_t gnk_convert_rows(const GnDev &p, const uint64_t *row64, uint64_t n_edges, GnCheck *chk,

@@ -249,115 +249,120 @@ gn_deliver_kernel(const GnDev p, const uint32_t slot_t, const uint32_t parity)
 // commute, so ring contents at every consumption are identical to direct delivery (eq. 30).
 //
 // Rows are sorted by delay at create time, so the events of one source that share a bucket are one
-// contiguous run of its row: run heads do the bookkeeping (one shared-memory atomic per run), and a CTA
-// reserves space in a bucket once per pass over kRouteSources sources (one global atomic per bucket).
-// Events due in the current group (its rows were already folded) and events of a pass that would overflow
-// a bucket go straight to the ring.
+// contiguous SEGMENT of its row.  With G = 2^q_log slots per bucket, nb = D / G buckets and the slot
+// pointer at g_cur * G + r, a row splits, in delay order, into
+//     segment 0       delays [1, G - r)                 slots of the current group still ahead: DIRECT to the ring
+//     segment k       delays [kG - r, (k+1)G - r)       bucket (g_cur + k) mod nb,   k = 1 .. nb-1
+//     segment nb      delays [D - r, D)                 bucket g_cur (wrapped: consumed on the next lap)
+// The segment boundaries (edge positions inside the row) depend only on r and are tabulated per source at
+// create time: q_seg[(src * G + r) * nb + k] = #edges of src with delay < (k+1)G - r.  So routing needs no
+// search and no intra-warp communication: a CTA pass (1) loads the boundaries of its sources, (2) one thread
+// per bucket lays the sources' segments out back to back and reserves the space with ONE global atomic,
+// (3) every lane computes its record's final position from its edge position alone.
+// A pass that would overflow a bucket delivers those events directly instead.
 constexpr int kRouteThreads = 512;
 constexpr int kRouteWarps = kRouteThreads / 32;
-constexpr uint32_t kDirect = 0xFFFFu;
+constexpr int kRouteMaxSources = 2 * kRouteWarps;      // sources per CTA pass
+constexpr int kRouteMaxBuckets = 64;
+constexpr int kRouteUnroll = 8;                         // 8 x 32 edges of a row in flight per warp
 constexpr unsigned long long kOverflow = ~0ull;
-
-struct RouteRun {
-    uint32_t key, s, head_lane, rank, len;
-    bool valid, head;
-};
-
-// Classify the 32 edges e0 .. e0+31 of a delay-sorted row: key = bucket, or kDirect for slots of the
-// current group that are still ahead of the slot pointer (d < dlim, no wrap).
-__device__ __forceinline__ RouteRun route_scan(const GnDev &p, const uint32_t slot_t, const uint32_t dlim,
-                                               const uint32_t e, const uint32_t end, const uint32_t lane)
-{
-    RouteRun r;
-    r.valid = e < end;
-    const uint32_t d = r.valid ? (uint32_t)p.s_dly[e] : 0u;
-    r.s = slot_t + d;
-    if (r.s >= p.D) r.s -= p.D;
-    r.key = !r.valid ? 0xFFFFFFFFu : (d < dlim ? kDirect : (r.s >> p.q_log));
-    const uint32_t prev = __shfl_up_sync(0xFFFFFFFFu, r.key, 1);
-    r.head = r.valid && (lane == 0u || r.key != prev);
-    const uint32_t hm = __ballot_sync(0xFFFFFFFFu, r.head);
-    const uint32_t n_valid = __popc(__ballot_sync(0xFFFFFFFFu, r.valid));
-    r.head_lane = 31u - __clz(hm & (0xFFFFFFFFu >> (31u - lane)));
-    const uint32_t above = hm & ~((2u << r.head_lane) - 1u);
-    const uint32_t next = above ? (uint32_t)(__ffs(above) - 1) : n_valid;
-    r.len = next - r.head_lane;
-    r.rank = lane - r.head_lane;
-    return r;
-}
 
 __global__ void __launch_bounds__(kRouteThreads, 2)
 gn_route_kernel(const GnDev p, const uint32_t slot_t, const uint32_t parity)
 {
-    __shared__ uint32_t s_cnt[256], s_cur[256];
-    __shared__ unsigned long long s_base[256];
+    __shared__ uint32_t s_seg[kRouteMaxSources][kRouteMaxBuckets + 1];   // boundaries; [nb] = out-degree
+    __shared__ int32_t s_adj[kRouteMaxSources][kRouteMaxBuckets + 1];    // record position - edge position, per segment
+    __shared__ unsigned long long s_base[kRouteMaxBuckets];
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     const uint32_t n = p.n_active[parity];
     const uint32_t *__restrict__ list = p.active + (size_t)parity * p.Npad;
     const uint32_t *__restrict__ row = p.row;
-    const uint32_t g_cur = slot_t >> p.q_log;
-    uint32_t g_end = (g_cur + 1u) << p.q_log;
-    if (g_end > p.D) g_end = p.D;
-    const uint32_t dlim = g_end - slot_t;
+    const uint32_t nb = p.q_nb, G = 1u << p.q_log;
+    const uint32_t g_cur = slot_t >> p.q_log, r = slot_t & (G - 1u);
+    const uint32_t d_direct = G - r;                       // delays below this are segment 0
     // sources per pass: one per warp while the step is quiet, two when there is plenty of work
-    const uint32_t per_warp = (n >= 2u * kRouteWarps * gridDim.x) ? 2u : 1u;
+    const uint32_t per_warp = (n >= (uint32_t)kRouteMaxSources * gridDim.x) ? 2u : 1u;
     const uint32_t per_pass = per_warp * kRouteWarps;
     unsigned long long events = 0ull;
 
     for (uint32_t c0 = blockIdx.x * per_pass; c0 < n; c0 += gridDim.x * per_pass) {
-        if (threadIdx.x < 256) s_cnt[threadIdx.x] = 0u;
-        __syncthreads();
-        // phase 1: how many records this pass appends to each bucket
+        // phase 1: segment boundaries of this pass's sources
+        uint32_t beg[2] = {0u, 0u}, deg[2] = {0u, 0u};
         for (uint32_t k = 0; k < per_warp; ++k) {
-            const uint32_t idx = c0 + k * kRouteWarps + warp;
-            if (idx >= n) break;
-            const uint32_t src = list[idx];
-            const uint32_t beg = row[src], end = row[src + 1];
-            for (uint32_t e0 = beg; e0 < end; e0 += 32u) {
-                const RouteRun r = route_scan(p, slot_t, dlim, e0 + lane, end, lane);
-                if (r.head && r.key != kDirect) atomicAdd(&s_cnt[r.key], r.len);
+            const uint32_t i = k * kRouteWarps + warp, idx = c0 + i;
+            uint32_t src = 0u;
+            if (idx < n) {
+                src = list[idx];
+                beg[k] = row[src];
+                deg[k] = row[src + 1] - beg[k];
             }
-            events += (unsigned long long)(end - beg);
+            const uint16_t *seg = p.q_seg + ((size_t)src * G + r) * nb;
+            for (uint32_t j = lane; j <= nb; j += 32u)
+                s_seg[i][j] = (idx < n) ? (j < nb ? (uint32_t)__ldg(seg + j) : deg[k]) : 0u;
+            events += (unsigned long long)deg[k];
         }
         __syncthreads();
-        // phase 2: reserve the space, one global atomic per bucket
-        if (threadIdx.x < p.q_nb) {
-            const uint32_t c = s_cnt[threadIdx.x];
+        // phase 2: thread b lays out bucket b -- segment k of every source back to back -- and reserves it
+        if (threadIdx.x < nb) {
+            const uint32_t b = threadIdx.x;
+            uint32_t k = b + nb - g_cur;
+            if (k > nb) k -= nb;                          // k in 1 .. nb  (b == g_cur -> the wrapped segment nb)
+            uint32_t run = 0u;
+            for (uint32_t i = 0; i < per_pass; ++i) {
+                const uint32_t lo = s_seg[i][k - 1], hi = s_seg[i][k];
+                s_adj[i][k] = (int32_t)(run - lo);
+                run += hi - lo;
+            }
             unsigned long long base = kOverflow;
-            if (c) {
-                const unsigned long long got = atomicAdd(&p.q_count[threadIdx.x], (unsigned long long)c);
-                if (got + c <= p.q_cap) {
+            if (run) {
+                const unsigned long long got = atomicAdd(&p.q_count[b], (unsigned long long)run);
+                if (got + run <= p.q_cap) {
                     base = got;
                 } else {                                  // bucket full: this pass delivers these directly;
-                    uint2 *q = p.queue + (size_t)threadIdx.x * p.q_cap;   // neutralise what it reserved
+                    uint2 *q = p.queue + (size_t)b * p.q_cap;             // neutralise what it reserved
                     for (unsigned long long i = got; i < p.q_cap; ++i) q[i] = make_uint2(0u, 0u);
                 }
             }
-            s_base[threadIdx.x] = base;
-            s_cur[threadIdx.x] = 0u;
+            s_base[b] = base;
         }
         __syncthreads();
-        // phase 3: append the records (or reduce straight into the ring)
+        // phase 3: every edge of every source becomes a record (or a direct ring reduction)
         for (uint32_t k = 0; k < per_warp; ++k) {
-            const uint32_t idx = c0 + k * kRouteWarps + warp;
-            if (idx >= n) break;
-            const uint32_t src = list[idx];
-            const uint32_t beg = row[src], end = row[src + 1];
-            for (uint32_t e0 = beg; e0 < end; e0 += 32u) {
-                const uint32_t e = e0 + lane;
-                const RouteRun r = route_scan(p, slot_t, dlim, e, end, lane);
-                uint32_t pos = 0u;
-                if (r.head && r.key != kDirect) pos = atomicAdd(&s_cur[r.key], r.len);
-                pos = __shfl_sync(0xFFFFFFFFu, pos, r.head_lane & 31u);
-                if (r.valid) {
-                    const uint32_t m = p.s_tgt[e];
-                    const int32_t w = p.s_wfx[e];
-                    const unsigned long long base = (r.key == kDirect) ? kOverflow : s_base[r.key];
+            const uint32_t i = k * kRouteWarps + warp;
+            const uint32_t e_beg = beg[k], n_e = deg[k];
+            for (uint32_t x0 = 0; x0 < n_e; x0 += 32u * kRouteUnroll) {
+                uint32_t d[kRouteUnroll], m[kRouteUnroll];
+                int32_t w[kRouteUnroll];
+#pragma unroll
+                for (int u = 0; u < kRouteUnroll; ++u) {   // all loads of the super-chunk first
+                    const uint32_t x = x0 + 32u * u + lane;
+                    d[u] = 0u; m[u] = 0u; w[u] = 0;
+                    if (x < n_e) {
+                        d[u] = (uint32_t)__ldg(p.s_dly + e_beg + x);
+                        m[u] = __ldg(p.s_tgt + e_beg + x);
+                        w[u] = __ldg(p.s_wfx + e_beg + x);
+                    }
+                }
+#pragma unroll
+                for (int u = 0; u < kRouteUnroll; ++u) {
+                    const uint32_t x = x0 + 32u * u + lane;
+                    if (x >= n_e) continue;
+                    uint32_t s = slot_t + d[u];
+                    if (s >= p.D) s -= p.D;
+                    unsigned long long base = kOverflow;
+                    uint32_t b = 0u, k_seg = 0u;
+                    if (d[u] >= d_direct) {
+                        k_seg = 1u + ((d[u] - d_direct) >> p.q_log);
+                        b = g_cur + k_seg;
+                        if (b >= nb) b -= nb;
+                        base = s_base[b];
+                    }
                     if (base == kOverflow) {
-                        atomicAdd(p.ring + (size_t)r.s * p.Npad + m, w);
+                        atomicAdd(p.ring + (size_t)s * p.Npad + m[u], w[u]);
                     } else {
-                        const uint32_t cell = (r.s - (r.key << p.q_log)) * p.Npad + m;
-                        p.queue[(size_t)r.key * p.q_cap + base + pos + r.rank] = make_uint2(cell, (uint32_t)w);
+                        const uint32_t cell = (s - (b << p.q_log)) * p.Npad + m[u];
+                        const unsigned long long pos = base + (unsigned long long)(long long)(s_adj[i][k_seg] + (int32_t)x);
+                        p.queue[(size_t)b * p.q_cap + pos] = make_uint2(cell, (uint32_t)w[u]);
                     }
                 }
             }
@@ -390,7 +395,7 @@ gn_fold_kernel(const GnDev p, const uint32_t bucket)
 
 // ---- create time, queue mode: copy every CSR row sorted by delay (counting sort, one warp per row) --------
 __global__ void __launch_bounds__(256)
-gn_sort_rows_kernel(const GnDev p)
+gn_sort_rows_kernel(const GnDev p, GnCheck *chk)
 {
     __shared__ uint32_t s_hist[8][256];
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
@@ -415,6 +420,18 @@ gn_sort_rows_kernel(const GnDev p)
         uint32_t run = incl - sum;
 #pragma unroll
         for (int k = 0; k < 8; ++k) { h[lane * 8 + k] = run; run += c[k]; }
+        __syncwarp();
+        // h[d] = #edges with delay < d.  Segment table (see gn_route_kernel): entry (r, k) = h[(k+1)G - r].
+        {
+            const uint32_t G = 1u << p.q_log, nb = p.q_nb, deg = end - beg;
+            if (deg > 0xFFFFu) chk->big_degree = 1u;
+            uint16_t *seg = p.q_seg + (size_t)i * G * nb;
+            for (uint32_t x = lane; x < G * nb; x += 32u) {
+                const uint32_t r = x / nb, k = x - r * nb;
+                const uint32_t dd = (k + 1u) * G - r;
+                seg[x] = (uint16_t)(dd >= p.D ? deg : h[dd]);
+            }
+        }
         __syncwarp();
         for (uint32_t e = beg + lane; e < end; e += 32u) {
             const uint32_t d = p.dly[e];
@@ -624,11 +641,11 @@ cudaError_t gnk_fold(const GnDev &p, uint32_t bucket, cudaStream_t st)
     return cudaGetLastError();
 }
 
-cudaError_t gnk_sort_rows(const GnDev &p, cudaStream_t st)
+cudaError_t gnk_sort_rows(const GnDev &p, GnCheck *chk, cudaStream_t st)
 {
     uint32_t grid = ceil_div((uint64_t)p.N * 32, 256);
     if (grid > 148u * 8u) grid = 148u * 8u;
-    gn_sort_rows_kernel<<<grid, 256, 0, st>>>(p);
+    gn_sort_rows_kernel<<<grid, 256, 0, st>>>(p, chk);
     return cudaGetLastError();
 }
 
