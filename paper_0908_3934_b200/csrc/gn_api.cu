@@ -16,7 +16,7 @@ namespace {
 thread_local char g_create_error[256] = "";
 
 struct Layout {
-    size_t V, W, r, c, acc, bias, refr, cls, ring, row, tgt, wfx, dly, active, n_active, counters, q_count;
+    size_t V, W, r, c, acc, bias, refr, cls, ring, row, tgt, wfx, dly, counters, q_count;
     size_t s_tgt, s_wfx, s_dly, q_seg, queue;
     size_t raster, trace, scratch_row64, scratch_abs, scratch_pos, scratch_net, scratch_chk, total;
 };
@@ -81,10 +81,10 @@ Layout make_layout(const gn_config *cfg)
     L.refr = take(Npad); L.cls = take(Npad);
     L.ring = take(D * Npad * 4);
     L.row = take((Npad + 1) * 4); L.tgt = take(E * 4); L.wfx = take(E * 4); L.dly = take(E);
-    L.active = take(2 * Npad * 4); L.n_active = take(8); L.counters = take(32);
+    L.counters = take(32);
     const QueuePlan qp = make_plan(cfg);
     L.q_count = take(256 * 8);
-    L.raster = take((size_t)cfg->raster_capacity_steps * (Npad / 32) * 4);
+    L.raster = take((size_t)(cfg->raster_capacity_steps < 2 ? 2 : cfg->raster_capacity_steps) * (Npad / 32) * 4);
     L.trace = take(obs ? (size_t)cfg->trace_capacity_frames * Npad * 4 : 0);
     L.s_tgt = take(qp.on ? E * 4 : 0); L.s_wfx = take(qp.on ? E * 4 : 0); L.s_dly = take(qp.on ? E : 0);
     L.q_seg = take(qp.on ? N * D * 2 : 0);
@@ -219,9 +219,9 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
     d.ring = (int32_t *)(ws + L.ring);
     d.row = (uint32_t *)(ws + L.row); d.tgt = (uint32_t *)(ws + L.tgt);
     d.wfx = (int32_t *)(ws + L.wfx); d.dly = ws + L.dly;
-    d.active = (uint32_t *)(ws + L.active); d.n_active = (uint32_t *)(ws + L.n_active);
     d.counters = (unsigned long long *)(ws + L.counters);
     d.raster = (uint32_t *)(ws + L.raster);
+    d.raster_rows = cfg->raster_capacity_steps < 2 ? 2u : cfg->raster_capacity_steps;
     const QueuePlan qp = make_plan(cfg);
     d.queue_mode = qp.on ? 1u : 0u;
     d.q_log = qp.q_log; d.q_nb = qp.q_nb; d.q_cap = qp.q_cap;
@@ -274,7 +274,7 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
 
     // zero everything the step loop accumulates into or reads before writing
     GN_CREATE_CUDA(cudaMemsetAsync(ws, 0, L.tgt, st));                       // state, bias, refr, cls, ring, row
-    GN_CREATE_CUDA(cudaMemsetAsync(ws + L.active, 0, L.s_tgt - L.active, st));   // lists, counters, bucket counts, raster, trace
+    GN_CREATE_CUDA(cudaMemsetAsync(ws + L.counters, 0, L.s_tgt - L.counters, st));   // counters, bucket counts, raster, trace
     GN_CREATE_CUDA(cudaMemsetAsync(abs_in, 0, (size_t)N * 8, st));
     GN_CREATE_CUDA(cudaMemsetAsync(chk_d, 0, sizeof(GnCheck), st));
     // uploads (host or device sources)
@@ -398,12 +398,10 @@ int gn_step(gn_net *net, uint64_t n_steps)
         if (prof && (rc = prof_mark(net, 0))) return rc;
         GN_CUDA(net, gnk_update(d, t, net->has_bias, reset_bucket, net->stream));
         net->launches++;
-        if (net->cfg.n_edges) {
-            if (prof && (rc = prof_mark(net, 1))) return rc;
-            if (d.queue_mode) GN_CUDA(net, gnk_route(d, t, net->stream));
-            else GN_CUDA(net, gnk_deliver(d, t, net->stream));
-            net->launches++;
-        }
+        if (prof && (rc = prof_mark(net, 1))) return rc;      // also counts the step's spikes: runs even with E = 0
+        if (d.queue_mode) GN_CUDA(net, gnk_route(d, t, net->stream));
+        else GN_CUDA(net, gnk_deliver(d, t, net->stream));
+        net->launches++;
         if (d.obs_stride && (t + 1) % d.obs_stride == 0) {
             if (prof && (rc = prof_mark(net, 2))) return rc;
             GN_CUDA(net, gnk_observe(d, (t + 1) / d.obs_stride - 1, net->stream));
@@ -540,7 +538,7 @@ int gn_read_raster(gn_net *net, uint64_t t0, uint64_t n_steps, uint32_t *bits, s
     if (t0 + n_steps > net->t || d.raster_cap == 0 || t0 + d.raster_cap < net->t)
         return set_err(net, GN_E_RANGE_EVICTED, "raster steps [%llu, %llu) not held: simulated %llu, window %u",
                        (unsigned long long)t0, (unsigned long long)(t0 + n_steps), (unsigned long long)net->t, d.raster_cap);
-    return copy_window(net, bits, (const uint8_t *)d.raster, (size_t)d.words_pad * 4, words * 4, d.raster_cap, t0, n_steps, dst_is_device);
+    return copy_window(net, bits, (const uint8_t *)d.raster, (size_t)d.words_pad * 4, words * 4, d.raster_rows, t0, n_steps, dst_is_device);
 }
 
 int gn_observe(gn_net *net, uint64_t frame0, uint64_t n_frames, float *trace, size_t dst_bytes, int dst_is_device)

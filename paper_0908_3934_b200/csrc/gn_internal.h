@@ -52,11 +52,9 @@ struct GnDev {
     uint2 *queue;            // [q_nb][q_cap] records {cell offset inside the bucket's ring rows, w_fx}
     unsigned long long q_cap;
     unsigned long long *q_count;   // [q_nb] records appended (may exceed q_cap: the excess went direct)
-    // per-step active list, double buffered by step parity
-    uint32_t *active;        // [2][Npad]
-    uint32_t *n_active;      // [2]
     unsigned long long *counters;   // steps, spikes, delivered events, kicks
-    uint32_t *raster;        // [raster_cap][words_pad]
+    uint32_t *raster;        // [raster_rows][words_pad]; row t % raster_rows is step t's spike list
+    uint32_t raster_rows;    // max(raster_cap, 2): the delivery kernels read the current row even when none is kept
     float *trace;            // [trace_cap][Npad]
     GnClassDev cls_tab[GN_MAX_CLASSES];
 };

@@ -78,23 +78,17 @@ __device__ __forceinline__ bool vertex_step(const GnClassDev &q, const float dt,
 // Thread g owns vertices 4g .. 4g+3 (128-bit SoA loads); a warp owns 128 vertices = 4 raster words.
 template <bool OBS, bool BIAS>
 __global__ void __launch_bounds__(kUpdateThreads)
-gn_update_kernel(const GnDev p, const uint64_t t, const uint32_t slot, const uint32_t parity,
-                 const uint32_t raster_row, const uint32_t reset_bucket)
+gn_update_kernel(const GnDev p, const uint64_t t, const uint32_t slot, const uint32_t raster_row,
+                 const uint32_t reset_bucket)
 {
     __shared__ GnClassDev s_cls[GN_MAX_CLASSES];
-    __shared__ uint32_t s_cnt[kUpdateThreads / 32];
-    __shared__ uint32_t s_kick[kUpdateThreads / 32];
-    __shared__ uint32_t s_base;
-
     if (threadIdx.x < p.n_classes * 13u)
         reinterpret_cast<uint32_t *>(s_cls)[threadIdx.x] = reinterpret_cast<const uint32_t *>(p.cls_tab)[threadIdx.x];
-    if (blockIdx.x == 0 && threadIdx.x == 0) {
-        p.n_active[parity ^ 1u] = 0u;                                        // list of step t+1
-        if (reset_bucket != kNoBucket) p.q_count[reset_bucket] = 0ull;      // folded just before this launch
-    }
+    if (blockIdx.x == 0 && threadIdx.x == 0 && reset_bucket != kNoBucket)
+        p.q_count[reset_bucket] = 0ull;                                      // folded just before this launch
     __syncthreads();
 
-    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    const uint32_t lane = threadIdx.x & 31u;
     const uint32_t g = blockIdx.x * kUpdateThreads + threadIdx.x;
     const uint32_t j0 = g * kVertsPerThread;
     uint32_t nib = 0u, kicks = 0u;                                        // bit q: vertex j0+q fired / kicked
@@ -158,76 +152,81 @@ gn_update_kernel(const GnDev p, const uint64_t t, const uint32_t slot, const uin
         }
     }
 
-    // a3: raster bits.  Lane l holds bits 4*(l%8) .. +3 of word l/8 of this warp's 4 words.
+    // a3: raster bits.  Lane l holds bits 4*(l%8) .. +3 of word l/8 of this warp's 4 words.  The raster row of
+    // step t is also the step's spike list: the delivery kernels compact it (popc prefix) CTA by CTA.
     uint32_t word = nib << (4u * (lane & 7u));
     word |= __shfl_xor_sync(0xFFFFFFFFu, word, 1);
     word |= __shfl_xor_sync(0xFFFFFFFFu, word, 2);
     word |= __shfl_xor_sync(0xFFFFFFFFu, word, 4);
-    if (p.raster_cap && (lane & 7u) == 0u && j0 < p.Npad)
+    if ((lane & 7u) == 0u && j0 < p.Npad)
         p.raster[(size_t)raster_row * p.words_pad + (j0 >> 5)] = word;
-
-    // a3: compaction.  Ballot per vertex slot q, popc ranks, one global atomic per CTA.
-    uint32_t b[4], warp_total = 0u, warp_kicks = 0u;
-#pragma unroll
-    for (int q = 0; q < 4; ++q) {
-        b[q] = __ballot_sync(0xFFFFFFFFu, (nib >> q) & 1u);
-        warp_total += __popc(b[q]);
-        warp_kicks += __popc(__ballot_sync(0xFFFFFFFFu, (kicks >> q) & 1u));
+    if (__any_sync(0xFFFFFFFFu, kicks != 0u)) {                           // rare: one atomic per warp with a kick
+        const uint32_t warp_kicks = __reduce_add_sync(0xFFFFFFFFu, __popc(kicks));
+        if (lane == 0) atomicAdd(&p.counters[3], (unsigned long long)warp_kicks);
     }
-    if (lane == 0) {
-        s_cnt[warp] = warp_total;
-        s_kick[warp] = warp_kicks;
-    }
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        uint32_t total = 0u, ktotal = 0u;
-#pragma unroll
-        for (int w = 0; w < kUpdateThreads / 32; ++w) {
-            total += s_cnt[w];
-            ktotal += s_kick[w];
-        }
-        uint32_t base = 0u;
-        if (total) {
-            base = atomicAdd(&p.n_active[parity], total);
-            atomicAdd(&p.counters[1], (unsigned long long)total);
-        }
-        if (ktotal) atomicAdd(&p.counters[3], (unsigned long long)ktotal);
-        if (blockIdx.x == 0) p.counters[0] = t + 1ull;
-        s_base = base;
-    }
-    __syncthreads();
-    if (warp_total) {
-        uint32_t off = s_base;
-        for (uint32_t w = 0; w < warp; ++w) off += s_cnt[w];
-        uint32_t *list = p.active + (size_t)parity * p.Npad;
-        const uint32_t lt = (1u << lane) - 1u;
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            if ((nib >> q) & 1u) list[off + __popc(b[q] & lt)] = j0 + q;
-            off += __popc(b[q]);
-        }
-    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) p.counters[0] = t + 1ull;
 }
 
-// ---- a4: event delivery -------------------------------------------------------------------------------
-// One warp per active source; lanes stride over the source's CSR row (coalesced target / weight /
+// ---- a3 (compaction) shared by the delivery kernels ------------------------------------------------------
+// The step's raster row is its spike list.  A delivery CTA owns kChunkWords-or-fewer consecutive raster
+// words (chosen on the host so the grid covers the row) and compacts the set bits into a shared-memory
+// source list with a popc prefix scan: no global list, no global cursor.  Returns the number of sources.
+constexpr uint32_t kMaxChunkWords = 128;                 // 4096 vertices per CTA at most
+
+template <int THREADS>
+__device__ __forceinline__ uint32_t gather_sources(const uint32_t *__restrict__ raster_row, const uint32_t w0,
+                                                   const uint32_t n_words, uint32_t *s_list, uint32_t *s_wsum)
+{
+    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    uint32_t word = (threadIdx.x < n_words) ? raster_row[w0 + threadIdx.x] : 0u;
+    const uint32_t pc = __popc(word);
+    uint32_t incl = pc;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t v = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+        if (lane >= (uint32_t)o) incl += v;
+    }
+    if (lane == 31u) s_wsum[warp] = incl;
+    __syncthreads();
+    uint32_t off = incl - pc, total = 0u;
+#pragma unroll
+    for (int w = 0; w < THREADS / 32; ++w) {
+        const uint32_t c = s_wsum[w];
+        if ((uint32_t)w < warp) off += c;
+        total += c;
+    }
+    const uint32_t j_base = (w0 + threadIdx.x) << 5;
+    while (word) {
+        const uint32_t bit = (uint32_t)__ffs(word) - 1u;
+        s_list[off++] = j_base + bit;
+        word &= word - 1u;
+    }
+    __syncthreads();
+    return total;
+}
+
+// ---- a4: event delivery, ring mode ---------------------------------------------------------------------
+// One warp per fired source; lanes stride over the source's CSR row (coalesced target / weight /
 // delay reads); each edge is one int32 reduction (RED.ADD, no return) into ring[(t+delay) mod D][tgt].
 // PAPER.md:311 eq. 30 / :297.
 __global__ void __launch_bounds__(kDeliverThreads)
-gn_deliver_kernel(const GnDev p, const uint32_t slot_t, const uint32_t parity)
+gn_deliver_kernel(const GnDev p, const uint32_t slot_t, const uint32_t raster_row, const uint32_t chunk_words)
 {
-    const uint32_t lane = threadIdx.x & 31u;
-    const uint32_t warp_global = (blockIdx.x * kDeliverThreads + threadIdx.x) >> 5;
-    const uint32_t n_warps = (gridDim.x * kDeliverThreads) >> 5;
-    const uint32_t n = p.n_active[parity];
-    const uint32_t *__restrict__ list = p.active + (size_t)parity * p.Npad;
+    __shared__ uint32_t s_list[kMaxChunkWords * 32];
+    __shared__ uint32_t s_wsum[kDeliverThreads / 32];
+    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    const uint32_t w0 = blockIdx.x * chunk_words;
+    const uint32_t n_words = min(chunk_words, p.words_pad - w0);
+    const uint32_t n = gather_sources<kDeliverThreads>(p.raster + (size_t)raster_row * p.words_pad, w0, n_words,
+                                                       s_list, s_wsum);
+    if (n == 0u) return;
     const uint32_t *__restrict__ row = p.row;
     const uint32_t *__restrict__ tgt = p.tgt;
     const int32_t *__restrict__ wfx = p.wfx;
     const uint8_t *__restrict__ dly = p.dly;
     unsigned long long events = 0ull;
-    for (uint32_t idx = warp_global; idx < n; idx += n_warps) {
-        const uint32_t src = list[idx];
+    for (uint32_t idx = warp; idx < n; idx += kDeliverThreads / 32) {
+        const uint32_t src = s_list[idx];
         const uint32_t beg = row[src], end = row[src + 1];
         for (uint32_t e = beg + lane; e < end; e += 32u) {
             const uint32_t m = tgt[e];
@@ -239,6 +238,7 @@ gn_deliver_kernel(const GnDev p, const uint32_t slot_t, const uint32_t parity)
         events += (unsigned long long)(end - beg);
     }
     if (lane == 0 && events) atomicAdd(&p.counters[2], events);
+    if (threadIdx.x == 0) atomicAdd(&p.counters[1], (unsigned long long)n);
 }
 
 // ---- a4, queue mode: routing -----------------------------------------------------------------------------
@@ -268,24 +268,30 @@ constexpr int kRouteUnroll = 8;                         // 8 x 32 edges of a row
 constexpr unsigned long long kOverflow = ~0ull;
 
 __global__ void __launch_bounds__(kRouteThreads, 2)
-gn_route_kernel(const GnDev p, const uint32_t slot_t, const uint32_t parity)
+gn_route_kernel(const GnDev p, const uint32_t slot_t, const uint32_t raster_row, const uint32_t chunk_words)
 {
+    __shared__ uint32_t s_list[kMaxChunkWords * 32];
+    __shared__ uint32_t s_wsum[kRouteWarps];
     __shared__ uint32_t s_seg[kRouteMaxSources][kRouteMaxBuckets + 1];   // boundaries; [nb] = out-degree
     __shared__ int32_t s_adj[kRouteMaxSources][kRouteMaxBuckets + 1];    // record position - edge position, per segment
     __shared__ unsigned long long s_base[kRouteMaxBuckets];
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
-    const uint32_t n = p.n_active[parity];
-    const uint32_t *__restrict__ list = p.active + (size_t)parity * p.Npad;
+    const uint32_t w0 = blockIdx.x * chunk_words;
+    const uint32_t n_words = min(chunk_words, p.words_pad - w0);
+    const uint32_t n = gather_sources<kRouteThreads>(p.raster + (size_t)raster_row * p.words_pad, w0, n_words,
+                                                     s_list, s_wsum);
+    if (n == 0u) return;
+    const uint32_t *__restrict__ list = s_list;
     const uint32_t *__restrict__ row = p.row;
     const uint32_t nb = p.q_nb, G = 1u << p.q_log;
     const uint32_t g_cur = slot_t >> p.q_log, r = slot_t & (G - 1u);
     const uint32_t d_direct = G - r;                       // delays below this are segment 0
     // sources per pass: one per warp while the step is quiet, two when there is plenty of work
-    const uint32_t per_warp = (n >= (uint32_t)kRouteMaxSources * gridDim.x) ? 2u : 1u;
+    const uint32_t per_warp = (n > (uint32_t)kRouteWarps) ? 2u : 1u;
     const uint32_t per_pass = per_warp * kRouteWarps;
     unsigned long long events = 0ull;
 
-    for (uint32_t c0 = blockIdx.x * per_pass; c0 < n; c0 += gridDim.x * per_pass) {
+    for (uint32_t c0 = 0; c0 < n; c0 += per_pass) {
         // phase 1: segment boundaries of this pass's sources
         uint32_t beg[2] = {0u, 0u}, deg[2] = {0u, 0u};
         for (uint32_t k = 0; k < per_warp; ++k) {
@@ -370,6 +376,7 @@ gn_route_kernel(const GnDev p, const uint32_t slot_t, const uint32_t parity)
         __syncthreads();
     }
     if (lane == 0 && events) atomicAdd(&p.counters[2], events);
+    if (threadIdx.x == 0) atomicAdd(&p.counters[1], (unsigned long long)n);
 }
 
 // ---- a4, queue mode: fold one bucket into its ring rows --------------------------------------------------
@@ -608,30 +615,38 @@ inline uint32_t ceil_div(uint64_t a, uint64_t b) { return (uint32_t)((a + b - 1)
 cudaError_t gnk_update(const GnDev &p, uint64_t t, bool has_bias, uint32_t reset_bucket, cudaStream_t st)
 {
     const uint32_t grid = ceil_div(p.Npad / kVertsPerThread, kUpdateThreads);
-    const uint32_t slot = (uint32_t)(t % p.D), parity = (uint32_t)(t & 1ull);
-    const uint32_t raster_row = p.raster_cap ? (uint32_t)(t % p.raster_cap) : 0u;
+    const uint32_t slot = (uint32_t)(t % p.D);
+    const uint32_t raster_row = (uint32_t)(t % p.raster_rows);
     const bool obs = p.obs_stride != 0u;
-    if (obs && has_bias) gn_update_kernel<true, true><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, parity, raster_row, reset_bucket);
-    else if (obs) gn_update_kernel<true, false><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, parity, raster_row, reset_bucket);
-    else if (has_bias) gn_update_kernel<false, true><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, parity, raster_row, reset_bucket);
-    else gn_update_kernel<false, false><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, parity, raster_row, reset_bucket);
+    if (obs && has_bias) gn_update_kernel<true, true><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, raster_row, reset_bucket);
+    else if (obs) gn_update_kernel<true, false><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, raster_row, reset_bucket);
+    else if (has_bias) gn_update_kernel<false, true><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, raster_row, reset_bucket);
+    else gn_update_kernel<false, false><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, raster_row, reset_bucket);
     return cudaGetLastError();
+}
+
+// Raster words per delivery CTA: enough CTAs to fill the chip, at most kMaxChunkWords words each.
+static uint32_t chunk_words_for(const GnDev &p, uint32_t resident_ctas)
+{
+    uint32_t w = ceil_div(p.words_pad, resident_ctas);
+    if (w < 4u) w = 4u;
+    if (w > kMaxChunkWords) w = kMaxChunkWords;
+    return w;
 }
 
 cudaError_t gnk_deliver(const GnDev &p, uint64_t t, cudaStream_t st)
 {
-    // enough warps for one source each up to full residency (148 SMs x 8 CTAs), never more than N
-    uint32_t grid = ceil_div(p.N, kDeliverThreads / 32);
-    if (grid > 148u * 8u) grid = 148u * 8u;
-    gn_deliver_kernel<<<grid, kDeliverThreads, 0, st>>>(p, (uint32_t)(t % p.D), (uint32_t)(t & 1ull));
+    const uint32_t w = chunk_words_for(p, 148u * 8u);
+    gn_deliver_kernel<<<ceil_div(p.words_pad, w), kDeliverThreads, 0, st>>>(p, (uint32_t)(t % p.D),
+                                                                          (uint32_t)(t % p.raster_rows), w);
     return cudaGetLastError();
 }
 
 cudaError_t gnk_route(const GnDev &p, uint64_t t, cudaStream_t st)
 {
-    uint32_t grid = ceil_div(p.N, kRouteWarps);
-    if (grid > 148u * 2u) grid = 148u * 2u;                      // two 512-thread CTAs per SM, persistent loop
-    gn_route_kernel<<<grid, kRouteThreads, 0, st>>>(p, (uint32_t)(t % p.D), (uint32_t)(t & 1ull));
+    const uint32_t w = chunk_words_for(p, 148u * 2u);            // two 512-thread CTAs per SM
+    gn_route_kernel<<<ceil_div(p.words_pad, w), kRouteThreads, 0, st>>>(p, (uint32_t)(t % p.D),
+                                                                      (uint32_t)(t % p.raster_rows), w);
     return cudaGetLastError();
 }
 
