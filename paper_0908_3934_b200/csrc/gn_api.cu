@@ -86,7 +86,7 @@ Layout make_layout(const gn_config *cfg)
     L.q_count = take(256 * 8);
     L.raster = take((size_t)(cfg->raster_capacity_steps < 2 ? 2 : cfg->raster_capacity_steps) * (Npad / 32) * 4);
     L.trace = take(obs ? (size_t)cfg->trace_capacity_frames * Npad * 4 : 0);
-    L.s_tgt = take(qp.on ? E * 4 : 0); L.s_wfx = take(qp.on ? E * 4 : 0); L.s_dly = take(qp.on ? E : 0);
+    L.s_tgt = take(E * 4); L.s_wfx = take(E * 4); L.s_dly = take(E);   // every row again, sorted by delay
     L.q_seg = take(qp.on ? N * D * 2 : 0);
     L.queue = take(qp.on ? (size_t)qp.q_nb * qp.q_cap * 8 : 0);
     L.scratch_row64 = take((N + 1) * 8); L.scratch_abs = take(N * 8);
@@ -105,6 +105,10 @@ struct gn_net {
     cudaStream_t stream;
     uint8_t *ws;
     uint64_t t;          // steps enqueued so far
+    // delivery of step t overlaps the update of step t+1 (see gn_step): side streams and their fences
+    cudaStream_t s_deliver, s_fold;
+    cudaEvent_t ev_update, ev_deliver[2], ev_fold;
+    bool fences_pending;
     bool has_bias;
     // measuring mode (gn_profile)
     bool profile;
@@ -189,6 +193,9 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
     net->stream = (cudaStream_t)cuda_stream;
     net->ws = (uint8_t *)workspace;
     net->t = 0;
+    net->s_deliver = net->s_fold = nullptr;
+    net->ev_update = net->ev_deliver[0] = net->ev_deliver[1] = net->ev_fold = nullptr;
+    net->fences_pending = false;
     net->has_bias = bias != nullptr;
     net->profile = false;
     net->ev_used = 0;
@@ -226,8 +233,8 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
     d.queue_mode = qp.on ? 1u : 0u;
     d.q_log = qp.q_log; d.q_nb = qp.q_nb; d.q_cap = qp.q_cap;
     d.q_count = (unsigned long long *)(ws + L.q_count);
+    d.s_tgt = (uint32_t *)(ws + L.s_tgt); d.s_wfx = (int32_t *)(ws + L.s_wfx); d.s_dly = ws + L.s_dly;
     if (qp.on) {
-        d.s_tgt = (uint32_t *)(ws + L.s_tgt); d.s_wfx = (int32_t *)(ws + L.s_wfx); d.s_dly = ws + L.s_dly;
         d.q_seg = (uint16_t *)(ws + L.q_seg);
         d.queue = (uint2 *)(ws + L.queue);
     }
@@ -317,7 +324,7 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
         GN_CREATE_CUDA(gnk_validate(d, net_offsets ? net_d : nullptr, cfg->n_networks, abs_in, chk_d, st));
     }
     GN_CREATE_CUDA(gnk_check_overflow(d, abs_in, chk_d, st));
-    if (d.queue_mode) GN_CREATE_CUDA(gnk_sort_rows(d, chk_d, st));
+    if (E) GN_CREATE_CUDA(gnk_sort_rows(d, chk_d, st));
     GN_CREATE_CUDA(cudaMemcpyAsync(&chk, chk_d, sizeof chk, cudaMemcpyDeviceToHost, st));
     GN_CREATE_CUDA(cudaStreamSynchronize(st));
 #undef GN_CREATE_CUDA
@@ -329,7 +336,7 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
                        : chk.cross_net ? "edge crosses two networks"
                                        : "weight is NaN or outside the int32 fixed-point range");
     }
-    if (chk.big_degree) {      // the 16-bit segment table cannot describe this graph
+    if (chk.big_degree && d.queue_mode) {      // the 16-bit segment table cannot describe this graph
         if (cfg->delivery_mode == GN_DELIVER_QUEUE) {
             delete net;
             return set_err(nullptr, GN_E_INVALID_ARG, "GN_DELIVER_QUEUE needs every out-degree <= 65535");
@@ -339,6 +346,20 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
     if (chk.overflow) {
         delete net;
         return set_err(nullptr, GN_E_OVERFLOW_RISK, "some target's sum |w_fx| + |kick_fx| exceeds 2^31 - 1");
+    }
+    // side streams: delivery of step t runs beside the update of step t+1; a bucket is folded beside the
+    // steps that consume the group before it
+    {
+        int lo = 0, hi = 0;
+        cudaError_t e = cudaDeviceGetStreamPriorityRange(&lo, &hi);
+        if (e == cudaSuccess) e = cudaStreamCreateWithPriority(&net->s_deliver, cudaStreamNonBlocking, hi);
+        if (e == cudaSuccess) e = cudaStreamCreateWithPriority(&net->s_fold, cudaStreamNonBlocking, lo);
+        cudaEvent_t *evs[4] = {&net->ev_update, &net->ev_deliver[0], &net->ev_deliver[1], &net->ev_fold};
+        for (int k = 0; k < 4 && e == cudaSuccess; ++k) e = cudaEventCreateWithFlags(evs[k], cudaEventDisableTiming);
+        if (e != cudaSuccess) {
+            gn_destroy(net);
+            return set_err(nullptr, GN_E_CUDA, "creating side streams failed: %s", cudaGetErrorString(e));
+        }
     }
     *out = net;
     return GN_OK;
@@ -377,6 +398,26 @@ static int prof_collect(gn_net *net)
     return GN_OK;
 }
 
+// Make the caller's stream wait for everything the side streams still have in flight.
+static int join_streams(gn_net *net)
+{
+    if (!net->fences_pending) return GN_OK;
+    GN_CUDA(net, cudaStreamWaitEvent(net->stream, net->ev_deliver[0], 0));
+    GN_CUDA(net, cudaStreamWaitEvent(net->stream, net->ev_deliver[1], 0));
+    GN_CUDA(net, cudaStreamWaitEvent(net->stream, net->ev_fold, 0));
+    net->fences_pending = false;
+    return GN_OK;
+}
+
+// One step t is   update(t)  ->  deliver(t)   [+ fold of the NEXT group's bucket at a group's first step].
+// Dependencies (everything else may overlap):
+//   update(t)   after update(t-1) and deliver(t-2): events with delay 1 are sent by update(t-1) itself, so the
+//               earliest slot deliver(t-1) writes is t+1;
+//   deliver(t)  after update(t) (it reads step t's raster row) and deliver(t-1) (same stream);
+//   fold(g+1)   at the first step of group g, after deliver(t-1) (the last one that appends to bucket g+1: while
+//               group g is consumed, events due in g or g+1 go straight to the ring); done (and the bucket's count
+//               zeroed) before the first step of group g+1.
+// In profiling mode everything runs on the caller's stream in that order, so per-kernel times are clean.
 int gn_step(gn_net *net, uint64_t n_steps)
 {
     if (!net) return GN_E_INVALID_ARG;
@@ -384,27 +425,46 @@ int gn_step(gn_net *net, uint64_t n_steps)
     for (uint64_t s = 0; s < n_steps; ++s) {
         const uint64_t t = net->t;
         const bool prof = net->profile;
+        cudaStream_t s_upd = net->stream;
+        cudaStream_t s_del = prof ? net->stream : net->s_deliver;
+        cudaStream_t s_fld = prof ? net->stream : net->s_fold;
         int rc;
-        uint32_t reset_bucket = 0xFFFFFFFFu;
-        if (d.queue_mode) {                       // fold the bucket whose first ring row is consumed now
+        if (d.queue_mode) {
             const uint32_t slot = (uint32_t)(t % d.D);
             if ((slot & ((1u << d.q_log) - 1u)) == 0u) {
-                reset_bucket = slot >> d.q_log;
+                const uint32_t g_next = ((slot >> d.q_log) + 1u) % d.q_nb;
+                if (!prof) {
+                    GN_CUDA(net, cudaStreamWaitEvent(s_upd, net->ev_fold, 0));          // the fold of bucket g
+                    GN_CUDA(net, cudaEventRecord(net->ev_update, s_upd));               // everything the caller queued
+                    GN_CUDA(net, cudaStreamWaitEvent(s_fld, net->ev_update, 0));
+                    GN_CUDA(net, cudaStreamWaitEvent(s_fld, net->ev_deliver[(t + 1) & 1ull], 0));   // deliver(t-1)
+                }
                 if (prof && (rc = prof_mark(net, 3))) return rc;
-                GN_CUDA(net, gnk_fold(d, reset_bucket, net->stream));
+                GN_CUDA(net, gnk_fold(d, g_next, s_fld));
+                GN_CUDA(net, cudaMemsetAsync(d.q_count + g_next, 0, 8, s_fld));         // the bucket is empty again
                 net->launches++;
+                if (!prof) GN_CUDA(net, cudaEventRecord(net->ev_fold, s_fld));
             }
         }
+        if (!prof && t >= 2) GN_CUDA(net, cudaStreamWaitEvent(s_upd, net->ev_deliver[t & 1ull], 0));   // deliver(t-2)
         if (prof && (rc = prof_mark(net, 0))) return rc;
-        GN_CUDA(net, gnk_update(d, t, net->has_bias, reset_bucket, net->stream));
+        GN_CUDA(net, gnk_update(d, t, net->has_bias, s_upd));
         net->launches++;
+        if (!prof) {
+            GN_CUDA(net, cudaEventRecord(net->ev_update, s_upd));
+            GN_CUDA(net, cudaStreamWaitEvent(s_del, net->ev_update, 0));
+        }
         if (prof && (rc = prof_mark(net, 1))) return rc;      // also counts the step's spikes: runs even with E = 0
-        if (d.queue_mode) GN_CUDA(net, gnk_route(d, t, net->stream));
-        else GN_CUDA(net, gnk_deliver(d, t, net->stream));
+        if (d.queue_mode) GN_CUDA(net, gnk_route(d, t, s_del));
+        else GN_CUDA(net, gnk_deliver(d, t, s_del));
         net->launches++;
+        if (!prof) {
+            GN_CUDA(net, cudaEventRecord(net->ev_deliver[t & 1ull], s_del));
+            net->fences_pending = true;
+        }
         if (d.obs_stride && (t + 1) % d.obs_stride == 0) {
             if (prof && (rc = prof_mark(net, 2))) return rc;
-            GN_CUDA(net, gnk_observe(d, (t + 1) / d.obs_stride - 1, net->stream));
+            GN_CUDA(net, gnk_observe(d, (t + 1) / d.obs_stride - 1, s_upd));
             net->launches++;
         }
         if (prof && (rc = prof_mark(net, 0xFF))) return rc;
@@ -412,12 +472,14 @@ int gn_step(gn_net *net, uint64_t n_steps)
         if (prof && (s + 1) % kProfChunk == 0 && (rc = prof_collect(net))) return rc;
     }
     if (net->profile) return prof_collect(net);
-    return GN_OK;
+    return join_streams(net);
 }
 
 int gn_profile(gn_net *net, int enable)
 {
     if (!net) return GN_E_INVALID_ARG;
+    int rc = join_streams(net);
+    if (rc) return rc;
     net->profile = enable != 0;
     if (enable) {
         for (int k = 0; k < 4; ++k) { net->prof_ms[k] = 0.0; net->prof_n[k] = 0; }
@@ -569,8 +631,14 @@ const char *gn_last_error(const gn_net *net) { return net ? net->err : g_create_
 int gn_destroy(gn_net *net)
 {
     if (!net) return GN_E_INVALID_ARG;
+    if (net->s_deliver) cudaStreamSynchronize(net->s_deliver);
+    if (net->s_fold) cudaStreamSynchronize(net->s_fold);
     cudaError_t e = cudaStreamSynchronize(net->stream);
     for (cudaEvent_t ev : net->ev) cudaEventDestroy(ev);
+    cudaEvent_t evs[4] = {net->ev_update, net->ev_deliver[0], net->ev_deliver[1], net->ev_fold};
+    for (cudaEvent_t ev : evs) if (ev) cudaEventDestroy(ev);
+    if (net->s_deliver) cudaStreamDestroy(net->s_deliver);
+    if (net->s_fold) cudaStreamDestroy(net->s_fold);
     delete net;
     return e == cudaSuccess ? GN_OK : GN_E_CUDA;
 }

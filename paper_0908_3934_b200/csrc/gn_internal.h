@@ -66,7 +66,7 @@ struct GnCheck {
 };
 
 // ---- launchers (gn_kernels.cu).  All asynchronous on `st`; return the launch error. ----
-cudaError_t gnk_update(const GnDev &p, uint64_t t, bool has_bias, uint32_t reset_bucket, cudaStream_t st);
+cudaError_t gnk_update(const GnDev &p, uint64_t t, bool has_bias, cudaStream_t st);
 cudaError_t gnk_deliver(const GnDev &p, uint64_t t, cudaStream_t st);
 cudaError_t gnk_route(const GnDev &p, uint64_t t, cudaStream_t st);
 cudaError_t gnk_fold(const GnDev &p, uint32_t bucket, cudaStream_t st);

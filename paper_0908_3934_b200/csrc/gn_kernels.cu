@@ -18,7 +18,6 @@ constexpr int kUpdateThreads = 256;          // 8 warps x 128 vertices = 1024 ve
 constexpr int kVertsPerThread = 4;           // one 128-bit load per SoA array
 constexpr int kDeliverThreads = 256;
 constexpr uint32_t kStreamDrive = 5, kStreamNoise = 6;
-constexpr uint32_t kNoBucket = 0xFFFFFFFFu;
 
 // ---- Philox4x32-10 (Salmon et al., SC'11), from its published description -------------------
 __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
@@ -78,14 +77,11 @@ __device__ __forceinline__ bool vertex_step(const GnClassDev &q, const float dt,
 // Thread g owns vertices 4g .. 4g+3 (128-bit SoA loads); a warp owns 128 vertices = 4 raster words.
 template <bool OBS, bool BIAS>
 __global__ void __launch_bounds__(kUpdateThreads)
-gn_update_kernel(const GnDev p, const uint64_t t, const uint32_t slot, const uint32_t raster_row,
-                 const uint32_t reset_bucket)
+gn_update_kernel(const GnDev p, const uint64_t t, const uint32_t slot, const uint32_t raster_row)
 {
     __shared__ GnClassDev s_cls[GN_MAX_CLASSES];
     if (threadIdx.x < p.n_classes * 13u)
         reinterpret_cast<uint32_t *>(s_cls)[threadIdx.x] = reinterpret_cast<const uint32_t *>(p.cls_tab)[threadIdx.x];
-    if (blockIdx.x == 0 && threadIdx.x == 0 && reset_bucket != kNoBucket)
-        p.q_count[reset_bucket] = 0ull;                                      // folded just before this launch
     __syncthreads();
 
     const uint32_t lane = threadIdx.x & 31u;
@@ -160,6 +156,21 @@ gn_update_kernel(const GnDev p, const uint64_t t, const uint32_t slot, const uin
     word |= __shfl_xor_sync(0xFFFFFFFFu, word, 4);
     if ((lane & 7u) == 0u && j0 < p.Npad)
         p.raster[(size_t)raster_row * p.words_pad + (j0 >> 5)] = word;
+    // a4, the urgent part: an event with delay 1 is due in the very next step, so the vertex that fired sends
+    // it itself (rows are sorted by delay: such edges lead the row).  Everything else is delivered by the
+    // delivery kernel of this step, which may then overlap the NEXT step's update (gn_api.cu, gn_step).
+    if (nib) {
+        uint32_t s1 = slot + 1u;
+        if (s1 >= p.D) s1 = 0u;
+        int32_t *next_row = p.ring + (size_t)s1 * p.Npad;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            if (!((nib >> q) & 1u)) continue;
+            const uint32_t end = p.row[j0 + q + 1];
+            for (uint32_t e = p.row[j0 + q]; e < end && p.s_dly[e] == 1; ++e)
+                atomicAdd(next_row + p.s_tgt[e], p.s_wfx[e]);
+        }
+    }
     if (__any_sync(0xFFFFFFFFu, kicks != 0u)) {                           // rare: one atomic per warp with a kick
         const uint32_t warp_kicks = __reduce_add_sync(0xFFFFFFFFu, __popc(kicks));
         if (lane == 0) atomicAdd(&p.counters[3], (unsigned long long)warp_kicks);
@@ -221,9 +232,9 @@ gn_deliver_kernel(const GnDev p, const uint32_t slot_t, const uint32_t raster_ro
                                                        s_list, s_wsum);
     if (n == 0u) return;
     const uint32_t *__restrict__ row = p.row;
-    const uint32_t *__restrict__ tgt = p.tgt;
-    const int32_t *__restrict__ wfx = p.wfx;
-    const uint8_t *__restrict__ dly = p.dly;
+    const uint32_t *__restrict__ tgt = p.s_tgt;
+    const int32_t *__restrict__ wfx = p.s_wfx;
+    const uint8_t *__restrict__ dly = p.s_dly;
     unsigned long long events = 0ull;
     for (uint32_t idx = warp; idx < n; idx += kDeliverThreads / 32) {
         const uint32_t src = s_list[idx];
@@ -231,9 +242,10 @@ gn_deliver_kernel(const GnDev p, const uint32_t slot_t, const uint32_t raster_ro
         for (uint32_t e = beg + lane; e < end; e += 32u) {
             const uint32_t m = tgt[e];
             const int32_t w = wfx[e];
-            uint32_t s = slot_t + (uint32_t)dly[e];
+            const uint32_t d = dly[e];
+            uint32_t s = slot_t + d;
             if (s >= p.D) s -= p.D;
-            atomicAdd(p.ring + (size_t)s * p.Npad + m, w);
+            if (d != 1u) atomicAdd(p.ring + (size_t)s * p.Npad + m, w);   // delay 1 was sent by the update kernel
         }
         events += (unsigned long long)(end - beg);
     }
@@ -251,11 +263,14 @@ gn_deliver_kernel(const GnDev p, const uint32_t slot_t, const uint32_t raster_ro
 // Rows are sorted by delay at create time, so the events of one source that share a bucket are one
 // contiguous SEGMENT of its row.  With G = 2^q_log slots per bucket, nb = D / G buckets and the slot
 // pointer at g_cur * G + r, a row splits, in delay order, into
-//     segment 0       delays [1, G - r)                 slots of the current group still ahead: DIRECT to the ring
-//     segment k       delays [kG - r, (k+1)G - r)       bucket (g_cur + k) mod nb,   k = 1 .. nb-1
-//     segment nb      delays [D - r, D)                 bucket g_cur (wrapped: consumed on the next lap)
+//     segment 0       delays [1, 2G - r)                slots of the current and of the NEXT group (whose bucket is
+//                                                       being folded while this group is consumed): DIRECT to the ring
+//     segment k       delays [(k+1)G - r, (k+2)G - r)   bucket (g_cur + 1 + k) mod nb,   k = 1 .. nb-2
+//     segment nb-1    delays [D - r, D)                 bucket g_cur (wrapped: consumed on the next lap)
+// (delay-1 events were already sent by the update kernel and become zero-weight records here.)
 // The segment boundaries (edge positions inside the row) depend only on r and are tabulated per source at
-// create time: q_seg[(src * G + r) * nb + k] = #edges of src with delay < (k+1)G - r.  So routing needs no
+// create time: q_seg[(src * G + r) * nb + k] = #edges of src with delay < (k+1)G - r, so segment k of a row
+// is edge positions [q_seg[k], q_seg[k+1]) with q_seg[nb] = out-degree.  So routing needs no
 // search and no intra-warp communication: a CTA pass (1) loads the boundaries of its sources, (2) one thread
 // per bucket lays the sources' segments out back to back and reserves the space with ONE global atomic,
 // (3) every lane computes its record's final position from its edge position alone.
@@ -285,7 +300,7 @@ gn_route_kernel(const GnDev p, const uint32_t slot_t, const uint32_t raster_row,
     const uint32_t *__restrict__ row = p.row;
     const uint32_t nb = p.q_nb, G = 1u << p.q_log;
     const uint32_t g_cur = slot_t >> p.q_log, r = slot_t & (G - 1u);
-    const uint32_t d_direct = G - r;                       // delays below this are segment 0
+    const uint32_t d_direct = 2u * G - r;                  // delays below this are segment 0
     // sources per pass: one per warp while the step is quiet, two when there is plenty of work
     const uint32_t per_warp = (n > (uint32_t)kRouteWarps) ? 2u : 1u;
     const uint32_t per_pass = per_warp * kRouteWarps;
@@ -311,11 +326,11 @@ gn_route_kernel(const GnDev p, const uint32_t slot_t, const uint32_t raster_row,
         // phase 2: thread b lays out bucket b -- segment k of every source back to back -- and reserves it
         if (threadIdx.x < nb) {
             const uint32_t b = threadIdx.x;
-            uint32_t k = b + nb - g_cur;
-            if (k > nb) k -= nb;                          // k in 1 .. nb  (b == g_cur -> the wrapped segment nb)
+            uint32_t k = b + 2u * nb - g_cur - 1u;
+            while (k >= nb) k -= nb;                      // k in 0 .. nb-1; k == 0 is the next group: never queued
             uint32_t run = 0u;
-            for (uint32_t i = 0; i < per_pass; ++i) {
-                const uint32_t lo = s_seg[i][k - 1], hi = s_seg[i][k];
+            for (uint32_t i = 0; i < per_pass && k != 0u; ++i) {
+                const uint32_t lo = s_seg[i][k], hi = s_seg[i][k + 1];
                 s_adj[i][k] = (int32_t)(run - lo);
                 run += hi - lo;
             }
@@ -357,14 +372,15 @@ gn_route_kernel(const GnDev p, const uint32_t slot_t, const uint32_t raster_row,
                     if (s >= p.D) s -= p.D;
                     unsigned long long base = kOverflow;
                     uint32_t b = 0u, k_seg = 0u;
+                    if (d[u] == 1u) w[u] = 0;                   // already sent by the update kernel
                     if (d[u] >= d_direct) {
                         k_seg = 1u + ((d[u] - d_direct) >> p.q_log);
-                        b = g_cur + k_seg;
+                        b = g_cur + 1u + k_seg;
                         if (b >= nb) b -= nb;
                         base = s_base[b];
                     }
                     if (base == kOverflow) {
-                        atomicAdd(p.ring + (size_t)s * p.Npad + m[u], w[u]);
+                        if (w[u]) atomicAdd(p.ring + (size_t)s * p.Npad + m[u], w[u]);
                     } else {
                         const uint32_t cell = (s - (b << p.q_log)) * p.Npad + m[u];
                         const unsigned long long pos = base + (unsigned long long)(long long)(s_adj[i][k_seg] + (int32_t)x);
@@ -429,7 +445,7 @@ gn_sort_rows_kernel(const GnDev p, GnCheck *chk)
         for (int k = 0; k < 8; ++k) { h[lane * 8 + k] = run; run += c[k]; }
         __syncwarp();
         // h[d] = #edges with delay < d.  Segment table (see gn_route_kernel): entry (r, k) = h[(k+1)G - r].
-        {
+        if (p.q_seg) {
             const uint32_t G = 1u << p.q_log, nb = p.q_nb, deg = end - beg;
             if (deg > 0xFFFFu) chk->big_degree = 1u;
             uint16_t *seg = p.q_seg + (size_t)i * G * nb;
@@ -612,16 +628,16 @@ inline uint32_t ceil_div(uint64_t a, uint64_t b) { return (uint32_t)((a + b - 1)
 }  // namespace
 
 // ---- launchers ------------------------------------------------------------------------------------------
-cudaError_t gnk_update(const GnDev &p, uint64_t t, bool has_bias, uint32_t reset_bucket, cudaStream_t st)
+cudaError_t gnk_update(const GnDev &p, uint64_t t, bool has_bias, cudaStream_t st)
 {
     const uint32_t grid = ceil_div(p.Npad / kVertsPerThread, kUpdateThreads);
     const uint32_t slot = (uint32_t)(t % p.D);
     const uint32_t raster_row = (uint32_t)(t % p.raster_rows);
     const bool obs = p.obs_stride != 0u;
-    if (obs && has_bias) gn_update_kernel<true, true><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, raster_row, reset_bucket);
-    else if (obs) gn_update_kernel<true, false><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, raster_row, reset_bucket);
-    else if (has_bias) gn_update_kernel<false, true><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, raster_row, reset_bucket);
-    else gn_update_kernel<false, false><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, raster_row, reset_bucket);
+    if (obs && has_bias) gn_update_kernel<true, true><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, raster_row);
+    else if (obs) gn_update_kernel<true, false><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, raster_row);
+    else if (has_bias) gn_update_kernel<false, true><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, raster_row);
+    else gn_update_kernel<false, false><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, raster_row);
     return cudaGetLastError();
 }
 
