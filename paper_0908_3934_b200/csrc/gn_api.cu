@@ -58,12 +58,13 @@ QueuePlan make_plan(const gn_config *cfg)
     while (group > 1 && (Npad * group > 0xFFFFFFFFull || D % group != 0)) group >>= 1;
     q.on = cfg->delivery_mode == GN_DELIVER_QUEUE ||
            (cfg->delivery_mode == GN_DELIVER_AUTO && D >= 32 && D * Npad * 4 > (48ull << 20));
-    if (E == 0 || D / group > 64) q.on = false;      // gn_route_kernel stages at most 64 buckets
+    if (E == 0 || D / group > 32) q.on = false;      // gn_route_kernel: one lane per bucket
     q.q_log = 0;
     while ((1u << q.q_log) < group) q.q_log++;
     q.q_nb = (uint32_t)((D + group - 1) / group);
     uint64_t cap = cfg->queue_capacity ? cfg->queue_capacity : (uint64_t)group * ((E + 15) / 16);
     if (cap < 64) cap = 64;
+    if (cap > 0xFFFFFF00ull) cap = 0xFFFFFF00ull;    // record positions are 32-bit
     q.q_cap = (cap + 31) / 32 * 32;
     return q;
 }

@@ -76,7 +76,7 @@ __device__ __forceinline__ bool vertex_step(const GnClassDev &q, const float dt,
 // ---- a1 + a2 + a3 (+ calcium of a5) ---------------------------------------------------------------
 // Thread g owns vertices 4g .. 4g+3 (128-bit SoA loads); a warp owns 128 vertices = 4 raster words.
 template <bool OBS, bool BIAS>
-__global__ void __launch_bounds__(kUpdateThreads)
+__global__ void __launch_bounds__(kUpdateThreads, 8)
 gn_update_kernel(const GnDev p, const uint64_t t, const uint32_t slot, const uint32_t raster_row)
 {
     __shared__ GnClassDev s_cls[GN_MAX_CLASSES];
@@ -90,59 +90,58 @@ gn_update_kernel(const GnDev p, const uint64_t t, const uint32_t slot, const uin
     uint32_t nib = 0u, kicks = 0u;                                        // bit q: vertex j0+q fired / kicked
 
     if (j0 < p.Npad) {
+        // drive first (its temporaries are dead before the state is loaded: the kernel must fit 32 registers
+        // so that all N/4 threads are resident in ONE wave): one Philox block per 4 vertices, counter
+        // {j/4, t lo, t hi, 5}, word j mod 4; Bernoulli kick when the word is below the class threshold
+        const uchar4 cl4 = *reinterpret_cast<const uchar4 *>(p.cls + j0);
+        const uint32_t cl[4] = {cl4.x, cl4.y, cl4.z, cl4.w};
+        if (p.any_drive) {
+            uint32_t x[4];
+            philox4x32_10(g, (uint32_t)t, (uint32_t)(t >> 32), kStreamDrive, p.seed_lo, p.seed_hi, x);
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+                if ((j0 + q) < p.N && x[q] < s_cls[cl[q]].drive_thr) kicks |= 1u << q;   // reading #12
+        }
         // a1: read this step's ring slot, clear it only if something arrived
         int4 *slot_ptr = reinterpret_cast<int4 *>(p.ring + (size_t)slot * p.Npad + j0);
-        int4 I4 = *slot_ptr;
-        if ((I4.x | I4.y | I4.z | I4.w) != 0) *slot_ptr = make_int4(0, 0, 0, 0);
-        float4 V4 = *reinterpret_cast<const float4 *>(p.V + j0);
-        float4 W4 = *reinterpret_cast<const float4 *>(p.W + j0);
-        float4 r4 = *reinterpret_cast<const float4 *>(p.r + j0);
+        const int4 I4 = *slot_ptr;
+        const float4 V4 = *reinterpret_cast<const float4 *>(p.V + j0);
+        const float4 W4 = *reinterpret_cast<const float4 *>(p.W + j0);
+        const float4 r4 = *reinterpret_cast<const float4 *>(p.r + j0);
         const uchar4 rf4 = *reinterpret_cast<const uchar4 *>(p.refr + j0);
-        const uchar4 cl4 = *reinterpret_cast<const uchar4 *>(p.cls + j0);
         float4 U4 = make_float4(0.f, 0.f, 0.f, 0.f);
         if (BIAS) U4 = *reinterpret_cast<const float4 *>(p.bias + j0);
-        float4 c4 = make_float4(0.f, 0.f, 0.f, 0.f), a4 = c4;
-        if (OBS) {
-            c4 = *reinterpret_cast<const float4 *>(p.c + j0);
-            a4 = *reinterpret_cast<const float4 *>(p.acc + j0);
-        }
+        if ((I4.x | I4.y | I4.z | I4.w) != 0) *slot_ptr = make_int4(0, 0, 0, 0);
 
         int32_t I[4] = {I4.x, I4.y, I4.z, I4.w};
         float V[4] = {V4.x, V4.y, V4.z, V4.w}, W[4] = {W4.x, W4.y, W4.z, W4.w};
         float r[4] = {r4.x, r4.y, r4.z, r4.w}, U[4] = {U4.x, U4.y, U4.z, U4.w};
-        float c[4] = {c4.x, c4.y, c4.z, c4.w}, acc[4] = {a4.x, a4.y, a4.z, a4.w};
         uint32_t refr[4] = {rf4.x, rf4.y, rf4.z, rf4.w};
-        const uint32_t cl[4] = {cl4.x, cl4.y, cl4.z, cl4.w};
-
-        // drive: one Philox block per 4 vertices, counter {j/4, t lo, t hi, 5}, word j mod 4
-        uint32_t x[4] = {0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu};
-        if (p.any_drive)
-            philox4x32_10(g, (uint32_t)t, (uint32_t)(t >> 32), kStreamDrive, p.seed_lo, p.seed_hi, x);
 
         uint32_t refr_changed = 0u;
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
             const GnClassDev &k = s_cls[cl[q]];
-            const bool live = (j0 + q) < p.N;
-            if (live && x[q] < k.drive_thr) {                              // Bernoulli kick (reading #12)
-                I[q] += k.kick_fx;
-                kicks |= 1u << q;
-            }
+            if ((kicks >> q) & 1u) I[q] += k.kick_fx;
             const uint32_t refr_old = refr[q];
-            const bool fired = vertex_step<BIAS>(k, p.dt, I[q], U[q], V[q], W[q], r[q], refr[q]) && live;
+            const bool fired = vertex_step<BIAS>(k, p.dt, I[q], U[q], V[q], W[q], r[q], refr[q]) && (j0 + q) < p.N;
             refr_changed |= (refr[q] != refr_old);
             if (fired) nib |= 1u << q;
-            if (OBS) {
-                c[q] = __fmaf_rn(p.keep_c, c[q], fired ? p.ca_jump : 0.0f);   // H_c
-                acc[q] = __fadd_rn(acc[q], c[q]);
-            }
         }
         *reinterpret_cast<float4 *>(p.V + j0) = make_float4(V[0], V[1], V[2], V[3]);
         *reinterpret_cast<float4 *>(p.W + j0) = make_float4(W[0], W[1], W[2], W[3]);
         *reinterpret_cast<float4 *>(p.r + j0) = make_float4(r[0], r[1], r[2], r[3]);
         if (refr_changed)
             *reinterpret_cast<uchar4 *>(p.refr + j0) = make_uchar4(refr[0], refr[1], refr[2], refr[3]);
-        if (OBS) {
+        if (OBS) {                                                            // calcium + frame accumulator
+            const float4 c4 = *reinterpret_cast<const float4 *>(p.c + j0);
+            const float4 a4 = *reinterpret_cast<const float4 *>(p.acc + j0);
+            float c[4] = {c4.x, c4.y, c4.z, c4.w}, acc[4] = {a4.x, a4.y, a4.z, a4.w};
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                c[q] = __fmaf_rn(p.keep_c, c[q], ((nib >> q) & 1u) ? p.ca_jump : 0.0f);   // H_c
+                acc[q] = __fadd_rn(acc[q], c[q]);
+            }
             *reinterpret_cast<float4 *>(p.c + j0) = make_float4(c[0], c[1], c[2], c[3]);
             *reinterpret_cast<float4 *>(p.acc + j0) = make_float4(acc[0], acc[1], acc[2], acc[3]);
         }
@@ -270,126 +269,132 @@ gn_deliver_kernel(const GnDev p, const uint32_t slot_t, const uint32_t raster_ro
 // (delay-1 events were already sent by the update kernel and become zero-weight records here.)
 // The segment boundaries (edge positions inside the row) depend only on r and are tabulated per source at
 // create time: q_seg[(src * G + r) * nb + k] = #edges of src with delay < (k+1)G - r, so segment k of a row
-// is edge positions [q_seg[k], q_seg[k+1]) with q_seg[nb] = out-degree.  So routing needs no
-// search and no intra-warp communication: a CTA pass (1) loads the boundaries of its sources, (2) one thread
-// per bucket lays the sources' segments out back to back and reserves the space with ONE global atomic,
-// (3) every lane computes its record's final position from its edge position alone.
-// A pass that would overflow a bucket delivers those events directly instead.
-constexpr int kRouteThreads = 512;
+// is edge positions [q_seg[k], q_seg[k+1]) with q_seg[nb] = out-degree.  Lane k of a warp owns segment k
+// (nb <= 32), so routing needs no search and two CTA barriers per step whatever the number of sources:
+//   A  every warp walks its share of the CTA's sources and sums, per lane, the segment sizes;
+//   B  warp 0 lays the warps' totals out back to back per bucket and reserves the space with ONE global
+//      atomic per bucket (a CTA that would overflow a bucket delivers those events directly instead);
+//   C  every warp walks its sources again (boundaries now come from L1/L2), keeps a running offset per
+//      segment in the owning lane, and each edge becomes a record whose position is
+//      [warp base + running offset - segment start](segment, by shuffle) + edge position.
+constexpr int kRouteThreads = 256;
 constexpr int kRouteWarps = kRouteThreads / 32;
-constexpr int kRouteMaxSources = 2 * kRouteWarps;      // sources per CTA pass
-constexpr int kRouteMaxBuckets = 64;
 constexpr int kRouteUnroll = 8;                         // 8 x 32 edges of a row in flight per warp
-constexpr unsigned long long kOverflow = ~0ull;
 
-__global__ void __launch_bounds__(kRouteThreads, 2)
+// Lane k: boundaries of segment k of `src` at alignment r -> lo (start position) and cnt (size); 0 for lanes
+// that own no queued segment (k = 0 or k >= nb).
+__device__ __forceinline__ void route_segments(const GnDev &p, const uint32_t src, const uint32_t r, const uint32_t nb,
+                                               const uint32_t deg, const uint32_t lane, uint32_t &lo, uint32_t &cnt)
+{
+    const uint16_t *seg = p.q_seg + ((size_t)src << p.q_log) * nb + (size_t)r * nb;
+    lo = (lane < nb) ? (uint32_t)__ldg(seg + lane) : deg;
+    uint32_t hi = __shfl_down_sync(0xFFFFFFFFu, lo, 1);
+    if (lane + 1u >= nb) hi = deg;
+    cnt = (lane >= 1u && lane < nb) ? hi - lo : 0u;
+}
+
+__global__ void __launch_bounds__(kRouteThreads, 4)
 gn_route_kernel(const GnDev p, const uint32_t slot_t, const uint32_t raster_row, const uint32_t chunk_words)
 {
     __shared__ uint32_t s_list[kMaxChunkWords * 32];
     __shared__ uint32_t s_wsum[kRouteWarps];
-    __shared__ uint32_t s_seg[kRouteMaxSources][kRouteMaxBuckets + 1];   // boundaries; [nb] = out-degree
-    __shared__ int32_t s_adj[kRouteMaxSources][kRouteMaxBuckets + 1];    // record position - edge position, per segment
-    __shared__ unsigned long long s_base[kRouteMaxBuckets];
+    __shared__ uint32_t s_wtot[kRouteWarps][32];         // A: records of warp w in segment k
+    __shared__ uint32_t s_wbase[kRouteWarps][32];        // B: where warp w's records of segment k start in the bucket
+    __shared__ uint32_t s_ovf;                           // B: bit k = segment k's bucket is full
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     const uint32_t w0 = blockIdx.x * chunk_words;
     const uint32_t n_words = min(chunk_words, p.words_pad - w0);
     const uint32_t n = gather_sources<kRouteThreads>(p.raster + (size_t)raster_row * p.words_pad, w0, n_words,
                                                      s_list, s_wsum);
     if (n == 0u) return;
-    const uint32_t *__restrict__ list = s_list;
     const uint32_t *__restrict__ row = p.row;
     const uint32_t nb = p.q_nb, G = 1u << p.q_log;
     const uint32_t g_cur = slot_t >> p.q_log, r = slot_t & (G - 1u);
     const uint32_t d_direct = 2u * G - r;                  // delays below this are segment 0
-    // sources per pass: one per warp while the step is quiet, two when there is plenty of work
-    const uint32_t per_warp = (n > (uint32_t)kRouteWarps) ? 2u : 1u;
-    const uint32_t per_pass = per_warp * kRouteWarps;
-    unsigned long long events = 0ull;
+    uint32_t my_bucket = g_cur + 1u + lane;               // bucket of the segment this lane owns
+    while (my_bucket >= nb) my_bucket -= nb;
 
-    for (uint32_t c0 = 0; c0 < n; c0 += per_pass) {
-        // phase 1: segment boundaries of this pass's sources
-        uint32_t beg[2] = {0u, 0u}, deg[2] = {0u, 0u};
-        for (uint32_t k = 0; k < per_warp; ++k) {
-            const uint32_t i = k * kRouteWarps + warp, idx = c0 + i;
-            uint32_t src = 0u;
-            if (idx < n) {
-                src = list[idx];
-                beg[k] = row[src];
-                deg[k] = row[src + 1] - beg[k];
-            }
-            const uint16_t *seg = p.q_seg + ((size_t)src * G + r) * nb;
-            for (uint32_t j = lane; j <= nb; j += 32u)
-                s_seg[i][j] = (idx < n) ? (j < nb ? (uint32_t)__ldg(seg + j) : deg[k]) : 0u;
-            events += (unsigned long long)deg[k];
-        }
-        __syncthreads();
-        // phase 2: thread b lays out bucket b -- segment k of every source back to back -- and reserves it
-        if (threadIdx.x < nb) {
-            const uint32_t b = threadIdx.x;
-            uint32_t k = b + 2u * nb - g_cur - 1u;
-            while (k >= nb) k -= nb;                      // k in 0 .. nb-1; k == 0 is the next group: never queued
-            uint32_t run = 0u;
-            for (uint32_t i = 0; i < per_pass && k != 0u; ++i) {
-                const uint32_t lo = s_seg[i][k], hi = s_seg[i][k + 1];
-                s_adj[i][k] = (int32_t)(run - lo);
-                run += hi - lo;
-            }
-            unsigned long long base = kOverflow;
-            if (run) {
-                const unsigned long long got = atomicAdd(&p.q_count[b], (unsigned long long)run);
-                if (got + run <= p.q_cap) {
-                    base = got;
-                } else {                                  // bucket full: this pass delivers these directly;
-                    uint2 *q = p.queue + (size_t)b * p.q_cap;             // neutralise what it reserved
-                    for (unsigned long long i = got; i < p.q_cap; ++i) q[i] = make_uint2(0u, 0u);
-                }
-            }
-            s_base[b] = base;
-        }
-        __syncthreads();
-        // phase 3: every edge of every source becomes a record (or a direct ring reduction)
-        for (uint32_t k = 0; k < per_warp; ++k) {
-            const uint32_t i = k * kRouteWarps + warp;
-            const uint32_t e_beg = beg[k], n_e = deg[k];
-            for (uint32_t x0 = 0; x0 < n_e; x0 += 32u * kRouteUnroll) {
-                uint32_t d[kRouteUnroll], m[kRouteUnroll];
-                int32_t w[kRouteUnroll];
+    // A: per-warp, per-segment record counts
+    uint32_t tot = 0u;
+    unsigned long long events = 0ull;
+    for (uint32_t idx = warp; idx < n; idx += kRouteWarps) {
+        const uint32_t src = s_list[idx];
+        const uint32_t deg = row[src + 1] - row[src];
+        uint32_t lo, cnt;
+        route_segments(p, src, r, nb, deg, lane, lo, cnt);
+        tot += cnt;
+        events += (unsigned long long)deg;
+    }
+    s_wtot[warp][lane] = tot;
+    __syncthreads();
+    // B: reserve
+    if (warp == 0) {
+        uint32_t run = 0u;
 #pragma unroll
-                for (int u = 0; u < kRouteUnroll; ++u) {   // all loads of the super-chunk first
-                    const uint32_t x = x0 + 32u * u + lane;
-                    d[u] = 0u; m[u] = 0u; w[u] = 0;
-                    if (x < n_e) {
-                        d[u] = (uint32_t)__ldg(p.s_dly + e_beg + x);
-                        m[u] = __ldg(p.s_tgt + e_beg + x);
-                        w[u] = __ldg(p.s_wfx + e_beg + x);
-                    }
-                }
+        for (int w = 0; w < kRouteWarps; ++w) {
+            const uint32_t c = s_wtot[w][lane];
+            s_wbase[w][lane] = run;
+            run += c;
+        }
+        bool full = false;
+        if (run) {
+            const unsigned long long got = atomicAdd(&p.q_count[my_bucket], (unsigned long long)run);
+            if (got + run <= p.q_cap) {
 #pragma unroll
-                for (int u = 0; u < kRouteUnroll; ++u) {
-                    const uint32_t x = x0 + 32u * u + lane;
-                    if (x >= n_e) continue;
-                    uint32_t s = slot_t + d[u];
-                    if (s >= p.D) s -= p.D;
-                    unsigned long long base = kOverflow;
-                    uint32_t b = 0u, k_seg = 0u;
-                    if (d[u] == 1u) w[u] = 0;                   // already sent by the update kernel
-                    if (d[u] >= d_direct) {
-                        k_seg = 1u + ((d[u] - d_direct) >> p.q_log);
-                        b = g_cur + 1u + k_seg;
-                        if (b >= nb) b -= nb;
-                        base = s_base[b];
-                    }
-                    if (base == kOverflow) {
-                        if (w[u]) atomicAdd(p.ring + (size_t)s * p.Npad + m[u], w[u]);
-                    } else {
-                        const uint32_t cell = (s - (b << p.q_log)) * p.Npad + m[u];
-                        const unsigned long long pos = base + (unsigned long long)(long long)(s_adj[i][k_seg] + (int32_t)x);
-                        p.queue[(size_t)b * p.q_cap + pos] = make_uint2(cell, (uint32_t)w[u]);
-                    }
+                for (int w = 0; w < kRouteWarps; ++w) s_wbase[w][lane] += (uint32_t)got;
+            } else {                                      // bucket full: this CTA delivers these directly;
+                full = true;                              // neutralise what it reserved
+                uint2 *q = p.queue + (size_t)my_bucket * p.q_cap;
+                for (unsigned long long i = got; i < p.q_cap; ++i) q[i] = make_uint2(0u, 0u);
+            }
+        }
+        const uint32_t mask = __ballot_sync(0xFFFFFFFFu, full);
+        if (lane == 0) s_ovf = mask;
+    }
+    __syncthreads();
+    // C: records
+    const uint32_t ovf = s_ovf;
+    uint32_t run = s_wbase[warp][lane];
+    for (uint32_t idx = warp; idx < n; idx += kRouteWarps) {
+        const uint32_t src = s_list[idx];
+        const uint32_t e_beg = row[src], n_e = row[src + 1] - e_beg;
+        uint32_t lo, cnt;
+        route_segments(p, src, r, nb, n_e, lane, lo, cnt);
+        const uint32_t adj = run - lo;                     // record position - edge position, for segment `lane`
+        run += cnt;
+        for (uint32_t x0 = 0; x0 < n_e; x0 += 32u * kRouteUnroll) {
+            uint32_t d[kRouteUnroll], m[kRouteUnroll];
+            int32_t w[kRouteUnroll];
+#pragma unroll
+            for (int u = 0; u < kRouteUnroll; ++u) {       // all loads of the super-chunk first
+                const uint32_t x = x0 + 32u * u + lane;
+                d[u] = 0u; m[u] = 0u; w[u] = 0;
+                if (x < n_e) {
+                    d[u] = (uint32_t)__ldg(p.s_dly + e_beg + x);
+                    m[u] = __ldg(p.s_tgt + e_beg + x);
+                    w[u] = __ldg(p.s_wfx + e_beg + x);
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < kRouteUnroll; ++u) {
+                if (x0 + 32u * u >= n_e) break;            // warp-uniform
+                const uint32_t x = x0 + 32u * u + lane;
+                uint32_t s = slot_t + d[u];
+                if (s >= p.D) s -= p.D;
+                const bool queued = d[u] >= d_direct;      // false for the padding lanes too (d = 0)
+                const uint32_t k_seg = queued ? 1u + ((d[u] - d_direct) >> p.q_log) : 0u;
+                const uint32_t pos = __shfl_sync(0xFFFFFFFFu, adj, k_seg) + x;
+                if (x >= n_e || d[u] == 1u) continue;      // delay 1 was sent by the update kernel
+                if (!queued || ((ovf >> k_seg) & 1u)) {
+                    atomicAdd(p.ring + (size_t)s * p.Npad + m[u], w[u]);
+                } else {
+                    uint32_t b = g_cur + 1u + k_seg;
+                    if (b >= nb) b -= nb;
+                    const uint32_t cell = (s - (b << p.q_log)) * p.Npad + m[u];
+                    p.queue[(size_t)b * p.q_cap + pos] = make_uint2(cell, (uint32_t)w[u]);
                 }
             }
         }
-        __syncthreads();
     }
     if (lane == 0 && events) atomicAdd(&p.counters[2], events);
     if (threadIdx.x == 0) atomicAdd(&p.counters[1], (unsigned long long)n);
@@ -405,10 +410,18 @@ gn_fold_kernel(const GnDev p, const uint32_t bucket)
     const uint4 *q4 = reinterpret_cast<const uint4 *>(p.queue + (size_t)bucket * p.q_cap);
     const unsigned long long pairs = n >> 1;
     const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
-    for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < pairs; i += stride) {
-        const uint4 v = __ldcs(q4 + i);
-        if (v.y) atomicAdd(rows + v.x, (int32_t)v.y);
-        if (v.w) atomicAdd(rows + v.z, (int32_t)v.w);
+    for (unsigned long long i0 = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i0 < pairs; i0 += 4ull * stride) {
+        uint4 v[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {                       // four 16-byte loads in flight per thread
+            const unsigned long long i = i0 + (unsigned long long)u * stride;
+            v[u] = (i < pairs) ? __ldcs(q4 + i) : make_uint4(0u, 0u, 0u, 0u);
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            if (v[u].y) atomicAdd(rows + v[u].x, (int32_t)v[u].y);
+            if (v[u].w) atomicAdd(rows + v[u].z, (int32_t)v[u].w);
+        }
     }
     if ((n & 1ull) && blockIdx.x == 0 && threadIdx.x == 0) {
         const uint2 v = p.queue[(size_t)bucket * p.q_cap + n - 1];
@@ -660,7 +673,7 @@ cudaError_t gnk_deliver(const GnDev &p, uint64_t t, cudaStream_t st)
 
 cudaError_t gnk_route(const GnDev &p, uint64_t t, cudaStream_t st)
 {
-    const uint32_t w = chunk_words_for(p, 148u * 2u);            // two 512-thread CTAs per SM
+    const uint32_t w = chunk_words_for(p, 148u * 4u);            // four 256-thread CTAs per SM
     gn_route_kernel<<<ceil_div(p.words_pad, w), kRouteThreads, 0, st>>>(p, (uint32_t)(t % p.D),
                                                                       (uint32_t)(t % p.raster_rows), w);
     return cudaGetLastError();

@@ -128,7 +128,7 @@ QUEUE_CASES = [
     (4, 9_001, None, 2000, 500, 8, 0),        # the mode config 4 runs in: D=128, 16 buckets of 8 slots
     (4, 9_001, None, 1000, 1000, 8, 0),       # ring never read back (no flush) until the end
     (4, 5_003, None, 1200, 300, 16, 0),       # 8 buckets of 16 slots
-    (4, 5_003, None, 1200, 300, 1, 0),        # one bucket per slot: folded every step
+    (4, 5_003, None, 1200, 300, 4, 0),        # 32 buckets of 4 slots (one per lane of the routing warp)
     (4, 5_003, None, 1200, 300, 8, 4096),     # buckets overflow: the excess is delivered directly
     (4, 5_003, None, 600, 300, 4, 64),        # overflow on nearly every pass
     (3, 6_007, None, 1500, 500, 8, 0),        # D=64
@@ -148,11 +148,12 @@ def test_queue_mode_bit_exact(gn, k, n, nb, steps, chunk, group, cap):
 
 
 def test_queue_mode_ring_depth_not_a_multiple_of_the_group(gn):
-    """D = 37 with groups of 8: the last bucket holds 5 slots; explicit delays up to D-1."""
+    """D = 36 with groups of 8 asked for: the library settles on groups of 4 (9 buckets); explicit delays up
+    to D-1, so every segment including the wrapped one is exercised."""
     rng = np.random.default_rng(11)
     net, cfg = make_config(2, n=2_500)
-    cfg = dict(cfg, ring_slots=37, obs_stride=0)
-    delays = rng.integers(1, 37, size=net.n_edges).astype(np.uint8)
+    cfg = dict(cfg, ring_slots=36, obs_stride=0)
+    delays = rng.integers(1, 36, size=net.n_edges).astype(np.uint8)
     _, o, _ = _run_exact(gn, net, cfg, 900, 300, delays=delays, delivery_mode=gn.GN_DELIVER_QUEUE, queue_group=8)
     assert o.counters()["delivered"] > 0
 
