@@ -85,7 +85,11 @@ Layout make_layout(const gn_config *cfg)
     L.counters = take(32);
     const QueuePlan qp = make_plan(cfg);
     L.q_count = take(256 * 8);
-    L.raster = take((size_t)(cfg->raster_capacity_steps < 2 ? 2 : cfg->raster_capacity_steps) * (Npad / 32) * 4);
+    {
+        size_t rows = cfg->raster_capacity_steps, need_rows = qp.on ? (size_t)2 << qp.q_log : 2;
+        if (rows < need_rows) rows = need_rows;
+        L.raster = take(rows * (Npad / 32) * 4);
+    }
     L.trace = take(obs ? (size_t)cfg->trace_capacity_frames * Npad * 4 : 0);
     L.s_tgt = take(E * 4); L.s_wfx = take(E * 4); L.s_dly = take(E);   // every row again, sorted by delay
     L.q_seg = take(qp.on ? N * D * 2 : 0);
@@ -106,6 +110,7 @@ struct gn_net {
     cudaStream_t stream;
     uint8_t *ws;
     uint64_t t;          // steps enqueued so far
+    uint64_t routed_upto; // queue mode: steps < routed_upto have had their queued events routed
     // delivery of step t overlaps the update of step t+1 (see gn_step): side streams and their fences
     cudaStream_t s_deliver, s_fold;
     cudaEvent_t ev_update, ev_deliver[2], ev_fold;
@@ -194,6 +199,7 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
     net->stream = (cudaStream_t)cuda_stream;
     net->ws = (uint8_t *)workspace;
     net->t = 0;
+    net->routed_upto = 0;
     net->s_deliver = net->s_fold = nullptr;
     net->ev_update = net->ev_deliver[0] = net->ev_deliver[1] = net->ev_fold = nullptr;
     net->fences_pending = false;
@@ -229,8 +235,12 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
     d.wfx = (int32_t *)(ws + L.wfx); d.dly = ws + L.dly;
     d.counters = (unsigned long long *)(ws + L.counters);
     d.raster = (uint32_t *)(ws + L.raster);
-    d.raster_rows = cfg->raster_capacity_steps < 2 ? 2u : cfg->raster_capacity_steps;
     const QueuePlan qp = make_plan(cfg);
+    d.raster_rows = cfg->raster_capacity_steps;   // the delivery kernels read the spike lists of up to two groups
+    {
+        const uint32_t need_rows = qp.on ? 2u << qp.q_log : 2u;
+        if (d.raster_rows < need_rows) d.raster_rows = need_rows;
+    }
     d.queue_mode = qp.on ? 1u : 0u;
     d.q_log = qp.q_log; d.q_nb = qp.q_nb; d.q_cap = qp.q_cap;
     d.q_count = (unsigned long long *)(ws + L.q_count);
@@ -405,63 +415,76 @@ static int join_streams(gn_net *net)
     if (!net->fences_pending) return GN_OK;
     GN_CUDA(net, cudaStreamWaitEvent(net->stream, net->ev_deliver[0], 0));
     GN_CUDA(net, cudaStreamWaitEvent(net->stream, net->ev_deliver[1], 0));
-    GN_CUDA(net, cudaStreamWaitEvent(net->stream, net->ev_fold, 0));
     net->fences_pending = false;
     return GN_OK;
 }
 
-// One step t is   update(t)  ->  deliver(t)   [+ fold of the NEXT group's bucket at a group's first step].
-// Dependencies (everything else may overlap):
-//   update(t)   after update(t-1) and deliver(t-2): events with delay 1 are sent by update(t-1) itself, so the
-//               earliest slot deliver(t-1) writes is t+1;
-//   deliver(t)  after update(t) (it reads step t's raster row) and deliver(t-1) (same stream);
-//   fold(g+1)   at the first step of group g, after deliver(t-1) (the last one that appends to bucket g+1: while
-//               group g is consumed, events due in g or g+1 go straight to the ring); done (and the bucket's count
-//               zeroed) before the first step of group g+1.
+// Ring mode.  One step t is  update(t) -> deliver(t).  update(t) needs update(t-1) and deliver(t-2): events
+// with delay 1 are sent by update(t-1) itself, so the earliest slot deliver(t-1) writes is t+1, and deliver(t)
+// runs on a side stream beside update(t+1).
+//
+// Queue mode.  Steps come in groups of G = 2^q_log (one bucket = the ring rows of one group).  update(t) sends
+// every event due in the group being consumed or in the next one itself; the rest of a whole group's events
+// is routed into buckets by ONE gn_route_kernel launched after the group's last update, followed by the
+// fold of the bucket two groups ahead -- both on the side stream, beside the updates of the next group:
+//   route(group g)  after update(last step of g);
+//   fold(g+2)       after route(g)  (the last routing that appends to bucket g+2);
+//   update(first step of g+2)  after fold(g+2).
 // In profiling mode everything runs on the caller's stream in that order, so per-kernel times are clean.
+static int route_pending(gn_net *net, cudaStream_t st, bool prof)
+{
+    const GnDev &d = net->dev;
+    if (!d.queue_mode || net->routed_upto >= net->t) return GN_OK;
+    int rc;
+    if (prof && (rc = prof_mark(net, 1))) return rc;
+    GN_CUDA(net, gnk_route(d, net->routed_upto, (uint32_t)(net->t - net->routed_upto), st));
+    net->launches++;
+    net->routed_upto = net->t;
+    return GN_OK;
+}
+
 int gn_step(gn_net *net, uint64_t n_steps)
 {
     if (!net) return GN_E_INVALID_ARG;
     const GnDev &d = net->dev;
+    const uint32_t G = 1u << d.q_log;
     for (uint64_t s = 0; s < n_steps; ++s) {
         const uint64_t t = net->t;
         const bool prof = net->profile;
         cudaStream_t s_upd = net->stream;
         cudaStream_t s_del = prof ? net->stream : net->s_deliver;
-        cudaStream_t s_fld = prof ? net->stream : net->s_fold;
         int rc;
-        if (d.queue_mode) {
-            const uint32_t slot = (uint32_t)(t % d.D);
-            if ((slot & ((1u << d.q_log) - 1u)) == 0u) {
-                const uint32_t g_next = ((slot >> d.q_log) + 1u) % d.q_nb;
-                if (!prof) {
-                    GN_CUDA(net, cudaStreamWaitEvent(s_upd, net->ev_fold, 0));          // the fold of bucket g
-                    GN_CUDA(net, cudaEventRecord(net->ev_update, s_upd));               // everything the caller queued
-                    GN_CUDA(net, cudaStreamWaitEvent(s_fld, net->ev_update, 0));
-                    GN_CUDA(net, cudaStreamWaitEvent(s_fld, net->ev_deliver[(t + 1) & 1ull], 0));   // deliver(t-1)
-                }
-                if (prof && (rc = prof_mark(net, 3))) return rc;
-                GN_CUDA(net, gnk_fold(d, g_next, s_fld));
-                GN_CUDA(net, cudaMemsetAsync(d.q_count + g_next, 0, 8, s_fld));         // the bucket is empty again
-                net->launches++;
-                if (!prof) GN_CUDA(net, cudaEventRecord(net->ev_fold, s_fld));
+        if (!prof) {
+            if (d.queue_mode) {
+                if (t % G == 0) GN_CUDA(net, cudaStreamWaitEvent(s_upd, net->ev_deliver[(t / G) & 1ull], 0));   // fold of this group
+            } else if (t >= 2) {
+                GN_CUDA(net, cudaStreamWaitEvent(s_upd, net->ev_deliver[t & 1ull], 0));                          // deliver(t-2)
             }
         }
-        if (!prof && t >= 2) GN_CUDA(net, cudaStreamWaitEvent(s_upd, net->ev_deliver[t & 1ull], 0));   // deliver(t-2)
         if (prof && (rc = prof_mark(net, 0))) return rc;
         GN_CUDA(net, gnk_update(d, t, net->has_bias, s_upd));
         net->launches++;
-        if (!prof) {
+        net->t = t + 1;
+        const bool group_end = d.queue_mode && (t % G == G - 1u);
+        if (!prof && (!d.queue_mode || group_end)) {
             GN_CUDA(net, cudaEventRecord(net->ev_update, s_upd));
             GN_CUDA(net, cudaStreamWaitEvent(s_del, net->ev_update, 0));
         }
-        if (prof && (rc = prof_mark(net, 1))) return rc;      // also counts the step's spikes: runs even with E = 0
-        if (d.queue_mode) GN_CUDA(net, gnk_route(d, t, s_del));
-        else GN_CUDA(net, gnk_deliver(d, t, s_del));
-        net->launches++;
-        if (!prof) {
-            GN_CUDA(net, cudaEventRecord(net->ev_deliver[t & 1ull], s_del));
-            net->fences_pending = true;
+        if (!d.queue_mode) {
+            if (prof && (rc = prof_mark(net, 1))) return rc;  // also counts the step's spikes: runs even with E = 0
+            GN_CUDA(net, gnk_deliver(d, t, s_del));
+            net->launches++;
+            if (!prof) GN_CUDA(net, cudaEventRecord(net->ev_deliver[t & 1ull], s_del));
+            net->fences_pending = !prof;
+        } else if (group_end) {
+            if ((rc = route_pending(net, s_del, prof))) return rc;
+            const uint32_t g = (uint32_t)(t % d.D) >> d.q_log;
+            if (prof && (rc = prof_mark(net, 3))) return rc;
+            GN_CUDA(net, gnk_fold(d, (g + 2u) % d.q_nb, s_del));
+            GN_CUDA(net, cudaMemsetAsync(d.q_count + (g + 2u) % d.q_nb, 0, 8, s_del));   // the bucket is empty again
+            net->launches++;
+            if (!prof) GN_CUDA(net, cudaEventRecord(net->ev_deliver[(t / G) & 1ull], s_del));
+            net->fences_pending = !prof;
         }
         if (d.obs_stride && (t + 1) % d.obs_stride == 0) {
             if (prof && (rc = prof_mark(net, 2))) return rc;
@@ -469,11 +492,25 @@ int gn_step(gn_net *net, uint64_t n_steps)
             net->launches++;
         }
         if (prof && (rc = prof_mark(net, 0xFF))) return rc;
-        net->t = t + 1;
         if (prof && (s + 1) % kProfChunk == 0 && (rc = prof_collect(net))) return rc;
     }
     if (net->profile) return prof_collect(net);
     return join_streams(net);
+}
+
+// Spikes and delivered events are counted, and queued events become visible in the ring, only once the
+// routing of the steps since the last group boundary has run: readers of counters and ring call this.
+static int flush_delivery(gn_net *net, bool fold_too)
+{
+    const GnDev &d = net->dev;
+    int rc = join_streams(net);
+    if (rc) return rc;
+    if ((rc = route_pending(net, net->stream, false))) return rc;
+    if (fold_too && d.queue_mode) {   // pending records are deferred ring adds: apply them all (a no-op for the results)
+        for (uint32_t b = 0; b < d.q_nb; ++b) GN_CUDA(net, gnk_fold(d, b, net->stream));
+        GN_CUDA(net, cudaMemsetAsync(d.q_count, 0, (size_t)d.q_nb * 8, net->stream));
+    }
+    return GN_OK;
 }
 
 int gn_profile(gn_net *net, int enable)
@@ -526,7 +563,11 @@ int gn_read_state(gn_net *net, int which, void *dst, size_t dst_bytes, int dst_i
         src = d.bias; need = N * 4; break;
     case GN_RING: need = (size_t)d.D * N * 4; break;
     case GN_STEP: src = d.counters; need = 8; break;
-    case GN_COUNTERS: src = d.counters; need = 32; break;
+    case GN_COUNTERS: {
+        int rc = flush_delivery(net, false);
+        if (rc) return rc;
+        src = d.counters; need = 32; break;
+    }
     case GN_DELAYS: src = d.dly; need = E; break;
     case GN_WEIGHTS_FX: src = d.wfx; need = E * 4; break;
     default: return set_err(net, GN_E_INVALID_ARG, "unknown state id %d", which);
@@ -534,10 +575,8 @@ int gn_read_state(gn_net *net, int which, void *dst, size_t dst_bytes, int dst_i
     if (dst_bytes < need) return set_err(net, GN_E_INVALID_ARG, "dst has %zu bytes, need %zu", dst_bytes, need);
     if (need == 0) return GN_OK;
     if (which == GN_RING) {   // internal rows are Npad wide; the caller's are N wide
-        if (d.queue_mode) {   // pending records are deferred ring adds: apply them all (a no-op for the results)
-            for (uint32_t b = 0; b < d.q_nb; ++b) GN_CUDA(net, gnk_fold(d, b, net->stream));
-            GN_CUDA(net, cudaMemsetAsync(d.q_count, 0, (size_t)d.q_nb * 8, net->stream));
-        }
+        int rc = flush_delivery(net, true);
+        if (rc) return rc;
         GN_CUDA(net, cudaMemcpy2DAsync(dst, N * 4, d.ring, (size_t)d.Npad * 4, N * 4, d.D,
                                        dst_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, net->stream));
         if (!dst_is_device) GN_CUDA(net, cudaStreamSynchronize(net->stream));

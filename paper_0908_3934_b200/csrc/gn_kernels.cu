@@ -77,7 +77,8 @@ __device__ __forceinline__ bool vertex_step(const GnClassDev &q, const float dt,
 // Thread g owns vertices 4g .. 4g+3 (128-bit SoA loads); a warp owns 128 vertices = 4 raster words.
 template <bool OBS, bool BIAS>
 __global__ void __launch_bounds__(kUpdateThreads, 8)
-gn_update_kernel(const GnDev p, const uint64_t t, const uint32_t slot, const uint32_t raster_row)
+gn_update_kernel(const GnDev p, const uint64_t t, const uint32_t slot, const uint32_t raster_row,
+                 const uint32_t d_direct)
 {
     __shared__ GnClassDev s_cls[GN_MAX_CLASSES];
     if (threadIdx.x < p.n_classes * 13u)
@@ -155,19 +156,22 @@ gn_update_kernel(const GnDev p, const uint64_t t, const uint32_t slot, const uin
     word |= __shfl_xor_sync(0xFFFFFFFFu, word, 4);
     if ((lane & 7u) == 0u && j0 < p.Npad)
         p.raster[(size_t)raster_row * p.words_pad + (j0 >> 5)] = word;
-    // a4, the urgent part: an event with delay 1 is due in the very next step, so the vertex that fired sends
-    // it itself (rows are sorted by delay: such edges lead the row).  Everything else is delivered by the
-    // delivery kernel of this step, which may then overlap the NEXT step's update (gn_api.cu, gn_step).
+    // a4, the urgent part: events due before the delivery kernel of this step is guaranteed to have run are
+    // sent by the vertex that fired (rows are sorted by delay: such edges lead the row).  Ring mode: delay 1
+    // (d_direct = 2), so that deliver(t) may overlap update(t+1).  Queue mode: every delay that lands in the
+    // group being consumed or in the next one (d_direct = 2G - r), so that routing runs once per group.
     if (nib) {
-        uint32_t s1 = slot + 1u;
-        if (s1 >= p.D) s1 = 0u;
-        int32_t *next_row = p.ring + (size_t)s1 * p.Npad;
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
             if (!((nib >> q) & 1u)) continue;
             const uint32_t end = p.row[j0 + q + 1];
-            for (uint32_t e = p.row[j0 + q]; e < end && p.s_dly[e] == 1; ++e)
-                atomicAdd(next_row + p.s_tgt[e], p.s_wfx[e]);
+            for (uint32_t e = p.row[j0 + q]; e < end; ++e) {
+                const uint32_t d = p.s_dly[e];
+                if (d >= d_direct) break;
+                uint32_t s1 = slot + d;
+                if (s1 >= p.D) s1 -= p.D;
+                atomicAdd(p.ring + (size_t)s1 * p.Npad + p.s_tgt[e], p.s_wfx[e]);
+            }
         }
     }
     if (__any_sync(0xFFFFFFFFu, kicks != 0u)) {                           // rare: one atomic per warp with a kick
@@ -184,11 +188,11 @@ gn_update_kernel(const GnDev p, const uint64_t t, const uint32_t slot, const uin
 constexpr uint32_t kMaxChunkWords = 128;                 // 4096 vertices per CTA at most
 
 template <int THREADS>
-__device__ __forceinline__ uint32_t gather_sources(const uint32_t *__restrict__ raster_row, const uint32_t w0,
-                                                   const uint32_t n_words, uint32_t *s_list, uint32_t *s_wsum)
+__device__ __forceinline__ uint32_t gather_scan(const uint32_t *__restrict__ raster_row, const uint32_t w0,
+                                                const uint32_t n_words, uint32_t *s_wsum, uint32_t &word, uint32_t &off)
 {
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
-    uint32_t word = (threadIdx.x < n_words) ? raster_row[w0 + threadIdx.x] : 0u;
+    word = (threadIdx.x < n_words) ? raster_row[w0 + threadIdx.x] : 0u;
     const uint32_t pc = __popc(word);
     uint32_t incl = pc;
 #pragma unroll
@@ -196,21 +200,41 @@ __device__ __forceinline__ uint32_t gather_sources(const uint32_t *__restrict__ 
         const uint32_t v = __shfl_up_sync(0xFFFFFFFFu, incl, o);
         if (lane >= (uint32_t)o) incl += v;
     }
+    __syncthreads();                                       // s_wsum may still be read from the previous scan
     if (lane == 31u) s_wsum[warp] = incl;
     __syncthreads();
-    uint32_t off = incl - pc, total = 0u;
+    uint32_t total = 0u;
+    off = incl - pc;
 #pragma unroll
     for (int w = 0; w < THREADS / 32; ++w) {
         const uint32_t c = s_wsum[w];
         if ((uint32_t)w < warp) off += c;
         total += c;
     }
+    return total;                                          // CTA-uniform
+}
+
+// Append this thread's fired vertices to the list at base + off (and tag them with `step` when asked).
+__device__ __forceinline__ void gather_write(uint32_t word, const uint32_t w0, uint32_t pos, uint32_t *s_list,
+                                             uint8_t *s_step, const uint32_t step)
+{
     const uint32_t j_base = (w0 + threadIdx.x) << 5;
     while (word) {
         const uint32_t bit = (uint32_t)__ffs(word) - 1u;
-        s_list[off++] = j_base + bit;
+        s_list[pos] = j_base + bit;
+        if (s_step) s_step[pos] = (uint8_t)step;
+        ++pos;
         word &= word - 1u;
     }
+}
+
+template <int THREADS>
+__device__ __forceinline__ uint32_t gather_sources(const uint32_t *__restrict__ raster_row, const uint32_t w0,
+                                                   const uint32_t n_words, uint32_t *s_list, uint32_t *s_wsum)
+{
+    uint32_t word, off;
+    const uint32_t total = gather_scan<THREADS>(raster_row, w0, n_words, s_wsum, word, off);
+    gather_write(word, w0, off, s_list, nullptr, 0u);
     __syncthreads();
     return total;
 }
@@ -293,35 +317,27 @@ __device__ __forceinline__ void route_segments(const GnDev &p, const uint32_t sr
     cnt = (lane >= 1u && lane < nb) ? hi - lo : 0u;
 }
 
-__global__ void __launch_bounds__(kRouteThreads, 4)
-gn_route_kernel(const GnDev p, const uint32_t slot_t, const uint32_t raster_row, const uint32_t chunk_words)
+constexpr uint32_t kRouteListCap = 4096;                // sources one A/B/C round of a CTA handles
+
+// Phases A, B, C over the n sources in s_list (each tagged with its step inside the group).
+__device__ __forceinline__ void route_round(const GnDev &p, const uint32_t n, const uint32_t slot0, const uint32_t *s_list,
+                                            const uint8_t *s_step, uint32_t (*s_wtot)[32], uint32_t (*s_wbase)[32],
+                                            uint32_t *s_ovf, unsigned long long &events)
 {
-    __shared__ uint32_t s_list[kMaxChunkWords * 32];
-    __shared__ uint32_t s_wsum[kRouteWarps];
-    __shared__ uint32_t s_wtot[kRouteWarps][32];         // A: records of warp w in segment k
-    __shared__ uint32_t s_wbase[kRouteWarps][32];        // B: where warp w's records of segment k start in the bucket
-    __shared__ uint32_t s_ovf;                           // B: bit k = segment k's bucket is full
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
-    const uint32_t w0 = blockIdx.x * chunk_words;
-    const uint32_t n_words = min(chunk_words, p.words_pad - w0);
-    const uint32_t n = gather_sources<kRouteThreads>(p.raster + (size_t)raster_row * p.words_pad, w0, n_words,
-                                                     s_list, s_wsum);
-    if (n == 0u) return;
     const uint32_t *__restrict__ row = p.row;
     const uint32_t nb = p.q_nb, G = 1u << p.q_log;
-    const uint32_t g_cur = slot_t >> p.q_log, r = slot_t & (G - 1u);
-    const uint32_t d_direct = 2u * G - r;                  // delays below this are segment 0
+    const uint32_t g_cur = slot0 >> p.q_log, r0 = slot0 & (G - 1u);
     uint32_t my_bucket = g_cur + 1u + lane;               // bucket of the segment this lane owns
     while (my_bucket >= nb) my_bucket -= nb;
 
     // A: per-warp, per-segment record counts
     uint32_t tot = 0u;
-    unsigned long long events = 0ull;
     for (uint32_t idx = warp; idx < n; idx += kRouteWarps) {
         const uint32_t src = s_list[idx];
         const uint32_t deg = row[src + 1] - row[src];
         uint32_t lo, cnt;
-        route_segments(p, src, r, nb, deg, lane, lo, cnt);
+        route_segments(p, src, r0 + s_step[idx], nb, deg, lane, lo, cnt);
         tot += cnt;
         events += (unsigned long long)deg;
     }
@@ -349,20 +365,24 @@ gn_route_kernel(const GnDev p, const uint32_t slot_t, const uint32_t raster_row,
             }
         }
         const uint32_t mask = __ballot_sync(0xFFFFFFFFu, full);
-        if (lane == 0) s_ovf = mask;
+        if (lane == 0) *s_ovf = mask;
     }
     __syncthreads();
     // C: records
-    const uint32_t ovf = s_ovf;
+    const uint32_t ovf = *s_ovf;
     uint32_t run = s_wbase[warp][lane];
     for (uint32_t idx = warp; idx < n; idx += kRouteWarps) {
         const uint32_t src = s_list[idx];
+        const uint32_t step = s_step[idx];
+        const uint32_t slot_t = slot0 + step;              // same group: no wrap
+        const uint32_t d_direct = 2u * G - (r0 + step);    // delays below this were sent by the update kernel
         const uint32_t e_beg = row[src], n_e = row[src + 1] - e_beg;
         uint32_t lo, cnt;
-        route_segments(p, src, r, nb, n_e, lane, lo, cnt);
+        route_segments(p, src, r0 + step, nb, n_e, lane, lo, cnt);
         const uint32_t adj = run - lo;                     // record position - edge position, for segment `lane`
         run += cnt;
-        for (uint32_t x0 = 0; x0 < n_e; x0 += 32u * kRouteUnroll) {
+        const uint32_t x_first = __shfl_sync(0xFFFFFFFFu, lo, 1) & ~31u;   // segment 0 needs no visit
+        for (uint32_t x0 = x_first; x0 < n_e; x0 += 32u * kRouteUnroll) {
             uint32_t d[kRouteUnroll], m[kRouteUnroll];
             int32_t w[kRouteUnroll];
 #pragma unroll
@@ -384,8 +404,8 @@ gn_route_kernel(const GnDev p, const uint32_t slot_t, const uint32_t raster_row,
                 const bool queued = d[u] >= d_direct;      // false for the padding lanes too (d = 0)
                 const uint32_t k_seg = queued ? 1u + ((d[u] - d_direct) >> p.q_log) : 0u;
                 const uint32_t pos = __shfl_sync(0xFFFFFFFFu, adj, k_seg) + x;
-                if (x >= n_e || d[u] == 1u) continue;      // delay 1 was sent by the update kernel
-                if (!queued || ((ovf >> k_seg) & 1u)) {
+                if (!queued) continue;
+                if ((ovf >> k_seg) & 1u) {
                     atomicAdd(p.ring + (size_t)s * p.Npad + m[u], w[u]);
                 } else {
                     uint32_t b = g_cur + 1u + k_seg;
@@ -396,8 +416,43 @@ gn_route_kernel(const GnDev p, const uint32_t slot_t, const uint32_t raster_row,
             }
         }
     }
-    if (lane == 0 && events) atomicAdd(&p.counters[2], events);
-    if (threadIdx.x == 0) atomicAdd(&p.counters[1], (unsigned long long)n);
+    __syncthreads();
+}
+
+// Routes the queued segments of every vertex that fired in steps t0 .. t0+n_batch-1, all inside ONE slot
+// group (slot0 = t0 mod D): one launch per group amortises the launch and the dependent memory round trips
+// over 2^q_log steps of work.  raster row of step t0+i is (row0 + i) mod raster_rows.
+__global__ void __launch_bounds__(kRouteThreads, 4)
+gn_route_kernel(const GnDev p, const uint32_t slot0, const uint32_t row0, const uint32_t n_batch,
+                const uint32_t chunk_words)
+{
+    __shared__ uint32_t s_list[kRouteListCap];
+    __shared__ uint8_t s_step[kRouteListCap];
+    __shared__ uint32_t s_wsum[kRouteWarps];
+    __shared__ uint32_t s_wtot[kRouteWarps][32];         // A: records of warp w in segment k
+    __shared__ uint32_t s_wbase[kRouteWarps][32];        // B: where warp w's records of segment k start in the bucket
+    __shared__ uint32_t s_ovf;                           // B: bit k = segment k's bucket is full
+    const uint32_t w0 = blockIdx.x * chunk_words;
+    const uint32_t n_words = min(chunk_words, p.words_pad - w0);
+    unsigned long long events = 0ull;
+    uint32_t n = 0u, spikes = 0u;
+    for (uint32_t i = 0; i < n_batch; ++i) {
+        uint32_t rr = row0 + i;
+        if (rr >= p.raster_rows) rr -= p.raster_rows;
+        uint32_t word, off;
+        const uint32_t total = gather_scan<kRouteThreads>(p.raster + (size_t)rr * p.words_pad, w0, n_words, s_wsum, word, off);
+        if (n + total > kRouteListCap) {                    // CTA-uniform: the list is full, work it off first
+            route_round(p, n, slot0, s_list, s_step, s_wtot, s_wbase, &s_ovf, events);
+            n = 0u;
+        }
+        gather_write(word, w0, n + off, s_list, s_step, i);
+        n += total;
+        spikes += total;
+    }
+    __syncthreads();
+    if (n) route_round(p, n, slot0, s_list, s_step, s_wtot, s_wbase, &s_ovf, events);
+    if ((threadIdx.x & 31u) == 0 && events) atomicAdd(&p.counters[2], events);
+    if (threadIdx.x == 0 && spikes) atomicAdd(&p.counters[1], (unsigned long long)spikes);
 }
 
 // ---- a4, queue mode: fold one bucket into its ring rows --------------------------------------------------
@@ -643,14 +698,16 @@ inline uint32_t ceil_div(uint64_t a, uint64_t b) { return (uint32_t)((a + b - 1)
 // ---- launchers ------------------------------------------------------------------------------------------
 cudaError_t gnk_update(const GnDev &p, uint64_t t, bool has_bias, cudaStream_t st)
 {
+    // delays below d_direct are delivered by the update kernel itself (see the kernel)
+    const uint32_t d_direct = p.queue_mode ? 2u * (1u << p.q_log) - ((uint32_t)(t % p.D) & ((1u << p.q_log) - 1u)) : 2u;
     const uint32_t grid = ceil_div(p.Npad / kVertsPerThread, kUpdateThreads);
     const uint32_t slot = (uint32_t)(t % p.D);
     const uint32_t raster_row = (uint32_t)(t % p.raster_rows);
     const bool obs = p.obs_stride != 0u;
-    if (obs && has_bias) gn_update_kernel<true, true><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, raster_row);
-    else if (obs) gn_update_kernel<true, false><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, raster_row);
-    else if (has_bias) gn_update_kernel<false, true><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, raster_row);
-    else gn_update_kernel<false, false><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, raster_row);
+    if (obs && has_bias) gn_update_kernel<true, true><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, raster_row, d_direct);
+    else if (obs) gn_update_kernel<true, false><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, raster_row, d_direct);
+    else if (has_bias) gn_update_kernel<false, true><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, raster_row, d_direct);
+    else gn_update_kernel<false, false><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, raster_row, d_direct);
     return cudaGetLastError();
 }
 
@@ -671,11 +728,11 @@ cudaError_t gnk_deliver(const GnDev &p, uint64_t t, cudaStream_t st)
     return cudaGetLastError();
 }
 
-cudaError_t gnk_route(const GnDev &p, uint64_t t, cudaStream_t st)
+cudaError_t gnk_route(const GnDev &p, uint64_t t0, uint32_t n_batch, cudaStream_t st)
 {
     const uint32_t w = chunk_words_for(p, 148u * 4u);            // four 256-thread CTAs per SM
-    gn_route_kernel<<<ceil_div(p.words_pad, w), kRouteThreads, 0, st>>>(p, (uint32_t)(t % p.D),
-                                                                      (uint32_t)(t % p.raster_rows), w);
+    gn_route_kernel<<<ceil_div(p.words_pad, w), kRouteThreads, 0, st>>>(p, (uint32_t)(t0 % p.D),
+                                                                      (uint32_t)(t0 % p.raster_rows), n_batch, w);
     return cudaGetLastError();
 }
 
