@@ -17,7 +17,7 @@ thread_local char g_create_error[256] = "";
 
 struct Layout {
     size_t V, W, r, c, acc, bias, refr, cls, ring, row, tgt, wfx, dly, counters, q_count;
-    size_t s_tgt, s_wfx, s_dly, q_seg, queue;
+    size_t s_edge, s_dly, q_seg, queue;
     size_t raster, trace, scratch_row64, scratch_abs, scratch_pos, scratch_net, scratch_chk, total;
 };
 
@@ -42,6 +42,9 @@ int check_config(const gn_config *cfg, char *err, size_t errn)
     return GN_OK;
 }
 
+// Groups beyond the current one whose events the update kernel delivers itself (GnDev::q_window).
+static const uint32_t kQueueWindow = 1u;
+
 // Resolved delivery plan: mode, log2(slots per bucket), buckets, records per bucket.
 struct QueuePlan {
     bool on;
@@ -65,7 +68,9 @@ QueuePlan make_plan(const gn_config *cfg)
     uint64_t cap = cfg->queue_capacity ? cfg->queue_capacity : (uint64_t)group * ((E + 15) / 16);
     if (cap < 64) cap = 64;
     if (cap > 0xFFFFFF00ull) cap = 0xFFFFFF00ull;    // record positions are 32-bit
-    q.q_cap = (cap + 31) / 32 * 32;
+    if (cap * q.q_nb > 0xFFFFFF00ull) cap = 0xFFFFFF00ull / q.q_nb;     // record indices are 32-bit
+    q.q_cap = cap / 32 * 32;
+    if (q.q_cap < 32) q.q_cap = 32;
     return q;
 }
 
@@ -86,12 +91,12 @@ Layout make_layout(const gn_config *cfg)
     const QueuePlan qp = make_plan(cfg);
     L.q_count = take(256 * 8);
     {
-        size_t rows = cfg->raster_capacity_steps, need_rows = qp.on ? (size_t)2 << qp.q_log : 2;
+        size_t rows = cfg->raster_capacity_steps, need_rows = qp.on ? (size_t)(kQueueWindow + 1u) << qp.q_log : 2;
         if (rows < need_rows) rows = need_rows;
         L.raster = take(rows * (Npad / 32) * 4);
     }
     L.trace = take(obs ? (size_t)cfg->trace_capacity_frames * Npad * 4 : 0);
-    L.s_tgt = take(E * 4); L.s_wfx = take(E * 4); L.s_dly = take(E);   // every row again, sorted by delay
+    L.s_edge = take(E * 8); L.s_dly = take(E);   // every row again, sorted by delay
     L.q_seg = take(qp.on ? N * D * 2 : 0);
     L.queue = take(qp.on ? (size_t)qp.q_nb * qp.q_cap * 8 : 0);
     L.scratch_row64 = take((N + 1) * 8); L.scratch_abs = take(N * 8);
@@ -113,7 +118,7 @@ struct gn_net {
     uint64_t routed_upto; // queue mode: steps < routed_upto have had their queued events routed
     // delivery of step t overlaps the update of step t+1 (see gn_step): side streams and their fences
     cudaStream_t s_deliver, s_fold;
-    cudaEvent_t ev_update, ev_deliver[2], ev_fold;
+    cudaEvent_t ev_update, ev_deliver[2], ev_fold[4];
     bool fences_pending;
     bool has_bias;
     // measuring mode (gn_profile)
@@ -201,7 +206,7 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
     net->t = 0;
     net->routed_upto = 0;
     net->s_deliver = net->s_fold = nullptr;
-    net->ev_update = net->ev_deliver[0] = net->ev_deliver[1] = net->ev_fold = nullptr;
+    net->ev_update = net->ev_deliver[0] = net->ev_deliver[1] = net->ev_fold[0] = net->ev_fold[1] = net->ev_fold[2] = net->ev_fold[3] = nullptr;
     net->fences_pending = false;
     net->has_bias = bias != nullptr;
     net->profile = false;
@@ -238,13 +243,15 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
     const QueuePlan qp = make_plan(cfg);
     d.raster_rows = cfg->raster_capacity_steps;   // the delivery kernels read the spike lists of up to two groups
     {
-        const uint32_t need_rows = qp.on ? 2u << qp.q_log : 2u;
+        const uint32_t need_rows = qp.on ? (kQueueWindow + 1u) << qp.q_log : 2u;
         if (d.raster_rows < need_rows) d.raster_rows = need_rows;
     }
     d.queue_mode = qp.on ? 1u : 0u;
     d.q_log = qp.q_log; d.q_nb = qp.q_nb; d.q_cap = qp.q_cap;
     d.q_count = (unsigned long long *)(ws + L.q_count);
-    d.s_tgt = (uint32_t *)(ws + L.s_tgt); d.s_wfx = (int32_t *)(ws + L.s_wfx); d.s_dly = ws + L.s_dly;
+    d.s_edge = (uint2 *)(ws + L.s_edge); d.s_dly = ws + L.s_dly;
+    d.packed = Npad <= (1u << 24) ? 1u : 0u;
+    d.q_window = kQueueWindow;
     if (qp.on) {
         d.q_seg = (uint16_t *)(ws + L.q_seg);
         d.queue = (uint2 *)(ws + L.queue);
@@ -292,7 +299,7 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
 
     // zero everything the step loop accumulates into or reads before writing
     GN_CREATE_CUDA(cudaMemsetAsync(ws, 0, L.tgt, st));                       // state, bias, refr, cls, ring, row
-    GN_CREATE_CUDA(cudaMemsetAsync(ws + L.counters, 0, L.s_tgt - L.counters, st));   // counters, bucket counts, raster, trace
+    GN_CREATE_CUDA(cudaMemsetAsync(ws + L.counters, 0, L.s_edge - L.counters, st));   // counters, bucket counts, raster, trace
     GN_CREATE_CUDA(cudaMemsetAsync(abs_in, 0, (size_t)N * 8, st));
     GN_CREATE_CUDA(cudaMemsetAsync(chk_d, 0, sizeof(GnCheck), st));
     // uploads (host or device sources)
@@ -365,8 +372,9 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
         cudaError_t e = cudaDeviceGetStreamPriorityRange(&lo, &hi);
         if (e == cudaSuccess) e = cudaStreamCreateWithPriority(&net->s_deliver, cudaStreamNonBlocking, hi);
         if (e == cudaSuccess) e = cudaStreamCreateWithPriority(&net->s_fold, cudaStreamNonBlocking, lo);
-        cudaEvent_t *evs[4] = {&net->ev_update, &net->ev_deliver[0], &net->ev_deliver[1], &net->ev_fold};
-        for (int k = 0; k < 4 && e == cudaSuccess; ++k) e = cudaEventCreateWithFlags(evs[k], cudaEventDisableTiming);
+        cudaEvent_t *evs[7] = {&net->ev_update, &net->ev_deliver[0], &net->ev_deliver[1], &net->ev_fold[0], &net->ev_fold[1],
+                               &net->ev_fold[2], &net->ev_fold[3]};
+        for (int k = 0; k < 7 && e == cudaSuccess; ++k) e = cudaEventCreateWithFlags(evs[k], cudaEventDisableTiming);
         if (e != cudaSuccess) {
             gn_destroy(net);
             return set_err(nullptr, GN_E_CUDA, "creating side streams failed: %s", cudaGetErrorString(e));
@@ -415,6 +423,7 @@ static int join_streams(gn_net *net)
     if (!net->fences_pending) return GN_OK;
     GN_CUDA(net, cudaStreamWaitEvent(net->stream, net->ev_deliver[0], 0));
     GN_CUDA(net, cudaStreamWaitEvent(net->stream, net->ev_deliver[1], 0));
+    for (int k = 0; k < 4; ++k) GN_CUDA(net, cudaStreamWaitEvent(net->stream, net->ev_fold[k], 0));
     net->fences_pending = false;
     return GN_OK;
 }
@@ -424,12 +433,12 @@ static int join_streams(gn_net *net)
 // runs on a side stream beside update(t+1).
 //
 // Queue mode.  Steps come in groups of G = 2^q_log (one bucket = the ring rows of one group).  update(t) sends
-// every event due in the group being consumed or in the next one itself; the rest of a whole group's events
-// is routed into buckets by ONE gn_route_kernel launched after the group's last update, followed by the
-// fold of the bucket two groups ahead -- both on the side stream, beside the updates of the next group:
-//   route(group g)  after update(last step of g);
-//   fold(g+2)       after route(g)  (the last routing that appends to bucket g+2);
-//   update(first step of g+2)  after fold(g+2).
+// every event due in the group being consumed or in the next W = q_window groups itself; the rest of a whole
+// group's events is routed into buckets by ONE gn_route_kernel launched after the group's last update,
+// followed by the fold of the bucket W+1 groups ahead -- both on the side stream, beside later updates:
+//   route(group g)  after update(last step of g); appends to buckets g+W+1 .. and (wrapped) g;
+//   fold(g+W+1)     after route(g), the last routing that appends to that bucket;
+//   update(first step of g+W+1)  after fold(g+W+1): W groups of slack.
 // In profiling mode everything runs on the caller's stream in that order, so per-kernel times are clean.
 static int route_pending(gn_net *net, cudaStream_t st, bool prof)
 {
@@ -456,7 +465,7 @@ int gn_step(gn_net *net, uint64_t n_steps)
         int rc;
         if (!prof) {
             if (d.queue_mode) {
-                if (t % G == 0) GN_CUDA(net, cudaStreamWaitEvent(s_upd, net->ev_deliver[(t / G) & 1ull], 0));   // fold of this group
+                if (t % G == 0) GN_CUDA(net, cudaStreamWaitEvent(s_upd, net->ev_fold[(t / G) & 3ull], 0));   // fold of this group
             } else if (t >= 2) {
                 GN_CUDA(net, cudaStreamWaitEvent(s_upd, net->ev_deliver[t & 1ull], 0));                          // deliver(t-2)
             }
@@ -478,12 +487,12 @@ int gn_step(gn_net *net, uint64_t n_steps)
             net->fences_pending = !prof;
         } else if (group_end) {
             if ((rc = route_pending(net, s_del, prof))) return rc;
-            const uint32_t g = (uint32_t)(t % d.D) >> d.q_log;
+            const uint32_t b_fold = (((uint32_t)(t % d.D) >> d.q_log) + d.q_window + 1u) % d.q_nb;
             if (prof && (rc = prof_mark(net, 3))) return rc;
-            GN_CUDA(net, gnk_fold(d, (g + 2u) % d.q_nb, s_del));
-            GN_CUDA(net, cudaMemsetAsync(d.q_count + (g + 2u) % d.q_nb, 0, 8, s_del));   // the bucket is empty again
+            GN_CUDA(net, gnk_fold(d, b_fold, s_del));
+            GN_CUDA(net, cudaMemsetAsync(d.q_count + b_fold, 0, 8, s_del));             // the bucket is empty again
             net->launches++;
-            if (!prof) GN_CUDA(net, cudaEventRecord(net->ev_deliver[(t / G) & 1ull], s_del));
+            if (!prof) GN_CUDA(net, cudaEventRecord(net->ev_fold[(t / G + d.q_window + 1u) & 3ull], s_del));
             net->fences_pending = !prof;
         }
         if (d.obs_stride && (t + 1) % d.obs_stride == 0) {
@@ -675,7 +684,7 @@ int gn_destroy(gn_net *net)
     if (net->s_fold) cudaStreamSynchronize(net->s_fold);
     cudaError_t e = cudaStreamSynchronize(net->stream);
     for (cudaEvent_t ev : net->ev) cudaEventDestroy(ev);
-    cudaEvent_t evs[4] = {net->ev_update, net->ev_deliver[0], net->ev_deliver[1], net->ev_fold};
+    cudaEvent_t evs[7] = {net->ev_update, net->ev_deliver[0], net->ev_deliver[1], net->ev_fold[0], net->ev_fold[1], net->ev_fold[2], net->ev_fold[3]};
     for (cudaEvent_t ev : evs) if (ev) cudaEventDestroy(ev);
     if (net->s_deliver) cudaStreamDestroy(net->s_deliver);
     if (net->s_fold) cudaStreamDestroy(net->s_fold);

@@ -45,9 +45,11 @@ struct GnDev {
     // 2^q_log ring slots
     uint32_t queue_mode;     // 0 ring, 1 queue
     uint32_t q_log, q_nb;    // slots per bucket = 1 << q_log; buckets = ceil(D / 2^q_log)
-    uint32_t *s_tgt;         // [E] the CSR rows again, each sorted by delay
-    int32_t *s_wfx;          // [E]
-    uint8_t *s_dly;          // [E]
+    uint2 *s_edge;           // [E] the CSR rows again, each sorted by delay: {target, w_fx}; when `packed`
+                             //     (Npad <= 2^24) the delay also sits in the target word's top byte
+    uint8_t *s_dly;          // [E] delay of s_edge[e]
+    uint32_t packed;
+    uint32_t q_window;       // queue mode: groups ahead of the current one whose events the update kernel sends itself
     uint16_t *q_seg;         // [N][2^q_log][q_nb] segment boundaries of every delay-sorted row (gn_route_kernel)
     uint2 *queue;            // [q_nb][q_cap] records {cell offset inside the bucket's ring rows, w_fx}
     unsigned long long q_cap;

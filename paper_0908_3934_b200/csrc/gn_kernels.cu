@@ -170,7 +170,8 @@ gn_update_kernel(const GnDev p, const uint64_t t, const uint32_t slot, const uin
                 if (d >= d_direct) break;
                 uint32_t s1 = slot + d;
                 if (s1 >= p.D) s1 -= p.D;
-                atomicAdd(p.ring + (size_t)s1 * p.Npad + p.s_tgt[e], p.s_wfx[e]);
+                const uint2 ev = p.s_edge[e];
+                atomicAdd(p.ring + (size_t)s1 * p.Npad + (p.packed ? ev.x & 0xFFFFFFu : ev.x), (int32_t)ev.y);
             }
         }
     }
@@ -255,20 +256,19 @@ gn_deliver_kernel(const GnDev p, const uint32_t slot_t, const uint32_t raster_ro
                                                        s_list, s_wsum);
     if (n == 0u) return;
     const uint32_t *__restrict__ row = p.row;
-    const uint32_t *__restrict__ tgt = p.s_tgt;
-    const int32_t *__restrict__ wfx = p.s_wfx;
+    const uint2 *__restrict__ edge = p.s_edge;
     const uint8_t *__restrict__ dly = p.s_dly;
     unsigned long long events = 0ull;
     for (uint32_t idx = warp; idx < n; idx += kDeliverThreads / 32) {
         const uint32_t src = s_list[idx];
         const uint32_t beg = row[src], end = row[src + 1];
         for (uint32_t e = beg + lane; e < end; e += 32u) {
-            const uint32_t m = tgt[e];
-            const int32_t w = wfx[e];
+            const uint2 ev = edge[e];
             const uint32_t d = dly[e];
             uint32_t s = slot_t + d;
             if (s >= p.D) s -= p.D;
-            if (d != 1u) atomicAdd(p.ring + (size_t)s * p.Npad + m, w);   // delay 1 was sent by the update kernel
+            if (d != 1u)                                                   // delay 1 was sent by the update kernel
+                atomicAdd(p.ring + (size_t)s * p.Npad + (p.packed ? ev.x & 0xFFFFFFu : ev.x), (int32_t)ev.y);
         }
         events += (unsigned long long)(end - beg);
     }
@@ -305,30 +305,33 @@ constexpr int kRouteThreads = 256;
 constexpr int kRouteWarps = kRouteThreads / 32;
 constexpr int kRouteUnroll = 8;                         // 8 x 32 edges of a row in flight per warp
 
-// Lane k: boundaries of segment k of `src` at alignment r -> lo (start position) and cnt (size); 0 for lanes
-// that own no queued segment (k = 0 or k >= nb).
+// Lane k owns the events due j = k + W groups after the current one (W = q_window groups are the update
+// kernel's; k = 1 .. nb-W): boundaries of that segment of `src` at alignment r -> lo (start position) and cnt.
 __device__ __forceinline__ void route_segments(const GnDev &p, const uint32_t src, const uint32_t r, const uint32_t nb,
                                                const uint32_t deg, const uint32_t lane, uint32_t &lo, uint32_t &cnt)
 {
     const uint16_t *seg = p.q_seg + ((size_t)src << p.q_log) * nb + (size_t)r * nb;
-    lo = (lane < nb) ? (uint32_t)__ldg(seg + lane) : deg;
+    const uint32_t i = lane + p.q_window - 1u;             // table entry i = #edges with delay < (i+1)G - r
+    lo = (i < nb) ? (uint32_t)__ldg(seg + i) : deg;
     uint32_t hi = __shfl_down_sync(0xFFFFFFFFu, lo, 1);
-    if (lane + 1u >= nb) hi = deg;
-    cnt = (lane >= 1u && lane < nb) ? hi - lo : 0u;
+    if (i + 1u >= nb || lane == 31u) hi = deg;
+    cnt = (lane >= 1u && i < nb) ? hi - lo : 0u;
 }
 
 constexpr uint32_t kRouteListCap = 4096;                // sources one A/B/C round of a CTA handles
 
 // Phases A, B, C over the n sources in s_list (each tagged with its step inside the group).
+template <bool PACKED>
 __device__ __forceinline__ void route_round(const GnDev &p, const uint32_t n, const uint32_t slot0, const uint32_t *s_list,
                                             const uint8_t *s_step, uint32_t (*s_wtot)[32], uint32_t (*s_wbase)[32],
                                             uint32_t *s_ovf, unsigned long long &events)
 {
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     const uint32_t *__restrict__ row = p.row;
-    const uint32_t nb = p.q_nb, G = 1u << p.q_log;
-    const uint32_t g_cur = slot0 >> p.q_log, r0 = slot0 & (G - 1u);
-    uint32_t my_bucket = g_cur + 1u + lane;               // bucket of the segment this lane owns
+    const uint32_t nb = p.q_nb, G = 1u << p.q_log, Gm1 = G - 1u;
+    const uint32_t g_cur = slot0 >> p.q_log, r0 = slot0 & Gm1;
+    const uint32_t rd_queued = (p.q_window + 1u) << p.q_log;   // r + delay at or above this: queued
+    uint32_t my_bucket = g_cur + p.q_window + lane;        // bucket of the segment this lane owns
     while (my_bucket >= nb) my_bucket -= nb;
 
     // A: per-warp, per-segment record counts
@@ -343,7 +346,8 @@ __device__ __forceinline__ void route_round(const GnDev &p, const uint32_t n, co
     }
     s_wtot[warp][lane] = tot;
     __syncthreads();
-    // B: reserve
+    // B: reserve; afterwards s_wbase[w][k] = index (in records, over the whole queue) of warp w's first record
+    // of segment k
     if (warp == 0) {
         uint32_t run = 0u;
 #pragma unroll
@@ -356,8 +360,9 @@ __device__ __forceinline__ void route_round(const GnDev &p, const uint32_t n, co
         if (run) {
             const unsigned long long got = atomicAdd(&p.q_count[my_bucket], (unsigned long long)run);
             if (got + run <= p.q_cap) {
+                const uint32_t first = (uint32_t)((unsigned long long)my_bucket * p.q_cap + got);
 #pragma unroll
-                for (int w = 0; w < kRouteWarps; ++w) s_wbase[w][lane] += (uint32_t)got;
+                for (int w = 0; w < kRouteWarps; ++w) s_wbase[w][lane] += first;
             } else {                                      // bucket full: this CTA delivers these directly;
                 full = true;                              // neutralise what it reserved
                 uint2 *q = p.queue + (size_t)my_bucket * p.q_cap;
@@ -368,50 +373,51 @@ __device__ __forceinline__ void route_round(const GnDev &p, const uint32_t n, co
         if (lane == 0) *s_ovf = mask;
     }
     __syncthreads();
-    // C: records
+    // C: records.  With rd = r + delay: queued iff rd >= (W+1)G; group offset j = rd >> q_log, owned by lane
+    // j - W; ring row inside the bucket = rd & (G-1).
     const uint32_t ovf = *s_ovf;
     uint32_t run = s_wbase[warp][lane];
     for (uint32_t idx = warp; idx < n; idx += kRouteWarps) {
         const uint32_t src = s_list[idx];
-        const uint32_t step = s_step[idx];
-        const uint32_t slot_t = slot0 + step;              // same group: no wrap
-        const uint32_t d_direct = 2u * G - (r0 + step);    // delays below this were sent by the update kernel
+        const uint32_t r = r0 + s_step[idx];
         const uint32_t e_beg = row[src], n_e = row[src + 1] - e_beg;
         uint32_t lo, cnt;
-        route_segments(p, src, r0 + step, nb, n_e, lane, lo, cnt);
-        const uint32_t adj = run - lo;                     // record position - edge position, for segment `lane`
+        route_segments(p, src, r, nb, n_e, lane, lo, cnt);
+        const uint32_t adj = run - lo;                     // record index - edge position, for this lane's segment
         run += cnt;
-        const uint32_t x_first = __shfl_sync(0xFFFFFFFFu, lo, 1) & ~31u;   // segment 0 needs no visit
+        const uint32_t x_first = __shfl_sync(0xFFFFFFFFu, lo, 1) & ~31u;   // the update kernel's edges need no visit
+        const uint2 *__restrict__ edge = p.s_edge + e_beg;
+        const uint8_t *__restrict__ dly = p.s_dly + e_beg;
         for (uint32_t x0 = x_first; x0 < n_e; x0 += 32u * kRouteUnroll) {
-            uint32_t d[kRouteUnroll], m[kRouteUnroll];
-            int32_t w[kRouteUnroll];
+            uint2 ev[kRouteUnroll];
+            uint32_t d[kRouteUnroll];
 #pragma unroll
             for (int u = 0; u < kRouteUnroll; ++u) {       // all loads of the super-chunk first
                 const uint32_t x = x0 + 32u * u + lane;
-                d[u] = 0u; m[u] = 0u; w[u] = 0;
+                ev[u] = make_uint2(0u, 0u);
+                d[u] = 0u;
                 if (x < n_e) {
-                    d[u] = (uint32_t)__ldg(p.s_dly + e_beg + x);
-                    m[u] = __ldg(p.s_tgt + e_beg + x);
-                    w[u] = __ldg(p.s_wfx + e_beg + x);
+                    ev[u] = __ldg(edge + x);
+                    if (!PACKED) d[u] = (uint32_t)__ldg(dly + x);
                 }
             }
 #pragma unroll
             for (int u = 0; u < kRouteUnroll; ++u) {
                 if (x0 + 32u * u >= n_e) break;            // warp-uniform
                 const uint32_t x = x0 + 32u * u + lane;
-                uint32_t s = slot_t + d[u];
-                if (s >= p.D) s -= p.D;
-                const bool queued = d[u] >= d_direct;      // false for the padding lanes too (d = 0)
-                const uint32_t k_seg = queued ? 1u + ((d[u] - d_direct) >> p.q_log) : 0u;
-                const uint32_t pos = __shfl_sync(0xFFFFFFFFu, adj, k_seg) + x;
+                const uint32_t rd = r + (PACKED ? ev[u].x >> 24 : d[u]);
+                const uint32_t m = PACKED ? ev[u].x & 0xFFFFFFu : ev[u].x;
+                const bool queued = rd >= rd_queued && x < n_e;
+                const uint32_t k_seg = queued ? (rd >> p.q_log) - p.q_window : 0u;
+                const uint32_t at = __shfl_sync(0xFFFFFFFFu, adj, k_seg) + x;
                 if (!queued) continue;
-                if ((ovf >> k_seg) & 1u) {
-                    atomicAdd(p.ring + (size_t)s * p.Npad + m[u], w[u]);
-                } else {
-                    uint32_t b = g_cur + 1u + k_seg;
+                const uint32_t cell = (rd & Gm1) * p.Npad + m;
+                if (ovf && ((ovf >> k_seg) & 1u)) {
+                    uint32_t b = g_cur + (rd >> p.q_log);
                     if (b >= nb) b -= nb;
-                    const uint32_t cell = (s - (b << p.q_log)) * p.Npad + m[u];
-                    p.queue[(size_t)b * p.q_cap + pos] = make_uint2(cell, (uint32_t)w[u]);
+                    atomicAdd(p.ring + ((size_t)b << p.q_log) * p.Npad + cell, (int32_t)ev[u].y);
+                } else {
+                    p.queue[at] = make_uint2(cell, ev[u].y);
                 }
             }
         }
@@ -422,6 +428,7 @@ __device__ __forceinline__ void route_round(const GnDev &p, const uint32_t n, co
 // Routes the queued segments of every vertex that fired in steps t0 .. t0+n_batch-1, all inside ONE slot
 // group (slot0 = t0 mod D): one launch per group amortises the launch and the dependent memory round trips
 // over 2^q_log steps of work.  raster row of step t0+i is (row0 + i) mod raster_rows.
+template <bool PACKED>
 __global__ void __launch_bounds__(kRouteThreads, 4)
 gn_route_kernel(const GnDev p, const uint32_t slot0, const uint32_t row0, const uint32_t n_batch,
                 const uint32_t chunk_words)
@@ -442,7 +449,7 @@ gn_route_kernel(const GnDev p, const uint32_t slot0, const uint32_t row0, const 
         uint32_t word, off;
         const uint32_t total = gather_scan<kRouteThreads>(p.raster + (size_t)rr * p.words_pad, w0, n_words, s_wsum, word, off);
         if (n + total > kRouteListCap) {                    // CTA-uniform: the list is full, work it off first
-            route_round(p, n, slot0, s_list, s_step, s_wtot, s_wbase, &s_ovf, events);
+            route_round<PACKED>(p, n, slot0, s_list, s_step, s_wtot, s_wbase, &s_ovf, events);
             n = 0u;
         }
         gather_write(word, w0, n + off, s_list, s_step, i);
@@ -450,7 +457,7 @@ gn_route_kernel(const GnDev p, const uint32_t slot0, const uint32_t row0, const 
         spikes += total;
     }
     __syncthreads();
-    if (n) route_round(p, n, slot0, s_list, s_step, s_wtot, s_wbase, &s_ovf, events);
+    if (n) route_round<PACKED>(p, n, slot0, s_list, s_step, s_wtot, s_wbase, &s_ovf, events);
     if ((threadIdx.x & 31u) == 0 && events) atomicAdd(&p.counters[2], events);
     if (threadIdx.x == 0 && spikes) atomicAdd(&p.counters[1], (unsigned long long)spikes);
 }
@@ -527,8 +534,7 @@ gn_sort_rows_kernel(const GnDev p, GnCheck *chk)
         for (uint32_t e = beg + lane; e < end; e += 32u) {
             const uint32_t d = p.dly[e];
             const uint32_t pos = beg + atomicAdd(&h[d], 1u);
-            p.s_tgt[pos] = p.tgt[e];
-            p.s_wfx[pos] = p.wfx[e];
+            p.s_edge[pos] = make_uint2(p.tgt[e] | (p.packed ? d << 24 : 0u), (uint32_t)p.wfx[e]);
             p.s_dly[pos] = (uint8_t)d;
         }
         __syncwarp();
@@ -699,7 +705,7 @@ inline uint32_t ceil_div(uint64_t a, uint64_t b) { return (uint32_t)((a + b - 1)
 cudaError_t gnk_update(const GnDev &p, uint64_t t, bool has_bias, cudaStream_t st)
 {
     // delays below d_direct are delivered by the update kernel itself (see the kernel)
-    const uint32_t d_direct = p.queue_mode ? 2u * (1u << p.q_log) - ((uint32_t)(t % p.D) & ((1u << p.q_log) - 1u)) : 2u;
+    const uint32_t d_direct = p.queue_mode ? ((p.q_window + 1u) << p.q_log) - ((uint32_t)(t % p.D) & ((1u << p.q_log) - 1u)) : 2u;
     const uint32_t grid = ceil_div(p.Npad / kVertsPerThread, kUpdateThreads);
     const uint32_t slot = (uint32_t)(t % p.D);
     const uint32_t raster_row = (uint32_t)(t % p.raster_rows);
@@ -731,14 +737,15 @@ cudaError_t gnk_deliver(const GnDev &p, uint64_t t, cudaStream_t st)
 cudaError_t gnk_route(const GnDev &p, uint64_t t0, uint32_t n_batch, cudaStream_t st)
 {
     const uint32_t w = chunk_words_for(p, 148u * 4u);            // four 256-thread CTAs per SM
-    gn_route_kernel<<<ceil_div(p.words_pad, w), kRouteThreads, 0, st>>>(p, (uint32_t)(t0 % p.D),
-                                                                      (uint32_t)(t0 % p.raster_rows), n_batch, w);
+    const uint32_t grid = ceil_div(p.words_pad, w), slot0 = (uint32_t)(t0 % p.D), row0 = (uint32_t)(t0 % p.raster_rows);
+    if (p.packed) gn_route_kernel<true><<<grid, kRouteThreads, 0, st>>>(p, slot0, row0, n_batch, w);
+    else gn_route_kernel<false><<<grid, kRouteThreads, 0, st>>>(p, slot0, row0, n_batch, w);
     return cudaGetLastError();
 }
 
 cudaError_t gnk_fold(const GnDev &p, uint32_t bucket, cudaStream_t st)
 {
-    gn_fold_kernel<<<148u * 8u, 256, 0, st>>>(p, bucket);
+    gn_fold_kernel<<<148u * 4u, 256, 0, st>>>(p, bucket);
     return cudaGetLastError();
 }
 
