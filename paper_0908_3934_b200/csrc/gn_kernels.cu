@@ -91,27 +91,25 @@ gn_update_kernel(const GnDev p, const uint64_t t, const uint32_t slot, const uin
     uint32_t nib = 0u, kicks = 0u;                                        // bit q: vertex j0+q fired / kicked
 
     if (j0 < p.Npad) {
-        // drive first (its temporaries are dead before the state is loaded: the kernel must fit 32 registers
-        // so that all N/4 threads are resident in ONE wave): one Philox block per 4 vertices, counter
-        // {j/4, t lo, t hi, 5}, word j mod 4; Bernoulli kick when the word is below the class threshold
-        const uchar4 cl4 = *reinterpret_cast<const uchar4 *>(p.cls + j0);
-        const uint32_t cl[4] = {cl4.x, cl4.y, cl4.z, cl4.w};
-        if (p.any_drive) {
-            uint32_t x[4];
-            philox4x32_10(g, (uint32_t)t, (uint32_t)(t >> 32), kStreamDrive, p.seed_lo, p.seed_hi, x);
-#pragma unroll
-            for (int q = 0; q < 4; ++q)
-                if ((j0 + q) < p.N && x[q] < s_cls[cl[q]].drive_thr) kicks |= 1u << q;   // reading #12
-        }
-        // a1: read this step's ring slot, clear it only if something arrived
+        // drive words first: they depend on no memory, and their temporaries are dead before the state is loaded
+        // (the kernel must fit 32 registers so that all N/4 threads are resident in ONE wave).  One Philox block
+        // per 4 vertices, counter {j/4, t lo, t hi, 5}, word j mod 4.
+        uint32_t x[4] = {0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu};
+        if (p.any_drive) philox4x32_10(g, (uint32_t)t, (uint32_t)(t >> 32), kStreamDrive, p.seed_lo, p.seed_hi, x);
+        // a1: read this step's ring slot (cleared below, only if something arrived) and the state, all at once
         int4 *slot_ptr = reinterpret_cast<int4 *>(p.ring + (size_t)slot * p.Npad + j0);
         const int4 I4 = *slot_ptr;
         const float4 V4 = *reinterpret_cast<const float4 *>(p.V + j0);
         const float4 W4 = *reinterpret_cast<const float4 *>(p.W + j0);
         const float4 r4 = *reinterpret_cast<const float4 *>(p.r + j0);
         const uchar4 rf4 = *reinterpret_cast<const uchar4 *>(p.refr + j0);
+        const uchar4 cl4 = *reinterpret_cast<const uchar4 *>(p.cls + j0);
         float4 U4 = make_float4(0.f, 0.f, 0.f, 0.f);
         if (BIAS) U4 = *reinterpret_cast<const float4 *>(p.bias + j0);
+        const uint32_t cl[4] = {cl4.x, cl4.y, cl4.z, cl4.w};
+#pragma unroll
+        for (int q = 0; q < 4; ++q)                                          // Bernoulli kick, reading #12
+            if ((j0 + q) < p.N && x[q] < s_cls[cl[q]].drive_thr) kicks |= 1u << q;
         if ((I4.x | I4.y | I4.z | I4.w) != 0) *slot_ptr = make_int4(0, 0, 0, 0);
 
         int32_t I[4] = {I4.x, I4.y, I4.z, I4.w};
@@ -166,11 +164,11 @@ gn_update_kernel(const GnDev p, const uint64_t t, const uint32_t slot, const uin
             if (!((nib >> q) & 1u)) continue;
             const uint32_t end = p.row[j0 + q + 1];
             for (uint32_t e = p.row[j0 + q]; e < end; ++e) {
-                const uint32_t d = p.s_dly[e];
+                const uint2 ev = p.s_edge[e];
+                const uint32_t d = p.packed ? ev.x >> 24 : (uint32_t)p.s_dly[e];
                 if (d >= d_direct) break;
                 uint32_t s1 = slot + d;
                 if (s1 >= p.D) s1 -= p.D;
-                const uint2 ev = p.s_edge[e];
                 atomicAdd(p.ring + (size_t)s1 * p.Npad + (p.packed ? ev.x & 0xFFFFFFu : ev.x), (int32_t)ev.y);
             }
         }
