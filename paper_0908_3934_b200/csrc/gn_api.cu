@@ -17,7 +17,7 @@ thread_local char g_create_error[256] = "";
 
 struct Layout {
     size_t V, W, r, c, acc, bias, refr, cls, ring, row, tgt, wfx, dly, counters, q_count;
-    size_t s_edge, s_dly, q_seg, queue;
+    size_t s_edge, s_dly, min_dly, q_seg, queue;
     size_t raster, trace, scratch_row64, scratch_abs, scratch_pos, scratch_net, scratch_chk, total;
 };
 
@@ -96,6 +96,7 @@ Layout make_layout(const gn_config *cfg)
         L.raster = take(rows * (Npad / 32) * 4);
     }
     L.trace = take(obs ? (size_t)cfg->trace_capacity_frames * Npad * 4 : 0);
+    L.min_dly = take(Npad);
     L.s_edge = take(E * 8); L.s_dly = take(E);   // every row again, sorted by delay
     L.q_seg = take(qp.on ? N * D * 2 : 0);
     L.queue = take(qp.on ? (size_t)qp.q_nb * qp.q_cap * 8 : 0);
@@ -249,7 +250,7 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
     d.queue_mode = qp.on ? 1u : 0u;
     d.q_log = qp.q_log; d.q_nb = qp.q_nb; d.q_cap = qp.q_cap;
     d.q_count = (unsigned long long *)(ws + L.q_count);
-    d.s_edge = (uint2 *)(ws + L.s_edge); d.s_dly = ws + L.s_dly;
+    d.s_edge = (uint2 *)(ws + L.s_edge); d.s_dly = ws + L.s_dly; d.min_dly = ws + L.min_dly;
     d.packed = Npad <= (1u << 24) ? 1u : 0u;
     d.q_window = kQueueWindow;
     if (qp.on) {
@@ -299,7 +300,7 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
 
     // zero everything the step loop accumulates into or reads before writing
     GN_CREATE_CUDA(cudaMemsetAsync(ws, 0, L.tgt, st));                       // state, bias, refr, cls, ring, row
-    GN_CREATE_CUDA(cudaMemsetAsync(ws + L.counters, 0, L.s_edge - L.counters, st));   // counters, bucket counts, raster, trace
+    GN_CREATE_CUDA(cudaMemsetAsync(ws + L.counters, 0, L.min_dly - L.counters, st));   // counters, bucket counts, raster, trace
     GN_CREATE_CUDA(cudaMemsetAsync(abs_in, 0, (size_t)N * 8, st));
     GN_CREATE_CUDA(cudaMemsetAsync(chk_d, 0, sizeof(GnCheck), st));
     // uploads (host or device sources)
@@ -342,6 +343,7 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
         GN_CREATE_CUDA(gnk_validate(d, net_offsets ? net_d : nullptr, cfg->n_networks, abs_in, chk_d, st));
     }
     GN_CREATE_CUDA(gnk_check_overflow(d, abs_in, chk_d, st));
+    GN_CREATE_CUDA(cudaMemsetAsync(d.min_dly, 0xFF, Npad, st));
     if (E) GN_CREATE_CUDA(gnk_sort_rows(d, chk_d, st));
     GN_CREATE_CUDA(cudaMemcpyAsync(&chk, chk_d, sizeof chk, cudaMemcpyDeviceToHost, st));
     GN_CREATE_CUDA(cudaStreamSynchronize(st));

@@ -48,6 +48,7 @@ struct GnDev {
     uint2 *s_edge;           // [E] the CSR rows again, each sorted by delay: {target, w_fx}; when `packed`
                              //     (Npad <= 2^24) the delay also sits in the target word's top byte
     uint8_t *s_dly;          // [E] delay of s_edge[e]
+    uint8_t *min_dly;        // [Npad] smallest out-delay of every vertex (255: no out-edge)
     uint32_t packed;
     uint32_t q_window;       // queue mode: groups ahead of the current one whose events the update kernel sends itself
     uint16_t *q_seg;         // [N][2^q_log][q_nb] segment boundaries of every delay-sorted row (gn_route_kernel)

@@ -159,9 +159,11 @@ gn_update_kernel(const GnDev p, const uint64_t t, const uint32_t slot, const uin
     // (d_direct = 2), so that deliver(t) may overlap update(t+1).  Queue mode: every delay that lands in the
     // group being consumed or in the next one (d_direct = 2G - r), so that routing runs once per group.
     if (nib) {
+        const uchar4 md4 = *reinterpret_cast<const uchar4 *>(p.min_dly + j0);   // smallest out-delay of each vertex
+        const uint32_t md[4] = {md4.x, md4.y, md4.z, md4.w};
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
-            if (!((nib >> q) & 1u)) continue;
+            if (!((nib >> q) & 1u) || md[q] >= d_direct) continue;          // most vertices have no such edge
             const uint32_t end = p.row[j0 + q + 1];
             for (uint32_t e = p.row[j0 + q]; e < end; ++e) {
                 const uint2 ev = p.s_edge[e];
@@ -502,7 +504,14 @@ gn_sort_rows_kernel(const GnDev p, GnCheck *chk)
 #pragma unroll
         for (int k = 0; k < 8; ++k) h[lane * 8 + k] = 0u;
         __syncwarp();
-        for (uint32_t e = beg + lane; e < end; e += 32u) atomicAdd(&h[p.dly[e]], 1u);
+        uint32_t dmin = 255u;
+        for (uint32_t e = beg + lane; e < end; e += 32u) {
+            const uint32_t d = p.dly[e];
+            atomicAdd(&h[d], 1u);
+            dmin = min(dmin, d);
+        }
+        dmin = __reduce_min_sync(0xFFFFFFFFu, dmin);
+        if (lane == 0) p.min_dly[i] = (uint8_t)dmin;
         __syncwarp();
         uint32_t c[8], sum = 0u;
 #pragma unroll
