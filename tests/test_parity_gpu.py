@@ -13,7 +13,7 @@ kernel and a ragged tail (N not a multiple of 128).
 import numpy as np
 import pytest
 
-from gn_inputs import make_config
+from gn_inputs import Network, make_config
 from helpers import base_cfg, hand_net, random_digraph, rs_class, unpack_raster
 from oracle import Oracle
 from oracle import binding as ob
@@ -156,6 +156,72 @@ def test_queue_mode_ring_depth_not_a_multiple_of_the_group(gn):
     delays = rng.integers(1, 36, size=net.n_edges).astype(np.uint8)
     _, o, _ = _run_exact(gn, net, cfg, 900, 300, delays=delays, delivery_mode=gn.GN_DELIVER_QUEUE, queue_group=8)
     assert o.counters()["delivered"] > 0
+
+
+def test_queue_mode_reads_inside_a_group_and_odd_step_counts(gn):
+    """Queue mode routes once per slot group and the update kernel sends the near events itself: stepping by
+    counts that are not multiples of the group, and reading ring / counters in the middle of a group, must
+    still show exactly the oracle's state (the read flushes the pending routing and folds every bucket)."""
+    net, cfg = make_config(4, n=4_001)
+    g = _make(gn, net, cfg, 700, delivery_mode=gn.GN_DELIVER_QUEUE, queue_group=8)
+    o = Oracle(net, cfg, "fp32", threads=4)
+    done = 0
+    for k in (1, 2, 3, 5, 7, 11, 13, 64, 1, 250, 9, 8, 8, 3, 315):
+        gn.gn_step(g, k)
+        o.step(k)
+        done += k
+        _compare_exact(gn, g, o, done)
+    np.testing.assert_array_equal(gn.gn_read_raster(g, 0, done), o.raster(0, done))
+    assert o.counters()["delivered"] > 0
+
+
+def test_queue_mode_profiling_mode_and_small_raster_window(gn):
+    """gn_profile serialises every kernel on the caller's stream: same results; and a raster window shorter
+    than the two groups of spike lists the delivery kernels need is still honoured at the boundary."""
+    net, cfg = make_config(4, n=4_001)
+    g = _make(gn, net, cfg, 5, delivery_mode=gn.GN_DELIVER_QUEUE, queue_group=8)     # raster_capacity_steps = 5
+    o = Oracle(net, cfg, "fp32", threads=4)
+    gn.gn_step(g, 203)
+    gn.gn_profile(g, True)
+    gn.gn_step(g, 301)
+    ms, n = gn.gn_profile_read(g)
+    assert n[0] == 301 and 36 <= n[1] <= 39 and ms[0] > 0            # one routing launch per group of 8 steps
+    gn.gn_profile(g, False)
+    gn.gn_step(g, 96)
+    o.step(600)
+    _compare_exact(gn, g, o, 600)
+    np.testing.assert_array_equal(gn.gn_read_raster(g, 595, 5), o.raster(595, 5))
+    with pytest.raises(gn.GnError) as ei:
+        gn.gn_read_raster(g, 594, 6)
+    assert ei.value.code == gn.GN_E_RANGE_EVICTED
+
+
+def test_out_degree_above_16_bits_falls_back_to_the_ring_path(gn):
+    """The queue mode's segment table is 16-bit: a hub with 70,000 out-edges makes AUTO use the ring path
+    (same results) and a forced GN_DELIVER_QUEUE fail loudly."""
+    n, deg = 100_032, 70_000                                           # ring 51 MB: AUTO would pick queue mode
+    rng = np.random.default_rng(3)
+    row = np.zeros(n + 1, np.uint64)
+    row[1:] = deg                                                      # vertex 0 is the only source
+    tgt = (1 + rng.permutation(n - 1)[:deg]).astype(np.uint32)
+    tgt.sort()
+    net = Network(n, 2, 1, np.zeros((n, 2), np.float32), row, tgt, rng.uniform(0, 6, deg).astype(np.float32),
+                  np.zeros(n, np.uint8))
+    cfg = base_cfg([rs_class()], ring_slots=128)
+    dl = rng.integers(1, 128, deg).astype(np.uint8)
+    with pytest.raises(gn.GnError) as ei:
+        _make(gn, net, cfg, 10, delays=dl, delivery_mode=gn.GN_DELIVER_QUEUE)
+    assert ei.value.code == gn.GN_E_INVALID_ARG
+    g = _make(gn, net, cfg, 300, delays=dl)
+    o = Oracle(net, cfg, "fp32", delays=dl)
+    v = np.full(n, -70.0, np.float32)
+    v[0] = 30.0
+    gn.gn_write_state(g, gn.GN_V, v)
+    o.set_state(ob.V, v.astype(np.float64))
+    gn.gn_step(g, 300)
+    o.step(300)
+    _compare_exact(gn, g, o, 300)
+    assert o.counters()["delivered"] >= deg
 
 
 @pytest.mark.parametrize("k,n,nb,steps", [(1, None, None, 2000), (2, None, None, 2000), (4, 9_001, None, 2000)])
