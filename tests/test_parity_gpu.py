@@ -158,6 +158,44 @@ def test_queue_mode_ring_depth_not_a_multiple_of_the_group(gn):
     assert o.counters()["delivered"] > 0
 
 
+def test_config4_full_size_in_the_benchmark_configuration(gn):
+    """BASELINE configs[3] at FULL size (10^6 vertices, ~2*10^8 edges, D = 128), created exactly as bench.py
+    creates it (AUTO delivery = queue mode, no raster window beyond the benchmark's): rasters, counters, state
+    words and the whole 512 MB ring bit-exact against the fp32-faithful oracle after 1,500 steps (the network is
+    bursting by then: > 10^8 events delivered)."""
+    import os
+    net, cfg = make_config(4)
+    cfg = dict(cfg, obs_stride=0)
+    steps = 1500
+    g = _make(gn, net, cfg, 100)
+    o = Oracle(net, cfg, "fp32", threads=len(os.sched_getaffinity(0)))
+    for done in range(100, steps + 1, 100):
+        gn.gn_step(g, 100)
+        o.step(100)
+        np.testing.assert_array_equal(gn.gn_read_raster(g, done - 100, 100), o.raster(done - 100, 100))
+    _compare_exact(gn, g, o, steps)
+    assert o.counters()["delivered"] > 10 ** 8
+
+
+def test_config3_full_size_2000_steps(gn):
+    """BASELINE configs[2] at full size (10^5 vertices, ~7.2*10^6 edges, D = 64): ring mode (25.6 MB ring)."""
+    import os
+    net, cfg = make_config(3)
+    _, o, _ = _run_exact(gn, net, cfg, 2000, 500, threads=len(os.sched_getaffinity(0)))
+    assert o.counters()["delivered"] > 10 ** 6
+
+
+def test_config5_full_size_batched(gn):
+    """BASELINE configs[4] at full size: 4,096 networks of 1,000 vertices in ONE handle (block-diagonal CSR,
+    ~7.7*10^7 edges, D = 32, observation stride 100), 500 steps, everything bit-exact, trace within tolerance."""
+    import os
+    net, cfg = make_config(5)
+    g, o, _ = _run_exact(gn, net, cfg, 500, 250, threads=len(os.sched_getaffinity(0)))
+    assert o.counters()["delivered"] > 10 ** 5
+    frames = 500 // cfg["obs_stride"]
+    np.testing.assert_allclose(gn.gn_observe(g, 0, frames).astype(np.float64), o.trace(0, frames), rtol=1e-6, atol=1e-5)
+
+
 def test_queue_mode_reads_inside_a_group_and_odd_step_counts(gn):
     """Queue mode routes once per slot group and the update kernel sends the near events itself: stepping by
     counts that are not multiples of the group, and reading ring / counters in the middle of a group, must
