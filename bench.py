@@ -103,6 +103,24 @@ class ClockSampler:
                 "samples": len(sm)}
 
 
+def rank_seed(config, rank):
+    """Replicas only: rank r steps its own independent network of the same recipe."""
+    from gn_inputs import MASTER_SEED
+    return MASTER_SEED + config + 1000 * rank
+
+
+def reduce_over_ranks(dist, device, ms, spikes, events):
+    """Whole-job figures: time = MAX over ranks, spikes / events = SUM over ranks (no data-path collective)."""
+    import torch
+    if dist is None:
+        return ms, spikes, events
+    tms = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(tms, op=dist.ReduceOp.MAX)
+    tot = torch.tensor([spikes, events], device=device, dtype=torch.float64)
+    dist.all_reduce(tot)
+    return float(tms.item()), float(tot[0]), float(tot[1])
+
+
 def workload_name(net_in, cfg, args):
     return (f"BASELINE configs[{args.config - 1}] {cfg['name']}: N={net_in.n_vertices}, E={net_in.n_edges}, "
             f"D={cfg['ring_slots']}, dt={cfg['dt_ms']} ms")
@@ -206,12 +224,12 @@ def main():
         dist.init_process_group("nccl", device_id=dev)
 
     import paper_0908_3934_b200 as gn
-    from gn_inputs import MASTER_SEED, make_config
+    from gn_inputs import make_config
 
     K, W, S = args.steps, max(args.warmup, 3), args.sim_steps
     t0 = time.time()
     # replicas only: rank r steps its own independent network of the same recipe
-    net_in, cfg = make_config(args.config, n=args.n, seed=MASTER_SEED + args.config + 1000 * rank)
+    net_in, cfg = make_config(args.config, n=args.n, seed=rank_seed(args.config, rank))
     N, E = net_in.n_vertices, net_in.n_edges
     log(f"[rank {rank}] inputs in {time.time() - t0:.1f} s: N={N} E={E} mean out-degree {E / N:.1f}")
     obs = int(cfg["obs_stride"])
@@ -259,15 +277,7 @@ def main():
     c1 = counters(g)
     _, l1 = gn.gn_profile_read(g)
     launches = int(l1[4] - l0[4])
-    if dist is not None:
-        tms = torch.tensor([ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
-        ms = float(tms.item())
-        tot = torch.tensor([c1[1] - c0[1], c1[2] - c0[2]], device=dev, dtype=torch.float64)
-        dist.all_reduce(tot)
-        spikes, events = float(tot[0]), float(tot[1])
-    else:
-        spikes, events = c1[1] - c0[1], c1[2] - c0[2]
+    ms, spikes, events = reduce_over_ranks(dist, dev, ms, c1[1] - c0[1], c1[2] - c0[2])
     sec = ms * 1e-3
     sim_steps = K * S
     value = world * N * sim_steps / sec
@@ -304,10 +314,11 @@ def main():
     a4["frac"] = a4["achieved"] / peak
     dom = max(kernels, key=lambda r: r["share"])
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")   # per-launch DRAM bytes from the committed ncu --set full capture
+    tpath = os.path.join(ROOT, "profiles", "traffic.csv")   # per-launch DRAM bytes from the committed ncu --set full capture
     if os.path.exists(tpath):
         try:
-            traffic = json.load(open(tpath)).get(dom["kernel"].split()[0])
+            table = dict(line.strip().split(",") for line in open(tpath).read().splitlines()[1:] if line.strip())
+            traffic = float(table[dom["kernel"].split()[0]])
         except Exception:
             traffic = None
     roofline = {"bound": "hbm", "kernel": dom["kernel"], "achieved": dom["achieved"], "peak": peak, "unit": "GB/s",
@@ -346,10 +357,7 @@ def main():
         e1.record()
         barrier()
         ems = e0.elapsed_time(e1)
-        if dist is not None:
-            tms = torch.tensor([ems], device=dev, dtype=torch.float64)
-            dist.all_reduce(tms, op=dist.ReduceOp.MAX)
-            ems = float(tms.item())
+        ems, _, _ = reduce_over_ranks(dist, dev, ems, 0, 0)
         e2e = {"value": world * N * sim_steps / (ems * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d / K,
                "d2h_bytes_per_step": d2h, "ms_total": ems,
                "what": "gn_create from pinned host arrays (upload + validation + quantisation + eq. 25 delays) + K x "

@@ -88,12 +88,17 @@ typedef struct {
                                     /* back to direct ring adds; 0 = default queue_group * ceil(E/16) */
 } gn_config;
 
-/* delivery_mode.  RING: every event is one int32 reduction straight into ring[(t+delay) mod D][target]
- * (best while the ring fits L2).  QUEUE: events are appended, as (ring cell, weight) records, to the
- * bucket of the slot group they are due in; a bucket is folded into its ring rows just before the
- * first of them is consumed, when those rows are L2-resident (best when the ring is >> L2: sequential
- * 8-byte appends instead of a 32-byte DRAM sector read-modify-write per event).  AUTO picks QUEUE when
- * the ring exceeds 48 MB and D >= 32, else RING. */
+/* delivery_mode.
+ * RING: every event is one int32 reduction straight into ring[(t+delay) mod D][target], by a delivery kernel
+ *   that runs beside the next step's update (best while the ring fits L2).
+ * QUEUE: ring slots are taken queue_group at a time; an event due in a later group is appended, as an 8-byte
+ *   {ring cell, weight} record, to that group's bucket, and a bucket is added ("folded") into its ring rows just
+ *   before they are consumed, while those rows sit in L2 (best when the ring is >> L2: sequential appends instead
+ *   of a 32-byte DRAM sector read-modify-write per event).  Routing runs once per group of steps; events due
+ *   within two groups are sent by the update kernel itself.  Needs D to be a multiple of the group, D / group <= 32
+ *   and every out-degree <= 65535; where that fails QUEUE is refused (GN_E_INVALID_ARG for the degree) or, for the
+ *   depth conditions and under AUTO, the ring path is used: results are identical either way.
+ * AUTO picks QUEUE when the ring exceeds 48 MB and D >= 32, else RING. */
 #define GN_DELIVER_AUTO 0
 #define GN_DELIVER_RING 1
 #define GN_DELIVER_QUEUE 2
@@ -109,7 +114,8 @@ enum {
                       /*                 slot s holds the arrivals due at steps a = s (mod D),       */
                       /*                 T <= a <= T + D - 2; slot (T-1) mod D is zero               */
     GN_STEP = 6,      /* uint64 [1]      completed steps t                                           */
-    GN_COUNTERS = 7,  /* uint64 [4]      { steps, spikes, delivered events, kicks }                  */
+    GN_COUNTERS = 7,  /* uint64 [4]      { steps, spikes, delivered events, kicks } up to the last completed */
+                      /*                 step (reading it first routes any step whose events are pending)  */
     GN_DELAYS = 8,    /* uint8  [E]      per-edge delay in steps (as given, or eq. 25)               */
     GN_WEIGHTS_FX = 9,/* int32  [E]      per-edge weight, rint(w * 2^16)                             */
     GN_BIAS = 10      /* float  [N]      user control U_j (write only through gn_write_state)        */
