@@ -182,11 +182,12 @@ int gn_observe(gn_net *net, uint64_t frame0, uint64_t n_frames, float *trace, si
 int gn_debug_words(void *cuda_stream, uint64_t seed, uint32_t stream_id, uint64_t idx,
                    uint32_t first_vertex, uint32_t n, uint32_t *out);
 
-/* Per-kernel timing for benchmarks.  While enabled, gn_step brackets every kernel it launches with
- * CUDA events on the net's stream (and synchronises every few hundred steps to collect them), so the
- * step is slower than normal: a measuring mode, never the mode a throughput number is taken in.
+/* Per-kernel timing for benchmarks.  While enabled, gn_step runs every kernel on the net's stream (no overlap
+ * between update and delivery) with a CUDA event wherever the kind of kernel changes, and synchronises every
+ * few hundred steps to collect them: a measuring mode, never the mode a throughput number is taken in.  A run
+ * of consecutive launches of one kernel (queue mode: the updates of one slot group) is timed as a whole.
  * gn_profile_read: ms[k] = summed device time, launches[k] = launch count of kernel k since the last
- * gn_profile(net, 1): k = 0 update (a1-a3), 1 delivery (a4: ring reductions or queue routing),
+ * gn_profile(net, 1): k = 0 update (a1-a3), 1 delivery (a4: ring reductions, or queue routing once per group),
  * 2 observation (a5), 3 bucket fold (a4, queue mode).  launches[4] is the total number of kernels this
  * handle has launched since gn_create, profiling or not. */
 int gn_profile(gn_net *net, int enable);

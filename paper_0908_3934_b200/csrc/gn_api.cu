@@ -129,6 +129,7 @@ struct gn_net {
     size_t ev_used;
     double prof_ms[4];
     uint64_t prof_n[4];
+    uint8_t prof_last;               // kind of the launch after the last event
     uint64_t launches;                // every kernel launched by gn_step since gn_create
     char err[256];
 };
@@ -211,6 +212,7 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
     net->fences_pending = false;
     net->has_bias = bias != nullptr;
     net->profile = false;
+    net->prof_last = 0xFF;
     net->ev_used = 0;
     net->launches = 0;
     for (int k = 0; k < 4; ++k) { net->prof_ms[k] = 0.0; net->prof_n[k] = 0; }
@@ -386,11 +388,15 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
     return GN_OK;
 }
 
-// ---- measuring mode: one event at every kernel boundary, collected every kProfChunk steps ----------
+// ---- measuring mode: one event wherever the KIND of kernel changes (a run of consecutive launches of one kernel
+// is timed as a whole, so an event's own cost is not charged to every launch), collected every kProfChunk steps ----
 static const size_t kProfChunk = 256;
 
 static int prof_mark(gn_net *net, uint8_t kind_after)
 {
+    if (kind_after <= 3) net->prof_n[kind_after] += 1;                  // every launch is counted ...
+    if (kind_after == net->prof_last && kind_after != 0xFF) return GN_OK;   // ... but only a change of kind is marked
+    net->prof_last = kind_after;
     if (net->ev_used == net->ev.size()) {
         cudaEvent_t e;
         GN_CUDA(net, cudaEventCreate(&e));
@@ -413,9 +419,9 @@ static int prof_collect(gn_net *net)
         float ms = 0.f;
         GN_CUDA(net, cudaEventElapsedTime(&ms, net->ev[i], net->ev[i + 1]));
         net->prof_ms[k] += (double)ms;
-        net->prof_n[k] += 1;
     }
     net->ev_used = 0;
+    net->prof_last = 0xFF;
     return GN_OK;
 }
 
@@ -502,10 +508,12 @@ int gn_step(gn_net *net, uint64_t n_steps)
             GN_CUDA(net, gnk_observe(d, (t + 1) / d.obs_stride - 1, s_upd));
             net->launches++;
         }
-        if (prof && (rc = prof_mark(net, 0xFF))) return rc;
-        if (prof && (s + 1) % kProfChunk == 0 && (rc = prof_collect(net))) return rc;
+        if (prof && (s + 1) % kProfChunk == 0 && ((rc = prof_mark(net, 0xFF)) || (rc = prof_collect(net)))) return rc;
     }
-    if (net->profile) return prof_collect(net);
+    if (net->profile) {
+        int rc = prof_mark(net, 0xFF);
+        return rc ? rc : prof_collect(net);
+    }
     return join_streams(net);
 }
 
