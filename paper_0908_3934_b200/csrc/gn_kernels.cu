@@ -81,6 +81,9 @@ gn_update_kernel(const GnDev p, const uint64_t t, const uint32_t slot, const uin
                  const uint32_t d_direct)
 {
     __shared__ GnClassDev s_cls[GN_MAX_CLASSES];
+    // Programmatic dependent launch: the next step's update may start launching now; its prologue (class table,
+    // Philox words -- nothing a previous kernel wrote) then overlaps this kernel's tail (see griddepcontrol.wait below).
+    asm volatile("griddepcontrol.launch_dependents;");
     if (threadIdx.x < p.n_classes * 13u)
         reinterpret_cast<uint32_t *>(s_cls)[threadIdx.x] = reinterpret_cast<const uint32_t *>(p.cls_tab)[threadIdx.x];
     __syncthreads();
@@ -90,12 +93,14 @@ gn_update_kernel(const GnDev p, const uint64_t t, const uint32_t slot, const uin
     const uint32_t j0 = g * kVertsPerThread;
     uint32_t nib = 0u, kicks = 0u;                                        // bit q: vertex j0+q fired / kicked
 
+    // drive words first: they depend on no memory, and their temporaries are dead before the state is loaded
+    // (the kernel must fit 32 registers so that all N/4 threads are resident in ONE wave).  One Philox block
+    // per 4 vertices, counter {j/4, t lo, t hi, 5}, word j mod 4.
+    uint32_t x[4] = {0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu};
+    if (p.any_drive && j0 < p.Npad)
+        philox4x32_10(g, (uint32_t)t, (uint32_t)(t >> 32), kStreamDrive, p.seed_lo, p.seed_hi, x);
+    asm volatile("griddepcontrol.wait;" ::: "memory");     // everything before this step is complete and visible
     if (j0 < p.Npad) {
-        // drive words first: they depend on no memory, and their temporaries are dead before the state is loaded
-        // (the kernel must fit 32 registers so that all N/4 threads are resident in ONE wave).  One Philox block
-        // per 4 vertices, counter {j/4, t lo, t hi, 5}, word j mod 4.
-        uint32_t x[4] = {0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu};
-        if (p.any_drive) philox4x32_10(g, (uint32_t)t, (uint32_t)(t >> 32), kStreamDrive, p.seed_lo, p.seed_hi, x);
         // a1: read this step's ring slot (cleared below, only if something arrived) and the state, all at once
         int4 *slot_ptr = reinterpret_cast<int4 *>(p.ring + (size_t)slot * p.Npad + j0);
         const int4 I4 = *slot_ptr;
@@ -717,11 +722,21 @@ cudaError_t gnk_update(const GnDev &p, uint64_t t, bool has_bias, cudaStream_t s
     const uint32_t slot = (uint32_t)(t % p.D);
     const uint32_t raster_row = (uint32_t)(t % p.raster_rows);
     const bool obs = p.obs_stride != 0u;
-    if (obs && has_bias) gn_update_kernel<true, true><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, raster_row, d_direct);
-    else if (obs) gn_update_kernel<true, false><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, raster_row, d_direct);
-    else if (has_bias) gn_update_kernel<false, true><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, raster_row, d_direct);
-    else gn_update_kernel<false, false><<<grid, kUpdateThreads, 0, st>>>(p, t, slot, raster_row, d_direct);
-    return cudaGetLastError();
+    // programmatic stream serialization: this launch may begin (up to its griddepcontrol.wait) while the previous
+    // kernel in the stream -- normally the previous step's update -- is still draining
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(kUpdateThreads);
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    if (obs && has_bias) return cudaLaunchKernelEx(&cfg, gn_update_kernel<true, true>, p, t, slot, raster_row, d_direct);
+    if (obs) return cudaLaunchKernelEx(&cfg, gn_update_kernel<true, false>, p, t, slot, raster_row, d_direct);
+    if (has_bias) return cudaLaunchKernelEx(&cfg, gn_update_kernel<false, true>, p, t, slot, raster_row, d_direct);
+    return cudaLaunchKernelEx(&cfg, gn_update_kernel<false, false>, p, t, slot, raster_row, d_direct);
 }
 
 // Raster words per delivery CTA: enough CTAs to fill the chip, at most kMaxChunkWords words each.
