@@ -96,9 +96,19 @@ gn_update_kernel(const GnDev p, const uint64_t t, const uint32_t slot, const uin
     // drive words first: they depend on no memory, and their temporaries are dead before the state is loaded
     // (the kernel must fit 32 registers so that all N/4 threads are resident in ONE wave).  One Philox block
     // per 4 vertices, counter {j/4, t lo, t hi, 5}, word j mod 4.
-    uint32_t x[4] = {0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu};
-    if (p.any_drive && j0 < p.Npad)
-        philox4x32_10(g, (uint32_t)t, (uint32_t)(t >> 32), kStreamDrive, p.seed_lo, p.seed_hi, x);
+    // The class ids are constant after gn_create, so the Bernoulli kicks (reading #12) are decided here too.
+    uchar4 cl4 = make_uchar4(0, 0, 0, 0);
+    if (j0 < p.Npad) {
+        cl4 = *reinterpret_cast<const uchar4 *>(p.cls + j0);
+        if (p.any_drive) {
+            uint32_t x[4];
+            philox4x32_10(g, (uint32_t)t, (uint32_t)(t >> 32), kStreamDrive, p.seed_lo, p.seed_hi, x);
+            const uint32_t cq[4] = {cl4.x, cl4.y, cl4.z, cl4.w};
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+                if ((j0 + q) < p.N && x[q] < s_cls[cq[q]].drive_thr) kicks |= 1u << q;
+        }
+    }
     asm volatile("griddepcontrol.wait;" ::: "memory");     // everything before this step is complete and visible
     if (j0 < p.Npad) {
         // a1: read this step's ring slot (cleared below, only if something arrived) and the state, all at once
@@ -108,13 +118,9 @@ gn_update_kernel(const GnDev p, const uint64_t t, const uint32_t slot, const uin
         const float4 W4 = *reinterpret_cast<const float4 *>(p.W + j0);
         const float4 r4 = *reinterpret_cast<const float4 *>(p.r + j0);
         const uchar4 rf4 = *reinterpret_cast<const uchar4 *>(p.refr + j0);
-        const uchar4 cl4 = *reinterpret_cast<const uchar4 *>(p.cls + j0);
         float4 U4 = make_float4(0.f, 0.f, 0.f, 0.f);
         if (BIAS) U4 = *reinterpret_cast<const float4 *>(p.bias + j0);
         const uint32_t cl[4] = {cl4.x, cl4.y, cl4.z, cl4.w};
-#pragma unroll
-        for (int q = 0; q < 4; ++q)                                          // Bernoulli kick, reading #12
-            if ((j0 + q) < p.N && x[q] < s_cls[cl[q]].drive_thr) kicks |= 1u << q;
         if ((I4.x | I4.y | I4.z | I4.w) != 0) *slot_ptr = make_int4(0, 0, 0, 0);
 
         int32_t I[4] = {I4.x, I4.y, I4.z, I4.w};
