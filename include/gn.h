@@ -81,7 +81,7 @@ typedef struct {
     uint32_t trace_capacity_frames; /* device trace window (most recent frames kept)                 */
     uint64_t seed;                  /* key of the counter generator (drive stream 5, noise stream 6) */
     /* How eq. 30's sum reaches the ring (the RESULT is identical in every mode: integer adds commute). */
-    uint32_t delivery_mode;         /* GN_DELIVER_AUTO (0), GN_DELIVER_RING, GN_DELIVER_QUEUE          */
+    uint32_t delivery_mode;         /* GN_DELIVER_AUTO (0), _RING, _QUEUE, _RESIDENT                   */
     uint32_t queue_group;           /* queue mode: ring slots per event bucket, power of two in 1..16; */
                                     /* 0 = default (8)                                                */
     uint64_t queue_capacity;        /* queue mode: events one bucket holds before later ones fall     */
@@ -98,10 +98,15 @@ typedef struct {
  *   within two groups are sent by the update kernel itself.  Needs D to be a multiple of the group, D / group <= 32
  *   and every out-degree <= 65535; where that fails QUEUE is refused (GN_E_INVALID_ARG for the degree) or, for the
  *   depth conditions and under AUTO, the ring path is used: results are identical either way.
- * AUTO picks QUEUE when the ring exceeds 48 MB and D >= 32, else RING. */
+ * RESIDENT: every network (n_networks >= 1) lives in ONE CTA for a whole gn_step call: vertex state in registers,
+ *   the network's delay ring in shared memory, delivery by shared-memory integer atomics, one barrier per step and
+ *   no per-step kernel launch (the paper's own workload shape: many networks of <= 1000 vertices).  Needs every
+ *   network to have <= 1024 vertices and ring_slots x vertices x 4 bytes <= 200 KB; otherwise GN_E_INVALID_ARG.
+ * AUTO picks RESIDENT whenever it is possible, else QUEUE when the ring exceeds 48 MB and D >= 32, else RING. */
 #define GN_DELIVER_AUTO 0
 #define GN_DELIVER_RING 1
 #define GN_DELIVER_QUEUE 2
+#define GN_DELIVER_RESIDENT 3
 
 /* `which` of gn_read_state / gn_write_state, with the element type of the caller's buffer.       */
 enum {

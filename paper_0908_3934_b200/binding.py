@@ -17,7 +17,7 @@ GN_E_INVALID_ARG, GN_E_BAD_GRAPH, GN_E_OVERFLOW_RISK = -1, -2, -3
 GN_E_WORKSPACE_TOO_SMALL, GN_E_RANGE_EVICTED, GN_E_CUDA = -4, -5, -6
 GN_V, GN_W, GN_R, GN_CA, GN_REFR, GN_RING, GN_STEP, GN_COUNTERS, GN_DELAYS, GN_WEIGHTS_FX, GN_BIAS = range(11)
 GN_MAX_CLASSES = 8
-GN_DELIVER_AUTO, GN_DELIVER_RING, GN_DELIVER_QUEUE = 0, 1, 2
+GN_DELIVER_AUTO, GN_DELIVER_RING, GN_DELIVER_QUEUE, GN_DELIVER_RESIDENT = 0, 1, 2, 3
 
 CLASS_FIELDS = ("a", "b", "c_reset", "d", "k2", "k1", "k0", "v_peak", "tau_syn_ms",
                 "refractory_ms", "drive_rate_hz", "drive_kick")

@@ -36,7 +36,7 @@ int check_config(const gn_config *cfg, char *err, size_t errn)
     if (cfg->n_networks < 1 || cfg->n_networks > cfg->n_vertices) return fail("n_networks must be in [1, n_vertices]");
     if (cfg->obs_stride > 0 && cfg->trace_capacity_frames == 0) return fail("obs_stride > 0 needs trace_capacity_frames > 0");
     if (cfg->obs_stride > 0 && !(cfg->tau_ca_ms > 0.0f)) return fail("obs_stride > 0 needs tau_ca_ms > 0");
-    if (cfg->delivery_mode > GN_DELIVER_QUEUE) return fail("delivery_mode must be GN_DELIVER_AUTO, _RING or _QUEUE");
+    if (cfg->delivery_mode > GN_DELIVER_RESIDENT) return fail("delivery_mode must be GN_DELIVER_AUTO, _RING, _QUEUE or _RESIDENT");
     const uint32_t qg = cfg->queue_group;
     if (qg != 0 && (qg > 16 || (qg & (qg - 1)) != 0)) return fail("queue_group must be 0 or a power of two in 1..16");
     return GN_OK;
@@ -328,15 +328,45 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
         return set_err(nullptr, GN_E_BAD_GRAPH, chk.bad_row ? "row_offsets: not monotone, row_offsets[0] != 0 or row_offsets[N] != n_edges"
                                                             : "vertex_class: id >= n_classes");
     }
-    if (net_offsets) {   // host check of the (small) network table
-        // read back from the device copy so device-resident inputs work too
-        uint32_t first = 0, last = 0;
-        GN_CREATE_CUDA(cudaMemcpyAsync(&first, net_d, 4, cudaMemcpyDeviceToHost, st));
-        GN_CREATE_CUDA(cudaMemcpyAsync(&last, net_d + cfg->n_networks, 4, cudaMemcpyDeviceToHost, st));
+    // the (small) network table: checked on the host, read back from the device copy so device-resident inputs work too
+    std::vector<uint32_t> net_h((size_t)cfg->n_networks + 1);
+    if (net_offsets) {
+        GN_CREATE_CUDA(cudaMemcpyAsync(net_h.data(), net_d, net_h.size() * 4, cudaMemcpyDeviceToHost, st));
         GN_CREATE_CUDA(cudaStreamSynchronize(st));
-        if (first != 0 || last != N) {
+    } else {
+        net_h[0] = 0; net_h[1] = N;
+        GN_CREATE_CUDA(cudaMemcpyAsync(net_d, net_h.data(), 8, cudaMemcpyHostToDevice, st));
+        GN_CREATE_CUDA(cudaStreamSynchronize(st));
+    }
+    uint32_t max_net = 0;
+    {
+        bool ok = net_h.front() == 0 && net_h.back() == N;
+        for (size_t b = 0; ok && b + 1 < net_h.size(); ++b) {
+            if (net_h[b + 1] < net_h[b]) ok = false;
+            else if (net_h[b + 1] - net_h[b] > max_net) max_net = net_h[b + 1] - net_h[b];
+        }
+        if (!ok) {
             delete net;
-            return set_err(nullptr, GN_E_BAD_GRAPH, "net_offsets must start at 0 and end at n_vertices");
+            return set_err(nullptr, GN_E_BAD_GRAPH, "net_offsets must start at 0, end at n_vertices and never decrease");
+        }
+    }
+    // resident mode: every network in one CTA, its ring in shared memory (gn_resident_kernel)
+    {
+        const uint32_t threads = max_net <= 32 ? 32u : (max_net + 31u) / 32u * 32u;
+        const size_t smem = (size_t)cfg->ring_slots * threads * 4 + (size_t)4 * (threads / 4 + 2) * 16;
+        const bool fits = max_net <= 1024 && smem <= 200u * 1024u;
+        if (cfg->delivery_mode == GN_DELIVER_RESIDENT && !fits) {
+            delete net;
+            return set_err(nullptr, GN_E_INVALID_ARG, "GN_DELIVER_RESIDENT needs every network to have <= 1024 vertices and its ring "
+                                                      "(ring_slots x vertices x 4 bytes) to fit 200 KB of shared memory");
+        }
+        d.n_networks = cfg->n_networks;
+        d.net_off = net_d;
+        if (fits && (cfg->delivery_mode == GN_DELIVER_RESIDENT || cfg->delivery_mode == GN_DELIVER_AUTO)) {
+            d.resident = 1u;
+            d.res_threads = threads;
+            d.res_smem = (uint32_t)smem;
+            d.queue_mode = 0u;
         }
     }
     if (E) {
@@ -465,6 +495,25 @@ int gn_step(gn_net *net, uint64_t n_steps)
     if (!net) return GN_E_INVALID_ARG;
     const GnDev &d = net->dev;
     const uint32_t G = 1u << d.q_log;
+    if (d.resident) {      // the whole call is one launch (or a few, so that a kept raster window is never lapped)
+        const bool raster_on = d.raster_cap > 0;
+        uint64_t left = n_steps;
+        while (left) {
+            uint64_t n = left > 0x40000000ull ? 0x40000000ull : left;
+            if (raster_on && n > d.raster_rows) n = d.raster_rows;
+            int rc;
+            if (net->profile && (rc = prof_mark(net, 0))) return rc;
+            GN_CUDA(net, gnk_resident(d, net->t, (uint32_t)n, net->has_bias, raster_on, net->stream));
+            net->launches++;
+            net->t += n;
+            left -= n;
+        }
+        if (net->profile) {
+            int rc = prof_mark(net, 0xFF);
+            return rc ? rc : prof_collect(net);
+        }
+        return GN_OK;
+    }
     for (uint64_t s = 0; s < n_steps; ++s) {
         const uint64_t t = net->t;
         const bool prof = net->profile;

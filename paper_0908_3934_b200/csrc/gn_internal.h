@@ -50,6 +50,12 @@ struct GnDev {
     uint8_t *s_dly;          // [E] delay of s_edge[e]
     uint8_t *min_dly;        // [Npad] smallest out-delay of every vertex (255: no out-edge)
     uint32_t packed;
+    // resident mode (gn_resident_kernel): every network in one CTA
+    uint32_t resident;       // 0 / 1
+    uint32_t n_networks;
+    uint32_t res_threads;    // CTA size = largest network rounded up to 32
+    uint32_t res_smem;       // dynamic shared memory: ring [D][res_threads] + drive words
+    const uint32_t *net_off; // [n_networks + 1] first vertex of every network
     uint32_t q_window;       // queue mode: groups ahead of the current one whose events the update kernel sends itself
     uint16_t *q_seg;         // [N][2^q_log][q_nb] segment boundaries of every delay-sorted row (gn_route_kernel)
     uint2 *queue;            // [q_nb][q_cap] records {cell offset inside the bucket's ring rows, w_fx}
@@ -75,6 +81,7 @@ cudaError_t gnk_route(const GnDev &p, uint64_t t0, uint32_t n_batch, cudaStream_
 cudaError_t gnk_fold(const GnDev &p, uint32_t bucket, cudaStream_t st);
 cudaError_t gnk_sort_rows(const GnDev &p, GnCheck *chk, cudaStream_t st);
 cudaError_t gnk_observe(const GnDev &p, uint64_t frame, cudaStream_t st);
+cudaError_t gnk_resident(const GnDev &p, uint64_t t0, uint32_t n_steps, bool has_bias, bool raster_on, cudaStream_t st);
 cudaError_t gnk_init_state(const GnDev &p, GnCheck *chk, cudaStream_t st);
 cudaError_t gnk_convert_rows(const GnDev &p, const uint64_t *row64, uint64_t n_edges, GnCheck *chk,
                              cudaStream_t st);

@@ -594,6 +594,155 @@ gn_observe_kernel(const GnDev p, const uint64_t frame, const uint32_t trace_row)
     *reinterpret_cast<float4 *>(p.acc + j0) = make_float4(0.f, 0.f, 0.f, 0.f);
 }
 
+// ---- resident mode: every network lives in one CTA (a1-a5 for configs whose networks have <= 1024 vertices) ----
+// The paper's own workload shape is many small networks (N <= 1000).  Here a CTA owns one
+// network for a whole gn_step(n) call: thread i <-> vertex i of the network, V/W/r/c/acc/refr in registers, the
+// network's whole delay ring in shared memory ([D][blockDim] int32), delivery by shared-memory integer atomics,
+// one __syncthreads per step.  No per-step launch, no HBM traffic for state or ring inside the call: only the CSR
+// rows of the vertices that fire (L2/HBM), the raster bits and the trace rows.  Same arithmetic, same generator
+// layout, same integer ring as the streaming kernels: results are bit-identical.
+// Drive words: the Philox block of vertex group j/4 at step t serves 4 vertices, so the CTA computes the blocks
+// of its groups for 4 steps at a time into shared memory (one block per thread) instead of one per thread per step.
+constexpr int kResidentPhiloxSteps = 4;
+
+template <bool OBS, bool BIAS, bool PACKED>
+__global__ void __launch_bounds__(1024, 1)
+gn_resident_kernel(const GnDev p, const uint64_t t0, const uint32_t n_steps, const uint32_t raster_on)
+{
+    extern __shared__ int32_t s_dyn[];
+    __shared__ GnClassDev s_cls[GN_MAX_CLASSES];
+    __shared__ unsigned long long s_tot[3];                 // spikes, events, kicks of this CTA
+    const uint32_t stride = blockDim.x;
+    int32_t *s_ring = s_dyn;                                  // [D][stride]
+    uint32_t *s_px = reinterpret_cast<uint32_t *>(s_dyn + (size_t)p.D * stride);   // [4 steps][groups][4 words]
+    const uint32_t i = threadIdx.x, lane = i & 31u;
+    const uint32_t v0 = p.net_off[blockIdx.x], nv = p.net_off[blockIdx.x + 1] - v0;
+    const bool live = i < nv;
+    const uint32_t j = v0 + i;                                // global vertex id (the caller's)
+    const uint32_t g0 = v0 >> 2, n_groups = ((v0 + nv + 3u) >> 2) - g0;
+
+    if (i < p.n_classes * 13u) reinterpret_cast<uint32_t *>(s_cls)[i] = reinterpret_cast<const uint32_t *>(p.cls_tab)[i];
+    if (i < 3u) s_tot[i] = 0ull;
+    float V = 0.f, W = 0.f, r = 0.f, c = 0.f, acc = 0.f, U = 0.f;
+    uint32_t refr = 0u, cl = 0u;
+    if (live) {
+        V = p.V[j]; W = p.W[j]; r = p.r[j]; refr = p.refr[j]; cl = p.cls[j];
+        if (OBS) { c = p.c[j]; acc = p.acc[j]; }
+        if (BIAS) U = p.bias[j];
+    }
+    for (uint32_t s = 0; s < p.D; ++s) s_ring[s * stride + i] = live ? p.ring[(size_t)s * p.Npad + j] : 0;
+    __syncthreads();
+    const GnClassDev k = s_cls[cl];
+
+    uint32_t slot = (uint32_t)(t0 % p.D);
+    uint32_t raster_row = (uint32_t)(t0 % p.raster_rows);
+    uint32_t in_frame = OBS ? (uint32_t)(t0 % p.obs_stride) : 0u;        // steps of the current frame already taken
+    uint64_t frame = OBS ? t0 / p.obs_stride : 0ull;
+    const uint32_t px_off = ((j >> 2) - g0) * 4u + (j & 3u), px_step = n_groups * 4u;
+    uint32_t n_spikes = 0u, n_kicks = 0u;
+    unsigned long long n_events = 0ull;
+    for (uint32_t st = 0; st < n_steps; ++st) {
+        const uint64_t t = t0 + st;
+        if (p.any_drive && (st % kResidentPhiloxSteps) == 0u) {       // drive words of the next 4 steps
+            for (uint32_t q = i; q < n_groups * kResidentPhiloxSteps; q += stride) {
+                const uint32_t ks = q / n_groups, gg = q - ks * n_groups;
+                const uint64_t tt = t + ks;
+                uint32_t x[4];
+                philox4x32_10(g0 + gg, (uint32_t)tt, (uint32_t)(tt >> 32), kStreamDrive, p.seed_lo, p.seed_hi, x);
+                *reinterpret_cast<uint4 *>(s_px + (size_t)q * 4u) = make_uint4(x[0], x[1], x[2], x[3]);
+            }
+            __syncthreads();
+        }
+        // a1: this step's ring word, cleared; Bernoulli kick (reading #12)
+        int32_t I = s_ring[slot * stride + i];
+        s_ring[slot * stride + i] = 0;
+        if (p.any_drive && live) {
+            const uint32_t x = s_px[(st % kResidentPhiloxSteps) * px_step + px_off];
+            if (x < k.drive_thr) { I += k.kick_fx; ++n_kicks; }
+        }
+        // a2 + a3
+        const bool fired = vertex_step<BIAS>(k, p.dt, I, U, V, W, r, refr) && live;
+        if (OBS) {
+            c = __fmaf_rn(p.keep_c, c, fired ? p.ca_jump : 0.0f);            // H_c
+            acc = __fadd_rn(acc, c);
+        }
+        const uint32_t fired_mask = __ballot_sync(0xFFFFFFFFu, fired);
+        n_spikes += fired ? 1u : 0u;
+        if (raster_on && fired_mask) {                        // rows were zeroed by the launcher; words may straddle CTAs
+            const uint32_t jw = j - lane, sh = jw & 31u;
+            uint32_t *rowp = p.raster + (size_t)raster_row * p.words_pad + (jw >> 5);
+            if (lane == 0u) {
+                atomicOr(rowp, fired_mask << sh);
+                if (sh) atomicOr(rowp + 1, fired_mask >> (32u - sh));
+            }
+        }
+        // a4: every fired vertex of the warp in turn, lanes over its row, shared-memory integer atomics
+        if (fired_mask) {
+            uint32_t beg = 0u, end = 0u;
+            if (fired) { beg = p.row[j]; end = p.row[j + 1]; }
+            uint32_t m = fired_mask;
+            while (m) {
+                const uint32_t src_lane = (uint32_t)__ffs(m) - 1u;
+                m &= m - 1u;
+                const uint32_t b = __shfl_sync(0xFFFFFFFFu, beg, src_lane), e_end = __shfl_sync(0xFFFFFFFFu, end, src_lane);
+                for (uint32_t e = b + lane; e < e_end; e += 32u) {
+                    const uint2 ev = p.s_edge[e];
+                    const uint32_t d = PACKED ? ev.x >> 24 : (uint32_t)p.s_dly[e];
+                    const uint32_t tgt = (PACKED ? ev.x & 0xFFFFFFu : ev.x) - v0;
+                    uint32_t s = slot + d;
+                    if (s >= p.D) s -= p.D;
+                    atomicAdd(&s_ring[s * stride + tgt], (int32_t)ev.y);
+                }
+                if (lane == 0u) n_events += (unsigned long long)(e_end - b);
+            }
+        }
+        __syncthreads();                                      // deliveries land before the next slot is read
+        // a5: camera frame
+        if (OBS && ++in_frame == p.obs_stride) {
+            float z = 0.f;
+            if (p.obs_sigma != 0.0f) {
+                uint32_t x[4];
+                philox4x32_10(j >> 2, (uint32_t)frame, (uint32_t)(frame >> 32), kStreamNoise, p.seed_lo, p.seed_hi, x);
+                const uint32_t h = (j & 3u) >> 1;
+                const float ua = __fmaf_rn((float)(x[2 * h] >> 9), 0x1p-23f, 0x1p-24f);
+                const float ub2 = __fmul_rn((float)(x[2 * h + 1] >> 8), 0x1p-23f);
+                const float rad = sqrtf(-2.0f * logf(ua));
+                float sn, cs;
+                sincospif(ub2, &sn, &cs);
+                z = (j & 1u) ? rad * sn : rad * cs;
+            }
+            if (live)
+                p.trace[(size_t)(frame % p.trace_cap) * p.Npad + j] = p.obs_gain * (acc * p.inv_stride) + p.obs_offset + p.obs_sigma * z;
+            acc = 0.f;
+            in_frame = 0u;
+            ++frame;
+        }
+        if (++slot == p.D) slot = 0u;
+        if (++raster_row == p.raster_rows) raster_row = 0u;
+    }
+    // back to global memory: the state at t0 + n_steps
+    if (live) {
+        p.V[j] = V; p.W[j] = W; p.r[j] = r; p.refr[j] = (uint8_t)refr;
+        if (OBS) { p.c[j] = c; p.acc[j] = acc; }
+    }
+    for (uint32_t s = 0; s < p.D; ++s)
+        if (live) p.ring[(size_t)s * p.Npad + j] = s_ring[s * stride + i];
+    n_spikes = __reduce_add_sync(0xFFFFFFFFu, n_spikes);
+    n_kicks = __reduce_add_sync(0xFFFFFFFFu, n_kicks);
+    if (lane == 0u) {
+        if (n_spikes) atomicAdd(&s_tot[0], (unsigned long long)n_spikes);
+        if (n_events) atomicAdd(&s_tot[1], n_events);
+        if (n_kicks) atomicAdd(&s_tot[2], (unsigned long long)n_kicks);
+    }
+    __syncthreads();
+    if (i == 0u) {
+        if (s_tot[0]) atomicAdd(&p.counters[1], s_tot[0]);
+        if (s_tot[1]) atomicAdd(&p.counters[2], s_tot[1]);
+        if (s_tot[2]) atomicAdd(&p.counters[3], s_tot[2]);
+        if (blockIdx.x == 0) p.counters[0] = t0 + n_steps;
+    }
+}
+
 // ---- create-time kernels --------------------------------------------------------------------------------
 __global__ void gn_init_state_kernel(const GnDev p, GnCheck *chk)
 {
@@ -743,6 +892,40 @@ cudaError_t gnk_update(const GnDev &p, uint64_t t, bool has_bias, cudaStream_t s
     if (obs) return cudaLaunchKernelEx(&cfg, gn_update_kernel<true, false>, p, t, slot, raster_row, d_direct);
     if (has_bias) return cudaLaunchKernelEx(&cfg, gn_update_kernel<false, true>, p, t, slot, raster_row, d_direct);
     return cudaLaunchKernelEx(&cfg, gn_update_kernel<false, false>, p, t, slot, raster_row, d_direct);
+}
+
+// Resident mode: one CTA per network for n_steps steps.  Raster rows of these steps are zeroed first (the kernel ORs bits
+// into words that may straddle two networks); the caller keeps n_steps <= raster_rows when a raster is kept.
+cudaError_t gnk_resident(const GnDev &p, uint64_t t0, uint32_t n_steps, bool has_bias, bool raster_on, cudaStream_t st)
+{
+    if (raster_on) {
+        const uint32_t r0 = (uint32_t)(t0 % p.raster_rows);
+        const uint32_t first = n_steps < p.raster_rows - r0 ? n_steps : p.raster_rows - r0;
+        cudaError_t e = cudaMemsetAsync(p.raster + (size_t)r0 * p.words_pad, 0, (size_t)first * p.words_pad * 4, st);
+        if (e == cudaSuccess && first < n_steps)
+            e = cudaMemsetAsync(p.raster, 0, (size_t)(n_steps - first) * p.words_pad * 4, st);
+        if (e != cudaSuccess) return e;
+    }
+    const size_t smem = p.res_smem;
+    const bool obs = p.obs_stride != 0u;
+#define GN_RES_LAUNCH(O, B, P)                                                                                  \
+    do {                                                                                                        \
+        cudaError_t e_ = cudaFuncSetAttribute(gn_resident_kernel<O, B, P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
+        if (e_ != cudaSuccess) return e_;                                                                       \
+        gn_resident_kernel<O, B, P><<<p.n_networks, p.res_threads, smem, st>>>(p, t0, n_steps, raster_on ? 1u : 0u); \
+        return cudaGetLastError();                                                                              \
+    } while (0)
+    if (p.packed) {
+        if (obs && has_bias) GN_RES_LAUNCH(true, true, true);
+        if (obs) GN_RES_LAUNCH(true, false, true);
+        if (has_bias) GN_RES_LAUNCH(false, true, true);
+        GN_RES_LAUNCH(false, false, true);
+    }
+    if (obs && has_bias) GN_RES_LAUNCH(true, true, false);
+    if (obs) GN_RES_LAUNCH(true, false, false);
+    if (has_bias) GN_RES_LAUNCH(false, true, false);
+    GN_RES_LAUNCH(false, false, false);
+#undef GN_RES_LAUNCH
 }
 
 // Raster words per delivery CTA: enough CTAs to fill the chip, at most kMaxChunkWords words each.

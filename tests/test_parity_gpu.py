@@ -196,6 +196,63 @@ def test_config5_full_size_batched(gn):
     np.testing.assert_allclose(gn.gn_observe(g, 0, frames).astype(np.float64), o.trace(0, frames), rtol=1e-6, atol=1e-5)
 
 
+# ---- resident mode (one CTA per network) and the streaming kernels on the same small inputs ------------
+@pytest.mark.parametrize("k,n,nb,steps,chunk,mode", [
+    (1, None, None, 2000, 700, "RING"), (1, None, None, 2000, 700, "RESIDENT"),
+    (5, 1000, 6, 1200, 400, "RING"), (5, 1000, 6, 1200, 400, "RESIDENT"),
+    (5, 333, 9, 900, 900, "RESIDENT"),          # network starts at multiples of 333: no 4- or 32-alignment
+    (2, 1_024, None, 800, 250, "RESIDENT"),     # one network filling the CTA, E/I classes, observation every step
+])
+def test_small_networks_every_delivery_mode(gn, k, n, nb, steps, chunk, mode):
+    net, cfg = make_config(k, n=n, n_networks=nb)
+    g, o, _ = _run_exact(gn, net, cfg, steps, chunk, delivery_mode=getattr(gn, "GN_DELIVER_" + mode))
+    assert o.counters()["spikes"] > 0
+    if cfg["obs_stride"]:
+        frames = steps // cfg["obs_stride"]
+        np.testing.assert_allclose(gn.gn_observe(g, 0, frames).astype(np.float64), o.trace(0, frames), rtol=1e-6, atol=1e-5)
+        np.testing.assert_array_equal(gn.gn_read_state(g, gn.GN_CA).view(np.uint32),
+                                      o.state(ob.CA).astype(np.float32).view(np.uint32))
+
+
+def test_resident_mode_ragged_batch_bias_and_short_raster_window(gn):
+    """Networks of 37, 1, 250 and 5 vertices in one handle (a network of one vertex, offsets with no alignment),
+    a bias above rheobase, a raster window of 7 steps stepped 50 at a time (the call is split so that the window
+    is never lapped inside a launch), explicit delays up to D-1."""
+    rng = np.random.default_rng(21)
+    sizes = [37, 1, 250, 5]
+    off = np.r_[0, np.cumsum(sizes)].astype(np.uint32)
+    edges = []
+    for b, nv in enumerate(sizes):
+        for (i, jj, w, d) in random_digraph(rng, nv, min(1.0, 6.0 / max(nv, 1)), 20):
+            edges.append((int(off[b]) + i, int(off[b]) + jj, w, d))
+    net, dl = hand_net(int(off[-1]), edges)
+    net = Network(net.n_vertices, 2, len(sizes), net.positions, net.row_offsets, net.targets, net.weights,
+                  net.vertex_class, net_offsets=off)
+    cfg = base_cfg([rs_class(drive_rate_hz=200.0)], ring_slots=20, obs_stride=25, obs_sigma=0.05)
+    bias = rng.uniform(0.0, 12.0, net.n_vertices).astype(np.float32)
+    g = gn.create_from_inputs(net, cfg, delays=dl, bias=bias, raster_capacity_steps=7, trace_capacity_frames=40,
+                              delivery_mode=gn.GN_DELIVER_RESIDENT)
+    o = Oracle(net, cfg, "fp32", delays=dl, bias=bias)
+    for done in range(50, 1001, 50):
+        gn.gn_step(g, 50)
+        o.step(50)
+        np.testing.assert_array_equal(gn.gn_read_raster(g, done - 7, 7), o.raster(done - 7, 7))
+    _compare_exact(gn, g, o, 1000)
+    np.testing.assert_allclose(gn.gn_observe(g, 0, 40).astype(np.float64), o.trace(0, 40), rtol=1e-6, atol=1e-5)
+    assert o.counters()["delivered"] > 0 and o.counters()["kicks"] > 0
+
+
+def test_resident_mode_refused_when_a_network_does_not_fit(gn):
+    net, cfg = make_config(2, n=1_500)                                   # 1,500 vertices in one network
+    with pytest.raises(gn.GnError) as ei:
+        _make(gn, net, cfg, 10, delivery_mode=gn.GN_DELIVER_RESIDENT)
+    assert ei.value.code == gn.GN_E_INVALID_ARG
+    net, cfg = make_config(1, n=900)                                     # 900 vertices x 255 slots x 4 B > 200 KB
+    cfg = dict(cfg, ring_slots=255)
+    with pytest.raises(gn.GnError):
+        _make(gn, net, cfg, 10, delays=np.ones(net.n_edges, np.uint8), delivery_mode=gn.GN_DELIVER_RESIDENT)
+
+
 def test_queue_mode_reads_inside_a_group_and_odd_step_counts(gn):
     """Queue mode routes once per slot group and the update kernel sends the near events itself: stepping by
     counts that are not multiples of the group, and reading ring / counters in the middle of a group, must
