@@ -98,10 +98,11 @@ typedef struct {
  *   within two groups are sent by the update kernel itself.  Needs D to be a multiple of the group, D / group <= 32
  *   and every out-degree <= 65535; where that fails QUEUE is refused (GN_E_INVALID_ARG for the degree) or, for the
  *   depth conditions and under AUTO, the ring path is used: results are identical either way.
- * RESIDENT: every network (n_networks >= 1) lives in ONE CTA for a whole gn_step call: vertex state in registers,
- *   the network's delay ring in shared memory, delivery by shared-memory integer atomics, one barrier per step and
- *   no per-step kernel launch (the paper's own workload shape: many networks of <= 1000 vertices).  Needs every
- *   network to have <= 1024 vertices and ring_slots x vertices x 4 bytes <= 200 KB; otherwise GN_E_INVALID_ARG.
+ * RESIDENT: every network (n_networks >= 1) lives in ONE CTA -- or, above 1,024 vertices, one thread-block cluster of
+ *   up to 16 CTAs -- for a whole gn_step call: vertex state in registers, the network's delay ring in (distributed)
+ *   shared memory, delivery by shared-memory integer atomics, one barrier per step and no per-step kernel launch
+ *   (the paper's own workload shape: many networks of <= 1000 vertices).  Needs every network to have <= 16,384
+ *   vertices and ring_slots x min(vertices, 1024) x 4 bytes <= 200 KB; otherwise GN_E_INVALID_ARG.
  * AUTO picks RESIDENT whenever it is possible, else QUEUE when the ring exceeds 48 MB and D >= 32, else RING. */
 #define GN_DELIVER_AUTO 0
 #define GN_DELIVER_RING 1

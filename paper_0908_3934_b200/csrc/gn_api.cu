@@ -350,20 +350,29 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
             return set_err(nullptr, GN_E_BAD_GRAPH, "net_offsets must start at 0, end at n_vertices and never decrease");
         }
     }
-    // resident mode: every network in one CTA, its ring in shared memory (gn_resident_kernel)
+    // resident mode: every network in one CTA -- or one thread-block cluster of up to 16 CTAs x 1,024 vertices --
+    // with its ring in shared memory (gn_resident_kernel)
     {
-        const uint32_t threads = max_net <= 32 ? 32u : (max_net + 31u) / 32u * 32u;
+        const uint32_t cluster = max_net <= 1024 ? 1u : (max_net + 1023u) / 1024u;
+        const uint32_t threads = cluster > 1 ? 1024u : (max_net <= 32 ? 32u : (max_net + 31u) / 32u * 32u);
         const size_t smem = (size_t)cfg->ring_slots * threads * 4 + (size_t)4 * (threads / 4 + 2) * 16;
-        const bool fits = max_net <= 1024 && smem <= 200u * 1024u;
+        bool fits = cluster <= 16 && smem <= 200u * 1024u;
+        if (fits && cluster > 1) {
+            GnDev probe = d;
+            probe.res_cluster = cluster; probe.res_threads = threads; probe.res_smem = (uint32_t)smem;
+            probe.n_networks = cfg->n_networks; probe.packed = Npad <= (1u << 24) ? 1u : 0u;
+            GN_CREATE_CUDA(gnk_resident_cluster_ok(probe, &fits));
+        }
         if (cfg->delivery_mode == GN_DELIVER_RESIDENT && !fits) {
             delete net;
-            return set_err(nullptr, GN_E_INVALID_ARG, "GN_DELIVER_RESIDENT needs every network to have <= 1024 vertices and its ring "
-                                                      "(ring_slots x vertices x 4 bytes) to fit 200 KB of shared memory");
+            return set_err(nullptr, GN_E_INVALID_ARG, "GN_DELIVER_RESIDENT needs every network to have <= 16,384 vertices and the ring "
+                                                      "of 1,024 vertices (ring_slots x 1,024 x 4 bytes) to fit 200 KB of shared memory");
         }
         d.n_networks = cfg->n_networks;
         d.net_off = net_d;
         if (fits && (cfg->delivery_mode == GN_DELIVER_RESIDENT || cfg->delivery_mode == GN_DELIVER_AUTO)) {
             d.resident = 1u;
+            d.res_cluster = cluster;
             d.res_threads = threads;
             d.res_smem = (uint32_t)smem;
             d.queue_mode = 0u;

@@ -53,7 +53,8 @@ struct GnDev {
     // resident mode (gn_resident_kernel): every network in one CTA
     uint32_t resident;       // 0 / 1
     uint32_t n_networks;
-    uint32_t res_threads;    // CTA size = largest network rounded up to 32
+    uint32_t res_cluster;    // CTAs per network: 1, or a thread-block cluster of up to 16 (1,024 vertices each)
+    uint32_t res_threads;    // CTA size = largest network rounded up to 32 (1,024 in cluster mode)
     uint32_t res_smem;       // dynamic shared memory: ring [D][res_threads] + drive words
     const uint32_t *net_off; // [n_networks + 1] first vertex of every network
     uint32_t q_window;       // queue mode: groups ahead of the current one whose events the update kernel sends itself
@@ -82,6 +83,7 @@ cudaError_t gnk_fold(const GnDev &p, uint32_t bucket, cudaStream_t st);
 cudaError_t gnk_sort_rows(const GnDev &p, GnCheck *chk, cudaStream_t st);
 cudaError_t gnk_observe(const GnDev &p, uint64_t frame, cudaStream_t st);
 cudaError_t gnk_resident(const GnDev &p, uint64_t t0, uint32_t n_steps, bool has_bias, bool raster_on, cudaStream_t st);
+cudaError_t gnk_resident_cluster_ok(const GnDev &p, bool *ok);
 cudaError_t gnk_init_state(const GnDev &p, GnCheck *chk, cudaStream_t st);
 cudaError_t gnk_convert_rows(const GnDev &p, const uint64_t *row64, uint64_t n_edges, GnCheck *chk,
                              cudaStream_t st);

@@ -10,7 +10,13 @@
 // round-to-nearest intrinsic in a fixed order, so the result is bit-identical to the fp32-faithful
 // CPU oracle.  Delivery and the drive decision are integer; atomics are order-independent.
 // Paper line numbers refer to /root/reference/PAPER.md.
+#include <cooperative_groups.h>
+
+#include <utility>
+
 #include "gn_internal.h"
+
+namespace cg = cooperative_groups;
 
 namespace {
 
@@ -605,21 +611,29 @@ gn_observe_kernel(const GnDev p, const uint64_t frame, const uint32_t trace_row)
 // of its groups for 4 steps at a time into shared memory (one block per thread) instead of one per thread per step.
 constexpr int kResidentPhiloxSteps = 4;
 
-template <bool OBS, bool BIAS, bool PACKED>
+template <bool OBS, bool BIAS, bool PACKED, bool CLUSTER>
 __global__ void __launch_bounds__(1024, 1)
 gn_resident_kernel(const GnDev p, const uint64_t t0, const uint32_t n_steps, const uint32_t raster_on)
 {
+    // CLUSTER: a network is spread over the p.res_cluster CTAs of one thread-block cluster (1,024 vertices each);
+    // an event whose target lives in another CTA is a shared-memory atomic through DSMEM, and the per-step barrier
+    // is the cluster's.
     extern __shared__ int32_t s_dyn[];
     __shared__ GnClassDev s_cls[GN_MAX_CLASSES];
     __shared__ unsigned long long s_tot[3];                 // spikes, events, kicks of this CTA
+    cg::cluster_group cluster = cg::this_cluster();
     const uint32_t stride = blockDim.x;
-    int32_t *s_ring = s_dyn;                                  // [D][stride]
+    int32_t *s_ring = s_dyn;                                  // [D][stride]: the ring words of this CTA's vertices
     uint32_t *s_px = reinterpret_cast<uint32_t *>(s_dyn + (size_t)p.D * stride);   // [4 steps][groups][4 words]
     const uint32_t i = threadIdx.x, lane = i & 31u;
-    const uint32_t v0 = p.net_off[blockIdx.x], nv = p.net_off[blockIdx.x + 1] - v0;
-    const bool live = i < nv;
-    const uint32_t j = v0 + i;                                // global vertex id (the caller's)
-    const uint32_t g0 = v0 >> 2, n_groups = ((v0 + nv + 3u) >> 2) - g0;
+    const uint32_t net = CLUSTER ? blockIdx.x / p.res_cluster : blockIdx.x;
+    const uint32_t rank = CLUSTER ? blockIdx.x - net * p.res_cluster : 0u;
+    const uint32_t v0 = p.net_off[net], nv = p.net_off[net + 1] - v0;      // the network
+    const uint32_t c0 = rank * stride;                        // first local vertex of this CTA
+    const bool live = c0 + i < nv;
+    const uint32_t j = v0 + c0 + i;                           // global vertex id (the caller's)
+    const uint32_t c_nv = c0 < nv ? min(stride, nv - c0) : 0u;             // vertices of this CTA
+    const uint32_t g0 = (v0 + c0) >> 2, n_groups = c_nv ? ((v0 + c0 + c_nv + 3u) >> 2) - g0 : 0u;
 
     if (i < p.n_classes * 13u) reinterpret_cast<uint32_t *>(s_cls)[i] = reinterpret_cast<const uint32_t *>(p.cls_tab)[i];
     if (i < 3u) s_tot[i] = 0ull;
@@ -631,7 +645,7 @@ gn_resident_kernel(const GnDev p, const uint64_t t0, const uint32_t n_steps, con
         if (BIAS) U = p.bias[j];
     }
     for (uint32_t s = 0; s < p.D; ++s) s_ring[s * stride + i] = live ? p.ring[(size_t)s * p.Npad + j] : 0;
-    __syncthreads();
+    if (CLUSTER) cluster.sync(); else __syncthreads();
     const GnClassDev k = s_cls[cl];
 
     uint32_t slot = (uint32_t)(t0 % p.D);
@@ -688,15 +702,22 @@ gn_resident_kernel(const GnDev p, const uint64_t t0, const uint32_t n_steps, con
                 for (uint32_t e = b + lane; e < e_end; e += 32u) {
                     const uint2 ev = p.s_edge[e];
                     const uint32_t d = PACKED ? ev.x >> 24 : (uint32_t)p.s_dly[e];
-                    const uint32_t tgt = (PACKED ? ev.x & 0xFFFFFFu : ev.x) - v0;
+                    const uint32_t tgt = (PACKED ? ev.x & 0xFFFFFFu : ev.x) - v0;     // local vertex of the target
                     uint32_t s = slot + d;
                     if (s >= p.D) s -= p.D;
-                    atomicAdd(&s_ring[s * stride + tgt], (int32_t)ev.y);
+                    if (CLUSTER) {
+                        const uint32_t owner = tgt >> 10;                               // stride is 1,024 in cluster mode
+                        atomicAdd(cluster.map_shared_rank(&s_ring[s * stride + (tgt & 1023u)], owner), (int32_t)ev.y);
+                    } else {
+                        atomicAdd(&s_ring[s * stride + tgt], (int32_t)ev.y);
+                    }
                 }
                 if (lane == 0u) n_events += (unsigned long long)(e_end - b);
             }
         }
-        __syncthreads();                                      // deliveries land before the next slot is read
+        // deliveries must land before the next slot is read: arrive now, wait after the frame work (which touches no ring)
+        cg::cluster_group::arrival_token tok;
+        if (CLUSTER) tok = cluster.barrier_arrive(); else __syncthreads();
         // a5: camera frame
         if (OBS && ++in_frame == p.obs_stride) {
             float z = 0.f;
@@ -717,6 +738,7 @@ gn_resident_kernel(const GnDev p, const uint64_t t0, const uint32_t n_steps, con
             in_frame = 0u;
             ++frame;
         }
+        if (CLUSTER) cluster.barrier_wait(std::move(tok));
         if (++slot == p.D) slot = 0u;
         if (++raster_row == p.raster_rows) raster_row = 0u;
     }
@@ -894,7 +916,52 @@ cudaError_t gnk_update(const GnDev &p, uint64_t t, bool has_bias, cudaStream_t s
     return cudaLaunchKernelEx(&cfg, gn_update_kernel<false, false>, p, t, slot, raster_row, d_direct);
 }
 
-// Resident mode: one CTA per network for n_steps steps.  Raster rows of these steps are zeroed first (the kernel ORs bits
+typedef void (*ResidentKernel)(const GnDev, const uint64_t, const uint32_t, const uint32_t);
+
+static cudaError_t resident_config(ResidentKernel k, const GnDev &p, cudaLaunchConfig_t &cfg, cudaLaunchAttribute *attr)
+{
+    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.res_smem);
+    if (e == cudaSuccess && p.res_cluster > 8u) e = cudaFuncSetAttribute(k, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+    cfg = cudaLaunchConfig_t{};
+    cfg.gridDim = dim3(p.n_networks * p.res_cluster);
+    cfg.blockDim = dim3(p.res_threads);
+    cfg.dynamicSmemBytes = p.res_smem;
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = p.res_cluster;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = p.res_cluster > 1u ? 1 : 0;
+    return e;
+}
+
+static cudaError_t resident_launch(ResidentKernel k, const GnDev &p, uint64_t t0, uint32_t n_steps, bool raster_on, cudaStream_t st)
+{
+    cudaLaunchConfig_t cfg;
+    cudaLaunchAttribute attr[1];
+    cudaError_t e = resident_config(k, p, cfg, attr);
+    if (e != cudaSuccess) return e;
+    cfg.stream = st;
+    return cudaLaunchKernelEx(&cfg, k, p, t0, n_steps, raster_on ? 1u : 0u);
+}
+
+// Can the device co-schedule a cluster of p.res_cluster CTAs of the resident kernel at all?
+cudaError_t gnk_resident_cluster_ok(const GnDev &p, bool *ok)
+{
+    *ok = true;
+    if (p.res_cluster <= 1u) return cudaSuccess;
+    ResidentKernel k = p.packed ? gn_resident_kernel<false, false, true, true> : gn_resident_kernel<false, false, false, true>;
+    cudaLaunchConfig_t cfg;
+    cudaLaunchAttribute attr[1];
+    cudaError_t e = resident_config(k, p, cfg, attr);
+    int n = 0;
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveClusters(&n, k, &cfg);
+    *ok = (e == cudaSuccess && n > 0);
+    cudaGetLastError();
+    return cudaSuccess;
+}
+
+// Resident mode: one CTA (or one cluster) per network for n_steps steps.  Raster rows of these steps are zeroed first (the kernel ORs bits
 // into words that may straddle two networks); the caller keeps n_steps <= raster_rows when a raster is kept.
 cudaError_t gnk_resident(const GnDev &p, uint64_t t0, uint32_t n_steps, bool has_bias, bool raster_on, cudaStream_t st)
 {
@@ -906,14 +973,11 @@ cudaError_t gnk_resident(const GnDev &p, uint64_t t0, uint32_t n_steps, bool has
             e = cudaMemsetAsync(p.raster, 0, (size_t)(n_steps - first) * p.words_pad * 4, st);
         if (e != cudaSuccess) return e;
     }
-    const size_t smem = p.res_smem;
     const bool obs = p.obs_stride != 0u;
 #define GN_RES_LAUNCH(O, B, P)                                                                                  \
     do {                                                                                                        \
-        cudaError_t e_ = cudaFuncSetAttribute(gn_resident_kernel<O, B, P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
-        if (e_ != cudaSuccess) return e_;                                                                       \
-        gn_resident_kernel<O, B, P><<<p.n_networks, p.res_threads, smem, st>>>(p, t0, n_steps, raster_on ? 1u : 0u); \
-        return cudaGetLastError();                                                                              \
+        if (p.res_cluster > 1u) return resident_launch(gn_resident_kernel<O, B, P, true>, p, t0, n_steps, raster_on, st);  \
+        return resident_launch(gn_resident_kernel<O, B, P, false>, p, t0, n_steps, raster_on, st);                \
     } while (0)
     if (p.packed) {
         if (obs && has_bias) GN_RES_LAUNCH(true, true, true);

@@ -202,6 +202,9 @@ def test_config5_full_size_batched(gn):
     (5, 1000, 6, 1200, 400, "RING"), (5, 1000, 6, 1200, 400, "RESIDENT"),
     (5, 333, 9, 900, 900, "RESIDENT"),          # network starts at multiples of 333: no 4- or 32-alignment
     (2, 1_024, None, 800, 250, "RESIDENT"),     # one network filling the CTA, E/I classes, observation every step
+    (2, 3_000, None, 800, 250, "RESIDENT"),     # a 3-CTA cluster: events cross CTAs through distributed shared memory
+    (2, None, None, 1000, 500, "RESIDENT"),     # config 2 at full size: a 10-CTA cluster
+    (5, 2_500, 5, 600, 300, "RESIDENT"),        # five 3-CTA clusters
 ])
 def test_small_networks_every_delivery_mode(gn, k, n, nb, steps, chunk, mode):
     net, cfg = make_config(k, n=n, n_networks=nb)
@@ -243,7 +246,7 @@ def test_resident_mode_ragged_batch_bias_and_short_raster_window(gn):
 
 
 def test_resident_mode_refused_when_a_network_does_not_fit(gn):
-    net, cfg = make_config(2, n=1_500)                                   # 1,500 vertices in one network
+    net, cfg = make_config(2, n=17_000)                                  # more than 16 CTAs x 1,024 vertices
     with pytest.raises(gn.GnError) as ei:
         _make(gn, net, cfg, 10, delivery_mode=gn.GN_DELIVER_RESIDENT)
     assert ei.value.code == gn.GN_E_INVALID_ARG
