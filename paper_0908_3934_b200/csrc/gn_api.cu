@@ -378,6 +378,8 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
             d.queue_mode = 0u;
         }
     }
+    // ring mode on a small network: one kernel per step (the update delivers), bound by launch latency not work
+    d.fused = (!d.resident && !d.queue_mode && Npad <= (1u << 18)) ? 1u : 0u;
     if (E) {
         GN_CREATE_CUDA(gnk_quantise(d, E, chk_d, st));
         if (!delays) GN_CREATE_CUDA(gnk_delays_from_positions(d, pos_d, cfg->dim, cfg->speed, st));
@@ -541,11 +543,13 @@ int gn_step(gn_net *net, uint64_t n_steps)
         net->launches++;
         net->t = t + 1;
         const bool group_end = d.queue_mode && (t % G == G - 1u);
-        if (!prof && (!d.queue_mode || group_end)) {
+        if (!prof && !d.fused && (!d.queue_mode || group_end)) {
             GN_CUDA(net, cudaEventRecord(net->ev_update, s_upd));
             GN_CUDA(net, cudaStreamWaitEvent(s_del, net->ev_update, 0));
         }
-        if (!d.queue_mode) {
+        if (d.fused) {
+            // the update kernel delivered everything itself
+        } else if (!d.queue_mode) {
             if (prof && (rc = prof_mark(net, 1))) return rc;  // also counts the step's spikes: runs even with E = 0
             GN_CUDA(net, gnk_deliver(d, t, s_del));
             net->launches++;

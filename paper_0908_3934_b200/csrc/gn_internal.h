@@ -50,6 +50,7 @@ struct GnDev {
     uint8_t *s_dly;          // [E] delay of s_edge[e]
     uint8_t *min_dly;        // [Npad] smallest out-delay of every vertex (255: no out-edge)
     uint32_t packed;
+    uint32_t fused;          // ring mode on a small network: the update kernel delivers every event itself (no delivery kernel)
     // resident mode (gn_resident_kernel): every network in one CTA
     uint32_t resident;       // 0 / 1
     uint32_t n_networks;

@@ -81,8 +81,8 @@ __device__ __forceinline__ bool vertex_step(const GnClassDev &q, const float dt,
 
 // ---- a1 + a2 + a3 (+ calcium of a5) ---------------------------------------------------------------
 // Thread g owns vertices 4g .. 4g+3 (128-bit SoA loads); a warp owns 128 vertices = 4 raster words.
-template <bool OBS, bool BIAS>
-__global__ void __launch_bounds__(kUpdateThreads, 8)
+template <bool OBS, bool BIAS, bool FUSED>
+__global__ void __launch_bounds__(kUpdateThreads, FUSED ? 4 : 8)
 gn_update_kernel(const GnDev p, const uint64_t t, const uint32_t slot, const uint32_t raster_row,
                  const uint32_t d_direct)
 {
@@ -175,7 +175,34 @@ gn_update_kernel(const GnDev p, const uint64_t t, const uint32_t slot, const uin
     // sent by the vertex that fired (rows are sorted by delay: such edges lead the row).  Ring mode: delay 1
     // (d_direct = 2), so that deliver(t) may overlap update(t+1).  Queue mode: every delay that lands in the
     // group being consumed or in the next one (d_direct = 2G - r), so that routing runs once per group.
-    if (nib) {
+    // FUSED (ring mode, small networks: a step is bound by launch latency, not by work): the whole of a4 happens here,
+    // warp-cooperatively -- every fired vertex of the warp in turn, lanes over its row -- and there is no delivery kernel.
+    if (FUSED) {
+        unsigned long long events = 0ull;
+        uint32_t spikes = 0u;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            uint32_t m = __ballot_sync(0xFFFFFFFFu, (nib >> q) & 1u);
+            spikes += __popc(m);
+            while (m) {
+                const uint32_t src = (j0 - 4u * lane) + 4u * ((uint32_t)__ffs(m) - 1u) + (uint32_t)q;
+                m &= m - 1u;
+                const uint32_t beg = p.row[src], end = p.row[src + 1];
+                for (uint32_t e = beg + lane; e < end; e += 32u) {
+                    const uint2 ev = p.s_edge[e];
+                    const uint32_t d = p.packed ? ev.x >> 24 : (uint32_t)p.s_dly[e];
+                    uint32_t s1 = slot + d;
+                    if (s1 >= p.D) s1 -= p.D;
+                    atomicAdd(p.ring + (size_t)s1 * p.Npad + (p.packed ? ev.x & 0xFFFFFFu : ev.x), (int32_t)ev.y);
+                }
+                events += (unsigned long long)(end - beg);
+            }
+        }
+        if (lane == 0 && spikes) {
+            atomicAdd(&p.counters[1], (unsigned long long)spikes);
+            atomicAdd(&p.counters[2], events);
+        }
+    } else if (nib) {
         const uchar4 md4 = *reinterpret_cast<const uchar4 *>(p.min_dly + j0);   // smallest out-delay of each vertex
         const uint32_t md[4] = {md4.x, md4.y, md4.z, md4.w};
 #pragma unroll
@@ -910,10 +937,14 @@ cudaError_t gnk_update(const GnDev &p, uint64_t t, bool has_bias, cudaStream_t s
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    if (obs && has_bias) return cudaLaunchKernelEx(&cfg, gn_update_kernel<true, true>, p, t, slot, raster_row, d_direct);
-    if (obs) return cudaLaunchKernelEx(&cfg, gn_update_kernel<true, false>, p, t, slot, raster_row, d_direct);
-    if (has_bias) return cudaLaunchKernelEx(&cfg, gn_update_kernel<false, true>, p, t, slot, raster_row, d_direct);
-    return cudaLaunchKernelEx(&cfg, gn_update_kernel<false, false>, p, t, slot, raster_row, d_direct);
+#define GN_UPD(O, B)                                                                                              \
+    return p.fused ? cudaLaunchKernelEx(&cfg, gn_update_kernel<O, B, true>, p, t, slot, raster_row, d_direct)       \
+                   : cudaLaunchKernelEx(&cfg, gn_update_kernel<O, B, false>, p, t, slot, raster_row, d_direct)
+    if (obs && has_bias) GN_UPD(true, true);
+    if (obs) GN_UPD(true, false);
+    if (has_bias) GN_UPD(false, true);
+    GN_UPD(false, false);
+#undef GN_UPD
 }
 
 typedef void (*ResidentKernel)(const GnDev, const uint64_t, const uint32_t, const uint32_t);
