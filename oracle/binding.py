@@ -13,8 +13,8 @@ _SO = os.path.join(_HERE, "libgn_oracle.so")
 _lib = None
 
 CLASS_FIELDS = ("a", "b", "c_reset", "d", "k2", "k1", "k0", "v_peak", "tau_syn_ms",
-                "refractory_ms", "drive_rate_hz", "drive_kick")
-V, W, R, CA = 0, 1, 2, 3
+                "refractory_ms", "drive_rate_hz", "drive_kick", "psc_alpha")
+V, W, R, CA, P = 0, 1, 2, 3, 4
 
 
 def build_lib(force: bool = False) -> str:
@@ -70,7 +70,8 @@ def _p(a):
 
 
 def class_table(classes) -> np.ndarray:
-    return np.array([[c[f] for f in CLASS_FIELDS] for c in classes], dtype=np.float32)
+    # psc_alpha (0 = exponential PSC, eq. 26; 1 = alpha-function, eq. 27-30) may be omitted: 0
+    return np.array([[c.get(f, 0.0) if f == "psc_alpha" else c[f] for f in CLASS_FIELDS] for c in classes], dtype=np.float32)
 
 
 class Oracle:

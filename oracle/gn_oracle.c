@@ -19,6 +19,9 @@
  *                reset (eq. 24) and the PSC term +r(t) (eq. 28);
  *                absolute refractory hold (reading #6)
  *   4. PSC       r' = r (1 - dt/tau_s) + I                               PAPER.md:283-286 eq. 26
+ *                or, for a class with psc_alpha != 0, the alpha-function of PAPER.md:288-312
+ *                eq. 27, 29, 30 with a = 1/tau_s:  r' = r + dt p,  p' = p + dt (-a^2 r - 2a p) + I
+ *                (the arriving weight is an impulse on p: eq. 27's p(t+) = p(t) + w, reading #4)
  *   5. calcium   c' = c (1 - dt/tau_c) + ca_jump * fired                 PAPER.md:364 H_c
  *   6. record    raster[t][j] = fired; deliver: every out-edge (j->m, w_fx, delay) of a fired j
  *                adds w_fx to ring[(t + delay) mod D][m]
@@ -32,7 +35,8 @@
  * Delivery, the ring, the drive decision and the raster are pure integer in both modes.
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): Philox known-answer vectors; fixed points and
- * closed forms of the update; geometric decay of r and c; chain arrival steps; event-count and
+ * closed forms of the update; geometric decay of r and c; the alpha-function PSC against the matrix
+ * power of its 2x2 Euler map, its exact discrete integral w tau^2 and w t e^(-at); chain arrival steps; event-count and
  * fixed-point-mass conservation; the pure-Python pull definition (oracle/pull_definition.py) on
  * <= 10-node graphs; the implementation-free ring-content definition; noise statistics.
  * Parity unpinned: none of the functions below; the chaotic tail beyond the first fp32/fp64
@@ -152,11 +156,14 @@ uint32_t orc_refractory_steps(float refractory_ms, float dt_ms)
  * ---------------------------------------------------------------------------------------- */
 typedef struct {
     /* as given (fp32 at the boundary) */
-    float a, b, c_reset, d, k2, k1, k0, v_peak, tau_syn_ms, refractory_ms, drive_rate_hz, drive_kick;
+    float a, b, c_reset, d, k2, k1, k0, v_peak, tau_syn_ms, refractory_ms, drive_rate_hz, drive_kick, psc_alpha;
     /* derived */
     int direct;          /* tau_syn_ms <= 0: arriving weight jumps V itself */
+    int alpha;           /* psc_alpha != 0: alpha-function PSC (eq. 27, 29, 30) instead of the exponential one (eq. 26) */
     double keep_s;       /* 1 - dt/tau_s */
     float keep_s_f;
+    double a2, two_a;    /* alpha-function: a^2 and 2a with a = 1/tau_s (per ms) */
+    float a2_f, two_a_f;
     uint32_t R;          /* refractory steps */
     uint32_t drive_thr;
     int64_t kick_fx;
@@ -175,8 +182,8 @@ typedef struct orc_net {
     uint8_t *cls;       /* [n] */
     float *bias;        /* [n] or NULL */
     /* state; mode 0 uses the double arrays, mode 1 the float arrays */
-    double *V, *W, *r, *c, *acc;
-    float *Vf, *Wf, *rf, *cf, *accf;
+    double *V, *W, *r, *p, *c, *acc;
+    float *Vf, *Wf, *rf, *pf, *cf, *accf;
     uint32_t *refr;
     int64_t *ring;      /* [D][n] */
     int64_t *consumed;  /* [n] I_fx (kick included) consumed by the last step */
@@ -202,14 +209,14 @@ void orc_destroy(orc_net *o)
     if (!o) return;
     free(o->cls_tab); free(o->row); free(o->tgt); free(o->w_fx); free(o->delay); free(o->cls);
     free(o->bias); free(o->V); free(o->W); free(o->r); free(o->c); free(o->acc);
-    free(o->Vf); free(o->Wf); free(o->rf); free(o->cf); free(o->accf);
+    free(o->Vf); free(o->Wf); free(o->rf); free(o->pf); free(o->cf); free(o->accf); free(o->p);
     free(o->refr); free(o->ring); free(o->consumed); free(o->fired); free(o->raster); free(o->trace);
     free(o);
 }
 
 /*
- * class_params: [n_classes][12] floats in the order
- *   a, b, c_reset, d, k2, k1, k0, v_peak, tau_syn_ms, refractory_ms, drive_rate_hz, drive_kick.
+ * class_params: [n_classes][13] floats in the order
+ *   a, b, c_reset, d, k2, k1, k0, v_peak, tau_syn_ms, refractory_ms, drive_rate_hz, drive_kick, psc_alpha.
  * delays: [E] steps, or NULL => eq. 25 from positions and speed.
  * Returns NULL on a malformed graph (row offsets, target range, delay outside [1, D-1]).
  * Initial state (reading #15): V = -70, W = b*V, r = c = 0, refr = 0, ring zero.
@@ -241,6 +248,7 @@ orc_net *orc_create(uint32_t n, uint32_t dim, uint64_t E, uint32_t D, float dt_m
     o->V = (double *)calloc(n1, sizeof(double)); o->W = (double *)calloc(n1, sizeof(double));
     o->r = (double *)calloc(n1, sizeof(double)); o->c = (double *)calloc(n1, sizeof(double));
     o->acc = (double *)calloc(n1, sizeof(double));
+    o->p = (double *)calloc(n1, sizeof(double)); o->pf = (float *)calloc(n1, sizeof(float));
     o->Vf = (float *)calloc(n1, sizeof(float)); o->Wf = (float *)calloc(n1, sizeof(float));
     o->rf = (float *)calloc(n1, sizeof(float)); o->cf = (float *)calloc(n1, sizeof(float));
     o->accf = (float *)calloc(n1, sizeof(float));
@@ -249,14 +257,22 @@ orc_net *orc_create(uint32_t n, uint32_t dim, uint64_t E, uint32_t D, float dt_m
         memcpy(o->bias, bias, (size_t)n * sizeof(float));
     }
     for (uint32_t k = 0; k < n_classes; ++k) {
-        const float *p = class_params + 12 * k;
+        const float *p = class_params + 13 * k;
         orc_class *q = &o->cls_tab[k];
         q->a = p[0]; q->b = p[1]; q->c_reset = p[2]; q->d = p[3];
         q->k2 = p[4]; q->k1 = p[5]; q->k0 = p[6]; q->v_peak = p[7];
         q->tau_syn_ms = p[8]; q->refractory_ms = p[9]; q->drive_rate_hz = p[10]; q->drive_kick = p[11];
+        q->psc_alpha = p[12];
         q->direct = !(q->tau_syn_ms > 0.0f);
+        q->alpha = !q->direct && q->psc_alpha != 0.0f;
         q->keep_s = q->direct ? 0.0 : orc_keep(dt_ms, q->tau_syn_ms);
         q->keep_s_f = (float)q->keep_s;
+        if (q->alpha) {      /* a = 1/tau_s: constants formed once in double, rounded once for the fp32-faithful mode */
+            q->a2 = 1.0 / ((double)q->tau_syn_ms * (double)q->tau_syn_ms);
+            q->two_a = 2.0 / (double)q->tau_syn_ms;
+            q->a2_f = (float)q->a2;
+            q->two_a_f = (float)q->two_a;
+        }
         q->R = orc_refractory_steps(q->refractory_ms, dt_ms);
         q->drive_thr = orc_drive_threshold(q->drive_rate_hz, dt_ms);
         q->kick_fx = orc_quantise(q->drive_kick);
@@ -343,7 +359,14 @@ static int orc_vertex_fp64(orc_net *o, uint32_t j, int64_t I_fx)
         Wn = W_euler;
     }
     o->V[j] = Vn; o->W[j] = Wn;
-    if (!q->direct) o->r[j] = fma(q->keep_s, r, I);                        /* eq. 26 */
+    if (q->alpha) {                                                        /* eq. 29-30 (impulse reading #4: p jumps by I) */
+        double pp = o->p[j];
+        double q2 = fma(q->two_a, pp, q->a2 * r);
+        o->r[j] = fma(dt, pp, r);                                          /* H_r = r + dt p */
+        o->p[j] = fma(-dt, q2, pp) + I;                                    /* H_p = p + dt(-a^2 r - 2a p) + arrivals */
+    } else if (!q->direct) {
+        o->r[j] = fma(q->keep_s, r, I);                                    /* eq. 26 */
+    }
     if (o->obs_stride) {
         double cn = fma(o->keep_c, o->c[j], fired ? o->ca_jump : 0.0);     /* H_c */
         o->c[j] = cn;
@@ -380,7 +403,16 @@ static int orc_vertex_fp32(orc_net *o, uint32_t j, int64_t I_fx)
         Wn = W_euler;
     }
     o->Vf[j] = Vn; o->Wf[j] = Wn;
-    if (!q->direct) o->rf[j] = fmaf(q->keep_s_f, r, If);
+    if (q->alpha) {
+        float pp = o->pf[j];
+        float q1 = q->a2_f * r;
+        float q2 = fmaf(q->two_a_f, pp, q1);
+        float p1 = fmaf(-dt, q2, pp);
+        o->rf[j] = fmaf(dt, pp, r);
+        o->pf[j] = p1 + If;
+    } else if (!q->direct) {
+        o->rf[j] = fmaf(q->keep_s_f, r, If);
+    }
     if (o->obs_stride) {
         float cn = fmaf(o->keep_c_f, o->cf[j], fired ? o->ca_jump_f : 0.0f);
         o->cf[j] = cn;
@@ -461,7 +493,7 @@ int orc_step(orc_net *o, uint64_t n_steps, int n_threads)
 }
 
 /* ---- accessors ---------------------------------------------------------------------------- */
-enum { ORC_V = 0, ORC_W = 1, ORC_R = 2, ORC_CA = 3 };
+enum { ORC_V = 0, ORC_W = 1, ORC_R = 2, ORC_CA = 3, ORC_P = 4 };
 
 int orc_get_state(const orc_net *o, int which, double *out)
 {
@@ -471,6 +503,7 @@ int orc_get_state(const orc_net *o, int which, double *out)
         case ORC_W: out[j] = o->mode ? (double)o->Wf[j] : o->W[j]; break;
         case ORC_R: out[j] = o->mode ? (double)o->rf[j] : o->r[j]; break;
         case ORC_CA: out[j] = o->mode ? (double)o->cf[j] : o->c[j]; break;
+        case ORC_P: out[j] = o->mode ? (double)o->pf[j] : o->p[j]; break;
         default: return -1;
         }
     }
@@ -485,6 +518,7 @@ int orc_set_state(orc_net *o, int which, const double *in)
         case ORC_W: o->W[j] = in[j]; o->Wf[j] = (float)in[j]; break;
         case ORC_R: o->r[j] = in[j]; o->rf[j] = (float)in[j]; break;
         case ORC_CA: o->c[j] = in[j]; o->cf[j] = (float)in[j]; break;
+        case ORC_P: o->p[j] = in[j]; o->pf[j] = (float)in[j]; break;
         default: return -1;
         }
     }

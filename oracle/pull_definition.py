@@ -79,6 +79,7 @@ class PullSimulator:
         self.V = [-70.0] * n
         self.W = [self.classes[self.cls[j]]["b"] * -70.0 for j in range(n)]
         self.r = [0.0] * n
+        self.p = [0.0] * n          # second PSC state of the alpha-function (eq. 27)
         self.c = [0.0] * n
         self.refr = [0] * n
         self.raster = []            # raster[t][j]
@@ -92,6 +93,7 @@ class PullSimulator:
             fired_now = [False] * self.n
             consumed = [0] * self.n
             V2, W2, r2, c2, refr2 = self.V[:], self.W[:], self.r[:], self.c[:], self.refr[:]
+            p2 = self.p[:]
             for j in range(self.n):
                 q = self.classes[self.cls[j]]
                 # eq. 30: sum of w_kj * spd(V_k(t - tau_kj)) over in-edges, from the raster history
@@ -118,10 +120,15 @@ class PullSimulator:
                     dV = q["k2"] * V * V + q["k1"] * V + q["k0"] - W + (0.0 if direct else r) + U
                     V2[j] = V + self.dt * dV + (I if direct else 0.0)
                     W2[j] = W_euler
-                if not direct:
+                if not direct and q.get("psc_alpha", 0.0) != 0.0:
+                    a = 1.0 / q["tau_syn_ms"]                      # eq. 29: H_r = r + dt p; eq. 30: H_p with the impulse reading
+                    r2[j] = r + self.dt * self.p[j]
+                    p2[j] = self.p[j] + self.dt * (-a * a * r - 2.0 * a * self.p[j]) + I
+                elif not direct:
                     r2[j] = r * (1.0 - self.dt / q["tau_syn_ms"]) + I
                 c2[j] = self.c[j] * (1.0 - self.dt / self.tau_ca) + (self.ca_jump if fired else 0.0)
                 fired_now[j] = fired
             self.V, self.W, self.r, self.c, self.refr = V2, W2, r2, c2, refr2
+            self.p = p2
             self.raster.append(fired_now)
             self.consumed.append(consumed)

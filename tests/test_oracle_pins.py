@@ -259,6 +259,53 @@ def test_psc_and_calcium_geometric_decay(mode):
         o.step(1)
 
 
+@pytest.mark.parametrize("mode", MODES)
+def test_alpha_function_psc_matrix_power_integral_and_shape(mode):
+    """PAPER.md:288-312 eq. 27, 29, 30 with a = 1/tau_s and the arriving weight as an impulse on p.  One event of
+    weight w consumed at step a leaves (r, p) = (0, w) at a+1 and then (r, p)(a+1+k) = M^k (0, w) with the Euler map
+    M = [[1, dt], [-dt a^2, 1 - 2 a dt]] (numpy matrix power, not the oracle's recurrence); summing the two
+    recurrences gives the EXACT discrete integral  dt * sum_k r_k = w / a^2 = w tau^2; and r tracks the paper's
+    continuous alpha function (w/a) * (a t e^{-a t}) = w t e^{-a t} to O(dt)."""
+    w, delay, tau = 3.25, 7, 2.0
+    net, dl = hand_net(2, [(0, 1, w, delay)])
+    cfg = base_cfg([rs_class(tau_syn_ms=tau, psc_alpha=1.0)])
+    o = Oracle(net, cfg, mode, delays=dl)
+    o.set_state(ob.V, np.array([30.0, -70.0]))
+    o.step(1 + delay)                           # vertex 0 fires at t = 0; the event is consumed at step a = 7; now t = a + 1
+    dt, a = float(np.float32(0.1)), 1.0 / tau
+    M = np.array([[1.0, dt], [-dt * a * a, 1.0 - 2.0 * a * dt]])
+    tol = 1e-12 if mode == "fp64" else 3e-6
+    total, peak_seen = 0.0, 0.0
+    for k in range(600):
+        y = np.linalg.matrix_power(M, k) @ np.array([0.0, w])
+        assert abs(o.state(ob.R)[1] - y[0]) < tol * w and abs(o.state(ob.P)[1] - y[1]) < tol * w, k
+        t_ms = k * dt
+        assert abs(o.state(ob.R)[1] - w * t_ms * math.exp(-a * t_ms)) < 0.03 * w       # O(dt) from the continuous curve
+        total += o.state(ob.R)[1] * dt
+        peak_seen = max(peak_seen, o.state(ob.R)[1])
+        assert o.state(ob.R)[0] == 0.0 and o.state(ob.P)[0] == 0.0                     # the source received nothing
+        o.step(1)
+    assert abs(total - w * tau * tau) < (1e-9 if mode == "fp64" else 1e-4) * w * tau * tau
+    assert abs(peak_seen - w / (a * math.e)) < 0.03 * w                                # peak w/(a e) at t = 1/a
+
+
+def test_alpha_function_psc_in_the_pull_definition():
+    """The ring simulator and the pure-Python eq.-30 evaluation agree on a small graph with alpha-function classes."""
+    rng = np.random.default_rng(4)
+    edges = [(i, j, float(rng.uniform(-4, 9)), int(rng.integers(1, 9))) for i in range(7) for j in range(7)
+             if i != j and rng.random() < 0.5]
+    net, dl = hand_net(7, edges)
+    cfg = base_cfg([rs_class(tau_syn_ms=1.5, psc_alpha=1.0, drive_rate_hz=400.0, drive_kick=40.0)], ring_slots=9)
+    o = Oracle(net, cfg, "fp64", delays=dl)
+    q = pd.PullSimulator(net, cfg, delays=dl)
+    o.step(400)
+    q.step(400)
+    np.testing.assert_array_equal(o.raster_bool(0, 400), np.array(q.raster, dtype=bool))
+    assert o.counters()["spikes"] > 0
+    np.testing.assert_allclose(o.state(ob.R), q.r, rtol=1e-9, atol=1e-9)
+    np.testing.assert_allclose(o.state(ob.P), q.p, rtol=1e-9, atol=1e-9)
+
+
 @pytest.mark.parametrize("direct", (True, False))
 @pytest.mark.parametrize("mode", MODES)
 def test_chain_arrival_steps(mode, direct):
