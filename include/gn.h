@@ -7,7 +7,8 @@
  *   y_j(t + dt) = H_j( y_j(t), Y_j(t), u_j(t), Theta_j )                     :68-71  eq. 5
  *
  * with  y_j = {V, W, r, c} an Izhikevich simple-model vertex with hard reset (:227-229 eq. 24,
- * :303 eq. 28), an exponential post-synaptic current (:283-286 eq. 26) and a calcium state
+ * :303 eq. 28), an exponential (:283-286 eq. 26) or alpha-function (:288-312 eq. 27-30, state p)
+ * post-synaptic current and a calcium state
  * (:364 H_c);  Y_j(t) the delayed, weighted spikes of the other vertices,
  * sum_k w_kj spd(V_k(t - tau_kj)) (:311 eq. 30, spd = [V >= V_peak] :316 eq. 31) with
  * tau_kj = |x_k - x_j| / s (:251 eq. 25);  u_j(t) the external control (:77-79 eq. 7); and the
@@ -63,6 +64,8 @@ typedef struct {
     float refractory_ms;    /* absolute refractory hold after a spike (:259, reading #6)             */
     float drive_rate_hz;    /* Bernoulli(rate*dt) kick per step from the counter generator           */
     float drive_kick;       /* kick weight, injected like an arriving event (reading #12)            */
+    float psc_alpha;        /* 0: exponential PSC (eq. 26).  != 0: alpha-function PSC (:288-312 eq. 27,  */
+                            /* 29, 30), a = 1/tau_syn_ms: r <- r + dt p, p <- p + dt(-a^2 r - 2a p) + I   */
 } gn_class_params;
 
 typedef struct {
@@ -124,7 +127,8 @@ enum {
                       /*                 step (reading it first routes any step whose events are pending)  */
     GN_DELAYS = 8,    /* uint8  [E]      per-edge delay in steps (as given, or eq. 25)               */
     GN_WEIGHTS_FX = 9,/* int32  [E]      per-edge weight, rint(w * 2^16)                             */
-    GN_BIAS = 10      /* float  [N]      user control U_j (write only through gn_write_state)        */
+    GN_BIAS = 10,     /* float  [N]      user control U_j (write only through gn_write_state)        */
+    GN_P = 11         /* float  [N]      second PSC state p of the alpha-function (zero for other classes) */
 };
 
 /* Bytes of device workspace gn_create needs for this configuration.
@@ -165,7 +169,7 @@ int gn_step(gn_net *net, uint64_t n_steps);
  * dst is device memory, written asynchronously on the stream.  Errors: INVALID_ARG, CUDA. */
 int gn_read_state(gn_net *net, int which, void *dst, size_t dst_bytes, int dst_is_device);
 
-/* Overwrite V, W, R, CA (float [N]), REFR (uint8 [N]) or BIAS (float [N]; enables the bias term).
+/* Overwrite V, W, R, P, CA (float [N]), REFR (uint8 [N]) or BIAS (float [N]; enables the bias term).
  * For checkpoint/restore and controlled experiments (PAPER.md:77-79 user control). */
 int gn_write_state(gn_net *net, int which, const void *src, size_t src_bytes, int src_is_device);
 

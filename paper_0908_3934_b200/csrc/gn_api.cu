@@ -16,7 +16,7 @@ namespace {
 thread_local char g_create_error[256] = "";
 
 struct Layout {
-    size_t V, W, r, c, acc, bias, refr, cls, ring, row, tgt, wfx, dly, counters, q_count;
+    size_t V, W, r, p2, c, acc, bias, refr, cls, ring, row, tgt, wfx, dly, counters, q_count;
     size_t s_edge, s_dly, min_dly, q_seg, queue;
     size_t raster, trace, scratch_row64, scratch_abs, scratch_pos, scratch_net, scratch_chk, total;
 };
@@ -81,7 +81,7 @@ Layout make_layout(const gn_config *cfg)
     Layout L{};
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off = align256(off + bytes); return o; };
-    L.V = take(Npad * 4); L.W = take(Npad * 4); L.r = take(Npad * 4);
+    L.V = take(Npad * 4); L.W = take(Npad * 4); L.r = take(Npad * 4); L.p2 = take(Npad * 4);
     L.c = take(obs ? Npad * 4 : 0); L.acc = take(obs ? Npad * 4 : 0);
     L.bias = take(Npad * 4);
     L.refr = take(Npad); L.cls = take(Npad);
@@ -233,7 +233,7 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
     d.ca_jump = cfg->ca_jump;
     d.obs_gain = cfg->obs_gain; d.obs_offset = cfg->obs_offset; d.obs_sigma = cfg->obs_sigma;
     d.inv_stride = cfg->obs_stride ? (float)(1.0 / (double)cfg->obs_stride) : 0.0f;
-    d.V = (float *)(ws + L.V); d.W = (float *)(ws + L.W); d.r = (float *)(ws + L.r);
+    d.V = (float *)(ws + L.V); d.W = (float *)(ws + L.W); d.r = (float *)(ws + L.r); d.p2 = (float *)(ws + L.p2);
     d.c = cfg->obs_stride ? (float *)(ws + L.c) : nullptr;
     d.acc = cfg->obs_stride ? (float *)(ws + L.acc) : nullptr;
     d.bias = (float *)(ws + L.bias);
@@ -267,6 +267,10 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
         q.k2 = c.k2; q.k1 = c.k1; q.k0 = c.k0; q.v_peak = c.v_peak;
         q.direct = !(c.tau_syn_ms > 0.0f);
         q.keep_s = q.direct ? 0.0f : (float)(1.0 - (double)cfg->dt_ms / (double)c.tau_syn_ms);
+        q.alpha = (!q.direct && c.psc_alpha != 0.0f) ? 1u : 0u;       // alpha-function PSC, a = 1/tau_syn
+        q.a2 = q.alpha ? (float)(1.0 / ((double)c.tau_syn_ms * (double)c.tau_syn_ms)) : 0.0f;
+        q.two_a = q.alpha ? (float)(2.0 / (double)c.tau_syn_ms) : 0.0f;
+        if (q.alpha) d.any_alpha = 1u;
         const double R = nearbyint((double)c.refractory_ms / (double)cfg->dt_ms);
         if (!(R >= 0.0) || R > 255.0) {
             delete net;
@@ -635,6 +639,7 @@ int gn_read_state(gn_net *net, int which, void *dst, size_t dst_bytes, int dst_i
     case GN_V: src = d.V; need = N * 4; break;
     case GN_W: src = d.W; need = N * 4; break;
     case GN_R: src = d.r; need = N * 4; break;
+    case GN_P: src = d.p2; need = N * 4; break;
     case GN_CA:
         if (!d.c) return set_err(net, GN_E_INVALID_ARG, "calcium is not maintained when obs_stride == 0");
         src = d.c; need = N * 4; break;
@@ -678,6 +683,7 @@ int gn_write_state(gn_net *net, int which, const void *src, size_t src_bytes, in
     case GN_V: dst = d.V; break;
     case GN_W: dst = d.W; break;
     case GN_R: dst = d.r; break;
+    case GN_P: dst = d.p2; break;
     case GN_CA:
         if (!d.c) return set_err(net, GN_E_INVALID_ARG, "calcium is not maintained when obs_stride == 0");
         dst = d.c; break;

@@ -8,7 +8,7 @@
 #include "../../include/gn.h"
 
 // Per-class constants, derived once on the host in double and rounded once (DESIGN.md
-// "Arithmetic contract"); 13 words each, staged into shared memory by the update kernel.
+// "Arithmetic contract"); kClassWords words each, staged into shared memory by the update kernel.
 struct GnClassDev {
     float a, b, c_reset, d;
     float k2, k1, k0, v_peak;
@@ -17,8 +17,13 @@ struct GnClassDev {
     uint32_t R;          // refractory steps, round(refractory_ms / dt)
     uint32_t drive_thr;  // floor(rate * dt * 1e-3 * 2^32)
     int32_t kick_fx;     // rint(kick * 2^16)
+    uint32_t alpha;      // alpha-function PSC (eq. 27, 29, 30) instead of the exponential one
+    float a2, two_a;     // (float)(1/tau_s^2), (float)(2/tau_s)
+    uint32_t pad_;       // 17 words on purpose: a 16-byte-aligned table invites 128-bit shared-memory loads of whole
+                         // rows, which costs the 32-register update kernel four live registers per vertex
 };
-static_assert(sizeof(GnClassDev) == 13 * 4, "GnClassDev must stay 13 words");
+constexpr uint32_t kClassWords = 17;
+static_assert(sizeof(GnClassDev) == kClassWords * 4, "GnClassDev must stay kClassWords words");
 
 // Everything a kernel needs, passed by value (kernel parameter space).
 struct GnDev {
@@ -33,6 +38,8 @@ struct GnDev {
     float obs_gain, obs_offset, obs_sigma, inv_stride;
     // vertex state, SoA, each Npad long
     float *V, *W, *r, *c, *acc, *bias;
+    float *p2;               // second PSC state of alpha-function classes (touched only when any_alpha)
+    uint32_t any_alpha;
     uint8_t *refr, *cls;
     // delay ring [D][Npad], int32 fixed point 2^-16
     int32_t *ring;

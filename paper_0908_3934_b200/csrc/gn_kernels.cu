@@ -45,9 +45,9 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
 
 // ---- one vertex, one step: eq. 24 + :303 eq. 28 + :283-286 eq. 26 ------------
 // Reads the state at t, writes the state at t+1, returns spd(V(t)) gated by refractoriness.
-template <bool BIAS>
+template <bool BIAS, bool ALPHA>
 __device__ __forceinline__ bool vertex_step(const GnClassDev &q, const float dt, const int32_t I_fx,
-                                            const float U, float &V, float &W, float &r, uint32_t &refr)
+                                            const float U, float &V, float &W, float &r, uint32_t &refr, float &pp)
 {
     const float If = __fmul_rn(__int2float_rn(I_fx), 0x1p-16f);
     const bool fired = (refr == 0u) && (V >= q.v_peak);                  // eq. 31 (>=)
@@ -73,7 +73,15 @@ __device__ __forceinline__ bool vertex_step(const GnClassDev &q, const float dt,
         if (q.direct) Vn = __fadd_rn(Vn, If);
         Wn = W_euler;
     }
-    if (!q.direct) r = __fmaf_rn(q.keep_s, r, If);                       // eq. 26
+    if (ALPHA && q.alpha) {                                              // alpha-function PSC, eq. 27, 29, 30
+        const float q1 = __fmul_rn(q.a2, r);
+        const float q2 = __fmaf_rn(q.two_a, pp, q1);
+        const float p1 = __fmaf_rn(-dt, q2, pp);
+        r = __fmaf_rn(dt, pp, r);                                        // H_r = r + dt p
+        pp = __fadd_rn(p1, If);                                          // H_p = p + dt(-a^2 r - 2a p) + arrivals
+    } else if (!q.direct) {
+        r = __fmaf_rn(q.keep_s, r, If);                                  // eq. 26
+    }
     V = Vn;
     W = Wn;
     return fired;
@@ -81,8 +89,8 @@ __device__ __forceinline__ bool vertex_step(const GnClassDev &q, const float dt,
 
 // ---- a1 + a2 + a3 (+ calcium of a5) ---------------------------------------------------------------
 // Thread g owns vertices 4g .. 4g+3 (128-bit SoA loads); a warp owns 128 vertices = 4 raster words.
-template <bool OBS, bool BIAS, bool FUSED>
-__global__ void __launch_bounds__(kUpdateThreads, FUSED ? 4 : 8)
+template <bool OBS, bool BIAS, bool FUSED, bool ALPHA>
+__global__ void __launch_bounds__(kUpdateThreads, (FUSED || ALPHA) ? 4 : 8)
 gn_update_kernel(const GnDev p, const uint64_t t, const uint32_t slot, const uint32_t raster_row,
                  const uint32_t d_direct)
 {
@@ -90,7 +98,7 @@ gn_update_kernel(const GnDev p, const uint64_t t, const uint32_t slot, const uin
     // Programmatic dependent launch: the next step's update may start launching now; its prologue (class table,
     // Philox words -- nothing a previous kernel wrote) then overlaps this kernel's tail (see griddepcontrol.wait below).
     asm volatile("griddepcontrol.launch_dependents;");
-    if (threadIdx.x < p.n_classes * 13u)
+    if (threadIdx.x < p.n_classes * kClassWords)
         reinterpret_cast<uint32_t *>(s_cls)[threadIdx.x] = reinterpret_cast<const uint32_t *>(p.cls_tab)[threadIdx.x];
     __syncthreads();
 
@@ -132,6 +140,11 @@ gn_update_kernel(const GnDev p, const uint64_t t, const uint32_t slot, const uin
         int32_t I[4] = {I4.x, I4.y, I4.z, I4.w};
         float V[4] = {V4.x, V4.y, V4.z, V4.w}, W[4] = {W4.x, W4.y, W4.z, W4.w};
         float r[4] = {r4.x, r4.y, r4.z, r4.w}, U[4] = {U4.x, U4.y, U4.z, U4.w};
+        float pp[4] = {0.f, 0.f, 0.f, 0.f};
+        if (ALPHA) {
+            const float4 p4 = *reinterpret_cast<const float4 *>(p.p2 + j0);
+            pp[0] = p4.x; pp[1] = p4.y; pp[2] = p4.z; pp[3] = p4.w;
+        }
         uint32_t refr[4] = {rf4.x, rf4.y, rf4.z, rf4.w};
 
         uint32_t refr_changed = 0u;
@@ -140,13 +153,14 @@ gn_update_kernel(const GnDev p, const uint64_t t, const uint32_t slot, const uin
             const GnClassDev &k = s_cls[cl[q]];
             if ((kicks >> q) & 1u) I[q] += k.kick_fx;
             const uint32_t refr_old = refr[q];
-            const bool fired = vertex_step<BIAS>(k, p.dt, I[q], U[q], V[q], W[q], r[q], refr[q]) && (j0 + q) < p.N;
+            const bool fired = vertex_step<BIAS, ALPHA>(k, p.dt, I[q], U[q], V[q], W[q], r[q], refr[q], pp[q]) && (j0 + q) < p.N;
             refr_changed |= (refr[q] != refr_old);
             if (fired) nib |= 1u << q;
         }
         *reinterpret_cast<float4 *>(p.V + j0) = make_float4(V[0], V[1], V[2], V[3]);
         *reinterpret_cast<float4 *>(p.W + j0) = make_float4(W[0], W[1], W[2], W[3]);
         *reinterpret_cast<float4 *>(p.r + j0) = make_float4(r[0], r[1], r[2], r[3]);
+        if (ALPHA) *reinterpret_cast<float4 *>(p.p2 + j0) = make_float4(pp[0], pp[1], pp[2], pp[3]);
         if (refr_changed)
             *reinterpret_cast<uchar4 *>(p.refr + j0) = make_uchar4(refr[0], refr[1], refr[2], refr[3]);
         if (OBS) {                                                            // calcium + frame accumulator
@@ -662,12 +676,14 @@ gn_resident_kernel(const GnDev p, const uint64_t t0, const uint32_t n_steps, con
     const uint32_t c_nv = c0 < nv ? min(stride, nv - c0) : 0u;             // vertices of this CTA
     const uint32_t g0 = (v0 + c0) >> 2, n_groups = c_nv ? ((v0 + c0 + c_nv + 3u) >> 2) - g0 : 0u;
 
-    if (i < p.n_classes * 13u) reinterpret_cast<uint32_t *>(s_cls)[i] = reinterpret_cast<const uint32_t *>(p.cls_tab)[i];
+    for (uint32_t q = i; q < p.n_classes * kClassWords; q += stride)   // a CTA may have as few as 32 threads
+        reinterpret_cast<uint32_t *>(s_cls)[q] = reinterpret_cast<const uint32_t *>(p.cls_tab)[q];
     if (i < 3u) s_tot[i] = 0ull;
-    float V = 0.f, W = 0.f, r = 0.f, c = 0.f, acc = 0.f, U = 0.f;
+    float V = 0.f, W = 0.f, r = 0.f, c = 0.f, acc = 0.f, U = 0.f, pp = 0.f;
     uint32_t refr = 0u, cl = 0u;
     if (live) {
         V = p.V[j]; W = p.W[j]; r = p.r[j]; refr = p.refr[j]; cl = p.cls[j];
+        if (p.any_alpha) pp = p.p2[j];
         if (OBS) { c = p.c[j]; acc = p.acc[j]; }
         if (BIAS) U = p.bias[j];
     }
@@ -702,7 +718,7 @@ gn_resident_kernel(const GnDev p, const uint64_t t0, const uint32_t n_steps, con
             if (x < k.drive_thr) { I += k.kick_fx; ++n_kicks; }
         }
         // a2 + a3
-        const bool fired = vertex_step<BIAS>(k, p.dt, I, U, V, W, r, refr) && live;
+        const bool fired = vertex_step<BIAS, true>(k, p.dt, I, U, V, W, r, refr, pp) && live;
         if (OBS) {
             c = __fmaf_rn(p.keep_c, c, fired ? p.ca_jump : 0.0f);            // H_c
             acc = __fadd_rn(acc, c);
@@ -772,6 +788,7 @@ gn_resident_kernel(const GnDev p, const uint64_t t0, const uint32_t n_steps, con
     // back to global memory: the state at t0 + n_steps
     if (live) {
         p.V[j] = V; p.W[j] = W; p.r[j] = r; p.refr[j] = (uint8_t)refr;
+        if (p.any_alpha) p.p2[j] = pp;
         if (OBS) { p.c[j] = c; p.acc[j] = acc; }
     }
     for (uint32_t s = 0; s < p.D; ++s)
@@ -806,6 +823,7 @@ __global__ void gn_init_state_kernel(const GnDev p, GnCheck *chk)
     p.V[j] = -70.0f;                                        // reading #15
     p.W[j] = __fmul_rn(p.cls_tab[k].b, -70.0f);
     p.r[j] = 0.0f;
+    p.p2[j] = 0.0f;
     p.refr[j] = 0;
     if (p.c) { p.c[j] = 0.0f; p.acc[j] = 0.0f; }
 }
@@ -938,8 +956,13 @@ cudaError_t gnk_update(const GnDev &p, uint64_t t, bool has_bias, cudaStream_t s
     cfg.attrs = attr;
     cfg.numAttrs = 1;
 #define GN_UPD(O, B)                                                                                              \
-    return p.fused ? cudaLaunchKernelEx(&cfg, gn_update_kernel<O, B, true>, p, t, slot, raster_row, d_direct)       \
-                   : cudaLaunchKernelEx(&cfg, gn_update_kernel<O, B, false>, p, t, slot, raster_row, d_direct)
+    do {                                                                                                          \
+        if (p.any_alpha)                                                                                          \
+            return p.fused ? cudaLaunchKernelEx(&cfg, gn_update_kernel<O, B, true, true>, p, t, slot, raster_row, d_direct)   \
+                           : cudaLaunchKernelEx(&cfg, gn_update_kernel<O, B, false, true>, p, t, slot, raster_row, d_direct); \
+        return p.fused ? cudaLaunchKernelEx(&cfg, gn_update_kernel<O, B, true, false>, p, t, slot, raster_row, d_direct)      \
+                       : cudaLaunchKernelEx(&cfg, gn_update_kernel<O, B, false, false>, p, t, slot, raster_row, d_direct);    \
+    } while (0)
     if (obs && has_bias) GN_UPD(true, true);
     if (obs) GN_UPD(true, false);
     if (has_bias) GN_UPD(false, true);

@@ -245,6 +245,18 @@ def test_resident_mode_ragged_batch_bias_and_short_raster_window(gn):
     assert o.counters()["delivered"] > 0 and o.counters()["kicks"] > 0
 
 
+def test_resident_mode_tiny_cta_with_many_classes(gn):
+    """A 20-vertex network (one 32-thread CTA) with 8 vertex classes: the class table is larger than the CTA."""
+    rng = np.random.default_rng(8)
+    edges = random_digraph(rng, 20, 0.3, 12)
+    net, dl = hand_net(20, edges, vertex_class=rng.integers(0, 8, 20))
+    classes = [rs_class(a=0.02 + 0.01 * k, d=8.0 - k, drive_rate_hz=300.0 + 50 * k, tau_syn_ms=1.0 + 0.5 * k,
+                        psc_alpha=float(k % 2)) for k in range(8)]
+    cfg = base_cfg(classes, ring_slots=12)
+    g, o, _ = _run_exact(gn, net, cfg, 1500, 500, delays=dl, delivery_mode=gn.GN_DELIVER_RESIDENT)
+    assert o.counters()["spikes"] > 0
+
+
 def test_resident_mode_refused_when_a_network_does_not_fit(gn):
     net, cfg = make_config(2, n=17_000)                                  # more than 16 CTAs x 1,024 vertices
     with pytest.raises(gn.GnError) as ei:
@@ -254,6 +266,46 @@ def test_resident_mode_refused_when_a_network_does_not_fit(gn):
     cfg = dict(cfg, ring_slots=255)
     with pytest.raises(gn.GnError):
         _make(gn, net, cfg, 10, delays=np.ones(net.n_edges, np.uint8), delivery_mode=gn.GN_DELIVER_RESIDENT)
+
+
+# ---- alpha-function PSC (eq. 27, 29, 30) in every delivery mode -----------------------
+def _alpha(cfg, weight_scale_tau=1.0):
+    return dict(cfg, classes=[dict(c, psc_alpha=1.0, tau_syn_ms=c["tau_syn_ms"] * weight_scale_tau) for c in cfg["classes"]])
+
+
+@pytest.mark.parametrize("k,n,nb,steps,chunk,mode", [
+    (2, 3_000, None, 1500, 500, "RING"),        # fused update + delivery
+    (2, 3_000, None, 1500, 500, "RESIDENT"),    # 3-CTA cluster
+    (4, 9_001, None, 1500, 500, "QUEUE"),
+    (4, 9_001, None, 1500, 500, "RING"),
+    (5, 1000, 4, 1000, 500, "RESIDENT"),
+    (3, 300_000, None, 300, 150, "RING"),       # above the fused limit: separate delivery kernel, 4 CTAs/SM update
+])
+def test_alpha_function_psc_bit_exact(gn, k, n, nb, steps, chunk, mode):
+    net, cfg = make_config(k, n=n, n_networks=nb)
+    cfg = _alpha(dict(cfg, obs_stride=0))
+    g, o, _ = _run_exact(gn, net, cfg, steps, chunk, delivery_mode=getattr(gn, "GN_DELIVER_" + mode), threads=8)
+    np.testing.assert_array_equal(gn.gn_read_state(g, gn.GN_P).view(np.uint32),
+                                  o.state(ob.P).astype(np.float32).view(np.uint32))
+    assert o.counters()["spikes"] > 0 and np.abs(o.state(ob.P)).max() > 0
+
+
+def test_alpha_function_mixed_classes_and_state_roundtrip(gn):
+    """One class with the alpha-function, one with the exponential PSC; P is readable / writable."""
+    net, cfg = make_config(2, n=2_000)
+    cl = [dict(cfg["classes"][0], psc_alpha=1.0), dict(cfg["classes"][1], psc_alpha=0.0)]
+    cfg = dict(cfg, classes=cl, obs_stride=0)
+    g = _make(gn, net, cfg, 600, delivery_mode=gn.GN_DELIVER_RING)
+    o = Oracle(net, cfg, "fp32", threads=4)
+    p0 = np.random.default_rng(2).uniform(0, 20, net.n_vertices).astype(np.float32) * (net.vertex_class == 0)
+    gn.gn_write_state(g, gn.GN_P, p0)
+    o.set_state(ob.P, p0.astype(np.float64))
+    gn.gn_step(g, 600)
+    o.step(600)
+    _compare_exact(gn, g, o, 600)
+    pg = gn.gn_read_state(g, gn.GN_P)
+    np.testing.assert_array_equal(pg.view(np.uint32), o.state(ob.P).astype(np.float32).view(np.uint32))
+    assert not pg[net.vertex_class == 1].any() and pg[net.vertex_class == 0].any()
 
 
 def test_queue_mode_reads_inside_a_group_and_odd_step_counts(gn):
