@@ -139,6 +139,8 @@ def run_reference(args):
     t0 = time.time()
     net_in, cfg = make_config(args.config, n=args.n)
     cfg = dict(cfg, obs_stride=0 if args.config == 4 else cfg["obs_stride"])
+    if args.psc_alpha:
+        cfg = dict(cfg, classes=[dict(c, psc_alpha=1.0) for c in cfg["classes"]], name=cfg["name"] + "+alpha_psc")
     log(f"[reference] inputs in {time.time() - t0:.1f} s: N={net_in.n_vertices} E={net_in.n_edges}")
     o = Oracle(net_in, cfg, "fp32", threads=cores)
     t0 = time.time()
@@ -204,6 +206,8 @@ def main():
     ap.add_argument("--sim-steps", type=int, default=100, help="simulated steps per bench step")
     ap.add_argument("--delivery", default="auto", choices=["auto", "ring", "queue"], help="gn_config.delivery_mode")
     ap.add_argument("--queue-group", type=int, default=0, help="gn_config.queue_group (0 = library default)")
+    ap.add_argument("--psc-alpha", action="store_true", help="every class uses the alpha-function PSC (DESIGN.md f-1) "
+                                                              "instead of the config's exponential one: a different workload")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -230,6 +234,8 @@ def main():
     t0 = time.time()
     # replicas only: rank r steps its own independent network of the same recipe
     net_in, cfg = make_config(args.config, n=args.n, seed=rank_seed(args.config, rank))
+    if args.psc_alpha:
+        cfg = dict(cfg, classes=[dict(c, psc_alpha=1.0) for c in cfg["classes"]], name=cfg["name"] + "+alpha_psc")
     N, E = net_in.n_vertices, net_in.n_edges
     log(f"[rank {rank}] inputs in {time.time() - t0:.1f} s: N={N} E={E} mean out-degree {E / N:.1f}")
     obs = int(cfg["obs_stride"])
