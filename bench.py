@@ -296,14 +296,20 @@ def main():
     gn.gn_profile(g, False)
     cp1 = counters(g)
     peak, peak_src = peaks()
-    queue_mode = kn[3] > 0
-    names = ["gn_update_kernel (a1-a3)", "gn_route_kernel (a4, queue mode)" if queue_mode else "gn_deliver_kernel (a4)",
-             "gn_observe_kernel (a5)", "gn_fold_kernel (a4, queue mode)"]
+    queue_mode = 0 < kn[1] < kn[0]      # queue mode delivers once per slot group, ring mode every step
+    resident = kn[1] == 0 and kn[0] < sim_steps
+    names = ["gn_resident_kernel (a1-a5, one CTA or cluster per network)" if resident else
+             "gn_update_kernel (a1-a3 + a4 fused)" if kn[1] == 0 else "gn_update_kernel (a1-a3)",
+             "gn_route_kernel (a4: routing + folding warps)" if queue_mode else "gn_deliver_kernel (a4)",
+             "gn_observe_kernel (a5)", "gn_fold_kernel (a4, read-back only)"]
     p_events, p_spikes = cp1[2] - cp0[2], cp1[1] - cp0[1]
-    # algorithmic bytes per launch: ring mode, one kernel does the whole 17 B event;
-    # queue mode splits it: routing reads the 9 B edge record (+12 B per fired source), folding does the 8 B ring RMW
-    kbytes = [N * (UPDATE_BYTES_PER_VERTEX + (UPDATE_BYTES_PER_VERTEX_OBS if obs else 0.0)),
-              (p_events * (9.0 if queue_mode else EVENT_BYTES) + p_spikes * SOURCE_BYTES) / max(int(kn[1]), 1),
+    # algorithmic bytes per launch: 17 B per event (+12 B per fired source) for the
+    # delivery kernel of either mode (queue mode: one launch per slot group routes the group's events and folds as
+    # many records of an earlier group)
+    delivery_bytes = p_events * EVENT_BYTES + p_spikes * SOURCE_BYTES
+    kbytes = [N * (UPDATE_BYTES_PER_VERTEX + (UPDATE_BYTES_PER_VERTEX_OBS if obs else 0.0)) * (sim_steps / max(int(kn[0]), 1))
+              + (delivery_bytes / max(int(kn[0]), 1) if kn[1] == 0 else 0.0),
+              delivery_bytes / max(int(kn[1]), 1),
               N * 8.0,
               p_events * 8.0 / max(int(kn[3]), 1)]
     kernels = []

@@ -43,7 +43,7 @@ int check_config(const gn_config *cfg, char *err, size_t errn)
 }
 
 // Groups beyond the current one whose events the update kernel delivers itself (GnDev::q_window).
-static const uint32_t kQueueWindow = 1u;
+static const uint32_t kQueueWindow = 2u;
 
 // Resolved delivery plan: mode, log2(slots per bucket), buckets, records per bucket.
 struct QueuePlan {
@@ -485,21 +485,22 @@ static int join_streams(gn_net *net)
 // with delay 1 are sent by update(t-1) itself, so the earliest slot deliver(t-1) writes is t+1, and deliver(t)
 // runs on a side stream beside update(t+1).
 //
-// Queue mode.  Steps come in groups of G = 2^q_log (one bucket = the ring rows of one group).  update(t) sends
-// every event due in the group being consumed or in the next W = q_window groups itself; the rest of a whole
-// group's events is routed into buckets by ONE gn_route_kernel launched after the group's last update,
-// followed by the fold of the bucket W+1 groups ahead -- both on the side stream, beside later updates:
-//   route(group g)  after update(last step of g); appends to buckets g+W+1 .. and (wrapped) g;
-//   fold(g+W+1)     after route(g), the last routing that appends to that bucket;
-//   update(first step of g+W+1)  after fold(g+W+1): W groups of slack.
+// Queue mode.  Steps come in groups of G = 2^q_log (one bucket = the ring rows of one group); W = q_window = 2.
+// update(t), t in group h, sends every event due in groups h .. h+W itself.  After the last update of group h ONE
+// gn_route_kernel runs on the side stream, beside the updates of group h+1:
+//   its routing warps append the rest of the group's events to buckets h+W+1 .. and (wrapped) h;
+//   its folding warps add bucket h+W -- complete since route(h-1), the previous launch on that stream -- into
+//   the ring rows of group h+W; the bucket's count is zeroed after the kernel.
+// update(first step of h+W) waits for that launch: a whole group of slack.  The raster rows a launch reads are
+// overwritten W+1 groups later, after the next launch on the side stream.
 // In profiling mode everything runs on the caller's stream in that order, so per-kernel times are clean.
-static int route_pending(gn_net *net, cudaStream_t st, bool prof)
+static int route_pending(gn_net *net, cudaStream_t st, bool prof, uint32_t fold_bucket)
 {
     const GnDev &d = net->dev;
     if (!d.queue_mode || net->routed_upto >= net->t) return GN_OK;
     int rc;
     if (prof && (rc = prof_mark(net, 1))) return rc;
-    GN_CUDA(net, gnk_route(d, net->routed_upto, (uint32_t)(net->t - net->routed_upto), st));
+    GN_CUDA(net, gnk_route(d, net->routed_upto, (uint32_t)(net->t - net->routed_upto), fold_bucket, st));
     net->launches++;
     net->routed_upto = net->t;
     return GN_OK;
@@ -560,13 +561,10 @@ int gn_step(gn_net *net, uint64_t n_steps)
             if (!prof) GN_CUDA(net, cudaEventRecord(net->ev_deliver[t & 1ull], s_del));
             net->fences_pending = !prof;
         } else if (group_end) {
-            if ((rc = route_pending(net, s_del, prof))) return rc;
-            const uint32_t b_fold = (((uint32_t)(t % d.D) >> d.q_log) + d.q_window + 1u) % d.q_nb;
-            if (prof && (rc = prof_mark(net, 3))) return rc;
-            GN_CUDA(net, gnk_fold(d, b_fold, s_del));
+            const uint32_t b_fold = (((uint32_t)(t % d.D) >> d.q_log) + d.q_window) % d.q_nb;
+            if ((rc = route_pending(net, s_del, prof, b_fold))) return rc;
             GN_CUDA(net, cudaMemsetAsync(d.q_count + b_fold, 0, 8, s_del));             // the bucket is empty again
-            net->launches++;
-            if (!prof) GN_CUDA(net, cudaEventRecord(net->ev_fold[(t / G + d.q_window + 1u) & 3ull], s_del));
+            if (!prof) GN_CUDA(net, cudaEventRecord(net->ev_fold[(t / G + d.q_window) & 3ull], s_del));
             net->fences_pending = !prof;
         }
         if (d.obs_stride && (t + 1) % d.obs_stride == 0) {
@@ -590,7 +588,7 @@ static int flush_delivery(gn_net *net, bool fold_too)
     const GnDev &d = net->dev;
     int rc = join_streams(net);
     if (rc) return rc;
-    if ((rc = route_pending(net, net->stream, false))) return rc;
+    if ((rc = route_pending(net, net->stream, false, 0xFFFFFFFFu))) return rc;
     if (fold_too && d.queue_mode) {   // pending records are deferred ring adds: apply them all (a no-op for the results)
         for (uint32_t b = 0; b < d.q_nb; ++b) GN_CUDA(net, gnk_fold(d, b, net->stream));
         GN_CUDA(net, cudaMemsetAsync(d.q_count, 0, (size_t)d.q_nb * 8, net->stream));

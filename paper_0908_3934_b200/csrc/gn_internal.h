@@ -86,7 +86,8 @@ struct GnCheck {
 // ---- launchers (gn_kernels.cu).  All asynchronous on `st`; return the launch error. ----
 cudaError_t gnk_update(const GnDev &p, uint64_t t, bool has_bias, cudaStream_t st);
 cudaError_t gnk_deliver(const GnDev &p, uint64_t t, cudaStream_t st);
-cudaError_t gnk_route(const GnDev &p, uint64_t t0, uint32_t n_batch, cudaStream_t st);
+// fold_bucket: the bucket the kernel's folding warps add into the ring beside the routing; 0xFFFFFFFF = none
+cudaError_t gnk_route(const GnDev &p, uint64_t t0, uint32_t n_batch, uint32_t fold_bucket, cudaStream_t st);
 cudaError_t gnk_fold(const GnDev &p, uint32_t bucket, cudaStream_t st);
 cudaError_t gnk_sort_rows(const GnDev &p, GnCheck *chk, cudaStream_t st);
 cudaError_t gnk_observe(const GnDev &p, uint64_t frame, cudaStream_t st);

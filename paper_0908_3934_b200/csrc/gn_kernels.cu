@@ -24,6 +24,7 @@ constexpr int kUpdateThreads = 256;          // 8 warps x 128 vertices = 1024 ve
 constexpr int kVertsPerThread = 4;           // one 128-bit load per SoA array
 constexpr int kDeliverThreads = 256;
 constexpr uint32_t kStreamDrive = 5, kStreamNoise = 6;
+constexpr uint32_t kNoBucket = 0xFFFFFFFFu;
 
 // ---- Philox4x32-10 (Salmon et al., SC'11), from its published description -------------------
 __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
@@ -246,7 +247,16 @@ gn_update_kernel(const GnDev p, const uint64_t t, const uint32_t slot, const uin
 // source list with a popc prefix scan: no global list, no global cursor.  Returns the number of sources.
 constexpr uint32_t kMaxChunkWords = 128;                 // 4096 vertices per CTA at most
 
-template <int THREADS>
+// CTA barrier over the first THREADS threads only: BAR = 0 is __syncthreads (the whole CTA), BAR > 0 a named barrier,
+// so that warps beyond THREADS (the folding warps of gn_route_kernel) never take part.
+template <int THREADS, int BAR>
+__device__ __forceinline__ void part_sync()
+{
+    if (BAR == 0) __syncthreads();
+    else asm volatile("bar.sync %0, %1;" ::"n"(BAR), "n"(THREADS) : "memory");
+}
+
+template <int THREADS, int BAR = 0>
 __device__ __forceinline__ uint32_t gather_scan(const uint32_t *__restrict__ raster_row, const uint32_t w0,
                                                 const uint32_t n_words, uint32_t *s_wsum, uint32_t &word, uint32_t &off)
 {
@@ -259,9 +269,9 @@ __device__ __forceinline__ uint32_t gather_scan(const uint32_t *__restrict__ ras
         const uint32_t v = __shfl_up_sync(0xFFFFFFFFu, incl, o);
         if (lane >= (uint32_t)o) incl += v;
     }
-    __syncthreads();                                       // s_wsum may still be read from the previous scan
+    part_sync<THREADS, BAR>();                             // s_wsum may still be read from the previous scan
     if (lane == 31u) s_wsum[warp] = incl;
-    __syncthreads();
+    part_sync<THREADS, BAR>();
     uint32_t total = 0u;
     off = incl - pc;
 #pragma unroll
@@ -403,7 +413,7 @@ __device__ __forceinline__ void route_round(const GnDev &p, const uint32_t n, co
         events += (unsigned long long)deg;
     }
     s_wtot[warp][lane] = tot;
-    __syncthreads();
+    part_sync<kRouteThreads, 1>();
     // B: reserve; afterwards s_wbase[w][k] = index (in records, over the whole queue) of warp w's first record
     // of segment k
     if (warp == 0) {
@@ -430,7 +440,7 @@ __device__ __forceinline__ void route_round(const GnDev &p, const uint32_t n, co
         const uint32_t mask = __ballot_sync(0xFFFFFFFFu, full);
         if (lane == 0) *s_ovf = mask;
     }
-    __syncthreads();
+    part_sync<kRouteThreads, 1>();
     // C: records.  With rd = r + delay: queued iff rd >= (W+1)G; group offset j = rd >> q_log, owned by lane
     // j - W; ring row inside the bucket = rd & (G-1).
     const uint32_t ovf = *s_ovf;
@@ -480,60 +490,25 @@ __device__ __forceinline__ void route_round(const GnDev &p, const uint32_t n, co
             }
         }
     }
-    __syncthreads();
+    part_sync<kRouteThreads, 1>();
 }
 
-// Routes the queued segments of every vertex that fired in steps t0 .. t0+n_batch-1, all inside ONE slot
-// group (slot0 = t0 mod D): one launch per group amortises the launch and the dependent memory round trips
-// over 2^q_log steps of work.  raster row of step t0+i is (row0 + i) mod raster_rows.
-template <bool PACKED>
-__global__ void __launch_bounds__(kRouteThreads, 4)
-gn_route_kernel(const GnDev p, const uint32_t slot0, const uint32_t row0, const uint32_t n_batch,
-                const uint32_t chunk_words)
-{
-    __shared__ uint32_t s_list[kRouteListCap];
-    __shared__ uint8_t s_step[kRouteListCap];
-    __shared__ uint32_t s_wsum[kRouteWarps];
-    __shared__ uint32_t s_wtot[kRouteWarps][32];         // A: records of warp w in segment k
-    __shared__ uint32_t s_wbase[kRouteWarps][32];        // B: where warp w's records of segment k start in the bucket
-    __shared__ uint32_t s_ovf;                           // B: bit k = segment k's bucket is full
-    const uint32_t w0 = blockIdx.x * chunk_words;
-    const uint32_t n_words = min(chunk_words, p.words_pad - w0);
-    unsigned long long events = 0ull;
-    uint32_t n = 0u, spikes = 0u;
-    for (uint32_t i = 0; i < n_batch; ++i) {
-        uint32_t rr = row0 + i;
-        if (rr >= p.raster_rows) rr -= p.raster_rows;
-        uint32_t word, off;
-        const uint32_t total = gather_scan<kRouteThreads>(p.raster + (size_t)rr * p.words_pad, w0, n_words, s_wsum, word, off);
-        if (n + total > kRouteListCap) {                    // CTA-uniform: the list is full, work it off first
-            route_round<PACKED>(p, n, slot0, s_list, s_step, s_wtot, s_wbase, &s_ovf, events);
-            n = 0u;
-        }
-        gather_write(word, w0, n + off, s_list, s_step, i);
-        n += total;
-        spikes += total;
-    }
-    __syncthreads();
-    if (n) route_round<PACKED>(p, n, slot0, s_list, s_step, s_wtot, s_wbase, &s_ovf, events);
-    if ((threadIdx.x & 31u) == 0 && events) atomicAdd(&p.counters[2], events);
-    if (threadIdx.x == 0 && spikes) atomicAdd(&p.counters[1], (unsigned long long)spikes);
-}
-
-// ---- a4, queue mode: fold one bucket into its ring rows --------------------------------------------------
-__global__ void __launch_bounds__(256)
-gn_fold_kernel(const GnDev p, const uint32_t bucket)
+// Adds the records of one bucket into the bucket's 2^q_log ring rows (int32 RED; the rows are L2-resident while a
+// bucket is folded); warp w of n_w cooperating warps.  Scattered REDs are bound by LSU issue (about one lane per
+// 1.3 cycles per SM), not by memory.
+__device__ __forceinline__ void fold_records(const GnDev &p, const uint32_t bucket, const uint32_t w, const uint32_t n_w,
+                                             const uint32_t lane)
 {
     unsigned long long n = p.q_count[bucket];
     if (n > p.q_cap) n = p.q_cap;
     int32_t *rows = p.ring + ((size_t)bucket << p.q_log) * p.Npad;
     const uint4 *q4 = reinterpret_cast<const uint4 *>(p.queue + (size_t)bucket * p.q_cap);
     const unsigned long long pairs = n >> 1;
-    const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
-    for (unsigned long long i0 = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i0 < pairs; i0 += 4ull * stride) {
+    const unsigned long long stride = (unsigned long long)n_w * 32ull;
+    for (unsigned long long i0 = (unsigned long long)w * 32ull + lane; i0 < pairs; i0 += 4ull * stride) {
         uint4 v[4];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {                       // four 16-byte loads in flight per thread
+        for (int u = 0; u < 4; ++u) {                       // four 16-byte loads in flight per lane
             const unsigned long long i = i0 + (unsigned long long)u * stride;
             v[u] = (i < pairs) ? __ldcs(q4 + i) : make_uint4(0u, 0u, 0u, 0u);
         }
@@ -543,10 +518,65 @@ gn_fold_kernel(const GnDev p, const uint32_t bucket)
             if (v[u].w) atomicAdd(rows + v[u].z, (int32_t)v[u].w);
         }
     }
-    if ((n & 1ull) && blockIdx.x == 0 && threadIdx.x == 0) {
+    if ((n & 1ull) && w == 0u && lane == 0u) {
         const uint2 v = p.queue[(size_t)bucket * p.q_cap + n - 1];
         if (v.y) atomicAdd(rows + v.x, (int32_t)v.y);
     }
+}
+
+// Routes the queued segments of every vertex that fired in steps t0 .. t0+n_batch-1, all inside ONE slot
+// group (slot0 = t0 mod D): one launch per group amortises the launch and the dependent memory round trips
+// over 2^q_log steps of work.  raster row of step t0+i is (row0 + i) mod raster_rows.
+// Warp specialisation: threads 0..255 route (their barriers are the named barrier 1); the kFoldWarps warps after
+// them fold bucket `fold_bucket` -- complete since the previous group's routing -- at the same time, in the same
+// CTAs: routing waits on DRAM, folding on LSU issue, and two separate kernels that each fill the SMs never overlap.
+constexpr int kFoldWarps = 2;
+
+template <bool PACKED>
+__global__ void __launch_bounds__(kRouteThreads + 32 * kFoldWarps, 3)
+gn_route_kernel(const GnDev p, const uint32_t slot0, const uint32_t row0, const uint32_t n_batch,
+                const uint32_t chunk_words, const uint32_t fold_bucket)
+{
+    __shared__ uint32_t s_list[kRouteListCap];
+    __shared__ uint8_t s_step[kRouteListCap];
+    __shared__ uint32_t s_wsum[kRouteWarps];
+    __shared__ uint32_t s_wtot[kRouteWarps][32];         // A: records of warp w in segment k
+    __shared__ uint32_t s_wbase[kRouteWarps][32];        // B: where warp w's records of segment k start in the bucket
+    __shared__ uint32_t s_ovf;                           // B: bit k = segment k's bucket is full
+    if (threadIdx.x >= kRouteThreads) {                  // folding warps
+        if (fold_bucket != kNoBucket)
+            fold_records(p, fold_bucket, blockIdx.x * kFoldWarps + ((threadIdx.x - kRouteThreads) >> 5),
+                         gridDim.x * kFoldWarps, threadIdx.x & 31u);
+        return;
+    }
+    const uint32_t w0 = blockIdx.x * chunk_words;
+    const uint32_t n_words = min(chunk_words, p.words_pad - w0);
+    unsigned long long events = 0ull;
+    uint32_t n = 0u, spikes = 0u;
+    for (uint32_t i = 0; i < n_batch; ++i) {
+        uint32_t rr = row0 + i;
+        if (rr >= p.raster_rows) rr -= p.raster_rows;
+        uint32_t word, off;
+        const uint32_t total = gather_scan<kRouteThreads, 1>(p.raster + (size_t)rr * p.words_pad, w0, n_words, s_wsum, word, off);
+        if (n + total > kRouteListCap) {                    // CTA-uniform: the list is full, work it off first
+            route_round<PACKED>(p, n, slot0, s_list, s_step, s_wtot, s_wbase, &s_ovf, events);
+            n = 0u;
+        }
+        gather_write(word, w0, n + off, s_list, s_step, i);
+        n += total;
+        spikes += total;
+    }
+    part_sync<kRouteThreads, 1>();
+    if (n) route_round<PACKED>(p, n, slot0, s_list, s_step, s_wtot, s_wbase, &s_ovf, events);
+    if ((threadIdx.x & 31u) == 0 && events) atomicAdd(&p.counters[2], events);
+    if (threadIdx.x == 0 && spikes) atomicAdd(&p.counters[1], (unsigned long long)spikes);
+}
+
+// ---- a4, queue mode: fold one bucket outside the step loop (ring read-back) ----------------------------------
+__global__ void __launch_bounds__(256)
+gn_fold_kernel(const GnDev p, const uint32_t bucket)
+{
+    fold_records(p, bucket, (blockIdx.x * blockDim.x + threadIdx.x) >> 5, (gridDim.x * blockDim.x) >> 5, threadIdx.x & 31u);
 }
 
 // ---- create time, queue mode: copy every CSR row sorted by delay (counting sort, one warp per row) --------
@@ -1063,12 +1093,13 @@ cudaError_t gnk_deliver(const GnDev &p, uint64_t t, cudaStream_t st)
     return cudaGetLastError();
 }
 
-cudaError_t gnk_route(const GnDev &p, uint64_t t0, uint32_t n_batch, cudaStream_t st)
+cudaError_t gnk_route(const GnDev &p, uint64_t t0, uint32_t n_batch, uint32_t fold_bucket, cudaStream_t st)
 {
-    const uint32_t w = chunk_words_for(p, 148u * 4u);            // four 256-thread CTAs per SM
+    const uint32_t w = chunk_words_for(p, 148u * 3u);            // three 320-thread CTAs per SM
     const uint32_t grid = ceil_div(p.words_pad, w), slot0 = (uint32_t)(t0 % p.D), row0 = (uint32_t)(t0 % p.raster_rows);
-    if (p.packed) gn_route_kernel<true><<<grid, kRouteThreads, 0, st>>>(p, slot0, row0, n_batch, w);
-    else gn_route_kernel<false><<<grid, kRouteThreads, 0, st>>>(p, slot0, row0, n_batch, w);
+    const uint32_t threads = kRouteThreads + 32 * kFoldWarps;
+    if (p.packed) gn_route_kernel<true><<<grid, threads, 0, st>>>(p, slot0, row0, n_batch, w, fold_bucket);
+    else gn_route_kernel<false><<<grid, threads, 0, st>>>(p, slot0, row0, n_batch, w, fold_bucket);
     return cudaGetLastError();
 }
 
