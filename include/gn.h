@@ -86,7 +86,7 @@ typedef struct {
     /* How eq. 30's sum reaches the ring (the RESULT is identical in every mode: integer adds commute). */
     uint32_t delivery_mode;         /* GN_DELIVER_AUTO (0), _RING, _QUEUE, _RESIDENT                   */
     uint32_t queue_group;           /* queue mode: ring slots per event bucket, power of two in 1..16; */
-                                    /* 0 = default (8)                                                */
+                                    /* 0 = default (4)                                                */
     uint64_t queue_capacity;        /* queue mode: events one bucket holds before later ones fall     */
                                     /* back to direct ring adds; 0 = default queue_group * ceil(E/16) */
 } gn_config;

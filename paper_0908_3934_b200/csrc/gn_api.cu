@@ -56,7 +56,7 @@ QueuePlan make_plan(const gn_config *cfg)
 {
     const uint64_t N = cfg->n_vertices, Npad = (N + 127) / 128 * 128, E = cfg->n_edges, D = cfg->ring_slots;
     QueuePlan q{};
-    uint32_t group = cfg->queue_group ? cfg->queue_group : 8u;
+    uint32_t group = cfg->queue_group ? cfg->queue_group : 4u;
     // cell offsets are 32-bit; the ring depth must be a whole number of groups
     while (group > 1 && (Npad * group > 0xFFFFFFFFull || D % group != 0)) group >>= 1;
     q.on = cfg->delivery_mode == GN_DELIVER_QUEUE ||
