@@ -189,7 +189,7 @@ gn_update_kernel(const GnDev p, const uint64_t t, const uint32_t slot, const uin
     // a4, the urgent part: events due before the delivery kernel of this step is guaranteed to have run are
     // sent by the vertex that fired (rows are sorted by delay: such edges lead the row).  Ring mode: delay 1
     // (d_direct = 2), so that deliver(t) may overlap update(t+1).  Queue mode: every delay that lands in the
-    // group being consumed or in the next one (d_direct = 2G - r), so that routing runs once per group.
+    // group being consumed or in the next W = q_window (d_direct = (W+1)G - r), so that routing runs once per group.
     // FUSED (ring mode, small networks: a step is bound by launch latency, not by work): the whole of a4 happens here,
     // warp-cooperatively -- every fired vertex of the warp in turn, lanes over its row -- and there is no delivery kernel.
     if (FUSED) {
