@@ -6,3 +6,4 @@ method's drive/noise numbers.  The oracle (``oracle/``) and the CUDA library
 """
 from .generate import build_lib, geometric_network, Network  # noqa: F401
 from .configs import make_config, CONFIG_NAMES, MASTER_SEED  # noqa: F401
+from . import paper_test_set  # noqa: F401  (the paper's 80-network test set, regenerated: PAPER.md:388-450)

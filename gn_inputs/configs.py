@@ -1,4 +1,5 @@
-"""The five BASELINE.json workloads as seeded synthetic inputs.
+"""The five BASELINE.json workloads (and, as config 6, the paper's own 80-network test set) as seeded synthetic inputs
+(DESIGN.md "Input recipe").
 
 Each entry fixes what BASELINE.json leaves open with the reading listed in DESIGN.md
 (SURVEY.md section 8(c) readings #5, #12, #16-#20).  A config can be generated at a reduced vertex
@@ -21,6 +22,7 @@ CONFIG_NAMES = {
     3: "cfg3_n100k_3d_exp",
     4: "cfg4_n1m_3d_rgg",
     5: "cfg5_batch4096x1000_2d_obs",
+    6: "paper_table1_80_networks",
 }
 
 
@@ -107,7 +109,17 @@ def make_config(k: int, n: int | None = None, n_networks: int | None = None,
                                 w_exc=(0.0, 8.0), w_inh=(-8.0, 0.0), n_networks=nb)
         cfg = dict(base, ring_slots=32, speed=0.0259, classes=[_rs(10.0), _rs(10.0)], steps=5_000,
                    obs_stride=100)
+    elif k == 6:
+        # Not a BASELINE config: the paper's own test set (Table 1), regenerated by paper_test_set.py and
+        # stepped as ONE batch of 80 independent networks (N = 10 .. 1000, 2D and 3D, four connectivity classes, two
+        # densities).  The paper leaves model, weights and speed to the user: config 5's classes and observation; the
+        # speed puts the longest possible distance (the cube's diagonal) at 31 steps.  `n` / `n_networks` are ignored.
+        from . import paper_test_set as ts
+        net = ts.batch(ts.table1(seed))
+        side = ts.SPACE
+        cfg = dict(base, ring_slots=32, speed=side * math.sqrt(3.0) / 31.0 / base["dt_ms"] * 1.0001,
+                   classes=[_rs(10.0), _rs(10.0)], steps=5_000, obs_stride=100)
     else:
-        raise ValueError("config must be 1..5")
+        raise ValueError("config must be 1..6")
     net.meta.update(config=k, side=side, seed=seed)
     return net, cfg

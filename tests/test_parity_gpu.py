@@ -308,6 +308,19 @@ def test_alpha_function_mixed_classes_and_state_roundtrip(gn):
     assert not pg[net.vertex_class == 1].any() and pg[net.vertex_class == 0].any()
 
 
+@pytest.mark.parametrize("mode", ["AUTO", "RING"])
+def test_paper_test_set_all_80_networks_in_one_handle(gn, mode):
+    """The paper's own workload shape (Table 1; regenerated by gn_inputs/paper_test_set.py): 80
+    networks of 10 .. 1000 vertices, 2D and 3D, lattice / small world / scale free / random at two densities, stepped
+    as one batch (AUTO = one CTA per network) -- bit-exact against the oracle, trace within tolerance."""
+    net, cfg = make_config(6)
+    assert net.n_networks == 80 and net.n_vertices == 23_040
+    g, o, _ = _run_exact(gn, net, cfg, 1500, 500, delivery_mode=getattr(gn, "GN_DELIVER_" + mode), threads=8)
+    assert o.counters()["delivered"] > 10 ** 5
+    frames = 1500 // cfg["obs_stride"]
+    np.testing.assert_allclose(gn.gn_observe(g, 0, frames).astype(np.float64), o.trace(0, frames), rtol=1e-6, atol=1e-5)
+
+
 def test_queue_mode_reads_inside_a_group_and_odd_step_counts(gn):
     """Queue mode routes once per slot group and the update kernel sends the near events itself: stepping by
     counts that are not multiples of the group, and reading ring / counters in the middle of a group, must
