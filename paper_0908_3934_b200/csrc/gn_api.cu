@@ -59,6 +59,9 @@ QueuePlan make_plan(const gn_config *cfg)
     uint32_t group = cfg->queue_group ? cfg->queue_group : 4u;
     // cell offsets are 32-bit; the ring depth must be a whole number of groups
     while (group > 1 && (Npad * group > 0xFFFFFFFFull || D % group != 0)) group >>= 1;
+    // one lane of a routing warp per bucket: deeper rings take larger groups when the caller left the choice open
+    while (cfg->queue_group == 0 && D / group > 32 && group < 16 && D % (group * 2) == 0 && Npad * group * 2 <= 0xFFFFFFFFull)
+        group <<= 1;
     q.on = cfg->delivery_mode == GN_DELIVER_QUEUE ||
            (cfg->delivery_mode == GN_DELIVER_AUTO && D >= 32 && D * Npad * 4 > (48ull << 20));
     if (E == 0 || D / group > 32) q.on = false;      // gn_route_kernel: one lane per bucket

@@ -139,6 +139,16 @@ QUEUE_CASES = [
 ]
 
 
+def test_queue_mode_deep_ring_picks_a_larger_group(gn):
+    """D = 160 with the group left open: groups of 4 would need 40 buckets (> 32 lanes), so the library takes 8."""
+    rng = np.random.default_rng(12)
+    net, cfg = make_config(2, n=2_500)
+    cfg = dict(cfg, ring_slots=160, obs_stride=0)
+    delays = rng.integers(1, 160, size=net.n_edges).astype(np.uint8)
+    _, o, _ = _run_exact(gn, net, cfg, 900, 300, delays=delays, delivery_mode=gn.GN_DELIVER_QUEUE)
+    assert o.counters()["delivered"] > 0
+
+
 @pytest.mark.parametrize("k,n,nb,steps,chunk,group,cap", QUEUE_CASES)
 def test_queue_mode_bit_exact(gn, k, n, nb, steps, chunk, group, cap):
     net, cfg = make_config(k, n=n, n_networks=nb)
