@@ -121,7 +121,7 @@ struct gn_net {
     uint64_t t;          // steps enqueued so far
     uint64_t routed_upto; // queue mode: steps < routed_upto have had their queued events routed
     // delivery of step t overlaps the update of step t+1 (see gn_step): side streams and their fences
-    cudaStream_t s_deliver, s_fold;
+    cudaStream_t s_deliver;
     cudaEvent_t ev_update, ev_deliver[2], ev_fold[4];
     bool fences_pending;
     bool has_bias;
@@ -210,7 +210,7 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
     net->ws = (uint8_t *)workspace;
     net->t = 0;
     net->routed_upto = 0;
-    net->s_deliver = net->s_fold = nullptr;
+    net->s_deliver = nullptr;
     net->ev_update = net->ev_deliver[0] = net->ev_deliver[1] = net->ev_fold[0] = net->ev_fold[1] = net->ev_fold[2] = net->ev_fold[3] = nullptr;
     net->fences_pending = false;
     net->has_bias = bias != nullptr;
@@ -417,13 +417,11 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
         delete net;
         return set_err(nullptr, GN_E_OVERFLOW_RISK, "some target's sum |w_fx| + |kick_fx| exceeds 2^31 - 1");
     }
-    // side streams: delivery of step t runs beside the update of step t+1; a bucket is folded beside the
-    // steps that consume the group before it
+    // side stream: the delivery kernel (ring mode: of step t; queue mode: of a slot group) runs beside later updates
     {
         int lo = 0, hi = 0;
         cudaError_t e = cudaDeviceGetStreamPriorityRange(&lo, &hi);
         if (e == cudaSuccess) e = cudaStreamCreateWithPriority(&net->s_deliver, cudaStreamNonBlocking, hi);
-        if (e == cudaSuccess) e = cudaStreamCreateWithPriority(&net->s_fold, cudaStreamNonBlocking, lo);
         cudaEvent_t *evs[7] = {&net->ev_update, &net->ev_deliver[0], &net->ev_deliver[1], &net->ev_fold[0], &net->ev_fold[1],
                                &net->ev_fold[2], &net->ev_fold[3]};
         for (int k = 0; k < 7 && e == cudaSuccess; ++k) e = cudaEventCreateWithFlags(evs[k], cudaEventDisableTiming);
@@ -760,13 +758,11 @@ int gn_destroy(gn_net *net)
 {
     if (!net) return GN_E_INVALID_ARG;
     if (net->s_deliver) cudaStreamSynchronize(net->s_deliver);
-    if (net->s_fold) cudaStreamSynchronize(net->s_fold);
     cudaError_t e = cudaStreamSynchronize(net->stream);
     for (cudaEvent_t ev : net->ev) cudaEventDestroy(ev);
     cudaEvent_t evs[7] = {net->ev_update, net->ev_deliver[0], net->ev_deliver[1], net->ev_fold[0], net->ev_fold[1], net->ev_fold[2], net->ev_fold[3]};
     for (cudaEvent_t ev : evs) if (ev) cudaEventDestroy(ev);
     if (net->s_deliver) cudaStreamDestroy(net->s_deliver);
-    if (net->s_fold) cudaStreamDestroy(net->s_fold);
     delete net;
     return e == cudaSuccess ? GN_OK : GN_E_CUDA;
 }

@@ -373,19 +373,9 @@ constexpr int kRouteThreads = 256;
 constexpr int kRouteWarps = kRouteThreads / 32;
 constexpr int kRouteUnroll = 8;                         // 8 x 32 edges of a row in flight per warp
 
-// Lane k owns the events due j = k + W groups after the current one (W = q_window groups are the update
-// kernel's; k = 1 .. nb-W): boundaries of that segment of `src` at alignment r -> lo (start position) and cnt.
-__device__ __forceinline__ void route_segments(const GnDev &p, const uint32_t src, const uint32_t r, const uint32_t nb,
-                                               const uint32_t deg, const uint32_t lane, uint32_t &lo, uint32_t &cnt)
-{
-    const uint16_t *seg = p.q_seg + ((size_t)src << p.q_log) * nb + (size_t)r * nb;
-    const uint32_t i = lane + p.q_window - 1u;             // table entry i = #edges with delay < (i+1)G - r
-    lo = (i < nb) ? (uint32_t)__ldg(seg + i) : deg;
-    uint32_t hi = __shfl_down_sync(0xFFFFFFFFu, lo, 1);
-    if (i + 1u >= nb || lane == 31u) hi = deg;
-    cnt = (lane >= 1u && i < nb) ? hi - lo : 0u;
-}
-
+// Lane k owns the events due j = k + W groups after the current one (W = q_window groups are the update kernel's;
+// k = 1 .. nb-W).  Its segment of a row starts at table entry i = k + W - 1 (#edges with delay < (i+1)G - r) and ends
+// at entry i + 1 (the out-degree past the table's end): lo from the lane's own load, hi by a shuffle from lane k + 1.
 constexpr uint32_t kRouteListCap = 4096;                // sources one A/B/C round of a CTA handles
 
 // Phases A, B, C over the n sources in s_list (each tagged with its step inside the group).
@@ -402,15 +392,34 @@ __device__ __forceinline__ void route_round(const GnDev &p, const uint32_t n, co
     uint32_t my_bucket = g_cur + p.q_window + lane;        // bucket of the segment this lane owns
     while (my_bucket >= nb) my_bucket -= nb;
 
-    // A: per-warp, per-segment record counts
+    // A: per-warp, per-segment record counts.  Four sources at a time: their row bounds and table entries (first
+    // touch: DRAM latency) are all requested before any is used.
     uint32_t tot = 0u;
-    for (uint32_t idx = warp; idx < n; idx += kRouteWarps) {
-        const uint32_t src = s_list[idx];
-        const uint32_t deg = row[src + 1] - row[src];
-        uint32_t lo, cnt;
-        route_segments(p, src, r0 + s_step[idx], nb, deg, lane, lo, cnt);
-        tot += cnt;
-        events += (unsigned long long)deg;
+    {
+        const uint32_t tab_i = lane + p.q_window - 1u;     // this lane's table entry (see above)
+        for (uint32_t idx0 = warp; idx0 < n; idx0 += 4u * kRouteWarps) {
+            uint32_t beg[4], end[4], seg[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const uint32_t idx = idx0 + (uint32_t)u * kRouteWarps;
+                beg[u] = end[u] = seg[u] = 0u;
+                if (idx < n) {
+                    const uint32_t src = s_list[idx];
+                    beg[u] = row[src]; end[u] = row[src + 1];
+                    if (tab_i < nb)
+                        seg[u] = (uint32_t)__ldg(p.q_seg + ((size_t)src << p.q_log) * nb + (size_t)(r0 + s_step[idx]) * nb + tab_i);
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const uint32_t deg = end[u] - beg[u];
+                const uint32_t lo = tab_i < nb ? seg[u] : deg;
+                uint32_t hi = __shfl_down_sync(0xFFFFFFFFu, lo, 1);
+                if (tab_i + 1u >= nb || lane == 31u) hi = deg;
+                tot += (lane >= 1u && tab_i < nb) ? hi - lo : 0u;
+                events += (unsigned long long)deg;
+            }
+        }
     }
     s_wtot[warp][lane] = tot;
     part_sync<kRouteThreads, 1>();
@@ -445,12 +454,28 @@ __device__ __forceinline__ void route_round(const GnDev &p, const uint32_t n, co
     // j - W; ring row inside the bucket = rd & (G-1).
     const uint32_t ovf = *s_ovf;
     uint32_t run = s_wbase[warp][lane];
+    // the row bounds and the segment-table entry of the NEXT source are requested before the current source's edges,
+    // so a source costs one memory round trip, not two
+    uint32_t nx_beg = 0u, nx_end = 0u, nx_seg = 0u, nx_r = 0u;
+    const uint32_t tab_i = lane + p.q_window - 1u;         // this lane's table entry (see above)
+    if (warp < n) {
+        const uint32_t src = s_list[warp];
+        nx_r = r0 + s_step[warp];
+        nx_beg = row[src]; nx_end = row[src + 1];
+        if (tab_i < nb) nx_seg = (uint32_t)__ldg(p.q_seg + ((size_t)src << p.q_log) * nb + (size_t)nx_r * nb + tab_i);
+    }
     for (uint32_t idx = warp; idx < n; idx += kRouteWarps) {
-        const uint32_t src = s_list[idx];
-        const uint32_t r = r0 + s_step[idx];
-        const uint32_t e_beg = row[src], n_e = row[src + 1] - e_beg;
-        uint32_t lo, cnt;
-        route_segments(p, src, r, nb, n_e, lane, lo, cnt);
+        const uint32_t r = nx_r, e_beg = nx_beg, n_e = nx_end - nx_beg, seg_lo = nx_seg;
+        if (idx + kRouteWarps < n) {
+            const uint32_t src = s_list[idx + kRouteWarps];
+            nx_r = r0 + s_step[idx + kRouteWarps];
+            nx_beg = row[src]; nx_end = row[src + 1];
+            if (tab_i < nb) nx_seg = (uint32_t)__ldg(p.q_seg + ((size_t)src << p.q_log) * nb + (size_t)nx_r * nb + tab_i);
+        }
+        const uint32_t lo = tab_i < nb ? seg_lo : n_e;     // from the prefetched entry
+        uint32_t hi = __shfl_down_sync(0xFFFFFFFFu, lo, 1);
+        if (tab_i + 1u >= nb || lane == 31u) hi = n_e;
+        const uint32_t cnt = (lane >= 1u && tab_i < nb) ? hi - lo : 0u;
         const uint32_t adj = run - lo;                     // record index - edge position, for this lane's segment
         run += cnt;
         const uint32_t x_first = __shfl_sync(0xFFFFFFFFu, lo, 1) & ~31u;   // the update kernel's edges need no visit
