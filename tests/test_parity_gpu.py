@@ -434,6 +434,39 @@ def test_state_within_tolerance_of_fp64_until_divergence(gn, k, n, nb, steps):
         np.testing.assert_array_equal(rg[:t_star], ro[:t_star])
 
 
+def test_full_run_raster_agreement_beyond_the_divergence(gn):
+    """BASELINE configs[1] for its whole 10,000 steps against the fp64 DEFINITION: after the first fp32/fp64 raster
+    divergence t* the two runs are different samples of a chaotic system, so only the cell agreement (>= 99.9 %,
+    north_star) is asserted; t*, the spike counts and the +-1-step coincidence F1 are printed, not hidden."""
+    net, cfg = make_config(2)
+    cfg = dict(cfg, obs_stride=0)
+    steps = cfg["steps"]
+    g = _make(gn, net, cfg, steps)
+    o = Oracle(net, cfg, "fp64", threads=8)
+    gn.gn_step(g, steps)
+    o.step(steps)
+    rg = unpack_raster(gn.gn_read_raster(g, 0, steps), net.n_vertices)
+    ro = o.raster_bool(0, steps)
+    diff = (rg != ro).any(axis=1)
+    t_star = int(np.nonzero(diff)[0][0]) if diff.any() else None
+    agree = float((rg == ro).mean())
+    near = ro.copy()
+    near[1:] |= ro[:-1]
+    near[:-1] |= ro[1:]
+    near_g = rg.copy()
+    near_g[1:] |= rg[:-1]
+    near_g[:-1] |= rg[1:]
+    prec = float((rg & near).sum()) / max(int(rg.sum()), 1)
+    rec = float((ro & near_g).sum()) / max(int(ro.sum()), 1)
+    f1 = 2 * prec * rec / max(prec + rec, 1e-12)
+    print(f"[cfg 2, {steps} steps] t* = {t_star}, spikes GPU {int(rg.sum())} / fp64 {int(ro.sum())}, "
+          f"cell agreement {agree:.6f}, +-1-step coincidence F1 {f1:.4f}")
+    assert agree >= 0.999
+    assert abs(int(rg.sum()) - int(ro.sum())) < 0.05 * int(ro.sum())       # same regime, different sample
+    if t_star is not None:
+        np.testing.assert_array_equal(rg[:t_star], ro[:t_star])
+
+
 # ---- invariants of north_star through the C ABI -----------------------------------------------------
 def test_zero_weights_isolated_trajectory(gn):
     """All weights zero: every vertex follows the stand-alone recurrence (eq. 17) -- here
