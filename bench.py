@@ -324,6 +324,15 @@ def main():
           "bytes": p_events * EVENT_BYTES + p_spikes * SOURCE_BYTES, "ms": a4_s * 1e3,
           "achieved": (p_events * EVENT_BYTES + p_spikes * SOURCE_BYTES) / max(a4_s, 1e-12) / 1e9}
     a4["frac"] = a4["achieved"] / peak
+    if queue_mode and a4_s > 0:
+        # the delivery kernel's real ceiling is the SMs' load/store units, not HBM (DESIGN.md 6.3 "LSU accounting"):
+        # ~1.7 LSU cycles per event per SM (scattered RED 1.3 + record store 0.3 + coalesced loads 0.1)
+        sm_hz = 1.965e9
+        lsu_peak = 148 * sm_hz / 1.7
+        a4["lsu"] = {"bound": "lsu-issue", "achieved": p_events / a4_s, "peak": lsu_peak, "unit": "events/s",
+                     "frac": p_events / a4_s / lsu_peak,
+                     "peak_source": "148 SMs x 1.965 GHz / 1.7 LSU cycles per event (B300_MICROARCH.md atomics table: REDG "
+                                    "1.29 cycles per lane; DESIGN.md 6.3)"}
     dom = max(kernels, key=lambda r: r["share"])
     traffic = None
     tpath = os.path.join(ROOT, "profiles", "traffic.csv")   # per-launch DRAM bytes from the committed ncu --set full capture
