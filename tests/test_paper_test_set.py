@@ -1,8 +1,29 @@
 """The regenerated test set of PAPER.md:388-450 (gn_inputs/paper_test_set.py): what the paper fixes about it."""
+import os
+
 import numpy as np
 import pytest
 
 from gn_inputs import paper_test_set as ts
+
+
+def _golden():
+    out = {}
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "paper_printed_values.txt")):
+        line = line.split("#")[0].split()
+        if len(line) == 2:
+            out[line[0]] = line[1]
+    return out
+
+
+def test_generator_against_the_values_the_paper_prints():
+    g = _golden()
+    assert ts.d_min(100.0, 1000, 3) == pytest.approx(float(g["d_min_L100_N1000_D3"]), rel=1e-12)
+    assert len(ts.table1()) == int(g["table1_networks"])
+    assert list(ts.SIZES) == [int(x) for x in g["table1_sizes"].split(",")]
+    assert list(ts._PARAM["lattice"]) == [int(x) for x in g["lattice_neighbours"].split(",")]
+    assert list(ts._PARAM["small_world"]) == [float(x) for x in g["small_world_rewiring"].split(",")]
+    assert list(ts._PARAM["random"]) == [float(x) for x in g["random_density"].split(",")]
 
 
 def test_d_min_worked_example():
