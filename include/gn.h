@@ -128,7 +128,8 @@ enum {
     GN_DELAYS = 8,    /* uint8  [E]      per-edge delay in steps (as given, or eq. 25)               */
     GN_WEIGHTS_FX = 9,/* int32  [E]      per-edge weight, rint(w * 2^16)                             */
     GN_BIAS = 10,     /* float  [N]      user control U_j (write only through gn_write_state)        */
-    GN_P = 11         /* float  [N]      second PSC state p of the alpha-function (zero for other classes) */
+    GN_P = 11,        /* float  [N]      second PSC state p of the alpha-function (zero for other classes) */
+    GN_ACC = 12       /* float  [N]      sum of c over the steps of the camera frame in progress (obs_stride > 0) */
 };
 
 /* Bytes of device workspace gn_create needs for this configuration.
@@ -169,8 +170,12 @@ int gn_step(gn_net *net, uint64_t n_steps);
  * dst is device memory, written asynchronously on the stream.  Errors: INVALID_ARG, CUDA. */
 int gn_read_state(gn_net *net, int which, void *dst, size_t dst_bytes, int dst_is_device);
 
-/* Overwrite V, W, R, P, CA (float [N]), REFR (uint8 [N]) or BIAS (float [N]; enables the bias term).
- * For checkpoint/restore and controlled experiments (PAPER.md:77-79 user control). */
+/* Overwrite V, W, R, P, CA, ACC (float [N]), REFR (uint8 [N]) or BIAS (float [N]; enables the bias term): controlled
+ * experiments (PAPER.md:77-79 user control).  Checkpoint / restore: together with RING (int32 [D][N], the layout GN_RING
+ * reads) and STEP (uint64 [1], or COUNTERS uint64 [4]) they are the whole state -- y_j and the in-flight delayed signals
+ * Y_j: a fresh handle of the same network given all of them continues bit-identically from step t.
+ * Writing STEP / COUNTERS sets the step index (generator counter, ring slot, frame phase); raster steps and trace
+ * frames before it are not held (GN_E_RANGE_EVICTED).  RING / STEP / COUNTERS writes synchronise the stream. */
 int gn_write_state(gn_net *net, int which, const void *src, size_t src_bytes, int src_is_device);
 
 /* Spike raster of steps t0 .. t0+n_steps-1 as bit words: bit (j mod 32) of bits[s][j / 32] is

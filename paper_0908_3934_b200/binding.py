@@ -15,7 +15,7 @@ from .build import build
 GN_OK = 0
 GN_E_INVALID_ARG, GN_E_BAD_GRAPH, GN_E_OVERFLOW_RISK = -1, -2, -3
 GN_E_WORKSPACE_TOO_SMALL, GN_E_RANGE_EVICTED, GN_E_CUDA = -4, -5, -6
-GN_V, GN_W, GN_R, GN_CA, GN_REFR, GN_RING, GN_STEP, GN_COUNTERS, GN_DELAYS, GN_WEIGHTS_FX, GN_BIAS, GN_P = range(12)
+GN_V, GN_W, GN_R, GN_CA, GN_REFR, GN_RING, GN_STEP, GN_COUNTERS, GN_DELAYS, GN_WEIGHTS_FX, GN_BIAS, GN_P, GN_ACC = range(13)
 GN_MAX_CLASSES = 8
 GN_DELIVER_AUTO, GN_DELIVER_RING, GN_DELIVER_QUEUE, GN_DELIVER_RESIDENT = 0, 1, 2, 3
 
@@ -154,7 +154,7 @@ def gn_step(net: GnNet, n_steps: int) -> None:
 
 _STATE_DTYPE = {GN_V: np.float32, GN_W: np.float32, GN_R: np.float32, GN_CA: np.float32, GN_REFR: np.uint8,
                 GN_RING: np.int32, GN_STEP: np.uint64, GN_COUNTERS: np.uint64, GN_DELAYS: np.uint8,
-                GN_WEIGHTS_FX: np.int32, GN_BIAS: np.float32, GN_P: np.float32}
+                GN_WEIGHTS_FX: np.int32, GN_BIAS: np.float32, GN_P: np.float32, GN_ACC: np.float32}
 
 
 def _state_shape(net, which):

@@ -119,6 +119,7 @@ struct gn_net {
     cudaStream_t stream;
     uint8_t *ws;
     uint64_t t;          // steps enqueued so far
+    uint64_t t_origin;   // first step simulated by this handle (0, or the t a checkpoint was restored at)
     uint64_t routed_upto; // queue mode: steps < routed_upto have had their queued events routed
     // delivery of step t overlaps the update of step t+1 (see gn_step): side streams and their fences
     cudaStream_t s_deliver;
@@ -209,6 +210,7 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
     net->stream = (cudaStream_t)cuda_stream;
     net->ws = (uint8_t *)workspace;
     net->t = 0;
+    net->t_origin = 0;
     net->routed_upto = 0;
     net->s_deliver = nullptr;
     net->ev_update = net->ev_deliver[0] = net->ev_deliver[1] = net->ev_fold[0] = net->ev_fold[1] = net->ev_fold[2] = net->ev_fold[3] = nullptr;
@@ -646,6 +648,9 @@ int gn_read_state(gn_net *net, int which, void *dst, size_t dst_bytes, int dst_i
     case GN_BIAS:
         if (!net->has_bias) return set_err(net, GN_E_INVALID_ARG, "no bias set");
         src = d.bias; need = N * 4; break;
+    case GN_ACC:
+        if (!d.acc) return set_err(net, GN_E_INVALID_ARG, "no frame accumulator when obs_stride == 0");
+        src = d.acc; need = N * 4; break;
     case GN_RING: need = (size_t)d.D * N * 4; break;
     case GN_STEP: src = d.counters; need = 8; break;
     case GN_COUNTERS: {
@@ -688,9 +693,37 @@ int gn_write_state(gn_net *net, int which, const void *src, size_t src_bytes, in
         dst = d.c; break;
     case GN_REFR: dst = d.refr; need = N; break;
     case GN_BIAS: dst = d.bias; break;
+    case GN_ACC:
+        if (!d.acc) return set_err(net, GN_E_INVALID_ARG, "no frame accumulator when obs_stride == 0");
+        dst = d.acc; break;
+    case GN_RING: need = (size_t)d.D * N * 4; break;
+    case GN_STEP: need = 8; break;
+    case GN_COUNTERS: need = 32; break;
     default: return set_err(net, GN_E_INVALID_ARG, "state id %d is not writable", which);
     }
     if (src_bytes < need) return set_err(net, GN_E_INVALID_ARG, "src has %zu bytes, need %zu", src_bytes, need);
+    if (which == GN_RING || which == GN_STEP || which == GN_COUNTERS) {      // checkpoint / restore
+        int rc = flush_delivery(net, true);       // queue mode: every pending record goes into the ring first, buckets end empty
+        if (rc) return rc;
+        const cudaMemcpyKind kind = src_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+        if (which == GN_RING) {                   // caller rows are N wide, internal rows Npad wide
+            GN_CUDA(net, cudaMemcpy2DAsync(d.ring, (size_t)d.Npad * 4, src, N * 4, N * 4, d.D, kind, net->stream));
+            GN_CUDA(net, cudaStreamSynchronize(net->stream));
+            return GN_OK;
+        }
+        // GN_STEP: the number of completed steps t (uint64) -- the generator index, ring slot and frame phase follow from
+        // it; GN_COUNTERS: all four counters (its first word is t as well).  The raster / trace windows start empty at t.
+        unsigned long long c[4] = {0, 0, 0, 0};
+        GN_CUDA(net, cudaMemcpyAsync(c, src, need, src_is_device ? cudaMemcpyDeviceToHost : cudaMemcpyHostToHost, net->stream));
+        GN_CUDA(net, cudaStreamSynchronize(net->stream));
+        if (which == GN_STEP) GN_CUDA(net, cudaMemcpyAsync(d.counters, c, 8, cudaMemcpyHostToDevice, net->stream));
+        else GN_CUDA(net, cudaMemcpyAsync(d.counters, c, 32, cudaMemcpyHostToDevice, net->stream));
+        GN_CUDA(net, cudaStreamSynchronize(net->stream));
+        net->t = c[0];
+        net->routed_upto = c[0];
+        net->t_origin = c[0];
+        return GN_OK;
+    }
     GN_CUDA(net, cudaMemcpyAsync(dst, src, need, src_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, net->stream));
     if (!src_is_device) GN_CUDA(net, cudaStreamSynchronize(net->stream));
     if (which == GN_BIAS) net->has_bias = true;
@@ -723,7 +756,7 @@ int gn_read_raster(gn_net *net, uint64_t t0, uint64_t n_steps, uint32_t *bits, s
     if (n_steps == 0) return GN_OK;
     if (!bits) return set_err(net, GN_E_INVALID_ARG, "bits is NULL");
     if (dst_bytes < n_steps * words * 4) return set_err(net, GN_E_INVALID_ARG, "dst has %zu bytes, need %zu", dst_bytes, (size_t)(n_steps * words * 4));
-    if (t0 + n_steps > net->t || d.raster_cap == 0 || t0 + d.raster_cap < net->t)
+    if (t0 + n_steps > net->t || d.raster_cap == 0 || t0 + d.raster_cap < net->t || t0 < net->t_origin)
         return set_err(net, GN_E_RANGE_EVICTED, "raster steps [%llu, %llu) not held: simulated %llu, window %u",
                        (unsigned long long)t0, (unsigned long long)(t0 + n_steps), (unsigned long long)net->t, d.raster_cap);
     return copy_window(net, bits, (const uint8_t *)d.raster, (size_t)d.words_pad * 4, words * 4, d.raster_rows, t0, n_steps, dst_is_device);
@@ -738,7 +771,7 @@ int gn_observe(gn_net *net, uint64_t frame0, uint64_t n_frames, float *trace, si
     if (!trace) return set_err(net, GN_E_INVALID_ARG, "trace is NULL");
     const uint64_t have = net->t / d.obs_stride;
     if (dst_bytes < n_frames * d.N * 4) return set_err(net, GN_E_INVALID_ARG, "dst has %zu bytes, need %zu", dst_bytes, (size_t)(n_frames * d.N * 4));
-    if (frame0 + n_frames > have || frame0 + d.trace_cap < have)
+    if (frame0 + n_frames > have || frame0 + d.trace_cap < have || frame0 < net->t_origin / d.obs_stride)
         return set_err(net, GN_E_RANGE_EVICTED, "frames [%llu, %llu) not held: emitted %llu, window %u",
                        (unsigned long long)frame0, (unsigned long long)(frame0 + n_frames), (unsigned long long)have, d.trace_cap);
     return copy_window(net, trace, (const uint8_t *)d.trace, (size_t)d.Npad * 4, (size_t)d.N * 4, d.trace_cap, frame0, n_frames, dst_is_device);

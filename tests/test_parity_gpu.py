@@ -331,6 +331,39 @@ def test_paper_test_set_all_80_networks_in_one_handle(gn, mode):
     np.testing.assert_allclose(gn.gn_observe(g, 0, frames).astype(np.float64), o.trace(0, frames), rtol=1e-6, atol=1e-5)
 
 
+@pytest.mark.parametrize("k,n,nb,mode", [(4, 6_001, None, "QUEUE"), (2, 3_000, None, "RING"), (5, 700, 5, "RESIDENT")])
+def test_checkpoint_restore_continues_bit_identically(gn, k, n, nb, mode):
+    """y_j plus the in-flight delayed signals Y_j are the whole state: V, W, R, P, CA, ACC, REFR,
+    RING and COUNTERS read from one handle at an arbitrary step (inside a slot group, inside a camera frame) and
+    written into a FRESH handle make it continue exactly like the original -- and like the oracle."""
+    net, cfg = make_config(k, n=n, n_networks=nb)
+    cfg = dict(cfg, obs_stride=25, classes=[dict(c, psc_alpha=1.0) if i == 0 else c for i, c in enumerate(cfg["classes"])])
+    dm = getattr(gn, "GN_DELIVER_" + mode)
+    t_save, t_more = 1013, 487
+    a = gn.create_from_inputs(net, cfg, raster_capacity_steps=t_more, trace_capacity_frames=64, delivery_mode=dm)
+    o = Oracle(net, cfg, "fp32", threads=4)
+    gn.gn_step(a, t_save)
+    o.step(t_save)
+    ids = (gn.GN_V, gn.GN_W, gn.GN_R, gn.GN_P, gn.GN_CA, gn.GN_ACC, gn.GN_REFR, gn.GN_RING, gn.GN_COUNTERS)
+    snap = {w: gn.gn_read_state(a, w).copy() for w in ids}
+    b = gn.create_from_inputs(net, cfg, raster_capacity_steps=t_more, trace_capacity_frames=64, delivery_mode=dm)
+    for w in ids:
+        gn.gn_write_state(b, w, snap[w])
+    with pytest.raises(gn.GnError):
+        gn.gn_read_raster(b, t_save - 1, 1)                       # before the restored step: not held
+    gn.gn_step(a, t_more)
+    gn.gn_step(b, t_more)
+    o.step(t_more)
+    _compare_exact(gn, b, o, t_save + t_more)
+    np.testing.assert_array_equal(gn.gn_read_raster(b, t_save, t_more), o.raster(t_save, t_more))
+    np.testing.assert_array_equal(gn.gn_read_raster(b, t_save, t_more), gn.gn_read_raster(a, t_save, t_more))
+    f0, f1 = t_save // 25, (t_save + t_more) // 25                # the frame in progress at the checkpoint included
+    np.testing.assert_array_equal(gn.gn_observe(b, f0, f1 - f0), gn.gn_observe(a, f0, f1 - f0))
+    for w in ids:
+        np.testing.assert_array_equal(gn.gn_read_state(b, w), gn.gn_read_state(a, w))
+    assert o.counters()["delivered"] > 0
+
+
 def test_queue_mode_reads_inside_a_group_and_odd_step_counts(gn):
     """Queue mode routes once per slot group and the update kernel sends the near events itself: stepping by
     counts that are not multiples of the group, and reading ring / counters in the middle of a group, must
