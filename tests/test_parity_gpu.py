@@ -169,22 +169,24 @@ def test_queue_mode_ring_depth_not_a_multiple_of_the_group(gn):
 
 
 def test_config4_full_size_in_the_benchmark_configuration(gn):
-    """BASELINE configs[3] at FULL size (10^6 vertices, ~2*10^8 edges, D = 128), created exactly as bench.py
-    creates it (AUTO delivery = queue mode, no raster window beyond the benchmark's): rasters, counters, state
-    words and the whole 512 MB ring bit-exact against the fp32-faithful oracle after 1,500 steps (the network is
-    bursting by then: > 10^8 events delivered)."""
+    """BASELINE configs[3] at FULL size (10^6 vertices, ~2*10^8 edges, D = 128), created exactly as bench.py creates it
+    (AUTO delivery = queue mode), for the config's WHOLE 10,000 steps: every raster row, the counters every 500 steps,
+    and at the end the state words and the whole 512 MB ring, bit-exact against the fp32-faithful oracle
+    (5.9e7 spikes, 1.2e10 delivered events, bursts of up to 5.8e6 events per step)."""
     import os
     net, cfg = make_config(4)
     cfg = dict(cfg, obs_stride=0)
-    steps = 1500
-    g = _make(gn, net, cfg, 100)
+    steps, chunk = cfg["steps"], 500
+    g = _make(gn, net, cfg, chunk)
     o = Oracle(net, cfg, "fp32", threads=len(os.sched_getaffinity(0)))
-    for done in range(100, steps + 1, 100):
-        gn.gn_step(g, 100)
-        o.step(100)
-        np.testing.assert_array_equal(gn.gn_read_raster(g, done - 100, 100), o.raster(done - 100, 100))
+    for done in range(chunk, steps + 1, chunk):
+        gn.gn_step(g, chunk)
+        o.step(chunk)
+        np.testing.assert_array_equal(gn.gn_read_raster(g, done - chunk, chunk), o.raster(done - chunk, chunk))
+        c, oc = gn.gn_read_state(g, gn.GN_COUNTERS), o.counters()
+        assert (int(c[1]), int(c[2]), int(c[3])) == (oc["spikes"], oc["delivered"], oc["kicks"]), done
     _compare_exact(gn, g, o, steps)
-    assert o.counters()["delivered"] > 10 ** 8
+    assert o.counters()["delivered"] > 10 ** 10
 
 
 def test_config3_full_size_2000_steps(gn):
