@@ -199,12 +199,12 @@ def test_config3_full_size_2000_steps(gn):
 
 def test_config5_full_size_batched(gn):
     """BASELINE configs[4] at full size: 4,096 networks of 1,000 vertices in ONE handle (block-diagonal CSR,
-    ~7.7*10^7 edges, D = 32, observation stride 100), 500 steps, everything bit-exact, trace within tolerance."""
+    ~7.7*10^7 edges, D = 32, observation stride 100), the first 2,000 steps, everything bit-exact, trace within tolerance."""
     import os
     net, cfg = make_config(5)
-    g, o, _ = _run_exact(gn, net, cfg, 500, 250, threads=len(os.sched_getaffinity(0)))
-    assert o.counters()["delivered"] > 10 ** 5
-    frames = 500 // cfg["obs_stride"]
+    g, o, _ = _run_exact(gn, net, cfg, 2000, 1000, threads=len(os.sched_getaffinity(0)))
+    assert o.counters()["delivered"] > 10 ** 6
+    frames = 2000 // cfg["obs_stride"]
     np.testing.assert_allclose(gn.gn_observe(g, 0, frames).astype(np.float64), o.trace(0, frames), rtol=1e-6, atol=1e-5)
 
 
