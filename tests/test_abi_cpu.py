@@ -34,6 +34,16 @@ def test_structs_match_header_layout():
     assert gn.gn_config.delivery_mode.offset == 80 and gn.gn_config.queue_capacity.offset == 88
 
 
+def test_binding_constants_match_the_header():
+    """Every GN_* id of include/gn.h (state ids, delivery modes, error codes) has the same value in the binding."""
+    text = open(os.path.join(ROOT, "include", "gn.h")).read()
+    enum = dict(re.findall(r"\b(GN_[A-Z_]+)\s*=\s*(\d+)", text))
+    defs = dict(re.findall(r"#define\s+(GN_[A-Z_]+)\s+\(?(-?\d+)\)?", text))
+    assert {"GN_V", "GN_RING", "GN_P", "GN_ACC"} <= set(enum) and {"GN_OK", "GN_E_CUDA", "GN_DELIVER_RESIDENT"} <= set(defs)
+    for name, val in {**enum, **defs}.items():
+        assert getattr(gn.binding, name) == int(val), name
+
+
 def test_query_workspace_sizes_and_errors():
     cfg = gn.make_config(1_000_000, 3, 200_000_000, 128, 0.1, 0.006, 2, raster_capacity_steps=0,
                          delivery_mode=gn.GN_DELIVER_RING)
