@@ -367,6 +367,27 @@ def test_checkpoint_restore_continues_bit_identically(gn, k, n, nb, mode):
     assert o.counters()["delivered"] > 0
 
 
+def test_two_handles_interleaved(gn):
+    """No global state: two networks in different delivery modes, stepped alternately in uneven chunks, each bit-exact."""
+    na, ca = make_config(4, n=5_003)
+    nb_, cb = make_config(5, n=400, n_networks=7)
+    a = _make(gn, na, ca, 900, delivery_mode=gn.GN_DELIVER_QUEUE)
+    b = _make(gn, nb_, cb, 900)
+    oa, ob_ = Oracle(na, ca, "fp32", threads=4), Oracle(nb_, cb, "fp32", threads=4)
+    done_a = done_b = 0
+    for ka, kb in ((7, 300), (293, 1), (100, 99), (500, 500)):
+        gn.gn_step(a, ka)
+        gn.gn_step(b, kb)
+        oa.step(ka)
+        ob_.step(kb)
+        done_a += ka
+        done_b += kb
+    _compare_exact(gn, a, oa, done_a)
+    _compare_exact(gn, b, ob_, done_b)
+    np.testing.assert_array_equal(gn.gn_read_raster(a, 0, done_a), oa.raster(0, done_a))
+    np.testing.assert_array_equal(gn.gn_read_raster(b, 0, done_b), ob_.raster(0, done_b))
+
+
 def test_queue_mode_reads_inside_a_group_and_odd_step_counts(gn):
     """Queue mode routes once per slot group and the update kernel sends the near events itself: stepping by
     counts that are not multiples of the group, and reading ring / counters in the middle of a group, must
