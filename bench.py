@@ -188,7 +188,18 @@ def cpu_baseline(net_in, cfg, budget_s=20.0):
     o.step(n_steps)
     dt = time.time() - t0
     c1 = o.counters()
-    return {"value": net_in.n_vertices * n_steps / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+    # one thread as well (the paper's own CPU baseline was a single thread): a shorter sample
+    o1 = Oracle(net_in, cfg, "fp32", threads=1)
+    t1 = time.time()
+    o1.step(2)
+    per1 = max((time.time() - t1) / 2, 1e-6)
+    n1 = int(max(3, min(500, 6.0 / per1)))
+    t1 = time.time()
+    o1.step(n1)
+    dt1 = time.time() - t1
+    one = {"value": net_in.n_vertices * n1 / dt1, "unit": UNIT, "cores": 1,
+           "sample": f"{n1} simulated steps of the same network from rest, one thread"}
+    return {"value": net_in.n_vertices * n_steps / dt, "unit": UNIT, "cores": cores, "kind": "oracle", "one_thread": one,
             "sample": f"{n_steps} simulated steps of the same full-size network from rest (fp32-faithful mode, OpenMP), "
                       f"{c1['delivered'] - c0['delivered']} events delivered",
             "events_per_s": (c1["delivered"] - c0["delivered"]) / dt,
