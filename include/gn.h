@@ -43,7 +43,8 @@ extern "C" {
 #define GN_OK 0
 #define GN_E_INVALID_ARG (-1)         /* NULL pointer, bad scalar, unsupported size               */
 #define GN_E_BAD_GRAPH (-2)           /* row offsets not monotone / target out of range / delay   */
-                                      /* 0 or >= ring_slots / edge crossing networks / class id   */
+                                      /* 0 or >= ring_slots / edge crossing networks / class id / */
+                                      /* NaN or infinite position on an edge when delays == NULL  */
 #define GN_E_OVERFLOW_RISK (-3)       /* some target's sum |w_fx| (+ largest kick) >= 2^31        */
 #define GN_E_WORKSPACE_TOO_SMALL (-4)
 #define GN_E_RANGE_EVICTED (-5)       /* raster / trace range not (or no longer) held             */

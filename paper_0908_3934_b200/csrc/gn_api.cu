@@ -113,6 +113,7 @@ Layout make_layout(const gn_config *cfg)
 }  // namespace
 
 struct gn_net {
+    int device;          // CUDA device of the workspace: every entry point runs with it current (DeviceGuard)
     gn_config cfg;
     GnDev dev;
     Layout lay;
@@ -149,6 +150,23 @@ int set_err(gn_net *net, int code, const char *fmt, ...)
     va_end(ap);
     return code;
 }
+
+// Makes `device` current for the lifetime of the guard and restores the caller's device afterwards: a handle works
+// from any thread whatever device is current there (multi-replica hosts).
+struct DeviceGuard {
+    int prev = -1, want;
+    explicit DeviceGuard(int device) : want(device)
+    {
+        if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
+        if (prev != want) cudaSetDevice(want);
+    }
+    ~DeviceGuard()
+    {
+        if (prev >= 0 && prev != want) cudaSetDevice(prev);
+    }
+    DeviceGuard(const DeviceGuard &) = delete;
+    DeviceGuard &operator=(const DeviceGuard &) = delete;
+};
 
 #define GN_CUDA(net, call)                                                                        \
     do {                                                                                          \
@@ -203,8 +221,10 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
     if (attr.type != cudaMemoryTypeDevice && attr.type != cudaMemoryTypeManaged)
         return set_err(nullptr, GN_E_INVALID_ARG, "workspace is not device memory");
 
+    DeviceGuard guard(attr.device);           // the workspace's device, whatever is current in this thread
     gn_net *net = new (std::nothrow) gn_net();
     if (!net) return set_err(nullptr, GN_E_INVALID_ARG, "out of host memory");
+    net->device = attr.device;
     net->cfg = *cfg;
     net->lay = L;
     net->stream = (cudaStream_t)cuda_stream;
@@ -304,6 +324,7 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
     do {                                                                                          \
         cudaError_t e_ = (call);                                                                  \
         if (e_ != cudaSuccess) {                                                                  \
+            cudaStreamSynchronize(st);   /* copies from caller buffers may still be in flight */  \
             delete net;                                                                           \
             return set_err(nullptr, GN_E_CUDA, "%s failed: %s", #call, cudaGetErrorString(e_));    \
         }                                                                                         \
@@ -391,7 +412,7 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
     d.fused = (!d.resident && !d.queue_mode && Npad <= (1u << 18)) ? 1u : 0u;
     if (E) {
         GN_CREATE_CUDA(gnk_quantise(d, E, chk_d, st));
-        if (!delays) GN_CREATE_CUDA(gnk_delays_from_positions(d, pos_d, cfg->dim, cfg->speed, st));
+        if (!delays) GN_CREATE_CUDA(gnk_delays_from_positions(d, pos_d, cfg->dim, cfg->speed, chk_d, st));
         GN_CREATE_CUDA(gnk_validate(d, net_offsets ? net_d : nullptr, cfg->n_networks, abs_in, chk_d, st));
     }
     GN_CREATE_CUDA(gnk_check_overflow(d, abs_in, chk_d, st));
@@ -400,10 +421,11 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
     GN_CREATE_CUDA(cudaMemcpyAsync(&chk, chk_d, sizeof chk, cudaMemcpyDeviceToHost, st));
     GN_CREATE_CUDA(cudaStreamSynchronize(st));
 #undef GN_CREATE_CUDA
-    if (chk.bad_target || chk.bad_delay || chk.cross_net || chk.bad_weight) {
+    if (chk.bad_target || chk.bad_delay || chk.cross_net || chk.bad_weight || chk.bad_position) {
         delete net;
         return set_err(nullptr, GN_E_BAD_GRAPH, "%s",
                        chk.bad_target ? "targets: id >= n_vertices"
+                       : chk.bad_position ? "positions: NaN or infinite coordinate on an edge (eq. 25 has no delay for it)"
                        : chk.bad_delay ? "delay outside [1, ring_slots-1]"
                        : chk.cross_net ? "edge crosses two networks"
                                        : "weight is NaN or outside the int32 fixed-point range");
@@ -512,6 +534,7 @@ static int route_pending(gn_net *net, cudaStream_t st, bool prof, uint32_t fold_
 int gn_step(gn_net *net, uint64_t n_steps)
 {
     if (!net) return GN_E_INVALID_ARG;
+    DeviceGuard guard(net->device);
     const GnDev &d = net->dev;
     const uint32_t G = 1u << d.q_log;
     if (d.resident) {      // the whole call is one launch (or a few, so that a kept raster window is never lapped)
@@ -602,6 +625,7 @@ static int flush_delivery(gn_net *net, bool fold_too)
 int gn_profile(gn_net *net, int enable)
 {
     if (!net) return GN_E_INVALID_ARG;
+    DeviceGuard guard(net->device);
     int rc = join_streams(net);
     if (rc) return rc;
     net->profile = enable != 0;
@@ -615,6 +639,7 @@ int gn_profile(gn_net *net, int enable)
 int gn_profile_read(gn_net *net, double ms[4], uint64_t launches[5])
 {
     if (!net) return GN_E_INVALID_ARG;
+    DeviceGuard guard(net->device);
     if (!ms || !launches) return set_err(net, GN_E_INVALID_ARG, "NULL output");
     for (int k = 0; k < 4; ++k) { ms[k] = net->prof_ms[k]; launches[k] = net->prof_n[k]; }
     launches[4] = net->launches;
@@ -631,6 +656,7 @@ static int copy_out(gn_net *net, void *dst, const void *src, size_t bytes, int d
 int gn_read_state(gn_net *net, int which, void *dst, size_t dst_bytes, int dst_is_device)
 {
     if (!net) return GN_E_INVALID_ARG;
+    DeviceGuard guard(net->device);
     if (!dst) return set_err(net, GN_E_INVALID_ARG, "dst is NULL");
     const GnDev &d = net->dev;
     const size_t N = d.N, E = net->cfg.n_edges;
@@ -678,6 +704,7 @@ int gn_read_state(gn_net *net, int which, void *dst, size_t dst_bytes, int dst_i
 int gn_write_state(gn_net *net, int which, const void *src, size_t src_bytes, int src_is_device)
 {
     if (!net) return GN_E_INVALID_ARG;
+    DeviceGuard guard(net->device);
     if (!src) return set_err(net, GN_E_INVALID_ARG, "src is NULL");
     const GnDev &d = net->dev;
     const size_t N = d.N;
@@ -751,6 +778,7 @@ static int copy_window(gn_net *net, void *dst, const uint8_t *base, size_t pitch
 int gn_read_raster(gn_net *net, uint64_t t0, uint64_t n_steps, uint32_t *bits, size_t dst_bytes, int dst_is_device)
 {
     if (!net) return GN_E_INVALID_ARG;
+    DeviceGuard guard(net->device);
     const GnDev &d = net->dev;
     const size_t words = ((size_t)d.N + 31) / 32;
     if (n_steps == 0) return GN_OK;
@@ -765,6 +793,7 @@ int gn_read_raster(gn_net *net, uint64_t t0, uint64_t n_steps, uint32_t *bits, s
 int gn_observe(gn_net *net, uint64_t frame0, uint64_t n_frames, float *trace, size_t dst_bytes, int dst_is_device)
 {
     if (!net) return GN_E_INVALID_ARG;
+    DeviceGuard guard(net->device);
     const GnDev &d = net->dev;
     if (!d.obs_stride) return set_err(net, GN_E_INVALID_ARG, "observation is off (obs_stride == 0)");
     if (n_frames == 0) return GN_OK;
@@ -790,6 +819,7 @@ const char *gn_last_error(const gn_net *net) { return net ? net->err : g_create_
 int gn_destroy(gn_net *net)
 {
     if (!net) return GN_E_INVALID_ARG;
+    DeviceGuard guard(net->device);
     if (net->s_deliver) cudaStreamSynchronize(net->s_deliver);
     cudaError_t e = cudaStreamSynchronize(net->stream);
     for (cudaEvent_t ev : net->ev) cudaEventDestroy(ev);

@@ -81,6 +81,7 @@ struct GnDev {
 struct GnCheck {
     uint32_t bad_row, bad_target, bad_delay, bad_class, bad_weight, cross_net, overflow;
     uint32_t big_degree;     // some out-degree > 65535: the 16-bit segment table of queue mode cannot hold it
+    uint32_t bad_position;   // a NaN / infinite coordinate reached eq. 25
 };
 
 // ---- launchers (gn_kernels.cu).  All asynchronous on `st`; return the launch error. ----
@@ -98,7 +99,7 @@ cudaError_t gnk_convert_rows(const GnDev &p, const uint64_t *row64, uint64_t n_e
                              cudaStream_t st);
 cudaError_t gnk_quantise(const GnDev &p, uint64_t n_edges, GnCheck *chk, cudaStream_t st);
 cudaError_t gnk_delays_from_positions(const GnDev &p, const float *pos, uint32_t dim, float speed,
-                                      cudaStream_t st);
+                                      GnCheck *chk, cudaStream_t st);
 cudaError_t gnk_validate(const GnDev &p, const uint32_t *net_of_vertex_offsets, uint32_t n_networks,
                          unsigned long long *abs_in, GnCheck *chk, cudaStream_t st);
 cudaError_t gnk_check_overflow(const GnDev &p, const unsigned long long *abs_in, GnCheck *chk,

@@ -785,7 +785,7 @@ gn_resident_kernel(const GnDev p, const uint64_t t0, const uint32_t n_steps, con
             uint32_t *rowp = p.raster + (size_t)raster_row * p.words_pad + (jw >> 5);
             if (lane == 0u) {
                 atomicOr(rowp, fired_mask << sh);
-                if (sh) atomicOr(rowp + 1, fired_mask >> (32u - sh));
+                if (sh && (fired_mask >> (32u - sh))) atomicOr(rowp + 1, fired_mask >> (32u - sh));   // never past the row
             }
         }
         // a4: every fired vertex of the warp in turn, lanes over its row, shared-memory integer atomics
@@ -911,7 +911,8 @@ __global__ void gn_quantise_kernel(const GnDev p, const uint64_t n_edges, GnChec
 }
 
 // PAPER.md:251 eq. 25 in steps: max(1, ceil(|x_i - x_j| / (speed * dt))), double, no contraction.
-__global__ void gn_delays_kernel(const GnDev p, const float *__restrict__ pos, const uint32_t dim, const float speed)
+__global__ void gn_delays_kernel(const GnDev p, const float *__restrict__ pos, const uint32_t dim, const float speed,
+                                 GnCheck *chk)
 {
     const uint32_t lane = threadIdx.x & 31u;
     const uint32_t i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
@@ -929,7 +930,8 @@ __global__ void gn_delays_kernel(const GnDev p, const float *__restrict__ pos, c
             }
         }
         double steps = ceil(__ddiv_rn(__dsqrt_rn(d2), per_step));
-        if (!(steps >= 1.0)) steps = 1.0;                   // coincident points (reading #7); NaN -> flagged below
+        if (!(d2 < 1e300)) chk->bad_position = 1u;          // NaN or infinite coordinate: no distance, no delay
+        if (!(steps >= 1.0)) steps = 1.0;                   // coincident points (reading #7)
         if (steps > 255.0) steps = 255.0;                   // >= D is rejected by the validation kernel
         p.dly[e] = (uint8_t)steps;
     }
@@ -1169,9 +1171,9 @@ cudaError_t gnk_quantise(const GnDev &p, uint64_t n_edges, GnCheck *chk, cudaStr
     return cudaGetLastError();
 }
 
-cudaError_t gnk_delays_from_positions(const GnDev &p, const float *pos, uint32_t dim, float speed, cudaStream_t st)
+cudaError_t gnk_delays_from_positions(const GnDev &p, const float *pos, uint32_t dim, float speed, GnCheck *chk, cudaStream_t st)
 {
-    gn_delays_kernel<<<ceil_div((uint64_t)p.N * 32, 256), 256, 0, st>>>(p, pos, dim, speed);
+    gn_delays_kernel<<<ceil_div((uint64_t)p.N * 32, 256), 256, 0, st>>>(p, pos, dim, speed, chk);
     return cudaGetLastError();
 }
 

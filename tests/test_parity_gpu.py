@@ -14,7 +14,7 @@ import numpy as np
 import pytest
 
 from gn_inputs import Network, make_config
-from helpers import base_cfg, hand_net, random_digraph, rs_class, unpack_raster
+from helpers import Fp64Gate, base_cfg, hand_net, random_digraph, rs_class, unpack_raster
 from oracle import Oracle
 from oracle import binding as ob
 
@@ -454,41 +454,34 @@ def test_out_degree_above_16_bits_falls_back_to_the_ring_path(gn):
     assert o.counters()["delivered"] >= deg
 
 
-@pytest.mark.parametrize("k,n,nb,steps", [(1, None, None, 2000), (2, None, None, 2000), (4, 9_001, None, 2000)])
+@pytest.mark.parametrize("k,n,nb,steps", [(1, None, None, 2000), (2, None, None, 2000), (3, 6_007, None, 2000),
+                                          (4, 9_001, None, 2000), (5, 1000, 6, 2000)])
 def test_state_within_tolerance_of_fp64_until_divergence(gn, k, n, nb, steps):
-    """GPU vs the fp64 DEFINITION: rasters identical up to t*, state within 1e-4 rel / 1e-5 abs for
-    >= 99.9 % of (vertex, checkpoint) samples up to t*; beyond it >= 99.9 % raster agreement.  t* is
-    printed (reported, not hidden)."""
+    """GPU vs the fp64 DEFINITION, every config: rasters identical up to the first divergence t* (printed), and up to
+    t* every (vertex, checkpoint, variable) sample classed from the rasters and the fp64 state alone (helpers.Fp64Gate,
+    DESIGN.md "fp64 gate"): quiet samples within 1e-4 rel / 1e-5 abs STRICTLY; recovery samples (a spike or an
+    excursion above V_exp within the last 1,000 steps) within 20 x that; upstroke samples (a spike within the next 30
+    steps) unbounded, counted and their worst error printed; violators of the plain tolerance < 0.1 % of all samples.
+    Beyond t*: >= 99.9 % raster cell agreement over the whole horizon."""
     net, cfg = make_config(k, n=n, n_networks=nb)
     cfg = dict(cfg, obs_stride=0)
-    g = _make(gn, net, cfg, steps)
+    gate, chunk = Fp64Gate(net.n_vertices), 50
+    g = _make(gn, net, cfg, steps + gate.pre)
     o = Oracle(net, cfg, "fp64", threads=4)
-    chunk, t_star, bad, tot = 50, None, 0, 0
+    names = (("V", gn.GN_V, ob.V), ("W", gn.GN_W, ob.W), ("R", gn.GN_R, ob.R))
     for done in range(chunk, steps + 1, chunk):
         gn.gn_step(g, chunk)
         o.step(chunk)
-        rg = gn.gn_read_raster(g, done - chunk, chunk)
-        ro = o.raster(done - chunk, chunk)
-        if t_star is None and not np.array_equal(rg, ro):
-            t_star = done - chunk + int(np.nonzero((rg != ro).any(axis=1))[0][0])
-        if t_star is None:
-            for which_g, which_o in ((gn.GN_V, ob.V), (gn.GN_W, ob.W), (gn.GN_R, ob.R)):
-                a = gn.gn_read_state(g, which_g).astype(np.float64)
-                b = o.state(which_o)
-                viol = np.abs(a - b) > ABS + REL * np.abs(b)
-                # exceptions (DESIGN.md "Tolerances"): a vertex on its spike upstroke amplifies any rounding
-                # difference super-linearly (quadratic term), the overshoot lands in W through b*V and lingers
-                # after the reset.  They must stay under 0.1 % of all (vertex, checkpoint) samples.
-                bad += int(viol.sum())
-                tot += viol.size
-    assert bad <= 1e-3 * tot, (bad, tot)
-    rg = unpack_raster(gn.gn_read_raster(g, 0, steps), net.n_vertices)
-    ro = o.raster_bool(0, steps)
+        gate.add(done, {w: gn.gn_read_state(g, wg) for w, wg, _ in names}, {w: o.state(wo) for w, _, wo in names})
+    gn.gn_step(g, gate.pre)
+    o.step(gate.pre)
+    rg = unpack_raster(gn.gn_read_raster(g, 0, steps + gate.pre), net.n_vertices)
+    ro = o.raster_bool(0, steps + gate.pre)
+    t_star, stats = gate.check(rg, ro, f"CUDA vs fp64 oracle, cfg {k}")
     agree = float((rg == ro).mean())
     print(f"[cfg {k}] fp32-GPU vs fp64-oracle: first raster divergence t* = {t_star}, cell agreement {agree:.6f}")
     assert agree >= 0.999
-    if t_star is not None:
-        np.testing.assert_array_equal(rg[:t_star], ro[:t_star])
+    assert stats["quiet"] > 0.3 * stats["samples"]
 
 
 def test_full_run_raster_agreement_beyond_the_divergence(gn):
@@ -696,6 +689,12 @@ def test_create_rejects_bad_graphs(gn):
     with pytest.raises(gn.GnError) as ei:
         gn.create_from_inputs(net, cfg, delays=dl)
     assert ei.value.code == gn.GN_E_OVERFLOW_RISK
+    pos = np.zeros((4, 2), np.float32)                                     # eq. 25 from a NaN coordinate: no delay exists
+    pos[1, 0] = np.nan
+    net, _ = hand_net(4, [(0, 1, 1.0, 0), (2, 3, 1.0, 0)], positions=pos)
+    with pytest.raises(gn.GnError) as ei:
+        gn.create_from_inputs(net, cfg)
+    assert ei.value.code == gn.GN_E_BAD_GRAPH
     net, dl = hand_net(4, [(0, 3, 1.0, 1)])                                # edge across two networks
     net.n_networks, net.net_offsets = 2, np.array([0, 2, 4], np.uint32)
     with pytest.raises(gn.GnError) as ei:
