@@ -103,6 +103,19 @@ class ClockSampler:
                 "samples": len(sm)}
 
 
+def measured_traffic():
+    """Per-launch DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of each kernel from the committed
+    `ncu --set full` capture: profiles/traffic.csv, whose first line names the capture and its step range."""
+    path = os.path.join(ROOT, "profiles", "traffic.csv")
+    try:
+        lines = [l.strip() for l in open(path).read().splitlines() if l.strip()]
+        src = lines[0].lstrip("# ") if lines[0].startswith("#") else "profiles/traffic.csv"
+        rows = [l for l in lines if not l.startswith("#")][1:]
+        return {k: float(v) for k, v in (r.split(",")[:2] for r in rows)}, src
+    except Exception:
+        return {}, None
+
+
 def rank_seed(config, rank):
     """Replicas only: rank r steps its own independent network of the same recipe."""
     from gn_inputs import MASTER_SEED
@@ -299,13 +312,20 @@ def main():
     sim_steps = K * S
     value = world * N * sim_steps / sec
 
-    # ---- per-kernel pass: the same K steps again, every launch bracketed by CUDA events ------------
-    gn.gn_profile(g, True)
+    # ---- per-kernel pass: EXACTLY the timed steps again (the run is deterministic and starts from rest, so a
+    # fresh handle stepped through the same W warm-up steps is in the state the timed pass started from), this
+    # time with a CUDA event wherever the kind of kernel changes (gn_profile: everything serialised on one stream)
+    del g
+    g = create()
+    for _ in range(W):
+        gn.gn_step(g, S)
     cp0 = counters(g)
+    gn.gn_profile(g, True)
     gn.gn_step(g, sim_steps)
     kms, kn = gn.gn_profile_read(g)
     gn.gn_profile(g, False)
     cp1 = counters(g)
+    assert cp0 == c0 and cp1 == c1, "the per-kernel pass did not replay the timed steps"
     peak, peak_src = peaks()
     queue_mode = 0 < kn[1] < kn[0]      # queue mode delivers once per slot group, ring mode every step
     resident = kn[1] == 0 and kn[0] < sim_steps
@@ -323,13 +343,19 @@ def main():
               delivery_bytes / max(int(kn[1]), 1),
               N * 8.0,
               p_events * 8.0 / max(int(kn[3]), 1)]
+    traffic_tab, traffic_src = measured_traffic()
     kernels = []
     for k in range(4):
         if kn[k] == 0:
             continue
         avg_s = kms[k] * 1e-3 / kn[k]
-        kernels.append({"kernel": names[k], "launches": int(kn[k]), "avg_us": avg_s * 1e6, "share": float(kms[k] / kms.sum()),
-                        "bytes_per_launch": kbytes[k], "achieved": kbytes[k] / avg_s / 1e9, "frac": kbytes[k] / avg_s / 1e9 / peak})
+        row = {"kernel": names[k], "launches": int(kn[k]), "avg_us": avg_s * 1e6, "share": float(kms[k] / kms.sum()),
+               "bytes_per_launch": kbytes[k], "achieved": kbytes[k] / avg_s / 1e9, "frac": kbytes[k] / avg_s / 1e9 / peak}
+        tr = traffic_tab.get(names[k].split()[0])
+        if tr is not None:      # what DRAM really moved for this kernel (ncu capture named in traffic_source) over the live time
+            row["traffic"] = tr
+            row["dram_frac"] = tr / avg_s / 1e9 / peak
+        kernels.append(row)
     a4_s = (kms[1] + kms[3]) * 1e-3
     a4 = {"what": "a4 delivery as a whole (routing + folding), 17 B per event + 12 B per fired source",
           "bytes": p_events * EVENT_BYTES + p_spikes * SOURCE_BYTES, "ms": a4_s * 1e3,
@@ -343,20 +369,20 @@ def main():
         a4["lsu"] = {"bound": "lsu-issue", "achieved": p_events / a4_s, "peak": lsu_peak, "unit": "events/s",
                      "frac": p_events / a4_s / lsu_peak,
                      "peak_source": "148 SMs x 1.965 GHz / 1.7 LSU cycles per event (B300_MICROARCH.md atomics table: REDG "
-                                    "1.29 cycles per lane; DESIGN.md 6.3)"}
+                                    "1.29 cycles per lane; DESIGN.md 6.3; measured scattered-RED ceiling in "
+                                    "profiles/r02_red_ceiling.md)"}
     dom = max(kernels, key=lambda r: r["share"])
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.csv")   # per-launch DRAM bytes from the committed ncu --set full capture
-    if os.path.exists(tpath):
-        try:
-            table = dict(line.strip().split(",") for line in open(tpath).read().splitlines()[1:] if line.strip())
-            traffic = float(table[dom["kernel"].split()[0]])
-        except Exception:
-            traffic = None
     roofline = {"bound": "hbm", "kernel": dom["kernel"], "achieved": dom["achieved"], "peak": peak, "unit": "GB/s",
-                "frac": dom["frac"], "traffic": traffic, "peak_source": peak_src,
-                "timing": "second pass of the same K steps with a CUDA event at every kernel boundary (gn_profile)",
-                "kernels": kernels, "a4_delivery": a4, "profile_pass_events_per_sim_step": p_events / sim_steps}
+                "frac": dom["frac"], "traffic": dom.get("traffic"), "traffic_source": traffic_src if "traffic" in dom else None,
+                "dram_frac": dom.get("dram_frac"), "peak_source": peak_src,
+                "note": "achieved / frac = ALGORITHMIC bytes over the live CUDA-event time (the contract's definition); "
+                        "dram_frac = DRAM bytes ncu counted for this kernel over the same live time: the update kernel's "
+                        "state is L2-resident and the delivery kernel is bound by scattered-RED issue, so neither is "
+                        "HBM-bound in the strict sense (DESIGN.md 7)",
+                "timing": "the SAME K steps as the timed pass, replayed from rest on a fresh handle with a CUDA event at every "
+                          "kernel boundary (gn_profile; serialised on one stream)",
+                "kernels": kernels, "a4_delivery": a4, "profile_pass_events_per_sim_step": p_events / sim_steps,
+                "timed_pass_events_per_sim_step": (c1[2] - c0[2]) / sim_steps}
     if dom["kernel"].startswith("gn_deliver"):   # ring mode only: what DRAM moves when every event misses L2
         sect = (p_events * SECTOR_EVENT_BYTES + p_spikes * SOURCE_BYTES) / max(int(kn[1]), 1)
         roofline["sector_granular"] = {"bytes_per_launch": sect, "achieved": sect / (dom["avg_us"] * 1e-6) / 1e9,

@@ -162,9 +162,11 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
               const uint32_t *net_offsets, void *workspace, size_t workspace_bytes,
               void *cuda_stream, gn_net **out);
 
-/* Advance n_steps time steps: per step, ring-slot read-and-clear + drive + vertex update + spike
- * detection/compaction (one kernel), event delivery (one kernel; in queue mode a routing kernel per step plus
- * a bucket fold every queue_group steps), and at frame boundaries the observation kernel.  Asynchronous: no host synchronisation inside. */
+/* Advance n_steps time steps (eq. 5, called in a loop).  Per step one update kernel: ring-slot
+ * read-and-clear + drive + vertex update + spike detection + raster word + the events due soonest; then the rest of the
+ * step's event delivery -- ring mode: a delivery kernel per step (small networks: inside the update kernel); queue mode:
+ * ONE routing + folding kernel per group of queue_group steps; resident mode: the whole call is one launch per network
+ * batch -- and at frame boundaries the observation kernel.  Asynchronous: no host synchronisation inside. */
 int gn_step(gn_net *net, uint64_t n_steps);
 
 /* Copy state out.  dst_bytes must be at least the size listed at the enum.  dst_is_device != 0:

@@ -256,13 +256,11 @@ __device__ __forceinline__ void part_sync()
     else asm volatile("bar.sync %0, %1;" ::"n"(BAR), "n"(THREADS) : "memory");
 }
 
+// CTA-wide exclusive prefix sum of one count per thread; returns the CTA total (CTA-uniform), `off` = this thread's offset.
 template <int THREADS, int BAR = 0>
-__device__ __forceinline__ uint32_t gather_scan(const uint32_t *__restrict__ raster_row, const uint32_t w0,
-                                                const uint32_t n_words, uint32_t *s_wsum, uint32_t &word, uint32_t &off)
+__device__ __forceinline__ uint32_t gather_scan(const uint32_t pc, uint32_t *s_wsum, uint32_t &off)
 {
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
-    word = (threadIdx.x < n_words) ? raster_row[w0 + threadIdx.x] : 0u;
-    const uint32_t pc = __popc(word);
     uint32_t incl = pc;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
@@ -301,8 +299,9 @@ template <int THREADS>
 __device__ __forceinline__ uint32_t gather_sources(const uint32_t *__restrict__ raster_row, const uint32_t w0,
                                                    const uint32_t n_words, uint32_t *s_list, uint32_t *s_wsum)
 {
-    uint32_t word, off;
-    const uint32_t total = gather_scan<THREADS>(raster_row, w0, n_words, s_wsum, word, off);
+    const uint32_t word = (threadIdx.x < n_words) ? raster_row[w0 + threadIdx.x] : 0u;
+    uint32_t off;
+    const uint32_t total = gather_scan<THREADS>(__popc(word), s_wsum, off);
     gather_write(word, w0, off, s_list, nullptr, 0u);
     __syncthreads();
     return total;
@@ -377,6 +376,7 @@ constexpr int kRouteUnroll = 8;                         // 8 x 32 edges of a row
 // k = 1 .. nb-W).  Its segment of a row starts at table entry i = k + W - 1 (#edges with delay < (i+1)G - r) and ends
 // at entry i + 1 (the out-degree past the table's end): lo from the lane's own load, hi by a shuffle from lane k + 1.
 constexpr uint32_t kRouteListCap = 4096;                // sources one A/B/C round of a CTA handles
+constexpr uint32_t kMaxBatch = 16;                      // steps one launch routes: a slot group (queue_group <= 16)
 
 // Phases A, B, C over the n sources in s_list (each tagged with its step inside the group).
 template <bool PACKED>
@@ -434,20 +434,28 @@ __device__ __forceinline__ void route_round(const GnDev &p, const uint32_t n, co
             run += c;
         }
         bool full = false;
+        unsigned long long got = 0ull;
         if (run) {
-            const unsigned long long got = atomicAdd(&p.q_count[my_bucket], (unsigned long long)run);
+            got = atomicAdd(&p.q_count[my_bucket], (unsigned long long)run);
             if (got + run <= p.q_cap) {
                 const uint32_t first = (uint32_t)((unsigned long long)my_bucket * p.q_cap + got);
 #pragma unroll
                 for (int w = 0; w < kRouteWarps; ++w) s_wbase[w][lane] += first;
-            } else {                                      // bucket full: this CTA delivers these directly;
-                full = true;                              // neutralise what it reserved
-                uint2 *q = p.queue + (size_t)my_bucket * p.q_cap;
-                for (unsigned long long i = got; i < p.q_cap; ++i) q[i] = make_uint2(0u, 0u);
+            } else {
+                full = true;                              // bucket full: this CTA delivers these events directly (phase C)
             }
         }
         const uint32_t mask = __ballot_sync(0xFFFFFFFFu, full);
         if (lane == 0) *s_ovf = mask;
+        // the records this CTA reserved below the capacity but will not write are neutralised (weight 0) by the whole
+        // warp, bucket after bucket: fewer than the CTA's own record count for that bucket
+        for (uint32_t m = mask; m; m &= m - 1u) {
+            const int k = __ffs(m) - 1;
+            const unsigned long long g_k = __shfl_sync(0xFFFFFFFFu, got, k);
+            const uint32_t b_k = __shfl_sync(0xFFFFFFFFu, my_bucket, k);
+            uint2 *q = p.queue + (size_t)b_k * p.q_cap;
+            for (unsigned long long i = g_k + lane; i < p.q_cap; i += 32ull) q[i] = make_uint2(0u, 0u);
+        }
     }
     part_sync<kRouteThreads, 1>();
     // C: records.  With rd = r + delay: queued iff rd >= (W+1)G; group offset j = rd >> q_log, owned by lane
@@ -578,18 +586,39 @@ gn_route_kernel(const GnDev p, const uint32_t slot0, const uint32_t row0, const 
     const uint32_t n_words = min(chunk_words, p.words_pad - w0);
     unsigned long long events = 0ull;
     uint32_t n = 0u, spikes = 0u;
-    for (uint32_t i = 0; i < n_batch; ++i) {
-        uint32_t rr = row0 + i;
+    // the spike lists of all the group's steps are requested at once (one memory round trip, not one per step)
+    uint32_t words[kMaxBatch], pc_all = 0u;
+#pragma unroll
+    for (int i = 0; i < (int)kMaxBatch; ++i) {
+        uint32_t rr = row0 + (uint32_t)i;
         if (rr >= p.raster_rows) rr -= p.raster_rows;
-        uint32_t word, off;
-        const uint32_t total = gather_scan<kRouteThreads, 1>(p.raster + (size_t)rr * p.words_pad, w0, n_words, s_wsum, word, off);
-        if (n + total > kRouteListCap) {                    // CTA-uniform: the list is full, work it off first
-            route_round<PACKED>(p, n, slot0, s_list, s_step, s_wtot, s_wbase, &s_ovf, events);
-            n = 0u;
+        words[i] = ((uint32_t)i < n_batch && threadIdx.x < n_words) ? p.raster[(size_t)rr * p.words_pad + w0 + threadIdx.x] : 0u;
+    }
+#pragma unroll
+    for (int i = 0; i < (int)kMaxBatch; ++i) pc_all += __popc(words[i]);
+    uint32_t off;
+    const uint32_t total_all = gather_scan<kRouteThreads, 1>(pc_all, s_wsum, off);
+    if (total_all <= kRouteListCap) {                       // the usual case: one scan, one round for the whole group
+#pragma unroll
+        for (int i = 0; i < (int)kMaxBatch; ++i) {
+            gather_write(words[i], w0, off, s_list, s_step, (uint32_t)i);
+            off += __popc(words[i]);
         }
-        gather_write(word, w0, n + off, s_list, s_step, i);
-        n += total;
-        spikes += total;
+        n = spikes = total_all;
+    } else {                                                // rare (a burst beyond the list): step by step, words read again
+        for (uint32_t i = 0; i < n_batch; ++i) {
+            uint32_t rr = row0 + i;
+            if (rr >= p.raster_rows) rr -= p.raster_rows;
+            const uint32_t word = threadIdx.x < n_words ? p.raster[(size_t)rr * p.words_pad + w0 + threadIdx.x] : 0u;
+            const uint32_t total = gather_scan<kRouteThreads, 1>(__popc(word), s_wsum, off);
+            if (n + total > kRouteListCap) {                // CTA-uniform: the list is full, work it off first
+                route_round<PACKED>(p, n, slot0, s_list, s_step, s_wtot, s_wbase, &s_ovf, events);
+                n = 0u;
+            }
+            gather_write(word, w0, n + off, s_list, s_step, i);
+            n += total;
+            spikes += total;
+        }
     }
     part_sync<kRouteThreads, 1>();
     if (n) route_round<PACKED>(p, n, slot0, s_list, s_step, s_wtot, s_wbase, &s_ovf, events);
