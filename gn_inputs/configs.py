@@ -33,6 +33,35 @@ def _cls(a, d, rate_hz, kick=10.0, tau_syn_ms=2.0):
                 tau_syn_ms=tau_syn_ms, refractory_ms=2.0, drive_rate_hz=rate_hz, drive_kick=kick)
 
 
+def hh_class(rate_hz=0.0, kick=10.0, tau_syn_ms=2.0, **over):
+    """One row of gn_class_params for a Hodgkin-Huxley vertex (model = 1).  The paper prints no
+    values: these are the squid-axon parameters of Hodgkin & Huxley (1952) in the modern convention (rest at -65 mV;
+    e_l chosen so that -65 mV is the resting point), C in uF/cm^2, g in mS/cm^2, potentials in mV, rates in 1/ms.
+    A spike is the upward crossing of v_peak = 0 mV; refractory_ms is the detection dead time (one action potential =
+    one event).  The Izhikevich-only fields are unused and zero."""
+    c = dict(a=0.0, b=0.0, c_reset=0.0, d=0.0, k2=0.0, k1=0.0, k0=0.0, v_peak=0.0, tau_syn_ms=tau_syn_ms,
+             refractory_ms=2.0, drive_rate_hz=rate_hz, drive_kick=kick, psc_alpha=0.0,
+             model=1.0, hh_c=1.0, hh_g_na=120.0, hh_g_k=36.0, hh_g_l=0.3, hh_e_na=50.0, hh_e_k=-77.0, hh_e_l=-54.387,
+             hh_v_rest=-65.0,
+             hh_am_a=0.1, hh_am_v=-40.0, hh_am_k=10.0,         # 0.1 (V+40) / (1 - exp(-(V+40)/10))
+             hh_bm_a=4.0, hh_bm_v=-65.0, hh_bm_k=18.0,         # 4 exp(-(V+65)/18)
+             hh_ah_a=0.07, hh_ah_v=-65.0, hh_ah_k=20.0,        # 0.07 exp(-(V+65)/20)
+             hh_bh_a=1.0, hh_bh_v=-35.0, hh_bh_k=10.0,         # 1 / (1 + exp(-(V+35)/10))
+             hh_an_a=0.01, hh_an_v=-55.0, hh_an_k=10.0,        # 0.01 (V+55) / (1 - exp(-(V+55)/10))
+             hh_bn_a=0.125, hh_bn_v=-65.0, hh_bn_k=80.0)       # 0.125 exp(-(V+65)/80)
+    c.update(over)
+    return c
+
+
+def as_hodgkin_huxley(cfg: dict, dt_ms: float = 0.03) -> dict:
+    """The same network stepped with Hodgkin-Huxley vertices at the paper's HH time step (0.03 ms, 1 s =
+    33,333 steps): every class keeps its drive and PSC and becomes hh_class(); the speed is scaled so that every delay
+    keeps its number of STEPS (the ring depth of the config stays valid); steps = one simulated second."""
+    classes = [hh_class(c["drive_rate_hz"], c["drive_kick"], c["tau_syn_ms"]) for c in cfg["classes"]]
+    return dict(cfg, classes=classes, dt_ms=dt_ms, speed=cfg["speed"] * cfg["dt_ms"] / dt_ms,
+                steps=int(round(1000.0 / dt_ms)), name=cfg["name"] + "+hh")
+
+
 def _rs(rate):  # regular spiking, excitatory
     return _cls(0.02, 8.0, rate)
 

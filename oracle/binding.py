@@ -12,9 +12,13 @@ _SRC = os.path.join(_HERE, "gn_oracle.c")
 _SO = os.path.join(_HERE, "libgn_oracle.so")
 _lib = None
 
+HH_RATES = ("am", "bm", "ah", "bh", "an", "bn")      # alpha_m, beta_m, alpha_h, beta_h, alpha_n, beta_n
 CLASS_FIELDS = ("a", "b", "c_reset", "d", "k2", "k1", "k0", "v_peak", "tau_syn_ms",
-                "refractory_ms", "drive_rate_hz", "drive_kick", "psc_alpha")
-V, W, R, CA, P = 0, 1, 2, 3, 4
+                "refractory_ms", "drive_rate_hz", "drive_kick", "psc_alpha",
+                "model", "hh_c", "hh_g_na", "hh_g_k", "hh_g_l", "hh_e_na", "hh_e_k", "hh_e_l", "hh_v_rest") + \
+    tuple(f"hh_{f}_{x}" for f in HH_RATES for x in ("a", "v", "k"))
+OPTIONAL_FROM = CLASS_FIELDS.index("psc_alpha")      # psc_alpha and every Hodgkin-Huxley field may be omitted: 0
+V, W, R, CA, P, HM, HH = 0, 1, 2, 3, 4, 5, 6
 
 
 def build_lib(force: bool = False) -> str:
@@ -44,6 +48,12 @@ def lib():
         L.orc_keep.argtypes = [f32, f32]
         L.orc_refractory_steps.restype = u32
         L.orc_refractory_steps.argtypes = [f32, f32]
+        L.orc_hh_rate.restype = C.c_double
+        L.orc_hh_rate.argtypes = [i32, C.c_double, C.c_double, C.c_double, C.c_double]
+        L.orc_hh_rate32.restype = f32
+        L.orc_hh_rate32.argtypes = [i32, f32, f32, f32, f32]
+        L.orc_exp32.restype = f32
+        L.orc_exp32.argtypes = [f32]
         L.orc_create.restype = vp
         L.orc_create.argtypes = [u32, u32, u64, u32, f32, f32, u32, vp, vp, vp, vp, vp, vp, vp, vp,
                                  f32, f32, f32, f32, f32, u32, u64, u32]
@@ -70,8 +80,10 @@ def _p(a):
 
 
 def class_table(classes) -> np.ndarray:
-    # psc_alpha (0 = exponential PSC, eq. 26; 1 = alpha-function, eq. 27-30) may be omitted: 0
-    return np.array([[c.get(f, 0.0) if f == "psc_alpha" else c[f] for f in CLASS_FIELDS] for c in classes], dtype=np.float32)
+    # psc_alpha (0 = exponential PSC, eq. 26; 1 = alpha-function, eq. 27-30) and the Hodgkin-Huxley fields (model = 1)
+    # may be omitted: 0
+    return np.array([[c.get(f, 0.0) if i >= OPTIONAL_FROM else c[f] for i, f in enumerate(CLASS_FIELDS)]
+                     for c in classes], dtype=np.float32)
 
 
 class Oracle:

@@ -22,6 +22,11 @@
  *                or, for a class with psc_alpha != 0, the alpha-function of PAPER.md:288-312
  *                eq. 27, 29, 30 with a = 1/tau_s:  r' = r + dt p,  p' = p + dt (-a^2 r - 2a p) + I
  *                (the arriving weight is an impulse on p: eq. 27's p(t+) = p(t) + w, reading #4)
+ *                A class with model = 1 is a Hodgkin-Huxley vertex instead ("states {v, m, n, h}", dt on the
+ *                order of 0.03 ms; the paper's second benchmarked model).  The paper prints no equations
+ *                for it: they are the textbook ones (Hodgkin & Huxley 1952 in the modern sign convention), restated
+ *                at orc_vertex_hh_fp64 below, forward Euler (eq. 19) like everything else; no reset, the
+ *                refractory counter is only the detection dead time that makes one action potential one event.
  *   5. calcium   c' = c (1 - dt/tau_c) + ca_jump * fired                 PAPER.md:364 H_c
  *   6. record    raster[t][j] = fired; deliver: every out-edge (j->m, w_fx, delay) of a fired j
  *                adds w_fx to ring[(t + delay) mod D][m]
@@ -35,7 +40,9 @@
  * Delivery, the ring, the drive decision and the raster are pure integer in both modes.
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): Philox known-answer vectors; fixed points and
- * closed forms of the update; geometric decay of r and c; the alpha-function PSC against the matrix
+ * closed forms of the update; Hodgkin-Huxley: textbook rate values and gating steady states at rest, the resting
+ * fixed point, one action potential per supra-threshold pulse, the textbook firing rate at 10 uA/cm^2, orc_exp32 against
+ * libm; geometric decay of r and c; the alpha-function PSC against the matrix
  * power of its 2x2 Euler map, its exact discrete integral w tau^2 and w t e^(-at); chain arrival steps; event-count and
  * fixed-point-mass conservation; the pure-Python pull definition (oracle/pull_definition.py) on
  * <= 10-node graphs; the implementation-free ring-content definition; noise statistics.
@@ -152,11 +159,88 @@ uint32_t orc_refractory_steps(float refractory_ms, float dt_ms)
 }
 
 /* ------------------------------------------------------------------------------------------
+ * Hodgkin-Huxley vertex class (the equations are the textbook ones, the paper
+ * prints none):
+ *     C dV/dt = -g_na m^3 h (V - e_na) - g_k n^4 (V - e_k) - g_l (V - e_l) + r + U
+ *     dx/dt   = alpha_x(V) (1 - x) - beta_x(V) x                      x = m, h, n
+ * with the three shapes of rate function of the 1952 paper, each {A, V_half, k}, u = (V - V_half)/k:
+ *     exponential  A exp(-u)                 beta_m, alpha_h, beta_n
+ *     sigmoid      A / (1 + exp(-u))         beta_h
+ *     linoid       A k u / (1 - exp(-u))     alpha_m, alpha_n  (-> A k at u = 0; the series 1 + u/2 + u^2/12 is used for
+ *                                            |u| < 0.05, where it is exact to 1e-8 and the quotient loses digits)
+ * Rate index f: 0 alpha_m, 1 beta_m, 2 alpha_h, 3 beta_h, 4 alpha_n, 5 beta_n.
+ * ---------------------------------------------------------------------------------------- */
+enum { ORC_HH_EXP = 0, ORC_HH_SIGMOID = 1, ORC_HH_LINOID = 2 };
+
+int orc_hh_kind(int f)
+{
+    return (f == 0 || f == 4) ? ORC_HH_LINOID : (f == 3 ? ORC_HH_SIGMOID : ORC_HH_EXP);
+}
+
+/* The definition, in double with libm's exp. */
+double orc_hh_rate(int f, double A, double v_half, double k, double V)
+{
+    const double u = (V - v_half) * (1.0 / k);
+    switch (orc_hh_kind(f)) {
+    case ORC_HH_LINOID:
+        if (fabs(u) < 0.05) return (A * k) * fma(u, fma(u, 1.0 / 12.0, 0.5), 1.0);
+        return (A * k) * (u / (1.0 - exp(-u)));
+    case ORC_HH_SIGMOID: return A / (1.0 + exp(-u));
+    default: return A * exp(-u);
+    }
+}
+
+/* exp for the fp32-faithful mode: every step one correctly rounded binary32 operation, so that the CUDA kernels can
+ * follow it bit for bit (Hodgkin-Huxley).  Argument clamped to [-87, 88] (a rate
+ * function never needs more); n = rint(x log2 e); r = x - n ln 2 in two steps (Cody-Waite); degree-7 Taylor polynomial
+ * of e^r on |r| <= ln2 / 2 (remainder 5e-9) by Horner with fmaf; scaled by 2^n through the exponent field. */
+float orc_exp32(float x)
+{
+    if (x > 88.0f) x = 88.0f;
+    if (x < -87.0f) x = -87.0f;
+    const float n = rintf(x * 0x1.715476p+0f);
+    float r = fmaf(n, -0x1.62e400p-1f, x);
+    r = fmaf(n, -0x1.7f7d1cp-20f, r);
+    float p = 0x1.a01a02p-13f;                 /* 1/5040 */
+    p = fmaf(p, r, 0x1.6c16c2p-10f);           /* 1/720  */
+    p = fmaf(p, r, 0x1.111112p-7f);            /* 1/120  */
+    p = fmaf(p, r, 0x1.555556p-5f);            /* 1/24   */
+    p = fmaf(p, r, 0x1.555556p-3f);            /* 1/6    */
+    p = fmaf(p, r, 0.5f);
+    p = fmaf(p, r, 1.0f);
+    p = fmaf(p, r, 1.0f);
+    union { uint32_t u; float f; } s;
+    s.u = (uint32_t)((int32_t)n + 127) << 23;  /* 2^n, n in [-126, 127] */
+    return p * s.f;
+}
+
+/* One rate in the fp32-faithful order: ak = (float)(A) or (float)(A k), inv_k = (float)(1/k). */
+float orc_hh_rate32(int f, float ak, float v_half, float inv_k, float V)
+{
+    const float u = (V - v_half) * inv_k;
+    switch (orc_hh_kind(f)) {
+    case ORC_HH_LINOID:
+        if (fabsf(u) < 0.05f) return ak * fmaf(u, fmaf(u, 0x1.555556p-4f, 0.5f), 1.0f);
+        return ak * (u / (1.0f - orc_exp32(-u)));
+    case ORC_HH_SIGMOID: return ak / (1.0f + orc_exp32(-u));
+    default: return ak * orc_exp32(-u);
+    }
+}
+
+/* ------------------------------------------------------------------------------------------
  * The simulator
  * ---------------------------------------------------------------------------------------- */
+enum { ORC_CLASS_FLOATS = 40 };
+
 typedef struct {
     /* as given (fp32 at the boundary) */
     float a, b, c_reset, d, k2, k1, k0, v_peak, tau_syn_ms, refractory_ms, drive_rate_hz, drive_kick, psc_alpha;
+    /* Hodgkin-Huxley class (model == 1): capacitance, conductances, reversal potentials, resting potential, and
+     * {A, V_half, k} of the six rate functions alpha_m, beta_m, alpha_h, beta_h, alpha_n, beta_n */
+    float model, hh_c, hh_g_na, hh_g_k, hh_g_l, hh_e_na, hh_e_k, hh_e_l, hh_v_rest, hh_rate[6][3];
+    int hh;              /* model == 1 */
+    double hh_dt_c, hh_ak[6], hh_inv_k[6];      /* dt/C, A (A*k for the two linoid rates), 1/k: formed once in double */
+    float hh_dt_c_f, hh_ak_f[6], hh_inv_k_f[6]; /* ... and rounded once for the fp32-faithful mode */
     /* derived */
     int direct;          /* tau_syn_ms <= 0: arriving weight jumps V itself */
     int alpha;           /* psc_alpha != 0: alpha-function PSC (eq. 27, 29, 30) instead of the exponential one (eq. 26) */
@@ -182,8 +266,8 @@ typedef struct orc_net {
     uint8_t *cls;       /* [n] */
     float *bias;        /* [n] or NULL */
     /* state; mode 0 uses the double arrays, mode 1 the float arrays */
-    double *V, *W, *r, *p, *c, *acc;
-    float *Vf, *Wf, *rf, *pf, *cf, *accf;
+    double *V, *W, *r, *p, *c, *acc, *hm, *hh;    /* hm, hh: the gates m and h of Hodgkin-Huxley vertices (n lives in W) */
+    float *Vf, *Wf, *rf, *pf, *cf, *accf, *hmf, *hhf;
     uint32_t *refr;
     int64_t *ring;      /* [D][n] */
     int64_t *consumed;  /* [n] I_fx (kick included) consumed by the last step */
@@ -210,13 +294,16 @@ void orc_destroy(orc_net *o)
     free(o->cls_tab); free(o->row); free(o->tgt); free(o->w_fx); free(o->delay); free(o->cls);
     free(o->bias); free(o->V); free(o->W); free(o->r); free(o->c); free(o->acc);
     free(o->Vf); free(o->Wf); free(o->rf); free(o->pf); free(o->cf); free(o->accf); free(o->p);
+    free(o->hm); free(o->hh); free(o->hmf); free(o->hhf);
     free(o->refr); free(o->ring); free(o->consumed); free(o->fired); free(o->raster); free(o->trace);
     free(o);
 }
 
 /*
- * class_params: [n_classes][13] floats in the order
- *   a, b, c_reset, d, k2, k1, k0, v_peak, tau_syn_ms, refractory_ms, drive_rate_hz, drive_kick, psc_alpha.
+ * class_params: [n_classes][ORC_CLASS_FLOATS = 40] floats in the order
+ *   a, b, c_reset, d, k2, k1, k0, v_peak, tau_syn_ms, refractory_ms, drive_rate_hz, drive_kick, psc_alpha,
+ *   model, hh_c, hh_g_na, hh_g_k, hh_g_l, hh_e_na, hh_e_k, hh_e_l, hh_v_rest, then {A, V_half, k} of alpha_m, beta_m,
+ *   alpha_h, beta_h, alpha_n, beta_n.
  * delays: [E] steps, or NULL => eq. 25 from positions and speed.
  * Returns NULL on a malformed graph (row offsets, target range, delay outside [1, D-1]).
  * Initial state (reading #15): V = -70, W = b*V, r = c = 0, refr = 0, ring zero.
@@ -252,17 +339,35 @@ orc_net *orc_create(uint32_t n, uint32_t dim, uint64_t E, uint32_t D, float dt_m
     o->Vf = (float *)calloc(n1, sizeof(float)); o->Wf = (float *)calloc(n1, sizeof(float));
     o->rf = (float *)calloc(n1, sizeof(float)); o->cf = (float *)calloc(n1, sizeof(float));
     o->accf = (float *)calloc(n1, sizeof(float));
+    o->hm = (double *)calloc(n1, sizeof(double)); o->hh = (double *)calloc(n1, sizeof(double));
+    o->hmf = (float *)calloc(n1, sizeof(float)); o->hhf = (float *)calloc(n1, sizeof(float));
     if (bias) {
         o->bias = (float *)malloc(n1 * sizeof(float));
         memcpy(o->bias, bias, (size_t)n * sizeof(float));
     }
     for (uint32_t k = 0; k < n_classes; ++k) {
-        const float *p = class_params + 13 * k;
+        const float *p = class_params + ORC_CLASS_FLOATS * k;
         orc_class *q = &o->cls_tab[k];
         q->a = p[0]; q->b = p[1]; q->c_reset = p[2]; q->d = p[3];
         q->k2 = p[4]; q->k1 = p[5]; q->k0 = p[6]; q->v_peak = p[7];
         q->tau_syn_ms = p[8]; q->refractory_ms = p[9]; q->drive_rate_hz = p[10]; q->drive_kick = p[11];
         q->psc_alpha = p[12];
+        q->model = p[13]; q->hh = q->model == 1.0f;
+        q->hh_c = p[14]; q->hh_g_na = p[15]; q->hh_g_k = p[16]; q->hh_g_l = p[17];
+        q->hh_e_na = p[18]; q->hh_e_k = p[19]; q->hh_e_l = p[20]; q->hh_v_rest = p[21];
+        for (int f = 0; f < 6; ++f)
+            for (int i = 0; i < 3; ++i) q->hh_rate[f][i] = p[22 + 3 * f + i];
+        if (q->hh) {
+            q->hh_dt_c = (double)dt_ms / (double)q->hh_c;
+            q->hh_dt_c_f = (float)q->hh_dt_c;
+            for (int f = 0; f < 6; ++f) {
+                const double A = q->hh_rate[f][0], kk = q->hh_rate[f][2];
+                q->hh_ak[f] = orc_hh_kind(f) == ORC_HH_LINOID ? A * kk : A;
+                q->hh_inv_k[f] = 1.0 / kk;
+                q->hh_ak_f[f] = (float)q->hh_ak[f];
+                q->hh_inv_k_f[f] = (float)q->hh_inv_k[f];
+            }
+        }
         q->direct = !(q->tau_syn_ms > 0.0f);
         q->alpha = !q->direct && q->psc_alpha != 0.0f;
         q->keep_s = q->direct ? 0.0 : orc_keep(dt_ms, q->tau_syn_ms);
@@ -304,6 +409,17 @@ orc_net *orc_create(uint32_t n, uint32_t dim, uint64_t E, uint32_t D, float dt_m
     if (bad) { orc_destroy(o); return NULL; }
     for (uint32_t j = 0; j < n; ++j) {
         const orc_class *q = &o->cls_tab[o->cls[j]];
+        if (q->hh) {         /* at rest: V = hh_v_rest, every gate at its steady state alpha / (alpha + beta) for that V */
+            double g[3];
+            for (int x = 0; x < 3; ++x) {
+                const double al = orc_hh_rate(2 * x, q->hh_rate[2 * x][0], q->hh_rate[2 * x][1], q->hh_rate[2 * x][2], q->hh_v_rest);
+                const double be = orc_hh_rate(2 * x + 1, q->hh_rate[2 * x + 1][0], q->hh_rate[2 * x + 1][1], q->hh_rate[2 * x + 1][2], q->hh_v_rest);
+                g[x] = al / (al + be);
+            }
+            o->V[j] = q->hh_v_rest; o->hm[j] = g[0]; o->hh[j] = g[1]; o->W[j] = g[2];
+            o->Vf[j] = q->hh_v_rest; o->hmf[j] = (float)g[0]; o->hhf[j] = (float)g[1]; o->Wf[j] = (float)g[2];
+            continue;
+        }
         o->V[j] = -70.0; o->W[j] = (double)q->b * -70.0;
         o->Vf[j] = -70.0f; o->Wf[j] = q->b * -70.0f;
     }
@@ -421,6 +537,83 @@ static int orc_vertex_fp32(orc_net *o, uint32_t j, int64_t I_fx)
     return fired;
 }
 
+/* Steps 2-5 for a Hodgkin-Huxley vertex in double: detect on the state at t (eq. 31), forward Euler (eq. 19) of the four
+ * textbook equations from the state at t, the PSC and the calcium as for every class.  There is no reset: `refr` only
+ * keeps one action potential (V stays above v_peak for many steps) from being detected again for refractory_ms. */
+static int orc_vertex_hh_fp64(orc_net *o, uint32_t j, int64_t I_fx)
+{
+    const orc_class *q = &o->cls_tab[o->cls[j]];
+    const double V = o->V[j], m = o->hm[j], h = o->hh[j], n = o->W[j], r = o->r[j];
+    const double I = (double)I_fx * (1.0 / 65536.0);
+    int fired = (o->refr[j] == 0) && (V >= (double)q->v_peak);
+    if (fired) o->refr[j] = q->R;
+    else if (o->refr[j] > 0) o->refr[j] -= 1;
+    double rate[6];
+    for (int f = 0; f < 6; ++f) rate[f] = orc_hh_rate(f, q->hh_rate[f][0], q->hh_rate[f][1], q->hh_rate[f][2], V);
+    const double i_na = (((double)q->hh_g_na * ((m * m) * m)) * h) * (V - (double)q->hh_e_na);
+    const double i_k = ((double)q->hh_g_k * ((n * n) * (n * n))) * (V - (double)q->hh_e_k);
+    const double i_l = (double)q->hh_g_l * (V - (double)q->hh_e_l);
+    double s = r - ((i_na + i_k) + i_l);
+    if (o->bias) s = s + (double)o->bias[j];
+    o->V[j] = fma(q->hh_dt_c, s, V);
+    o->hm[j] = fma(o->dt, fma(-rate[1], m, rate[0] * (1.0 - m)), m);
+    o->hh[j] = fma(o->dt, fma(-rate[3], h, rate[2] * (1.0 - h)), h);
+    o->W[j] = fma(o->dt, fma(-rate[5], n, rate[4] * (1.0 - n)), n);
+    if (q->alpha) {
+        double pp = o->p[j];
+        double q2 = fma(q->two_a, pp, q->a2 * r);
+        o->r[j] = fma(o->dt, pp, r);
+        o->p[j] = fma(-o->dt, q2, pp) + I;
+    } else if (!q->direct) {
+        o->r[j] = fma(q->keep_s, r, I);
+    }
+    if (o->obs_stride) {
+        double cn = fma(o->keep_c, o->c[j], fired ? o->ca_jump : 0.0);
+        o->c[j] = cn;
+        o->acc[j] = o->acc[j] + cn;
+    }
+    return fired;
+}
+
+/* The same sequence, every operation one correctly rounded binary32 operation (exp by orc_exp32). */
+static int orc_vertex_hh_fp32(orc_net *o, uint32_t j, int64_t I_fx)
+{
+    const orc_class *q = &o->cls_tab[o->cls[j]];
+    const float dt = o->dt_f;
+    const float V = o->Vf[j], m = o->hmf[j], h = o->hhf[j], n = o->Wf[j], r = o->rf[j];
+    const float If = (float)(int32_t)I_fx * 0x1p-16f;
+    int fired = (o->refr[j] == 0) && (V >= q->v_peak);
+    if (fired) o->refr[j] = q->R;
+    else if (o->refr[j] > 0) o->refr[j] -= 1;
+    float rate[6];
+    for (int f = 0; f < 6; ++f) rate[f] = orc_hh_rate32(f, q->hh_ak_f[f], q->hh_rate[f][1], q->hh_inv_k_f[f], V);
+    const float m2 = m * m, m3 = m2 * m, gna = (q->hh_g_na * m3) * h, i_na = gna * (V - q->hh_e_na);
+    const float n2 = n * n, n4 = n2 * n2, i_k = (q->hh_g_k * n4) * (V - q->hh_e_k);
+    const float i_l = q->hh_g_l * (V - q->hh_e_l);
+    float s = r - ((i_na + i_k) + i_l);
+    if (o->bias) s = s + o->bias[j];
+    o->Vf[j] = fmaf(q->hh_dt_c_f, s, V);
+    o->hmf[j] = fmaf(dt, fmaf(-rate[1], m, rate[0] * (1.0f - m)), m);
+    o->hhf[j] = fmaf(dt, fmaf(-rate[3], h, rate[2] * (1.0f - h)), h);
+    o->Wf[j] = fmaf(dt, fmaf(-rate[5], n, rate[4] * (1.0f - n)), n);
+    if (q->alpha) {
+        float pp = o->pf[j];
+        float q1 = q->a2_f * r;
+        float q2 = fmaf(q->two_a_f, pp, q1);
+        float p1 = fmaf(-dt, q2, pp);
+        o->rf[j] = fmaf(dt, pp, r);
+        o->pf[j] = p1 + If;
+    } else if (!q->direct) {
+        o->rf[j] = fmaf(q->keep_s_f, r, If);
+    }
+    if (o->obs_stride) {
+        float cn = fmaf(o->keep_c_f, o->cf[j], fired ? o->ca_jump_f : 0.0f);
+        o->cf[j] = cn;
+        o->accf[j] = o->accf[j] + cn;
+    }
+    return fired;
+}
+
 /* Advance n_steps.  Returns 0, -1 (out of memory) or -2 (a ring slot left the int32 range). */
 int orc_step(orc_net *o, uint64_t n_steps, int n_threads)
 {
@@ -452,7 +645,8 @@ int orc_step(orc_net *o, uint64_t n_steps, int n_threads)
                 kicks += 1;
             }
             o->consumed[j] = I_fx;
-            int f = o->mode ? orc_vertex_fp32(o, j, I_fx) : orc_vertex_fp64(o, j, I_fx);
+            int f = q->hh ? (o->mode ? orc_vertex_hh_fp32(o, j, I_fx) : orc_vertex_hh_fp64(o, j, I_fx))
+                          : (o->mode ? orc_vertex_fp32(o, j, I_fx) : orc_vertex_fp64(o, j, I_fx));
             o->fired[j] = (uint8_t)f;
             spikes += (uint64_t)f;
         }
@@ -493,7 +687,7 @@ int orc_step(orc_net *o, uint64_t n_steps, int n_threads)
 }
 
 /* ---- accessors ---------------------------------------------------------------------------- */
-enum { ORC_V = 0, ORC_W = 1, ORC_R = 2, ORC_CA = 3, ORC_P = 4 };
+enum { ORC_V = 0, ORC_W = 1, ORC_R = 2, ORC_CA = 3, ORC_P = 4, ORC_HM = 5, ORC_HH = 6 };
 
 int orc_get_state(const orc_net *o, int which, double *out)
 {
@@ -504,6 +698,8 @@ int orc_get_state(const orc_net *o, int which, double *out)
         case ORC_R: out[j] = o->mode ? (double)o->rf[j] : o->r[j]; break;
         case ORC_CA: out[j] = o->mode ? (double)o->cf[j] : o->c[j]; break;
         case ORC_P: out[j] = o->mode ? (double)o->pf[j] : o->p[j]; break;
+        case ORC_HM: out[j] = o->mode ? (double)o->hmf[j] : o->hm[j]; break;
+        case ORC_HH: out[j] = o->mode ? (double)o->hhf[j] : o->hh[j]; break;
         default: return -1;
         }
     }
@@ -519,6 +715,8 @@ int orc_set_state(orc_net *o, int which, const double *in)
         case ORC_R: o->r[j] = in[j]; o->rf[j] = (float)in[j]; break;
         case ORC_CA: o->c[j] = in[j]; o->cf[j] = (float)in[j]; break;
         case ORC_P: o->p[j] = in[j]; o->pf[j] = (float)in[j]; break;
+        case ORC_HM: o->hm[j] = in[j]; o->hmf[j] = (float)in[j]; break;
+        case ORC_HH: o->hh[j] = in[j]; o->hhf[j] = (float)in[j]; break;
         default: return -1;
         }
     }
