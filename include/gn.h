@@ -67,7 +67,26 @@ typedef struct {
     float drive_kick;       /* kick weight, injected like an arriving event (reading #12)            */
     float psc_alpha;        /* 0: exponential PSC (eq. 26).  != 0: alpha-function PSC (:288-312 eq. 27,  */
                             /* 29, 30), a = 1/tau_syn_ms: r <- r + dt p, p <- p + dt(-a^2 r - 2a p) + I   */
+    /* Vertex model of the class.  0 (GN_MODEL_IZHIKEVICH): the fields above.  1 (GN_MODEL_HODGKIN_HUXLEY): the      */
+    /* paper's second benchmarked model (PAPER.md:235 "states {v, m, n, h}", dt ~ 0.03 ms; :382), textbook form:     */
+    /*   C dV/dt = -g_na m^3 h (V - e_na) - g_k n^4 (V - e_k) - g_l (V - e_l) + r + U,                               */
+    /*   dx/dt = alpha_x(V) (1 - x) - beta_x(V) x  for x = m, h, n,  forward Euler (:184 eq. 19), no reset.          */
+    /* Of the fields above it uses v_peak (a spike is V >= v_peak while not in the dead time, eq. 31),               */
+    /* refractory_ms (the detection dead time: one action potential is one event), tau_syn_ms, psc_alpha and the     */
+    /* drive; a .. k0 are ignored.  The state n is read / written as GN_W, m and h as GN_M and GN_H.                 */
+    float model;
+    float hh_c;                          /* membrane capacitance, uF/cm^2 (> 0)                                      */
+    float hh_g_na, hh_g_k, hh_g_l;       /* maximal conductances, mS/cm^2                                            */
+    float hh_e_na, hh_e_k, hh_e_l;       /* reversal potentials, mV                                                  */
+    float hh_v_rest;                     /* initial V; the gates start at alpha/(alpha+beta) of this potential        */
+    /* The six rate functions, each {A, V_half, k} (k != 0), u = (V - V_half)/k, in 1/ms:                            */
+    /*   alpha_m, alpha_n: linoid A k u / (1 - exp(-u)); beta_h: sigmoid A / (1 + exp(-u)); beta_m, alpha_h, beta_n: */
+    /*   exponential A exp(-u)                                                                                       */
+    float hh_am[3], hh_bm[3], hh_ah[3], hh_bh[3], hh_an[3], hh_bn[3];
 } gn_class_params;
+
+#define GN_MODEL_IZHIKEVICH 0
+#define GN_MODEL_HODGKIN_HUXLEY 1
 
 typedef struct {
     uint32_t n_vertices;            /* N (total over all networks in batched mode)                   */
@@ -130,7 +149,9 @@ enum {
     GN_WEIGHTS_FX = 9,/* int32  [E]      per-edge weight, rint(w * 2^16)                             */
     GN_BIAS = 10,     /* float  [N]      user control U_j (write only through gn_write_state)        */
     GN_P = 11,        /* float  [N]      second PSC state p of the alpha-function (zero for other classes) */
-    GN_ACC = 12       /* float  [N]      sum of c over the steps of the camera frame in progress (obs_stride > 0) */
+    GN_ACC = 12,      /* float  [N]      sum of c over the steps of the camera frame in progress (obs_stride > 0) */
+    GN_M = 13,        /* float  [N]      sodium activation m of Hodgkin-Huxley vertices (zero for other classes)  */
+    GN_H = 14         /* float  [N]      sodium inactivation h of Hodgkin-Huxley vertices (zero for other classes) */
 };
 
 /* Bytes of device workspace gn_create needs for this configuration.
@@ -152,7 +173,8 @@ int gn_query_workspace(const gn_config *cfg, size_t *bytes);
  *                 n_networks == 1; an edge whose endpoints lie in different networks is rejected
  *   workspace     device memory, >= gn_query_workspace bytes, 256-byte aligned; owned by the caller
  *   cuda_stream   cudaStream_t (NULL = legacy default stream)
- * Initial state (reading #15): V = -70, W = b V, r = c = 0, not refractory, ring empty, t = 0.
+ * Initial state (reading #15): V = -70, W = b V, r = c = 0, not refractory, ring empty, t = 0; a Hodgkin-Huxley
+ * vertex starts at V = hh_v_rest with m, h, n at their steady states for that potential.
  * Synchronises the stream once (validation results are read back).  On failure *out = NULL.
  * Errors: INVALID_ARG, BAD_GRAPH, OVERFLOW_RISK, WORKSPACE_TOO_SMALL, CUDA.
  */
@@ -173,7 +195,7 @@ int gn_step(gn_net *net, uint64_t n_steps);
  * dst is device memory, written asynchronously on the stream.  Errors: INVALID_ARG, CUDA. */
 int gn_read_state(gn_net *net, int which, void *dst, size_t dst_bytes, int dst_is_device);
 
-/* Overwrite V, W, R, P, CA, ACC (float [N]), REFR (uint8 [N]) or BIAS (float [N]; enables the bias term): controlled
+/* Overwrite V, W, R, P, M, H, CA, ACC (float [N]), REFR (uint8 [N]) or BIAS (float [N]; enables the bias term): controlled
  * experiments (PAPER.md:77-79 user control).  Checkpoint / restore: together with RING (int32 [D][N], the layout GN_RING
  * reads) and STEP (uint64 [1], or COUNTERS uint64 [4]) they are the whole state -- y_j and the in-flight delayed signals
  * Y_j: a fresh handle of the same network given all of them continues bit-identically from step t.

@@ -15,16 +15,22 @@ from .build import build
 GN_OK = 0
 GN_E_INVALID_ARG, GN_E_BAD_GRAPH, GN_E_OVERFLOW_RISK = -1, -2, -3
 GN_E_WORKSPACE_TOO_SMALL, GN_E_RANGE_EVICTED, GN_E_CUDA = -4, -5, -6
-GN_V, GN_W, GN_R, GN_CA, GN_REFR, GN_RING, GN_STEP, GN_COUNTERS, GN_DELAYS, GN_WEIGHTS_FX, GN_BIAS, GN_P, GN_ACC = range(13)
+(GN_V, GN_W, GN_R, GN_CA, GN_REFR, GN_RING, GN_STEP, GN_COUNTERS, GN_DELAYS, GN_WEIGHTS_FX, GN_BIAS, GN_P, GN_ACC, GN_M,
+ GN_H) = range(15)
+GN_MODEL_IZHIKEVICH, GN_MODEL_HODGKIN_HUXLEY = 0, 1
 GN_MAX_CLASSES = 8
 GN_DELIVER_AUTO, GN_DELIVER_RING, GN_DELIVER_QUEUE, GN_DELIVER_RESIDENT = 0, 1, 2, 3
 
+# gn_class_params in declaration order; a class dict may omit psc_alpha, model and the Hodgkin-Huxley fields (0)
 CLASS_FIELDS = ("a", "b", "c_reset", "d", "k2", "k1", "k0", "v_peak", "tau_syn_ms",
-                "refractory_ms", "drive_rate_hz", "drive_kick", "psc_alpha")
+                "refractory_ms", "drive_rate_hz", "drive_kick", "psc_alpha",
+                "model", "hh_c", "hh_g_na", "hh_g_k", "hh_g_l", "hh_e_na", "hh_e_k", "hh_e_l", "hh_v_rest") + \
+    tuple(f"hh_{f}_{x}" for f in ("am", "bm", "ah", "bh", "an", "bn") for x in ("a", "v", "k"))
+_OPTIONAL_FROM = CLASS_FIELDS.index("psc_alpha")
 
 
 class gn_class_params(C.Structure):
-    _fields_ = [(f, C.c_float) for f in CLASS_FIELDS]
+    _fields_ = [(f, C.c_float) for f in CLASS_FIELDS]        # hh_am[3] ... hh_bn[3] laid out as consecutive floats
 
 
 class gn_config(C.Structure):
@@ -136,7 +142,8 @@ def gn_create(cfg: gn_config, classes, positions, row_offsets, targets, weights,
     need = gn_query_workspace(cfg)
     if workspace is None:
         workspace = torch.empty(need, dtype=torch.uint8, device=dev)
-    tab = (gn_class_params * len(classes))(*[gn_class_params(*[c.get(f, 0.0) if f == "psc_alpha" else c[f] for f in CLASS_FIELDS]) for c in classes])
+    tab = (gn_class_params * len(classes))(*[gn_class_params(*[c.get(f, 0.0) if i >= _OPTIONAL_FROM else c[f]
+                                                               for i, f in enumerate(CLASS_FIELDS)]) for c in classes])
     handle = C.c_void_p(None)
     with torch.cuda.device(dev):
         stream = torch.cuda.current_stream(dev)
@@ -154,7 +161,8 @@ def gn_step(net: GnNet, n_steps: int) -> None:
 
 _STATE_DTYPE = {GN_V: np.float32, GN_W: np.float32, GN_R: np.float32, GN_CA: np.float32, GN_REFR: np.uint8,
                 GN_RING: np.int32, GN_STEP: np.uint64, GN_COUNTERS: np.uint64, GN_DELAYS: np.uint8,
-                GN_WEIGHTS_FX: np.int32, GN_BIAS: np.float32, GN_P: np.float32, GN_ACC: np.float32}
+                GN_WEIGHTS_FX: np.int32, GN_BIAS: np.float32, GN_P: np.float32, GN_ACC: np.float32, GN_M: np.float32,
+                GN_H: np.float32}
 
 
 def _state_shape(net, which):

@@ -16,7 +16,7 @@ namespace {
 thread_local char g_create_error[256] = "";
 
 struct Layout {
-    size_t V, W, r, p2, c, acc, bias, refr, cls, ring, row, tgt, wfx, dly, counters, q_count;
+    size_t V, W, r, p2, hm, hh, c, acc, bias, refr, cls, ring, row, tgt, wfx, dly, counters, q_count;
     size_t s_edge, s_dly, min_dly, q_seg, queue;
     size_t raster, trace, scratch_row64, scratch_abs, scratch_pos, scratch_net, scratch_chk, total;
 };
@@ -85,6 +85,7 @@ Layout make_layout(const gn_config *cfg)
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off = align256(off + bytes); return o; };
     L.V = take(Npad * 4); L.W = take(Npad * 4); L.r = take(Npad * 4); L.p2 = take(Npad * 4);
+    L.hm = take(Npad * 4); L.hh = take(Npad * 4);
     L.c = take(obs ? Npad * 4 : 0); L.acc = take(obs ? Npad * 4 : 0);
     L.bias = take(Npad * 4);
     L.refr = take(Npad); L.cls = take(Npad);
@@ -259,6 +260,7 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
     d.obs_gain = cfg->obs_gain; d.obs_offset = cfg->obs_offset; d.obs_sigma = cfg->obs_sigma;
     d.inv_stride = cfg->obs_stride ? (float)(1.0 / (double)cfg->obs_stride) : 0.0f;
     d.V = (float *)(ws + L.V); d.W = (float *)(ws + L.W); d.r = (float *)(ws + L.r); d.p2 = (float *)(ws + L.p2);
+    d.hm = (float *)(ws + L.hm); d.hh = (float *)(ws + L.hh);
     d.c = cfg->obs_stride ? (float *)(ws + L.c) : nullptr;
     d.acc = cfg->obs_stride ? (float *)(ws + L.acc) : nullptr;
     d.bias = (float *)(ws + L.bias);
@@ -296,6 +298,38 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
         q.a2 = q.alpha ? (float)(1.0 / ((double)c.tau_syn_ms * (double)c.tau_syn_ms)) : 0.0f;
         q.two_a = q.alpha ? (float)(2.0 / (double)c.tau_syn_ms) : 0.0f;
         if (q.alpha) d.any_alpha = 1u;
+        if (c.model != 0.0f && c.model != 1.0f) {
+            delete net;
+            return set_err(nullptr, GN_E_INVALID_ARG, "class %u: model must be 0 (Izhikevich) or 1 (Hodgkin-Huxley)", k);
+        }
+        q.hh = c.model == 1.0f ? 1u : 0u;
+        if (q.hh) {            // Hodgkin-Huxley constants: formed once in double, rounded once
+            const float *rate[6] = {c.hh_am, c.hh_bm, c.hh_ah, c.hh_bh, c.hh_an, c.hh_bn};
+            bool ok = c.hh_c > 0.0f;
+            for (int f = 0; f < 6; ++f) ok = ok && rate[f][2] != 0.0f && isfinite(rate[f][0]) && isfinite(rate[f][1]) && isfinite(rate[f][2]);
+            if (!ok) {
+                delete net;
+                return set_err(nullptr, GN_E_INVALID_ARG, "class %u (Hodgkin-Huxley): hh_c must be > 0 and every rate function needs finite {A, V_half, k} with k != 0", k);
+            }
+            d.any_hh = 1u;
+            q.hh_dt_c = (float)((double)cfg->dt_ms / (double)c.hh_c);
+            q.hh_g_na = c.hh_g_na; q.hh_g_k = c.hh_g_k; q.hh_g_l = c.hh_g_l;
+            q.hh_e_na = c.hh_e_na; q.hh_e_k = c.hh_e_k; q.hh_e_l = c.hh_e_l;
+            double val[6];     // the rates at hh_v_rest, for the gates' initial steady states alpha / (alpha + beta)
+            for (int f = 0; f < 6; ++f) {
+                const double A = rate[f][0], vh = rate[f][1], kk = rate[f][2], u = ((double)c.hh_v_rest - vh) * (1.0 / kk);
+                const bool linoid = f == 0 || f == 4, sigmoid = f == 3;
+                q.hh_ak[f] = (float)(linoid ? A * kk : A);
+                q.hh_vh[f] = rate[f][1];
+                q.hh_inv_k[f] = (float)(1.0 / kk);
+                val[f] = linoid ? (A * kk) * (fabs(u) < 0.05 ? fma(u, fma(u, 1.0 / 12.0, 0.5), 1.0) : u / (1.0 - exp(-u)))
+                       : sigmoid ? A / (1.0 + exp(-u)) : A * exp(-u);
+            }
+            q.hh_v0 = c.hh_v_rest;
+            q.hh_m0 = (float)(val[0] / (val[0] + val[1]));
+            q.hh_h0 = (float)(val[2] / (val[2] + val[3]));
+            q.hh_n0 = (float)(val[4] / (val[4] + val[5]));
+        }
         const double R = nearbyint((double)c.refractory_ms / (double)cfg->dt_ms);
         if (!(R >= 0.0) || R > 255.0) {
             delete net;
@@ -667,6 +701,8 @@ int gn_read_state(gn_net *net, int which, void *dst, size_t dst_bytes, int dst_i
     case GN_W: src = d.W; need = N * 4; break;
     case GN_R: src = d.r; need = N * 4; break;
     case GN_P: src = d.p2; need = N * 4; break;
+    case GN_M: src = d.hm; need = N * 4; break;
+    case GN_H: src = d.hh; need = N * 4; break;
     case GN_CA:
         if (!d.c) return set_err(net, GN_E_INVALID_ARG, "calcium is not maintained when obs_stride == 0");
         src = d.c; need = N * 4; break;
@@ -715,6 +751,8 @@ int gn_write_state(gn_net *net, int which, const void *src, size_t src_bytes, in
     case GN_W: dst = d.W; break;
     case GN_R: dst = d.r; break;
     case GN_P: dst = d.p2; break;
+    case GN_M: dst = d.hm; break;
+    case GN_H: dst = d.hh; break;
     case GN_CA:
         if (!d.c) return set_err(net, GN_E_INVALID_ARG, "calcium is not maintained when obs_stride == 0");
         dst = d.c; break;

@@ -19,10 +19,19 @@ struct GnClassDev {
     int32_t kick_fx;     // rint(kick * 2^16)
     uint32_t alpha;      // alpha-function PSC (eq. 27, 29, 30) instead of the exponential one
     float a2, two_a;     // (float)(1/tau_s^2), (float)(2/tau_s)
-    uint32_t pad_;       // 17 words on purpose: a 16-byte-aligned table invites 128-bit shared-memory loads of whole
-                         // rows, which costs the 32-register update kernel four live registers per vertex
+    uint32_t hh;         // Hodgkin-Huxley class (gn_class_params.model == 1)
+    // Hodgkin-Huxley constants, each formed once in double on the host and rounded once:
+    float hh_dt_c;       // dt / C
+    float hh_g_na, hh_g_k, hh_g_l, hh_e_na, hh_e_k, hh_e_l;
+    float hh_ak[6];      // A of each rate function (A k for the two linoid ones): alpha_m, beta_m, alpha_h, beta_h, alpha_n, beta_n
+    float hh_vh[6];      // V_half
+    float hh_inv_k[6];   // 1 / k
+    float hh_v0, hh_m0, hh_h0, hh_n0;   // initial state: hh_v_rest and the gates' steady states there
+    uint32_t pad_;
+    // kClassWords is odd on purpose: a 16-byte-aligned table invites 128-bit shared-memory loads of whole rows, which
+    // costs the 32-register update kernel four live registers per vertex
 };
-constexpr uint32_t kClassWords = 17;
+constexpr uint32_t kClassWords = 47;
 static_assert(sizeof(GnClassDev) == kClassWords * 4, "GnClassDev must stay kClassWords words");
 
 // Everything a kernel needs, passed by value (kernel parameter space).
@@ -40,6 +49,8 @@ struct GnDev {
     float *V, *W, *r, *c, *acc, *bias;
     float *p2;               // second PSC state of alpha-function classes (touched only when any_alpha)
     uint32_t any_alpha;
+    float *hm, *hh;          // gates m and h of Hodgkin-Huxley vertices (touched only when any_hh); n lives in W
+    uint32_t any_hh;
     uint8_t *refr, *cls;
     // delay ring [D][Npad], int32 fixed point 2^-16
     int32_t *ring;

@@ -88,10 +88,81 @@ __device__ __forceinline__ bool vertex_step(const GnClassDev &q, const float dt,
     return fired;
 }
 
+// ---- Hodgkin-Huxley vertex (textbook equations, forward Euler PAPER.md:184 eq. 19) ----------
+// exp of the arithmetic contract: clamp to [-87, 88]; n = rint(x log2 e); r = x - n ln 2 in two steps; degree-7 Taylor
+// polynomial of e^r by Horner; scaled by 2^n through the exponent field.  Every step one rounded binary32 operation,
+// the same sequence as the oracle's fp32-faithful mode, so Hodgkin-Huxley vertices are bit-exact too.
+__device__ __forceinline__ float exp32(float x)
+{
+    x = fminf(fmaxf(x, -87.0f), 88.0f);
+    const float n = rintf(__fmul_rn(x, 0x1.715476p+0f));
+    float r = __fmaf_rn(n, -0x1.62e400p-1f, x);
+    r = __fmaf_rn(n, -0x1.7f7d1cp-20f, r);
+    float p = 0x1.a01a02p-13f;
+    p = __fmaf_rn(p, r, 0x1.6c16c2p-10f);
+    p = __fmaf_rn(p, r, 0x1.111112p-7f);
+    p = __fmaf_rn(p, r, 0x1.555556p-5f);
+    p = __fmaf_rn(p, r, 0x1.555556p-3f);
+    p = __fmaf_rn(p, r, 0.5f);
+    p = __fmaf_rn(p, r, 1.0f);
+    p = __fmaf_rn(p, r, 1.0f);
+    return __fmul_rn(p, __int_as_float((__float2int_rn(n) + 127) << 23));
+}
+
+// Rate function F of the six (0 alpha_m, 1 beta_m, 2 alpha_h, 3 beta_h, 4 alpha_n, 5 beta_n) at V.
+template <int F>
+__device__ __forceinline__ float hh_rate(const GnClassDev &q, const float V)
+{
+    const float u = __fmul_rn(__fsub_rn(V, q.hh_vh[F]), q.hh_inv_k[F]);
+    if (F == 0 || F == 4) {                                   // linoid A k u / (1 - exp(-u)); series near u = 0
+        if (fabsf(u) < 0.05f) return __fmul_rn(q.hh_ak[F], __fmaf_rn(u, __fmaf_rn(u, 0x1.555556p-4f, 0.5f), 1.0f));
+        return __fmul_rn(q.hh_ak[F], __fdiv_rn(u, __fsub_rn(1.0f, exp32(-u))));
+    }
+    if (F == 3) return __fdiv_rn(q.hh_ak[F], __fadd_rn(1.0f, exp32(-u)));      // sigmoid
+    return __fmul_rn(q.hh_ak[F], exp32(-u));                                    // exponential
+}
+
+// One Hodgkin-Huxley vertex, one step: state at t in, state at t+1 out (n lives in W); returns spd(V(t)) outside the
+// detection dead time.  No reset: `refr` only keeps one action potential from being detected twice.
+template <bool BIAS>
+__device__ __forceinline__ bool vertex_step_hh(const GnClassDev &q, const float dt, const int32_t I_fx, const float U,
+                                               float &V, float &n, float &r, uint32_t &refr, float &pp, float &m, float &h)
+{
+    const float If = __fmul_rn(__int2float_rn(I_fx), 0x1p-16f);
+    const bool fired = (refr == 0u) && (V >= q.v_peak);                  // eq. 31 (>=)
+    if (fired) refr = q.R;
+    else if (refr > 0u) refr -= 1u;
+    const float am = hh_rate<0>(q, V), bm = hh_rate<1>(q, V), ah = hh_rate<2>(q, V);
+    const float bh = hh_rate<3>(q, V), an = hh_rate<4>(q, V), bn = hh_rate<5>(q, V);
+    const float m2 = __fmul_rn(m, m), m3 = __fmul_rn(m2, m);
+    const float i_na = __fmul_rn(__fmul_rn(__fmul_rn(q.hh_g_na, m3), h), __fsub_rn(V, q.hh_e_na));
+    const float n2 = __fmul_rn(n, n), n4 = __fmul_rn(n2, n2);
+    const float i_k = __fmul_rn(__fmul_rn(q.hh_g_k, n4), __fsub_rn(V, q.hh_e_k));
+    const float i_l = __fmul_rn(q.hh_g_l, __fsub_rn(V, q.hh_e_l));
+    float s = __fsub_rn(r, __fadd_rn(__fadd_rn(i_na, i_k), i_l));
+    if (BIAS) s = __fadd_rn(s, U);
+    const float Vn = __fmaf_rn(q.hh_dt_c, s, V);
+    m = __fmaf_rn(dt, __fmaf_rn(-bm, m, __fmul_rn(am, __fsub_rn(1.0f, m))), m);
+    h = __fmaf_rn(dt, __fmaf_rn(-bh, h, __fmul_rn(ah, __fsub_rn(1.0f, h))), h);
+    n = __fmaf_rn(dt, __fmaf_rn(-bn, n, __fmul_rn(an, __fsub_rn(1.0f, n))), n);
+    if (q.alpha) {
+        const float q1 = __fmul_rn(q.a2, r);
+        const float q2 = __fmaf_rn(q.two_a, pp, q1);
+        const float p1 = __fmaf_rn(-dt, q2, pp);
+        r = __fmaf_rn(dt, pp, r);
+        pp = __fadd_rn(p1, If);
+    } else if (!q.direct) {
+        r = __fmaf_rn(q.keep_s, r, If);
+    }
+    V = Vn;
+    return fired;
+}
+
 // ---- a1 + a2 + a3 (+ calcium of a5) ---------------------------------------------------------------
 // Thread g owns vertices 4g .. 4g+3 (128-bit SoA loads); a warp owns 128 vertices = 4 raster words.
-template <bool OBS, bool BIAS, bool FUSED, bool ALPHA>
-__global__ void __launch_bounds__(kUpdateThreads, (FUSED || ALPHA) ? 4 : 8)
+// HH: some class is a Hodgkin-Huxley one (two more fp32 streams, m and h; a vertex takes its class's transition function).
+template <bool OBS, bool BIAS, bool FUSED, bool ALPHA, bool HH>
+__global__ void __launch_bounds__(kUpdateThreads, HH ? 3 : (FUSED || ALPHA) ? 4 : 8)
 gn_update_kernel(const GnDev p, const uint64_t t, const uint32_t slot, const uint32_t raster_row,
                  const uint32_t d_direct)
 {
@@ -99,8 +170,8 @@ gn_update_kernel(const GnDev p, const uint64_t t, const uint32_t slot, const uin
     // Programmatic dependent launch: the next step's update may start launching now; its prologue (class table,
     // Philox words -- nothing a previous kernel wrote) then overlaps this kernel's tail (see griddepcontrol.wait below).
     asm volatile("griddepcontrol.launch_dependents;");
-    if (threadIdx.x < p.n_classes * kClassWords)
-        reinterpret_cast<uint32_t *>(s_cls)[threadIdx.x] = reinterpret_cast<const uint32_t *>(p.cls_tab)[threadIdx.x];
+    for (uint32_t q = threadIdx.x; q < p.n_classes * kClassWords; q += kUpdateThreads)
+        reinterpret_cast<uint32_t *>(s_cls)[q] = reinterpret_cast<const uint32_t *>(p.cls_tab)[q];
     __syncthreads();
 
     const uint32_t lane = threadIdx.x & 31u;
@@ -146,6 +217,13 @@ gn_update_kernel(const GnDev p, const uint64_t t, const uint32_t slot, const uin
             const float4 p4 = *reinterpret_cast<const float4 *>(p.p2 + j0);
             pp[0] = p4.x; pp[1] = p4.y; pp[2] = p4.z; pp[3] = p4.w;
         }
+        float gm[4] = {0.f, 0.f, 0.f, 0.f}, gh[4] = {0.f, 0.f, 0.f, 0.f};
+        if (HH) {
+            const float4 m4 = *reinterpret_cast<const float4 *>(p.hm + j0);
+            const float4 h4 = *reinterpret_cast<const float4 *>(p.hh + j0);
+            gm[0] = m4.x; gm[1] = m4.y; gm[2] = m4.z; gm[3] = m4.w;
+            gh[0] = h4.x; gh[1] = h4.y; gh[2] = h4.z; gh[3] = h4.w;
+        }
         uint32_t refr[4] = {rf4.x, rf4.y, rf4.z, rf4.w};
 
         uint32_t refr_changed = 0u;
@@ -154,7 +232,9 @@ gn_update_kernel(const GnDev p, const uint64_t t, const uint32_t slot, const uin
             const GnClassDev &k = s_cls[cl[q]];
             if ((kicks >> q) & 1u) I[q] += k.kick_fx;
             const uint32_t refr_old = refr[q];
-            const bool fired = vertex_step<BIAS, ALPHA>(k, p.dt, I[q], U[q], V[q], W[q], r[q], refr[q], pp[q]) && (j0 + q) < p.N;
+            const bool fired = ((HH && k.hh) ? vertex_step_hh<BIAS>(k, p.dt, I[q], U[q], V[q], W[q], r[q], refr[q], pp[q], gm[q], gh[q])
+                                             : vertex_step<BIAS, ALPHA>(k, p.dt, I[q], U[q], V[q], W[q], r[q], refr[q], pp[q])) &&
+                               (j0 + q) < p.N;
             refr_changed |= (refr[q] != refr_old);
             if (fired) nib |= 1u << q;
         }
@@ -162,6 +242,10 @@ gn_update_kernel(const GnDev p, const uint64_t t, const uint32_t slot, const uin
         *reinterpret_cast<float4 *>(p.W + j0) = make_float4(W[0], W[1], W[2], W[3]);
         *reinterpret_cast<float4 *>(p.r + j0) = make_float4(r[0], r[1], r[2], r[3]);
         if (ALPHA) *reinterpret_cast<float4 *>(p.p2 + j0) = make_float4(pp[0], pp[1], pp[2], pp[3]);
+        if (HH) {
+            *reinterpret_cast<float4 *>(p.hm + j0) = make_float4(gm[0], gm[1], gm[2], gm[3]);
+            *reinterpret_cast<float4 *>(p.hh + j0) = make_float4(gh[0], gh[1], gh[2], gh[3]);
+        }
         if (refr_changed)
             *reinterpret_cast<uchar4 *>(p.refr + j0) = make_uchar4(refr[0], refr[1], refr[2], refr[3]);
         if (OBS) {                                                            // calcium + frame accumulator
@@ -736,7 +820,7 @@ gn_observe_kernel(const GnDev p, const uint64_t frame, const uint32_t trace_row)
 // of its groups for 4 steps at a time into shared memory (one block per thread) instead of one per thread per step.
 constexpr int kResidentPhiloxSteps = 4;
 
-template <bool OBS, bool BIAS, bool PACKED, bool CLUSTER>
+template <bool OBS, bool BIAS, bool PACKED, bool CLUSTER, bool HH>
 __global__ void __launch_bounds__(1024, 1)
 gn_resident_kernel(const GnDev p, const uint64_t t0, const uint32_t n_steps, const uint32_t raster_on)
 {
@@ -763,11 +847,12 @@ gn_resident_kernel(const GnDev p, const uint64_t t0, const uint32_t n_steps, con
     for (uint32_t q = i; q < p.n_classes * kClassWords; q += stride)   // a CTA may have as few as 32 threads
         reinterpret_cast<uint32_t *>(s_cls)[q] = reinterpret_cast<const uint32_t *>(p.cls_tab)[q];
     if (i < 3u) s_tot[i] = 0ull;
-    float V = 0.f, W = 0.f, r = 0.f, c = 0.f, acc = 0.f, U = 0.f, pp = 0.f;
+    float V = 0.f, W = 0.f, r = 0.f, c = 0.f, acc = 0.f, U = 0.f, pp = 0.f, gm = 0.f, gh = 0.f;
     uint32_t refr = 0u, cl = 0u;
     if (live) {
         V = p.V[j]; W = p.W[j]; r = p.r[j]; refr = p.refr[j]; cl = p.cls[j];
         if (p.any_alpha) pp = p.p2[j];
+        if (HH) { gm = p.hm[j]; gh = p.hh[j]; }
         if (OBS) { c = p.c[j]; acc = p.acc[j]; }
         if (BIAS) U = p.bias[j];
     }
@@ -802,7 +887,8 @@ gn_resident_kernel(const GnDev p, const uint64_t t0, const uint32_t n_steps, con
             if (x < k.drive_thr) { I += k.kick_fx; ++n_kicks; }
         }
         // a2 + a3
-        const bool fired = vertex_step<BIAS, true>(k, p.dt, I, U, V, W, r, refr, pp) && live;
+        const bool fired = ((HH && k.hh) ? vertex_step_hh<BIAS>(k, p.dt, I, U, V, W, r, refr, pp, gm, gh)
+                                         : vertex_step<BIAS, true>(k, p.dt, I, U, V, W, r, refr, pp)) && live;
         if (OBS) {
             c = __fmaf_rn(p.keep_c, c, fired ? p.ca_jump : 0.0f);            // H_c
             acc = __fadd_rn(acc, c);
@@ -873,6 +959,7 @@ gn_resident_kernel(const GnDev p, const uint64_t t0, const uint32_t n_steps, con
     if (live) {
         p.V[j] = V; p.W[j] = W; p.r[j] = r; p.refr[j] = (uint8_t)refr;
         if (p.any_alpha) p.p2[j] = pp;
+        if (HH) { p.hm[j] = gm; p.hh[j] = gh; }
         if (OBS) { p.c[j] = c; p.acc[j] = acc; }
     }
     for (uint32_t s = 0; s < p.D; ++s)
@@ -904,8 +991,11 @@ __global__ void gn_init_state_kernel(const GnDev p, GnCheck *chk)
         chk->bad_class = 1u;
         k = 0u;
     }
-    p.V[j] = -70.0f;                                        // reading #15
-    p.W[j] = __fmul_rn(p.cls_tab[k].b, -70.0f);
+    const GnClassDev &q = p.cls_tab[k];
+    p.V[j] = q.hh ? q.hh_v0 : -70.0f;                       // reading #15; Hodgkin-Huxley: at rest, gates at their steady states
+    p.W[j] = q.hh ? q.hh_n0 : __fmul_rn(q.b, -70.0f);
+    p.hm[j] = q.hh ? q.hh_m0 : 0.0f;
+    p.hh[j] = q.hh ? q.hh_h0 : 0.0f;
     p.r[j] = 0.0f;
     p.p2[j] = 0.0f;
     p.refr[j] = 0;
@@ -1041,18 +1131,20 @@ cudaError_t gnk_update(const GnDev &p, uint64_t t, bool has_bias, cudaStream_t s
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
+#define GN_UPD2(O, B, A, H)                                                                                      \
+    return p.fused ? cudaLaunchKernelEx(&cfg, gn_update_kernel<O, B, true, A, H>, p, t, slot, raster_row, d_direct)  \
+                   : cudaLaunchKernelEx(&cfg, gn_update_kernel<O, B, false, A, H>, p, t, slot, raster_row, d_direct)
 #define GN_UPD(O, B)                                                                                              \
     do {                                                                                                          \
-        if (p.any_alpha)                                                                                          \
-            return p.fused ? cudaLaunchKernelEx(&cfg, gn_update_kernel<O, B, true, true>, p, t, slot, raster_row, d_direct)   \
-                           : cudaLaunchKernelEx(&cfg, gn_update_kernel<O, B, false, true>, p, t, slot, raster_row, d_direct); \
-        return p.fused ? cudaLaunchKernelEx(&cfg, gn_update_kernel<O, B, true, false>, p, t, slot, raster_row, d_direct)      \
-                       : cudaLaunchKernelEx(&cfg, gn_update_kernel<O, B, false, false>, p, t, slot, raster_row, d_direct);    \
+        if (p.any_hh) GN_UPD2(O, B, true, true);      /* a Hodgkin-Huxley network: one variant for either PSC */     \
+        if (p.any_alpha) GN_UPD2(O, B, true, false);                                                              \
+        GN_UPD2(O, B, false, false);                                                                              \
     } while (0)
     if (obs && has_bias) GN_UPD(true, true);
     if (obs) GN_UPD(true, false);
     if (has_bias) GN_UPD(false, true);
     GN_UPD(false, false);
+#undef GN_UPD2
 #undef GN_UPD
 }
 
@@ -1090,7 +1182,7 @@ cudaError_t gnk_resident_cluster_ok(const GnDev &p, bool *ok)
 {
     *ok = true;
     if (p.res_cluster <= 1u) return cudaSuccess;
-    ResidentKernel k = p.packed ? gn_resident_kernel<false, false, true, true> : gn_resident_kernel<false, false, false, true>;
+    ResidentKernel k = p.packed ? gn_resident_kernel<false, false, true, true, false> : gn_resident_kernel<false, false, false, true, false>;
     cudaLaunchConfig_t cfg;
     cudaLaunchAttribute attr[1];
     cudaError_t e = resident_config(k, p, cfg, attr);
@@ -1114,10 +1206,15 @@ cudaError_t gnk_resident(const GnDev &p, uint64_t t0, uint32_t n_steps, bool has
         if (e != cudaSuccess) return e;
     }
     const bool obs = p.obs_stride != 0u;
+#define GN_RES_LAUNCH2(O, B, P, H)                                                                               \
+    do {                                                                                                        \
+        if (p.res_cluster > 1u) return resident_launch(gn_resident_kernel<O, B, P, true, H>, p, t0, n_steps, raster_on, st);  \
+        return resident_launch(gn_resident_kernel<O, B, P, false, H>, p, t0, n_steps, raster_on, st);              \
+    } while (0)
 #define GN_RES_LAUNCH(O, B, P)                                                                                  \
     do {                                                                                                        \
-        if (p.res_cluster > 1u) return resident_launch(gn_resident_kernel<O, B, P, true>, p, t0, n_steps, raster_on, st);  \
-        return resident_launch(gn_resident_kernel<O, B, P, false>, p, t0, n_steps, raster_on, st);                \
+        if (p.any_hh) GN_RES_LAUNCH2(O, B, P, true);                                                            \
+        GN_RES_LAUNCH2(O, B, P, false);                                                                         \
     } while (0)
     if (p.packed) {
         if (obs && has_bias) GN_RES_LAUNCH(true, true, true);
@@ -1129,6 +1226,7 @@ cudaError_t gnk_resident(const GnDev &p, uint64_t t0, uint32_t n_steps, bool has
     if (obs) GN_RES_LAUNCH(true, false, false);
     if (has_bias) GN_RES_LAUNCH(false, true, false);
     GN_RES_LAUNCH(false, false, false);
+#undef GN_RES_LAUNCH2
 #undef GN_RES_LAUNCH
 }
 

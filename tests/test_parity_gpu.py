@@ -717,3 +717,96 @@ def test_device_destinations_and_write_state_roundtrip(gn):
     np.testing.assert_array_equal(r_dev.cpu().numpy().view(np.uint32), gn.gn_read_raster(g, 0, 100))
     gn.gn_write_state(g, gn.GN_V, v_host[::-1].copy())
     np.testing.assert_array_equal(gn.gn_read_state(g, gn.GN_V), v_host[::-1])
+
+
+# ---- Hodgkin-Huxley vertex class ----------------------------------------------------------
+def _compare_hh_gates(gn, g, o):
+    for wg, wo in ((gn.GN_M, ob.HM), (gn.GN_H, ob.HH)):
+        np.testing.assert_array_equal(gn.gn_read_state(g, wg).view(np.uint32),
+                                      o.state(wo).astype(np.float32).view(np.uint32))
+
+
+@pytest.mark.parametrize("k,n,nb,steps,chunk,mode", [
+    (5, 1000, 6, 3000, 1000, "RESIDENT"),       # the paper's workload shape: small networks, one CTA each
+    (5, 1000, 6, 3000, 1000, "RING"),           # the same through the streaming kernels (fused update + delivery)
+    (2, 3_000, None, 2400, 800, "RESIDENT"),    # a 3-CTA cluster, observation every step
+    (4, 9_001, None, 2000, 500, "QUEUE"),       # D = 128, routing + folding
+    (3, 300_000, None, 300, 150, "RING"),       # above the fused limit: separate delivery kernel
+])
+def test_hodgkin_huxley_bit_exact(gn, k, n, nb, steps, chunk, mode):
+    """Every class a Hodgkin-Huxley vertex at the paper's HH time step (0.03 ms): rasters, ring, counters and the state
+    words V, n (GN_W), r, m, h bit-exact against the oracle's fp32-faithful mode -- the contract pins exp, so the
+    transcendental model is as exact as the polynomial one."""
+    from gn_inputs import as_hodgkin_huxley
+    net, cfg = make_config(k, n=n, n_networks=nb)
+    cfg = as_hodgkin_huxley(cfg)
+    g, o, _ = _run_exact(gn, net, cfg, steps, chunk, delivery_mode=getattr(gn, "GN_DELIVER_" + mode), threads=8)
+    _compare_hh_gates(gn, g, o)
+    assert o.counters()["spikes"] > 0 and o.counters()["delivered"] > 0
+    if cfg["obs_stride"]:
+        frames = steps // cfg["obs_stride"]
+        np.testing.assert_allclose(gn.gn_observe(g, 0, frames).astype(np.float64), o.trace(0, frames), rtol=1e-6, atol=1e-5)
+
+
+def test_hodgkin_huxley_mixed_with_izhikevich_alpha_psc_and_bias(gn):
+    """One network, three classes: Hodgkin-Huxley with the alpha-function PSC, Hodgkin-Huxley with the exponential one,
+    Izhikevich regular spiking; a bias current on every vertex; gates written through gn_write_state."""
+    from gn_inputs import hh_class
+    rng = np.random.default_rng(17)
+    net, _ = make_config(2, n=2_500)
+    vc = rng.integers(0, 3, net.n_vertices).astype(np.uint8)
+    net = Network(net.n_vertices, net.dim, 1, net.positions, net.row_offsets, net.targets, net.weights, vc)
+    cfg = base_cfg([hh_class(200.0, psc_alpha=1.0), hh_class(200.0, tau_syn_ms=1.0), rs_class(drive_rate_hz=200.0)],
+                   dt_ms=0.03, speed=0.5, ring_slots=16)
+    bias = rng.uniform(0.0, 8.0, net.n_vertices).astype(np.float32)
+    g = _make(gn, net, cfg, 1500, bias=bias, delivery_mode=gn.GN_DELIVER_RING)
+    o = Oracle(net, cfg, "fp32", bias=bias, threads=4)
+    h0 = rng.uniform(0.3, 0.7, net.n_vertices).astype(np.float32) * (vc < 2)
+    gn.gn_write_state(g, gn.GN_H, h0)
+    o.set_state(ob.HH, h0.astype(np.float64))
+    gn.gn_step(g, 1500)
+    o.step(1500)
+    _compare_exact(gn, g, o, 1500)
+    _compare_hh_gates(gn, g, o)
+    np.testing.assert_array_equal(gn.gn_read_state(g, gn.GN_P).view(np.uint32), o.state(ob.P).astype(np.float32).view(np.uint32))
+    np.testing.assert_array_equal(gn.gn_read_raster(g, 0, 1500), o.raster(0, 1500))
+    r = unpack_raster(gn.gn_read_raster(g, 0, 1500), net.n_vertices)
+    assert all(r[:, vc == c].any() for c in range(3)), "every class fired"
+    assert not gn.gn_read_state(g, gn.GN_M)[vc == 2].any()
+
+
+def test_hodgkin_huxley_textbook_behaviour_on_the_device(gn):
+    """The pins of the oracle's Hodgkin-Huxley class, asked of the kernels directly: rest is a fixed point, a constant
+    10 uA/cm^2 fires at the textbook ~68.5 Hz, 2 uA/cm^2 never fires."""
+    from gn_inputs import hh_class
+    net, dl = hand_net(3, [])
+    cfg = base_cfg([hh_class()], dt_ms=0.03)
+    g = _make(gn, net, cfg, 20_000, delays=dl, bias=np.array([10.0, 2.0, 0.0], np.float32))
+    gn.gn_step(g, 20_000)
+    r = unpack_raster(gn.gn_read_raster(g, 0, 20_000), 3)
+    t = np.flatnonzero(r[:, 0])
+    assert 1000.0 / (np.diff(t[3:]).mean() * 0.03) == pytest.approx(68.5, abs=3.0)
+    assert not r[:, 1].any() and not r[:, 2].any()
+    assert abs(float(gn.gn_read_state(g, gn.GN_V)[2]) + 65.0) < 0.01
+
+
+def test_hodgkin_huxley_state_within_tolerance_of_fp64(gn):
+    """CUDA Hodgkin-Huxley vertices against the fp64 DEFINITION (libm exp, double state) through the fp64 gate with the
+    windows of this model (helpers.HH_GATE)."""
+    from gn_inputs import as_hodgkin_huxley
+    from helpers import HH_GATE
+    net, cfg = make_config(5, n=1000, n_networks=3)
+    cfg = dict(as_hodgkin_huxley(cfg), obs_stride=0)
+    gate, chunk, steps = Fp64Gate(net.n_vertices, **HH_GATE), 50, 6000
+    g = _make(gn, net, cfg, steps + gate.pre)
+    o = Oracle(net, cfg, "fp64", threads=4)
+    names = (("V", gn.GN_V, ob.V), ("W", gn.GN_W, ob.W), ("R", gn.GN_R, ob.R), ("M", gn.GN_M, ob.HM), ("H", gn.GN_H, ob.HH))
+    for done in range(chunk, steps + 1, chunk):
+        gn.gn_step(g, chunk)
+        o.step(chunk)
+        gate.add(done, {w: gn.gn_read_state(g, wg) for w, wg, _ in names}, {w: o.state(wo) for w, _, wo in names})
+    gn.gn_step(g, gate.pre)
+    o.step(gate.pre)
+    rg = unpack_raster(gn.gn_read_raster(g, 0, steps + gate.pre), net.n_vertices)
+    t_star, stats = gate.check(rg, o.raster_bool(0, steps + gate.pre), "CUDA Hodgkin-Huxley vs fp64 oracle")
+    assert o.counters()["spikes"] > 100
