@@ -33,6 +33,10 @@ if ROOT not in sys.path:
 METRIC, UNIT = "vertex-steps/s", "vertex-steps/s"
 UPDATE_BYTES_PER_VERTEX = 35.125       # V,W,r r+w 24, ring slot r+clear 8, refr 2, class 1, raster bit 1/8
 UPDATE_BYTES_PER_VERTEX_OBS = 12.0     # + c r+w 8, frame accumulator amortised / trace row 4 per frame (counted per step as 4)
+HH_BYTES_PER_VERTEX = 51.125           # Hodgkin-Huxley class: V, n, r, m, h r+w 40, ring slot r+clear 8, refr 2, class 1, raster bit 1/8
+HH_FP32_PER_VERTEX = 141.0             # fp32 operations of the contract per Hodgkin-Huxley vertex-step (6 exp32 x 14,
+                                       # rate arguments and shapes 25, currents 16, gates 12, V, PSC, input 4; a division counts 1)
+FP32_LANES_PER_SM, SM_COUNT, SM_HZ = 128, 148, 1.965e9   # B200_PROFILING.md: 148 SMs, 1965 MHz; 4 x 32 fp32 lanes per SM
 EVENT_BYTES = 17.0                     # edge record 9 (target 4, weight 4, delay 1) + ring word read-modify-write 8
 SOURCE_BYTES = 12.0                    # two row offsets + active-list entry per fired source
 SECTOR_EVENT_BYTES = 73.0              # 9 + one 32 B sector fetched + one written back (ring >> L2)
@@ -152,6 +156,9 @@ def run_reference(args):
     t0 = time.time()
     net_in, cfg = make_config(args.config, n=args.n)
     cfg = dict(cfg, obs_stride=0 if args.config == 4 else cfg["obs_stride"])
+    if args.model == "hh":
+        from gn_inputs import as_hodgkin_huxley
+        cfg = as_hodgkin_huxley(cfg)
     if args.psc_alpha:
         cfg = dict(cfg, classes=[dict(c, psc_alpha=1.0) for c in cfg["classes"]], name=cfg["name"] + "+alpha_psc")
     log(f"[reference] inputs in {time.time() - t0:.1f} s: N={net_in.n_vertices} E={net_in.n_edges}")
@@ -232,6 +239,9 @@ def main():
     ap.add_argument("--queue-group", type=int, default=0, help="gn_config.queue_group (0 = library default)")
     ap.add_argument("--psc-alpha", action="store_true", help="every class uses the alpha-function PSC (DESIGN.md f-1) "
                                                               "instead of the config's exponential one: a different workload")
+    ap.add_argument("--model", default="izhikevich", choices=["izhikevich", "hh"],
+                    help="hh: every class a Hodgkin-Huxley vertex at dt = 0.03 ms (the paper's second benchmarked model, "
+                         "PAPER.md:382): a different workload, reported with an fp32-ALU roofline beside the HBM one")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -258,6 +268,9 @@ def main():
     t0 = time.time()
     # replicas only: rank r steps its own independent network of the same recipe
     net_in, cfg = make_config(args.config, n=args.n, seed=rank_seed(args.config, rank))
+    if args.model == "hh":
+        from gn_inputs import as_hodgkin_huxley
+        cfg = as_hodgkin_huxley(cfg)
     if args.psc_alpha:
         cfg = dict(cfg, classes=[dict(c, psc_alpha=1.0) for c in cfg["classes"]], name=cfg["name"] + "+alpha_psc")
     N, E = net_in.n_vertices, net_in.n_edges
@@ -338,7 +351,8 @@ def main():
     # delivery kernel of either mode (queue mode: one launch per slot group routes the group's events and folds as
     # many records of an earlier group)
     delivery_bytes = p_events * EVENT_BYTES + p_spikes * SOURCE_BYTES
-    kbytes = [N * (UPDATE_BYTES_PER_VERTEX + (UPDATE_BYTES_PER_VERTEX_OBS if obs else 0.0)) * (sim_steps / max(int(kn[0]), 1))
+    per_vertex = HH_BYTES_PER_VERTEX if args.model == "hh" else UPDATE_BYTES_PER_VERTEX
+    kbytes = [N * (per_vertex + (UPDATE_BYTES_PER_VERTEX_OBS if obs else 0.0)) * (sim_steps / max(int(kn[0]), 1))
               + (delivery_bytes / max(int(kn[0]), 1) if kn[1] == 0 else 0.0),
               delivery_bytes / max(int(kn[1]), 1),
               N * 8.0,
@@ -383,6 +397,14 @@ def main():
                           "kernel boundary (gn_profile; serialised on one stream)",
                 "kernels": kernels, "a4_delivery": a4, "profile_pass_events_per_sim_step": p_events / sim_steps,
                 "timed_pass_events_per_sim_step": (c1[2] - c0[2]) / sim_steps}
+    if args.model == "hh":      # the update kernel against the fp32 pipe as well: which of the two bounds it depends on the measurement
+        upd = kernels[0]
+        fp32_peak = FP32_LANES_PER_SM * SM_COUNT * SM_HZ
+        ach = N * HH_FP32_PER_VERTEX * (sim_steps / max(int(kn[0]), 1)) / (upd["avg_us"] * 1e-6)
+        roofline["alu"] = {"bound": "alu", "kernel": upd["kernel"], "achieved": ach / 1e12, "peak": fp32_peak / 1e12,
+                           "unit": "T fp32 instr/s", "frac": ach / fp32_peak,
+                           "peak_source": "148 SMs x 128 fp32 lanes x 1.965 GHz (B200_PROFILING.md unit counts and clock; an FMA "
+                                          "counts once); 141 fp32 operations of the contract per vertex-step"}
     if dom["kernel"].startswith("gn_deliver"):   # ring mode only: what DRAM moves when every event misses L2
         sect = (p_events * SECTOR_EVENT_BYTES + p_spikes * SOURCE_BYTES) / max(int(kn[1]), 1)
         roofline["sector_granular"] = {"bytes_per_launch": sect, "achieved": sect / (dom["avg_us"] * 1e-6) / 1e9,

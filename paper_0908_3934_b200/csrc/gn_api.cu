@@ -4,6 +4,7 @@
 #include <math.h>
 #include <stdarg.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <new>
@@ -122,6 +123,7 @@ struct gn_net {
     uint8_t *ws;
     uint64_t t;          // steps enqueued so far
     uint64_t t_origin;   // first step simulated by this handle (0, or the t a checkpoint was restored at)
+    unsigned long long sync_base;   // persistent step driver: value of its barrier counter when the next launch starts
     uint64_t routed_upto; // queue mode: steps < routed_upto have had their queued events routed
     // delivery of step t overlaps the update of step t+1 (see gn_step): side streams and their fences
     cudaStream_t s_deliver;
@@ -233,6 +235,7 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
     net->t = 0;
     net->t_origin = 0;
     net->routed_upto = 0;
+    net->sync_base = 0;
     net->s_deliver = nullptr;
     net->ev_update = net->ev_deliver[0] = net->ev_deliver[1] = net->ev_fold[0] = net->ev_fold[1] = net->ev_fold[2] = net->ev_fold[3] = nullptr;
     net->fences_pending = false;
@@ -444,6 +447,13 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
     }
     // ring mode on a small network: one kernel per step (the update delivers), bound by launch latency not work
     d.fused = (!d.resident && !d.queue_mode && Npad <= (1u << 18)) ? 1u : 0u;
+    // ... and when its whole update grid can be co-resident, one cooperative launch per gn_step call (gn_persist_kernel).
+    // GN_NO_PERSIST (environment): measurements of the per-step path only.
+    if (d.fused && !getenv("GN_NO_PERSIST")) {
+        bool ok = false;
+        GN_CREATE_CUDA(gnk_persist_ok(d, &ok));
+        d.persist = ok ? 1u : 0u;
+    }
     if (E) {
         GN_CREATE_CUDA(gnk_quantise(d, E, chk_d, st));
         if (!delays) GN_CREATE_CUDA(gnk_delays_from_positions(d, pos_d, cfg->dim, cfg->speed, chk_d, st));
@@ -580,6 +590,24 @@ int gn_step(gn_net *net, uint64_t n_steps)
             int rc;
             if (net->profile && (rc = prof_mark(net, 0))) return rc;
             GN_CUDA(net, gnk_resident(d, net->t, (uint32_t)n, net->has_bias, raster_on, net->stream));
+            net->launches++;
+            net->t += n;
+            left -= n;
+        }
+        if (net->profile) {
+            int rc = prof_mark(net, 0xFF);
+            return rc ? rc : prof_collect(net);
+        }
+        return GN_OK;
+    }
+    if (d.persist) {       // ring mode, co-resident grid: the whole call is one cooperative launch
+        uint64_t left = n_steps;
+        while (left) {
+            const uint64_t n = left > 0x40000000ull ? 0x40000000ull : left;
+            int rc;
+            if (net->profile && (rc = prof_mark(net, 0))) return rc;
+            // the barrier counter lives in the (otherwise unused in ring mode) bucket-count words, zeroed at create
+            GN_CUDA(net, gnk_persist(d, net->t, (uint32_t)n, net->has_bias, d.q_count, &net->sync_base, net->stream));
             net->launches++;
             net->t += n;
             left -= n;

@@ -68,6 +68,7 @@ struct GnDev {
     uint8_t *s_dly;          // [E] delay of s_edge[e]
     uint8_t *min_dly;        // [Npad] smallest out-delay of every vertex (255: no out-edge)
     uint32_t packed;
+    uint32_t persist;        // ring mode on a network whose update grid is co-resident: gn_persist_kernel steps a whole gn_step call in one cooperative launch
     uint32_t fused;          // ring mode on a small network: the update kernel delivers every event itself (no delivery kernel)
     // resident mode (gn_resident_kernel): every network in one CTA
     uint32_t resident;       // 0 / 1
@@ -105,6 +106,10 @@ cudaError_t gnk_sort_rows(const GnDev &p, GnCheck *chk, cudaStream_t st);
 cudaError_t gnk_observe(const GnDev &p, uint64_t frame, cudaStream_t st);
 cudaError_t gnk_resident(const GnDev &p, uint64_t t0, uint32_t n_steps, bool has_bias, bool raster_on, cudaStream_t st);
 cudaError_t gnk_resident_cluster_ok(const GnDev &p, bool *ok);
+cudaError_t gnk_persist_ok(const GnDev &p, bool *ok);
+// sync: a device counter the launch's grid barrier counts on (it only grows); *sync_base: its value before / after the launch
+cudaError_t gnk_persist(const GnDev &p, uint64_t t0, uint32_t n_steps, bool has_bias, unsigned long long *sync,
+                        unsigned long long *sync_base, cudaStream_t st);
 cudaError_t gnk_init_state(const GnDev &p, GnCheck *chk, cudaStream_t st);
 cudaError_t gnk_convert_rows(const GnDev &p, const uint64_t *row64, uint64_t n_edges, GnCheck *chk,
                              cudaStream_t st);

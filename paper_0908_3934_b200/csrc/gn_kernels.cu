@@ -980,6 +980,216 @@ gn_resident_kernel(const GnDev p, const uint64_t t0, const uint32_t n_steps, con
     }
 }
 
+// ---- persistent step driver for ring-mode networks that fit one co-resident grid (a1-a5) --------
+// On a network of up to ~3*10^5 vertices a step is a few microseconds of work, the same order as a kernel launch, so
+// one launch per step is bound by launch latency.  Here a whole gn_step(n) call is ONE cooperative launch: thread g
+// owns vertices 4g .. 4g+3 for all n steps and keeps their state in registers (V, W, r, p, m, h, c, acc, refr); per
+// step it reads and clears its ring words, draws the kicks, advances its vertices, writes its raster nibble, delivers
+// the events of its warp's fired vertices (warp-cooperative REDs into the L2-resident ring, as the FUSED update
+// kernel) and emits its trace values at a frame boundary; one grid-wide barrier per step makes every delivery visible
+// before the slot it lands in is read.  The barrier is split: a CTA ARRIVES as soon as its delay-1 events -- the only
+// ones the very next step can read -- are out and fenced, then delivers the rest of its events, does the frame work
+// and draws the next step's kicks (none of which the next step's ring read depends on), and only then WAITS; those
+// later events are fenced by the arrival of the following step, one step before the earliest slot they touch is read.
+// No host call, no launch and no state traffic inside the call.  Same vertex_step, same generator layout, same
+// integer ring: bit-identical to the per-step kernels.  `sync` is a device counter that only grows (sync_base = its
+// value when the launch starts); a wait that would never end (a bug, never an input) gives up after ~1 s.
+template <bool OBS, bool BIAS, bool HH>
+__global__ void __launch_bounds__(kUpdateThreads, 2)
+gn_persist_kernel(const GnDev p, const uint64_t t0, const uint32_t n_steps, unsigned long long *sync,
+                  const unsigned long long sync_base)
+{
+    __shared__ GnClassDev s_cls[GN_MAX_CLASSES];
+    for (uint32_t q = threadIdx.x; q < p.n_classes * kClassWords; q += kUpdateThreads)
+        reinterpret_cast<uint32_t *>(s_cls)[q] = reinterpret_cast<const uint32_t *>(p.cls_tab)[q];
+    __syncthreads();
+    const uint32_t lane = threadIdx.x & 31u;
+    const uint32_t g = blockIdx.x * kUpdateThreads + threadIdx.x;
+    const uint32_t j0 = g * kVertsPerThread;
+    const bool mine = j0 < p.Npad;
+    float V[4] = {0.f, 0.f, 0.f, 0.f}, W[4] = {0.f, 0.f, 0.f, 0.f}, r[4] = {0.f, 0.f, 0.f, 0.f}, pp[4] = {0.f, 0.f, 0.f, 0.f};
+    float gm[4] = {0.f, 0.f, 0.f, 0.f}, gh[4] = {0.f, 0.f, 0.f, 0.f}, c[4] = {0.f, 0.f, 0.f, 0.f}, acc[4] = {0.f, 0.f, 0.f, 0.f};
+    float U[4] = {0.f, 0.f, 0.f, 0.f};
+    uint32_t refr[4] = {0u, 0u, 0u, 0u}, cl[4] = {0u, 0u, 0u, 0u};
+    uint32_t urgent = 0u;                                     // bit q: vertex j0+q has an out-edge of delay 1
+    uint32_t rbeg[4] = {0u, 0u, 0u, 0u}, rdeg[4] = {0u, 0u, 0u, 0u};   // row start and out-degree of the thread's vertices (static)
+    auto ld4 = [&](const float *a, float (&x)[4]) {
+        const float4 v = *reinterpret_cast<const float4 *>(a + j0);
+        x[0] = v.x; x[1] = v.y; x[2] = v.z; x[3] = v.w;
+    };
+    auto st4 = [&](float *a, const float (&x)[4]) { *reinterpret_cast<float4 *>(a + j0) = make_float4(x[0], x[1], x[2], x[3]); };
+    if (mine) {
+        ld4(p.V, V); ld4(p.W, W); ld4(p.r, r);
+        if (p.any_alpha) ld4(p.p2, pp);
+        if (HH) { ld4(p.hm, gm); ld4(p.hh, gh); }
+        if (OBS) { ld4(p.c, c); ld4(p.acc, acc); }
+        if (BIAS) ld4(p.bias, U);
+        const uchar4 rf4 = *reinterpret_cast<const uchar4 *>(p.refr + j0), cl4 = *reinterpret_cast<const uchar4 *>(p.cls + j0);
+        refr[0] = rf4.x; refr[1] = rf4.y; refr[2] = rf4.z; refr[3] = rf4.w;
+        cl[0] = cl4.x; cl[1] = cl4.y; cl[2] = cl4.z; cl[3] = cl4.w;
+        const uchar4 md4 = *reinterpret_cast<const uchar4 *>(p.min_dly + j0);
+        urgent = (md4.x == 1u) | ((md4.y == 1u) << 1) | ((md4.z == 1u) << 2) | ((md4.w == 1u) << 3);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            rbeg[q] = p.row[j0 + q];
+            rdeg[q] = p.row[j0 + q + 1] - rbeg[q];
+        }
+    }
+    uint32_t slot = (uint32_t)(t0 % p.D), raster_row = (uint32_t)(t0 % p.raster_rows);
+    uint32_t in_frame = OBS ? (uint32_t)(t0 % p.obs_stride) : 0u;
+    uint64_t frame = OBS ? t0 / p.obs_stride : 0ull;
+    uint32_t n_spikes = 0u, n_kicks = 0u;
+    unsigned long long n_events = 0ull;
+    // bit q: vertex j0+q is kicked at step t (reading #12); drawn one step ahead, behind the barrier
+    auto draw_kicks = [&](const uint64_t t) -> uint32_t {
+        uint32_t k = 0u;
+        if (mine && p.any_drive) {
+            uint32_t x[4];
+            philox4x32_10(g, (uint32_t)t, (uint32_t)(t >> 32), kStreamDrive, p.seed_lo, p.seed_hi, x);
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+                if ((j0 + q) < p.N && x[q] < s_cls[cl[q]].drive_thr) k |= 1u << q;
+        }
+        return k;
+    };
+    // the edges of the warp's fired vertices (bits of `nib`) with delay == 1 (URGENT) or delay >= 2, lanes over each row
+    auto deliver = [&](const uint32_t nib, const bool urgent_pass) {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            uint32_t m = __ballot_sync(0xFFFFFFFFu, (nib >> q) & 1u);
+            while (m) {
+                const int src_lane = __ffs(m) - 1;
+                m &= m - 1u;
+                const uint32_t beg = __shfl_sync(0xFFFFFFFFu, rbeg[q], src_lane), deg = __shfl_sync(0xFFFFFFFFu, rdeg[q], src_lane);
+                const uint2 *__restrict__ edge = p.s_edge + beg;
+                const uint8_t *__restrict__ dly = p.s_dly + beg;
+                for (uint32_t x0 = 0u; x0 < deg; x0 += 128u) {          // four 32-edge blocks requested at once
+                    uint2 ev[4];
+                    uint32_t d[4];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const uint32_t x = x0 + 32u * u + lane;
+                        ev[u] = make_uint2(0u, 0u);
+                        d[u] = 0u;
+                        if (x < deg) {
+                            ev[u] = __ldg(edge + x);
+                            d[u] = p.packed ? ev[u].x >> 24 : (uint32_t)__ldg(dly + x);
+                        }
+                    }
+                    bool beyond = false;                                 // urgent pass: an edge with delay > 1 seen (rows are sorted)
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        if (d[u] == 0u) continue;
+                        if ((d[u] == 1u) != urgent_pass) { beyond = true; continue; }
+                        uint32_t s1 = slot + d[u];
+                        if (s1 >= p.D) s1 -= p.D;
+                        atomicAdd(p.ring + (size_t)s1 * p.Npad + (p.packed ? ev[u].x & 0xFFFFFFu : ev[u].x), (int32_t)ev[u].y);
+                    }
+                    if (urgent_pass && __any_sync(0xFFFFFFFFu, beyond)) break;
+                }
+                if (!urgent_pass && lane == 0u) n_events += (unsigned long long)deg;
+            }
+        }
+    };
+    uint32_t kicks = draw_kicks(t0);
+    for (uint32_t st = 0; st < n_steps; ++st) {
+        const uint64_t t = t0 + st;
+        uint32_t nib = 0u;
+        if (mine) {
+            int4 *slot_ptr = reinterpret_cast<int4 *>(p.ring + (size_t)slot * p.Npad + j0);
+            const int4 I4 = __ldcg(slot_ptr);                 // written by other SMs' REDs: read it where they landed (L2)
+            if ((I4.x | I4.y | I4.z | I4.w) != 0) *slot_ptr = make_int4(0, 0, 0, 0);
+            int32_t I[4] = {I4.x, I4.y, I4.z, I4.w};
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+                if ((kicks >> q) & 1u) { I[q] += s_cls[cl[q]].kick_fx; ++n_kicks; }
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const GnClassDev &k = s_cls[cl[q]];
+                const bool fired = ((HH && k.hh) ? vertex_step_hh<BIAS>(k, p.dt, I[q], U[q], V[q], W[q], r[q], refr[q], pp[q], gm[q], gh[q])
+                                                 : vertex_step<BIAS, true>(k, p.dt, I[q], U[q], V[q], W[q], r[q], refr[q], pp[q])) &&
+                                   (j0 + q) < p.N;
+                if (fired) nib |= 1u << q;
+                if (OBS) {
+                    c[q] = __fmaf_rn(p.keep_c, c[q], fired ? p.ca_jump : 0.0f);           // H_c
+                    acc[q] = __fadd_rn(acc[q], c[q]);
+                }
+            }
+        }
+        // a3: raster word (as gn_update_kernel)
+        uint32_t word = nib << (4u * (lane & 7u));
+        word |= __shfl_xor_sync(0xFFFFFFFFu, word, 1);
+        word |= __shfl_xor_sync(0xFFFFFFFFu, word, 2);
+        word |= __shfl_xor_sync(0xFFFFFFFFu, word, 4);
+        // a4, urgent part: delay-1 events land in the slot the next step reads.  Then ARRIVE at the step's barrier.
+        n_spikes += __popc(nib);
+        if (__any_sync(0xFFFFFFFFu, (nib & urgent) != 0u)) deliver(nib & urgent, true);
+        __threadfence();
+        __syncthreads();
+        if (threadIdx.x == 0) atomicAdd(sync, 1ull);
+        // a4, the rest, and the raster word: nothing the next step reads
+        if ((lane & 7u) == 0u && mine) p.raster[(size_t)raster_row * p.words_pad + (j0 >> 5)] = word;
+        if (__any_sync(0xFFFFFFFFu, nib != 0u)) deliver(nib, false);
+        // a5: camera frame (as gn_observe_kernel)
+        if (OBS && ++in_frame == p.obs_stride) {
+            float z[4] = {0.f, 0.f, 0.f, 0.f};
+            if (p.obs_sigma != 0.0f) {
+                uint32_t x[4];
+                philox4x32_10(g, (uint32_t)frame, (uint32_t)(frame >> 32), kStreamNoise, p.seed_lo, p.seed_hi, x);
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const float ua = __fmaf_rn((float)(x[2 * h] >> 9), 0x1p-23f, 0x1p-24f);
+                    const float ub2 = __fmul_rn((float)(x[2 * h + 1] >> 8), 0x1p-23f);
+                    const float rad = sqrtf(-2.0f * logf(ua));
+                    float sn, cs;
+                    sincospif(ub2, &sn, &cs);
+                    z[2 * h] = rad * cs;
+                    z[2 * h + 1] = rad * sn;
+                }
+            }
+            if (mine) {
+                float out[4];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) out[q] = p.obs_gain * (acc[q] * p.inv_stride) + p.obs_offset + p.obs_sigma * z[q];
+                *reinterpret_cast<float4 *>(p.trace + (size_t)(frame % p.trace_cap) * p.Npad + j0) = make_float4(out[0], out[1], out[2], out[3]);
+            }
+#pragma unroll
+            for (int q = 0; q < 4; ++q) acc[q] = 0.f;
+            in_frame = 0u;
+            ++frame;
+        }
+        kicks = draw_kicks(t + 1ull);
+        // WAIT: every CTA has arrived, so every delay-1 event of step t (and every event of the steps before) has landed
+        if (threadIdx.x == 0) {
+            const unsigned long long target = sync_base + (unsigned long long)(st + 1u) * gridDim.x;
+            long long c0 = 0;
+            for (uint32_t spins = 0; *reinterpret_cast<volatile unsigned long long *>(sync) < target; ++spins) {
+                if (spins == 1024u) c0 = clock64();
+                if (spins > 1024u && clock64() - c0 > 2000000000ll) break;
+            }
+            __threadfence();
+        }
+        __syncthreads();
+        if (++slot == p.D) slot = 0u;
+        if (++raster_row == p.raster_rows) raster_row = 0u;
+    }
+    if (mine) {
+        st4(p.V, V); st4(p.W, W); st4(p.r, r);
+        if (p.any_alpha) st4(p.p2, pp);
+        if (HH) { st4(p.hm, gm); st4(p.hh, gh); }
+        if (OBS) { st4(p.c, c); st4(p.acc, acc); }
+        *reinterpret_cast<uchar4 *>(p.refr + j0) = make_uchar4(refr[0], refr[1], refr[2], refr[3]);
+    }
+    n_kicks = __reduce_add_sync(0xFFFFFFFFu, n_kicks);
+    n_spikes = __reduce_add_sync(0xFFFFFFFFu, n_spikes);
+    if (lane == 0u) {
+        if (n_spikes) atomicAdd(&p.counters[1], (unsigned long long)n_spikes);
+        if (n_events) atomicAdd(&p.counters[2], n_events);
+        if (n_kicks) atomicAdd(&p.counters[3], (unsigned long long)n_kicks);
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) p.counters[0] = t0 + n_steps;
+}
+
 // ---- create-time kernels --------------------------------------------------------------------------------
 __global__ void gn_init_state_kernel(const GnDev p, GnCheck *chk)
 {
@@ -1146,6 +1356,45 @@ cudaError_t gnk_update(const GnDev &p, uint64_t t, bool has_bias, cudaStream_t s
     GN_UPD(false, false);
 #undef GN_UPD2
 #undef GN_UPD
+}
+
+typedef void (*PersistKernel)(const GnDev, const uint64_t, const uint32_t, unsigned long long *, const unsigned long long);
+
+static PersistKernel persist_kernel_for(const GnDev &p, bool has_bias)
+{
+    const bool obs = p.obs_stride != 0u;
+    if (p.any_hh) return obs ? (has_bias ? gn_persist_kernel<true, true, true> : gn_persist_kernel<true, false, true>)
+                             : (has_bias ? gn_persist_kernel<false, true, true> : gn_persist_kernel<false, false, true>);
+    return obs ? (has_bias ? gn_persist_kernel<true, true, false> : gn_persist_kernel<true, false, false>)
+               : (has_bias ? gn_persist_kernel<false, true, false> : gn_persist_kernel<false, false, false>);
+}
+
+// Can the whole grid of the persistent step driver be co-resident on this device (a cooperative launch needs it)?
+cudaError_t gnk_persist_ok(const GnDev &p, bool *ok)
+{
+    *ok = false;
+    int dev = 0, coop = 0, sms = 0, per_sm = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    // the variant with the largest footprint decides for all of them
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, gn_persist_kernel<true, true, true>, kUpdateThreads, 0);
+    if (e != cudaSuccess) { cudaGetLastError(); return cudaSuccess; }
+    *ok = coop && (uint64_t)ceil_div(p.Npad / kVertsPerThread, kUpdateThreads) <= (uint64_t)sms * (uint64_t)per_sm;
+    return cudaSuccess;
+}
+
+cudaError_t gnk_persist(const GnDev &p, uint64_t t0, uint32_t n_steps, bool has_bias, unsigned long long *sync,
+                        unsigned long long *sync_base, cudaStream_t st)
+{
+    GnDev pv = p;
+    uint64_t t = t0;
+    uint32_t n = n_steps;
+    unsigned long long base = *sync_base;
+    void *args[5] = {&pv, &t, &n, &sync, &base};
+    *sync_base += (unsigned long long)n_steps * ceil_div(p.Npad / kVertsPerThread, kUpdateThreads);   // where the counter ends
+    return cudaLaunchCooperativeKernel((const void *)persist_kernel_for(p, has_bias),
+                                       dim3(ceil_div(p.Npad / kVertsPerThread, kUpdateThreads)), dim3(kUpdateThreads), args, 0, st);
 }
 
 typedef void (*ResidentKernel)(const GnDev, const uint64_t, const uint32_t, const uint32_t);

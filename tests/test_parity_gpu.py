@@ -810,3 +810,24 @@ def test_hodgkin_huxley_state_within_tolerance_of_fp64(gn):
     rg = unpack_raster(gn.gn_read_raster(g, 0, steps + gate.pre), net.n_vertices)
     t_star, stats = gate.check(rg, o.raster_bool(0, steps + gate.pre), "CUDA Hodgkin-Huxley vs fp64 oracle")
     assert o.counters()["spikes"] > 100
+
+
+# ---- step drivers of ring mode: one cooperative launch per gn_step call, or one launch per step -------------------
+@pytest.mark.parametrize("persist", [True, False])
+@pytest.mark.parametrize("k,n,steps,chunk", [(3, 6_007, 1500, 500), (2, 3_000, 900, 300), (3, 100_000, 400, 137)])
+def test_ring_mode_step_drivers_agree(gn, monkeypatch, k, n, steps, chunk, persist):
+    """gn_persist_kernel (the whole call in one cooperative launch, state in registers, one grid barrier per step) and
+    the per-step FUSED update kernel (GN_NO_PERSIST set) give the oracle's results bit for bit, observation included,
+    also when a call ends inside a camera frame (chunk 137) and with a bias current."""
+    if not persist:
+        monkeypatch.setenv("GN_NO_PERSIST", "1")
+    net, cfg = make_config(k, n=n)
+    cfg = dict(cfg, obs_stride=25, obs_sigma=0.05)
+    bias = np.random.default_rng(k).uniform(0.0, 3.0, net.n_vertices).astype(np.float32) if k == 2 else None
+    g, o, _ = _run_exact(gn, net, cfg, steps, chunk, bias=bias, delivery_mode=gn.GN_DELIVER_RING, threads=8)
+    frames = steps // 25
+    np.testing.assert_allclose(gn.gn_observe(g, 0, frames).astype(np.float64), o.trace(0, frames), rtol=1e-6, atol=1e-5)
+    np.testing.assert_array_equal(gn.gn_read_state(g, gn.GN_CA).view(np.uint32), o.state(ob.CA).astype(np.float32).view(np.uint32))
+    _, launches = gn.gn_profile_read(g)
+    n_calls = -(-steps // chunk)
+    assert int(launches[4]) == (n_calls if persist else steps + frames)      # O(calls), not O(steps), runtime launches
