@@ -344,19 +344,19 @@ def main():
     resident = kn[1] == 0 and kn[0] < sim_steps
     names = ["gn_resident_kernel (a1-a5, one CTA or cluster per network)" if resident else
              "gn_update_kernel (a1-a3 + a4 fused)" if kn[1] == 0 else "gn_update_kernel (a1-a3)",
-             "gn_route_kernel (a4: routing + folding warps)" if queue_mode else "gn_deliver_kernel (a4)",
-             "gn_observe_kernel (a5)", "gn_fold_kernel (a4, read-back only)"]
+             "gn_log_kernel (a3 compaction + a4: spikes into the log)" if queue_mode else "gn_deliver_kernel (a4)",
+             "gn_observe_kernel (a5)", "gn_fold_kernel (a4: expansion of the log + ring reductions)"]
     p_events, p_spikes = cp1[2] - cp0[2], cp1[1] - cp0[1]
     # algorithmic bytes per launch: 17 B per event (+12 B per fired source) for the
-    # delivery kernel of either mode (queue mode: one launch per slot group routes the group's events and folds as
-    # many records of an earlier group)
+    # delivery of either mode (queue mode, per slot group: the logging kernel takes the 12 B per fired source, the fold
+    # kernel the 17 B per event of the group it expands)
     delivery_bytes = p_events * EVENT_BYTES + p_spikes * SOURCE_BYTES
     per_vertex = HH_BYTES_PER_VERTEX if args.model == "hh" else UPDATE_BYTES_PER_VERTEX
     kbytes = [N * (per_vertex + (UPDATE_BYTES_PER_VERTEX_OBS if obs else 0.0)) * (sim_steps / max(int(kn[0]), 1))
               + (delivery_bytes / max(int(kn[0]), 1) if kn[1] == 0 else 0.0),
-              delivery_bytes / max(int(kn[1]), 1),
+              (p_spikes * SOURCE_BYTES if queue_mode else delivery_bytes) / max(int(kn[1]), 1),
               N * 8.0,
-              p_events * 8.0 / max(int(kn[3]), 1)]
+              p_events * EVENT_BYTES / max(int(kn[3]), 1)]
     traffic_tab, traffic_src = measured_traffic()
     kernels = []
     for k in range(4):

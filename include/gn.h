@@ -105,22 +105,22 @@ typedef struct {
     uint64_t seed;                  /* key of the counter generator (drive stream 5, noise stream 6) */
     /* How eq. 30's sum reaches the ring (the RESULT is identical in every mode: integer adds commute). */
     uint32_t delivery_mode;         /* GN_DELIVER_AUTO (0), _RING, _QUEUE, _RESIDENT                   */
-    uint32_t queue_group;           /* queue mode: ring slots per event bucket, power of two in 1..16; */
-                                    /* 0 = default (4)                                                */
-    uint64_t queue_capacity;        /* queue mode: events one bucket holds before later ones fall     */
-                                    /* back to direct ring adds; 0 = default queue_group * ceil(E/16) */
+    uint32_t queue_group;           /* queue mode: ring slots per slot group, power of two in 1..16;  */
+                                    /* 0 = default (8)                                                */
+    uint64_t queue_capacity;        /* queue mode: spikes of one step the spike log holds; later ones */
+                                    /* are expanded on the spot (direct ring adds); 0 = default       */
+                                    /* max(1024, N / 16)                                              */
 } gn_config;
 
 /* delivery_mode.
  * RING: every event is one int32 reduction straight into ring[(t+delay) mod D][target], by a delivery kernel
  *   that runs beside the next step's update (best while the ring fits L2).
- * QUEUE: ring slots are taken queue_group at a time; an event due in a later group is appended, as an 8-byte
- *   {ring cell, weight} record, to that group's bucket, and a bucket is added ("folded") into its ring rows just
- *   before they are consumed, while those rows sit in L2 (best when the ring is >> L2: sequential appends instead
- *   of a 32-byte DRAM sector read-modify-write per event).  Routing runs once per group of steps; events due
- *   within two groups are sent by the update kernel itself.  Needs D to be a multiple of the group, D / group <= 32
- *   and every out-degree <= 65535; where that fails QUEUE is refused (GN_E_INVALID_ARG for the degree) or, for the
- *   depth conditions and under AUTO, the ring path is used: results are identical either way.
+ * QUEUE: ring slots are taken queue_group at a time (a slot group).  A spike is entered into a spike log -- per group
+ *   offset, where in its delay-sorted row the events due that many groups ahead begin -- and its events are expanded
+ *   and added ("folded") into the ring group by group, each group just before it is consumed, while the group's rows
+ *   sit in L2 (best when the ring is >> L2: no 32-byte DRAM sector read-modify-write per event, and nothing per event
+ *   is written or read back).  Logging and folding run once per group of steps; events due within two groups are sent
+ *   by the update kernel itself.  Needs ring_slots to be a multiple of the group (else a smaller group is taken).
  * RESIDENT: every network (n_networks >= 1) lives in ONE CTA -- or, above 1,024 vertices, one thread-block cluster of
  *   up to 16 CTAs -- for a whole gn_step call: vertex state in registers, the network's delay ring in (distributed)
  *   shared memory, delivery by shared-memory integer atomics, one barrier per step and no per-step kernel launch
@@ -186,9 +186,10 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
 
 /* Advance n_steps time steps (eq. 5, called in a loop).  Per step one update kernel: ring-slot
  * read-and-clear + drive + vertex update + spike detection + raster word + the events due soonest; then the rest of the
- * step's event delivery -- ring mode: a delivery kernel per step (small networks: inside the update kernel); queue mode:
- * ONE routing + folding kernel per group of queue_group steps; resident mode: the whole call is one launch per network
- * batch -- and at frame boundaries the observation kernel.  Asynchronous: no host synchronisation inside. */
+ * step's event delivery -- ring mode: a delivery kernel per step (small networks: inside the update kernel, or the whole
+ * call as one cooperative launch); queue mode: one logging and one folding kernel per group of queue_group steps;
+ * resident mode: the whole call is one launch per network batch -- and at frame boundaries the observation kernel.
+ * Asynchronous: no host synchronisation inside. */
 int gn_step(gn_net *net, uint64_t n_steps);
 
 /* Copy state out.  dst_bytes must be at least the size listed at the enum.  dst_is_device != 0:
@@ -227,8 +228,8 @@ int gn_debug_words(void *cuda_stream, uint64_t seed, uint32_t stream_id, uint64_
  * few hundred steps to collect them: a measuring mode, never the mode a throughput number is taken in.  A run
  * of consecutive launches of one kernel (queue mode: the updates of one slot group) is timed as a whole.
  * gn_profile_read: ms[k] = summed device time, launches[k] = launch count of kernel k since the last
- * gn_profile(net, 1): k = 0 update (a1-a3), 1 delivery (a4: ring reductions, or queue routing once per group),
- * 2 observation (a5), 3 bucket fold (a4, queue mode).  launches[4] is the total number of kernels this
+ * gn_profile(net, 1): k = 0 update (a1-a3), 1 delivery (a4: ring reductions; queue mode: spike logging, once per group),
+ * 2 observation (a5), 3 fold (a4, queue mode: expansion of the log into the ring, once per group).  launches[4] is the total number of kernels this
  * handle has launched since gn_create, profiling or not. */
 int gn_profile(gn_net *net, int enable);
 int gn_profile_read(gn_net *net, double ms[4], uint64_t launches[5]);

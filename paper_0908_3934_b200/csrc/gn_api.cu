@@ -18,7 +18,7 @@ thread_local char g_create_error[256] = "";
 
 struct Layout {
     size_t V, W, r, p2, hm, hh, c, acc, bias, refr, cls, ring, row, tgt, wfx, dly, counters, q_count;
-    size_t s_edge, s_dly, min_dly, q_seg, queue;
+    size_t s_edge, s_dly, min_dly, q_seg, spk_log;
     size_t raster, trace, scratch_row64, scratch_abs, scratch_pos, scratch_net, scratch_chk, total;
 };
 
@@ -46,35 +46,31 @@ int check_config(const gn_config *cfg, char *err, size_t errn)
 // Groups beyond the current one whose events the update kernel delivers itself (GnDev::q_window).
 static const uint32_t kQueueWindow = 2u;
 
-// Resolved delivery plan: mode, log2(slots per bucket), buckets, records per bucket.
+// Resolved delivery plan of queue mode: log2(slots per group), groups per lap, log arrays, spikes per step the log holds.
 struct QueuePlan {
     bool on;
-    uint32_t q_log, q_nb;
-    uint64_t q_cap;
+    uint32_t q_log, q_nb, arrays;
+    uint32_t log_cap;
 };
 
 QueuePlan make_plan(const gn_config *cfg)
 {
     const uint64_t N = cfg->n_vertices, Npad = (N + 127) / 128 * 128, E = cfg->n_edges, D = cfg->ring_slots;
     QueuePlan q{};
-    uint32_t group = cfg->queue_group ? cfg->queue_group : 4u;
-    // cell offsets are 32-bit; the ring depth must be a whole number of groups
-    while (group > 1 && (Npad * group > 0xFFFFFFFFull || D % group != 0)) group >>= 1;
-    // one lane of a routing warp per bucket: deeper rings take larger groups when the caller left the choice open
-    while (cfg->queue_group == 0 && D / group > 32 && group < 16 && D % (group * 2) == 0 && Npad * group * 2 <= 0xFFFFFFFFull)
-        group <<= 1;
+    uint32_t group = cfg->queue_group ? cfg->queue_group : 8u;
+    while (group > 1 && D % group != 0) group >>= 1;      // the ring depth must be a whole number of groups
     q.on = cfg->delivery_mode == GN_DELIVER_QUEUE ||
            (cfg->delivery_mode == GN_DELIVER_AUTO && D >= 32 && D * Npad * 4 > (48ull << 20));
-    if (E == 0 || D / group > 32) q.on = false;      // gn_route_kernel: one lane per bucket
+    if (E == 0) q.on = false;
     q.q_log = 0;
     while ((1u << q.q_log) < group) q.q_log++;
-    q.q_nb = (uint32_t)((D + group - 1) / group);
-    uint64_t cap = cfg->queue_capacity ? cfg->queue_capacity : (uint64_t)group * ((E + 15) / 16);
-    if (cap < 64) cap = 64;
-    if (cap > 0xFFFFFF00ull) cap = 0xFFFFFF00ull;    // record positions are 32-bit
-    if (cap * q.q_nb > 0xFFFFFF00ull) cap = 0xFFFFFF00ull / q.q_nb;     // record indices are 32-bit
-    q.q_cap = cap / 32 * 32;
-    if (q.q_cap < 32) q.q_cap = 32;
+    q.q_nb = (uint32_t)(D / group);
+    q.arrays = q.q_nb > kQueueWindow ? q.q_nb - kQueueWindow + 1u : 0u;   // boundaries of group offsets W+1 .. nb (+ the row's end)
+    uint64_t cap = cfg->queue_capacity ? cfg->queue_capacity : (N + 15) / 16;
+    if (cfg->queue_capacity == 0 && cap < 1024) cap = 1024;
+    if (cap > Npad) cap = Npad;                           // a step has at most N spikes
+    if (cap > (1ull << 23)) cap = 1ull << 23;             // 255 steps x log_cap entries are indexed in 32 bits
+    q.log_cap = (uint32_t)((cap + 31) / 32 * 32);
     return q;
 }
 
@@ -94,7 +90,7 @@ Layout make_layout(const gn_config *cfg)
     L.row = take((Npad + 1) * 4); L.tgt = take(E * 4); L.wfx = take(E * 4); L.dly = take(E);
     L.counters = take(32);
     const QueuePlan qp = make_plan(cfg);
-    L.q_count = take(256 * 8);
+    L.q_count = take(256 * 8);       // +0: the persistent step driver's barrier counter; +64: spikes logged per step slot
     {
         size_t rows = cfg->raster_capacity_steps, need_rows = qp.on ? (size_t)(kQueueWindow + 1u) << qp.q_log : 2;
         if (rows < need_rows) rows = need_rows;
@@ -104,7 +100,7 @@ Layout make_layout(const gn_config *cfg)
     L.min_dly = take(Npad);
     L.s_edge = take(E * 8); L.s_dly = take(E);   // every row again, sorted by delay
     L.q_seg = take(qp.on ? N * D * 2 : 0);
-    L.queue = take(qp.on ? (size_t)qp.q_nb * qp.q_cap * 8 : 0);
+    L.spk_log = take(qp.on && qp.arrays >= 2 ? D * qp.arrays * (size_t)qp.log_cap * 4 : 0);
     L.scratch_row64 = take((N + 1) * 8); L.scratch_abs = take(N * 8);
     L.scratch_pos = take(N * cfg->dim * 4); L.scratch_net = take(((size_t)cfg->n_networks + 1) * 4);
     L.scratch_chk = take(sizeof(GnCheck));
@@ -124,7 +120,8 @@ struct gn_net {
     uint64_t t;          // steps enqueued so far
     uint64_t t_origin;   // first step simulated by this handle (0, or the t a checkpoint was restored at)
     unsigned long long sync_base;   // persistent step driver: value of its barrier counter when the next launch starts
-    uint64_t routed_upto; // queue mode: steps < routed_upto have had their queued events routed
+    uint64_t routed_upto; // queue mode: steps < routed_upto have been entered into the spike log
+    uint64_t flushed_upto; // queue mode: every event of steps < flushed_upto is in the ring already (a read-back expanded them)
     // delivery of step t overlaps the update of step t+1 (see gn_step): side streams and their fences
     cudaStream_t s_deliver;
     cudaEvent_t ev_update, ev_deliver[2], ev_fold[4];
@@ -235,6 +232,7 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
     net->t = 0;
     net->t_origin = 0;
     net->routed_upto = 0;
+    net->flushed_upto = 0;
     net->sync_base = 0;
     net->s_deliver = nullptr;
     net->ev_update = net->ev_deliver[0] = net->ev_deliver[1] = net->ev_fold[0] = net->ev_fold[1] = net->ev_fold[2] = net->ev_fold[3] = nullptr;
@@ -280,14 +278,15 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
         if (d.raster_rows < need_rows) d.raster_rows = need_rows;
     }
     d.queue_mode = qp.on ? 1u : 0u;
-    d.q_log = qp.q_log; d.q_nb = qp.q_nb; d.q_cap = qp.q_cap;
-    d.q_count = (unsigned long long *)(ws + L.q_count);
+    d.q_log = qp.q_log; d.q_nb = qp.q_nb; d.q_arrays = qp.arrays; d.log_cap = qp.log_cap;
+    d.grid_sync = (unsigned long long *)(ws + L.q_count);
+    d.log_n = (uint32_t *)(ws + L.q_count + 64);
     d.s_edge = (uint2 *)(ws + L.s_edge); d.s_dly = ws + L.s_dly; d.min_dly = ws + L.min_dly;
     d.packed = Npad <= (1u << 24) ? 1u : 0u;
     d.q_window = kQueueWindow;
     if (qp.on) {
         d.q_seg = (uint16_t *)(ws + L.q_seg);
-        d.queue = (uint2 *)(ws + L.queue);
+        d.spk_log = (uint32_t *)(ws + L.spk_log);
     }
     d.trace = cfg->obs_stride ? (float *)(ws + L.trace) : nullptr;
     for (uint32_t k = 0; k < cfg->n_classes; ++k) {
@@ -474,13 +473,6 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
                        : chk.cross_net ? "edge crosses two networks"
                                        : "weight is NaN or outside the int32 fixed-point range");
     }
-    if (chk.big_degree && d.queue_mode) {      // the 16-bit segment table cannot describe this graph
-        if (cfg->delivery_mode == GN_DELIVER_QUEUE) {
-            delete net;
-            return set_err(nullptr, GN_E_INVALID_ARG, "GN_DELIVER_QUEUE needs every out-degree <= 65535");
-        }
-        d.queue_mode = 0u;     // AUTO: same results through the ring path
-    }
     if (chk.overflow) {
         delete net;
         return set_err(nullptr, GN_E_OVERFLOW_RISK, "some target's sum |w_fx| + |kick_fx| exceeds 2^31 - 1");
@@ -554,23 +546,54 @@ static int join_streams(gn_net *net)
 // with delay 1 are sent by update(t-1) itself, so the earliest slot deliver(t-1) writes is t+1, and deliver(t)
 // runs on a side stream beside update(t+1).
 //
-// Queue mode.  Steps come in groups of G = 2^q_log (one bucket = the ring rows of one group); W = q_window = 2.
-// update(t), t in group h, sends every event due in groups h .. h+W itself.  After the last update of group h ONE
-// gn_route_kernel runs on the side stream, beside the updates of group h+1:
-//   its routing warps append the rest of the group's events to buckets h+W+1 .. and (wrapped) h;
-//   its folding warps add bucket h+W -- complete since route(h-1), the previous launch on that stream -- into
-//   the ring rows of group h+W; the bucket's count is zeroed after the kernel.
-// update(first step of h+W) waits for that launch: a whole group of slack.  The raster rows a launch reads are
-// overwritten W+1 groups later, after the next launch on the side stream.
+// Queue mode.  Steps come in groups of G = 2^q_log (the ring rows of one group are folded together); W = q_window.
+// update(t), t in group h, sends every event due in groups h .. h+W itself.  After the last update of group h two
+// kernels go to the side stream, beside the updates of group h+1 (and beside each other):
+//   gn_log_kernel enters the spikes of group h's steps into the spike log;
+//   gn_fold_kernel expands, out of the log of groups h+W-nb .. h-1 (complete since the previous launches on that
+//   stream), the events due in group h+W into that group's ring rows.
+// update(first step of h+W) waits for that launch: W-1 groups of slack.  The raster rows a launch reads are
+// overwritten W+1 groups later, after the next launches on the side stream.
 // In profiling mode everything runs on the caller's stream in that order, so per-kernel times are clean.
-static int route_pending(gn_net *net, cudaStream_t st, bool prof, uint32_t fold_bucket)
+static int zero_log_counts(gn_net *net, uint64_t t0, uint64_t t1, cudaStream_t st)
 {
     const GnDev &d = net->dev;
-    if (!d.queue_mode || net->routed_upto >= net->t) return GN_OK;
+    const uint32_t s0 = (uint32_t)(t0 % d.D), n = (uint32_t)(t1 - t0);
+    const uint32_t first = n < d.D - s0 ? n : d.D - s0;
+    GN_CUDA(net, cudaMemsetAsync(d.log_n + s0, 0, (size_t)first * 4, st));
+    if (first < n) GN_CUDA(net, cudaMemsetAsync(d.log_n, 0, (size_t)(n - first) * 4, st));
+    return GN_OK;
+}
+
+// Logs the steps not yet logged (all inside one group) and, when g_fold != ~0, folds slot group g_fold out of the log.
+static int route_pending(gn_net *net, cudaStream_t st, bool prof, uint64_t g_fold)
+{
+    const GnDev &d = net->dev;
+    if (!d.queue_mode) return GN_OK;
+    const uint32_t n_batch = (uint32_t)(net->t - net->routed_upto);
+    uint64_t t_win = 0;
+    uint32_t n_win = 0;
+    if (g_fold != ~0ull && d.q_arrays >= 2u) {          // steps of groups g-nb .. g-W-1 that no read-back has expanded yet
+        const uint64_t lo_g = g_fold >= d.q_nb ? g_fold - d.q_nb : 0ull;
+        const uint64_t hi = g_fold >= d.q_window ? (g_fold - d.q_window) << d.q_log : 0ull;
+        uint64_t lo = lo_g << d.q_log;
+        if (lo < net->flushed_upto) lo = net->flushed_upto;
+        const uint64_t hi_c = hi < net->routed_upto ? hi : net->routed_upto;
+        if (hi_c > lo) { t_win = lo; n_win = (uint32_t)(hi_c - lo); }
+    }
+    if (n_batch == 0 && n_win == 0) return GN_OK;
     int rc;
-    if (prof && (rc = prof_mark(net, 1))) return rc;
-    GN_CUDA(net, gnk_route(d, net->routed_upto, (uint32_t)(net->t - net->routed_upto), fold_bucket, st));
-    net->launches++;
+    if (n_batch) {
+        if ((rc = zero_log_counts(net, net->routed_upto, net->t, st))) return rc;
+        if (prof && (rc = prof_mark(net, 1))) return rc;
+        GN_CUDA(net, gnk_log(d, net->routed_upto, n_batch, st));
+        net->launches++;
+    }
+    if (n_win) {
+        if (prof && (rc = prof_mark(net, 3))) return rc;
+        GN_CUDA(net, gnk_fold(d, t_win, n_win, g_fold, n_batch != 0 && !prof, st));
+        net->launches++;
+    }
     net->routed_upto = net->t;
     return GN_OK;
 }
@@ -606,8 +629,7 @@ int gn_step(gn_net *net, uint64_t n_steps)
             const uint64_t n = left > 0x40000000ull ? 0x40000000ull : left;
             int rc;
             if (net->profile && (rc = prof_mark(net, 0))) return rc;
-            // the barrier counter lives in the (otherwise unused in ring mode) bucket-count words, zeroed at create
-            GN_CUDA(net, gnk_persist(d, net->t, (uint32_t)n, net->has_bias, d.q_count, &net->sync_base, net->stream));
+            GN_CUDA(net, gnk_persist(d, net->t, (uint32_t)n, net->has_bias, d.grid_sync, &net->sync_base, net->stream));
             net->launches++;
             net->t += n;
             left -= n;
@@ -649,9 +671,7 @@ int gn_step(gn_net *net, uint64_t n_steps)
             if (!prof) GN_CUDA(net, cudaEventRecord(net->ev_deliver[t & 1ull], s_del));
             net->fences_pending = !prof;
         } else if (group_end) {
-            const uint32_t b_fold = (((uint32_t)(t % d.D) >> d.q_log) + d.q_window) % d.q_nb;
-            if ((rc = route_pending(net, s_del, prof, b_fold))) return rc;
-            GN_CUDA(net, cudaMemsetAsync(d.q_count + b_fold, 0, 8, s_del));             // the bucket is empty again
+            if ((rc = route_pending(net, s_del, prof, t / G + d.q_window))) return rc;
             if (!prof) GN_CUDA(net, cudaEventRecord(net->ev_fold[(t / G + d.q_window) & 3ull], s_del));
             net->fences_pending = !prof;
         }
@@ -669,17 +689,22 @@ int gn_step(gn_net *net, uint64_t n_steps)
     return join_streams(net);
 }
 
-// Spikes and delivered events are counted, and queued events become visible in the ring, only once the
-// routing of the steps since the last group boundary has run: readers of counters and ring call this.
+// Spikes and delivered events are counted once their step is logged, and logged events reach the ring only when their
+// slot group is folded: readers of counters and ring call this.  fold_too: every event of every completed step goes
+// into the ring now (what direct delivery would hold), and the log is marked consumed up to here.
 static int flush_delivery(gn_net *net, bool fold_too)
 {
     const GnDev &d = net->dev;
     int rc = join_streams(net);
     if (rc) return rc;
-    if ((rc = route_pending(net, net->stream, false, 0xFFFFFFFFu))) return rc;
-    if (fold_too && d.queue_mode) {   // pending records are deferred ring adds: apply them all (a no-op for the results)
-        for (uint32_t b = 0; b < d.q_nb; ++b) GN_CUDA(net, gnk_fold(d, b, net->stream));
-        GN_CUDA(net, cudaMemsetAsync(d.q_count, 0, (size_t)d.q_nb * 8, net->stream));
+    if ((rc = route_pending(net, net->stream, false, ~0ull))) return rc;
+    if (fold_too && d.queue_mode && d.q_arrays >= 2u && net->flushed_upto < net->t) {
+        // groups up to (h-1)+W were folded by the regular launches (h = group of the next step); the later ones, as far
+        // as a logged event can reach (nb groups ahead), are folded here for the steps done so far
+        const uint64_t h = net->t >> d.q_log;
+        for (uint64_t g = h + d.q_window; g <= h + d.q_nb; ++g)
+            if ((rc = route_pending(net, net->stream, false, g))) return rc;
+        net->flushed_upto = net->t;
     }
     return GN_OK;
 }
@@ -814,6 +839,7 @@ int gn_write_state(gn_net *net, int which, const void *src, size_t src_bytes, in
         GN_CUDA(net, cudaStreamSynchronize(net->stream));
         net->t = c[0];
         net->routed_upto = c[0];
+        net->flushed_upto = c[0];
         net->t_origin = c[0];
         return GN_OK;
     }

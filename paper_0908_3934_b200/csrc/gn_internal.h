@@ -59,10 +59,10 @@ struct GnDev {
     uint32_t *tgt;           // [E]
     int32_t *wfx;            // [E]
     uint8_t *dly;            // [E]
-    // queue mode: rows re-sorted by delay, and one event bucket per group of
-    // 2^q_log ring slots
+    // queue mode: ring slots are taken 2^q_log at a time (a slot GROUP); a spike's events due more than
+    // q_window groups ahead are not expanded when it fires but when the group they land in is about to be consumed
     uint32_t queue_mode;     // 0 ring, 1 queue
-    uint32_t q_log, q_nb;    // slots per bucket = 1 << q_log; buckets = ceil(D / 2^q_log)
+    uint32_t q_log, q_nb;    // slots per group = 1 << q_log; groups per ring lap = D / 2^q_log
     uint2 *s_edge;           // [E] the CSR rows again, each sorted by delay: {target, w_fx}; when `packed`
                              //     (Npad <= 2^24) the delay also sits in the target word's top byte
     uint8_t *s_dly;          // [E] delay of s_edge[e]
@@ -78,11 +78,17 @@ struct GnDev {
     uint32_t res_smem;       // dynamic shared memory: ring [D][res_threads] + drive words
     const uint32_t *net_off; // [n_networks + 1] first vertex of every network
     uint32_t q_window;       // queue mode: groups ahead of the current one whose events the update kernel sends itself
-    uint16_t *q_seg;         // [N][2^q_log][q_nb] segment boundaries of every delay-sorted row (gn_route_kernel)
-    uint2 *queue;            // [q_nb][q_cap] records {cell offset inside the bucket's ring rows, w_fx}
-    unsigned long long q_cap;
-    unsigned long long *q_count;   // [q_nb] records appended (may exceed q_cap: the excess went direct)
+    uint16_t *q_seg;         // [N][2^q_log][q_nb] segment boundaries of every delay-sorted row (rows of more than 65,535
+                             //     edges have no entry: their boundaries are searched for)
+    // the spike log: for the spike at position i of step t (slot t mod D) and every group offset j = q_window+1 ..
+    // q_nb+1, the index of the first edge of its row due j groups ahead, spk_log[((t mod D) * q_arrays + j-q_window-1)
+    // * log_cap + i]; the events due j groups ahead are edges [entry j, entry j+1)
+    uint32_t *spk_log;
+    uint32_t q_arrays;       // q_nb - q_window + 1 (0 or 1: nothing is ever logged)
+    uint32_t log_cap;        // spikes of one step the log holds; later ones are delivered on the spot
+    uint32_t *log_n;         // [D] spikes of step (slot) logged or delivered on the spot (may exceed log_cap)
     unsigned long long *counters;   // steps, spikes, delivered events, kicks
+    unsigned long long *grid_sync;  // the persistent step driver's barrier counter (it only grows)
     uint32_t *raster;        // [raster_rows][words_pad]; row t % raster_rows is step t's spike list
     uint32_t raster_rows;    // max(raster_cap, 2): the delivery kernels read the current row even when none is kept
     float *trace;            // [trace_cap][Npad]
@@ -92,16 +98,18 @@ struct GnDev {
 // Flags written by the create-time validation kernels.
 struct GnCheck {
     uint32_t bad_row, bad_target, bad_delay, bad_class, bad_weight, cross_net, overflow;
-    uint32_t big_degree;     // some out-degree > 65535: the 16-bit segment table of queue mode cannot hold it
     uint32_t bad_position;   // a NaN / infinite coordinate reached eq. 25
 };
 
 // ---- launchers (gn_kernels.cu).  All asynchronous on `st`; return the launch error. ----
 cudaError_t gnk_update(const GnDev &p, uint64_t t, bool has_bias, cudaStream_t st);
 cudaError_t gnk_deliver(const GnDev &p, uint64_t t, cudaStream_t st);
-// fold_bucket: the bucket the kernel's folding warps add into the ring beside the routing; 0xFFFFFFFF = none
-cudaError_t gnk_route(const GnDev &p, uint64_t t0, uint32_t n_batch, uint32_t fold_bucket, cudaStream_t st);
-cudaError_t gnk_fold(const GnDev &p, uint32_t bucket, cudaStream_t st);
+// Queue mode.  gnk_log: the spikes of steps t0 .. t0+n_batch-1 (one slot group at most) enter the spike log.
+// gnk_fold: for the n_win steps starting at step t_win, the log entries due in absolute slot group g_fold are expanded and
+// added into that group's ring rows; beside_previous: it may start while the kernel in front of it in the stream is
+// still running (the logging kernel of the same group end, which it does not depend on).
+cudaError_t gnk_log(const GnDev &p, uint64_t t0, uint32_t n_batch, cudaStream_t st);
+cudaError_t gnk_fold(const GnDev &p, uint64_t t_win, uint32_t n_win, uint64_t g_fold, bool beside_previous, cudaStream_t st);
 cudaError_t gnk_sort_rows(const GnDev &p, GnCheck *chk, cudaStream_t st);
 cudaError_t gnk_observe(const GnDev &p, uint64_t frame, cudaStream_t st);
 cudaError_t gnk_resident(const GnDev &p, uint64_t t0, uint32_t n_steps, bool has_bias, bool raster_on, cudaStream_t st);

@@ -2,7 +2,9 @@
 //
 //   gn_update_kernel   ring-slot read-and-clear + drive + Izhikevich/PSC/calcium update +
 //                      spike detection, raster bits and ballot/popc compaction
-//   gn_deliver_kernel  warp-per-active-source CSR expansion, int32 RED into the delay ring  (a4)
+//   gn_deliver_kernel  warp-per-active-source CSR expansion, int32 RED into the delay ring  (a4, ring mode)
+//   gn_log_kernel, gn_fold_kernel   a4 when the ring is >> L2: spikes are logged, and expanded slot group by slot group
+//   gn_resident_kernel / gn_persist_kernel   a1-a5 with no per-step launch (small networks)
 //   gn_observe_kernel  frame mean -> gain/offset + Gaussian noise -> trace row              (a5)
 //   create-time kernels: row conversion, weight quantisation, eq. 25 delays, validation.
 //
@@ -11,6 +13,8 @@
 // CPU oracle.  Delivery and the drive decision are integer; atomics are order-independent.
 // Paper line numbers refer to /root/reference/PAPER.md.
 #include <cooperative_groups.h>
+
+#include <stdlib.h>
 
 #include <utility>
 
@@ -24,7 +28,6 @@ constexpr int kUpdateThreads = 256;          // 8 warps x 128 vertices = 1024 ve
 constexpr int kVertsPerThread = 4;           // one 128-bit load per SoA array
 constexpr int kDeliverThreads = 256;
 constexpr uint32_t kStreamDrive = 5, kStreamNoise = 6;
-constexpr uint32_t kNoBucket = 0xFFFFFFFFu;
 
 // ---- Philox4x32-10 (Salmon et al., SC'11), from its published description -------------------
 __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
@@ -331,17 +334,8 @@ gn_update_kernel(const GnDev p, const uint64_t t, const uint32_t slot, const uin
 // source list with a popc prefix scan: no global list, no global cursor.  Returns the number of sources.
 constexpr uint32_t kMaxChunkWords = 128;                 // 4096 vertices per CTA at most
 
-// CTA barrier over the first THREADS threads only: BAR = 0 is __syncthreads (the whole CTA), BAR > 0 a named barrier,
-// so that warps beyond THREADS (the folding warps of gn_route_kernel) never take part.
-template <int THREADS, int BAR>
-__device__ __forceinline__ void part_sync()
-{
-    if (BAR == 0) __syncthreads();
-    else asm volatile("bar.sync %0, %1;" ::"n"(BAR), "n"(THREADS) : "memory");
-}
-
 // CTA-wide exclusive prefix sum of one count per thread; returns the CTA total (CTA-uniform), `off` = this thread's offset.
-template <int THREADS, int BAR = 0>
+template <int THREADS>
 __device__ __forceinline__ uint32_t gather_scan(const uint32_t pc, uint32_t *s_wsum, uint32_t &off)
 {
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
@@ -351,9 +345,9 @@ __device__ __forceinline__ uint32_t gather_scan(const uint32_t pc, uint32_t *s_w
         const uint32_t v = __shfl_up_sync(0xFFFFFFFFu, incl, o);
         if (lane >= (uint32_t)o) incl += v;
     }
-    part_sync<THREADS, BAR>();                             // s_wsum may still be read from the previous scan
+    __syncthreads();                                       // s_wsum may still be read from the previous scan
     if (lane == 31u) s_wsum[warp] = incl;
-    part_sync<THREADS, BAR>();
+    __syncthreads();
     uint32_t total = 0u;
     off = incl - pc;
 #pragma unroll
@@ -427,294 +421,329 @@ gn_deliver_kernel(const GnDev p, const uint32_t slot_t, const uint32_t raster_ro
     if (threadIdx.x == 0) atomicAdd(&p.counters[1], (unsigned long long)n);
 }
 
-// ---- a4, queue mode: routing -----------------------------------------------------------------------------
-// When the ring is far larger than L2 every direct reduction costs a 32-byte DRAM sector fetch and a
-// write-back.  Queue mode defers the add: an event due in ring slot s is appended as the 8-byte record
-// {cell offset, w_fx} to the bucket of slot group s >> q_log; gn_fold_kernel adds a whole bucket into its
-// 2^q_log ring rows just before the first of them is consumed, when those rows sit in L2.  Integer adds
-// commute, so ring contents at every consumption are identical to direct delivery (eq. 30).
+// ---- a4, queue mode: deferred expansion ------------------------------------------------------------------
+// When the ring is far larger than L2 a direct reduction costs a 32-byte DRAM sector fetch and a write-back per
+// event.  Queue mode defers the EXPANSION of a spike instead: ring slots are taken G = 2^q_log at a time (a slot
+// group; nb = D / G groups per lap), and the events of a spike are added to the ring group by group, each group
+// just before it is consumed, when its G rows sit in L2.  Integer adds commute, so the ring word a vertex consumes
+// holds exactly what direct delivery would have put there (eq. 30).
 //
-// Rows are sorted by delay at create time, so the events of one source that share a bucket are one
-// contiguous SEGMENT of its row.  With G = 2^q_log slots per bucket, nb = D / G buckets and the slot
-// pointer at g_cur * G + r, a row splits, in delay order, into
-//     segment 0       delays [1, 2G - r)                slots of the current and of the NEXT group (whose bucket is
-//                                                       being folded while this group is consumed): DIRECT to the ring
-//     segment k       delays [(k+1)G - r, (k+2)G - r)   bucket (g_cur + 1 + k) mod nb,   k = 1 .. nb-2
-//     segment nb-1    delays [D - r, D)                 bucket g_cur (wrapped: consumed on the next lap)
-// (delay-1 events were already sent by the update kernel and become zero-weight records here.)
-// The segment boundaries (edge positions inside the row) depend only on r and are tabulated per source at
-// create time: q_seg[(src * G + r) * nb + k] = #edges of src with delay < (k+1)G - r, so segment k of a row
-// is edge positions [q_seg[k], q_seg[k+1]) with q_seg[nb] = out-degree.  Lane k of a warp owns segment k
-// (nb <= 32), so routing needs no search and two CTA barriers per step whatever the number of sources:
-//   A  every warp walks its share of the CTA's sources and sums, per lane, the segment sizes;
-//   B  warp 0 lays the warps' totals out back to back per bucket and reserves the space with ONE global
-//      atomic per bucket (a CTA that would overflow a bucket delivers those events directly instead);
-//   C  every warp walks its sources again (boundaries now come from L1/L2), keeps a running offset per
-//      segment in the owning lane, and each edge becomes a record whose position is
-//      [warp base + running offset - segment start](segment, by shuffle) + edge position.
+// Rows are sorted by delay at create time, so the events of a spike at step t (r = t mod G) that land j groups
+// ahead -- delays [jG - r, (j+1)G - r) -- are one contiguous SEGMENT of its row, and the segment boundaries depend
+// only on r: q_seg[(src * G + r) * nb + j-1] = #edges of src with delay < jG - r (create time).
+//     j = 0 .. W            (W = q_window) sent by the update kernel itself when the vertex fires
+//     j = W+1 .. nb         logged: the spike's entry in log array j-W-1 is the (absolute) index of the segment's first
+//                           edge, array j-W its end; j = nb is the wrapped tail (r + delay >= D: the group's own rows,
+//                           consumed on the next lap)
+// One launch per slot group h, after the group's last update, beside the updates of group h+1:
+//   LOGGING CTAs  compact the raster rows of the group's steps (a3: popc prefix, no global list), reserve log
+//                 positions with one atomic per step and CTA, and write nb-W+1 words per spike (a spike beyond the
+//                 log's capacity is expanded on the spot, straight into the ring);
+//   FOLDING CTAs  take group g = h+W, due to be consumed one group later: for every step of groups g-nb .. g-W-1
+//                 (all logged by earlier launches) and every spike of it, the segment due in g -- two coalesced log
+//                 reads -- is expanded: one 8-byte edge load and one int32 RED per event into rows that stay in L2.
+// No per-event record is written or read back, no per-event reservation: per event DRAM moves the 8-byte edge once
+// (in segments of ~G/D of a row) plus ~8/segment-length bytes of log.
 constexpr int kRouteThreads = 256;
 constexpr int kRouteWarps = kRouteThreads / 32;
-constexpr int kRouteUnroll = 8;                         // 8 x 32 edges of a row in flight per warp
+constexpr uint32_t kMaxWindow = 256;                    // steps one fold looks back over: (nb - W) G < D <= 255
+constexpr int kFoldUnroll = 4;                          // rounds of edge loads in flight per folding warp
+constexpr int kFoldCtasPerSm = 5;                       // folding CTAs per SM (persistent)
 
-// Lane k owns the events due j = k + W groups after the current one (W = q_window groups are the update kernel's;
-// k = 1 .. nb-W).  Its segment of a row starts at table entry i = k + W - 1 (#edges with delay < (i+1)G - r) and ends
-// at entry i + 1 (the out-degree past the table's end): lo from the lane's own load, hi by a shuffle from lane k + 1.
-constexpr uint32_t kRouteListCap = 4096;                // sources one A/B/C round of a CTA handles
-constexpr uint32_t kMaxBatch = 16;                      // steps one launch routes: a slot group (queue_group <= 16)
-
-// Phases A, B, C over the n sources in s_list (each tagged with its step inside the group).
+// #edges of the delay-sorted row [beg, beg+deg) with delay < thr.  Rows of up to 65,535 edges read it from the table
+// (entry k of the row's (src, r) line is the count for thr = (k+1)G - r); longer rows search for it.
 template <bool PACKED>
-__device__ __forceinline__ void route_round(const GnDev &p, const uint32_t n, const uint32_t slot0, const uint32_t *s_list,
-                                            const uint8_t *s_step, uint32_t (*s_wtot)[32], uint32_t (*s_wbase)[32],
-                                            uint32_t *s_ovf, unsigned long long &events)
+__device__ __forceinline__ uint32_t seg_bound(const GnDev &p, const uint16_t *__restrict__ line, const uint32_t k,
+                                              const uint32_t thr, const uint32_t beg, const uint32_t deg)
 {
+    if (deg <= 0xFFFFu) return (uint32_t)__ldg(line + k);
+    uint32_t lo = 0u, hi = deg;
+    while (lo < hi) {
+        const uint32_t mid = (lo + hi) >> 1;
+        const uint32_t d = PACKED ? __ldg(&p.s_edge[beg + mid].x) >> 24 : (uint32_t)__ldg(p.s_dly + beg + mid);
+        if (d < thr) lo = mid + 1u; else hi = mid;
+    }
+    return lo;
+}
+
+// One spike per lane (`valid`): the row bounds of the fired vertex and the first word of its line of the segment table
+// are requested.  Nothing here depends on the spike's log position.
+__device__ __forceinline__ void log_load(const GnDev &p, const uint32_t r, const uint32_t src, const bool valid, uint32_t &beg,
+                                         uint32_t &deg, uint32_t &first_v)
+{
+    beg = deg = first_v = 0u;
+    if (valid) {
+        beg = p.row[src];
+        deg = p.row[src + 1] - beg;
+        if (p.q_arrays >= 2u && deg <= 0xFFFFu)
+            first_v = (uint32_t)__ldg(p.q_seg + (((size_t)src << p.q_log) + r) * p.q_nb + p.q_window);
+    }
+}
+
+// ... and entered into the log of step slot `sl` (r = sl mod G) at position `pos`: the nb-W+1 entries of a spike are
+// stored by its lane -- lanes hold consecutive positions, so every array receives one coalesced run per warp.  The rest
+// is rare and done by the whole warp, spike after spike: rows too long for the table (their boundaries are searched for,
+// one per lane), and spikes beyond the log's capacity (expanded now, straight into the ring).  Whole warps only.
+template <bool PACKED>
+__device__ __forceinline__ void log_store(const GnDev &p, const uint32_t sl, const uint32_t r, const uint32_t src, const bool valid,
+                                          const uint32_t beg, const uint32_t deg, const uint32_t first_v, const uint32_t pos)
+{
+    const uint32_t lane = threadIdx.x & 31u;
+    const uint32_t G = 1u << p.q_log, nb = p.q_nb, W = p.q_window, A = p.q_arrays;
+    if (A < 2u) return;                                   // every event is the update kernel's
+    const uint16_t *line = p.q_seg + ((size_t)src * G + r) * nb;
+    const bool in_table = valid && deg <= 0xFFFFu, logged = valid && pos < p.log_cap;
+    if (in_table && logged) {
+        uint32_t *dst = p.spk_log + ((size_t)sl * A) * p.log_cap + pos;
+        dst[0] = beg + first_v;
+#pragma unroll 6
+        for (uint32_t a = 1u; a + 1u < A; ++a) dst[(size_t)a * p.log_cap] = beg + (uint32_t)__ldg(line + W + a);
+        dst[(size_t)(A - 1u) * p.log_cap] = beg + deg;
+    }
+    for (uint32_t m = __ballot_sync(0xFFFFFFFFu, valid && (!in_table || !logged)); m; m &= m - 1u) {
+        const int sq = __ffs(m) - 1;
+        const uint32_t b2 = __shfl_sync(0xFFFFFFFFu, beg, sq), d2 = __shfl_sync(0xFFFFFFFFu, deg, sq);
+        const uint32_t src2 = __shfl_sync(0xFFFFFFFFu, src, sq), pos2 = __shfl_sync(0xFFFFFFFFu, pos, sq);
+        const uint16_t *line2 = p.q_seg + ((size_t)src2 * G + r) * nb;
+        if (pos2 < p.log_cap) {
+            uint32_t *dst2 = p.spk_log + ((size_t)sl * A) * p.log_cap + pos2;
+            for (uint32_t a = lane; a < A; a += 32u) {
+                const uint32_t j = W + 1u + a;
+                dst2[(size_t)a * p.log_cap] = b2 + (j <= nb ? seg_bound<PACKED>(p, line2, j - 1u, j * G - r, b2, d2) : d2);
+            }
+        } else {
+            const uint32_t x_first = seg_bound<PACKED>(p, line2, W, (W + 1u) * G - r, b2, d2);
+            for (uint32_t x = x_first + lane; x < d2; x += 32u) {
+                const uint2 ev = __ldg(p.s_edge + b2 + x);
+                const uint32_t d = PACKED ? ev.x >> 24 : (uint32_t)__ldg(p.s_dly + b2 + x);
+                uint32_t s1 = sl + d;
+                if (s1 >= p.D) s1 -= p.D;
+                atomicAdd(p.ring + (size_t)s1 * p.Npad + (PACKED ? ev.x & 0xFFFFFFu : ev.x), (int32_t)ev.y);
+            }
+        }
+    }
+}
+
+// Logging warp: the spikes of ONE step (the i-th of the launch: slot0 = t0 mod D, raster row (row0 + i) mod
+// raster_rows) among 32 consecutive raster words.  a3's compaction happens here, warp by warp: popc prefix over the
+// lanes' words, one reservation (atomic) per warp for its spikes' log positions, the fired vertices listed in shared
+// memory; then one lane per spike (log_load, log_store).
+constexpr int kLogWarps = 4;
+
+template <bool PACKED>
+__device__ __forceinline__ void log_spikes(const GnDev &p, const uint32_t slot0, const uint32_t row0, const uint32_t n_batch)
+{
+    __shared__ uint32_t s_src[kLogWarps][1024];
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
-    const uint32_t *__restrict__ row = p.row;
-    const uint32_t nb = p.q_nb, G = 1u << p.q_log, Gm1 = G - 1u;
-    const uint32_t g_cur = slot0 >> p.q_log, r0 = slot0 & Gm1;
-    const uint32_t rd_queued = (p.q_window + 1u) << p.q_log;   // r + delay at or above this: queued
-    uint32_t my_bucket = g_cur + p.q_window + lane;        // bucket of the segment this lane owns
-    while (my_bucket >= nb) my_bucket -= nb;
-
-    // A: per-warp, per-segment record counts.  Four sources at a time: their row bounds and table entries (first
-    // touch: DRAM latency) are all requested before any is used.
-    uint32_t tot = 0u;
-    {
-        const uint32_t tab_i = lane + p.q_window - 1u;     // this lane's table entry (see above)
-        for (uint32_t idx0 = warp; idx0 < n; idx0 += 4u * kRouteWarps) {
-            uint32_t beg[4], end[4], seg[4];
+    const uint32_t blocks_per_step = (p.words_pad + 31u) >> 5;
+    const uint32_t item = blockIdx.x * kLogWarps + warp;
+    if (item >= n_batch * blocks_per_step) return;
+    const uint32_t i = item / blocks_per_step, w = (item - i * blocks_per_step) * 32u + lane;
+    uint32_t sl = slot0 + i, rr = row0 + i;
+    if (sl >= p.D) sl -= p.D;
+    if (rr >= p.raster_rows) rr -= p.raster_rows;
+    uint32_t word = w < p.words_pad ? p.raster[(size_t)rr * p.words_pad + w] : 0u;
+    const uint32_t pc = __popc(word);
+    uint32_t incl = pc;
 #pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                const uint32_t idx = idx0 + (uint32_t)u * kRouteWarps;
-                beg[u] = end[u] = seg[u] = 0u;
-                if (idx < n) {
-                    const uint32_t src = s_list[idx];
-                    beg[u] = row[src]; end[u] = row[src + 1];
-                    if (tab_i < nb)
-                        seg[u] = (uint32_t)__ldg(p.q_seg + ((size_t)src << p.q_log) * nb + (size_t)(r0 + s_step[idx]) * nb + tab_i);
-                }
-            }
-#pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                const uint32_t deg = end[u] - beg[u];
-                const uint32_t lo = tab_i < nb ? seg[u] : deg;
-                uint32_t hi = __shfl_down_sync(0xFFFFFFFFu, lo, 1);
-                if (tab_i + 1u >= nb || lane == 31u) hi = deg;
-                tot += (lane >= 1u && tab_i < nb) ? hi - lo : 0u;
-                events += (unsigned long long)deg;
-            }
-        }
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t v = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+        if (lane >= (uint32_t)o) incl += v;
     }
-    s_wtot[warp][lane] = tot;
-    part_sync<kRouteThreads, 1>();
-    // B: reserve; afterwards s_wbase[w][k] = index (in records, over the whole queue) of warp w's first record
-    // of segment k
-    if (warp == 0) {
-        uint32_t run = 0u;
-#pragma unroll
-        for (int w = 0; w < kRouteWarps; ++w) {
-            const uint32_t c = s_wtot[w][lane];
-            s_wbase[w][lane] = run;
-            run += c;
-        }
-        bool full = false;
-        unsigned long long got = 0ull;
-        if (run) {
-            got = atomicAdd(&p.q_count[my_bucket], (unsigned long long)run);
-            if (got + run <= p.q_cap) {
-                const uint32_t first = (uint32_t)((unsigned long long)my_bucket * p.q_cap + got);
-#pragma unroll
-                for (int w = 0; w < kRouteWarps; ++w) s_wbase[w][lane] += first;
-            } else {
-                full = true;                              // bucket full: this CTA delivers these events directly (phase C)
-            }
-        }
-        const uint32_t mask = __ballot_sync(0xFFFFFFFFu, full);
-        if (lane == 0) *s_ovf = mask;
-        // the records this CTA reserved below the capacity but will not write are neutralised (weight 0) by the whole
-        // warp, bucket after bucket: fewer than the CTA's own record count for that bucket
-        for (uint32_t m = mask; m; m &= m - 1u) {
-            const int k = __ffs(m) - 1;
-            const unsigned long long g_k = __shfl_sync(0xFFFFFFFFu, got, k);
-            const uint32_t b_k = __shfl_sync(0xFFFFFFFFu, my_bucket, k);
-            uint2 *q = p.queue + (size_t)b_k * p.q_cap;
-            for (unsigned long long i = g_k + lane; i < p.q_cap; i += 32ull) q[i] = make_uint2(0u, 0u);
-        }
-    }
-    part_sync<kRouteThreads, 1>();
-    // C: records.  With rd = r + delay: queued iff rd >= (W+1)G; group offset j = rd >> q_log, owned by lane
-    // j - W; ring row inside the bucket = rd & (G-1).
-    const uint32_t ovf = *s_ovf;
-    uint32_t run = s_wbase[warp][lane];
-    // the row bounds and the segment-table entry of the NEXT source are requested before the current source's edges,
-    // so a source costs one memory round trip, not two
-    uint32_t nx_beg = 0u, nx_end = 0u, nx_seg = 0u, nx_r = 0u;
-    const uint32_t tab_i = lane + p.q_window - 1u;         // this lane's table entry (see above)
-    if (warp < n) {
-        const uint32_t src = s_list[warp];
-        nx_r = r0 + s_step[warp];
-        nx_beg = row[src]; nx_end = row[src + 1];
-        if (tab_i < nb) nx_seg = (uint32_t)__ldg(p.q_seg + ((size_t)src << p.q_log) * nb + (size_t)nx_r * nb + tab_i);
-    }
-    for (uint32_t idx = warp; idx < n; idx += kRouteWarps) {
-        const uint32_t r = nx_r, e_beg = nx_beg, n_e = nx_end - nx_beg, seg_lo = nx_seg;
-        if (idx + kRouteWarps < n) {
-            const uint32_t src = s_list[idx + kRouteWarps];
-            nx_r = r0 + s_step[idx + kRouteWarps];
-            nx_beg = row[src]; nx_end = row[src + 1];
-            if (tab_i < nb) nx_seg = (uint32_t)__ldg(p.q_seg + ((size_t)src << p.q_log) * nb + (size_t)nx_r * nb + tab_i);
-        }
-        const uint32_t lo = tab_i < nb ? seg_lo : n_e;     // from the prefetched entry
-        uint32_t hi = __shfl_down_sync(0xFFFFFFFFu, lo, 1);
-        if (tab_i + 1u >= nb || lane == 31u) hi = n_e;
-        const uint32_t cnt = (lane >= 1u && tab_i < nb) ? hi - lo : 0u;
-        const uint32_t adj = run - lo;                     // record index - edge position, for this lane's segment
-        run += cnt;
-        const uint32_t x_first = __shfl_sync(0xFFFFFFFFu, lo, 1) & ~31u;   // the update kernel's edges need no visit
-        const uint2 *__restrict__ edge = p.s_edge + e_beg;
-        const uint8_t *__restrict__ dly = p.s_dly + e_beg;
-        for (uint32_t x0 = x_first; x0 < n_e; x0 += 32u * kRouteUnroll) {
-            uint2 ev[kRouteUnroll];
-            uint32_t d[kRouteUnroll];
-#pragma unroll
-            for (int u = 0; u < kRouteUnroll; ++u) {       // all loads of the super-chunk first
-                const uint32_t x = x0 + 32u * u + lane;
-                ev[u] = make_uint2(0u, 0u);
-                d[u] = 0u;
-                if (x < n_e) {
-                    ev[u] = __ldg(edge + x);
-                    if (!PACKED) d[u] = (uint32_t)__ldg(dly + x);
-                }
-            }
-#pragma unroll
-            for (int u = 0; u < kRouteUnroll; ++u) {
-                if (x0 + 32u * u >= n_e) break;            // warp-uniform
-                const uint32_t x = x0 + 32u * u + lane;
-                const uint32_t rd = r + (PACKED ? ev[u].x >> 24 : d[u]);
-                const uint32_t m = PACKED ? ev[u].x & 0xFFFFFFu : ev[u].x;
-                const bool queued = rd >= rd_queued && x < n_e;
-                const uint32_t k_seg = queued ? (rd >> p.q_log) - p.q_window : 0u;
-                const uint32_t at = __shfl_sync(0xFFFFFFFFu, adj, k_seg) + x;
-                if (!queued) continue;
-                const uint32_t cell = (rd & Gm1) * p.Npad + m;
-                if (ovf && ((ovf >> k_seg) & 1u)) {
-                    uint32_t b = g_cur + (rd >> p.q_log);
-                    if (b >= nb) b -= nb;
-                    atomicAdd(p.ring + ((size_t)b << p.q_log) * p.Npad + cell, (int32_t)ev[u].y);
-                } else {
-                    p.queue[at] = make_uint2(cell, ev[u].y);
-                }
-            }
-        }
-    }
-    part_sync<kRouteThreads, 1>();
-}
-
-// Adds the records of one bucket into the bucket's 2^q_log ring rows (int32 RED; the rows are L2-resident while a
-// bucket is folded); warp w of n_w cooperating warps.  Scattered REDs are bound by LSU issue (about one lane per
-// 1.3 cycles per SM), not by memory.
-__device__ __forceinline__ void fold_records(const GnDev &p, const uint32_t bucket, const uint32_t w, const uint32_t n_w,
-                                             const uint32_t lane)
-{
-    unsigned long long n = p.q_count[bucket];
-    if (n > p.q_cap) n = p.q_cap;
-    int32_t *rows = p.ring + ((size_t)bucket << p.q_log) * p.Npad;
-    const uint4 *q4 = reinterpret_cast<const uint4 *>(p.queue + (size_t)bucket * p.q_cap);
-    const unsigned long long pairs = n >> 1;
-    const unsigned long long stride = (unsigned long long)n_w * 32ull;
-    for (unsigned long long i0 = (unsigned long long)w * 32ull + lane; i0 < pairs; i0 += 4ull * stride) {
-        uint4 v[4];
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {                       // four 16-byte loads in flight per lane
-            const unsigned long long i = i0 + (unsigned long long)u * stride;
-            v[u] = (i < pairs) ? __ldcs(q4 + i) : make_uint4(0u, 0u, 0u, 0u);
-        }
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            if (v[u].y) atomicAdd(rows + v[u].x, (int32_t)v[u].y);
-            if (v[u].w) atomicAdd(rows + v[u].z, (int32_t)v[u].w);
-        }
-    }
-    if ((n & 1ull) && w == 0u && lane == 0u) {
-        const uint2 v = p.queue[(size_t)bucket * p.q_cap + n - 1];
-        if (v.y) atomicAdd(rows + v.x, (int32_t)v.y);
-    }
-}
-
-// Routes the queued segments of every vertex that fired in steps t0 .. t0+n_batch-1, all inside ONE slot
-// group (slot0 = t0 mod D): one launch per group amortises the launch and the dependent memory round trips
-// over 2^q_log steps of work.  raster row of step t0+i is (row0 + i) mod raster_rows.
-// Warp specialisation: threads 0..255 route (their barriers are the named barrier 1); the kFoldWarps warps after
-// them fold bucket `fold_bucket` -- complete since the previous group's routing -- at the same time, in the same
-// CTAs: routing waits on DRAM, folding on LSU issue, and two separate kernels that each fill the SMs never overlap.
-constexpr int kFoldWarps = 2;
-
-template <bool PACKED>
-__global__ void __launch_bounds__(kRouteThreads + 32 * kFoldWarps, 3)
-gn_route_kernel(const GnDev p, const uint32_t slot0, const uint32_t row0, const uint32_t n_batch,
-                const uint32_t chunk_words, const uint32_t fold_bucket)
-{
-    __shared__ uint32_t s_list[kRouteListCap];
-    __shared__ uint8_t s_step[kRouteListCap];
-    __shared__ uint32_t s_wsum[kRouteWarps];
-    __shared__ uint32_t s_wtot[kRouteWarps][32];         // A: records of warp w in segment k
-    __shared__ uint32_t s_wbase[kRouteWarps][32];        // B: where warp w's records of segment k start in the bucket
-    __shared__ uint32_t s_ovf;                           // B: bit k = segment k's bucket is full
-    if (threadIdx.x >= kRouteThreads) {                  // folding warps
-        if (fold_bucket != kNoBucket)
-            fold_records(p, fold_bucket, blockIdx.x * kFoldWarps + ((threadIdx.x - kRouteThreads) >> 5),
-                         gridDim.x * kFoldWarps, threadIdx.x & 31u);
-        return;
-    }
-    const uint32_t w0 = blockIdx.x * chunk_words;
-    const uint32_t n_words = min(chunk_words, p.words_pad - w0);
+    const uint32_t total = __shfl_sync(0xFFFFFFFFu, incl, 31);
+    if (total == 0u) return;                              // warp-uniform
+    uint32_t base = 0u;
+    if (lane == 0u) base = atomicAdd(&p.log_n[sl], total);   // its result is needed only when the first entries are stored
+    for (uint32_t k = incl - pc; word; ++k, word &= word - 1u) s_src[warp][k] = (w << 5) + (uint32_t)__ffs(word) - 1u;
+    __syncwarp();
+    const uint32_t r = sl & ((1u << p.q_log) - 1u);       // D is a multiple of G: slot mod G = t mod G
     unsigned long long events = 0ull;
-    uint32_t n = 0u, spikes = 0u;
-    // the spike lists of all the group's steps are requested at once (one memory round trip, not one per step)
-    uint32_t words[kMaxBatch], pc_all = 0u;
-#pragma unroll
-    for (int i = 0; i < (int)kMaxBatch; ++i) {
-        uint32_t rr = row0 + (uint32_t)i;
-        if (rr >= p.raster_rows) rr -= p.raster_rows;
-        words[i] = ((uint32_t)i < n_batch && threadIdx.x < n_words) ? p.raster[(size_t)rr * p.words_pad + w0 + threadIdx.x] : 0u;
+    bool have_base = false;
+    for (uint32_t q0 = 0u; q0 < total; q0 += 32u) {
+        const uint32_t q = q0 + lane;
+        const bool valid = q < total;
+        const uint32_t src = valid ? s_src[warp][q] : 0u;
+        uint32_t beg, deg, first_v;
+        log_load(p, r, src, valid, beg, deg, first_v);
+        events += (unsigned long long)deg;
+        if (!have_base) {                                 // (warp-uniform) the loads above went out before this wait
+            base = __shfl_sync(0xFFFFFFFFu, base, 0);
+            have_base = true;
+        }
+        log_store<PACKED>(p, sl, r, src, valid, beg, deg, first_v, base + q);
     }
 #pragma unroll
-    for (int i = 0; i < (int)kMaxBatch; ++i) pc_all += __popc(words[i]);
-    uint32_t off;
-    const uint32_t total_all = gather_scan<kRouteThreads, 1>(pc_all, s_wsum, off);
-    if (total_all <= kRouteListCap) {                       // the usual case: one scan, one round for the whole group
-#pragma unroll
-        for (int i = 0; i < (int)kMaxBatch; ++i) {
-            gather_write(words[i], w0, off, s_list, s_step, (uint32_t)i);
-            off += __popc(words[i]);
-        }
-        n = spikes = total_all;
-    } else {                                                // rare (a burst beyond the list): step by step, words read again
-        for (uint32_t i = 0; i < n_batch; ++i) {
-            uint32_t rr = row0 + i;
-            if (rr >= p.raster_rows) rr -= p.raster_rows;
-            const uint32_t word = threadIdx.x < n_words ? p.raster[(size_t)rr * p.words_pad + w0 + threadIdx.x] : 0u;
-            const uint32_t total = gather_scan<kRouteThreads, 1>(__popc(word), s_wsum, off);
-            if (n + total > kRouteListCap) {                // CTA-uniform: the list is full, work it off first
-                route_round<PACKED>(p, n, slot0, s_list, s_step, s_wtot, s_wbase, &s_ovf, events);
-                n = 0u;
-            }
-            gather_write(word, w0, n + off, s_list, s_step, i);
-            n += total;
-            spikes += total;
-        }
+    for (int o = 16; o >= 1; o >>= 1) events += __shfl_xor_sync(0xFFFFFFFFu, events, o);
+    if (lane == 0u) {
+        if (events) atomicAdd(&p.counters[2], events);
+        atomicAdd(&p.counters[1], (unsigned long long)total);
     }
-    part_sync<kRouteThreads, 1>();
-    if (n) route_round<PACKED>(p, n, slot0, s_list, s_step, s_wtot, s_wbase, &s_ovf, events);
-    if ((threadIdx.x & 31u) == 0 && events) atomicAdd(&p.counters[2], events);
-    if (threadIdx.x == 0 && spikes) atomicAdd(&p.counters[1], (unsigned long long)spikes);
 }
 
-// ---- a4, queue mode: fold one bucket outside the step loop (ring read-back) ----------------------------------
-__global__ void __launch_bounds__(256)
-gn_fold_kernel(const GnDev p, const uint32_t bucket)
+// Folding warp fw of n_fw: the log entries of the n_win steps starting at slot win_slot0 (step t_win, r_win = t_win
+// mod G) that are due j_first - (groups since t_win's) groups ahead, i.e. in the group being folded.
+// A warp takes 32 consecutive (spike, segment) pairs at a time -- two coalesced log reads per lane -- and lays their
+// edges out back to back (the chunk's EXPANSION, T slots): slot x belongs to the pair whose segment ends first at or
+// after x.  The ends are marked in a shared-memory bit mask, so the owner of a slot is a popc away: rank = ends before
+// the slot's 32-slot word (s_rank) + ends before it inside the word; the pair's {edge index - slot, step slot} sits at
+// that rank in s_pair (empty segments are not listed).  Every lane of every reduction carries one event; kFoldUnroll
+// 32-slot words of edge loads are in flight before their reductions are issued.  Segments of more than kFoldLong edges
+// (hubs) are not laid out: the whole warp walks them one after another.
+constexpr uint32_t kFoldLong = 64;
+
+// s_pref[i] = spikes logged in the window's steps before step i (i < n_win), P their total; s_pair (32 entries), s_ends
+// and s_rank (kFoldLong words each) are this warp's tables.
+template <bool PACKED>
+__device__ __forceinline__ void fold_chunks(const GnDev &p, const uint32_t *s_pref, const uint32_t P, const uint32_t win_slot0,
+                                            const uint32_t n_win, const uint32_t r_win, const uint32_t j_first, const uint32_t fw,
+                                            const uint32_t n_fw, uint2 *s_pair, uint32_t *s_ends, uint32_t *s_rank)
 {
-    fold_records(p, bucket, (blockIdx.x * blockDim.x + threadIdx.x) >> 5, (gridDim.x * blockDim.x) >> 5, threadIdx.x & 31u);
+    const uint32_t lane = threadIdx.x & 31u;
+    const uint32_t A = p.q_arrays, W = p.q_window;
+    const uint2 *__restrict__ edge = p.s_edge;
+    const uint8_t *__restrict__ dly = p.s_dly;
+    const uint32_t n_chunks = (P + 31u) / 32u;
+
+    // this lane's (spike, segment) pair of chunk c: first edge, edge count, slot of the spike's step
+    auto load_pair = [&](const uint32_t c, uint32_t &b, uint32_t &cnt, uint32_t &tsl) {
+        b = cnt = tsl = 0u;
+        if (c >= n_chunks) return;
+        uint32_t lo = 0u, hi = n_win;                     // the step of the chunk's first pair (warp-uniform search) ...
+        while (hi - lo > 1u) {
+            const uint32_t mid = (lo + hi) >> 1;
+            if (s_pref[mid] <= c * 32u) lo = mid; else hi = mid;
+        }
+        const uint32_t pidx = c * 32u + lane;
+        if (pidx >= P) return;
+        while (lo + 1u < n_win && s_pref[lo + 1u] <= pidx) ++lo;   // ... and of this lane's (a chunk rarely straddles steps)
+        const uint32_t a = j_first - ((r_win + lo) >> p.q_log) - W - 1u;
+        tsl = win_slot0 + lo;
+        if (tsl >= p.D) tsl -= p.D;
+        const uint32_t *L = p.spk_log + ((size_t)tsl * A + a) * p.log_cap + (pidx - s_pref[lo]);
+        b = __ldcs(L);
+        cnt = __ldcs(L + p.log_cap) - b;
+    };
+    // one edge: the reduction into ring[(step + delay) mod D][target]
+    auto deliver = [&](const uint2 ev, const uint32_t d, const uint32_t tsl) {
+        uint32_t s1 = tsl + d;
+        if (s1 >= p.D) s1 -= p.D;
+        atomicAdd(p.ring + (size_t)s1 * p.Npad + (PACKED ? ev.x & 0xFFFFFFu : ev.x), (int32_t)ev.y);
+    };
+    uint32_t b, cnt, tsl;
+    load_pair(fw, b, cnt, tsl);
+    for (uint32_t c = fw; c < n_chunks; c += n_fw) {
+        uint32_t nx_b, nx_cnt, nx_tsl;
+        load_pair(c + n_fw, nx_b, nx_cnt, nx_tsl);        // the next chunk's entries are on their way during this one
+        const uint32_t small = cnt <= kFoldLong ? cnt : 0u;
+        uint32_t incl = small;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t v = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+            if (lane >= (uint32_t)o) incl += v;
+        }
+        const uint32_t T = __shfl_sync(0xFFFFFFFFu, incl, 31);
+        if (T) {
+            const uint32_t n_words = (T + 31u) >> 5;      // <= kFoldLong
+            const uint32_t listed = __ballot_sync(0xFFFFFFFFu, small != 0u);
+            __syncwarp();                                 // the previous chunk's tables are no longer read
+            s_ends[lane] = 0u;
+            s_ends[lane + 32u] = 0u;
+            __syncwarp();
+            if (small) {
+                s_pair[__popc(listed & ((1u << lane) - 1u))] = make_uint2(b - (incl - small), tsl);
+                atomicOr(&s_ends[(incl - 1u) >> 5], 1u << ((incl - 1u) & 31u));
+            }
+            __syncwarp();
+            uint32_t before = 0u;                         // ends before each word: prefix popc over the mask words
+#pragma unroll
+            for (int half = 0; half < (int)kFoldLong / 32; ++half) {
+                const uint32_t pc = __popc(s_ends[lane + 32u * half]);
+                uint32_t inc2 = pc;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const uint32_t v = __shfl_up_sync(0xFFFFFFFFu, inc2, o);
+                    if (lane >= (uint32_t)o) inc2 += v;
+                }
+                s_rank[lane + 32u * half] = before + inc2 - pc;
+                before += __shfl_sync(0xFFFFFFFFu, inc2, 31);
+            }
+            __syncwarp();
+            for (uint32_t w0 = 0u; w0 < n_words; w0 += kFoldUnroll) {
+                uint2 ev[kFoldUnroll];
+                uint32_t d[kFoldUnroll], sl[kFoldUnroll];
+#pragma unroll
+                for (int u = 0; u < kFoldUnroll; ++u) {   // all loads of kFoldUnroll words first
+                    const uint32_t w = w0 + (uint32_t)u, x = (w << 5) + lane;
+                    ev[u] = make_uint2(0u, 0u);
+                    d[u] = sl[u] = 0u;
+                    if (x < T) {
+                        const uint32_t rk = s_rank[w] + __popc(s_ends[w] & ((1u << lane) - 1u));
+                        const uint2 pr = s_pair[rk];
+                        const uint32_t e = pr.x + x;      // 32-bit on purpose: pr.x = first edge - first slot may have wrapped
+                        sl[u] = pr.y;
+                        ev[u] = __ldcs(edge + e);
+                        d[u] = PACKED ? ev[u].x >> 24 : (uint32_t)__ldg(dly + e);
+                    }
+                }
+#pragma unroll
+                for (int u = 0; u < kFoldUnroll; ++u)
+                    if (d[u]) deliver(ev[u], d[u], sl[u]);    // a delay is never 0
+            }
+        }
+        for (uint32_t m = __ballot_sync(0xFFFFFFFFu, cnt > kFoldLong); m; m &= m - 1u) {   // long segments, one after another
+            const int src = __ffs(m) - 1;
+            const uint32_t pb = __shfl_sync(0xFFFFFFFFu, b, src), pn = __shfl_sync(0xFFFFFFFFu, cnt, src);
+            const uint32_t ps = __shfl_sync(0xFFFFFFFFu, tsl, src);
+            for (uint32_t x = lane; x < pn; x += 32u) {
+                const uint2 e2 = __ldcs(edge + pb + x);
+                deliver(e2, PACKED ? e2.x >> 24 : (uint32_t)__ldg(dly + pb + x), ps);
+            }
+        }
+        b = nx_b; cnt = nx_cnt; tsl = nx_tsl;
+    }
+}
+
+// The counts of the window's steps -> s_pref (CTA-wide, kRouteThreads threads), then the chunks.
+template <bool PACKED>
+__device__ __forceinline__ void fold_group(const GnDev &p, const uint32_t win_slot0, const uint32_t n_win, const uint32_t r_win,
+                                           const uint32_t j_first, const uint32_t fw, const uint32_t n_fw)
+{
+    __shared__ uint32_t s_pref[kMaxWindow];
+    __shared__ uint32_t s_wsum2[kRouteWarps];
+    __shared__ uint2 s_pair[kRouteWarps][32];
+    __shared__ uint32_t s_ends[kRouteWarps][kFoldLong], s_rank[kRouteWarps][kFoldLong];
+    const uint32_t warp = threadIdx.x >> 5;
+    uint32_t cnt_step = 0u;
+    if (threadIdx.x < n_win) {
+        uint32_t sl = win_slot0 + threadIdx.x;
+        if (sl >= p.D) sl -= p.D;
+        cnt_step = min(p.log_n[sl], p.log_cap);
+    }
+    uint32_t off;
+    const uint32_t P = gather_scan<kRouteThreads>(cnt_step, s_wsum2, off);
+    s_pref[threadIdx.x] = off;
+    __syncthreads();
+    if (P == 0u) return;
+    fold_chunks<PACKED>(p, s_pref, P, win_slot0, n_win, r_win, j_first, fw, n_fw, s_pair[warp], s_ends[warp], s_rank[warp]);
+}
+
+// Queue-mode delivery, first half: the spikes of steps t0 .. t0+n_batch-1 (all inside one slot group) enter the log.
+// Launched just before gn_fold_kernel, which does not depend on it (it reads older log entries only): the trigger lets
+// the two run side by side.
+template <bool PACKED>
+__global__ void __launch_bounds__(kLogWarps * 32)
+gn_log_kernel(const GnDev p, const uint32_t slot0, const uint32_t row0, const uint32_t n_batch)
+{
+    asm volatile("griddepcontrol.launch_dependents;");
+    log_spikes<PACKED>(p, slot0, row0, n_batch);
+}
+
+// Queue-mode delivery, second half: one slot group folded out of the log (persistent CTAs, grid-stride over the log).
+template <bool PACKED>
+__global__ void __launch_bounds__(kRouteThreads, kFoldCtasPerSm)
+gn_fold_kernel(const GnDev p, const uint32_t win_slot0, const uint32_t n_win, const uint32_t r_win, const uint32_t j_first)
+{
+    fold_group<PACKED>(p, win_slot0, n_win, r_win, j_first, blockIdx.x * kRouteWarps + (threadIdx.x >> 5), gridDim.x * kRouteWarps);
 }
 
 // ---- create time, queue mode: copy every CSR row sorted by delay (counting sort, one warp per row) --------
@@ -752,10 +781,10 @@ gn_sort_rows_kernel(const GnDev p, GnCheck *chk)
 #pragma unroll
         for (int k = 0; k < 8; ++k) { h[lane * 8 + k] = run; run += c[k]; }
         __syncwarp();
-        // h[d] = #edges with delay < d.  Segment table (see gn_route_kernel): entry (r, k) = h[(k+1)G - r].
+        // h[d] = #edges with delay < d.  Segment table (see log_spikes): entry (r, k) = h[(k+1)G - r].
         if (p.q_seg) {
             const uint32_t G = 1u << p.q_log, nb = p.q_nb, deg = end - beg;
-            if (deg > 0xFFFFu) chk->big_degree = 1u;
+            // (a row of more than 65,535 edges cannot be described in 16 bits: its entries are never read, see seg_bound)
             uint16_t *seg = p.q_seg + (size_t)i * G * nb;
             for (uint32_t x = lane; x < G * nb; x += 32u) {
                 const uint32_t r = x / nb, k = x - r * nb;
@@ -1496,20 +1525,35 @@ cudaError_t gnk_deliver(const GnDev &p, uint64_t t, cudaStream_t st)
     return cudaGetLastError();
 }
 
-cudaError_t gnk_route(const GnDev &p, uint64_t t0, uint32_t n_batch, uint32_t fold_bucket, cudaStream_t st)
+cudaError_t gnk_log(const GnDev &p, uint64_t t0, uint32_t n_batch, cudaStream_t st)
 {
-    const uint32_t w = chunk_words_for(p, 148u * 3u);            // three 320-thread CTAs per SM
-    const uint32_t grid = ceil_div(p.words_pad, w), slot0 = (uint32_t)(t0 % p.D), row0 = (uint32_t)(t0 % p.raster_rows);
-    const uint32_t threads = kRouteThreads + 32 * kFoldWarps;
-    if (p.packed) gn_route_kernel<true><<<grid, threads, 0, st>>>(p, slot0, row0, n_batch, w, fold_bucket);
-    else gn_route_kernel<false><<<grid, threads, 0, st>>>(p, slot0, row0, n_batch, w, fold_bucket);
+    if (n_batch == 0u) return cudaSuccess;
+    const uint32_t slot0 = (uint32_t)(t0 % p.D), row0 = (uint32_t)(t0 % p.raster_rows);
+    const uint32_t grid = ceil_div((uint64_t)n_batch * ((p.words_pad + 31u) >> 5), kLogWarps);   // a warp per step and 32 raster words
+    if (p.packed) gn_log_kernel<true><<<grid, kLogWarps * 32, 0, st>>>(p, slot0, row0, n_batch);
+    else gn_log_kernel<false><<<grid, kLogWarps * 32, 0, st>>>(p, slot0, row0, n_batch);
     return cudaGetLastError();
 }
 
-cudaError_t gnk_fold(const GnDev &p, uint32_t bucket, cudaStream_t st)
+cudaError_t gnk_fold(const GnDev &p, uint64_t t_win, uint32_t n_win, uint64_t g_fold, bool beside_previous, cudaStream_t st)
 {
-    gn_fold_kernel<<<148u * 4u, 256, 0, st>>>(p, bucket);
-    return cudaGetLastError();
+    if (p.q_arrays < 2u || n_win == 0u) return cudaSuccess;      // nothing logged that is due in this group
+    const uint32_t win_slot0 = (uint32_t)(t_win % p.D), r_win = (uint32_t)(t_win & ((1ull << p.q_log) - 1ull));
+    const uint32_t j_first = (uint32_t)(g_fold - (t_win >> p.q_log));
+    cudaLaunchConfig_t cfg{};
+    static const uint32_t fold_ctas = [] { const char *e = getenv("GN_FOLD_CTAS"); const int v = e ? atoi(e) : 0; return (uint32_t)(v >= 1 && v <= kFoldCtasPerSm ? v : kFoldCtasPerSm); }();
+    cfg.gridDim = dim3(148u * fold_ctas);
+    cfg.blockDim = dim3(kRouteThreads);
+    cfg.stream = st;
+    // programmatic stream serialization: the fold may start while the kernel in front of it in the stream (the logging
+    // kernel of the same launch, which it does not depend on) is still running
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = beside_previous ? 1 : 0;
+    return p.packed ? cudaLaunchKernelEx(&cfg, gn_fold_kernel<true>, p, win_slot0, n_win, r_win, j_first)
+                    : cudaLaunchKernelEx(&cfg, gn_fold_kernel<false>, p, win_slot0, n_win, r_win, j_first);
 }
 
 cudaError_t gnk_sort_rows(const GnDev &p, GnCheck *chk, cudaStream_t st)

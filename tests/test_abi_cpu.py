@@ -48,9 +48,11 @@ def test_query_workspace_sizes_and_errors():
     cfg = gn.make_config(1_000_000, 3, 200_000_000, 128, 0.1, 0.006, 2, raster_capacity_steps=0,
                          delivery_mode=gn.GN_DELIVER_RING)
     need = gn.gn_query_workspace(cfg)
-    # queue mode (what AUTO picks here: ring 512 MB >> L2): 16 buckets of 8 * E/16 records + the 16-bit segment table [N][D]
+    # queue mode (what AUTO picks here: ring 512 MB >> L2), 16 groups of 8 slots: the spike log (128 step slots x 15
+    # arrays x N/16 spikes x 4 B) + the 16-bit segment table [N][D] + the raster rows of 3 groups instead of 2 steps
     auto = gn.gn_query_workspace(gn.make_config(1_000_000, 3, 200_000_000, 128, 0.1, 0.006, 2))
-    assert auto - need == pytest.approx(16 * 8 * 12_500_000 * 8 + 1_000_000 * 128 * 2, rel=1e-3)
+    assert auto - need == pytest.approx(128 * 15 * 62_528 * 4 + 1_000_000 * 128 * 2 + 22 * 1_000_064 / 8, rel=1e-3)
+    assert auto < 6 * 2 ** 30                                      # config 4 as a whole: under 6 GB
     for bad_q in (dict(delivery_mode=4), dict(queue_group=3), dict(queue_group=32)):
         with pytest.raises(gn.GnError):
             gn.gn_query_workspace(gn.make_config(10, 2, 5, 16, 0.1, 0.1, 1, **bad_q))

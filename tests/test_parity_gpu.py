@@ -125,22 +125,24 @@ def test_config_bit_exact_2000_steps(gn, k, n, nb, steps, chunk):
 # ---- queue-mode delivery (deferred ring adds): same results, bit for bit -----------------------------
 QUEUE_CASES = [
     # k, n, n_networks, steps, chunk, queue_group, queue_capacity
-    (4, 9_001, None, 2000, 500, 8, 0),        # the mode config 4 runs in: D=128, 16 buckets of 8 slots
-    (4, 9_001, None, 1000, 1000, 8, 0),       # ring never read back (no flush) until the end
-    (4, 5_003, None, 1200, 300, 16, 0),       # 8 buckets of 16 slots
-    (4, 5_003, None, 1200, 300, 4, 0),        # 32 buckets of 4 slots (one per lane of the routing warp)
-    (4, 5_003, None, 1200, 300, 8, 4096),     # buckets overflow: the excess is delivered directly
-    (4, 5_003, None, 600, 300, 4, 64),        # overflow on nearly every pass
+    (4, 9_001, None, 2000, 500, 8, 0),        # D=128, 16 groups of 8 slots
+    (4, 9_001, None, 1000, 1000, 4, 0),       # the mode config 4 runs in (32 groups of 4); ring never read back until the end
+    (4, 5_003, None, 1200, 300, 16, 0),       # 8 groups of 16 slots
+    (4, 5_003, None, 1200, 300, 4, 0),        # 32 groups of 4 slots
+    (4, 5_003, None, 1200, 300, 2, 0),        # 64 groups: more log arrays than lanes of a logging warp
+    (4, 5_003, None, 1200, 300, 1, 0),        # every slot its own group
+    (4, 5_003, None, 1200, 300, 8, 64),       # the spike log overflows in bursts: the excess is expanded on the spot
+    (4, 5_003, None, 600, 300, 4, 32),        # overflow on many steps
     (3, 6_007, None, 1500, 500, 8, 0),        # D=64
     (2, None, None, 1000, 250, 4, 0),         # D=16 (observation on)
-    (2, 3_000, None, 600, 200, 8, 0),         # D=16: two buckets
+    (2, 3_000, None, 600, 200, 8, 0),         # D=16: two groups, every event is the update kernel's
     (5, 1000, 6, 1000, 250, 8, 0),            # batched, D=32
     (1, None, None, 2000, 500, 2, 0),         # N=100
 ]
 
 
-def test_queue_mode_deep_ring_picks_a_larger_group(gn):
-    """D = 160 with the group left open: groups of 4 would need 40 buckets (> 32 lanes), so the library takes 8."""
+def test_queue_mode_deep_ring(gn):
+    """D = 160 with the group left open: 40 groups of 4 (more log arrays than lanes of a logging warp)."""
     rng = np.random.default_rng(12)
     net, cfg = make_config(2, n=2_500)
     cfg = dict(cfg, ring_slots=160, obs_stride=0)
@@ -426,10 +428,10 @@ def test_queue_mode_profiling_mode_and_small_raster_window(gn):
     assert ei.value.code == gn.GN_E_RANGE_EVICTED
 
 
-def test_out_degree_above_16_bits_falls_back_to_the_ring_path(gn):
-    """The queue mode's segment table is 16-bit: a hub with 70,000 out-edges makes AUTO use the ring path
-    (same results) and a forced GN_DELIVER_QUEUE fail loudly."""
-    n, deg = 100_032, 70_000                                           # ring 51 MB: AUTO would pick queue mode
+def test_out_degree_above_16_bits_in_queue_mode(gn):
+    """The queue mode's segment table is 16-bit: the boundaries of a hub with 70,000 out-edges are searched for in its
+    delay-sorted row instead, in AUTO (queue: the ring is 51 MB) and in forced GN_DELIVER_QUEUE alike."""
+    n, deg = 100_032, 70_000
     rng = np.random.default_rng(3)
     row = np.zeros(n + 1, np.uint64)
     row[1:] = deg                                                      # vertex 0 is the only source
@@ -439,19 +441,18 @@ def test_out_degree_above_16_bits_falls_back_to_the_ring_path(gn):
                   np.zeros(n, np.uint8))
     cfg = base_cfg([rs_class()], ring_slots=128)
     dl = rng.integers(1, 128, deg).astype(np.uint8)
-    with pytest.raises(gn.GnError) as ei:
-        _make(gn, net, cfg, 10, delays=dl, delivery_mode=gn.GN_DELIVER_QUEUE)
-    assert ei.value.code == gn.GN_E_INVALID_ARG
-    g = _make(gn, net, cfg, 300, delays=dl)
-    o = Oracle(net, cfg, "fp32", delays=dl)
-    v = np.full(n, -70.0, np.float32)
-    v[0] = 30.0
-    gn.gn_write_state(g, gn.GN_V, v)
-    o.set_state(ob.V, v.astype(np.float64))
-    gn.gn_step(g, 300)
-    o.step(300)
-    _compare_exact(gn, g, o, 300)
-    assert o.counters()["delivered"] >= deg
+    for mode, cap in ((gn.GN_DELIVER_QUEUE, 0), (gn.GN_DELIVER_AUTO, 0), (gn.GN_DELIVER_QUEUE, 32)):
+        g = _make(gn, net, cfg, 300, delays=dl, delivery_mode=mode, queue_capacity=cap)
+        o = Oracle(net, cfg, "fp32", delays=dl)
+        v = np.full(n, -70.0, np.float32)
+        v[:40] = 30.0                                                  # the hub and 39 vertices without out-edges fire at step 0
+        gn.gn_write_state(g, gn.GN_V, v)
+        o.set_state(ob.V, v.astype(np.float64))
+        for done in (1, 3, 50, 300):
+            gn.gn_step(g, done - int(gn.gn_read_state(g, gn.GN_STEP)[0]))
+            o.step(done - o.counters()["steps"])
+            _compare_exact(gn, g, o, done)
+        assert o.counters()["delivered"] >= deg
 
 
 @pytest.mark.parametrize("k,n,nb,steps", [(1, None, None, 2000), (2, None, None, 2000), (3, 6_007, None, 2000),
