@@ -524,21 +524,23 @@ __device__ __forceinline__ void log_store(const GnDev &p, const uint32_t sl, con
     }
 }
 
-// Logging warp: the spikes of ONE step (the i-th of the launch: slot0 = t0 mod D, raster row (row0 + i) mod
-// raster_rows) among 32 consecutive raster words.  a3's compaction happens here, warp by warp: popc prefix over the
-// lanes' words, one reservation (atomic) per warp for its spikes' log positions, the fired vertices listed in shared
-// memory; then one lane per spike (log_load, log_store).
-constexpr int kLogWarps = 4;
+// Logging CTA: the spikes of ONE step (the i-th of the launch: slot0 = t0 mod D, raster row (row0 + i) mod raster_rows)
+// among kLogWarps x 32 consecutive raster words.  a3's compaction happens here: popc prefix over the lanes' words and
+// over the CTA's warps, ONE reservation (atomic) per CTA for its spikes' log positions -- every warp a stretch of it --
+// the fired vertices listed in shared memory; then one lane per spike (log_load, log_store).  The counters take one
+// atomic per CTA as well: thousands of same-address atomics serialise in the L2.
+constexpr int kLogWarps = 8;
 
 template <bool PACKED>
 __device__ __forceinline__ void log_spikes(const GnDev &p, const uint32_t slot0, const uint32_t row0, const uint32_t n_batch)
 {
     __shared__ uint32_t s_src[kLogWarps][1024];
+    __shared__ uint32_t s_tot[kLogWarps], s_base;
+    __shared__ unsigned long long s_events;
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
-    const uint32_t blocks_per_step = (p.words_pad + 31u) >> 5;
-    const uint32_t item = blockIdx.x * kLogWarps + warp;
-    if (item >= n_batch * blocks_per_step) return;
-    const uint32_t i = item / blocks_per_step, w = (item - i * blocks_per_step) * 32u + lane;
+    const uint32_t ctas_per_step = (p.words_pad + kLogWarps * 32u - 1u) / (kLogWarps * 32u);
+    const uint32_t i = blockIdx.x / ctas_per_step;       // (the grid is n_batch x ctas_per_step CTAs)
+    const uint32_t w = ((blockIdx.x - i * ctas_per_step) * kLogWarps + warp) * 32u + lane;
     uint32_t sl = slot0 + i, rr = row0 + i;
     if (sl >= p.D) sl -= p.D;
     if (rr >= p.raster_rows) rr -= p.raster_rows;
@@ -551,32 +553,44 @@ __device__ __forceinline__ void log_spikes(const GnDev &p, const uint32_t slot0,
         if (lane >= (uint32_t)o) incl += v;
     }
     const uint32_t total = __shfl_sync(0xFFFFFFFFu, incl, 31);
-    if (total == 0u) return;                              // warp-uniform
-    uint32_t base = 0u;
-    if (lane == 0u) base = atomicAdd(&p.log_n[sl], total);   // its result is needed only when the first entries are stored
+    if (lane == 0u) s_tot[warp] = total;
+    if (threadIdx.x == 0) s_events = 0ull;
     for (uint32_t k = incl - pc; word; ++k, word &= word - 1u) s_src[warp][k] = (w << 5) + (uint32_t)__ffs(word) - 1u;
-    __syncwarp();
+    __syncthreads();
+    uint32_t before = 0u, cta_total = 0u;                 // spikes of the warps in front of this one, of the whole CTA
+#pragma unroll
+    for (int k = 0; k < kLogWarps; ++k) {
+        const uint32_t c = s_tot[k];
+        if ((uint32_t)k < warp) before += c;
+        cta_total += c;
+    }
+    if (cta_total == 0u) return;                          // CTA-uniform
+    if (threadIdx.x == 0) s_base = atomicAdd(&p.log_n[sl], cta_total);   // its result is needed only when the first entries are stored
     const uint32_t r = sl & ((1u << p.q_log) - 1u);       // D is a multiple of G: slot mod G = t mod G
-    unsigned long long events = 0ull;
-    bool have_base = false;
-    for (uint32_t q0 = 0u; q0 < total; q0 += 32u) {
+    // the first 32 spikes of every warp: their loads go out before anybody waits for the reservation
+    const bool valid0 = lane < total;
+    const uint32_t src0 = valid0 ? s_src[warp][lane] : 0u;
+    uint32_t beg, deg, first_v;
+    log_load(p, r, src0, valid0, beg, deg, first_v);
+    unsigned long long events = (unsigned long long)deg;
+    __syncthreads();
+    const uint32_t base = s_base + before;
+    log_store<PACKED>(p, sl, r, src0, valid0, beg, deg, first_v, base + lane);
+    for (uint32_t q0 = 32u; q0 < total; q0 += 32u) {      // (a burst: more than 32 spikes among the warp's 1,024 vertices)
         const uint32_t q = q0 + lane;
         const bool valid = q < total;
         const uint32_t src = valid ? s_src[warp][q] : 0u;
-        uint32_t beg, deg, first_v;
         log_load(p, r, src, valid, beg, deg, first_v);
         events += (unsigned long long)deg;
-        if (!have_base) {                                 // (warp-uniform) the loads above went out before this wait
-            base = __shfl_sync(0xFFFFFFFFu, base, 0);
-            have_base = true;
-        }
         log_store<PACKED>(p, sl, r, src, valid, beg, deg, first_v, base + q);
     }
 #pragma unroll
     for (int o = 16; o >= 1; o >>= 1) events += __shfl_xor_sync(0xFFFFFFFFu, events, o);
-    if (lane == 0u) {
-        if (events) atomicAdd(&p.counters[2], events);
-        atomicAdd(&p.counters[1], (unsigned long long)total);
+    if (lane == 0u && events) atomicAdd(&s_events, events);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        if (s_events) atomicAdd(&p.counters[2], s_events);
+        atomicAdd(&p.counters[1], (unsigned long long)cta_total);
     }
 }
 
@@ -1529,7 +1543,7 @@ cudaError_t gnk_log(const GnDev &p, uint64_t t0, uint32_t n_batch, cudaStream_t 
 {
     if (n_batch == 0u) return cudaSuccess;
     const uint32_t slot0 = (uint32_t)(t0 % p.D), row0 = (uint32_t)(t0 % p.raster_rows);
-    const uint32_t grid = ceil_div((uint64_t)n_batch * ((p.words_pad + 31u) >> 5), kLogWarps);   // a warp per step and 32 raster words
+    const uint32_t grid = n_batch * ceil_div(p.words_pad, kLogWarps * 32u);   // a warp per step and 32 raster words
     if (p.packed) gn_log_kernel<true><<<grid, kLogWarps * 32, 0, st>>>(p, slot0, row0, n_batch);
     else gn_log_kernel<false><<<grid, kLogWarps * 32, 0, st>>>(p, slot0, row0, n_batch);
     return cudaGetLastError();
@@ -1541,8 +1555,7 @@ cudaError_t gnk_fold(const GnDev &p, uint64_t t_win, uint32_t n_win, uint64_t g_
     const uint32_t win_slot0 = (uint32_t)(t_win % p.D), r_win = (uint32_t)(t_win & ((1ull << p.q_log) - 1ull));
     const uint32_t j_first = (uint32_t)(g_fold - (t_win >> p.q_log));
     cudaLaunchConfig_t cfg{};
-    static const uint32_t fold_ctas = [] { const char *e = getenv("GN_FOLD_CTAS"); const int v = e ? atoi(e) : 0; return (uint32_t)(v >= 1 && v <= kFoldCtasPerSm ? v : kFoldCtasPerSm); }();
-    cfg.gridDim = dim3(148u * fold_ctas);
+    cfg.gridDim = dim3(148u * (uint32_t)kFoldCtasPerSm);
     cfg.blockDim = dim3(kRouteThreads);
     cfg.stream = st;
     // programmatic stream serialization: the fold may start while the kernel in front of it in the stream (the logging
