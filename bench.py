@@ -376,23 +376,30 @@ def main():
           "achieved": (p_events * EVENT_BYTES + p_spikes * SOURCE_BYTES) / max(a4_s, 1e-12) / 1e9}
     a4["frac"] = a4["achieved"] / peak
     if queue_mode and a4_s > 0:
-        # the delivery kernel's real ceiling is the SMs' load/store units, not HBM (DESIGN.md 6.3 "LSU accounting"):
-        # ~1.7 LSU cycles per event per SM (scattered RED 1.3 + record store 0.3 + coalesced loads 0.1)
-        sm_hz = 1.965e9
-        lsu_peak = 148 * sm_hz / 1.7
-        a4["lsu"] = {"bound": "lsu-issue", "achieved": p_events / a4_s, "peak": lsu_peak, "unit": "events/s",
-                     "frac": p_events / a4_s / lsu_peak,
-                     "peak_source": "148 SMs x 1.965 GHz / 1.7 LSU cycles per event (B300_MICROARCH.md atomics table: REDG "
-                                    "1.29 cycles per lane; DESIGN.md 6.3; measured scattered-RED ceiling in "
-                                    "profiles/r02_red_ceiling.md)"}
+        # what bounds event delivery is not HBM but the L2's atomic path: one int32 reduction per event is the
+        # least any atomic delivery does, and the fold gathers each event's 8-byte edge in short random segments on top.  Both
+        # ceilings are MEASURED here, on this device, with the bare access pattern (gn_debug_ceilings).
+        group = args.queue_group or 8
+        seg = max(1, int(round(E / N * group / cfg["ring_slots"])))
+        red_only, gather_red = gn.gn_debug_ceilings(seg, device=dev)
+        fold_s = kms[3] * 1e-3
+        a4["atomic_path"] = {"bound": "l2-atomics", "unit": "events/s", "achieved": p_events / max(fold_s, 1e-12),
+                             "peak": gather_red, "frac": p_events / max(fold_s, 1e-12) / gather_red,
+                             "achieved_incl_logging": p_events / a4_s, "frac_incl_logging": p_events / a4_s / gather_red,
+                             "red_only_peak": red_only, "segment_edges": seg,
+                             "peak_source": "measured in this run by gn_debug_ceilings: scattered int32 RED.ADD into a 16 MB "
+                                            "L2-resident region, each preceded by the gather of its 8-byte edge in random "
+                                            f"{seg}-edge segments of a 2 GB array (red_only_peak: the reductions alone); "
+                                            "achieved = delivered events / summed gn_fold_kernel time"}
     dom = max(kernels, key=lambda r: r["share"])
     roofline = {"bound": "hbm", "kernel": dom["kernel"], "achieved": dom["achieved"], "peak": peak, "unit": "GB/s",
                 "frac": dom["frac"], "traffic": dom.get("traffic"), "traffic_source": traffic_src if "traffic" in dom else None,
                 "dram_frac": dom.get("dram_frac"), "peak_source": peak_src,
                 "note": "achieved / frac = ALGORITHMIC bytes over the live CUDA-event time (the contract's definition); "
-                        "dram_frac = DRAM bytes ncu counted for this kernel over the same live time: the update kernel's "
-                        "state is L2-resident and the delivery kernel is bound by scattered-RED issue, so neither is "
-                        "HBM-bound in the strict sense (DESIGN.md 7)",
+                        "dram_frac = DRAM bytes ncu counted for this kernel (traffic) over the same live time.  Neither kernel is "
+                        "HBM-bound in the strict sense: the update kernel's state is largely L2-resident, and the fold kernel is "
+                        "bound by the L2's atomic path -- a4_delivery.atomic_path rates it against that ceiling, measured in "
+                        "this run (DESIGN.md 6.3, 7)",
                 "timing": "the SAME K steps as the timed pass, replayed from rest on a fresh handle with a CUDA event at every "
                           "kernel boundary (gn_profile; serialised on one stream)",
                 "kernels": kernels, "a4_delivery": a4, "profile_pass_events_per_sim_step": p_events / sim_steps,

@@ -223,6 +223,14 @@ int gn_observe(gn_net *net, uint64_t frame0, uint64_t n_frames, float *trace, si
 int gn_debug_words(void *cuda_stream, uint64_t seed, uint32_t stream_id, uint64_t idx,
                    uint32_t first_vertex, uint32_t n, uint32_t *out);
 
+/* Benchmark hook: the measured ceilings of event delivery's access pattern on this device, with everything
+ * else of the kernels stripped off.  out[0] = scattered int32 reductions per second into a 16 MB region (one per event is
+ * the least any atomic delivery does); out[1] = the same with each reduction's 8-byte edge gathered first, in random
+ * contiguous segments of `segment_edges` edges from the rest of `scratch` (what folding a slot group does; mean segment
+ * = out-degree x queue_group / ring_slots).  `scratch` is DEVICE memory, >= 320 MB (the edge array should dwarf L2), and is
+ * overwritten.  Synchronises.  Errors: INVALID_ARG, CUDA. */
+int gn_debug_ceilings(void *cuda_stream, void *scratch, size_t scratch_bytes, uint32_t segment_edges, double out[2]);
+
 /* Per-kernel timing for benchmarks.  While enabled, gn_step runs every kernel on the net's stream (no overlap
  * between update and delivery) with a CUDA event wherever the kind of kernel changes, and synchronises every
  * few hundred steps to collect them: a measuring mode, never the mode a throughput number is taken in.  A run

@@ -87,6 +87,17 @@ class PullSimulator:
         self.tau_ca = f32(cfg["tau_ca_ms"])
         self.ca_jump = f32(cfg["ca_jump"])
 
+    def _arrivals(self, j, t):
+        """eq. 30: sum of w_kj * spd(V_k(t - tau_kj)) over the in-edges of j, from the raster history (fixed point)."""
+        I_fx = 0
+        for (k, w_fx, dl) in self.in_edges[j]:
+            if t - dl >= 0 and self.raster[t - dl][k]:
+                I_fx += w_fx
+        return I_fx
+
+    def _after_step(self, t, fired_now):
+        """Hook for transition functions beyond the vertex states (oracle/stdp_definition.py)."""
+
     def step(self, n_steps=1):
         for _ in range(n_steps):
             t = len(self.raster)
@@ -96,11 +107,7 @@ class PullSimulator:
             p2 = self.p[:]
             for j in range(self.n):
                 q = self.classes[self.cls[j]]
-                # eq. 30: sum of w_kj * spd(V_k(t - tau_kj)) over in-edges, from the raster history
-                I_fx = 0
-                for (k, w_fx, dl) in self.in_edges[j]:
-                    if t - dl >= 0 and self.raster[t - dl][k]:
-                        I_fx += w_fx
+                I_fx = self._arrivals(j, t)
                 thr = math.floor(q["drive_rate_hz"] * self.dt * 1e-3 * 4294967296.0)
                 if thr > 0 and word(self.seed, 5, j, t) < thr:
                     I_fx += quantise(q["drive_kick"])
@@ -132,3 +139,4 @@ class PullSimulator:
             self.p = p2
             self.raster.append(fired_now)
             self.consumed.append(consumed)
+            self._after_step(t, fired_now)

@@ -45,7 +45,7 @@ class gn_config(C.Structure):
 
 
 EXPORTS = ("gn_query_workspace", "gn_create", "gn_step", "gn_read_state", "gn_write_state",
-           "gn_read_raster", "gn_observe", "gn_debug_words", "gn_profile", "gn_profile_read", "gn_last_error",
+           "gn_read_raster", "gn_observe", "gn_debug_words", "gn_debug_ceilings", "gn_profile", "gn_profile_read", "gn_last_error",
            "gn_destroy")
 
 _lib = None
@@ -65,6 +65,7 @@ def lib() -> C.CDLL:
         L.gn_read_raster.argtypes = [vp, u64, u64, vp, sz, i32]
         L.gn_observe.argtypes = [vp, u64, u64, vp, sz, i32]
         L.gn_debug_words.argtypes = [vp, u64, u32, u64, u32, u32, vp]
+        L.gn_debug_ceilings.argtypes = [vp, vp, sz, u32, vp]
         L.gn_profile.argtypes = [vp, i32]
         L.gn_profile_read.argtypes = [vp, vp, vp]
         L.gn_last_error.argtypes = [vp]
@@ -213,6 +214,18 @@ def gn_debug_words(seed: int, stream_id: int, idx: int, first_vertex: int, n: in
     _check(lib().gn_debug_words(C.c_void_p(st.cuda_stream), seed, stream_id, idx, first_vertex, n,
                                 C.c_void_p(out.data_ptr())))
     return out.cpu().numpy().view(np.uint32)
+
+
+def gn_debug_ceilings(segment_edges: int, scratch_mb: int = 2048, device="cuda:0"):
+    """(scattered reductions / s, gathers of `segment_edges`-edge segments + reductions / s) measured on the device."""
+    import torch
+    scratch = torch.empty(int(scratch_mb) << 20, dtype=torch.uint8, device=device)
+    st = torch.cuda.current_stream(scratch.device)
+    out = (C.c_double * 2)()
+    with torch.cuda.device(scratch.device):
+        _check(lib().gn_debug_ceilings(C.c_void_p(st.cuda_stream), C.c_void_p(scratch.data_ptr()), scratch.numel(),
+                                       int(segment_edges), out))
+    return float(out[0]), float(out[1])
 
 
 def gn_profile(net: GnNet, enable: bool) -> None:

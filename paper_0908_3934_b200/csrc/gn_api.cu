@@ -906,6 +906,19 @@ int gn_debug_words(void *cuda_stream, uint64_t seed, uint32_t stream_id, uint64_
     return GN_OK;
 }
 
+int gn_debug_ceilings(void *cuda_stream, void *scratch, size_t scratch_bytes, uint32_t segment_edges, double out[2])
+{
+    if (!scratch || !out) return set_err(nullptr, GN_E_INVALID_ARG, "NULL argument");
+    cudaPointerAttributes attr{};
+    GN_CUDA(nullptr, cudaPointerGetAttributes(&attr, scratch));
+    if (attr.type != cudaMemoryTypeDevice && attr.type != cudaMemoryTypeManaged)
+        return set_err(nullptr, GN_E_INVALID_ARG, "scratch is not device memory");
+    if (scratch_bytes < (320u << 20) || segment_edges == 0) return set_err(nullptr, GN_E_INVALID_ARG, "scratch must hold at least 320 MB and segment_edges be > 0");
+    DeviceGuard guard(attr.device);
+    GN_CUDA(nullptr, gnk_ceilings(scratch, scratch_bytes, segment_edges, out, (cudaStream_t)cuda_stream));
+    return GN_OK;
+}
+
 const char *gn_last_error(const gn_net *net) { return net ? net->err : g_create_error; }
 
 int gn_destroy(gn_net *net)

@@ -47,6 +47,12 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
     out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
+// One int32 reduction with no return value (RED.ADD), spelled out.
+__device__ __forceinline__ void ring_add(int32_t *cell, const int32_t w)
+{
+    asm volatile("red.relaxed.gpu.global.add.s32 [%0], %1;" ::"l"(cell), "r"(w) : "memory");
+}
+
 // ---- one vertex, one step: eq. 24 + :303 eq. 28 + :283-286 eq. 26 ------------
 // Reads the state at t, writes the state at t+1, returns spd(V(t)) gated by refractoriness.
 template <bool BIAS, bool ALPHA>
@@ -1360,6 +1366,42 @@ __global__ void gn_debug_words_kernel(const uint32_t seed_lo, const uint32_t see
     out[i] = x[j & 3u];
 }
 
+// ---- measured ceilings of the delivery pattern (gn_debug_ceilings: the roofline bench.py rates a4 against) -----------
+// Scattered int32 reductions into a region of `mask + 1` words that stays in L2 -- and the same preceded by the gather of
+// the 8-byte edge each reduction carries, read in random contiguous segments of seg_len edges (unaligned starts) from an
+// array far larger than L2, 32 edges per load instruction, four loads in flight per warp: the access pattern of
+// gn_fold_kernel with everything else stripped off.
+__device__ __forceinline__ uint32_t ceil_mix(uint32_t x)
+{
+    x ^= x >> 16; x *= 0x7feb352du; x ^= x >> 15; x *= 0x846ca68bu; x ^= x >> 16;
+    return x;
+}
+
+template <bool GATHER>
+__global__ void __launch_bounds__(256)
+gn_ceiling_kernel(int32_t *region, const uint32_t mask, const uint2 *edges, const uint32_t n_edges, const uint32_t seg_len,
+                  const uint32_t iters, const uint32_t seed)
+{
+    const uint32_t lane = threadIdx.x & 31u, gw = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    for (uint32_t it = 0; it < iters; it += 4u) {
+        uint2 e[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const uint32_t slot = (it + u) * 32u + lane;
+            if (GATHER) {
+                const uint32_t seg = slot / seg_len, k = slot - seg * seg_len;
+                const uint32_t start = ceil_mix(gw * 0x9E3779B9u + seg * 0x85EBCA6Bu + seed) % (n_edges - seg_len);
+                e[u] = __ldcs(edges + start + k);
+                e[u].x ^= ceil_mix(slot + gw);
+            } else {
+                e[u] = make_uint2(ceil_mix(ceil_mix(gw * 0x9E3779B9u + seed) + slot), 1u);
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) ring_add(region + (e[u].x & mask), (int32_t)e[u].y);
+    }
+}
+
 inline uint32_t ceil_div(uint64_t a, uint64_t b) { return (uint32_t)((a + b - 1) / b); }
 
 }  // namespace
@@ -1629,4 +1671,42 @@ cudaError_t gnk_debug_words(uint64_t seed, uint32_t stream_id, uint64_t idx, uin
     if (n == 0) return cudaSuccess;
     gn_debug_words_kernel<<<ceil_div(n, 256), 256, 0, st>>>((uint32_t)seed, (uint32_t)(seed >> 32), stream_id, idx, first, n, out);
     return cudaGetLastError();
+}
+
+// out[0] = scattered reductions per second into a 16 MB region; out[1] = gathers of seg_len-edge segments + reductions
+// per second.  `scratch` (>= 64 MB + 256 MB; the larger the better: the edge array should dwarf L2) is overwritten.
+// Best of 5 launches each, timed with CUDA events on `st`; synchronises.
+cudaError_t gnk_ceilings(void *scratch, size_t scratch_bytes, uint32_t seg_len, double out[2], cudaStream_t st)
+{
+    const size_t region_bytes = 16u << 20;
+    if (scratch_bytes < (64u << 20) + (256u << 20) || seg_len == 0u) return cudaErrorInvalidValue;
+    int32_t *region = reinterpret_cast<int32_t *>(scratch);
+    const uint2 *edges = reinterpret_cast<const uint2 *>(reinterpret_cast<uint8_t *>(scratch) + (64u << 20));
+    size_t n_edges = (scratch_bytes - (64u << 20)) / 8;
+    if (n_edges > 0xFFFFFF00ull) n_edges = 0xFFFFFF00ull;
+    cudaError_t e = cudaMemsetAsync(scratch, 1, scratch_bytes, st);
+    cudaEvent_t e0, e1;
+    if (e == cudaSuccess) e = cudaEventCreate(&e0);
+    if (e != cudaSuccess) return e;
+    e = cudaEventCreate(&e1);
+    if (e != cudaSuccess) { cudaEventDestroy(e0); return e; }
+    const uint32_t grid = 148u * 8u, iters = 64u, mask = (uint32_t)(region_bytes / 4 - 1);
+    const double n = (double)grid * 256.0 * iters;
+    for (int mode = 0; mode < 2 && e == cudaSuccess; ++mode) {
+        float best = 1e30f;
+        for (int rep = 0; rep < 5 && e == cudaSuccess; ++rep) {
+            cudaEventRecord(e0, st);
+            if (mode == 0) gn_ceiling_kernel<false><<<grid, 256, 0, st>>>(region, mask, edges, (uint32_t)n_edges, seg_len, iters, 7919u * rep);
+            else gn_ceiling_kernel<true><<<grid, 256, 0, st>>>(region, mask, edges, (uint32_t)n_edges, seg_len, iters, 7919u * rep);
+            cudaEventRecord(e1, st);
+            e = cudaEventSynchronize(e1);
+            float ms = 0.f;
+            if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+            if (ms < best) best = ms;
+        }
+        out[mode] = n / ((double)best * 1e-3);
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    return e;
 }
