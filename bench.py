@@ -108,14 +108,14 @@ class ClockSampler:
 
 
 def measured_traffic():
-    """Per-launch DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of each kernel from the committed
-    `ncu --set full` capture: profiles/traffic.csv, whose first line names the capture and its step range."""
+    """DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of each kernel from the committed `ncu --set full` captures:
+    profiles/traffic.csv, whose first line names the capture and its step range.  {kernel: (per launch, per event or None)}."""
     path = os.path.join(ROOT, "profiles", "traffic.csv")
     try:
         lines = [l.strip() for l in open(path).read().splitlines() if l.strip()]
         src = lines[0].lstrip("# ") if lines[0].startswith("#") else "profiles/traffic.csv"
-        rows = [l for l in lines if not l.startswith("#")][1:]
-        return {k: float(v) for k, v in (r.split(",")[:2] for r in rows)}, src
+        rows = [l.split(",") for l in lines if not l.startswith("#")][1:]
+        return {r[0]: (float(r[1]), float(r[2]) if len(r) > 2 and r[2] else None) for r in rows}, src
     except Exception:
         return {}, None
 
@@ -342,7 +342,9 @@ def main():
     peak, peak_src = peaks()
     queue_mode = 0 < kn[1] < kn[0]      # queue mode delivers once per slot group, ring mode every step
     resident = kn[1] == 0 and kn[0] < sim_steps
-    names = ["gn_resident_kernel (a1-a5, one CTA or cluster per network)" if resident else
+    persist = resident and net_in.n_networks == 1 and N > 16384
+    names = ["gn_persist_kernel (a1-a5, one cooperative launch per call)" if persist else
+             "gn_resident_kernel (a1-a5, one CTA or cluster per network)" if resident else
              "gn_update_kernel (a1-a3 + a4 fused)" if kn[1] == 0 else "gn_update_kernel (a1-a3)",
              "gn_log_kernel (a3 compaction + a4: spikes into the log)" if queue_mode else "gn_deliver_kernel (a4)",
              "gn_observe_kernel (a5)", "gn_fold_kernel (a4: expansion of the log + ring reductions)"]
@@ -367,8 +369,8 @@ def main():
                "bytes_per_launch": kbytes[k], "achieved": kbytes[k] / avg_s / 1e9, "frac": kbytes[k] / avg_s / 1e9 / peak}
         tr = traffic_tab.get(names[k].split()[0])
         if tr is not None:      # what DRAM really moved for this kernel (ncu capture named in traffic_source) over the live time
-            row["traffic"] = tr
-            row["dram_frac"] = tr / avg_s / 1e9 / peak
+            row["traffic"] = tr[1] * p_events / kn[k] if tr[1] is not None else tr[0]
+            row["dram_frac"] = row["traffic"] / avg_s / 1e9 / peak
         kernels.append(row)
     a4_s = (kms[1] + kms[3]) * 1e-3
     a4 = {"what": "a4 delivery as a whole (routing + folding), 17 B per event + 12 B per fired source",
@@ -384,13 +386,15 @@ def main():
         red_only, gather_red = gn.gn_debug_ceilings(seg, device=dev)
         fold_s = kms[3] * 1e-3
         a4["atomic_path"] = {"bound": "l2-atomics", "unit": "events/s", "achieved": p_events / max(fold_s, 1e-12),
-                             "peak": gather_red, "frac": p_events / max(fold_s, 1e-12) / gather_red,
-                             "achieved_incl_logging": p_events / a4_s, "frac_incl_logging": p_events / a4_s / gather_red,
-                             "red_only_peak": red_only, "segment_edges": seg,
+                             "peak": red_only, "frac": p_events / max(fold_s, 1e-12) / red_only,
+                             "achieved_incl_logging": p_events / a4_s, "frac_incl_logging": p_events / a4_s / red_only,
+                             "gather_plus_red_reference": gather_red, "segment_edges": seg,
                              "peak_source": "measured in this run by gn_debug_ceilings: scattered int32 RED.ADD into a 16 MB "
-                                            "L2-resident region, each preceded by the gather of its 8-byte edge in random "
-                                            f"{seg}-edge segments of a 2 GB array (red_only_peak: the reductions alone); "
-                                            "achieved = delivered events / summed gn_fold_kernel time"}
+                                            "L2-resident region, one per event -- the least any atomic delivery does "
+                                            "(gather_plus_red_reference: the same loop with each event's 8-byte edge gathered "
+                                            f"first, in random {seg}-edge segments of a 2 GB array: a reference point, not a "
+                                            "ceiling -- the fold kernel keeps more loads in flight); achieved = delivered "
+                                            "events / summed gn_fold_kernel time"}
     dom = max(kernels, key=lambda r: r["share"])
     roofline = {"bound": "hbm", "kernel": dom["kernel"], "achieved": dom["achieved"], "peak": peak, "unit": "GB/s",
                 "frac": dom["frac"], "traffic": dom.get("traffic"), "traffic_source": traffic_src if "traffic" in dom else None,

@@ -110,6 +110,13 @@ typedef struct {
     uint64_t queue_capacity;        /* queue mode: spikes of one step the spike log holds; later ones */
                                     /* are expanded on the spot (direct ring adds); 0 = default       */
                                     /* max(1024, N / 16)                                              */
+    /* Plasticity (eq. 32-33, readings #22, #23).  stdp_alpha != 0 makes every weight a state   */
+    /* of its own: w_ij(t+dt) = w_ij(t) + dt alpha sign(q) exp(-beta |q|), q = s~_i(t - tau_ij) - s~_j(t) whenever the      */
+    /* spike of i arrives at j or j fires at t (s~: time since the last spike, 0 for a vertex spiking at the step).  An   */
+    /* arriving spike is weighed with the weight AT THE ARRIVAL step (eq. 30), so delivery then happens at arrival time:  */
+    /* delivery_mode must be AUTO or RING, observation and checkpoint writes of RING / STEP are not supported with it.    */
+    float    stdp_alpha;            /* per ms; 0 = static weights                                     */
+    float    stdp_beta;             /* 1/ms, >= 0                                                     */
 } gn_config;
 
 /* delivery_mode.
@@ -151,7 +158,8 @@ enum {
     GN_P = 11,        /* float  [N]      second PSC state p of the alpha-function (zero for other classes) */
     GN_ACC = 12,      /* float  [N]      sum of c over the steps of the camera frame in progress (obs_stride > 0) */
     GN_M = 13,        /* float  [N]      sodium activation m of Hodgkin-Huxley vertices (zero for other classes)  */
-    GN_H = 14         /* float  [N]      sodium inactivation h of Hodgkin-Huxley vertices (zero for other classes) */
+    GN_H = 14,        /* float  [N]      sodium inactivation h of Hodgkin-Huxley vertices (zero for other classes) */
+    GN_WEIGHTS = 15   /* float  [E]      current weight of every edge, caller's edge order (plastic: evolving; else w_fx 2^-16) */
 };
 
 /* Bytes of device workspace gn_create needs for this configuration.

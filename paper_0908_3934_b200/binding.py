@@ -16,7 +16,7 @@ GN_OK = 0
 GN_E_INVALID_ARG, GN_E_BAD_GRAPH, GN_E_OVERFLOW_RISK = -1, -2, -3
 GN_E_WORKSPACE_TOO_SMALL, GN_E_RANGE_EVICTED, GN_E_CUDA = -4, -5, -6
 (GN_V, GN_W, GN_R, GN_CA, GN_REFR, GN_RING, GN_STEP, GN_COUNTERS, GN_DELAYS, GN_WEIGHTS_FX, GN_BIAS, GN_P, GN_ACC, GN_M,
- GN_H) = range(15)
+ GN_H, GN_WEIGHTS) = range(16)
 GN_MODEL_IZHIKEVICH, GN_MODEL_HODGKIN_HUXLEY = 0, 1
 GN_MAX_CLASSES = 8
 GN_DELIVER_AUTO, GN_DELIVER_RING, GN_DELIVER_QUEUE, GN_DELIVER_RESIDENT = 0, 1, 2, 3
@@ -41,7 +41,7 @@ class gn_config(C.Structure):
                 ("obs_sigma", C.c_float), ("obs_stride", C.c_uint32),
                 ("raster_capacity_steps", C.c_uint32), ("trace_capacity_frames", C.c_uint32),
                 ("seed", C.c_uint64), ("delivery_mode", C.c_uint32), ("queue_group", C.c_uint32),
-                ("queue_capacity", C.c_uint64)]
+                ("queue_capacity", C.c_uint64), ("stdp_alpha", C.c_float), ("stdp_beta", C.c_float)]
 
 
 EXPORTS = ("gn_query_workspace", "gn_create", "gn_step", "gn_read_state", "gn_write_state",
@@ -103,10 +103,10 @@ def _ptr(a):
 def make_config(n_vertices, dim, n_edges, ring_slots, dt_ms, speed, n_classes, *, n_networks=1, tau_ca_ms=500.0,
                 ca_jump=1.0, obs_gain=1.0, obs_offset=0.0, obs_sigma=0.0, obs_stride=0, raster_capacity_steps=0,
                 trace_capacity_frames=0, seed=0, delivery_mode=GN_DELIVER_AUTO, queue_group=0,
-                queue_capacity=0) -> gn_config:
+                queue_capacity=0, stdp_alpha=0.0, stdp_beta=0.0) -> gn_config:
     return gn_config(n_vertices, dim, n_edges, n_networks, ring_slots, dt_ms, speed, n_classes, tau_ca_ms, ca_jump,
                      obs_gain, obs_offset, obs_sigma, obs_stride, raster_capacity_steps, trace_capacity_frames, seed,
-                     delivery_mode, queue_group, queue_capacity)
+                     delivery_mode, queue_group, queue_capacity, stdp_alpha, stdp_beta)
 
 
 def gn_query_workspace(cfg: gn_config) -> int:
@@ -163,12 +163,12 @@ def gn_step(net: GnNet, n_steps: int) -> None:
 _STATE_DTYPE = {GN_V: np.float32, GN_W: np.float32, GN_R: np.float32, GN_CA: np.float32, GN_REFR: np.uint8,
                 GN_RING: np.int32, GN_STEP: np.uint64, GN_COUNTERS: np.uint64, GN_DELAYS: np.uint8,
                 GN_WEIGHTS_FX: np.int32, GN_BIAS: np.float32, GN_P: np.float32, GN_ACC: np.float32, GN_M: np.float32,
-                GN_H: np.float32}
+                GN_H: np.float32, GN_WEIGHTS: np.float32}
 
 
 def _state_shape(net, which):
     return {GN_RING: (net.d, net.n), GN_STEP: (1,), GN_COUNTERS: (4,), GN_DELAYS: (net.e,),
-            GN_WEIGHTS_FX: (net.e,)}.get(which, (net.n,))
+            GN_WEIGHTS_FX: (net.e,), GN_WEIGHTS: (net.e,)}.get(which, (net.n,))
 
 
 def gn_read_state(net: GnNet, which: int, out=None):
@@ -246,7 +246,7 @@ def gn_destroy(net: GnNet) -> None:
 
 def create_from_inputs(net_in, cfg_in, *, delays=None, bias=None, raster_capacity_steps=0,
                        trace_capacity_frames=0, device="cuda:0", delivery_mode=GN_DELIVER_AUTO, queue_group=0,
-                       queue_capacity=0) -> GnNet:
+                       queue_capacity=0, stdp_alpha=0.0, stdp_beta=0.0) -> GnNet:
     """Convenience: build from a gn_inputs.Network + config dict (marshalling only)."""
     obs = int(cfg_in.get("obs_stride", 0))
     cfg = make_config(net_in.n_vertices, net_in.dim, net_in.n_edges, cfg_in["ring_slots"], cfg_in["dt_ms"],
@@ -255,7 +255,8 @@ def create_from_inputs(net_in, cfg_in, *, delays=None, bias=None, raster_capacit
                       obs_offset=cfg_in["obs_offset"], obs_sigma=cfg_in["obs_sigma"], obs_stride=obs,
                       raster_capacity_steps=raster_capacity_steps,
                       trace_capacity_frames=trace_capacity_frames if obs else 0, seed=cfg_in["seed"],
-                      delivery_mode=delivery_mode, queue_group=queue_group, queue_capacity=queue_capacity)
+                      delivery_mode=delivery_mode, queue_group=queue_group, queue_capacity=queue_capacity,
+                      stdp_alpha=stdp_alpha, stdp_beta=stdp_beta)
     return gn_create(cfg, cfg_in["classes"], net_in.positions, net_in.row_offsets, net_in.targets, net_in.weights,
                      None if delays is None else np.ascontiguousarray(delays, dtype=np.uint8),
                      net_in.vertex_class,

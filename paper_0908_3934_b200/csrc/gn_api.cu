@@ -19,6 +19,7 @@ thread_local char g_create_error[256] = "";
 struct Layout {
     size_t V, W, r, p2, hm, hh, c, acc, bias, refr, cls, ring, row, tgt, wfx, dly, counters, q_count;
     size_t s_edge, s_dly, min_dly, q_seg, spk_log;
+    size_t w_f32, perm, ls_hist, csc_off, csc_edge, csc_src, w_stage;
     size_t raster, trace, scratch_row64, scratch_abs, scratch_pos, scratch_net, scratch_chk, total;
 };
 
@@ -38,6 +39,12 @@ int check_config(const gn_config *cfg, char *err, size_t errn)
     if (cfg->obs_stride > 0 && cfg->trace_capacity_frames == 0) return fail("obs_stride > 0 needs trace_capacity_frames > 0");
     if (cfg->obs_stride > 0 && !(cfg->tau_ca_ms > 0.0f)) return fail("obs_stride > 0 needs tau_ca_ms > 0");
     if (cfg->delivery_mode > GN_DELIVER_RESIDENT) return fail("delivery_mode must be GN_DELIVER_AUTO, _RING, _QUEUE or _RESIDENT");
+    if (cfg->stdp_alpha != 0.0f) {
+        if (!(cfg->stdp_beta >= 0.0f) || !isfinite(cfg->stdp_alpha) || !isfinite(cfg->stdp_beta)) return fail("stdp_alpha must be finite and stdp_beta finite and >= 0");
+        if (cfg->delivery_mode != GN_DELIVER_AUTO && cfg->delivery_mode != GN_DELIVER_RING)
+            return fail("plastic weights (stdp_alpha != 0) need delivery_mode GN_DELIVER_AUTO or GN_DELIVER_RING");
+        if (cfg->obs_stride > 0) return fail("plastic weights (stdp_alpha != 0) do not support observation (obs_stride > 0)");
+    }
     const uint32_t qg = cfg->queue_group;
     if (qg != 0 && (qg > 16 || (qg & (qg - 1)) != 0)) return fail("queue_group must be 0 or a power of two in 1..16");
     return GN_OK;
@@ -61,7 +68,7 @@ QueuePlan make_plan(const gn_config *cfg)
     while (group > 1 && D % group != 0) group >>= 1;      // the ring depth must be a whole number of groups
     q.on = cfg->delivery_mode == GN_DELIVER_QUEUE ||
            (cfg->delivery_mode == GN_DELIVER_AUTO && D >= 32 && D * Npad * 4 > (48ull << 20));
-    if (E == 0) q.on = false;
+    if (E == 0 || cfg->stdp_alpha != 0.0f) q.on = false;    // plastic weights: delivery at arrival time (gn_arrive_kernel)
     q.q_log = 0;
     while ((1u << q.q_log) < group) q.q_log++;
     q.q_nb = (uint32_t)(D / group);
@@ -93,13 +100,18 @@ Layout make_layout(const gn_config *cfg)
     L.q_count = take(256 * 8);       // +0: the persistent step driver's barrier counter; +64: spikes logged per step slot
     {
         size_t rows = cfg->raster_capacity_steps, need_rows = qp.on ? (size_t)(kQueueWindow + 1u) << qp.q_log : 2;
+        if (cfg->stdp_alpha != 0.0f) need_rows = D;     // plastic mode: the raster is the spikes in flight
         if (rows < need_rows) rows = need_rows;
         L.raster = take(rows * (Npad / 32) * 4);
     }
     L.trace = take(obs ? (size_t)cfg->trace_capacity_frames * Npad * 4 : 0);
     L.min_dly = take(Npad);
     L.s_edge = take(E * 8); L.s_dly = take(E);   // every row again, sorted by delay
-    L.q_seg = take(qp.on ? N * D * 2 : 0);
+    const bool plastic = cfg->stdp_alpha != 0.0f;
+    L.q_seg = take(qp.on || plastic ? N * D * 2 : 0);
+    L.w_f32 = take(plastic ? E * 4 : 0); L.perm = take(plastic ? E * 4 : 0); L.w_stage = take(plastic ? E * 4 : 0);
+    L.ls_hist = take(plastic ? D * Npad * 4 : 0);
+    L.csc_off = take(plastic ? (Npad + 2) * 4 : 0); L.csc_edge = take(plastic ? E * 4 : 0); L.csc_src = take(plastic ? E * 4 : 0);
     L.spk_log = take(qp.on && qp.arrays >= 2 ? D * qp.arrays * (size_t)qp.log_cap * 4 : 0);
     L.scratch_row64 = take((N + 1) * 8); L.scratch_abs = take(N * 8);
     L.scratch_pos = take(N * cfg->dim * 4); L.scratch_net = take(((size_t)cfg->n_networks + 1) * 4);
@@ -274,7 +286,8 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
     const QueuePlan qp = make_plan(cfg);
     d.raster_rows = cfg->raster_capacity_steps;   // the delivery kernels read the spike lists of up to two groups
     {
-        const uint32_t need_rows = qp.on ? (kQueueWindow + 1u) << qp.q_log : 2u;
+        uint32_t need_rows = qp.on ? (kQueueWindow + 1u) << qp.q_log : 2u;
+        if (cfg->stdp_alpha != 0.0f) need_rows = cfg->ring_slots;
         if (d.raster_rows < need_rows) d.raster_rows = need_rows;
     }
     d.queue_mode = qp.on ? 1u : 0u;
@@ -287,6 +300,16 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
     if (qp.on) {
         d.q_seg = (uint16_t *)(ws + L.q_seg);
         d.spk_log = (uint32_t *)(ws + L.spk_log);
+    }
+    if (cfg->stdp_alpha != 0.0f) {       // plastic weights: per-delay boundaries = the segment table with groups of one slot
+        d.plastic = 1u;
+        d.stdp_dta = (float)((double)cfg->dt_ms * (double)cfg->stdp_alpha);
+        d.stdp_beta = cfg->stdp_beta;
+        d.q_log = 0u; d.q_nb = cfg->ring_slots; d.q_arrays = 0u;
+        d.q_seg = (uint16_t *)(ws + L.q_seg);
+        d.w_f32 = (float *)(ws + L.w_f32); d.perm = (uint32_t *)(ws + L.perm); d.w_stage = (float *)(ws + L.w_stage);
+        d.ls_hist = (int32_t *)(ws + L.ls_hist);
+        d.csc_off = (uint32_t *)(ws + L.csc_off); d.csc_edge = (uint32_t *)(ws + L.csc_edge); d.csc_src = (uint32_t *)(ws + L.csc_src);
     }
     d.trace = cfg->obs_stride ? (float *)(ws + L.trace) : nullptr;
     for (uint32_t k = 0; k < cfg->n_classes; ++k) {
@@ -436,7 +459,7 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
         }
         d.n_networks = cfg->n_networks;
         d.net_off = net_d;
-        if (fits && (cfg->delivery_mode == GN_DELIVER_RESIDENT || cfg->delivery_mode == GN_DELIVER_AUTO)) {
+        if (fits && !d.plastic && (cfg->delivery_mode == GN_DELIVER_RESIDENT || cfg->delivery_mode == GN_DELIVER_AUTO)) {
             d.resident = 1u;
             d.res_cluster = cluster;
             d.res_threads = threads;
@@ -445,7 +468,7 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
         }
     }
     // ring mode on a small network: one kernel per step (the update delivers), bound by launch latency not work
-    d.fused = (!d.resident && !d.queue_mode && Npad <= (1u << 18)) ? 1u : 0u;
+    d.fused = (!d.resident && !d.queue_mode && !d.plastic && Npad <= (1u << 18)) ? 1u : 0u;
     // ... and when its whole update grid can be co-resident, one cooperative launch per gn_step call (gn_persist_kernel).
     // GN_NO_PERSIST (environment): measurements of the per-step path only.
     if (d.fused && !getenv("GN_NO_PERSIST")) {
@@ -461,6 +484,12 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
     GN_CREATE_CUDA(gnk_check_overflow(d, abs_in, chk_d, st));
     GN_CREATE_CUDA(cudaMemsetAsync(d.min_dly, 0xFF, Npad, st));
     if (E) GN_CREATE_CUDA(gnk_sort_rows(d, chk_d, st));
+    if (d.plastic) {                     // in-edge lists (scratch: the per-target sums, no longer needed), no spike yet
+        GN_CREATE_CUDA(cudaMemsetAsync(d.csc_off, 0, ((size_t)Npad + 2) * 4, st));
+        GN_CREATE_CUDA(cudaMemsetAsync(abs_in, 0, (size_t)N * 4, st));
+        GN_CREATE_CUDA(gnk_build_csc(d, E, (uint32_t *)abs_in, st));
+        GN_CREATE_CUDA(cudaMemsetAsync(d.ls_hist, 0xFF, (size_t)cfg->ring_slots * Npad * 4, st));
+    }
     GN_CREATE_CUDA(cudaMemcpyAsync(&chk, chk_d, sizeof chk, cudaMemcpyDeviceToHost, st));
     GN_CREATE_CUDA(cudaStreamSynchronize(st));
 #undef GN_CREATE_CUDA
@@ -623,6 +652,17 @@ int gn_step(gn_net *net, uint64_t n_steps)
         }
         return GN_OK;
     }
+    if (d.plastic) {       // plastic weights: arrivals of step t, the update, then eq. 33 and eq. 32, all on the caller's stream
+        for (uint64_t s = 0; s < n_steps; ++s) {
+            const uint64_t t = net->t;
+            GN_CUDA(net, gnk_arrive(d, t, net->t_origin, net->stream));
+            GN_CUDA(net, gnk_update(d, t, net->has_bias, net->stream));
+            GN_CUDA(net, gnk_plasticity(d, t, net->t_origin, net->stream));
+            net->launches += 5;
+            net->t = t + 1;
+        }
+        return GN_OK;
+    }
     if (d.persist) {       // ring mode, co-resident grid: the whole call is one cooperative launch
         uint64_t left = n_steps;
         while (left) {
@@ -775,10 +815,14 @@ int gn_read_state(gn_net *net, int which, void *dst, size_t dst_bytes, int dst_i
     }
     case GN_DELAYS: src = d.dly; need = E; break;
     case GN_WEIGHTS_FX: src = d.wfx; need = E * 4; break;
+    case GN_WEIGHTS:
+        if (!d.plastic) return set_err(net, GN_E_INVALID_ARG, "GN_WEIGHTS is the evolving weights of a plastic network (stdp_alpha != 0); static ones are GN_WEIGHTS_FX");
+        src = d.w_stage; need = E * 4; break;
     default: return set_err(net, GN_E_INVALID_ARG, "unknown state id %d", which);
     }
     if (dst_bytes < need) return set_err(net, GN_E_INVALID_ARG, "dst has %zu bytes, need %zu", dst_bytes, need);
     if (need == 0) return GN_OK;
+    if (which == GN_WEIGHTS) GN_CUDA(net, gnk_weights_out(d, E, net->stream));     // back to the caller's edge order
     if (which == GN_RING) {   // internal rows are Npad wide; the caller's are N wide
         int rc = flush_delivery(net, true);
         if (rc) return rc;
@@ -820,6 +864,8 @@ int gn_write_state(gn_net *net, int which, const void *src, size_t src_bytes, in
     default: return set_err(net, GN_E_INVALID_ARG, "state id %d is not writable", which);
     }
     if (src_bytes < need) return set_err(net, GN_E_INVALID_ARG, "src has %zu bytes, need %zu", src_bytes, need);
+    if (d.plastic && (which == GN_RING || which == GN_STEP || which == GN_COUNTERS))
+        return set_err(net, GN_E_INVALID_ARG, "a plastic network (stdp_alpha != 0) cannot be restored from a checkpoint: its spikes in flight are its raster history");
     if (which == GN_RING || which == GN_STEP || which == GN_COUNTERS) {      // checkpoint / restore
         int rc = flush_delivery(net, true);       // queue mode: every pending record goes into the ring first, buckets end empty
         if (rc) return rc;

@@ -87,6 +87,14 @@ struct GnDev {
     uint32_t q_arrays;       // q_nb - q_window + 1 (0 or 1: nothing is ever logged)
     uint32_t log_cap;        // spikes of one step the log holds; later ones are delivered on the spot
     uint32_t *log_n;         // [D] spikes of step (slot) logged or delivered on the spot (may exceed log_cap)
+    // plastic mode (gn_config.stdp_alpha != 0; eq. 32-33): weights are state, delivery happens at arrival
+    uint32_t plastic;
+    float stdp_dta, stdp_beta;      // (float)(dt * alpha), beta
+    float *w_f32;                   // [E] current weight of s_edge[e] (the int32 in s_edge[e].y is the initial one)
+    uint32_t *perm;                 // [E] caller's edge index of s_edge[e]
+    int32_t *ls_hist;               // [D][Npad] row t mod D: last spike step of every vertex strictly before t (-1: none)
+    uint32_t *csc_off, *csc_edge, *csc_src;   // in-edges by target: [Npad+1] offsets, [E] position in s_edge, [E] source
+    float *w_stage;                 // [E] staging of GN_WEIGHTS read-back (caller's edge order)
     unsigned long long *counters;   // steps, spikes, delivered events, kicks
     unsigned long long *grid_sync;  // the persistent step driver's barrier counter (it only grows)
     uint32_t *raster;        // [raster_rows][words_pad]; row t % raster_rows is step t's spike list
@@ -111,6 +119,11 @@ cudaError_t gnk_deliver(const GnDev &p, uint64_t t, cudaStream_t st);
 cudaError_t gnk_log(const GnDev &p, uint64_t t0, uint32_t n_batch, cudaStream_t st);
 cudaError_t gnk_fold(const GnDev &p, uint64_t t_win, uint32_t n_win, uint64_t g_fold, bool beside_previous, cudaStream_t st);
 cudaError_t gnk_sort_rows(const GnDev &p, GnCheck *chk, cudaStream_t st);
+// plastic mode: in-edge lists (csc_*; csc_off must hold zeros), then per step arrive -> update -> plasticity
+cudaError_t gnk_build_csc(const GnDev &p, uint64_t n_edges, uint32_t *cursor, cudaStream_t st);
+cudaError_t gnk_arrive(const GnDev &p, uint64_t t, uint64_t t_origin, cudaStream_t st);
+cudaError_t gnk_plasticity(const GnDev &p, uint64_t t, uint64_t t_origin, cudaStream_t st);
+cudaError_t gnk_weights_out(const GnDev &p, uint64_t n_edges, cudaStream_t st);
 cudaError_t gnk_observe(const GnDev &p, uint64_t frame, cudaStream_t st);
 cudaError_t gnk_resident(const GnDev &p, uint64_t t0, uint32_t n_steps, bool has_bias, bool raster_on, cudaStream_t st);
 cudaError_t gnk_resident_cluster_ok(const GnDev &p, bool *ok);

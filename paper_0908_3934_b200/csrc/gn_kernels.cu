@@ -818,6 +818,10 @@ gn_sort_rows_kernel(const GnDev p, GnCheck *chk)
             const uint32_t pos = beg + atomicAdd(&h[d], 1u);
             p.s_edge[pos] = make_uint2(p.tgt[e] | (p.packed ? d << 24 : 0u), (uint32_t)p.wfx[e]);
             p.s_dly[pos] = (uint8_t)d;
+            if (p.plastic) {                                // weights become state: they start at the quantised value
+                p.perm[pos] = e;
+                p.w_f32[pos] = __fmul_rn(__int2float_rn(p.wfx[e]), 0x1p-16f);
+            }
         }
         __syncwarp();
     }
@@ -1239,6 +1243,162 @@ gn_persist_kernel(const GnDev p, const uint64_t t0, const uint32_t n_steps, unsi
     if (blockIdx.x == 0 && threadIdx.x == 0) p.counters[0] = t0 + n_steps;
 }
 
+// ---- plastic mode: spike-time dependent plasticity (eq. 32-33; readings #22, #23) ----------
+// Every weight is a state of its own (eq. 9) and eq. 30 weighs an arriving spike with the weight AT THE ARRIVAL step, so
+// nothing is delivered when a vertex fires: per step t
+//   gn_arrive_kernel<false>  for every delay d and every vertex i that fired at t - d (raster row of that step), the edges
+//                            of i with delay exactly d -- a contiguous run of its delay-sorted row, boundaries from the
+//                            per-delay table (q_seg with groups of one slot) -- add rint(w(t) 2^16) to ring[t mod D][target];
+//   gn_update_kernel         as ever (a1-a3); it sends nothing itself;
+//   gn_arrive_kernel<true>   the same enumeration again, now that the spikes of step t are known: an arrival at a target
+//                            that does not fire at t weakens its edge, w -= dt alpha exp(-beta s_j(t));
+//   gn_ltp_kernel            every vertex j that fired at t strengthens each in-edge (i -> j, d) on which nothing arrives
+//                            at t: w += dt alpha exp(-beta s_i(t - d)), the age read from the history of last-spike steps;
+//   gn_age_kernel            eq. 32 as integers: row t+1 of ls_hist = t where the vertex fired, else row t.
+// An edge is touched by at most one thread per step (one arrival per step; weakening needs the target silent,
+// strengthening needs it firing), so the weights need no atomics.  Arithmetic (fp32, one rounded operation each):
+// age = steps * dt with steps = t - last - 1 (eq. 32: the age is 0 for the step after a spike, so steps = 0 is q = 0: no
+// change); dw = (dt alpha) * exp32(-(beta * age)); w +- dw.
+template <bool PACKED>
+__device__ __forceinline__ uint32_t delay_bound(const GnDev &p, const uint32_t i, const uint32_t d, const uint32_t beg, const uint32_t deg)
+{
+    // #edges of vertex i with delay < d, 1 <= d <= D: table entry d - 1 of its line (groups of one slot)
+    return seg_bound<PACKED>(p, p.q_seg + (size_t)i * p.D, d - 1u, d, beg, deg);
+}
+
+__device__ __forceinline__ float stdp_dw(const GnDev &p, const uint32_t steps)
+{
+    const float age = __fmul_rn(__uint2float_rn(steps), p.dt);
+    return __fmul_rn(p.stdp_dta, exp32(-__fmul_rn(p.stdp_beta, age)));
+}
+
+template <bool LTD, bool PACKED>
+__global__ void __launch_bounds__(256)
+gn_arrive_kernel(const GnDev p, const uint64_t t, const uint32_t n_d)
+{
+    const uint32_t idx = blockIdx.x * 256u + threadIdx.x;
+    unsigned long long events = 0ull;
+    if (idx < n_d * p.words_pad) {
+        const uint32_t d = idx / p.words_pad + 1u, w = idx - (d - 1u) * p.words_pad;
+        uint32_t word = p.raster[(size_t)((t - d) % p.raster_rows) * p.words_pad + w];
+        const uint32_t slot = (uint32_t)(t % p.D);
+        const uint32_t *fired_now = p.raster + (size_t)(t % p.raster_rows) * p.words_pad;
+        const int32_t *last = p.ls_hist + (size_t)slot * p.Npad;
+        for (; word; word &= word - 1u) {
+            const uint32_t i = (w << 5) + (uint32_t)__ffs(word) - 1u;
+            const uint32_t beg = p.row[i], deg = p.row[i + 1] - beg;
+            const uint32_t lo = delay_bound<PACKED>(p, i, d, beg, deg), hi = delay_bound<PACKED>(p, i, d + 1u, beg, deg);
+            for (uint32_t e = beg + lo; e < beg + hi; ++e) {
+                const uint32_t m = PACKED ? p.s_edge[e].x & 0xFFFFFFu : p.s_edge[e].x;
+                if (!LTD) {
+                    ring_add(p.ring + (size_t)slot * p.Npad + m, __float2int_rn(__fmul_rn(p.w_f32[e], 65536.0f)));
+                } else if (!((fired_now[m >> 5] >> (m & 31u)) & 1u)) {     // (a coincidence changes nothing)
+                    const int32_t ls = last[m];
+                    if (ls >= 0 && (uint64_t)ls + 1ull < t)
+                        p.w_f32[e] = __fsub_rn(p.w_f32[e], stdp_dw(p, (uint32_t)(t - 1ull - (uint64_t)ls)));
+                }
+            }
+            events += (unsigned long long)(hi - lo);
+        }
+    }
+    if (!LTD) {
+#pragma unroll
+        for (int o = 16; o >= 1; o >>= 1) events += __shfl_xor_sync(0xFFFFFFFFu, events, o);
+        if ((threadIdx.x & 31u) == 0u && events) atomicAdd(&p.counters[2], events);
+    }
+}
+
+// One warp per raster word of step t: every fired vertex in turn, lanes over its in-edges.
+template <bool PACKED>
+__global__ void __launch_bounds__(256)
+gn_ltp_kernel(const GnDev p, const uint64_t t)
+{
+    const uint32_t lane = threadIdx.x & 31u, w = (blockIdx.x * 256u + threadIdx.x) >> 5;
+    if (w >= p.words_pad) return;
+    uint32_t word = p.raster[(size_t)(t % p.raster_rows) * p.words_pad + w];
+    for (; word; word &= word - 1u) {
+        const uint32_t j = (w << 5) + (uint32_t)__ffs(word) - 1u;
+        for (uint32_t k = p.csc_off[j] + lane; k < p.csc_off[j + 1]; k += 32u) {
+            const uint32_t e = p.csc_edge[k], i = p.csc_src[k];
+            const uint32_t d = PACKED ? p.s_edge[e].x >> 24 : (uint32_t)p.s_dly[e];
+            if ((uint64_t)d > t) continue;                 // nothing of i can have arrived yet, and i has no age d steps ago
+            const uint64_t td = t - d;
+            const uint32_t arr = p.raster[(size_t)(td % p.raster_rows) * p.words_pad + (i >> 5)];
+            if ((arr >> (i & 31u)) & 1u) continue;        // the spike of i arrives now: coincidence
+            const int32_t ls = p.ls_hist[(size_t)(td % p.D) * p.Npad + i];
+            if (ls >= 0 && (uint64_t)ls + 1ull < td)
+                p.w_f32[e] = __fadd_rn(p.w_f32[e], stdp_dw(p, (uint32_t)(td - 1ull - (uint64_t)ls)));
+        }
+    }
+}
+
+__global__ void __launch_bounds__(256)
+gn_age_kernel(const GnDev p, const uint64_t t)
+{
+    const uint32_t j = blockIdx.x * 256u + threadIdx.x;
+    uint32_t n = 0u;
+    if (j < p.Npad) {
+        const uint32_t word = p.raster[(size_t)(t % p.raster_rows) * p.words_pad + (j >> 5)];
+        const bool fired = (word >> (j & 31u)) & 1u;
+        p.ls_hist[(size_t)((t + 1ull) % p.D) * p.Npad + j] = fired ? (int32_t)t : p.ls_hist[(size_t)(t % p.D) * p.Npad + j];
+        n = fired ? 1u : 0u;
+    }
+    n = __reduce_add_sync(0xFFFFFFFFu, n);
+    if ((threadIdx.x & 31u) == 0u && n) atomicAdd(&p.counters[1], (unsigned long long)n);
+}
+
+// in-edge lists: count, scan, fill
+__global__ void gn_csc_count_kernel(const GnDev p, const uint32_t n_edges, const bool packed)
+{
+    const uint32_t e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e < n_edges) atomicAdd(&p.csc_off[(packed ? p.s_edge[e].x & 0xFFFFFFu : p.s_edge[e].x) + 1u], 1u);
+}
+
+__global__ void __launch_bounds__(1024)
+gn_csc_scan_kernel(uint32_t *a, const uint32_t n)         // in place, inclusive (a[0] = 0 makes it the offsets); one CTA
+{
+    __shared__ uint32_t s_w[32];
+    __shared__ uint32_t s_carry;
+    if (threadIdx.x == 0) s_carry = 0u;
+    __syncthreads();
+    for (uint32_t b = 0; b < n; b += 1024u) {
+        const uint32_t idx = b + threadIdx.x, lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+        uint32_t v = idx < n ? a[idx] : 0u;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t u = __shfl_up_sync(0xFFFFFFFFu, v, o);
+            if (lane >= (uint32_t)o) v += u;
+        }
+        if (lane == 31u) s_w[warp] = v;
+        __syncthreads();
+        uint32_t before = s_carry;
+        for (uint32_t k = 0; k < warp; ++k) before += s_w[k];
+        if (idx < n) a[idx] = v + before;
+        __syncthreads();
+        if (threadIdx.x == 1023u) s_carry = v + before;
+        __syncthreads();
+    }
+}
+
+__global__ void gn_csc_fill_kernel(const GnDev p, uint32_t *cursor, const bool packed)
+{
+    const uint32_t lane = threadIdx.x & 31u;
+    const uint32_t i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    if (i >= p.N) return;
+    for (uint32_t e = p.row[i] + lane; e < p.row[i + 1]; e += 32u) {
+        const uint32_t m = packed ? p.s_edge[e].x & 0xFFFFFFu : p.s_edge[e].x;
+        const uint32_t k = p.csc_off[m] + atomicAdd(&cursor[m], 1u);
+        p.csc_edge[k] = e;
+        p.csc_src[k] = i;
+    }
+}
+
+__global__ void gn_weights_out_kernel(const GnDev p, const uint32_t n_edges)
+{
+    const uint32_t e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e < n_edges) p.w_stage[p.perm[e]] = p.w_f32[e];
+}
+
 // ---- create-time kernels --------------------------------------------------------------------------------
 __global__ void gn_init_state_kernel(const GnDev p, GnCheck *chk)
 {
@@ -1410,7 +1570,8 @@ inline uint32_t ceil_div(uint64_t a, uint64_t b) { return (uint32_t)((a + b - 1)
 cudaError_t gnk_update(const GnDev &p, uint64_t t, bool has_bias, cudaStream_t st)
 {
     // delays below d_direct are delivered by the update kernel itself (see the kernel)
-    const uint32_t d_direct = p.queue_mode ? ((p.q_window + 1u) << p.q_log) - ((uint32_t)(t % p.D) & ((1u << p.q_log) - 1u)) : 2u;
+    const uint32_t d_direct = p.plastic ? 1u      // plastic mode: nothing is sent when a vertex fires (delivery happens at arrival)
+                            : p.queue_mode ? ((p.q_window + 1u) << p.q_log) - ((uint32_t)(t % p.D) & ((1u << p.q_log) - 1u)) : 2u;
     const uint32_t grid = ceil_div(p.Npad / kVertsPerThread, kUpdateThreads);
     const uint32_t slot = (uint32_t)(t % p.D);
     const uint32_t raster_row = (uint32_t)(t % p.raster_rows);
@@ -1609,6 +1770,50 @@ cudaError_t gnk_fold(const GnDev &p, uint64_t t_win, uint32_t n_win, uint64_t g_
     cfg.numAttrs = beside_previous ? 1 : 0;
     return p.packed ? cudaLaunchKernelEx(&cfg, gn_fold_kernel<true>, p, win_slot0, n_win, r_win, j_first)
                     : cudaLaunchKernelEx(&cfg, gn_fold_kernel<false>, p, win_slot0, n_win, r_win, j_first);
+}
+
+// plastic mode: in-edge lists.  csc_off and cursor ([N] words of scratch) hold zeros on entry.
+cudaError_t gnk_build_csc(const GnDev &p, uint64_t n_edges, uint32_t *cursor, cudaStream_t st)
+{
+    if (n_edges) gn_csc_count_kernel<<<ceil_div(n_edges, 256), 256, 0, st>>>(p, (uint32_t)n_edges, p.packed != 0u);
+    gn_csc_scan_kernel<<<1, 1024, 0, st>>>(p.csc_off, p.Npad + 1u);
+    if (n_edges) gn_csc_fill_kernel<<<ceil_div((uint64_t)p.N * 32, 256), 256, 0, st>>>(p, cursor, p.packed != 0u);
+    return cudaGetLastError();
+}
+
+// plastic mode, before update(t): the spikes arriving at step t (fired at t - d, d = 1 .. min(D - 1, t - t_origin)) are
+// added to ring row t mod D with the weights of step t
+cudaError_t gnk_arrive(const GnDev &p, uint64_t t, uint64_t t_origin, cudaStream_t st)
+{
+    const uint64_t back = t - t_origin;
+    const uint32_t n_d = (uint32_t)(back < p.D - 1u ? back : p.D - 1u);
+    if (n_d == 0u) return cudaSuccess;
+    const uint32_t grid = ceil_div((uint64_t)n_d * p.words_pad, 256);
+    if (p.packed) gn_arrive_kernel<false, true><<<grid, 256, 0, st>>>(p, t, n_d);
+    else gn_arrive_kernel<false, false><<<grid, 256, 0, st>>>(p, t, n_d);
+    return cudaGetLastError();
+}
+
+// plastic mode, after update(t): eq. 33 for the arrivals and the spikes of step t, then eq. 32
+cudaError_t gnk_plasticity(const GnDev &p, uint64_t t, uint64_t t_origin, cudaStream_t st)
+{
+    const uint64_t back = t - t_origin;
+    const uint32_t n_d = (uint32_t)(back < p.D - 1u ? back : p.D - 1u);
+    if (n_d) {
+        const uint32_t grid = ceil_div((uint64_t)n_d * p.words_pad, 256);
+        if (p.packed) gn_arrive_kernel<true, true><<<grid, 256, 0, st>>>(p, t, n_d);
+        else gn_arrive_kernel<true, false><<<grid, 256, 0, st>>>(p, t, n_d);
+    }
+    if (p.packed) gn_ltp_kernel<true><<<ceil_div((uint64_t)p.words_pad * 32, 256), 256, 0, st>>>(p, t);
+    else gn_ltp_kernel<false><<<ceil_div((uint64_t)p.words_pad * 32, 256), 256, 0, st>>>(p, t);
+    gn_age_kernel<<<ceil_div(p.Npad, 256), 256, 0, st>>>(p, t);
+    return cudaGetLastError();
+}
+
+cudaError_t gnk_weights_out(const GnDev &p, uint64_t n_edges, cudaStream_t st)
+{
+    if (n_edges) gn_weights_out_kernel<<<ceil_div(n_edges, 256), 256, 0, st>>>(p, (uint32_t)n_edges);
+    return cudaGetLastError();
 }
 
 cudaError_t gnk_sort_rows(const GnDev &p, GnCheck *chk, cudaStream_t st)

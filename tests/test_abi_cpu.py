@@ -28,8 +28,8 @@ def test_library_exports_every_declared_symbol():
 
 def test_structs_match_header_layout():
     assert C.sizeof(gn.gn_class_params) == 40 * 4          # 13 + model + 8 Hodgkin-Huxley scalars + 6 rate functions x 3
-    # uint32 x2, uint64, uint32 x2, float x2, uint32, float x5, uint32 x3, (pad), uint64, uint32 x2, uint64
-    assert C.sizeof(gn.gn_config) == 96
+    # uint32 x2, uint64, uint32 x2, float x2, uint32, float x5, uint32 x3, (pad), uint64, uint32 x2, uint64, float x2
+    assert C.sizeof(gn.gn_config) == 104
     assert gn.gn_config.seed.offset == 72 and gn.gn_config.n_edges.offset == 8
     assert gn.gn_config.delivery_mode.offset == 80 and gn.gn_config.queue_capacity.offset == 88
 

@@ -832,3 +832,127 @@ def test_ring_mode_step_drivers_agree(gn, monkeypatch, k, n, steps, chunk, persi
     _, launches = gn.gn_profile_read(g)
     n_calls = -(-steps // chunk)
     assert int(launches[4]) == (n_calls if persist else steps + frames)      # O(calls), not O(steps), runtime launches
+
+
+# ---- plastic weights: spike-time dependent plasticity (eq. 32-33; f-3) ------------------------------------
+STDP_ALPHA, STDP_BETA = 0.5, 0.05
+
+
+def _plastic(gn, net, cfg, steps, dl, alpha=STDP_ALPHA, beta=STDP_BETA, **kw):
+    return gn.create_from_inputs(net, cfg, delays=dl, raster_capacity_steps=steps, stdp_alpha=alpha, stdp_beta=beta, **kw)
+
+
+def _csr_edges(net):
+    row = net.row_offsets.astype(np.int64)
+    return [(i, int(net.targets[e])) for i in range(net.n_vertices) for e in range(row[i], row[i + 1])]
+
+
+def test_plastic_mode_delivers_at_arrival_exactly_like_the_ring(gn):
+    """The arrival-time delivery of plastic mode with a vanishing learning rate (alpha = 1e-30: every change underflows to
+    nothing) must reproduce static delivery bit for bit: rasters, state words, kicks and spikes against the fp32-faithful
+    oracle, over 2,000 steps of config 3's and config 4's densities (D = 64 and 128, ragged N)."""
+    for k, n in ((3, 3_001), (4, 2_500)):
+        net, cfg = make_config(k, n=n)
+        cfg = dict(cfg, obs_stride=0)
+        steps = 2000
+        g = _plastic(gn, net, cfg, steps, None, alpha=1e-30, beta=1.0)
+        o = Oracle(net, cfg, "fp32", threads=4)
+        gn.gn_step(g, steps)
+        o.step(steps)
+        np.testing.assert_array_equal(gn.gn_read_raster(g, 0, steps), o.raster(0, steps))
+        for which_g, which_o in ((gn.GN_V, ob.V), (gn.GN_W, ob.W), (gn.GN_R, ob.R)):
+            np.testing.assert_array_equal(gn.gn_read_state(g, which_g).view(np.uint32),
+                                          o.state(which_o).astype(np.float32).view(np.uint32))
+        c, oc = gn.gn_read_state(g, gn.GN_COUNTERS), o.counters()
+        assert (int(c[0]), int(c[1]), int(c[3])) == (oc["steps"], oc["spikes"], oc["kicks"]) and oc["spikes"] > 0
+        np.testing.assert_array_equal(gn.gn_read_state(g, gn.GN_WEIGHTS),
+                                      (o.w_fx().astype(np.float64) / 65536.0).astype(np.float32))
+
+
+@pytest.mark.parametrize("delay", [1, 7])
+@pytest.mark.parametrize("k", [-30, -5, -2, -1, 0, 1, 2, 5, 30])
+def test_plastic_single_pairing_closed_form(gn, delay, k):
+    """One pre-synaptic arrival at step a, one post-synaptic spike at a + k, after a warm-up pairing (as the oracle's own pin,
+    tests/test_oracle_stdp.py): the weight change is the closed form of eq. 33 with eq. 32's ages, and equals the definition's."""
+    import math
+    from oracle.stdp_definition import StdpSimulator
+    net, dl = hand_net(2, [(0, 1, 0.0, delay)])
+    cfg = base_cfg([rs_class(drive_rate_hz=0.0, refractory_ms=0.0)], ring_slots=64, dt_ms=0.1)
+    a, post0 = 500, 100
+    spikes = {60 - delay: [0], post0: [1], a - delay: [0]}
+    spikes.setdefault(a + k, []).append(1)
+    g = _plastic(gn, net, cfg, 560, dl)
+    sim = StdpSimulator(net, cfg, STDP_ALPHA, STDP_BETA, delays=dl)
+    for t in range(560):
+        if t in spikes:
+            v = gn.gn_read_state(g, gn.GN_V)
+            for j in spikes[t]:
+                v[j] = 30.0
+                sim.V[j] = 30.0
+            gn.gn_write_state(g, gn.GN_V, v)
+        gn.gn_step(g, 1)
+        sim.step(1)
+    r = unpack_raster(gn.gn_read_raster(g, 0, 560), 2)
+    assert np.array_equal(r, np.array(sim.raster, dtype=bool)) and r.sum() == 4
+    w = float(gn.gn_read_state(g, gn.GN_WEIGHTS)[0])
+    dt = 0.1
+    near = 0.0 if abs(k) == 1 else 1.0
+    warm = dt * STDP_ALPHA * math.exp(-STDP_BETA * 39 * dt)
+    if k == 0:
+        expect = warm
+    elif k > 0:
+        expect = warm + dt * STDP_ALPHA * (near * math.exp(-STDP_BETA * (k - 1) * dt) - math.exp(-STDP_BETA * (a - post0 - 1) * dt))
+    else:
+        expect = warm + dt * STDP_ALPHA * (-near * math.exp(-STDP_BETA * (-k - 1) * dt) + math.exp(-STDP_BETA * (a + k - 60 - 1) * dt))
+    assert w == pytest.approx(expect, rel=2e-6, abs=1e-8)
+    assert w == pytest.approx(sim.weight(0, 1), rel=2e-6, abs=1e-8)
+
+
+@pytest.mark.parametrize("seed", [3, 8])
+def test_plastic_random_network_tracks_the_definition(gn, seed):
+    """A random plastic network with kicks against oracle/stdp_definition.py (fp64, pure Python): identical rasters up to the
+    first divergence t* (fp32 against fp64 dynamics: printed), which must lie beyond 300 steps, and at every checkpoint up
+    to it every weight within 1e-4 relative / 2e-5 absolute (fp32 weights, a quantised delivery, exp in fp32)."""
+    from oracle.stdp_definition import StdpSimulator
+    rng = np.random.default_rng(seed)
+    n = 24
+    net, dl = hand_net(n, random_digraph(rng, n, 0.3, 16, w_lo=0.0, w_hi=7.0))
+    cfg = base_cfg([rs_class(drive_rate_hz=300.0)], ring_slots=16, dt_ms=0.1)
+    steps, chunk = 1000, 100
+    g = _plastic(gn, net, cfg, steps, dl)
+    sim = StdpSimulator(net, cfg, STDP_ALPHA, STDP_BETA, delays=dl)
+    edges = _csr_edges(net)
+    w0 = gn.gn_read_state(g, gn.GN_WEIGHTS).copy()
+    t_star = steps
+    for done in range(chunk, steps + 1, chunk):
+        gn.gn_step(g, chunk)
+        sim.step(chunk)
+        rg = unpack_raster(gn.gn_read_raster(g, done - chunk, chunk), n)
+        ro = np.array(sim.raster[done - chunk:done], dtype=bool)
+        if not np.array_equal(rg, ro):
+            t_star = done - chunk + int(np.flatnonzero((rg != ro).any(axis=1))[0])
+            break
+        wg = gn.gn_read_state(g, gn.GN_WEIGHTS).astype(np.float64)
+        wo = np.array([sim.weight(i, j) for (i, j) in edges])
+        np.testing.assert_allclose(wg, wo, rtol=1e-4, atol=2e-5)
+    print(f"plastic network seed {seed}: rasters identical up to t* = {t_star}; "
+          f"{int(np.array(sim.raster[:t_star]).sum())} spikes, largest weight change {np.abs(wg - w0).max():.3f}")
+    assert t_star > 300
+    assert np.abs(wg - w0).max() > 0.05, "degenerate test: the weights hardly moved"
+
+
+def test_plastic_mode_argument_checks(gn):
+    net, dl = hand_net(2, [(0, 1, 1.0, 3)])
+    cfg = base_cfg([rs_class()], ring_slots=16)
+    for bad in (dict(delivery_mode=gn.GN_DELIVER_QUEUE), dict(delivery_mode=gn.GN_DELIVER_RESIDENT), dict(stdp_beta=-1.0)):
+        kw = dict(stdp_alpha=0.5, stdp_beta=0.05)
+        kw.update(bad)
+        with pytest.raises(gn.GnError) as ei:
+            gn.create_from_inputs(net, cfg, delays=dl, **kw)
+        assert ei.value.code == gn.GN_E_INVALID_ARG
+    g = gn.create_from_inputs(net, cfg, delays=dl)
+    with pytest.raises(gn.GnError):
+        gn.gn_read_state(g, gn.GN_WEIGHTS)                      # static network: GN_WEIGHTS_FX
+    g = _plastic(gn, net, cfg, 10, dl)
+    with pytest.raises(gn.GnError):
+        gn.gn_write_state(g, gn.GN_STEP, np.array([5], np.uint64))
