@@ -34,7 +34,7 @@ METRIC, UNIT = "vertex-steps/s", "vertex-steps/s"
 UPDATE_BYTES_PER_VERTEX = 35.125       # V,W,r r+w 24, ring slot r+clear 8, refr 2, class 1, raster bit 1/8
 UPDATE_BYTES_PER_VERTEX_OBS = 12.0     # + c r+w 8, frame accumulator amortised / trace row 4 per frame (counted per step as 4)
 HH_BYTES_PER_VERTEX = 51.125           # Hodgkin-Huxley class: V, n, r, m, h r+w 40, ring slot r+clear 8, refr 2, class 1, raster bit 1/8
-HH_FP32_PER_VERTEX = 141.0             # fp32 operations of the contract per Hodgkin-Huxley vertex-step (DESIGN.md 6.7: 6 exp32 x 14,
+HH_FP32_PER_VERTEX = 141.0             # fp32 operations of the contract per Hodgkin-Huxley vertex-step (DESIGN.md 6.6: 6 exp32 x 14,
                                        # rate arguments and shapes 25, currents 16, gates 12, V, PSC, input 4; a division counts 1)
 FP32_LANES_PER_SM, SM_COUNT, SM_HZ = 128, 148, 1.965e9   # B200_PROFILING.md: 148 SMs, 1965 MHz; 4 x 32 fp32 lanes per SM
 EVENT_BYTES = 17.0                     # edge record 9 (target 4, weight 4, delay 1) + ring word read-modify-write 8
@@ -242,6 +242,9 @@ def main():
     ap.add_argument("--model", default="izhikevich", choices=["izhikevich", "hh"],
                     help="hh: every class a Hodgkin-Huxley vertex at dt = 0.03 ms (the paper's second benchmarked model, "
                          "PAPER.md:382): a different workload, reported with an fp32-ALU roofline beside the HBM one")
+    ap.add_argument("--stdp", action="store_true", help="plastic weights (gn_config.stdp_alpha = 0.5 / ms, stdp_beta = 0.05 / ms; "
+                                                       "DESIGN.md 6.7): delivery at arrival time, eq. 32-33 every step -- a different "
+                                                       "workload; the CPU baseline (static oracle) is skipped")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -273,6 +276,8 @@ def main():
         cfg = as_hodgkin_huxley(cfg)
     if args.psc_alpha:
         cfg = dict(cfg, classes=[dict(c, psc_alpha=1.0) for c in cfg["classes"]], name=cfg["name"] + "+alpha_psc")
+    if args.stdp:
+        cfg = dict(cfg, obs_stride=0, name=cfg["name"] + "+stdp")      # plastic mode has no observation
     N, E = net_in.n_vertices, net_in.n_edges
     log(f"[rank {rank}] inputs in {time.time() - t0:.1f} s: N={N} E={E} mean out-degree {E / N:.1f}")
     obs = int(cfg["obs_stride"])
@@ -286,7 +291,7 @@ def main():
                            obs_gain=cfg["obs_gain"], obs_offset=cfg["obs_offset"], obs_sigma=cfg["obs_sigma"],
                            obs_stride=obs, raster_capacity_steps=S, trace_capacity_frames=max(frames_per_step, 1) if obs else 0,
                            seed=cfg["seed"], delivery_mode={"auto": 0, "ring": 1, "queue": 2}[args.delivery],
-                           queue_group=args.queue_group)
+                           queue_group=args.queue_group, stdp_alpha=0.5 if args.stdp else 0.0, stdp_beta=0.05 if args.stdp else 0.0)
         return gn.gn_create(c, cfg["classes"], a["pos"], a["row"], a["tgt"], a["w"], None, a["cls"], None, a["net"],
                             device=dev)
 
@@ -340,25 +345,35 @@ def main():
     cp1 = counters(g)
     assert cp0 == c0 and cp1 == c1, "the per-kernel pass did not replay the timed steps"
     peak, peak_src = peaks()
-    queue_mode = 0 < kn[1] < kn[0]      # queue mode delivers once per slot group, ring mode every step
+    queue_mode = 0 < kn[1] < kn[0]      # queue mode delivers once per slot group, ring mode (and plastic mode) every step
     resident = kn[1] == 0 and kn[0] < sim_steps
     persist = resident and net_in.n_networks == 1 and N > 16384
     names = ["gn_persist_kernel (a1-a5, one cooperative launch per call)" if persist else
              "gn_resident_kernel (a1-a5, one CTA or cluster per network)" if resident else
              "gn_update_kernel (a1-a3 + a4 fused)" if kn[1] == 0 else "gn_update_kernel (a1-a3)",
-             "gn_log_kernel (a3 compaction + a4: spikes into the log)" if queue_mode else "gn_deliver_kernel (a4)",
-             "gn_observe_kernel (a5)", "gn_fold_kernel (a4: expansion of the log + ring reductions)"]
+             "gn_log_kernel (a3 compaction + a4: spikes into the log)" if queue_mode else
+             "gn_arrive_kernel (a4 at arrival time: plastic weights)" if args.stdp else "gn_deliver_kernel (a4)",
+             "gn_observe_kernel (a5)",
+             "gn_arrive_kernel<LTD> + gn_ltp_kernel + gn_age_kernel (eq. 33, eq. 32)" if args.stdp else
+             "gn_fold_kernel (a4: expansion of the log + ring reductions)"]
     p_events, p_spikes = cp1[2] - cp0[2], cp1[1] - cp0[1]
     # algorithmic bytes per launch: 17 B per event (+12 B per fired source) for the
     # delivery of either mode (queue mode, per slot group: the logging kernel takes the 12 B per fired source, the fold
     # kernel the 17 B per event of the group it expands)
     delivery_bytes = p_events * EVENT_BYTES + p_spikes * SOURCE_BYTES
     per_vertex = HH_BYTES_PER_VERTEX if args.model == "hh" else UPDATE_BYTES_PER_VERTEX
+    if args.stdp:
+        # plastic mode, per step: arrivals re-read the raster of the last D - 1 steps (N/8 bytes each) and move 8 B edge + 4 B
+        # weight + 8 B ring word per event; eq. 33 moves 8 B edge + 8 B weight per arrival (weakening), 8 B in-edge entry + 8 B
+        # edge + 8 B weight per in-edge of a fired vertex (strengthening; as many as events in the long run), and eq. 32 8 B per vertex
+        ring_d = cfg["ring_slots"]
+        arrive_b = (p_events * 20.0 + sim_steps * (ring_d - 1) * N / 8.0)
+        plast_b = (p_events * (16.0 + 24.0) + sim_steps * ((ring_d - 1) * N / 8.0 + N * 8.0))
     kbytes = [N * (per_vertex + (UPDATE_BYTES_PER_VERTEX_OBS if obs else 0.0)) * (sim_steps / max(int(kn[0]), 1))
               + (delivery_bytes / max(int(kn[0]), 1) if kn[1] == 0 else 0.0),
-              (p_spikes * SOURCE_BYTES if queue_mode else delivery_bytes) / max(int(kn[1]), 1),
+              (arrive_b if args.stdp else p_spikes * SOURCE_BYTES if queue_mode else delivery_bytes) / max(int(kn[1]), 1),
               N * 8.0,
-              p_events * EVENT_BYTES / max(int(kn[3]), 1)]
+              (plast_b if args.stdp else p_events * EVENT_BYTES) / max(int(kn[3]), 1)]
     traffic_tab, traffic_src = measured_traffic()
     kernels = []
     for k in range(4):
@@ -376,7 +391,9 @@ def main():
     a4 = {"what": "a4 delivery as a whole (routing + folding), 17 B per event + 12 B per fired source",
           "bytes": p_events * EVENT_BYTES + p_spikes * SOURCE_BYTES, "ms": a4_s * 1e3,
           "achieved": (p_events * EVENT_BYTES + p_spikes * SOURCE_BYTES) / max(a4_s, 1e-12) / 1e9}
-    a4["frac"] = a4["achieved"] / peak
+    a4["frac"] = a4["achieved"] / peak if a4_s > 0 else None      # (no separate delivery kernel: a4 is inside the update / persistent kernel)
+    if a4_s <= 0:
+        a4["achieved"] = None
     if queue_mode and a4_s > 0:
         # what bounds event delivery is not HBM but the L2's atomic path: one int32 reduction per event is the
         # least any atomic delivery does, and the fold gathers each event's 8-byte edge in short random segments on top.  Both
@@ -468,7 +485,9 @@ def main():
         "events_per_sim_step": events / world / sim_steps,
         "roofline": roofline, "clocks": clocks, "gpu_launches": launches, "e2e": e2e,
     }
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+    if args.stdp:
+        line["config"]["workload"] += " + STDP (alpha 0.5 / ms, beta 0.05 / ms)"
+    if rank == 0 and world == 1 and not args.no_cpu_baseline and not args.stdp:
         line["cpu_baseline"] = cpu_baseline(net_in, cfg)
     if rank == 0:
         print(json.dumps(line), flush=True)

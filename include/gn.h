@@ -7,9 +7,9 @@
  *   y_j(t + dt) = H_j( y_j(t), Y_j(t), u_j(t), Theta_j )                     :68-71  eq. 5
  *
  * with  y_j = {V, W, r, c} an Izhikevich simple-model vertex with hard reset (:227-229 eq. 24,
- * :303 eq. 28), an exponential (:283-286 eq. 26) or alpha-function (:288-312 eq. 27-30, state p)
- * post-synaptic current and a calcium state
- * (:364 H_c);  Y_j(t) the delayed, weighted spikes of the other vertices,
+ * :303 eq. 28) or a Hodgkin-Huxley vertex {V, m, h, n} (:235, :382), an exponential (:283-286 eq. 26)
+ * or alpha-function (:288-312 eq. 27-30, state p) post-synaptic current and a calcium state
+ * (:364 H_c); optionally plastic weights w_ij(t) with the STDP transition function (:323-349 eq. 32-33);  Y_j(t) the delayed, weighted spikes of the other vertices,
  * sum_k w_kj spd(V_k(t - tau_kj)) (:311 eq. 30, spd = [V >= V_peak] :316 eq. 31) with
  * tau_kj = |x_k - x_j| / s (:251 eq. 25);  u_j(t) the external control (:77-79 eq. 7); and the
  * observation I_j = n c_j + b + N(0, gamma^2) averaged over camera frames (:370-374).

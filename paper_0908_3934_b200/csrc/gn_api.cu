@@ -655,11 +655,21 @@ int gn_step(gn_net *net, uint64_t n_steps)
     if (d.plastic) {       // plastic weights: arrivals of step t, the update, then eq. 33 and eq. 32, all on the caller's stream
         for (uint64_t s = 0; s < n_steps; ++s) {
             const uint64_t t = net->t;
+            const bool prof = net->profile;
+            int rc;
+            if (prof && (rc = prof_mark(net, 1))) return rc;
             GN_CUDA(net, gnk_arrive(d, t, net->t_origin, net->stream));
+            if (prof && (rc = prof_mark(net, 0))) return rc;
             GN_CUDA(net, gnk_update(d, t, net->has_bias, net->stream));
+            if (prof && (rc = prof_mark(net, 3))) return rc;
             GN_CUDA(net, gnk_plasticity(d, t, net->t_origin, net->stream));
             net->launches += 5;
             net->t = t + 1;
+            if (prof && (s + 1) % kProfChunk == 0 && ((rc = prof_mark(net, 0xFF)) || (rc = prof_collect(net)))) return rc;
+        }
+        if (net->profile) {
+            int rc = prof_mark(net, 0xFF);
+            return rc ? rc : prof_collect(net);
         }
         return GN_OK;
     }
