@@ -19,7 +19,7 @@ thread_local char g_create_error[256] = "";
 struct Layout {
     size_t V, W, r, p2, hm, hh, c, acc, bias, refr, cls, ring, row, tgt, wfx, dly, counters, q_count;
     size_t s_edge, s_dly, min_dly, q_seg, spk_log;
-    size_t w_f32, perm, ls_hist, csc_off, csc_edge, csc_src, w_stage;
+    size_t w_f32, perm, ls_hist, pl_list, csc_off, csc_edge, csc_src, w_stage;
     size_t raster, trace, scratch_row64, scratch_abs, scratch_pos, scratch_net, scratch_chk, total;
 };
 
@@ -110,7 +110,7 @@ Layout make_layout(const gn_config *cfg)
     const bool plastic = cfg->stdp_alpha != 0.0f;
     L.q_seg = take(qp.on || plastic ? N * D * 2 : 0);
     L.w_f32 = take(plastic ? E * 4 : 0); L.perm = take(plastic ? E * 4 : 0); L.w_stage = take(plastic ? E * 4 : 0);
-    L.ls_hist = take(plastic ? D * Npad * 4 : 0);
+    L.ls_hist = take(plastic ? D * Npad * 4 : 0); L.pl_list = take(plastic ? D * Npad * 4 : 0);
     L.csc_off = take(plastic ? (Npad + 2) * 4 : 0); L.csc_edge = take(plastic ? E * 4 : 0); L.csc_src = take(plastic ? E * 4 : 0);
     L.spk_log = take(qp.on && qp.arrays >= 2 ? D * qp.arrays * (size_t)qp.log_cap * 4 : 0);
     L.scratch_row64 = take((N + 1) * 8); L.scratch_abs = take(N * 8);
@@ -308,7 +308,7 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
         d.q_log = 0u; d.q_nb = cfg->ring_slots; d.q_arrays = 0u;
         d.q_seg = (uint16_t *)(ws + L.q_seg);
         d.w_f32 = (float *)(ws + L.w_f32); d.perm = (uint32_t *)(ws + L.perm); d.w_stage = (float *)(ws + L.w_stage);
-        d.ls_hist = (int32_t *)(ws + L.ls_hist);
+        d.ls_hist = (int32_t *)(ws + L.ls_hist); d.pl_list = (uint32_t *)(ws + L.pl_list);
         d.csc_off = (uint32_t *)(ws + L.csc_off); d.csc_edge = (uint32_t *)(ws + L.csc_edge); d.csc_src = (uint32_t *)(ws + L.csc_src);
     }
     d.trace = cfg->obs_stride ? (float *)(ws + L.trace) : nullptr;
@@ -663,7 +663,7 @@ int gn_step(gn_net *net, uint64_t n_steps)
             GN_CUDA(net, gnk_update(d, t, net->has_bias, net->stream));
             if (prof && (rc = prof_mark(net, 3))) return rc;
             GN_CUDA(net, gnk_plasticity(d, t, net->t_origin, net->stream));
-            net->launches += 5;
+            net->launches += 6;
             net->t = t + 1;
             if (prof && (s + 1) % kProfChunk == 0 && ((rc = prof_mark(net, 0xFF)) || (rc = prof_collect(net)))) return rc;
         }

@@ -1246,10 +1246,11 @@ gn_persist_kernel(const GnDev p, const uint64_t t0, const uint32_t n_steps, unsi
 // ---- plastic mode: spike-time dependent plasticity (eq. 32-33; readings #22, #23) ----------
 // Every weight is a state of its own (eq. 9) and eq. 30 weighs an arriving spike with the weight AT THE ARRIVAL step, so
 // nothing is delivered when a vertex fires: per step t
-//   gn_arrive_kernel<false>  for every delay d and every vertex i that fired at t - d (raster row of that step), the edges
+//   gn_arrive_kernel<false>  for every delay d and every vertex i that fired at t - d (the spike list of that step), the edges
 //                            of i with delay exactly d -- a contiguous run of its delay-sorted row, boundaries from the
 //                            per-delay table (q_seg with groups of one slot) -- add rint(w(t) 2^16) to ring[t mod D][target];
 //   gn_update_kernel         as ever (a1-a3); it sends nothing itself;
+//   gn_spikes_kernel         the fired vertices of step t, listed (row t mod D of pl_list: the spikes in flight are these lists);
 //   gn_arrive_kernel<true>   the same enumeration again, now that the spikes of step t are known: an arrival at a target
 //                            that does not fire at t weakens its edge, w -= dt alpha exp(-beta s_j(t));
 //   gn_ltp_kernel            every vertex j that fired at t strengthens each in-edge (i -> j, d) on which nothing arrives
@@ -1272,34 +1273,63 @@ __device__ __forceinline__ float stdp_dw(const GnDev &p, const uint32_t steps)
     return __fmul_rn(p.stdp_dta, exp32(-__fmul_rn(p.stdp_beta, age)));
 }
 
+// The fired vertices of step t, listed (any order) in row t mod D of pl_list; log_n[t mod D] = how many (zeroed by the launcher).
+__global__ void __launch_bounds__(256)
+gn_spikes_kernel(const GnDev p, const uint64_t t)
+{
+    const uint32_t j = blockIdx.x * 256u + threadIdx.x, lane = threadIdx.x & 31u;
+    const uint32_t slot = (uint32_t)(t % p.D);
+    bool fired = false;
+    if (j < p.Npad) fired = (p.raster[(size_t)(t % p.raster_rows) * p.words_pad + (j >> 5)] >> (j & 31u)) & 1u;
+    const uint32_t m = __ballot_sync(0xFFFFFFFFu, fired);
+    if (m == 0u) return;
+    uint32_t base = 0u;
+    if (lane == 0u) {
+        base = atomicAdd(&p.log_n[slot], (uint32_t)__popc(m));
+        atomicAdd(&p.counters[1], (unsigned long long)__popc(m));
+    }
+    base = __shfl_sync(0xFFFFFFFFu, base, 0);
+    if (fired) p.pl_list[(size_t)slot * p.Npad + base + __popc(m & ((1u << lane) - 1u))] = j;
+}
+
+// One thread per (delay d, vertex that fired at t - d), the pairs flattened over the lists of the last n_d steps.
 template <bool LTD, bool PACKED>
 __global__ void __launch_bounds__(256)
 gn_arrive_kernel(const GnDev p, const uint64_t t, const uint32_t n_d)
 {
-    const uint32_t idx = blockIdx.x * 256u + threadIdx.x;
+    __shared__ uint32_t s_pref[256];
+    __shared__ uint32_t s_wsum[8];
+    uint32_t cnt = 0u;
+    if (threadIdx.x < n_d) cnt = p.log_n[(t - 1ull - threadIdx.x) % p.D];      // delay d = threadIdx.x + 1
+    uint32_t off;
+    const uint32_t P = gather_scan<256>(cnt, s_wsum, off);
+    s_pref[threadIdx.x] = off;
+    __syncthreads();
     unsigned long long events = 0ull;
-    if (idx < n_d * p.words_pad) {
-        const uint32_t d = idx / p.words_pad + 1u, w = idx - (d - 1u) * p.words_pad;
-        uint32_t word = p.raster[(size_t)((t - d) % p.raster_rows) * p.words_pad + w];
-        const uint32_t slot = (uint32_t)(t % p.D);
-        const uint32_t *fired_now = p.raster + (size_t)(t % p.raster_rows) * p.words_pad;
-        const int32_t *last = p.ls_hist + (size_t)slot * p.Npad;
-        for (; word; word &= word - 1u) {
-            const uint32_t i = (w << 5) + (uint32_t)__ffs(word) - 1u;
-            const uint32_t beg = p.row[i], deg = p.row[i + 1] - beg;
-            const uint32_t lo = delay_bound<PACKED>(p, i, d, beg, deg), hi = delay_bound<PACKED>(p, i, d + 1u, beg, deg);
-            for (uint32_t e = beg + lo; e < beg + hi; ++e) {
-                const uint32_t m = PACKED ? p.s_edge[e].x & 0xFFFFFFu : p.s_edge[e].x;
-                if (!LTD) {
-                    ring_add(p.ring + (size_t)slot * p.Npad + m, __float2int_rn(__fmul_rn(p.w_f32[e], 65536.0f)));
-                } else if (!((fired_now[m >> 5] >> (m & 31u)) & 1u)) {     // (a coincidence changes nothing)
-                    const int32_t ls = last[m];
-                    if (ls >= 0 && (uint64_t)ls + 1ull < t)
-                        p.w_f32[e] = __fsub_rn(p.w_f32[e], stdp_dw(p, (uint32_t)(t - 1ull - (uint64_t)ls)));
-                }
-            }
-            events += (unsigned long long)(hi - lo);
+    const uint32_t slot = (uint32_t)(t % p.D);
+    const uint32_t *fired_now = p.raster + (size_t)(t % p.raster_rows) * p.words_pad;
+    const int32_t *last = p.ls_hist + (size_t)slot * p.Npad;
+    for (uint32_t pidx = blockIdx.x * 256u + threadIdx.x; pidx < P; pidx += gridDim.x * 256u) {
+        uint32_t lo = 0u, hi_s = n_d;                       // the last delay index whose pairs start at or before pidx
+        while (hi_s - lo > 1u) {
+            const uint32_t mid = (lo + hi_s) >> 1;
+            if (s_pref[mid] <= pidx) lo = mid; else hi_s = mid;
         }
+        const uint32_t d = lo + 1u;
+        const uint32_t i = p.pl_list[(size_t)((t - d) % p.D) * p.Npad + (pidx - s_pref[lo])];
+        const uint32_t beg = p.row[i], deg = p.row[i + 1] - beg;
+        const uint32_t e_lo = delay_bound<PACKED>(p, i, d, beg, deg), e_hi = delay_bound<PACKED>(p, i, d + 1u, beg, deg);
+        for (uint32_t e = beg + e_lo; e < beg + e_hi; ++e) {
+            const uint32_t m = PACKED ? p.s_edge[e].x & 0xFFFFFFu : p.s_edge[e].x;
+            if (!LTD) {
+                ring_add(p.ring + (size_t)slot * p.Npad + m, __float2int_rn(__fmul_rn(p.w_f32[e], 65536.0f)));
+            } else if (!((fired_now[m >> 5] >> (m & 31u)) & 1u)) {         // (a coincidence changes nothing)
+                const int32_t ls = last[m];
+                if (ls >= 0 && (uint64_t)ls + 1ull < t)
+                    p.w_f32[e] = __fsub_rn(p.w_f32[e], stdp_dw(p, (uint32_t)(t - 1ull - (uint64_t)ls)));
+            }
+        }
+        events += (unsigned long long)(e_hi - e_lo);
     }
     if (!LTD) {
 #pragma unroll
@@ -1308,16 +1338,15 @@ gn_arrive_kernel(const GnDev p, const uint64_t t, const uint32_t n_d)
     }
 }
 
-// One warp per raster word of step t: every fired vertex in turn, lanes over its in-edges.
+// One warp per vertex that fired at t (its list), lanes over its in-edges.
 template <bool PACKED>
 __global__ void __launch_bounds__(256)
 gn_ltp_kernel(const GnDev p, const uint64_t t)
 {
-    const uint32_t lane = threadIdx.x & 31u, w = (blockIdx.x * 256u + threadIdx.x) >> 5;
-    if (w >= p.words_pad) return;
-    uint32_t word = p.raster[(size_t)(t % p.raster_rows) * p.words_pad + w];
-    for (; word; word &= word - 1u) {
-        const uint32_t j = (w << 5) + (uint32_t)__ffs(word) - 1u;
+    const uint32_t lane = threadIdx.x & 31u, n_warps = (gridDim.x * 256u) >> 5;
+    const uint32_t slot = (uint32_t)(t % p.D), n = p.log_n[slot];
+    for (uint32_t q = (blockIdx.x * 256u + threadIdx.x) >> 5; q < n; q += n_warps) {
+        const uint32_t j = p.pl_list[(size_t)slot * p.Npad + q];
         for (uint32_t k = p.csc_off[j] + lane; k < p.csc_off[j + 1]; k += 32u) {
             const uint32_t e = p.csc_edge[k], i = p.csc_src[k];
             const uint32_t d = PACKED ? p.s_edge[e].x >> 24 : (uint32_t)p.s_dly[e];
@@ -1336,15 +1365,9 @@ __global__ void __launch_bounds__(256)
 gn_age_kernel(const GnDev p, const uint64_t t)
 {
     const uint32_t j = blockIdx.x * 256u + threadIdx.x;
-    uint32_t n = 0u;
-    if (j < p.Npad) {
-        const uint32_t word = p.raster[(size_t)(t % p.raster_rows) * p.words_pad + (j >> 5)];
-        const bool fired = (word >> (j & 31u)) & 1u;
-        p.ls_hist[(size_t)((t + 1ull) % p.D) * p.Npad + j] = fired ? (int32_t)t : p.ls_hist[(size_t)(t % p.D) * p.Npad + j];
-        n = fired ? 1u : 0u;
-    }
-    n = __reduce_add_sync(0xFFFFFFFFu, n);
-    if ((threadIdx.x & 31u) == 0u && n) atomicAdd(&p.counters[1], (unsigned long long)n);
+    if (j >= p.Npad) return;
+    const bool fired = (p.raster[(size_t)(t % p.raster_rows) * p.words_pad + (j >> 5)] >> (j & 31u)) & 1u;
+    p.ls_hist[(size_t)((t + 1ull) % p.D) * p.Npad + j] = fired ? (int32_t)t : p.ls_hist[(size_t)(t % p.D) * p.Npad + j];
 }
 
 // in-edge lists: count, scan, fill
@@ -1788,24 +1811,25 @@ cudaError_t gnk_arrive(const GnDev &p, uint64_t t, uint64_t t_origin, cudaStream
     const uint64_t back = t - t_origin;
     const uint32_t n_d = (uint32_t)(back < p.D - 1u ? back : p.D - 1u);
     if (n_d == 0u) return cudaSuccess;
-    const uint32_t grid = ceil_div((uint64_t)n_d * p.words_pad, 256);
-    if (p.packed) gn_arrive_kernel<false, true><<<grid, 256, 0, st>>>(p, t, n_d);
-    else gn_arrive_kernel<false, false><<<grid, 256, 0, st>>>(p, t, n_d);
+    if (p.packed) gn_arrive_kernel<false, true><<<148u * 8u, 256, 0, st>>>(p, t, n_d);
+    else gn_arrive_kernel<false, false><<<148u * 8u, 256, 0, st>>>(p, t, n_d);
     return cudaGetLastError();
 }
 
-// plastic mode, after update(t): eq. 33 for the arrivals and the spikes of step t, then eq. 32
+// plastic mode, after update(t): the step's spike list, eq. 33 for the arrivals and the spikes of step t, then eq. 32
 cudaError_t gnk_plasticity(const GnDev &p, uint64_t t, uint64_t t_origin, cudaStream_t st)
 {
     const uint64_t back = t - t_origin;
     const uint32_t n_d = (uint32_t)(back < p.D - 1u ? back : p.D - 1u);
+    cudaError_t e = cudaMemsetAsync(p.log_n + (t % p.D), 0, 4, st);
+    if (e != cudaSuccess) return e;
+    gn_spikes_kernel<<<ceil_div(p.Npad, 256), 256, 0, st>>>(p, t);
     if (n_d) {
-        const uint32_t grid = ceil_div((uint64_t)n_d * p.words_pad, 256);
-        if (p.packed) gn_arrive_kernel<true, true><<<grid, 256, 0, st>>>(p, t, n_d);
-        else gn_arrive_kernel<true, false><<<grid, 256, 0, st>>>(p, t, n_d);
+        if (p.packed) gn_arrive_kernel<true, true><<<148u * 8u, 256, 0, st>>>(p, t, n_d);
+        else gn_arrive_kernel<true, false><<<148u * 8u, 256, 0, st>>>(p, t, n_d);
     }
-    if (p.packed) gn_ltp_kernel<true><<<ceil_div((uint64_t)p.words_pad * 32, 256), 256, 0, st>>>(p, t);
-    else gn_ltp_kernel<false><<<ceil_div((uint64_t)p.words_pad * 32, 256), 256, 0, st>>>(p, t);
+    if (p.packed) gn_ltp_kernel<true><<<148u * 8u, 256, 0, st>>>(p, t);
+    else gn_ltp_kernel<false><<<148u * 8u, 256, 0, st>>>(p, t);
     gn_age_kernel<<<ceil_div(p.Npad, 256), 256, 0, st>>>(p, t);
     return cudaGetLastError();
 }
