@@ -540,7 +540,7 @@ constexpr int kLogWarps = 8;
 template <bool PACKED>
 __device__ __forceinline__ void log_spikes(const GnDev &p, const uint32_t slot0, const uint32_t row0, const uint32_t n_batch)
 {
-    __shared__ uint32_t s_src[kLogWarps][1024];
+    __shared__ uint16_t s_src[kLogWarps][1024];          // fired vertices of the warp's 1,024, as offsets (16 KB: 8 CTAs per SM)
     __shared__ uint32_t s_tot[kLogWarps], s_base;
     __shared__ unsigned long long s_events;
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
@@ -561,7 +561,8 @@ __device__ __forceinline__ void log_spikes(const GnDev &p, const uint32_t slot0,
     const uint32_t total = __shfl_sync(0xFFFFFFFFu, incl, 31);
     if (lane == 0u) s_tot[warp] = total;
     if (threadIdx.x == 0) s_events = 0ull;
-    for (uint32_t k = incl - pc; word; ++k, word &= word - 1u) s_src[warp][k] = (w << 5) + (uint32_t)__ffs(word) - 1u;
+    const uint32_t v_warp = (w - lane) << 5;              // first vertex of the warp's 32 words
+    for (uint32_t k = incl - pc; word; ++k, word &= word - 1u) s_src[warp][k] = (uint16_t)((lane << 5) + (uint32_t)__ffs(word) - 1u);
     __syncthreads();
     uint32_t before = 0u, cta_total = 0u;                 // spikes of the warps in front of this one, of the whole CTA
 #pragma unroll
@@ -575,7 +576,7 @@ __device__ __forceinline__ void log_spikes(const GnDev &p, const uint32_t slot0,
     const uint32_t r = sl & ((1u << p.q_log) - 1u);       // D is a multiple of G: slot mod G = t mod G
     // the first 32 spikes of every warp: their loads go out before anybody waits for the reservation
     const bool valid0 = lane < total;
-    const uint32_t src0 = valid0 ? s_src[warp][lane] : 0u;
+    const uint32_t src0 = valid0 ? v_warp + s_src[warp][lane] : 0u;
     uint32_t beg, deg, first_v;
     log_load(p, r, src0, valid0, beg, deg, first_v);
     unsigned long long events = (unsigned long long)deg;
@@ -585,7 +586,7 @@ __device__ __forceinline__ void log_spikes(const GnDev &p, const uint32_t slot0,
     for (uint32_t q0 = 32u; q0 < total; q0 += 32u) {      // (a burst: more than 32 spikes among the warp's 1,024 vertices)
         const uint32_t q = q0 + lane;
         const bool valid = q < total;
-        const uint32_t src = valid ? s_src[warp][q] : 0u;
+        const uint32_t src = valid ? v_warp + s_src[warp][q] : 0u;
         log_load(p, r, src, valid, beg, deg, first_v);
         events += (unsigned long long)deg;
         log_store<PACKED>(p, sl, r, src, valid, beg, deg, first_v, base + q);
@@ -751,7 +752,7 @@ __device__ __forceinline__ void fold_group(const GnDev &p, const uint32_t win_sl
 // Launched just before gn_fold_kernel, which does not depend on it (it reads older log entries only): the trigger lets
 // the two run side by side.
 template <bool PACKED>
-__global__ void __launch_bounds__(kLogWarps * 32)
+__global__ void __launch_bounds__(kLogWarps * 32, 8)     // 984 CTAs at config 4: one wave, so that the fold behind it starts at once
 gn_log_kernel(const GnDev p, const uint32_t slot0, const uint32_t row0, const uint32_t n_batch)
 {
     asm volatile("griddepcontrol.launch_dependents;");
