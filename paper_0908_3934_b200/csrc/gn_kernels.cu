@@ -454,7 +454,7 @@ constexpr int kRouteThreads = 256;
 constexpr int kRouteWarps = kRouteThreads / 32;
 constexpr uint32_t kMaxWindow = 256;                    // steps one fold looks back over: (nb - W) G < D <= 255
 constexpr int kFoldUnroll = 4;                          // rounds of edge loads in flight per folding warp
-constexpr int kFoldCtasPerSm = 5;                       // folding CTAs per SM (persistent)
+constexpr int kFoldCtasPerSm = 4;                       // folding CTAs per SM (persistent)
 
 // #edges of the delay-sorted row [beg, beg+deg) with delay < thr.  Rows of up to 65,535 edges read it from the table
 // (entry k of the row's (src, r) line is the count for thr = (k+1)G - r); longer rows search for it.
