@@ -447,21 +447,37 @@ def main():
                     w=pin(net_in.weights), cls=pin(net_in.vertex_class),
                     net=None if net_in.net_offsets is None else pin(net_in.net_offsets.view(np.int32)))
         words = (N + 31) // 32
-        rast_host = torch.empty((S, words), dtype=torch.int32).pin_memory()
+        # the step's result (the raster of its S simulated steps) leaves through a device staging buffer and a copy stream,
+        # so that its device -> host copy runs beside the next step's kernels (two of each: a buffer is reused two steps on)
+        rast_host = [torch.empty((S, words), dtype=torch.int32).pin_memory() for _ in range(2)]
+        rast_dev = [torch.empty((S, words), dtype=torch.int32, device=dev) for _ in range(2)]
+        copied = [torch.cuda.Event() for _ in range(2)]
+        copy_stream = torch.cuda.Stream(device=dev)
         v_host = torch.empty(N, dtype=torch.float32).pin_memory()
         z_host = torch.empty((max(frames_per_step, 1), N), dtype=torch.float32).pin_memory() if obs else None
         h2d = sum(t.numel() * t.element_size() for t in host.values() if t is not None)
-        d2h = rast_host.numel() * 4 + (z_host.numel() * 4 if obs else 0) + v_host.numel() * 4 / K
+        d2h = rast_host[0].numel() * 4 + (z_host.numel() * 4 if obs else 0) + v_host.numel() * 4 / K
         barrier()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record()
         g2 = create(host)                                    # host -> device of every input, validation, quantisation, delays
+        main = torch.cuda.current_stream(dev)
         for k in range(K):
             gn.gn_step(g2, S)
-            gn.gn_read_raster(g2, k * S, S, rast_host.numpy().view(np.uint32))   # device -> host of the step's result
+            b = k & 1
+            if k >= 2:
+                main.wait_event(copied[b])                   # the buffer's previous copy has left
+            gn.gn_read_raster(g2, k * S, S, rast_dev[b])     # device destination: asynchronous on the handle's stream
+            ready = torch.cuda.Event()
+            ready.record(main)
+            copy_stream.wait_event(ready)
+            with torch.cuda.stream(copy_stream):
+                rast_host[b].copy_(rast_dev[b], non_blocking=True)      # device -> host of the step's result
+                copied[b].record(copy_stream)
             if obs:
                 gn.gn_observe(g2, k * frames_per_step, frames_per_step, z_host.numpy())
         gn.gn_read_state(g2, gn.GN_V, v_host.numpy())
+        main.wait_stream(copy_stream)
         e1.record()
         barrier()
         ems = e0.elapsed_time(e1)
@@ -469,7 +485,8 @@ def main():
         e2e = {"value": world * N * sim_steps / (ems * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d / K,
                "d2h_bytes_per_step": d2h, "ms_total": ems,
                "what": "gn_create from pinned host arrays (upload + validation + quantisation + eq. 25 delays) + K x "
-                       "[gn_step(S) + gn_read_raster of the S steps to pinned host memory] + final V to host"}
+                       "[gn_step(S) + gn_read_raster of the S steps, through a device staging buffer and a copy stream, to pinned "
+                       "host memory] + final V to host"}
         del g2
 
     line = {
