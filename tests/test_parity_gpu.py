@@ -956,3 +956,16 @@ def test_plastic_mode_argument_checks(gn):
     g = _plastic(gn, net, cfg, 10, dl)
     with pytest.raises(gn.GnError):
         gn.gn_write_state(g, gn.GN_STEP, np.array([5], np.uint64))
+
+
+def test_debug_ceilings_measure_something_sane(gn):
+    """gn_debug_ceilings (the roofline bench.py rates event delivery against): both rates positive, the gather in front of
+    the reductions can only cost, longer segments can only help, and bad arguments are refused."""
+    red7, both7 = gn.gn_debug_ceilings(7, scratch_mb=512)
+    red100, both100 = gn.gn_debug_ceilings(100, scratch_mb=512)
+    assert 2e10 < both7 < red7 * 1.05 and 2e10 < both100 < red100 * 1.05
+    assert both100 > 0.9 * both7
+    with pytest.raises(gn.GnError):
+        gn.gn_debug_ceilings(0, scratch_mb=512)
+    with pytest.raises(gn.GnError):
+        gn.gn_debug_ceilings(7, scratch_mb=64)
