@@ -382,7 +382,7 @@ def main():
         avg_s = kms[k] * 1e-3 / kn[k]
         row = {"kernel": names[k], "launches": int(kn[k]), "avg_us": avg_s * 1e6, "share": float(kms[k] / kms.sum()),
                "bytes_per_launch": kbytes[k], "achieved": kbytes[k] / avg_s / 1e9, "frac": kbytes[k] / avg_s / 1e9 / peak}
-        tr = traffic_tab.get(names[k].split()[0])
+        tr = traffic_tab.get(names[k].split()[0] + ("_hh" if args.model == "hh" and k == 0 else ""))
         if tr is not None:      # what DRAM really moved for this kernel (ncu capture named in traffic_source) over the live time
             row["traffic"] = tr[1] * p_events / kn[k] if tr[1] is not None else tr[0]
             row["dram_frac"] = row["traffic"] / avg_s / 1e9 / peak

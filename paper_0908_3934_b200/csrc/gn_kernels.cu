@@ -171,7 +171,7 @@ __device__ __forceinline__ bool vertex_step_hh(const GnClassDev &q, const float 
 // Thread g owns vertices 4g .. 4g+3 (128-bit SoA loads); a warp owns 128 vertices = 4 raster words.
 // HH: some class is a Hodgkin-Huxley one (two more fp32 streams, m and h; a vertex takes its class's transition function).
 template <bool OBS, bool BIAS, bool FUSED, bool ALPHA, bool HH>
-__global__ void __launch_bounds__(kUpdateThreads, HH ? 3 : (FUSED || ALPHA) ? 4 : 8)
+__global__ void __launch_bounds__(kUpdateThreads, HH ? 4 : (FUSED || ALPHA) ? 4 : 8)
 gn_update_kernel(const GnDev p, const uint64_t t, const uint32_t slot, const uint32_t raster_row,
                  const uint32_t d_direct)
 {
