@@ -576,9 +576,9 @@ static int join_streams(gn_net *net)
 // runs on a side stream beside update(t+1).
 //
 // Queue mode.  Steps come in groups of G = 2^q_log (the ring rows of one group are folded together); W = q_window.
-// update(t), t in group h, sends every event due in groups h .. h+W itself.  After the last update of group h two
+// update(t), t in group h, sends every event due in groups h .. h+W-1 itself.  After the last update of group h two
 // kernels go to the side stream, beside the updates of group h+1 (and beside each other):
-//   gn_log_kernel enters the spikes of group h's steps into the spike log;
+//   gn_log_kernel sends the events of group h's spikes due in group h+W and enters the spikes into the spike log;
 //   gn_fold_kernel expands, out of the log of groups h+W-nb .. h-1 (complete since the previous launches on that
 //   stream), the events due in group h+W into that group's ring rows.
 // update(first step of h+W) waits for that launch: W-1 groups of slack.  The raster rows a launch reads are

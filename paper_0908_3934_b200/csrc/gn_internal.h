@@ -77,7 +77,8 @@ struct GnDev {
     uint32_t res_threads;    // CTA size = largest network rounded up to 32 (1,024 in cluster mode)
     uint32_t res_smem;       // dynamic shared memory: ring [D][res_threads] + drive words
     const uint32_t *net_off; // [n_networks + 1] first vertex of every network
-    uint32_t q_window;       // queue mode: groups ahead of the current one whose events the update kernel sends itself
+    uint32_t q_window;       // queue mode, W: the update kernel sends the events due fewer than W groups ahead itself, the
+                             //     logging kernel those due exactly W groups ahead; later ones are logged
     uint16_t *q_seg;         // [N][2^q_log][q_nb] segment boundaries of every delay-sorted row (rows of more than 65,535
                              //     edges have no entry: their boundaries are searched for)
     // the spike log: for the spike at position i of step t (slot t mod D) and every group offset j = q_window+1 ..

@@ -282,7 +282,8 @@ gn_update_kernel(const GnDev p, const uint64_t t, const uint32_t slot, const uin
     // a4, the urgent part: events due before the delivery kernel of this step is guaranteed to have run are
     // sent by the vertex that fired (rows are sorted by delay: such edges lead the row).  Ring mode: delay 1
     // (d_direct = 2), so that deliver(t) may overlap update(t+1).  Queue mode: every delay that lands in the
-    // group being consumed or in the next W = q_window (d_direct = (W+1)G - r), so that routing runs once per group.
+    // group being consumed or in the next W - 1 (W = q_window; d_direct = WG - r): the logging kernel at the group's end
+    // sends what is due W groups ahead, the fold kernels the rest.
     // FUSED (ring mode, small networks: a step is bound by launch latency, not by work): the whole of a4 happens here,
     // warp-cooperatively -- every fired vertex of the warp in turn, lanes over its row -- and there is no delivery kernel.
     if (FUSED) {
@@ -437,14 +438,15 @@ gn_deliver_kernel(const GnDev p, const uint32_t slot_t, const uint32_t raster_ro
 // Rows are sorted by delay at create time, so the events of a spike at step t (r = t mod G) that land j groups
 // ahead -- delays [jG - r, (j+1)G - r) -- are one contiguous SEGMENT of its row, and the segment boundaries depend
 // only on r: q_seg[(src * G + r) * nb + j-1] = #edges of src with delay < jG - r (create time).
-//     j = 0 .. W            (W = q_window) sent by the update kernel itself when the vertex fires
+//     j = 0 .. W-1          (W = q_window) sent by the update kernel itself when the vertex fires
+//     j = W                 sent by the logging kernel of the spike's group (it runs a whole group before group h+W is read)
 //     j = W+1 .. nb         logged: the spike's entry in log array j-W-1 is the (absolute) index of the segment's first
 //                           edge, array j-W its end; j = nb is the wrapped tail (r + delay >= D: the group's own rows,
 //                           consumed on the next lap)
 // One launch per slot group h, after the group's last update, beside the updates of group h+1:
 //   LOGGING CTAs  compact the raster rows of the group's steps (a3: popc prefix, no global list), reserve log
-//                 positions with one atomic per step and CTA, and write nb-W+1 words per spike (a spike beyond the
-//                 log's capacity is expanded on the spot, straight into the ring);
+//                 positions with one atomic per step and CTA, send the spike's events due W groups ahead and write
+//                 nb-W+1 words per spike (a spike beyond the log's capacity is expanded on the spot, into the ring);
 //   FOLDING CTAs  take group g = h+W, due to be consumed one group later: for every step of groups g-nb .. g-W-1
 //                 (all logged by earlier launches) and every spike of it, the segment due in g -- two coalesced log
 //                 reads -- is expanded: one 8-byte edge load and one int32 RED per event into rows that stay in L2.
@@ -472,60 +474,74 @@ __device__ __forceinline__ uint32_t seg_bound(const GnDev &p, const uint16_t *__
     return lo;
 }
 
-// One spike per lane (`valid`): the row bounds of the fired vertex and the first word of its line of the segment table
-// are requested.  Nothing here depends on the spike's log position.
+// One spike per lane (`valid`): the row bounds of the fired vertex and two words of its line of the segment table are
+// requested: where the events due exactly q_window groups ahead begin (lo_v) and end (first_v = where the logged ones
+// begin).  Nothing here depends on the spike's log position.
 __device__ __forceinline__ void log_load(const GnDev &p, const uint32_t r, const uint32_t src, const bool valid, uint32_t &beg,
-                                         uint32_t &deg, uint32_t &first_v)
+                                         uint32_t &deg, uint32_t &lo_v, uint32_t &first_v)
 {
-    beg = deg = first_v = 0u;
+    beg = deg = lo_v = first_v = 0u;
     if (valid) {
         beg = p.row[src];
         deg = p.row[src + 1] - beg;
-        if (p.q_arrays >= 2u && deg <= 0xFFFFu)
-            first_v = (uint32_t)__ldg(p.q_seg + (((size_t)src << p.q_log) + r) * p.q_nb + p.q_window);
+        lo_v = first_v = deg;
+        if (deg <= 0xFFFFu) {
+            const uint16_t *line = p.q_seg + (((size_t)src << p.q_log) + r) * p.q_nb;
+            if (p.q_window - 1u < p.q_nb) lo_v = (uint32_t)__ldg(line + p.q_window - 1u);
+            if (p.q_window < p.q_nb) first_v = (uint32_t)__ldg(line + p.q_window);
+        }
     }
 }
 
-// ... and entered into the log of step slot `sl` (r = sl mod G) at position `pos`: the nb-W+1 entries of a spike are
-// stored by its lane -- lanes hold consecutive positions, so every array receives one coalesced run per warp.  The rest
-// is rare and done by the whole warp, spike after spike: rows too long for the table (their boundaries are searched for,
-// one per lane), and spikes beyond the log's capacity (expanded now, straight into the ring).  Whole warps only.
+// ... then (whole warps only), with r = sl mod G and W = q_window:
+//   the events due exactly W groups ahead -- edges [lo_v, first_v) of the row, about one per spike -- are sent here, straight
+//   into the ring (the update kernel sends only what is due sooner: this launch runs a whole group before their slots are read);
+//   the spike is entered into the log of step slot `sl` at position `pos`: its nb-W+1 entries are stored by its lane -- lanes
+//   hold consecutive positions, so every array receives one coalesced run per warp.
+// The rest is rare and done by the whole warp, spike after spike: rows too long for the table (their boundaries are searched
+// for, one per lane), and spikes beyond the log's capacity (expanded now, straight into the ring).
 template <bool PACKED>
 __device__ __forceinline__ void log_store(const GnDev &p, const uint32_t sl, const uint32_t r, const uint32_t src, const bool valid,
-                                          const uint32_t beg, const uint32_t deg, const uint32_t first_v, const uint32_t pos)
+                                          const uint32_t beg, const uint32_t deg, const uint32_t lo_v, const uint32_t first_v,
+                                          const uint32_t pos)
 {
     const uint32_t lane = threadIdx.x & 31u;
     const uint32_t G = 1u << p.q_log, nb = p.q_nb, W = p.q_window, A = p.q_arrays;
-    if (A < 2u) return;                                   // every event is the update kernel's
-    const uint16_t *line = p.q_seg + ((size_t)src * G + r) * nb;
+    auto send = [&](const uint32_t e) {
+        const uint2 ev = __ldg(p.s_edge + e);
+        const uint32_t d = PACKED ? ev.x >> 24 : (uint32_t)__ldg(p.s_dly + e);
+        uint32_t s1 = sl + d;
+        if (s1 >= p.D) s1 -= p.D;
+        atomicAdd(p.ring + (size_t)s1 * p.Npad + (PACKED ? ev.x & 0xFFFFFFu : ev.x), (int32_t)ev.y);
+    };
     const bool in_table = valid && deg <= 0xFFFFu, logged = valid && pos < p.log_cap;
-    if (in_table && logged) {
+    if (in_table)
+        for (uint32_t x = lo_v; x < first_v; ++x) send(beg + x);
+    const uint16_t *line = p.q_seg + ((size_t)src * G + r) * nb;
+    if (A >= 2u && in_table && logged) {
         uint32_t *dst = p.spk_log + ((size_t)sl * A) * p.log_cap + pos;
         dst[0] = beg + first_v;
 #pragma unroll 6
         for (uint32_t a = 1u; a + 1u < A; ++a) dst[(size_t)a * p.log_cap] = beg + (uint32_t)__ldg(line + W + a);
         dst[(size_t)(A - 1u) * p.log_cap] = beg + deg;
     }
-    for (uint32_t m = __ballot_sync(0xFFFFFFFFu, valid && (!in_table || !logged)); m; m &= m - 1u) {
+    for (uint32_t m = __ballot_sync(0xFFFFFFFFu, valid && (!in_table || (A >= 2u && !logged))); m; m &= m - 1u) {
         const int sq = __ffs(m) - 1;
         const uint32_t b2 = __shfl_sync(0xFFFFFFFFu, beg, sq), d2 = __shfl_sync(0xFFFFFFFFu, deg, sq);
         const uint32_t src2 = __shfl_sync(0xFFFFFFFFu, src, sq), pos2 = __shfl_sync(0xFFFFFFFFu, pos, sq);
+        uint32_t x_w = __shfl_sync(0xFFFFFFFFu, first_v, sq);       // where the logged events begin
         const uint16_t *line2 = p.q_seg + ((size_t)src2 * G + r) * nb;
-        if (pos2 < p.log_cap) {
+        auto bound = [&](const uint32_t k) { return k < nb ? seg_bound<PACKED>(p, line2, k, (k + 1u) * G - r, b2, d2) : d2; };
+        if (d2 > 0xFFFFu) {                               // a long row: its events due W groups ahead, by the warp
+            x_w = bound(W);
+            for (uint32_t x = bound(W - 1u) + lane; x < x_w; x += 32u) send(b2 + x);
+        }
+        if (A < 2u) continue;                             // nothing is ever logged
+        if (pos2 < p.log_cap) {                           // (a long row: an in-table row with a position was logged above)
             uint32_t *dst2 = p.spk_log + ((size_t)sl * A) * p.log_cap + pos2;
-            for (uint32_t a = lane; a < A; a += 32u) {
-                const uint32_t j = W + 1u + a;
-                dst2[(size_t)a * p.log_cap] = b2 + (j <= nb ? seg_bound<PACKED>(p, line2, j - 1u, j * G - r, b2, d2) : d2);
-            }
+            for (uint32_t a = lane; a < A; a += 32u) dst2[(size_t)a * p.log_cap] = b2 + bound(W + a);
         } else {
-            const uint32_t x_first = seg_bound<PACKED>(p, line2, W, (W + 1u) * G - r, b2, d2);
-            for (uint32_t x = x_first + lane; x < d2; x += 32u) {
-                const uint2 ev = __ldg(p.s_edge + b2 + x);
-                const uint32_t d = PACKED ? ev.x >> 24 : (uint32_t)__ldg(p.s_dly + b2 + x);
-                uint32_t s1 = sl + d;
-                if (s1 >= p.D) s1 -= p.D;
-                atomicAdd(p.ring + (size_t)s1 * p.Npad + (PACKED ? ev.x & 0xFFFFFFu : ev.x), (int32_t)ev.y);
-            }
+            for (uint32_t x = x_w + lane; x < d2; x += 32u) send(b2 + x);
         }
     }
 }
@@ -577,19 +593,19 @@ __device__ __forceinline__ void log_spikes(const GnDev &p, const uint32_t slot0,
     // the first 32 spikes of every warp: their loads go out before anybody waits for the reservation
     const bool valid0 = lane < total;
     const uint32_t src0 = valid0 ? v_warp + s_src[warp][lane] : 0u;
-    uint32_t beg, deg, first_v;
-    log_load(p, r, src0, valid0, beg, deg, first_v);
+    uint32_t beg, deg, lo_v, first_v;
+    log_load(p, r, src0, valid0, beg, deg, lo_v, first_v);
     unsigned long long events = (unsigned long long)deg;
     __syncthreads();
     const uint32_t base = s_base + before;
-    log_store<PACKED>(p, sl, r, src0, valid0, beg, deg, first_v, base + lane);
+    log_store<PACKED>(p, sl, r, src0, valid0, beg, deg, lo_v, first_v, base + lane);
     for (uint32_t q0 = 32u; q0 < total; q0 += 32u) {      // (a burst: more than 32 spikes among the warp's 1,024 vertices)
         const uint32_t q = q0 + lane;
         const bool valid = q < total;
         const uint32_t src = valid ? v_warp + s_src[warp][q] : 0u;
-        log_load(p, r, src, valid, beg, deg, first_v);
+        log_load(p, r, src, valid, beg, deg, lo_v, first_v);
         events += (unsigned long long)deg;
-        log_store<PACKED>(p, sl, r, src, valid, beg, deg, first_v, base + q);
+        log_store<PACKED>(p, sl, r, src, valid, beg, deg, lo_v, first_v, base + q);
     }
 #pragma unroll
     for (int o = 16; o >= 1; o >>= 1) events += __shfl_xor_sync(0xFFFFFFFFu, events, o);
@@ -1595,7 +1611,7 @@ cudaError_t gnk_update(const GnDev &p, uint64_t t, bool has_bias, cudaStream_t s
 {
     // delays below d_direct are delivered by the update kernel itself (see the kernel)
     const uint32_t d_direct = p.plastic ? 1u      // plastic mode: nothing is sent when a vertex fires (delivery happens at arrival)
-                            : p.queue_mode ? ((p.q_window + 1u) << p.q_log) - ((uint32_t)(t % p.D) & ((1u << p.q_log) - 1u)) : 2u;
+                            : p.queue_mode ? (p.q_window << p.q_log) - ((uint32_t)(t % p.D) & ((1u << p.q_log) - 1u)) : 2u;
     const uint32_t grid = ceil_div(p.Npad / kVertsPerThread, kUpdateThreads);
     const uint32_t slot = (uint32_t)(t % p.D);
     const uint32_t raster_row = (uint32_t)(t % p.raster_rows);
