@@ -133,6 +133,7 @@ struct gn_net {
     uint64_t t_origin;   // first step simulated by this handle (0, or the t a checkpoint was restored at)
     unsigned long long sync_base;   // persistent step driver: value of its barrier counter when the next launch starts
     uint64_t routed_upto; // queue mode: steps < routed_upto have been entered into the spike log
+    uint64_t zeroed_upto;  // queue mode: the log's spike counts of steps < zeroed_upto (not logged yet) are zero already
     uint64_t flushed_upto; // queue mode: every event of steps < flushed_upto is in the ring already (a read-back expanded them)
     // delivery of step t overlaps the update of step t+1 (see gn_step): side streams and their fences
     cudaStream_t s_deliver;
@@ -245,6 +246,7 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
     net->t_origin = 0;
     net->routed_upto = 0;
     net->flushed_upto = 0;
+    net->zeroed_upto = 0;
     net->sync_base = 0;
     net->s_deliver = nullptr;
     net->ev_update = net->ev_deliver[0] = net->ev_deliver[1] = net->ev_fold[0] = net->ev_fold[1] = net->ev_fold[2] = net->ev_fold[3] = nullptr;
@@ -613,9 +615,16 @@ static int route_pending(gn_net *net, cudaStream_t st, bool prof, uint64_t g_fol
     if (n_batch == 0 && n_win == 0) return GN_OK;
     int rc;
     if (n_batch) {
-        if ((rc = zero_log_counts(net, net->routed_upto, net->t, st))) return rc;
+        const uint64_t z0 = net->routed_upto > net->zeroed_upto ? net->routed_upto : net->zeroed_upto;
+        if (z0 < net->t && (rc = zero_log_counts(net, z0, net->t, st))) return rc;      // (steady state: the previous launch did it)
+        // at a group's end the next group's counts are zeroed by this launch: what they hold now -- the counts of the group a lap
+        // earlier -- was last wanted by the fold of the next group itself, issued a launch ago (or clipped away by a read-back)
+        const uint32_t G = 1u << d.q_log;
+        const bool at_group_end = (net->t & (uint64_t)(G - 1u)) == 0;
+        const uint32_t zero_next = (at_group_end && d.D >= 2u * G) ? G : 0u;
         if (prof && (rc = prof_mark(net, 1))) return rc;
-        GN_CUDA(net, gnk_log(d, net->routed_upto, n_batch, st));
+        GN_CUDA(net, gnk_log(d, net->routed_upto, n_batch, zero_next, st));
+        if (net->zeroed_upto < net->t + zero_next) net->zeroed_upto = net->t + zero_next;
         net->launches++;
     }
     if (n_win) {
@@ -896,6 +905,7 @@ int gn_write_state(gn_net *net, int which, const void *src, size_t src_bytes, in
         net->t = c[0];
         net->routed_upto = c[0];
         net->flushed_upto = c[0];
+        net->zeroed_upto = 0;
         net->t_origin = c[0];
         return GN_OK;
     }

@@ -118,7 +118,8 @@ cudaError_t gnk_deliver(const GnDev &p, uint64_t t, cudaStream_t st);
 // gnk_fold: for the n_win steps starting at step t_win, the log entries due in absolute slot group g_fold are expanded and
 // added into that group's ring rows; beside_previous: it may start while the kernel in front of it in the stream is
 // still running (the logging kernel of the same group end, which it does not depend on).
-cudaError_t gnk_log(const GnDev &p, uint64_t t0, uint32_t n_batch, cudaStream_t st);
+// zero_next: the spike counts of that many steps after the batch are zeroed as well (at most D - n_batch, at most 256)
+cudaError_t gnk_log(const GnDev &p, uint64_t t0, uint32_t n_batch, uint32_t zero_next, cudaStream_t st);
 cudaError_t gnk_fold(const GnDev &p, uint64_t t_win, uint32_t n_win, uint64_t g_fold, bool beside_previous, cudaStream_t st);
 cudaError_t gnk_sort_rows(const GnDev &p, GnCheck *chk, cudaStream_t st);
 // plastic mode: in-edge lists (csc_*; csc_off must hold zeros), then per step arrive -> update -> plasticity

@@ -769,9 +769,16 @@ __device__ __forceinline__ void fold_group(const GnDev &p, const uint32_t win_sl
 // the two run side by side.
 template <bool PACKED>
 __global__ void __launch_bounds__(kLogWarps * 32, 8)     // 984 CTAs at config 4: one wave, so that the fold behind it starts at once
-gn_log_kernel(const GnDev p, const uint32_t slot0, const uint32_t row0, const uint32_t n_batch)
+gn_log_kernel(const GnDev p, const uint32_t slot0, const uint32_t row0, const uint32_t n_batch, const uint32_t zero_next)
 {
     asm volatile("griddepcontrol.launch_dependents;");
+    // the spike counts of the zero_next steps after this batch are zeroed for the next launch (their slots hold the counts of
+    // D steps earlier, which no fold still to come reads: the launcher checks that)
+    if (blockIdx.x == 0 && threadIdx.x < zero_next) {
+        uint32_t sl = slot0 + n_batch + threadIdx.x;
+        while (sl >= p.D) sl -= p.D;
+        p.log_n[sl] = 0u;
+    }
     log_spikes<PACKED>(p, slot0, row0, n_batch);
 }
 
@@ -1782,13 +1789,13 @@ cudaError_t gnk_deliver(const GnDev &p, uint64_t t, cudaStream_t st)
     return cudaGetLastError();
 }
 
-cudaError_t gnk_log(const GnDev &p, uint64_t t0, uint32_t n_batch, cudaStream_t st)
+cudaError_t gnk_log(const GnDev &p, uint64_t t0, uint32_t n_batch, uint32_t zero_next, cudaStream_t st)
 {
     if (n_batch == 0u) return cudaSuccess;
     const uint32_t slot0 = (uint32_t)(t0 % p.D), row0 = (uint32_t)(t0 % p.raster_rows);
     const uint32_t grid = n_batch * ceil_div(p.words_pad, kLogWarps * 32u);   // a warp per step and 32 raster words
-    if (p.packed) gn_log_kernel<true><<<grid, kLogWarps * 32, 0, st>>>(p, slot0, row0, n_batch);
-    else gn_log_kernel<false><<<grid, kLogWarps * 32, 0, st>>>(p, slot0, row0, n_batch);
+    if (p.packed) gn_log_kernel<true><<<grid, kLogWarps * 32, 0, st>>>(p, slot0, row0, n_batch, zero_next);
+    else gn_log_kernel<false><<<grid, kLogWarps * 32, 0, st>>>(p, slot0, row0, n_batch, zero_next);
     return cudaGetLastError();
 }
 
