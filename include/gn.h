@@ -126,8 +126,8 @@ typedef struct {
  *   offset, where in its delay-sorted row the events due that many groups ahead begin -- and its events are expanded
  *   and added ("folded") into the ring group by group, each group just before it is consumed, while the group's rows
  *   sit in L2 (best when the ring is >> L2: no 32-byte DRAM sector read-modify-write per event, and nothing per event
- *   is written or read back).  Logging and folding run once per group of steps; events due within two groups are sent
- *   by the update kernel itself.  Needs ring_slots to be a multiple of the group (else a smaller group is taken).
+ *   is written or read back).  Logging and folding run once per group of steps; events due in the current or the next
+ *   group are sent by the update kernel itself, those due in the group after by the logging kernel.  Needs ring_slots to be a multiple of the group (else a smaller group is taken).
  * RESIDENT: every network (n_networks >= 1) lives in ONE CTA -- or, above 1,024 vertices, one thread-block cluster of
  *   up to 16 CTAs -- for a whole gn_step call: vertex state in registers, the network's delay ring in (distributed)
  *   shared memory, delivery by shared-memory integer atomics, one barrier per step and no per-step kernel launch
