@@ -354,7 +354,7 @@ def main():
              "gn_log_kernel (a3 compaction + a4: spikes into the log)" if queue_mode else
              "gn_arrive_kernel (a4 at arrival time: plastic weights)" if args.stdp else "gn_deliver_kernel (a4)",
              "gn_observe_kernel (a5)",
-             "gn_arrive_kernel<LTD> + gn_ltp_kernel + gn_age_kernel (eq. 33, eq. 32)" if args.stdp else
+             "gn_spikes_kernel + gn_plast_kernel (eq. 32, eq. 33)" if args.stdp else
              "gn_fold_kernel (a4: expansion of the log + ring reductions)"]
     p_events, p_spikes = cp1[2] - cp0[2], cp1[1] - cp0[1]
     # algorithmic bytes per launch: 17 B per event (+12 B per fired source) for the

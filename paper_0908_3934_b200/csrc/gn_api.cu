@@ -110,7 +110,7 @@ Layout make_layout(const gn_config *cfg)
     const bool plastic = cfg->stdp_alpha != 0.0f;
     L.q_seg = take(qp.on || plastic ? N * D * 2 : 0);
     L.w_f32 = take(plastic ? E * 4 : 0); L.perm = take(plastic ? E * 4 : 0); L.w_stage = take(plastic ? E * 4 : 0);
-    L.ls_hist = take(plastic ? D * Npad * 4 : 0); L.pl_list = take(plastic ? D * Npad * 4 : 0);
+    L.ls_hist = take(plastic ? (D + 1) * Npad * 4 : 0); L.pl_list = take(plastic ? D * Npad * 4 : 0);
     L.csc_off = take(plastic ? (Npad + 2) * 4 : 0); L.csc_edge = take(plastic ? E * 4 : 0); L.csc_src = take(plastic ? E * 4 : 0);
     L.spk_log = take(qp.on && qp.arrays >= 2 ? D * qp.arrays * (size_t)qp.log_cap * 4 : 0);
     L.scratch_row64 = take((N + 1) * 8); L.scratch_abs = take(N * 8);
@@ -490,7 +490,7 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
         GN_CREATE_CUDA(cudaMemsetAsync(d.csc_off, 0, ((size_t)Npad + 2) * 4, st));
         GN_CREATE_CUDA(cudaMemsetAsync(abs_in, 0, (size_t)N * 4, st));
         GN_CREATE_CUDA(gnk_build_csc(d, E, (uint32_t *)abs_in, st));
-        GN_CREATE_CUDA(cudaMemsetAsync(d.ls_hist, 0xFF, (size_t)cfg->ring_slots * Npad * 4, st));
+        GN_CREATE_CUDA(cudaMemsetAsync(d.ls_hist, 0xFF, ((size_t)cfg->ring_slots + 1) * Npad * 4, st));
     }
     GN_CREATE_CUDA(cudaMemcpyAsync(&chk, chk_d, sizeof chk, cudaMemcpyDeviceToHost, st));
     GN_CREATE_CUDA(cudaStreamSynchronize(st));
@@ -672,7 +672,7 @@ int gn_step(gn_net *net, uint64_t n_steps)
             GN_CUDA(net, gnk_update(d, t, net->has_bias, net->stream));
             if (prof && (rc = prof_mark(net, 3))) return rc;
             GN_CUDA(net, gnk_plasticity(d, t, net->t_origin, net->stream));
-            net->launches += 6;
+            net->launches += 4;
             net->t = t + 1;
             if (prof && (s + 1) % kProfChunk == 0 && ((rc = prof_mark(net, 0xFF)) || (rc = prof_collect(net)))) return rc;
         }

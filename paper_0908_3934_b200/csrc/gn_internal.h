@@ -93,7 +93,7 @@ struct GnDev {
     float stdp_dta, stdp_beta;      // (float)(dt * alpha), beta
     float *w_f32;                   // [E] current weight of s_edge[e] (the int32 in s_edge[e].y is the initial one)
     uint32_t *perm;                 // [E] caller's edge index of s_edge[e]
-    int32_t *ls_hist;               // [D][Npad] row t mod D: last spike step of every vertex strictly before t (-1: none)
+    int32_t *ls_hist;               // [D+1][Npad] row t mod (D+1): last spike step of every vertex strictly before t (-1: none)
     uint32_t *pl_list;              // [D][Npad] row t mod D: the vertices that fired at step t (log_n[t mod D] of them)
     uint32_t *csc_off, *csc_edge, *csc_src;   // in-edges by target: [Npad+1] offsets, [E] position in s_edge, [E] source
     float *w_stage;                 // [E] staging of GN_WEIGHTS read-back (caller's edge order)

@@ -1270,16 +1270,17 @@ gn_persist_kernel(const GnDev p, const uint64_t t0, const uint32_t n_steps, unsi
 // ---- plastic mode: spike-time dependent plasticity (eq. 32-33; readings #22, #23) ----------
 // Every weight is a state of its own (eq. 9) and eq. 30 weighs an arriving spike with the weight AT THE ARRIVAL step, so
 // nothing is delivered when a vertex fires: per step t
-//   gn_arrive_kernel<false>  for every delay d and every vertex i that fired at t - d (the spike list of that step), the edges
+//   gn_arrive_kernel         for every delay d and every vertex i that fired at t - d (the spike list of that step), the edges
 //                            of i with delay exactly d -- a contiguous run of its delay-sorted row, boundaries from the
 //                            per-delay table (q_seg with groups of one slot) -- add rint(w(t) 2^16) to ring[t mod D][target];
 //   gn_update_kernel         as ever (a1-a3); it sends nothing itself;
-//   gn_spikes_kernel         the fired vertices of step t, listed (row t mod D of pl_list: the spikes in flight are these lists);
-//   gn_arrive_kernel<true>   the same enumeration again, now that the spikes of step t are known: an arrival at a target
+//   gn_spikes_kernel         the fired vertices of step t, listed (row t mod D of pl_list: the spikes in flight are these
+//                            lists), and eq. 32 as integers: row t+1 of ls_hist = t where the vertex fired, else row t;
+//   gn_plast_kernel          eq. 33, its two halves in alternate CTAs:
+//     (weakening)            the same enumeration again, now that the spikes of step t are known: an arrival at a target
 //                            that does not fire at t weakens its edge, w -= dt alpha exp(-beta s_j(t));
-//   gn_ltp_kernel            every vertex j that fired at t strengthens each in-edge (i -> j, d) on which nothing arrives
+//     (strengthening)        every vertex j that fired at t strengthens each in-edge (i -> j, d) on which nothing arrives
 //                            at t: w += dt alpha exp(-beta s_i(t - d)), the age read from the history of last-spike steps;
-//   gn_age_kernel            eq. 32 as integers: row t+1 of ls_hist = t where the vertex fired, else row t.
 // An edge is touched by at most one thread per step (one arrival per step; weakening needs the target silent,
 // strengthening needs it firing), so the weights need no atomics.  Arithmetic (fp32, one rounded operation each):
 // age = steps * dt with steps = t - last - 1 (eq. 32: the age is 0 for the step after a spike, so steps = 0 is q = 0: no
@@ -1297,14 +1298,19 @@ __device__ __forceinline__ float stdp_dw(const GnDev &p, const uint32_t steps)
     return __fmul_rn(p.stdp_dta, exp32(-__fmul_rn(p.stdp_beta, age)));
 }
 
-// The fired vertices of step t, listed (any order) in row t mod D of pl_list; log_n[t mod D] = how many (zeroed by the launcher).
+// The fired vertices of step t, listed (any order) in row t mod D of pl_list; log_n[t mod D] = how many (zeroed by the
+// launcher).  And eq. 32 as integers: row t+1 of ls_hist (D + 1 rows, so that the row of step t - (D-1) survives) = t where
+// the vertex fired, else row t.
 __global__ void __launch_bounds__(256)
 gn_spikes_kernel(const GnDev p, const uint64_t t)
 {
     const uint32_t j = blockIdx.x * 256u + threadIdx.x, lane = threadIdx.x & 31u;
     const uint32_t slot = (uint32_t)(t % p.D);
     bool fired = false;
-    if (j < p.Npad) fired = (p.raster[(size_t)(t % p.raster_rows) * p.words_pad + (j >> 5)] >> (j & 31u)) & 1u;
+    if (j < p.Npad) {
+        fired = (p.raster[(size_t)(t % p.raster_rows) * p.words_pad + (j >> 5)] >> (j & 31u)) & 1u;
+        p.ls_hist[(size_t)((t + 1ull) % (p.D + 1u)) * p.Npad + j] = fired ? (int32_t)t : p.ls_hist[(size_t)(t % (p.D + 1u)) * p.Npad + j];
+    }
     const uint32_t m = __ballot_sync(0xFFFFFFFFu, fired);
     if (m == 0u) return;
     uint32_t base = 0u;
@@ -1318,8 +1324,7 @@ gn_spikes_kernel(const GnDev p, const uint64_t t)
 
 // One thread per (delay d, vertex that fired at t - d), the pairs flattened over the lists of the last n_d steps.
 template <bool LTD, bool PACKED>
-__global__ void __launch_bounds__(256)
-gn_arrive_kernel(const GnDev p, const uint64_t t, const uint32_t n_d)
+__device__ __forceinline__ void arrive_body(const GnDev &p, const uint64_t t, const uint32_t n_d, const uint32_t bid, const uint32_t n_blocks)
 {
     __shared__ uint32_t s_pref[256];
     __shared__ uint32_t s_wsum[8];
@@ -1332,8 +1337,8 @@ gn_arrive_kernel(const GnDev p, const uint64_t t, const uint32_t n_d)
     unsigned long long events = 0ull;
     const uint32_t slot = (uint32_t)(t % p.D);
     const uint32_t *fired_now = p.raster + (size_t)(t % p.raster_rows) * p.words_pad;
-    const int32_t *last = p.ls_hist + (size_t)slot * p.Npad;
-    for (uint32_t pidx = blockIdx.x * 256u + threadIdx.x; pidx < P; pidx += gridDim.x * 256u) {
+    const int32_t *last = p.ls_hist + (size_t)(t % (p.D + 1u)) * p.Npad;
+    for (uint32_t pidx = bid * 256u + threadIdx.x; pidx < P; pidx += n_blocks * 256u) {
         uint32_t lo = 0u, hi_s = n_d;                       // the last delay index whose pairs start at or before pidx
         while (hi_s - lo > 1u) {
             const uint32_t mid = (lo + hi_s) >> 1;
@@ -1364,12 +1369,11 @@ gn_arrive_kernel(const GnDev p, const uint64_t t, const uint32_t n_d)
 
 // One warp per vertex that fired at t (its list), lanes over its in-edges.
 template <bool PACKED>
-__global__ void __launch_bounds__(256)
-gn_ltp_kernel(const GnDev p, const uint64_t t)
+__device__ __forceinline__ void ltp_body(const GnDev &p, const uint64_t t, const uint32_t bid, const uint32_t n_blocks)
 {
-    const uint32_t lane = threadIdx.x & 31u, n_warps = (gridDim.x * 256u) >> 5;
+    const uint32_t lane = threadIdx.x & 31u, n_warps = (n_blocks * 256u) >> 5;
     const uint32_t slot = (uint32_t)(t % p.D), n = p.log_n[slot];
-    for (uint32_t q = (blockIdx.x * 256u + threadIdx.x) >> 5; q < n; q += n_warps) {
+    for (uint32_t q = (bid * 256u + threadIdx.x) >> 5; q < n; q += n_warps) {
         const uint32_t j = p.pl_list[(size_t)slot * p.Npad + q];
         for (uint32_t k = p.csc_off[j] + lane; k < p.csc_off[j + 1]; k += 32u) {
             const uint32_t e = p.csc_edge[k], i = p.csc_src[k];
@@ -1378,20 +1382,32 @@ gn_ltp_kernel(const GnDev p, const uint64_t t)
             const uint64_t td = t - d;
             const uint32_t arr = p.raster[(size_t)(td % p.raster_rows) * p.words_pad + (i >> 5)];
             if ((arr >> (i & 31u)) & 1u) continue;        // the spike of i arrives now: coincidence
-            const int32_t ls = p.ls_hist[(size_t)(td % p.D) * p.Npad + i];
+            const int32_t ls = p.ls_hist[(size_t)(td % (p.D + 1u)) * p.Npad + i];
             if (ls >= 0 && (uint64_t)ls + 1ull < td)
                 p.w_f32[e] = __fadd_rn(p.w_f32[e], stdp_dw(p, (uint32_t)(td - 1ull - (uint64_t)ls)));
         }
     }
 }
 
+// Delivery at arrival time (before the update of step t).
+template <bool PACKED>
 __global__ void __launch_bounds__(256)
-gn_age_kernel(const GnDev p, const uint64_t t)
+gn_arrive_kernel(const GnDev p, const uint64_t t, const uint32_t n_d)
 {
-    const uint32_t j = blockIdx.x * 256u + threadIdx.x;
-    if (j >= p.Npad) return;
-    const bool fired = (p.raster[(size_t)(t % p.raster_rows) * p.words_pad + (j >> 5)] >> (j & 31u)) & 1u;
-    p.ls_hist[(size_t)((t + 1ull) % p.D) * p.Npad + j] = fired ? (int32_t)t : p.ls_hist[(size_t)(t % p.D) * p.Npad + j];
+    arrive_body<false, PACKED>(p, t, n_d, blockIdx.x, gridDim.x);
+}
+
+// eq. 33 (after the update of step t and gn_spikes_kernel): even CTAs weaken at the step's arrivals, odd CTAs strengthen at
+// its spikes -- different edges, so the two halves need nothing from each other.
+template <bool PACKED>
+__global__ void __launch_bounds__(256)
+gn_plast_kernel(const GnDev p, const uint64_t t, const uint32_t n_d)
+{
+    if ((blockIdx.x & 1u) == 0u) {
+        if (n_d) arrive_body<true, PACKED>(p, t, n_d, blockIdx.x >> 1, gridDim.x >> 1);
+    } else {
+        ltp_body<PACKED>(p, t, blockIdx.x >> 1, gridDim.x >> 1);
+    }
 }
 
 // in-edge lists: count, scan, fill
@@ -1835,12 +1851,12 @@ cudaError_t gnk_arrive(const GnDev &p, uint64_t t, uint64_t t_origin, cudaStream
     const uint64_t back = t - t_origin;
     const uint32_t n_d = (uint32_t)(back < p.D - 1u ? back : p.D - 1u);
     if (n_d == 0u) return cudaSuccess;
-    if (p.packed) gn_arrive_kernel<false, true><<<148u * 8u, 256, 0, st>>>(p, t, n_d);
-    else gn_arrive_kernel<false, false><<<148u * 8u, 256, 0, st>>>(p, t, n_d);
+    if (p.packed) gn_arrive_kernel<true><<<148u * 8u, 256, 0, st>>>(p, t, n_d);
+    else gn_arrive_kernel<false><<<148u * 8u, 256, 0, st>>>(p, t, n_d);
     return cudaGetLastError();
 }
 
-// plastic mode, after update(t): the step's spike list, eq. 33 for the arrivals and the spikes of step t, then eq. 32
+// plastic mode, after update(t): the step's spike list and eq. 32, then eq. 33 for the arrivals and the spikes of step t
 cudaError_t gnk_plasticity(const GnDev &p, uint64_t t, uint64_t t_origin, cudaStream_t st)
 {
     const uint64_t back = t - t_origin;
@@ -1848,13 +1864,8 @@ cudaError_t gnk_plasticity(const GnDev &p, uint64_t t, uint64_t t_origin, cudaSt
     cudaError_t e = cudaMemsetAsync(p.log_n + (t % p.D), 0, 4, st);
     if (e != cudaSuccess) return e;
     gn_spikes_kernel<<<ceil_div(p.Npad, 256), 256, 0, st>>>(p, t);
-    if (n_d) {
-        if (p.packed) gn_arrive_kernel<true, true><<<148u * 8u, 256, 0, st>>>(p, t, n_d);
-        else gn_arrive_kernel<true, false><<<148u * 8u, 256, 0, st>>>(p, t, n_d);
-    }
-    if (p.packed) gn_ltp_kernel<true><<<148u * 8u, 256, 0, st>>>(p, t);
-    else gn_ltp_kernel<false><<<148u * 8u, 256, 0, st>>>(p, t);
-    gn_age_kernel<<<ceil_div(p.Npad, 256), 256, 0, st>>>(p, t);
+    if (p.packed) gn_plast_kernel<true><<<148u * 16u, 256, 0, st>>>(p, t, n_d);
+    else gn_plast_kernel<false><<<148u * 16u, 256, 0, st>>>(p, t, n_d);
     return cudaGetLastError();
 }
 
