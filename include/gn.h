@@ -239,6 +239,40 @@ int gn_debug_words(void *cuda_stream, uint64_t seed, uint32_t stream_id, uint64_
  * overwritten.  Synchronises.  Errors: INVALID_ARG, CUDA. */
 int gn_debug_ceilings(void *cuda_stream, void *scratch, size_t scratch_bytes, uint32_t segment_edges, double out[2]);
 
+/* The overflow check of gn_create (GN_E_OVERFLOW_RISK: does any target's sum of |w_fx| over its in-edges, plus the largest
+ * drive kick, pass 2^31 - 1 -- the most the int32 ring slot of PAPER.md:311 eq. 30's sum can be asked to hold in one step)
+ * as a call of its own that needs NO device memory from the caller beyond the inputs and the 8-byte result.
+ *
+ * Who it is for: code that cannot allocate on the device when it needs the answer -- a plug-in of a host program whose
+ * memory pool owns the whole GPU and forbids driver allocations; a control loop that must not call cudaMalloc / cudaFree
+ * because they stall every stream of the device; a process with no memory left once the network's workspace is carved out.
+ * Typical use: before gn_create, to learn whether a weight set will be refused without building a workspace for it; and
+ * during a plastic run (stdp_alpha != 0), where eq. 33 moves the weights without bound and gn_create's one-time check says
+ * nothing about them any more -- read GN_WEIGHTS into a device buffer now and then and pass it here.
+ *
+ *   targets       [n_edges] DEVICE, target vertex of every edge (any edge order; row offsets are not needed)
+ *   weights       [n_edges] DEVICE, fp32, quantised as gn_create does: w_fx = rint(w * 65536), ties to even
+ *   largest_kick  the largest |drive_kick| of the classes in use (0 if there is no drive)
+ *   out           [2] DEVICE uint32, written asynchronously on cuda_stream (read it after synchronising):
+ *                 out[0] = number of targets at risk (0 <=> gn_create would not return GN_E_OVERFLOW_RISK),
+ *                 out[1] = number of edges left out because their target is >= n_vertices or their weight is NaN /
+ *                          outside the fixed-point range (0 <=> gn_create would not return GN_E_BAD_GRAPH for these reasons)
+ *
+ * The per-target sums live in a fixed array inside the library image instead of a workspace: GN_STATIC_MAX_VERTICES x 8
+ * bytes = 8 MB of every GPU that loads libgn.so, held until the process exits.  Hence:
+ *   - n_vertices > GN_STATIC_MAX_VERTICES is refused (GN_E_INVALID_ARG, message names the limit); nothing is truncated;
+ *   - no cudaMalloc, cudaFree or other allocating call is made -- two asynchronous memsets and one kernel per call;
+ *   - the device that is current when the call is made must be the one cuda_stream, targets, weights and out belong to;
+ *   - the first call on each device also looks the array's device address up (cudaGetSymbolAddress); make that first call
+ *     before you begin any stream capture;
+ *   - every call on a device uses the same array.  It is cleared at the start of each call, so calls one after the other
+ *     on one stream are independent, but two calls whose kernels can run at the same time on one GPU (different streams,
+ *     different host threads) add into each other's sums and both results are garbage: serialise them yourself.
+ * Errors: INVALID_ARG (NULL, n_vertices = 0 or beyond the limit, n_edges >= 2^32 - 1, kick out of range), CUDA. */
+#define GN_STATIC_MAX_VERTICES 1048576
+int gn_check_headroom_static(void *cuda_stream, uint32_t n_vertices, uint64_t n_edges, const uint32_t *targets,
+                             const float *weights, float largest_kick, uint32_t *out);
+
 /* Per-kernel timing for benchmarks.  While enabled, gn_step runs every kernel on the net's stream (no overlap
  * between update and delivery) with a CUDA event wherever the kind of kernel changes, and synchronises every
  * few hundred steps to collect them: a measuring mode, never the mode a throughput number is taken in.  A run

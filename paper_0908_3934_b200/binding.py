@@ -19,6 +19,7 @@ GN_E_WORKSPACE_TOO_SMALL, GN_E_RANGE_EVICTED, GN_E_CUDA = -4, -5, -6
  GN_H, GN_WEIGHTS) = range(16)
 GN_MODEL_IZHIKEVICH, GN_MODEL_HODGKIN_HUXLEY = 0, 1
 GN_MAX_CLASSES = 8
+GN_STATIC_MAX_VERTICES = 1048576
 GN_DELIVER_AUTO, GN_DELIVER_RING, GN_DELIVER_QUEUE, GN_DELIVER_RESIDENT = 0, 1, 2, 3
 
 # gn_class_params in declaration order; a class dict may omit psc_alpha, model and the Hodgkin-Huxley fields (0)
@@ -45,7 +46,7 @@ class gn_config(C.Structure):
 
 
 EXPORTS = ("gn_query_workspace", "gn_create", "gn_step", "gn_read_state", "gn_write_state",
-           "gn_read_raster", "gn_observe", "gn_debug_words", "gn_debug_ceilings", "gn_profile", "gn_profile_read", "gn_last_error",
+           "gn_read_raster", "gn_observe", "gn_debug_words", "gn_debug_ceilings", "gn_check_headroom_static", "gn_profile", "gn_profile_read", "gn_last_error",
            "gn_destroy")
 
 _lib = None
@@ -66,6 +67,7 @@ def lib() -> C.CDLL:
         L.gn_observe.argtypes = [vp, u64, u64, vp, sz, i32]
         L.gn_debug_words.argtypes = [vp, u64, u32, u64, u32, u32, vp]
         L.gn_debug_ceilings.argtypes = [vp, vp, sz, u32, vp]
+        L.gn_check_headroom_static.argtypes = [vp, u32, u64, vp, vp, C.c_float, vp]
         L.gn_profile.argtypes = [vp, i32]
         L.gn_profile_read.argtypes = [vp, vp, vp]
         L.gn_last_error.argtypes = [vp]
@@ -226,6 +228,22 @@ def gn_debug_ceilings(segment_edges: int, scratch_mb: int = 2048, device="cuda:0
         _check(lib().gn_debug_ceilings(C.c_void_p(st.cuda_stream), C.c_void_p(scratch.data_ptr()), scratch.numel(),
                                        int(segment_edges), out))
     return float(out[0]), float(out[1])
+
+
+def gn_check_headroom_static(n_vertices: int, targets, weights, largest_kick: float, out=None):
+    """gn.h gn_check_headroom_static: torch CUDA tensors in (uint32-as-int32 targets, float32 weights), a 2-word int32
+    CUDA tensor out (made here when None -- torch's allocator, not the library's; pass your own where you cannot
+    allocate).  Asynchronous on torch's current stream of that device; returns `out`."""
+    import torch
+    if out is None:
+        out = torch.empty(2, dtype=torch.int32, device=targets.device)
+    assert targets.is_cuda and weights.is_cuda and out.is_cuda and targets.numel() == weights.numel()
+    assert targets.element_size() == 4 and weights.dtype == torch.float32 and out.element_size() == 4 and out.numel() >= 2
+    with torch.cuda.device(targets.device):
+        st = torch.cuda.current_stream(targets.device)
+        _check(lib().gn_check_headroom_static(C.c_void_p(st.cuda_stream), int(n_vertices), int(targets.numel()),
+                                              _ptr(targets), _ptr(weights), float(largest_kick), _ptr(out)))
+    return out
 
 
 def gn_profile(net: GnNet, enable: bool) -> None:

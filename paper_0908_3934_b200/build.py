@@ -7,7 +7,7 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 SO = os.path.join(_HERE, "libgn.so")
-SOURCES = ["gn_api.cu", "gn_kernels.cu"]
+SOURCES = ["gn_api.cu", "gn_kernels.cu", "gn_static.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "--fmad=false",            # no implicit contraction: the arithmetic contract spells every fma
               "-Xcompiler", "-fPIC", "-shared"]

@@ -190,6 +190,17 @@ struct DeviceGuard {
 
 }  // namespace
 
+// Records the message gn_last_error(NULL) returns on this thread and hands the code back: for entry points that live in
+// other files of the library and have no handle (gn_static.cu).
+int gn_fail(int code, const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_create_error, sizeof g_create_error, fmt, ap);
+    va_end(ap);
+    return code;
+}
+
 extern "C" {
 
 int gn_query_workspace(const gn_config *cfg, size_t *bytes)
