@@ -556,6 +556,7 @@ static int orc_vertex_hh_fp64(orc_net *o, uint32_t j, int64_t I_fx)
     double s = r - ((i_na + i_k) + i_l);
     if (o->bias) s = s + (double)o->bias[j];
     o->V[j] = fma(q->hh_dt_c, s, V);
+    if (q->direct) o->V[j] = o->V[j] + I;      /* DESIGN.md reading #4: tau_syn_ms <= 0, the arriving weight jumps V itself */
     o->hm[j] = fma(o->dt, fma(-rate[1], m, rate[0] * (1.0 - m)), m);
     o->hh[j] = fma(o->dt, fma(-rate[3], h, rate[2] * (1.0 - h)), h);
     o->W[j] = fma(o->dt, fma(-rate[5], n, rate[4] * (1.0 - n)), n);
@@ -593,6 +594,7 @@ static int orc_vertex_hh_fp32(orc_net *o, uint32_t j, int64_t I_fx)
     float s = r - ((i_na + i_k) + i_l);
     if (o->bias) s = s + o->bias[j];
     o->Vf[j] = fmaf(q->hh_dt_c_f, s, V);
+    if (q->direct) o->Vf[j] = o->Vf[j] + If;   /* reading #4, as above */
     o->hmf[j] = fmaf(dt, fmaf(-rate[1], m, rate[0] * (1.0f - m)), m);
     o->hhf[j] = fmaf(dt, fmaf(-rate[3], h, rate[2] * (1.0f - h)), h);
     o->Wf[j] = fmaf(dt, fmaf(-rate[5], n, rate[4] * (1.0f - n)), n);

@@ -198,3 +198,53 @@ def test_hh_fp32_mode_tracks_fp64(n):
     t_star, stats = gate.check(a.raster_bool(), b.raster_bool(), "oracle HH fp32 vs fp64")
     assert b.counters()["spikes"] > 50
     assert t_star is None or t_star > 1000
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_hh_direct_injection_jumps_v_by_the_weight(mode):
+    """tau_syn_ms <= 0 (reading #4; gn.h: "the arriving weight jumps V itself") holds for Hodgkin-Huxley
+    vertices as for Izhikevich ones: there is no synaptic current state, and V of the target is higher by exactly the
+    weight after the step at which the event arrives.  Two runs that differ only in the weight of the one edge 0 -> 1
+    (w against 0) are identical at vertex 1 up to the arrival step f + delay and differ by w right after it; a drive
+    kick (reading #12: injected like an arriving event) does the same; r stays 0 throughout; a weight large enough
+    relays the spike."""
+    w, d = 3.0, 7
+    cfg = base_cfg([hh_class(tau_syn_ms=0.0)], dt_ms=DT, ring_slots=16)
+    runs = []
+    for weight in (w, 0.0):
+        net, dl = hand_net(2, [(0, 1, weight, d)])
+        o = Oracle(net, cfg, mode, delays=dl, bias=np.array([10.0, 0.0], np.float32))
+        v1 = []
+        for _ in range(400):
+            o.step(1)
+            v1.append(o.state(ob.V)[1])
+            assert o.state(ob.R)[1] == 0.0
+        runs.append((np.array(v1), np.flatnonzero(o.raster_bool()[:, 0])))
+    (va, fa), (vb, fb) = runs
+    assert len(fa) >= 1 and np.array_equal(fa, fb)
+    arrive = int(fa[0]) + d                                   # the step that consumes the event; v1[t] is V after step t
+    assert np.array_equal(va[:arrive], vb[:arrive])
+    tol = 1e-12 if mode == "fp64" else 4e-6                   # one rounding of a number of magnitude ~65
+    assert abs((va[arrive] - vb[arrive]) - w) <= tol
+    # strong enough an edge relays the spike: 0 fires, 1 fires shortly after the arrival
+    net, dl = hand_net(2, [(0, 1, 30.0, d)])
+    o = Oracle(net, cfg, mode, delays=dl, bias=np.array([10.0, 0.0], np.float32))
+    o.step(400)
+    r = o.raster_bool()
+    f0, f1 = np.flatnonzero(r[:, 0]), np.flatnonzero(r[:, 1])
+    assert len(f1) >= 1 and f0[0] + d < f1[0] < f0[0] + d + 100
+    # drive kicks enter the same way: a lone vertex with a 2,000 Hz drive of +2 mV kicks depolarises by 2 per kick
+    cfgk = base_cfg([hh_class(tau_syn_ms=0.0, drive_rate_hz=2000.0, drive_kick=2.0)], dt_ms=DT, ring_slots=16)
+    cfgq = base_cfg([hh_class(tau_syn_ms=0.0, drive_rate_hz=2000.0, drive_kick=0.0)], dt_ms=DT, ring_slots=16)
+    net, dl = hand_net(1, [])
+    ok, oq = Oracle(net, cfgk, mode, delays=dl), Oracle(net, cfgq, mode, delays=dl)
+    for _ in range(200):
+        before = ok.counters()["kicks"]
+        ok.step(1)
+        oq.step(1)
+        if ok.counters()["kicks"] > before:
+            assert abs((ok.state(ob.V)[0] - oq.state(ob.V)[0]) - 2.0) <= tol
+            break
+        assert ok.state(ob.V)[0] == oq.state(ob.V)[0]
+    else:
+        raise AssertionError("no kick in 200 steps at 2 kHz")
