@@ -37,8 +37,8 @@ def hh_class(rate_hz=0.0, kick=10.0, tau_syn_ms=2.0, **over):
     """One row of gn_class_params for a Hodgkin-Huxley vertex (model = 1).  The paper prints no
     values: these are the squid-axon parameters of Hodgkin & Huxley (1952) in the modern convention (rest at -65 mV;
     e_l chosen so that -65 mV is the resting point), C in uF/cm^2, g in mS/cm^2, potentials in mV, rates in 1/ms.
-    A spike is the upward crossing of v_peak = 0 mV; refractory_ms is the detection dead time (one action potential =
-    one event).  The Izhikevich-only fields are unused and zero."""
+    A spike is V >= v_peak = 0 mV (eq. 31) outside the detection dead time refractory_ms, which is what makes one action
+    potential one event (a vertex held above v_peak for longer than that is detected again every dead time).  The Izhikevich-only fields are unused and zero."""
     c = dict(a=0.0, b=0.0, c_reset=0.0, d=0.0, k2=0.0, k1=0.0, k0=0.0, v_peak=0.0, tau_syn_ms=tau_syn_ms,
              refractory_ms=2.0, drive_rate_hz=rate_hz, drive_kick=kick, psc_alpha=0.0,
              model=1.0, hh_c=1.0, hh_g_na=120.0, hh_g_k=36.0, hh_g_l=0.3, hh_e_na=50.0, hh_e_k=-77.0, hh_e_l=-54.387,

@@ -104,7 +104,7 @@ typedef struct {
     uint32_t trace_capacity_frames; /* device trace window (most recent frames kept)                 */
     uint64_t seed;                  /* key of the counter generator (drive stream 5, noise stream 6) */
     /* How eq. 30's sum reaches the ring (the RESULT is identical in every mode: integer adds commute). */
-    uint32_t delivery_mode;         /* GN_DELIVER_AUTO (0), _RING, _QUEUE, _RESIDENT                   */
+    uint32_t delivery_mode;         /* GN_DELIVER_AUTO (0), _RING, _QUEUE, _RESIDENT, _RING_STEPWISE   */
     uint32_t queue_group;           /* queue mode: ring slots per slot group, power of two in 1..16;  */
                                     /* 0 = default (8)                                                */
     uint64_t queue_capacity;        /* queue mode: spikes of one step the spike log holds; later ones */
@@ -115,6 +115,12 @@ typedef struct {
     /* spike of i arrives at j or j fires at t (s~: time since the last spike, 0 for a vertex spiking at the step).  An   */
     /* arriving spike is weighed with the weight AT THE ARRIVAL step (eq. 30), so delivery then happens at arrival time:  */
     /* delivery_mode must be AUTO or RING, observation and checkpoint writes of RING / STEP are not supported with it.    */
+    /* Overflow: GN_E_OVERFLOW_RISK of gn_create bounds the INITIAL weights only, and eq. 33 has no ceiling.  GN_FAULTS   */
+    /* is the guard of a plastic network: [0] counts, at delivery, every weight that no longer fits the fixed point (it is */
+    /* delivered saturated); [1] is gn_create's own bound (a target's sum of |w_fx| + kick <= 2^31 - 1, so that no ring    */
+    /* slot can wrap) re-evaluated over the current weights whenever GN_FAULTS or GN_WEIGHTS is read -- nothing is added   */
+    /* to the step for it, so read one of them as often as the learning rate makes prudent.  A read into HOST memory (of   */
+    /* these or of GN_COUNTERS) tells the handle; once a count is non-zero gn_step returns GN_E_OVERFLOW_RISK.             */
     float    stdp_alpha;            /* per ms; 0 = static weights                                     */
     float    stdp_beta;             /* 1/ms, >= 0                                                     */
 } gn_config;
@@ -133,11 +139,23 @@ typedef struct {
  *   shared memory, delivery by shared-memory integer atomics, one barrier per step and no per-step kernel launch
  *   (the paper's own workload shape: many networks of <= 1000 vertices).  Needs every network to have <= 16,384
  *   vertices and ring_slots x min(vertices, 1024) x 4 bytes <= 200 KB; otherwise GN_E_INVALID_ARG.
- * AUTO picks RESIDENT whenever it is possible, else QUEUE when the ring exceeds 48 MB and D >= 32, else RING. */
+ * AUTO picks RESIDENT whenever it is possible, else QUEUE when the ring exceeds 48 MB and D >= 32, else RING.
+ * GN_DRIVER (gn_read_state) tells which step driver a handle ended up with. */
 #define GN_DELIVER_AUTO 0
 #define GN_DELIVER_RING 1
 #define GN_DELIVER_QUEUE 2
 #define GN_DELIVER_RESIDENT 3
+/* RING with one kernel launch per step even where the whole gn_step call could be one cooperative launch (the persistent
+ * step driver, small networks): for measuring and testing the per-step path.  Same results. */
+#define GN_DELIVER_RING_STEPWISE 4
+
+/* GN_DRIVER values: which step driver gn_create chose for this network. */
+#define GN_DRIVER_RING 0        /* update kernel + delivery kernel per step                                  */
+#define GN_DRIVER_FUSED 1       /* one kernel per step, the update delivers                                  */
+#define GN_DRIVER_PERSISTENT 2  /* one cooperative launch per gn_step call (gn_persist_kernel)               */
+#define GN_DRIVER_QUEUE 3       /* update per step, logging + folding per slot group                         */
+#define GN_DRIVER_RESIDENT 4    /* one launch per call, a CTA or cluster per network                         */
+#define GN_DRIVER_PLASTIC 5     /* arrival-time delivery, update, eq. 32-33: four launches per step          */
 
 /* `which` of gn_read_state / gn_write_state, with the element type of the caller's buffer.       */
 enum {
@@ -159,7 +177,12 @@ enum {
     GN_ACC = 12,      /* float  [N]      sum of c over the steps of the camera frame in progress (obs_stride > 0) */
     GN_M = 13,        /* float  [N]      sodium activation m of Hodgkin-Huxley vertices (zero for other classes)  */
     GN_H = 14,        /* float  [N]      sodium inactivation h of Hodgkin-Huxley vertices (zero for other classes) */
-    GN_WEIGHTS = 15   /* float  [E]      current weight of every edge, caller's edge order (plastic: evolving; else w_fx 2^-16) */
+    GN_WEIGHTS = 15,  /* float  [E]      current weight of every edge, caller's edge order (plastic: evolving; else w_fx 2^-16) */
+    GN_DRIVER = 17,   /* uint32 [1]      the step driver in use, a GN_DRIVER_* value (read only)                                */
+    GN_FAULTS = 16    /* uint64 [2]      plastic mode's overflow guard (read only; zeros otherwise): { deliveries, since       */
+                      /*                 gn_create, of a weight outside the fixed-point range +-32768 (or NaN); targets whose  */
+                      /*                 sum of |w_fx| (+ kick) passes 2^31 - 1 for the weights as they are at this read } --  */
+                      /*                 see stdp_alpha                                                                         */
 };
 
 /* Bytes of device workspace gn_create needs for this configuration.
@@ -209,7 +232,11 @@ int gn_read_state(gn_net *net, int which, void *dst, size_t dst_bytes, int dst_i
  * reads) and STEP (uint64 [1], or COUNTERS uint64 [4]) they are the whole state -- y_j and the in-flight delayed signals
  * Y_j: a fresh handle of the same network given all of them continues bit-identically from step t.
  * Writing STEP / COUNTERS sets the step index (generator counter, ring slot, frame phase); raster steps and trace
- * frames before it are not held (GN_E_RANGE_EVICTED).  RING / STEP / COUNTERS writes synchronise the stream. */
+ * frames before it are not held (GN_E_RANGE_EVICTED).  RING / STEP / COUNTERS writes synchronise the stream.
+ * Not covered: a plastic network (stdp_alpha != 0).  Its state also includes the weights (GN_WEIGHTS, read-only), the
+ * spikes in flight -- which it keeps as the spike lists of the last ring_slots - 1 steps, not in the ring -- and the
+ * last-spike steps of eq. 32; none of these can be written, so RING / STEP / COUNTERS writes are refused there
+ * (GN_E_INVALID_ARG) and a plastic run cannot be resumed from a checkpoint. */
 int gn_write_state(gn_net *net, int which, const void *src, size_t src_bytes, int src_is_device);
 
 /* Spike raster of steps t0 .. t0+n_steps-1 as bit words: bit (j mod 32) of bits[s][j / 32] is

@@ -1,6 +1,7 @@
 """Spike-time dependent plasticity as the paper writes it (eq. 32-33; eq. 9-10), in pure
-Python on top of the pull definition (oracle/pull_definition.py).  TEST INFRASTRUCTURE -- and, so far, a definition
-only: no CUDA path implements it yet, so nothing is compared against it on the GPU.
+Python on top of the pull definition (oracle/pull_definition.py).  TEST INFRASTRUCTURE: the definition that plastic mode
+of the CUDA path is compared with in tests/test_parity_gpu.py::test_plastic_* -- at the sizes pure Python
+reaches (tens of vertices); it shares nothing with that path.
 
 State added to the framework:
   s_j(t)      time since the last spike of vertex j, transition function eq. 32 verbatim,

@@ -16,11 +16,12 @@ GN_OK = 0
 GN_E_INVALID_ARG, GN_E_BAD_GRAPH, GN_E_OVERFLOW_RISK = -1, -2, -3
 GN_E_WORKSPACE_TOO_SMALL, GN_E_RANGE_EVICTED, GN_E_CUDA = -4, -5, -6
 (GN_V, GN_W, GN_R, GN_CA, GN_REFR, GN_RING, GN_STEP, GN_COUNTERS, GN_DELAYS, GN_WEIGHTS_FX, GN_BIAS, GN_P, GN_ACC, GN_M,
- GN_H, GN_WEIGHTS) = range(16)
+ GN_H, GN_WEIGHTS, GN_FAULTS, GN_DRIVER) = range(18)
+(GN_DRIVER_RING, GN_DRIVER_FUSED, GN_DRIVER_PERSISTENT, GN_DRIVER_QUEUE, GN_DRIVER_RESIDENT, GN_DRIVER_PLASTIC) = range(6)
 GN_MODEL_IZHIKEVICH, GN_MODEL_HODGKIN_HUXLEY = 0, 1
 GN_MAX_CLASSES = 8
 GN_STATIC_MAX_VERTICES = 1048576
-GN_DELIVER_AUTO, GN_DELIVER_RING, GN_DELIVER_QUEUE, GN_DELIVER_RESIDENT = 0, 1, 2, 3
+GN_DELIVER_AUTO, GN_DELIVER_RING, GN_DELIVER_QUEUE, GN_DELIVER_RESIDENT, GN_DELIVER_RING_STEPWISE = 0, 1, 2, 3, 4
 
 # gn_class_params in declaration order; a class dict may omit psc_alpha, model and the Hodgkin-Huxley fields (0)
 CLASS_FIELDS = ("a", "b", "c_reset", "d", "k2", "k1", "k0", "v_peak", "tau_syn_ms",
@@ -165,12 +166,13 @@ def gn_step(net: GnNet, n_steps: int) -> None:
 _STATE_DTYPE = {GN_V: np.float32, GN_W: np.float32, GN_R: np.float32, GN_CA: np.float32, GN_REFR: np.uint8,
                 GN_RING: np.int32, GN_STEP: np.uint64, GN_COUNTERS: np.uint64, GN_DELAYS: np.uint8,
                 GN_WEIGHTS_FX: np.int32, GN_BIAS: np.float32, GN_P: np.float32, GN_ACC: np.float32, GN_M: np.float32,
-                GN_H: np.float32, GN_WEIGHTS: np.float32}
+                GN_H: np.float32, GN_WEIGHTS: np.float32, GN_FAULTS: np.uint64,
+                GN_DRIVER: np.uint32}
 
 
 def _state_shape(net, which):
     return {GN_RING: (net.d, net.n), GN_STEP: (1,), GN_COUNTERS: (4,), GN_DELAYS: (net.e,),
-            GN_WEIGHTS_FX: (net.e,), GN_WEIGHTS: (net.e,)}.get(which, (net.n,))
+            GN_WEIGHTS_FX: (net.e,), GN_WEIGHTS: (net.e,), GN_FAULTS: (2,), GN_DRIVER: (1,)}.get(which, (net.n,))
 
 
 def gn_read_state(net: GnNet, which: int, out=None):
@@ -251,7 +253,7 @@ def gn_profile(net: GnNet, enable: bool) -> None:
 
 
 def gn_profile_read(net: GnNet):
-    """-> (ms[4] summed device time of update / delivery / observation / bucket fold, launches[5])."""
+    """-> (ms[4] summed device time of update / delivery (queue mode: spike logging) / observation / fold, launches[5])."""
     ms = np.zeros(4, dtype=np.float64)
     n = np.zeros(5, dtype=np.uint64)
     _check(lib().gn_profile_read(net.handle, _ptr(ms), _ptr(n)), net.handle)

@@ -38,7 +38,7 @@ int check_config(const gn_config *cfg, char *err, size_t errn)
     if (cfg->n_networks < 1 || cfg->n_networks > cfg->n_vertices) return fail("n_networks must be in [1, n_vertices]");
     if (cfg->obs_stride > 0 && cfg->trace_capacity_frames == 0) return fail("obs_stride > 0 needs trace_capacity_frames > 0");
     if (cfg->obs_stride > 0 && !(cfg->tau_ca_ms > 0.0f)) return fail("obs_stride > 0 needs tau_ca_ms > 0");
-    if (cfg->delivery_mode > GN_DELIVER_RESIDENT) return fail("delivery_mode must be GN_DELIVER_AUTO, _RING, _QUEUE or _RESIDENT");
+    if (cfg->delivery_mode > GN_DELIVER_RING_STEPWISE) return fail("delivery_mode must be GN_DELIVER_AUTO, _RING, _QUEUE, _RESIDENT or _RING_STEPWISE");
     if (cfg->stdp_alpha != 0.0f) {
         if (!(cfg->stdp_beta >= 0.0f) || !isfinite(cfg->stdp_alpha) || !isfinite(cfg->stdp_beta)) return fail("stdp_alpha must be finite and stdp_beta finite and >= 0");
         if (cfg->delivery_mode != GN_DELIVER_AUTO && cfg->delivery_mode != GN_DELIVER_RING)
@@ -98,6 +98,7 @@ Layout make_layout(const gn_config *cfg)
     L.counters = take(32);
     const QueuePlan qp = make_plan(cfg);
     L.q_count = take(256 * 8);       // +0: the persistent step driver's barrier counter; +64: spikes logged per step slot
+                                     // (at most 255 x 4 bytes); +1536: the two GN_FAULTS counters
     {
         size_t rows = cfg->raster_capacity_steps, need_rows = qp.on ? (size_t)(kQueueWindow + 1u) << qp.q_log : 2;
         if (cfg->stdp_alpha != 0.0f) need_rows = D;     // plastic mode: the raster is the spikes in flight
@@ -140,6 +141,9 @@ struct gn_net {
     cudaEvent_t ev_update, ev_deliver[2], ev_fold[4];
     bool fences_pending;
     bool has_bias;
+    unsigned long long faults_seen[2];   // GN_FAULTS as last read to the host (plastic mode): non-zero stops gn_step
+    unsigned long long barrier_broken;   // grid_sync[1] as last read: the persistent driver's barrier timed out
+    unsigned long long *scratch_abs;     // N x 8 bytes of the workspace, free after gn_create (per-target sums of |w_fx|)
     // measuring mode (gn_profile)
     bool profile;
     std::vector<cudaEvent_t> ev;      // pool, reused chunk after chunk
@@ -307,6 +311,7 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
     d.q_log = qp.q_log; d.q_nb = qp.q_nb; d.q_arrays = qp.arrays; d.log_cap = qp.log_cap;
     d.grid_sync = (unsigned long long *)(ws + L.q_count);
     d.log_n = (uint32_t *)(ws + L.q_count + 64);
+    d.faults = (unsigned long long *)(ws + L.q_count + 1536);
     d.s_edge = (uint2 *)(ws + L.s_edge); d.s_dly = ws + L.s_dly; d.min_dly = ws + L.min_dly;
     d.packed = Npad <= (1u << 24) ? 1u : 0u;
     d.q_window = kQueueWindow;
@@ -388,6 +393,7 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
     cudaStream_t st = net->stream;
     uint64_t *row64 = (uint64_t *)(ws + L.scratch_row64);
     unsigned long long *abs_in = (unsigned long long *)(ws + L.scratch_abs);
+    net->scratch_abs = abs_in;
     float *pos_d = (float *)(ws + L.scratch_pos);
     uint32_t *net_d = (uint32_t *)(ws + L.scratch_net);
     GnCheck *chk_d = (GnCheck *)(ws + L.scratch_chk);
@@ -483,8 +489,8 @@ int gn_create(const gn_config *cfg, const gn_class_params *classes, const float 
     // ring mode on a small network: one kernel per step (the update delivers), bound by launch latency not work
     d.fused = (!d.resident && !d.queue_mode && !d.plastic && Npad <= (1u << 18)) ? 1u : 0u;
     // ... and when its whole update grid can be co-resident, one cooperative launch per gn_step call (gn_persist_kernel).
-    // GN_NO_PERSIST (environment): measurements of the per-step path only.
-    if (d.fused && !getenv("GN_NO_PERSIST")) {
+    // (GN_DELIVER_RING_STEPWISE keeps the per-step path: measurements and tests of it.)
+    if (d.fused && cfg->delivery_mode != GN_DELIVER_RING_STEPWISE) {
         bool ok = false;
         GN_CREATE_CUDA(gnk_persist_ok(d, &ok));
         d.persist = ok ? 1u : 0u;
@@ -673,6 +679,10 @@ int gn_step(gn_net *net, uint64_t n_steps)
         return GN_OK;
     }
     if (d.plastic) {       // plastic weights: arrivals of step t, the update, then eq. 33 and eq. 32, all on the caller's stream
+        if (net->faults_seen[0] || net->faults_seen[1])
+            return set_err(net, GN_E_OVERFLOW_RISK, "the plastic weights outgrew the fixed-point ring (GN_FAULTS: %llu deliveries of a weight outside "
+                           "+-32768, %llu targets whose sum of |w| no longer fits int32): stepping is refused",
+                           net->faults_seen[0], net->faults_seen[1]);
         for (uint64_t s = 0; s < n_steps; ++s) {
             const uint64_t t = net->t;
             const bool prof = net->profile;
@@ -694,6 +704,8 @@ int gn_step(gn_net *net, uint64_t n_steps)
         return GN_OK;
     }
     if (d.persist) {       // ring mode, co-resident grid: the whole call is one cooperative launch
+        if (net->barrier_broken)
+            return set_err(net, GN_E_CUDA, "the persistent step driver's grid barrier timed out: the results of this handle are invalid");
         uint64_t left = n_steps;
         while (left) {
             const uint64_t n = left > 0x40000000ull ? 0x40000000ull : left;
@@ -843,6 +855,15 @@ int gn_read_state(gn_net *net, int which, void *dst, size_t dst_bytes, int dst_i
         if (rc) return rc;
         src = d.counters; need = 32; break;
     }
+    case GN_FAULTS: src = d.faults; need = 16; break;
+    case GN_DRIVER: {
+        if (dst_bytes < 4) return set_err(net, GN_E_INVALID_ARG, "dst has %zu bytes, need 4", dst_bytes);
+        const uint32_t drv = d.plastic ? GN_DRIVER_PLASTIC : d.resident ? GN_DRIVER_RESIDENT : d.queue_mode ? GN_DRIVER_QUEUE
+                           : d.persist ? GN_DRIVER_PERSISTENT : d.fused ? GN_DRIVER_FUSED : GN_DRIVER_RING;
+        if (!dst_is_device) { memcpy(dst, &drv, 4); return GN_OK; }
+        GN_CUDA(net, cudaMemcpyAsync(dst, &drv, 4, cudaMemcpyHostToDevice, net->stream));   // pageable source: staged before the call returns
+        return GN_OK;
+    }
     case GN_DELAYS: src = d.dly; need = E; break;
     case GN_WEIGHTS_FX: src = d.wfx; need = E * 4; break;
     case GN_WEIGHTS:
@@ -860,6 +881,19 @@ int gn_read_state(gn_net *net, int which, void *dst, size_t dst_bytes, int dst_i
                                        dst_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, net->stream));
         if (!dst_is_device) GN_CUDA(net, cudaStreamSynchronize(net->stream));
         return GN_OK;
+    }
+    if (d.plastic && (which == GN_FAULTS || which == GN_WEIGHTS))      // gn_create's bound over the weights as they are now
+        GN_CUDA(net, gnk_plastic_headroom(d, E, net->scratch_abs, net->stream));
+    if (d.persist && !dst_is_device && (which == GN_COUNTERS || which == GN_STEP)) {
+        // the persistent step driver's barrier gave up waiting (gn_persist_kernel): nothing since then can be trusted
+        GN_CUDA(net, cudaMemcpyAsync(&net->barrier_broken, d.grid_sync + 1, 8, cudaMemcpyDeviceToHost, net->stream));
+        GN_CUDA(net, cudaStreamSynchronize(net->stream));
+        if (net->barrier_broken)
+            return set_err(net, GN_E_CUDA, "the persistent step driver's grid barrier timed out: the results of this handle are invalid");
+    }
+    if (d.plastic && !dst_is_device && (which == GN_FAULTS || which == GN_COUNTERS || which == GN_WEIGHTS)) {
+        // these reads wait for the stream anyway: the host learns of a fault here, and gn_step refuses to go on after one
+        GN_CUDA(net, cudaMemcpyAsync(net->faults_seen, d.faults, 16, cudaMemcpyDeviceToHost, net->stream));
     }
     return copy_out(net, dst, src, need, dst_is_device);
 }

@@ -97,6 +97,7 @@ struct GnDev {
     uint32_t *pl_list;              // [D][Npad] row t mod D: the vertices that fired at step t (log_n[t mod D] of them)
     uint32_t *csc_off, *csc_edge, *csc_src;   // in-edges by target: [Npad+1] offsets, [E] position in s_edge, [E] source
     float *w_stage;                 // [E] staging of GN_WEIGHTS read-back (caller's edge order)
+    unsigned long long *faults;     // [2] GN_FAULTS: deliveries of a weight outside the fixed-point range; targets over gn_create's bound when last evaluated
     unsigned long long *counters;   // steps, spikes, delivered events, kicks
     unsigned long long *grid_sync;  // the persistent step driver's barrier counter (it only grows)
     uint32_t *raster;        // [raster_rows][words_pad]; row t % raster_rows is step t's spike list
@@ -127,6 +128,8 @@ cudaError_t gnk_build_csc(const GnDev &p, uint64_t n_edges, uint32_t *cursor, cu
 cudaError_t gnk_arrive(const GnDev &p, uint64_t t, uint64_t t_origin, cudaStream_t st);
 cudaError_t gnk_plasticity(const GnDev &p, uint64_t t, uint64_t t_origin, cudaStream_t st);
 cudaError_t gnk_weights_out(const GnDev &p, uint64_t n_edges, cudaStream_t st);
+// plastic mode: faults[1] = targets whose current sum |w_fx| (+ kick) passes 2^31 - 1; abs_in: N x 8 bytes of scratch
+cudaError_t gnk_plastic_headroom(const GnDev &p, uint64_t n_edges, unsigned long long *abs_in, cudaStream_t st);
 cudaError_t gnk_observe(const GnDev &p, uint64_t frame, cudaStream_t st);
 cudaError_t gnk_resident(const GnDev &p, uint64_t t0, uint32_t n_steps, bool has_bias, bool raster_on, cudaStream_t st);
 cudaError_t gnk_resident_cluster_ok(const GnDev &p, bool *ok);

@@ -150,7 +150,8 @@ __device__ __forceinline__ bool vertex_step_hh(const GnClassDev &q, const float 
     const float i_l = __fmul_rn(q.hh_g_l, __fsub_rn(V, q.hh_e_l));
     float s = __fsub_rn(r, __fadd_rn(__fadd_rn(i_na, i_k), i_l));
     if (BIAS) s = __fadd_rn(s, U);
-    const float Vn = __fmaf_rn(q.hh_dt_c, s, V);
+    float Vn = __fmaf_rn(q.hh_dt_c, s, V);
+    if (q.direct) Vn = __fadd_rn(Vn, If);                                // reading #4: the arriving weight jumps V itself
     m = __fmaf_rn(dt, __fmaf_rn(-bm, m, __fmul_rn(am, __fsub_rn(1.0f, m))), m);
     h = __fmaf_rn(dt, __fmaf_rn(-bh, h, __fmul_rn(ah, __fsub_rn(1.0f, h))), h);
     n = __fmaf_rn(dt, __fmaf_rn(-bn, n, __fmul_rn(an, __fsub_rn(1.0f, n))), n);
@@ -1242,7 +1243,10 @@ gn_persist_kernel(const GnDev p, const uint64_t t0, const uint32_t n_steps, unsi
             long long c0 = 0;
             for (uint32_t spins = 0; *reinterpret_cast<volatile unsigned long long *>(sync) < target; ++spins) {
                 if (spins == 1024u) c0 = clock64();
-                if (spins > 1024u && clock64() - c0 > 2000000000ll) break;
+                if (spins > 1024u && clock64() - c0 > 2000000000ll) {       // never seen: the grid is co-resident by construction
+                    sync[1] = 1ull;                                         // sticky: the host turns it into GN_E_CUDA
+                    break;
+                }
             }
             __threadfence();
         }
@@ -1351,7 +1355,11 @@ __device__ __forceinline__ void arrive_body(const GnDev &p, const uint64_t t, co
         for (uint32_t e = beg + e_lo; e < beg + e_hi; ++e) {
             const uint32_t m = PACKED ? p.s_edge[e].x & 0xFFFFFFu : p.s_edge[e].x;
             if (!LTD) {
-                ring_add(p.ring + (size_t)slot * p.Npad + m, __float2int_rn(__fmul_rn(p.w_f32[e], 65536.0f)));
+                // eq. 33 has no ceiling: unlike a static weight (checked once by gn_create) a plastic one can leave the
+                // fixed-point range; the conversion saturates, and the delivery is counted (GN_FAULTS[0])
+                const float s = __fmul_rn(p.w_f32[e], 65536.0f);
+                ring_add(p.ring + (size_t)slot * p.Npad + m, __float2int_rn(s));
+                if (!(fabsf(s) < 2147483648.0f)) atomicAdd(&p.faults[0], 1ull);
             } else if (!((fired_now[m >> 5] >> (m & 31u)) & 1u)) {         // (a coincidence changes nothing)
                 const int32_t ls = last[m];
                 if (ls >= 0 && (uint64_t)ls + 1ull < t)
@@ -1463,6 +1471,27 @@ __global__ void gn_weights_out_kernel(const GnDev p, const uint32_t n_edges)
 }
 
 // ---- create-time kernels --------------------------------------------------------------------------------
+// gn_create's overflow bound (gn_validate_kernel + gn_check_overflow_kernel) over the CURRENT plastic weights: a target
+// whose sum of |w_fx| over its in-edges plus its class's kick passes 2^31 - 1 is counted in faults[1].  The sums only
+// grow, so the one addition that carries a sum across its limit counts the target, once.  abs_in and faults[1] hold zeros.
+__global__ void gn_plastic_headroom_kernel(const GnDev p, const uint32_t n_edges, unsigned long long *abs_in)
+{
+    const uint32_t e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= n_edges) return;
+    const uint32_t m = p.packed ? p.s_edge[e].x & 0xFFFFFFu : p.s_edge[e].x;
+    const float s = __fmul_rn(p.w_f32[e], 65536.0f);
+    const long long w = __float2int_rn(s);
+    // a weight outside the fixed-point range (or NaN) counts as 2^31: its target is over the bound whatever else arrives
+    const unsigned long long a = !(fabsf(s) < 2147483648.0f) ? 2147483648ull : (unsigned long long)(w < 0 ? -w : w);
+    if (a == 0ull) return;
+    uint32_t k = p.cls[m];
+    if (k >= p.n_classes) k = 0u;
+    const long long kick = p.cls_tab[k].kick_fx;
+    const unsigned long long limit = 2147483647ull - (unsigned long long)(kick < 0 ? -kick : kick);
+    const unsigned long long before = atomicAdd(&abs_in[m], a);
+    if (before <= limit && before + a > limit) atomicAdd(&p.faults[1], 1ull);
+}
+
 __global__ void gn_init_state_kernel(const GnDev p, GnCheck *chk)
 {
     const uint32_t j = blockIdx.x * blockDim.x + threadIdx.x;
@@ -1872,6 +1901,15 @@ cudaError_t gnk_plasticity(const GnDev &p, uint64_t t, uint64_t t_origin, cudaSt
 cudaError_t gnk_weights_out(const GnDev &p, uint64_t n_edges, cudaStream_t st)
 {
     if (n_edges) gn_weights_out_kernel<<<ceil_div(n_edges, 256), 256, 0, st>>>(p, (uint32_t)n_edges);
+    return cudaGetLastError();
+}
+
+cudaError_t gnk_plastic_headroom(const GnDev &p, uint64_t n_edges, unsigned long long *abs_in, cudaStream_t st)
+{
+    cudaError_t e = cudaMemsetAsync(abs_in, 0, (size_t)p.N * 8, st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(p.faults + 1, 0, 8, st);
+    if (e != cudaSuccess) return e;
+    if (n_edges) gn_plastic_headroom_kernel<<<ceil_div(n_edges, 256), 256, 0, st>>>(p, (uint32_t)n_edges, abs_in);
     return cudaGetLastError();
 }
 

@@ -53,7 +53,7 @@ def test_query_workspace_sizes_and_errors():
     auto = gn.gn_query_workspace(gn.make_config(1_000_000, 3, 200_000_000, 128, 0.1, 0.006, 2))
     assert auto - need == pytest.approx(128 * 15 * 62_528 * 4 + 1_000_000 * 128 * 2 + 22 * 1_000_064 / 8, rel=1e-3)
     assert auto < 6 * 2 ** 30                                      # config 4 as a whole: under 6 GB
-    for bad_q in (dict(delivery_mode=4), dict(queue_group=3), dict(queue_group=32)):
+    for bad_q in (dict(delivery_mode=5), dict(queue_group=3), dict(queue_group=32)):
         with pytest.raises(gn.GnError):
             gn.gn_query_workspace(gn.make_config(10, 2, 5, 16, 0.1, 0.1, 1, **bad_q))
     ring, edges = 128 * 1_000_064 * 4, 2 * 200_000_000 * 9   # rows are held twice: caller order and sorted by delay

@@ -749,6 +749,26 @@ def test_hodgkin_huxley_bit_exact(gn, k, n, nb, steps, chunk, mode):
         np.testing.assert_allclose(gn.gn_observe(g, 0, frames).astype(np.float64), o.trace(0, frames), rtol=1e-6, atol=1e-5)
 
 
+@pytest.mark.parametrize("k,n,nb,steps,mode", [
+    (5, 1000, 6, 2000, "RESIDENT"),
+    (5, 1000, 6, 2000, "RING"),                 # fused update + delivery
+    (4, 9_001, None, 1500, "QUEUE"),
+    (3, 300_000, None, 200, "RING"),            # separate delivery kernel (and the persistent driver's sibling path)
+])
+def test_hodgkin_huxley_direct_injection_bit_exact(gn, k, n, nb, steps, mode):
+    """Hodgkin-Huxley classes with tau_syn_ms <= 0 (reading #4: the arriving weight and the drive kick jump V itself, no
+    PSC state): events and kicks reach V in every step driver, bit-exact against the fp32-faithful oracle, and r stays 0."""
+    from gn_inputs import as_hodgkin_huxley
+    net, cfg = make_config(k, n=n, n_networks=nb)
+    cfg = as_hodgkin_huxley(cfg)
+    cfg = dict(cfg, classes=[dict(c, tau_syn_ms=0.0) for c in cfg["classes"]])
+    g, o, _ = _run_exact(gn, net, cfg, steps, steps // 2, delivery_mode=getattr(gn, "GN_DELIVER_" + mode), threads=8)
+    _compare_hh_gates(gn, g, o)
+    c = o.counters()
+    assert c["spikes"] > 0 and c["delivered"] > 0 and c["kicks"] > 0
+    assert not gn.gn_read_state(g, gn.GN_R).any()
+
+
 def test_hodgkin_huxley_mixed_with_izhikevich_alpha_psc_and_bias(gn):
     """One network, three classes: Hodgkin-Huxley with the alpha-function PSC, Hodgkin-Huxley with the exponential one,
     Izhikevich regular spiking; a bias current on every vertex; gates written through gn_write_state."""
@@ -816,16 +836,16 @@ def test_hodgkin_huxley_state_within_tolerance_of_fp64(gn):
 # ---- step drivers of ring mode: one cooperative launch per gn_step call, or one launch per step -------------------
 @pytest.mark.parametrize("persist", [True, False])
 @pytest.mark.parametrize("k,n,steps,chunk", [(3, 6_007, 1500, 500), (2, 3_000, 900, 300), (3, 100_000, 400, 137)])
-def test_ring_mode_step_drivers_agree(gn, monkeypatch, k, n, steps, chunk, persist):
+def test_ring_mode_step_drivers_agree(gn, k, n, steps, chunk, persist):
     """gn_persist_kernel (the whole call in one cooperative launch, state in registers, one grid barrier per step) and
-    the per-step FUSED update kernel (GN_NO_PERSIST set) give the oracle's results bit for bit, observation included,
+    the per-step FUSED update kernel (GN_DELIVER_RING_STEPWISE) give the oracle's results bit for bit, observation included,
     also when a call ends inside a camera frame (chunk 137) and with a bias current."""
-    if not persist:
-        monkeypatch.setenv("GN_NO_PERSIST", "1")
     net, cfg = make_config(k, n=n)
     cfg = dict(cfg, obs_stride=25, obs_sigma=0.05)
     bias = np.random.default_rng(k).uniform(0.0, 3.0, net.n_vertices).astype(np.float32) if k == 2 else None
-    g, o, _ = _run_exact(gn, net, cfg, steps, chunk, bias=bias, delivery_mode=gn.GN_DELIVER_RING, threads=8)
+    g, o, _ = _run_exact(gn, net, cfg, steps, chunk, bias=bias, threads=8,
+                         delivery_mode=gn.GN_DELIVER_RING if persist else gn.GN_DELIVER_RING_STEPWISE)
+    assert int(gn.gn_read_state(g, gn.GN_DRIVER)[0]) == (gn.GN_DRIVER_PERSISTENT if persist else gn.GN_DRIVER_FUSED)
     frames = steps // 25
     np.testing.assert_allclose(gn.gn_observe(g, 0, frames).astype(np.float64), o.trace(0, frames), rtol=1e-6, atol=1e-5)
     np.testing.assert_array_equal(gn.gn_read_state(g, gn.GN_CA).view(np.uint32), o.state(ob.CA).astype(np.float32).view(np.uint32))
@@ -939,6 +959,54 @@ def test_plastic_random_network_tracks_the_definition(gn, seed):
           f"{int(np.array(sim.raster[:t_star]).sum())} spikes, largest weight change {np.abs(wg - w0).max():.3f}")
     assert t_star > 300
     assert np.abs(wg - w0).max() > 0.05, "degenerate test: the weights hardly moved"
+    np.testing.assert_array_equal(gn.gn_read_state(g, gn.GN_FAULTS), [0, 0])
+
+
+def _force_spikes(gn, g, vertices):
+    v = gn.gn_read_state(g, gn.GN_V)
+    v[list(vertices)] = 30.0
+    gn.gn_write_state(g, gn.GN_V, v)
+
+
+@pytest.mark.parametrize("case", ["weight_out_of_range", "sum_out_of_int32"])
+def test_plastic_overflow_guard(gn, case):
+    """Eq. 33 has no ceiling and gn_create's GN_E_OVERFLOW_RISK looks at the initial weights only: a plastic network counts
+    the deliveries of weights it cannot represent, re-evaluates gn_create's bound over the current weights when GN_FAULTS or
+    GN_WEIGHTS is read, and refuses to step on once the host has seen either (gn.h, stdp_alpha).
+    weight_out_of_range: one edge of weight 32,000 (legal: below 32,768) is strengthened past the fixed-point range by one
+    pairing and delivered again, unobserved: the delivery is counted.  sum_out_of_int32: two edges of 16,000 into one target,
+    both strengthened to about 18,000: each still fits, their sum no longer does -- caught at the read, before any delivery."""
+    quiet = rs_class(drive_kick=0.0, refractory_ms=25.5)
+    if case == "weight_out_of_range":
+        net, dl = hand_net(2, [(0, 1, 32_000.0, 3)])
+        sources, target = [0], 1
+    else:
+        net, dl = hand_net(3, [(0, 2, 16_000.0, 3), (1, 2, 16_000.0, 3)])
+        sources, target = [0, 1], 2
+    cfg = base_cfg([quiet], ring_slots=16, dt_ms=0.1)
+    g = _plastic(gn, net, cfg, 400, dl, alpha=2e4, beta=0.05)       # dt alpha = 2,000 per pairing
+    np.testing.assert_array_equal(gn.gn_read_state(g, gn.GN_FAULTS), [0, 0])     # the initial weights pass, as in gn_create
+    gn.gn_step(g, 10)
+    _force_spikes(gn, g, sources)
+    gn.gn_step(g, 290)                 # arrival at 13, the target fires on it a step or two later: strengthening
+    r = unpack_raster(gn.gn_read_raster(g, 0, 300), net.n_vertices)
+    assert r[10, sources].all() and r[13:20, target].sum() == 1
+    if case == "weight_out_of_range":
+        _force_spikes(gn, g, sources)
+        gn.gn_step(g, 10)              # the second spike arrives at 303 with a weight of about 34,000
+        np.testing.assert_array_equal(gn.gn_read_state(g, gn.GN_FAULTS), [1, 1])
+        assert gn.gn_read_state(g, gn.GN_WEIGHTS)[0] > 32_768.0
+    else:
+        w = gn.gn_read_state(g, gn.GN_WEIGHTS)
+        assert (w > 17_000.0).all() and (w < 18_100.0).all()
+        np.testing.assert_array_equal(gn.gn_read_state(g, gn.GN_FAULTS), [0, 1])
+    with pytest.raises(gn.GnError) as ei:
+        gn.gn_step(g, 1)
+    assert ei.value.code == gn.GN_E_OVERFLOW_RISK and "GN_FAULTS" in str(ei.value)
+    # a static network has nothing to count
+    g2 = gn.create_from_inputs(net, cfg, delays=dl)
+    gn.gn_step(g2, 20)
+    np.testing.assert_array_equal(gn.gn_read_state(g2, gn.GN_FAULTS), [0, 0])
 
 
 def test_plastic_mode_argument_checks(gn):
