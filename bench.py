@@ -37,6 +37,10 @@ HH_BYTES_PER_VERTEX = 51.125           # Hodgkin-Huxley class: V, n, r, m, h r+w
 HH_FP32_PER_VERTEX = 141.0             # fp32 operations of the contract per Hodgkin-Huxley vertex-step (6 exp32 x 14,
                                        # rate arguments and shapes 25, currents 16, gates 12, V, PSC, input 4; a division counts 1)
 FP32_LANES_PER_SM, SM_COUNT, SM_HZ = 128, 148, 1.965e9   # B200_PROFILING.md: 148 SMs, 1965 MHz; 4 x 32 fp32 lanes per SM
+IZH_OPS_PER_VERTEX = 46.0              # lane-instructions of the contract per Izhikevich vertex-step, counted from the kernel source:
+                                       # vertex_step 12 fp32 (W line 3, V line 6, PSC 1, calcium 2) + detection / hold / raster 2 +
+                                       # a quarter of a Philox4x32-10 block (10 rounds x 2 mul.lo, 2 mul.hi, 4 xor + 2 key adds = 102
+                                       # + counter set-up ~26 = ~128 per block of 4 vertices: 32)
 EVENT_BYTES = 17.0                     # edge record 9 (target 4, weight 4, delay 1) + ring word read-modify-write 8
 SOURCE_BYTES = 12.0                    # two row offsets + active-list entry per fired source
 SECTOR_EVENT_BYTES = 73.0              # 9 + one 32 B sector fetched + one written back (ring >> L2)
@@ -345,9 +349,10 @@ def main():
     cp1 = counters(g)
     assert cp0 == c0 and cp1 == c1, "the per-kernel pass did not replay the timed steps"
     peak, peak_src = peaks()
-    queue_mode = 0 < kn[1] < kn[0]      # queue mode delivers once per slot group, ring mode (and plastic mode) every step
-    resident = kn[1] == 0 and kn[0] < sim_steps
-    persist = resident and net_in.n_networks == 1 and N > 16384
+    driver = int(gn.gn_read_state(g, gn.GN_DRIVER)[0])      # which step driver gn_create chose: read back, not guessed
+    queue_mode = driver == gn.GN_DRIVER_QUEUE       # delivers once per slot group; ring mode (and plastic mode) every step
+    persist = driver == gn.GN_DRIVER_PERSISTENT
+    resident = persist or driver == gn.GN_DRIVER_RESIDENT
     names = ["gn_persist_kernel (a1-a5, one cooperative launch per call)" if persist else
              "gn_resident_kernel (a1-a5, one CTA or cluster per network)" if resident else
              "gn_update_kernel (a1-a3 + a4 fused)" if kn[1] == 0 else "gn_update_kernel (a1-a3)",
@@ -375,6 +380,7 @@ def main():
               N * 8.0,
               (plast_b if args.stdp else p_events * EVENT_BYTES) / max(int(kn[3]), 1)]
     traffic_tab, traffic_src = measured_traffic()
+    l2_bw, hbm_rmw = gn.gn_debug_stream_ceilings(device=dev)       # streaming read-modify-write, from L2 and from HBM: measured here
     kernels = []
     for k in range(4):
         if kn[k] == 0:
@@ -383,9 +389,27 @@ def main():
         row = {"kernel": names[k], "launches": int(kn[k]), "avg_us": avg_s * 1e6, "share": float(kms[k] / kms.sum()),
                "bytes_per_launch": kbytes[k], "achieved": kbytes[k] / avg_s / 1e9, "frac": kbytes[k] / avg_s / 1e9 / peak}
         tr = traffic_tab.get(names[k].split()[0] + ("_hh" if args.model == "hh" and k == 0 else ""))
-        if tr is not None:      # what DRAM really moved for this kernel (ncu capture named in traffic_source) over the live time
+        if tr is not None and not resident:
+            # what DRAM moved for this kernel in the committed ncu capture named in traffic_source (NOT measured in this run;
+            # per event where the kernel's work is per event, scaled by this run's event count) over the live time
             row["traffic"] = tr[1] * p_events / kn[k] if tr[1] is not None else tr[0]
             row["dram_frac"] = row["traffic"] / avg_s / 1e9 / peak
+        # what binds the kernel: "hbm" only when DRAM really carries at least half of the algorithmic bytes AND one of the two
+        # fractions is past one half; a working set served by L2 is rated against the L2 ceiling measured in this run
+        if k == 0 and resident:
+            row["bound"] = "alu"             # state in registers, ring in shared memory: the algorithmic bytes are not moved at all
+            row["frac"] = row["achieved"] = None
+            row["bytes_not_moved"] = row.pop("bytes_per_launch")
+        elif k == 3 and queue_mode or k == 1 and not queue_mode and not args.stdp:
+            row["bound"] = "l2-atomics"      # one int32 reduction per event in the L2 (a4_delivery.atomic_path has the ceiling)
+        elif args.stdp and k in (1, 3):
+            row["bound"] = "latency"
+        else:
+            df = row.get("dram_frac")
+            if k == 0:
+                row["l2_frac"] = kbytes[k] / avg_s / l2_bw
+            row["bound"] = ("hbm" if df is not None and df >= 0.5 * row["frac"] and max(df, row["frac"]) >= 0.5 else
+                            "l2" if df is not None and df < 0.5 * row["frac"] else "latency")
         kernels.append(row)
     a4_s = (kms[1] + kms[3]) * 1e-3
     a4 = {"what": "a4 delivery as a whole (routing + folding), 17 B per event + 12 B per fired source",
@@ -413,19 +437,35 @@ def main():
                                             "ceiling -- the fold kernel keeps more loads in flight); achieved = delivered "
                                             "events / summed gn_fold_kernel time"}
     dom = max(kernels, key=lambda r: r["share"])
-    roofline = {"bound": "hbm", "kernel": dom["kernel"], "achieved": dom["achieved"], "peak": peak, "unit": "GB/s",
+    roofline = {"bound": dom["bound"], "kernel": dom["kernel"], "achieved": dom["achieved"], "peak": peak, "unit": "GB/s",
                 "frac": dom["frac"], "traffic": dom.get("traffic"), "traffic_source": traffic_src if "traffic" in dom else None,
                 "dram_frac": dom.get("dram_frac"), "peak_source": peak_src,
-                "note": "achieved / frac = ALGORITHMIC bytes over the live CUDA-event time (the contract's definition); "
-                        "dram_frac = DRAM bytes ncu counted for this kernel (traffic) over the same live time.  Neither kernel is "
-                        "HBM-bound in the strict sense: the update kernel's state is largely L2-resident, and the fold kernel is "
-                        "bound by the L2's atomic path -- a4_delivery.atomic_path rates it against that ceiling, measured in "
-                        "this run (DESIGN.md 6.3, 7)",
+                "stream_ceilings": {"l2_gbs": l2_bw / 1e9, "hbm_read_modify_write_gbs": hbm_rmw / 1e9,
+                                    "source": "gn_debug_stream_ceilings, measured in this run: 128-bit read-modify-write over a "
+                                              "32 MB (L2-resident) and a 2 GB buffer, bytes read + written per second"},
+                "note": "achieved / frac = ALGORITHMIC bytes over the live CUDA-event time against the HBM peak (the contract's "
+                        "definition), whatever `bound` says; `bound` names what really limits the kernel (rule in bench.py: hbm only "
+                        "when DRAM carries at least half of the algorithmic bytes) and the matching rating sits beside it: "
+                        "l2-atomics -> a4_delivery.atomic_path (measured RED ceiling), l2 / hbm -> kernels[].l2_frac and "
+                        "dram_frac (traffic from the committed ncu capture in traffic_source, not from this run), alu -> alu "
+                        "(DESIGN.md 6.3, 6.5, 7)",
                 "timing": "the SAME K steps as the timed pass, replayed from rest on a fresh handle with a CUDA event at every "
                           "kernel boundary (gn_profile; serialised on one stream)",
                 "kernels": kernels, "a4_delivery": a4, "profile_pass_events_per_sim_step": p_events / sim_steps,
                 "timed_pass_events_per_sim_step": (c1[2] - c0[2]) / sim_steps}
-    if args.model == "hh":      # the update kernel against the fp32 pipe as well: which of the two bounds it depends on the measurement
+    if resident:                # nothing moves through HBM: lane-instructions of the contract against the SMs' issue rate
+        upd = kernels[0]
+        ops = HH_FP32_PER_VERTEX + 34.0 if args.model == "hh" else IZH_OPS_PER_VERTEX
+        alu_peak = FP32_LANES_PER_SM * SM_COUNT * SM_HZ
+        ach = N * ops * sim_steps / (kms[0] * 1e-3)
+        roofline.update({"achieved": ach / 1e12, "peak": alu_peak / 1e12, "unit": "T lane-instr/s", "frac": ach / alu_peak,
+                         "traffic": None, "dram_frac": None,
+                         "peak_source": "148 SMs x 128 lanes x 1.965 GHz (B200_PROFILING.md unit counts and clock)",
+                         "ops_per_vertex_step": ops,
+                         "ops_source": "counted from the arithmetic contract (bench.py IZH_OPS_PER_VERTEX / HH_FP32_PER_VERTEX + "
+                                       "generator and detection), an FMA counts once; the kernel is below this ceiling because "
+                                       "one barrier per step serialises it (DESIGN.md 6.5)"})
+    if args.model == "hh" and not resident:      # the update kernel against the fp32 pipe as well: which of the two bounds it depends on the measurement
         upd = kernels[0]
         fp32_peak = FP32_LANES_PER_SM * SM_COUNT * SM_HZ
         ach = N * HH_FP32_PER_VERTEX * (sim_steps / max(int(kn[0]), 1)) / (upd["avg_us"] * 1e-6)

@@ -266,6 +266,14 @@ int gn_debug_words(void *cuda_stream, uint64_t seed, uint32_t stream_id, uint64_
  * overwritten.  Synchronises.  Errors: INVALID_ARG, CUDA. */
 int gn_debug_ceilings(void *cuda_stream, void *scratch, size_t scratch_bytes, uint32_t segment_edges, double out[2]);
 
+/* Benchmark hook: the streaming ceilings the update kernel (a1-a3) is rated against, measured on this device with a bare
+ * read-modify-write of 128-bit words (every byte read once and written once per pass).  out[0] = bytes/s (read + written)
+ * over a 32 MB buffer that stays in L2 between passes -- the update kernel's situation while a network's state fits L2
+ * ("limited by memory and bus speeds"; a working set in L2 is rated against L2 bandwidth);
+ * out[1] = the same over all of `scratch`, which must be DEVICE memory of >= 1 GB (HBM).  Overwrites scratch; synchronises.
+ * Errors: INVALID_ARG, CUDA. */
+int gn_debug_stream_ceilings(void *cuda_stream, void *scratch, size_t scratch_bytes, double out[2]);
+
 /* The overflow check of gn_create (GN_E_OVERFLOW_RISK: does any target's sum of |w_fx| over its in-edges, plus the largest
  * drive kick, pass 2^31 - 1 -- the most the int32 ring slot of PAPER.md:311 eq. 30's sum can be asked to hold in one step)
  * as a call of its own that needs NO device memory from the caller beyond the inputs and the 8-byte result.

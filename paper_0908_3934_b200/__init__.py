@@ -8,6 +8,6 @@ from .binding import (  # noqa: F401
     GN_DRIVER_PLASTIC, GN_DRIVER_QUEUE, GN_DRIVER_RESIDENT, GN_DRIVER_RING, GN_COUNTERS, GN_DELAYS, GN_E_BAD_GRAPH, GN_E_CUDA, GN_E_INVALID_ARG, GN_E_OVERFLOW_RISK,
     GN_E_RANGE_EVICTED, GN_E_WORKSPACE_TOO_SMALL, GN_FAULTS, GN_H, GN_M, GN_MODEL_HODGKIN_HUXLEY, GN_MODEL_IZHIKEVICH, GN_OK, GN_P, GN_R, GN_REFR, GN_RING, GN_STEP, GN_V, GN_W,
     GN_STATIC_MAX_VERTICES, GN_WEIGHTS, GN_WEIGHTS_FX, EXPORTS, GnError, GnNet, create_from_inputs, gn_class_params, gn_config, gn_create,
-    gn_check_headroom_static, gn_debug_ceilings, gn_debug_words, gn_destroy, gn_observe, gn_profile, gn_profile_read, gn_query_workspace, gn_read_raster, gn_read_state, gn_step,
+    gn_check_headroom_static, gn_debug_ceilings, gn_debug_stream_ceilings, gn_debug_words, gn_destroy, gn_observe, gn_profile, gn_profile_read, gn_query_workspace, gn_read_raster, gn_read_state, gn_step,
     gn_write_state, lib, make_config)
 from .build import build  # noqa: F401

@@ -47,7 +47,7 @@ class gn_config(C.Structure):
 
 
 EXPORTS = ("gn_query_workspace", "gn_create", "gn_step", "gn_read_state", "gn_write_state",
-           "gn_read_raster", "gn_observe", "gn_debug_words", "gn_debug_ceilings", "gn_check_headroom_static", "gn_profile", "gn_profile_read", "gn_last_error",
+           "gn_read_raster", "gn_observe", "gn_debug_words", "gn_debug_ceilings", "gn_debug_stream_ceilings", "gn_check_headroom_static", "gn_profile", "gn_profile_read", "gn_last_error",
            "gn_destroy")
 
 _lib = None
@@ -68,6 +68,7 @@ def lib() -> C.CDLL:
         L.gn_observe.argtypes = [vp, u64, u64, vp, sz, i32]
         L.gn_debug_words.argtypes = [vp, u64, u32, u64, u32, u32, vp]
         L.gn_debug_ceilings.argtypes = [vp, vp, sz, u32, vp]
+        L.gn_debug_stream_ceilings.argtypes = [vp, vp, sz, vp]
         L.gn_check_headroom_static.argtypes = [vp, u32, u64, vp, vp, C.c_float, vp]
         L.gn_profile.argtypes = [vp, i32]
         L.gn_profile_read.argtypes = [vp, vp, vp]
@@ -229,6 +230,17 @@ def gn_debug_ceilings(segment_edges: int, scratch_mb: int = 2048, device="cuda:0
     with torch.cuda.device(scratch.device):
         _check(lib().gn_debug_ceilings(C.c_void_p(st.cuda_stream), C.c_void_p(scratch.data_ptr()), scratch.numel(),
                                        int(segment_edges), out))
+    return float(out[0]), float(out[1])
+
+
+def gn_debug_stream_ceilings(scratch_mb: int = 2048, device="cuda:0"):
+    """(bytes/s read + written by a streaming read-modify-write that stays in L2, the same from HBM), measured on the device."""
+    import torch
+    scratch = torch.empty(int(scratch_mb) << 20, dtype=torch.uint8, device=device)
+    st = torch.cuda.current_stream(scratch.device)
+    out = (C.c_double * 2)()
+    with torch.cuda.device(scratch.device):
+        _check(lib().gn_debug_stream_ceilings(C.c_void_p(st.cuda_stream), C.c_void_p(scratch.data_ptr()), scratch.numel(), out))
     return float(out[0]), float(out[1])
 
 

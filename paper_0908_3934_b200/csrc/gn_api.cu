@@ -1030,6 +1030,19 @@ int gn_debug_ceilings(void *cuda_stream, void *scratch, size_t scratch_bytes, ui
     return GN_OK;
 }
 
+int gn_debug_stream_ceilings(void *cuda_stream, void *scratch, size_t scratch_bytes, double out[2])
+{
+    if (!scratch || !out) return set_err(nullptr, GN_E_INVALID_ARG, "NULL argument");
+    cudaPointerAttributes attr{};
+    GN_CUDA(nullptr, cudaPointerGetAttributes(&attr, scratch));
+    if (attr.type != cudaMemoryTypeDevice && attr.type != cudaMemoryTypeManaged)
+        return set_err(nullptr, GN_E_INVALID_ARG, "scratch is not device memory");
+    if (scratch_bytes < (1024u << 20)) return set_err(nullptr, GN_E_INVALID_ARG, "scratch must hold at least 1 GB");
+    DeviceGuard guard(attr.device);
+    GN_CUDA(nullptr, gnk_stream_ceilings(scratch, scratch_bytes, out, (cudaStream_t)cuda_stream));
+    return GN_OK;
+}
+
 const char *gn_last_error(const gn_net *net) { return net ? net->err : g_create_error; }
 
 int gn_destroy(gn_net *net)

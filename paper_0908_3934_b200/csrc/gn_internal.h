@@ -150,5 +150,6 @@ cudaError_t gnk_check_overflow(const GnDev &p, const unsigned long long *abs_in,
 cudaError_t gnk_debug_words(uint64_t seed, uint32_t stream_id, uint64_t idx, uint32_t first,
                             uint32_t n, uint32_t *out, cudaStream_t st);
 cudaError_t gnk_ceilings(void *scratch, size_t scratch_bytes, uint32_t seg_len, double out[2], cudaStream_t st);
+cudaError_t gnk_stream_ceilings(void *scratch, size_t scratch_bytes, double out[2], cudaStream_t st);
 // message for gn_last_error(NULL) on this thread; returns `code` (gn_api.cu)
 int gn_fail(int code, const char *fmt, ...);

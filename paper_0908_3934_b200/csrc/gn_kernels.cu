@@ -1978,6 +1978,52 @@ cudaError_t gnk_debug_words(uint64_t seed, uint32_t stream_id, uint64_t idx, uin
 // out[0] = scattered reductions per second into a 16 MB region; out[1] = gathers of seg_len-edge segments + reductions
 // per second.  `scratch` (>= 64 MB + 256 MB; the larger the better: the edge array should dwarf L2) is overwritten.
 // Best of 5 launches each, timed with CUDA events on `st`; synchronises.
+// Streaming read-modify-write of `n4` float4 words, `passes` times over: with a buffer that fits L2 every pass after the
+// first is served by L2 (the update kernel's situation when its state stays resident between steps); with one far larger
+// than L2 every pass goes to HBM.  128-bit accesses, consecutive threads on consecutive words, like the update kernel's.
+__global__ void __launch_bounds__(256)
+gn_stream_ceiling_kernel(float4 *x, const uint32_t n4, const uint32_t passes)
+{
+    for (uint32_t pass = 0; pass < passes; ++pass)
+        for (uint32_t i = blockIdx.x * 256u + threadIdx.x; i < n4; i += gridDim.x * 256u) {
+            float4 v = x[i];
+            v.x += 1.0f; v.y += 1.0f; v.z += 1.0f; v.w += 1.0f;
+            x[i] = v;
+        }
+}
+
+cudaError_t gnk_stream_ceilings(void *scratch, size_t scratch_bytes, double out[2], cudaStream_t st)
+{
+    if (scratch_bytes < (1024u << 20)) return cudaErrorInvalidValue;
+    cudaError_t e = cudaMemsetAsync(scratch, 0, scratch_bytes, st);
+    cudaEvent_t e0, e1;
+    if (e == cudaSuccess) e = cudaEventCreate(&e0);
+    if (e != cudaSuccess) return e;
+    e = cudaEventCreate(&e1);
+    if (e != cudaSuccess) { cudaEventDestroy(e0); return e; }
+    const uint32_t grid = 148u * 8u;
+    for (int mode = 0; mode < 2 && e == cudaSuccess; ++mode) {
+        const size_t bytes = mode == 0 ? (size_t)(32u << 20) : (scratch_bytes & ~(size_t)4095);
+        const uint32_t passes = mode == 0 ? 32u : 2u;
+        size_t n4 = bytes / 16;
+        if (n4 > 0xFFFF0000ull) n4 = 0xFFFF0000ull;
+        float best = 1e30f;
+        for (int rep = 0; rep < 4 && e == cudaSuccess; ++rep) {     // rep 0 also warms L2 for mode 0
+            cudaEventRecord(e0, st);
+            gn_stream_ceiling_kernel<<<grid, 256, 0, st>>>(reinterpret_cast<float4 *>(scratch), (uint32_t)n4, passes);
+            cudaEventRecord(e1, st);
+            e = cudaEventSynchronize(e1);
+            float ms = 0.f;
+            if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+            if (rep > 0 && ms < best) best = ms;
+        }
+        out[mode] = 2.0 * 16.0 * (double)n4 * passes / ((double)best * 1e-3);     // bytes read + bytes written per second
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    return e;
+}
+
 cudaError_t gnk_ceilings(void *scratch, size_t scratch_bytes, uint32_t seg_len, double out[2], cudaStream_t st)
 {
     const size_t region_bytes = 16u << 20;

@@ -1037,3 +1037,12 @@ def test_debug_ceilings_measure_something_sane(gn):
         gn.gn_debug_ceilings(0, scratch_mb=512)
     with pytest.raises(gn.GnError):
         gn.gn_debug_ceilings(7, scratch_mb=64)
+
+
+def test_debug_stream_ceilings_measure_something_sane(gn):
+    """gn_debug_stream_ceilings (what bench.py rates the update kernel against): the L2-resident pass is faster than the HBM
+    one, the HBM one is in the range of the device's copy bandwidth, and too small a scratch is refused."""
+    l2, hbm = gn.gn_debug_stream_ceilings(scratch_mb=1024)
+    assert 2e12 < hbm < 9e12 and hbm < l2 < 1e14
+    with pytest.raises(gn.GnError):
+        gn.gn_debug_stream_ceilings(scratch_mb=512)
