@@ -281,7 +281,7 @@ def main():
     if args.psc_alpha:
         cfg = dict(cfg, classes=[dict(c, psc_alpha=1.0) for c in cfg["classes"]], name=cfg["name"] + "+alpha_psc")
     if args.stdp:
-        cfg = dict(cfg, obs_stride=0, name=cfg["name"] + "+stdp")      # plastic mode has no observation
+        cfg = dict(cfg, name=cfg["name"] + "+stdp")
     N, E = net_in.n_vertices, net_in.n_edges
     log(f"[rank {rank}] inputs in {time.time() - t0:.1f} s: N={N} E={E} mean out-degree {E / N:.1f}")
     obs = int(cfg["obs_stride"])

@@ -114,7 +114,7 @@ typedef struct {
     /* of its own: w_ij(t+dt) = w_ij(t) + dt alpha sign(q) exp(-beta |q|), q = s~_i(t - tau_ij) - s~_j(t) whenever the      */
     /* spike of i arrives at j or j fires at t (s~: time since the last spike, 0 for a vertex spiking at the step).  An   */
     /* arriving spike is weighed with the weight AT THE ARRIVAL step (eq. 30), so delivery then happens at arrival time:  */
-    /* delivery_mode must be AUTO or RING, observation and checkpoint writes of RING / STEP are not supported with it.    */
+    /* delivery_mode must be AUTO or RING, and checkpoint writes of RING / STEP / COUNTERS are not supported with it.    */
     /* Overflow: GN_E_OVERFLOW_RISK of gn_create bounds the INITIAL weights only, and eq. 33 has no ceiling.  GN_FAULTS   */
     /* is the guard of a plastic network: [0] counts, at delivery, every weight that no longer fits the fixed point (it is */
     /* delivered saturated); [1] is gn_create's own bound (a target's sum of |w_fx| + kick <= 2^31 - 1, so that no ring    */

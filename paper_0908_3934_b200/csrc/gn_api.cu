@@ -43,7 +43,6 @@ int check_config(const gn_config *cfg, char *err, size_t errn)
         if (!(cfg->stdp_beta >= 0.0f) || !isfinite(cfg->stdp_alpha) || !isfinite(cfg->stdp_beta)) return fail("stdp_alpha must be finite and stdp_beta finite and >= 0");
         if (cfg->delivery_mode != GN_DELIVER_AUTO && cfg->delivery_mode != GN_DELIVER_RING)
             return fail("plastic weights (stdp_alpha != 0) need delivery_mode GN_DELIVER_AUTO or GN_DELIVER_RING");
-        if (cfg->obs_stride > 0) return fail("plastic weights (stdp_alpha != 0) do not support observation (obs_stride > 0)");
     }
     const uint32_t qg = cfg->queue_group;
     if (qg != 0 && (qg > 16 || (qg & (qg - 1)) != 0)) return fail("queue_group must be 0 or a power of two in 1..16");
@@ -695,6 +694,11 @@ int gn_step(gn_net *net, uint64_t n_steps)
             GN_CUDA(net, gnk_plasticity(d, t, net->t_origin, net->stream));
             net->launches += 4;
             net->t = t + 1;
+            if (d.obs_stride && (t + 1) % d.obs_stride == 0) {      // a5 reads the calcium state only: nothing in it depends on the weights
+                if (prof && (rc = prof_mark(net, 2))) return rc;
+                GN_CUDA(net, gnk_observe(d, (t + 1) / d.obs_stride - 1, net->stream));
+                net->launches++;
+            }
             if (prof && (s + 1) % kProfChunk == 0 && ((rc = prof_mark(net, 0xFF)) || (rc = prof_collect(net)))) return rc;
         }
         if (net->profile) {

@@ -873,9 +873,9 @@ def test_plastic_mode_delivers_at_arrival_exactly_like_the_ring(gn):
     oracle, over 2,000 steps of config 3's and config 4's densities (D = 64 and 128, ragged N)."""
     for k, n in ((3, 3_001), (4, 2_500)):
         net, cfg = make_config(k, n=n)
-        cfg = dict(cfg, obs_stride=0)
+        cfg = dict(cfg, obs_stride=25 if k == 3 else 0, obs_sigma=0.05)      # observation (a5) rides along unchanged
         steps = 2000
-        g = _plastic(gn, net, cfg, steps, None, alpha=1e-30, beta=1.0)
+        g = _plastic(gn, net, cfg, steps, None, alpha=1e-30, beta=1.0, trace_capacity_frames=steps // 25)
         o = Oracle(net, cfg, "fp32", threads=4)
         gn.gn_step(g, steps)
         o.step(steps)
@@ -887,6 +887,11 @@ def test_plastic_mode_delivers_at_arrival_exactly_like_the_ring(gn):
         assert (int(c[0]), int(c[1]), int(c[3])) == (oc["steps"], oc["spikes"], oc["kicks"]) and oc["spikes"] > 0
         np.testing.assert_array_equal(gn.gn_read_state(g, gn.GN_WEIGHTS),
                                       (o.w_fx().astype(np.float64) / 65536.0).astype(np.float32))
+        if cfg["obs_stride"]:
+            frames = steps // cfg["obs_stride"]
+            np.testing.assert_allclose(gn.gn_observe(g, 0, frames).astype(np.float64), o.trace(0, frames), rtol=1e-6, atol=1e-5)
+            np.testing.assert_array_equal(gn.gn_read_state(g, gn.GN_CA).view(np.uint32),
+                                          o.state(ob.CA).astype(np.float32).view(np.uint32))
 
 
 @pytest.mark.parametrize("delay", [1, 7])
