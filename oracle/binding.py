@@ -67,6 +67,10 @@ def lib():
                      "orc_get_w_fx", "orc_get_counters"):
             getattr(L, name).restype = None
             getattr(L, name).argtypes = [vp, vp]
+        L.orc_enable_stdp.restype = i32
+        L.orc_enable_stdp.argtypes = [vp, f32, f32]
+        L.orc_get_weights.restype = None
+        L.orc_get_weights.argtypes = [vp, vp]
         L.orc_get_raster.restype = i32
         L.orc_get_raster.argtypes = [vp, u64, u64, vp]
         L.orc_get_trace.restype = i32
@@ -89,7 +93,8 @@ def class_table(classes) -> np.ndarray:
 class Oracle:
     """One simulated network.  mode: "fp64" (the definition) or "fp32" (fp32-faithful)."""
 
-    def __init__(self, net, cfg, mode="fp64", delays=None, bias=None, threads=1):
+    def __init__(self, net, cfg, mode="fp64", delays=None, bias=None, threads=1, stdp=None):
+        """stdp = (alpha per ms, beta per ms): plastic weights (eq. 32-33), from step 0."""
         L = lib()
         self.n = int(net.n_vertices)
         self.D = int(cfg["ring_slots"])
@@ -114,6 +119,8 @@ class Oracle:
                                {"fp64": 0, "fp32": 1}[mode])
         if not self._h:
             raise ValueError("orc_create rejected the network (row offsets / target range / delay)")
+        if stdp is not None and L.orc_enable_stdp(self._h, float(stdp[0]), float(stdp[1])) != 0:
+            raise ValueError("orc_enable_stdp refused (beta < 0, or out of memory)")
 
     def __del__(self):
         if getattr(self, "_h", None):
@@ -157,6 +164,12 @@ class Oracle:
     def w_fx(self):
         out = np.empty(self.E, dtype=np.int64)
         lib().orc_get_w_fx(self._h, _p(out))
+        return out
+
+    def weights(self):
+        """w_ij(t) of every edge in the caller's (CSR) edge order."""
+        out = np.empty(self.E, dtype=np.float64)
+        lib().orc_get_weights(self._h, _p(out))
         return out
 
     def counters(self):

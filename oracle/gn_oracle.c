@@ -286,6 +286,14 @@ typedef struct orc_net {
     uint64_t spikes, delivered, kicks;
     int64_t mass_delivered, mass_consumed; /* fixed-point sums, kicks excluded */
     int overflow;       /* a ring slot left the int32 range */
+    /* plastic weights (orc_enable_stdp; PAPER.md:323-349 eq. 32-33, :103-119 eq. 9): every weight a state of its own */
+    int plastic;
+    double stdp_alpha, stdp_beta;   /* as given (fp32 at the boundary), in double */
+    float stdp_dta_f, stdp_beta_f;  /* (float)(dt alpha) rounded once, beta: the fp32-faithful mode's constants */
+    double *wd;         /* [E] w_ij(t), mode 0 */
+    float *wf;          /* [E] w_ij(t), mode 1 */
+    int64_t *age;       /* [D+1][n] row tau mod (D+1): s_j(tau) of eq. 32 in steps, -1 = j has not fired yet (reading #23) */
+    int64_t *I_in;      /* [n] eq. 30's sum at the step in hand, fixed point */
 } orc_net;
 
 void orc_destroy(orc_net *o)
@@ -296,6 +304,7 @@ void orc_destroy(orc_net *o)
     free(o->Vf); free(o->Wf); free(o->rf); free(o->pf); free(o->cf); free(o->accf); free(o->p);
     free(o->hm); free(o->hh); free(o->hmf); free(o->hhf);
     free(o->refr); free(o->ring); free(o->consumed); free(o->fired); free(o->raster); free(o->trace);
+    free(o->wd); free(o->wf); free(o->age); free(o->I_in);
     free(o);
 }
 
@@ -616,10 +625,164 @@ static int orc_vertex_hh_fp32(orc_net *o, uint32_t j, int64_t I_fx)
     return fired;
 }
 
+/* ---- plastic weights: PAPER.md:323-349 (section 3.2.3, eq. 32-33) on top of eq. 30 (:311) and eq. 9 (:103-119) -------------
+ * Written for sizes the pure-Python definition (oracle/stdp_definition.py) cannot reach; pinned against it and against eq. 33's
+ * closed form in tests/test_oracle_stdp.py.  Nothing is pushed into a ring here: eq. 30 weighs the spike of k arriving at j at
+ * step t with w_kj(t), the weight AT THE ARRIVAL step, so the sum is PULLED at step t from the raster history by visiting every
+ * edge, and eq. 33 is then applied to every edge, one by one, in the paper's order:
+ *   s_j(t + dt) = (1 - spd(V_j(t))) (s_j(t) + dt)                                                      eq. 32, kept in steps
+ *   q_ij(t) = (s~_i(t - tau_ij) - s~_j(t)) max(spd(V_i(t - tau_ij)), spd(V_j(t)))                       eq. 33
+ *   w_ij(t + dt) = w_ij(t) + dt alpha sign(q_ij) exp(-beta |q_ij|)
+ * with s~ the age after eq. 32's reset factor (reading #22: 0 for a vertex spiking at the step) and no age before the first
+ * spike (reading #23).  Hence, per edge i -> j of delay d at step t (pre: i fired at t - d; post: j fires at t):
+ *   pre and not post:  q = -s_j(t)        the weight falls by dt alpha exp(-beta s_j(t))       if s_j(t) > 0
+ *   post and not pre:  q = +s_i(t - d)    the weight rises by dt alpha exp(-beta s_i(t - d))   if s_i(t - d) > 0
+ *   both, neither, or an age of 0 (sign(0) = 0):  no change.
+ * mode 0: weights, ages and the exponential in double (libm).  mode 1 (fp32-faithful): one
+ * rounded binary32 operation each, age = (float)steps * dt, dw = (float)(dt alpha) * exp32(-(beta * age)), w -+ dw.
+ * Either way an arriving weight enters eq. 30's fixed-point sum as rint(w 2^16), ties to even (mode 1 saturates at int32 as
+ * the conversion instruction does), like every static weight. */
+int orc_enable_stdp(orc_net *o, float alpha, float beta)
+{
+    if (!o || o->t != 0 || !(beta >= 0.0f)) return -1;
+    o->plastic = 1;
+    o->stdp_alpha = (double)alpha; o->stdp_beta = (double)beta;
+    o->stdp_dta_f = (float)(o->dt * (double)alpha); o->stdp_beta_f = beta;
+    const size_t E1 = o->E ? (size_t)o->E : 1, n1 = o->n ? o->n : 1;
+    o->wd = (double *)malloc(E1 * sizeof(double));
+    o->wf = (float *)malloc(E1 * sizeof(float));
+    o->age = (int64_t *)malloc((size_t)(o->D + 1) * n1 * sizeof(int64_t));
+    o->I_in = (int64_t *)calloc(n1, sizeof(int64_t));
+    if (!o->wd || !o->wf || !o->age || !o->I_in) return -1;
+    for (uint64_t e = 0; e < o->E; ++e) {          /* the weights start at the quantised values the static network has */
+        o->wd[e] = (double)o->w_fx[e] / 65536.0;
+        o->wf[e] = (float)o->wd[e];
+    }
+    for (size_t k = 0; k < (size_t)(o->D + 1) * n1; ++k) o->age[k] = -1;
+    return 0;
+}
+
+static inline int orc_fired_at(const orc_net *o, uint64_t t, uint32_t i)
+{
+    return (o->raster[(size_t)t * o->words + (i >> 5)] >> (i & 31)) & 1u;
+}
+
+static int orc_step_plastic(orc_net *o, uint64_t n_steps)
+{
+    const uint32_t n = o->n, D = o->D;
+    for (uint64_t s = 0; s < n_steps; ++s) {
+        const uint64_t t = o->t;
+        uint32_t *rast = o->raster + (size_t)t * o->words;
+        memset(rast, 0, (size_t)o->words * sizeof(uint32_t));
+        memset(o->I_in, 0, (size_t)n * sizeof(int64_t));
+        /* eq. 30 at step t: every edge whose source fired exactly `delay` steps ago contributes its CURRENT weight */
+        uint64_t delivered = 0;
+        int64_t mass_delivered = 0;
+#pragma omp parallel for schedule(dynamic, 64) reduction(+ : delivered, mass_delivered)
+        for (int64_t ii = 0; ii < (int64_t)n; ++ii) {
+            for (uint64_t e = o->row[ii]; e < o->row[ii + 1]; ++e) {
+                const uint64_t d = o->delay[e];
+                if (t < d || !orc_fired_at(o, t - d, (uint32_t)ii)) continue;
+                int64_t w_fx;
+                if (o->mode) {
+                    const float sc = o->wf[e] * 65536.0f;
+                    w_fx = sc != sc ? 0 : sc >= 2147483648.0f ? 2147483647ll : sc <= -2147483648.0f ? -2147483648ll : (int64_t)rintf(sc);
+                } else {
+                    w_fx = (int64_t)llrint(o->wd[e] * 65536.0);
+                }
+#pragma omp atomic
+                o->I_in[o->tgt[e]] += w_fx;
+                delivered += 1;
+                mass_delivered += w_fx;
+            }
+        }
+        uint64_t spikes = 0, kicks = 0;
+        int64_t mass_consumed = 0;
+        int overflow = 0;
+#pragma omp parallel for schedule(static) reduction(+ : spikes, kicks, mass_consumed) reduction(| : overflow)
+        for (int64_t jj = 0; jj < (int64_t)n; ++jj) {      /* the vertex transition, exactly as in orc_step */
+            const uint32_t j = (uint32_t)jj;
+            int64_t I_fx = o->I_in[j];
+            if (I_fx > 2147483647ll || I_fx < -2147483648ll) overflow = 1;
+            mass_consumed += I_fx;
+            const orc_class *q = &o->cls_tab[o->cls[j]];
+            if (q->drive_thr && orc_word(o->seed, ORC_STREAM_DRIVE, j, t) < q->drive_thr) {
+                I_fx += q->kick_fx;
+                kicks += 1;
+            }
+            o->consumed[j] = I_fx;
+            int f = q->hh ? (o->mode ? orc_vertex_hh_fp32(o, j, I_fx) : orc_vertex_hh_fp64(o, j, I_fx))
+                          : (o->mode ? orc_vertex_fp32(o, j, I_fx) : orc_vertex_fp64(o, j, I_fx));
+            o->fired[j] = (uint8_t)f;
+            spikes += (uint64_t)f;
+        }
+        for (uint32_t j = 0; j < n; ++j)
+            if (o->fired[j]) rast[j >> 5] |= 1u << (j & 31);
+        /* eq. 33, edge by edge */
+        const int64_t *age_t = o->age + (size_t)(t % (D + 1)) * n;
+#pragma omp parallel for schedule(dynamic, 64)
+        for (int64_t ii = 0; ii < (int64_t)n; ++ii) {
+            for (uint64_t e = o->row[ii]; e < o->row[ii + 1]; ++e) {
+                const uint64_t d = o->delay[e];
+                const uint32_t j = o->tgt[e];
+                const int pre = t >= d && orc_fired_at(o, t - d, (uint32_t)ii);
+                const int post = o->fired[j];
+                if (pre == post) continue;                                  /* neither: max(..) = 0; both: q = 0 */
+                int64_t steps;
+                if (pre) steps = age_t[j];                                  /* q = -s_j(t) */
+                else if (t >= d) steps = o->age[(size_t)((t - d) % (D + 1)) * n + (uint32_t)ii];   /* q = +s_i(t - d) */
+                else steps = -1;                                            /* i has no age d steps before the start */
+                if (steps <= 0) continue;                                   /* no age yet (reading #23), or q = 0 */
+                if (o->mode) {
+                    const float a = (float)steps * o->dt_f;
+                    const float dw = o->stdp_dta_f * orc_exp32(-(o->stdp_beta_f * a));
+                    o->wf[e] = pre ? o->wf[e] - dw : o->wf[e] + dw;
+                } else {
+                    const double a = (double)steps * o->dt;
+                    const double dw = (o->dt * o->stdp_alpha) * exp(-(o->stdp_beta * a));
+                    o->wd[e] = pre ? o->wd[e] - dw : o->wd[e] + dw;
+                }
+            }
+        }
+        /* eq. 32: s_j(t + dt) = (1 - spd(V_j(t))) (s_j(t) + dt), in steps; no age before the first spike */
+        int64_t *age_n = o->age + (size_t)((t + 1) % (D + 1)) * n;
+        for (uint32_t j = 0; j < n; ++j) age_n[j] = o->fired[j] ? 0 : (age_t[j] < 0 ? -1 : age_t[j] + 1);
+        if (o->obs_stride && (t + 1) % o->obs_stride == 0) {   /* step 7: emit one frame (as in orc_step) */
+            const uint64_t frame = (t + 1) / o->obs_stride - 1;
+            double *z = o->trace + (size_t)frame * n;
+            for (uint32_t j = 0; j < n; ++j) {
+                double sum = o->mode ? (double)o->accf[j] : o->acc[j];
+                double g = o->obs_sigma != 0.0 ? orc_gauss(o->seed, j, frame) : 0.0;
+                z[j] = o->obs_gain * (sum / (double)o->obs_stride) + o->obs_offset + o->obs_sigma * g;
+                o->acc[j] = 0.0; o->accf[j] = 0.0f;
+            }
+            o->frames = frame + 1;
+        }
+        o->spikes += spikes; o->kicks += kicks; o->delivered += delivered;
+        o->mass_consumed += mass_consumed; o->mass_delivered += mass_delivered;
+        o->overflow |= overflow;
+        o->t = t + 1;
+    }
+    return o->overflow ? -2 : 0;
+}
+
+/* w_ij(t) of every edge, in the caller's (CSR) edge order; the static weights when orc_enable_stdp was not called. */
+void orc_get_weights(const orc_net *o, double *out)
+{
+    for (uint64_t e = 0; e < o->E; ++e)
+        out[e] = !o->plastic ? (double)o->w_fx[e] / 65536.0 : o->mode ? (double)o->wf[e] : o->wd[e];
+}
+
 /* Advance n_steps.  Returns 0, -1 (out of memory) or -2 (a ring slot left the int32 range). */
 int orc_step(orc_net *o, uint64_t n_steps, int n_threads)
 {
     if (orc_reserve_history(o, n_steps)) return -1;
+    if (o->plastic) {
+#ifdef _OPENMP
+        if (n_threads > 0) omp_set_num_threads(n_threads);
+#endif
+        return orc_step_plastic(o, n_steps);
+    }
 #ifdef _OPENMP
     if (n_threads > 0) omp_set_num_threads(n_threads);
 #else
