@@ -967,6 +967,44 @@ def test_plastic_random_network_tracks_the_definition(gn, seed):
     np.testing.assert_array_equal(gn.gn_read_state(g, gn.GN_FAULTS), [0, 0])
 
 
+@pytest.mark.parametrize("k,n,steps", [
+    (3, 20_000, 1000),        # config 3's density, D = 64: 79 update CTAs, spike lists longer than a warp, many CTAs in both halves of gn_plast_kernel
+    (4, 9_001, 1000),         # config 4's density (200 out-edges per vertex), D = 128, ragged N
+    (2, 5_000, 1200),         # excitatory / inhibitory classes: negative weights, observation every step
+    (3, 100_000, 400),        # config 3 at FULL size (7.2e6 edges), the network bench.py --stdp --config 3 times
+])
+def test_plastic_weights_bit_exact_at_scale(gn, k, n, steps):
+    """Eq. 33 with a real learning rate (alpha = 0.5 / ms) at sizes that span many CTAs, against the C oracle's plastic mode
+    in its fp32-faithful arithmetic (oracle/gn_oracle.c orc_step_plastic, pinned in tests/test_oracle_stdp_c.py): rasters,
+    state words and counters bit-exact at every checkpoint, and EVERY weight bit-equal -- an edge is touched at most once per
+    step on both sides and the contract fixes the operation sequence, so nothing weaker is needed."""
+    net, cfg = make_config(k, n=n)
+    g = _plastic(gn, net, cfg, steps, None, trace_capacity_frames=steps)
+    o = Oracle(net, cfg, "fp32", threads=16, stdp=(STDP_ALPHA, STDP_BETA))
+    w0 = gn.gn_read_state(g, gn.GN_WEIGHTS).copy()
+    np.testing.assert_array_equal(w0.view(np.uint32), o.weights().astype(np.float32).view(np.uint32))
+    chunk = steps // 4
+    for done in range(chunk, steps + 1, chunk):
+        gn.gn_step(g, chunk)
+        o.step(chunk)
+        np.testing.assert_array_equal(gn.gn_read_raster(g, done - chunk, chunk), o.raster(done - chunk, chunk))
+        wg = gn.gn_read_state(g, gn.GN_WEIGHTS)
+        np.testing.assert_array_equal(wg.view(np.uint32), o.weights().astype(np.float32).view(np.uint32))
+        for which_g, which_o in ((gn.GN_V, ob.V), (gn.GN_W, ob.W), (gn.GN_R, ob.R)):
+            np.testing.assert_array_equal(gn.gn_read_state(g, which_g).view(np.uint32),
+                                          o.state(which_o).astype(np.float32).view(np.uint32))
+        c, oc = gn.gn_read_state(g, gn.GN_COUNTERS), o.counters()
+        assert (int(c[0]), int(c[1]), int(c[2]), int(c[3])) == (oc["steps"], oc["spikes"], oc["delivered"], oc["kicks"])
+    moved = np.abs(wg - w0)
+    print(f"plastic config {k} n={n}: {oc['spikes']} spikes, {oc['delivered']} arrivals, {int((moved > 0).sum())} of {len(wg)} "
+          f"weights moved, largest change {moved.max():.3f}")
+    assert oc["spikes"] > 20 * 32 and (moved > 0).sum() > len(wg) // 10 and moved.max() > 0.1
+    np.testing.assert_array_equal(gn.gn_read_state(g, gn.GN_FAULTS), [0, 0])
+    if cfg["obs_stride"]:
+        frames = steps // cfg["obs_stride"]
+        np.testing.assert_allclose(gn.gn_observe(g, 0, frames).astype(np.float64), o.trace(0, frames), rtol=1e-6, atol=1e-5)
+
+
 def _force_spikes(gn, g, vertices):
     v = gn.gn_read_state(g, gn.GN_V)
     v[list(vertices)] = 30.0
