@@ -971,7 +971,7 @@ def test_plastic_random_network_tracks_the_definition(gn, seed):
     (3, 20_000, 1000),        # config 3's density, D = 64: 79 update CTAs, spike lists longer than a warp, many CTAs in both halves of gn_plast_kernel
     (4, 9_001, 1000),         # config 4's density (200 out-edges per vertex), D = 128, ragged N
     (2, 5_000, 1200),         # excitatory / inhibitory classes: negative weights, observation every step
-    (3, 100_000, 400),        # config 3 at FULL size (7.2e6 edges), the network bench.py --stdp --config 3 times
+    (3, 100_000, 1000),       # config 3 at FULL size (7.2e6 edges), the network bench.py --stdp --config 3 times
 ])
 def test_plastic_weights_bit_exact_at_scale(gn, k, n, steps):
     """Eq. 33 with a real learning rate (alpha = 0.5 / ms) at sizes that span many CTAs, against the C oracle's plastic mode
